@@ -1,0 +1,821 @@
+/*
+ * spin_oracle.c -- TEST INFRASTRUCTURE, NOT PRODUCT CODE.
+ *
+ * Plain, slow, fp64 CPU implementation of the hot path of "Spirit: Multifunctional
+ * Framework for Atomistic Spin Simulations" (arXiv 1901.11350), written from the
+ * paper's equations only.  It shares no code, header, table or constant generator
+ * with the CUDA library under paper_1901_11350_b200/; only tests/, bench.py's
+ * cpu_baseline / --impl reference legs and __graft_entry__.smoke() may call it.
+ *
+ * What it follows (PAPER.md line numbers):
+ *   energy            Eq. 1 (:61-67), Eq. 2 (:75)           -> orc_energy
+ *   gradient F=-dH/dn ":155  B_eff = -dH/dn_i"              -> orc_gradient (gather), orc_gradient_scatter
+ *   dipole-dipole     :81-89 direct sum / FFT convolution   -> orc_ddi_direct, orc_ddi_fft
+ *   LLG explicit form Eq. 10 (:147-153)                     -> rot_field()
+ *   thermal field     Eq. 11 (:157-160)                     -> orc_thermal_xi, sigma
+ *   Depondt solver    App. B, B5-B7 (:369-380)              -> orc_llg_step
+ *   Heun solver       App. B, B3-B4 (:355-367)              -> orc_heun_step (pin only)
+ * Readings of silent / garbled passages are listed in DESIGN.md ("Readings") under the
+ * same R-numbers as SURVEY.md 8(c).
+ *
+ * Units: energy meV, field T, moments mu_B, time ps, length Angstrom.
+ * Spin index (same as the C-ABI boundary): i = b + n_basis*(ia + Na*(ib + Nb*ic)).
+ * Spins are stored AoS: n[3*i + {0,1,2}].
+ *
+ * Parity pins (tests/test_oracle_*.py): FM closed form, Larmor Eq. 12 with the paper's
+ * printed 3e-7 error, finite differences, Euler identity, brute-force DDI, two-dipole and
+ * monolayer closed forms, spin-spiral closed form, Langevin <n_z>, Philox known answers.
+ * "parity unpinned" (convention only): DMI chirality sign of the helper
+ * conventions (R15), DDI image count (R16), periodic self-wrap (R21), max-torque norm (R22).
+ *
+ * Build: gcc -O2 -ffp-contract=off -fopenmp -shared -fPIC (see oracle/build.py).
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+#include <stdio.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+/* CODATA-2018 (paper is silent on constants, reading R5) */
+#define ORC_MU_B   0.057883818060   /* meV / T            */
+#define ORC_K_B    0.08617333262    /* meV / K            */
+#define ORC_GAMMA  0.176085963023   /* rad / (ps T)       */
+#define ORC_C_DD   0.0536815112     /* mu0 mu_B^2/(4 pi A^3), meV */
+#define ORC_PI     3.14159265358979323846
+
+enum { T_ZEE = 1, T_ANI = 2, T_EXC = 4, T_DMI = 8, T_QUAD = 16, T_DDI = 32, T_ALL = 63 };
+
+typedef struct orc_system {
+    double brav[9];          /* rows a, b, c in units of alat                      */
+    int nb;                  /* atoms in the basis                                 */
+    double *basis;           /* 3*nb fractional coordinates                        */
+    int nc[3], per[3];       /* cells and periodic flags per direction             */
+    double alat;             /* lattice constant, Angstrom                         */
+    long ncell, N;
+    double *mu;              /* nb, mu_B                                           */
+    double Bext[3];          /* Tesla                                              */
+    double *K, *Kax;         /* nb, 3*nb (unit axes)                               */
+    int npairs; int *pi, *pj, *pt; double *pJ, *pD;
+    int nquads; int *qb, *qt; double *qK;
+    int ddi, nimg[3];
+    int ddi_direct;          /* 1: stepping/energy use the O(N^2) sum              */
+    /* padded-FFT cache */
+    int P[3]; long Ptot; double *Khat;   /* [a][b][6][Ptot] complex interleaved     */
+    /* LLG */
+    double dt, alpha, T, u, jdir[3], beta;
+    uint64_t seed, step;
+    double *n;               /* 3N */
+    int nthreads;
+} orc_system;
+
+/* ------------------------------------------------------------------ helpers */
+static inline long cell_index(const orc_system *s, const int c[3]) {
+    return c[0] + (long)s->nc[0] * (c[1] + (long)s->nc[1] * c[2]);
+}
+static inline void cell_coords(const orc_system *s, long cell, int c[3]) {
+    c[0] = (int)(cell % s->nc[0]);
+    c[1] = (int)((cell / s->nc[0]) % s->nc[1]);
+    c[2] = (int)(cell / ((long)s->nc[0] * s->nc[1]));
+}
+/* cell c + sign*t with boundary conditions; returns 0 if it falls off an open edge
+ * (reading R20), wraps modulo n_cells in periodic directions (reading R21).        */
+static inline int shifted_cell(const orc_system *s, const int c[3], const int t[3], int sign, int out[3]) {
+    for (int d = 0; d < 3; ++d) {
+        int x = c[d] + sign * t[d];
+        if (x < 0 || x >= s->nc[d]) {
+            if (!s->per[d]) return 0;
+            x %= s->nc[d];
+            if (x < 0) x += s->nc[d];
+        }
+        out[d] = x;
+    }
+    return 1;
+}
+static inline long spin_index(const orc_system *s, const int c[3], int b) {
+    return b + (long)s->nb * cell_index(s, c);
+}
+static inline double dot3(const double *a, const double *b) { return a[0]*b[0] + a[1]*b[1] + a[2]*b[2]; }
+static inline void cross3(const double *a, const double *b, double *o) {
+    o[0] = a[1]*b[2] - a[2]*b[1];
+    o[1] = a[2]*b[0] - a[0]*b[2];
+    o[2] = a[0]*b[1] - a[1]*b[0];
+}
+/* Cartesian position (Angstrom) of fractional lattice coordinate f (cells + basis) */
+static inline void frac_to_cart(const orc_system *s, const double f[3], double r[3]) {
+    for (int k = 0; k < 3; ++k)
+        r[k] = s->alat * (f[0]*s->brav[0+k] + f[1]*s->brav[3+k] + f[2]*s->brav[6+k]);
+}
+
+/* ------------------------------------------------------------------ lifecycle */
+orc_system *orc_create(const double brav[9], int nb, const double *basis, const int nc[3],
+                       const int per[3], double alat) {
+    orc_system *s = (orc_system *)calloc(1, sizeof(orc_system));
+    memcpy(s->brav, brav, 9 * sizeof(double));
+    s->nb = nb;
+    s->basis = (double *)malloc(3 * nb * sizeof(double));
+    memcpy(s->basis, basis, 3 * nb * sizeof(double));
+    for (int d = 0; d < 3; ++d) { s->nc[d] = nc[d]; s->per[d] = per[d]; }
+    s->alat = alat;
+    s->ncell = (long)nc[0] * nc[1] * nc[2];
+    s->N = s->ncell * nb;
+    s->mu = (double *)malloc(nb * sizeof(double));
+    s->K = (double *)calloc(nb, sizeof(double));
+    s->Kax = (double *)calloc(3 * nb, sizeof(double));
+    for (int b = 0; b < nb; ++b) { s->mu[b] = 1.0; s->Kax[3*b+2] = 1.0; }
+    s->n = (double *)calloc(3 * s->N, sizeof(double));
+    for (long i = 0; i < s->N; ++i) s->n[3*i+2] = 1.0;
+    s->dt = 1e-3; s->alpha = 0.1; s->jdir[0] = 1.0;
+#ifdef _OPENMP
+    s->nthreads = omp_get_max_threads();
+#else
+    s->nthreads = 1;
+#endif
+    return s;
+}
+void orc_destroy(orc_system *s) {
+    if (!s) return;
+    free(s->basis); free(s->mu); free(s->K); free(s->Kax);
+    free(s->pi); free(s->pj); free(s->pt); free(s->pJ); free(s->pD);
+    free(s->qb); free(s->qt); free(s->qK); free(s->Khat); free(s->n);
+    free(s);
+}
+long orc_nspins(const orc_system *s) { return s->N; }
+int orc_threads(const orc_system *s) { return s->nthreads; }
+void orc_set_threads(orc_system *s, int n) {
+#ifdef _OPENMP
+    if (n < 1) n = 1;
+    s->nthreads = n;
+#else
+    (void)n; s->nthreads = 1;
+#endif
+}
+void orc_set_mu_s(orc_system *s, const double *mu) { memcpy(s->mu, mu, s->nb * sizeof(double)); free(s->Khat); s->Khat = NULL; }
+void orc_set_field(orc_system *s, double B, const double dir[3]) {
+    double nrm = sqrt(dot3(dir, dir));
+    for (int k = 0; k < 3; ++k) s->Bext[k] = (nrm > 0) ? B * dir[k] / nrm : 0.0;
+}
+void orc_set_anisotropy(orc_system *s, int n, const int *bidx, const double *K, const double *axis) {
+    for (int b = 0; b < s->nb; ++b) s->K[b] = 0.0;
+    for (int e = 0; e < n; ++e) {
+        int b = bidx[e];
+        double nrm = sqrt(dot3(axis + 3*e, axis + 3*e));
+        s->K[b] = K[e];
+        for (int k = 0; k < 3; ++k) s->Kax[3*b+k] = axis[3*e+k] / nrm;
+    }
+}
+void orc_set_pairs(orc_system *s, int np, const int *pi, const int *pj, const int *pt,
+                   const double *J, const double *D) {
+    free(s->pi); free(s->pj); free(s->pt); free(s->pJ); free(s->pD);
+    s->npairs = np;
+    s->pi = (int *)malloc((np + 1) * sizeof(int));     memcpy(s->pi, pi, np * sizeof(int));
+    s->pj = (int *)malloc((np + 1) * sizeof(int));     memcpy(s->pj, pj, np * sizeof(int));
+    s->pt = (int *)malloc((3 * np + 1) * sizeof(int)); memcpy(s->pt, pt, 3 * np * sizeof(int));
+    s->pJ = (double *)malloc((np + 1) * sizeof(double)); memcpy(s->pJ, J, np * sizeof(double));
+    s->pD = (double *)calloc(3 * np + 1, sizeof(double));
+    if (D) memcpy(s->pD, D, 3 * np * sizeof(double));
+}
+void orc_set_quadruplets(orc_system *s, int nq, const int *qb, const int *qt, const double *K) {
+    free(s->qb); free(s->qt); free(s->qK);
+    s->nquads = nq;
+    s->qb = (int *)malloc((4 * nq + 1) * sizeof(int)); memcpy(s->qb, qb, 4 * nq * sizeof(int));
+    s->qt = (int *)malloc((9 * nq + 1) * sizeof(int)); memcpy(s->qt, qt, 9 * nq * sizeof(int));
+    s->qK = (double *)malloc((nq + 1) * sizeof(double)); memcpy(s->qK, K, nq * sizeof(double));
+}
+void orc_set_ddi(orc_system *s, int enabled, const int nimg[3], int direct) {
+    s->ddi = enabled; s->ddi_direct = direct;
+    for (int d = 0; d < 3; ++d) s->nimg[d] = nimg[d];
+    free(s->Khat); s->Khat = NULL;
+}
+void orc_set_spins(orc_system *s, const double *n) { memcpy(s->n, n, 3 * s->N * sizeof(double)); }
+void orc_get_spins(const orc_system *s, double *n) { memcpy(n, s->n, 3 * s->N * sizeof(double)); }
+void orc_llg_configure(orc_system *s, double dt_fs, double alpha, double T, uint64_t seed,
+                       double u, const double jdir[3], double beta) {
+    s->dt = dt_fs * 1e-3; s->alpha = alpha; s->T = T; s->seed = seed; s->u = u; s->beta = beta;
+    double nrm = sqrt(dot3(jdir, jdir));
+    for (int k = 0; k < 3; ++k) s->jdir[k] = (nrm > 0) ? jdir[k] / nrm : 0.0;
+    s->step = 0;
+}
+uint64_t orc_get_step(const orc_system *s) { return s->step; }
+void orc_set_step(orc_system *s, uint64_t st) { s->step = st; }
+
+/* ------------------------------------------------------------------ energy, Eq. 1 and Eq. 2
+ * Written as the sums are printed: one loop per term over cells and list entries.
+ * Reading R3: anisotropy axis/strength per basis atom.  Reading R4: each pair once, weight J.
+ * Reading R1: dipolar term in its textbook form
+ *     -1/2 C_dd sum_{i != j} mu_i mu_j [3 (n_i.r^)(n_j.r^) - n_i.n_j] / r^3 .             */
+void orc_ddi_direct(const orc_system *s, const double *n, double *F);
+void orc_ddi_fft(orc_system *s, const double *n, double *F);
+
+void orc_energy(orc_system *s, const double *n, double E[6]) {
+    long double ez = 0, ea = 0, ex = 0, ed = 0, eq = 0, edd = 0;
+    int c[3], cj[3], ck[3], cl[3];
+    for (long cell = 0; cell < s->ncell; ++cell) {
+        cell_coords(s, cell, c);
+        for (int b = 0; b < s->nb; ++b) {
+            const double *ni = n + 3 * spin_index(s, c, b);
+            ez -= (long double)(s->mu[b] * ORC_MU_B * dot3(s->Bext, ni));
+            double p = dot3(s->Kax + 3*b, ni);
+            ea -= (long double)(s->K[b] * p * p);
+        }
+        for (int p = 0; p < s->npairs; ++p) {
+            if (!shifted_cell(s, c, s->pt + 3*p, +1, cj)) continue;
+            const double *ni = n + 3 * spin_index(s, c, s->pi[p]);
+            const double *nj = n + 3 * spin_index(s, cj, s->pj[p]);
+            double cr[3]; cross3(ni, nj, cr);
+            ex -= (long double)(s->pJ[p] * dot3(ni, nj));
+            ed -= (long double)(dot3(s->pD + 3*p, cr));
+        }
+        for (int q = 0; q < s->nquads; ++q) {
+            if (!shifted_cell(s, c, s->qt + 9*q + 0, +1, cj)) continue;
+            if (!shifted_cell(s, c, s->qt + 9*q + 3, +1, ck)) continue;
+            if (!shifted_cell(s, c, s->qt + 9*q + 6, +1, cl)) continue;
+            const double *ni = n + 3 * spin_index(s, c,  s->qb[4*q+0]);
+            const double *nj = n + 3 * spin_index(s, cj, s->qb[4*q+1]);
+            const double *nk = n + 3 * spin_index(s, ck, s->qb[4*q+2]);
+            const double *nl = n + 3 * spin_index(s, cl, s->qb[4*q+3]);
+            eq -= (long double)(s->qK[q] * dot3(ni, nj) * dot3(nk, nl));
+        }
+    }
+    if (s->ddi) {
+        /* E_dd = -1/2 sum_i n_i . F_i^dd  (F^dd is linear in n; the 1/2 is the one printed in Eq. 1) */
+        double *F = (double *)calloc(3 * s->N, sizeof(double));
+        if (s->ddi_direct) orc_ddi_direct(s, n, F); else orc_ddi_fft(s, n, F);
+        for (long i = 0; i < s->N; ++i) edd -= 0.5L * (long double)dot3(n + 3*i, F + 3*i);
+        free(F);
+    }
+    E[0] = (double)ez; E[1] = (double)ea; E[2] = (double)ex; E[3] = (double)ed; E[4] = (double)eq; E[5] = (double)edd;
+}
+
+/* Dipolar energy straight from the double sum of Eq. 1 (reading R1), pair by pair. Tiny lattices only. */
+double orc_energy_ddi_pairsum(const orc_system *s, const double *n) {
+    long double e = 0;
+    int ci[3], cj[3];
+    for (long celli = 0; celli < s->ncell; ++celli) for (int a = 0; a < s->nb; ++a) {
+        cell_coords(s, celli, ci);
+        const double *ni = n + 3 * spin_index(s, ci, a);
+        for (long cellj = 0; cellj < s->ncell; ++cellj) for (int b = 0; b < s->nb; ++b) {
+            cell_coords(s, cellj, cj);
+            const double *nj = n + 3 * spin_index(s, cj, b);
+            for (int t0 = -(s->per[0] ? s->nimg[0] : 0); t0 <= (s->per[0] ? s->nimg[0] : 0); ++t0)
+            for (int t1 = -(s->per[1] ? s->nimg[1] : 0); t1 <= (s->per[1] ? s->nimg[1] : 0); ++t1)
+            for (int t2 = -(s->per[2] ? s->nimg[2] : 0); t2 <= (s->per[2] ? s->nimg[2] : 0); ++t2) {
+                if (celli == cellj && a == b && t0 == 0 && t1 == 0 && t2 == 0) continue;
+                double f[3] = { cj[0] - ci[0] + (double)t0 * s->nc[0] + s->basis[3*b+0] - s->basis[3*a+0],
+                                cj[1] - ci[1] + (double)t1 * s->nc[1] + s->basis[3*b+1] - s->basis[3*a+1],
+                                cj[2] - ci[2] + (double)t2 * s->nc[2] + s->basis[3*b+2] - s->basis[3*a+2] };
+                double r[3]; frac_to_cart(s, f, r);
+                double r2 = dot3(r, r), rn = sqrt(r2);
+                double rh[3] = { r[0]/rn, r[1]/rn, r[2]/rn };
+                e -= 0.5L * (long double)(ORC_C_DD * s->mu[a] * s->mu[b] *
+                        (3.0 * dot3(ni, rh) * dot3(nj, rh) - dot3(ni, nj)) / (r2 * rn));
+            }
+        }
+    }
+    return (double)e;
+}
+
+/* ------------------------------------------------------------------ gradient, scatter form
+ * F_i = -dH/dn_i in the embedding space, term by term as the derivative of orc_energy's sums:
+ *   pair (i,j,J,D):   F_i += J n_j + n_j x D ;  F_j += J n_i - n_i x D
+ *                     (from D.(n_i x n_j) = n_i.(n_j x D) = -n_j.(n_i x D))
+ *   quad (i,j,k,l,K): F_i += K (n_k.n_l) n_j ; F_j += K (n_k.n_l) n_i ;
+ *                     F_k += K (n_i.n_j) n_l ; F_l += K (n_i.n_j) n_k
+ * Serial; used to pin the parallel gather form below.                                   */
+void orc_gradient_scatter(orc_system *s, const double *n, double *F, int mask) {
+    memset(F, 0, 3 * s->N * sizeof(double));
+    int c[3], cj[3], ck[3], cl[3];
+    for (long cell = 0; cell < s->ncell; ++cell) {
+        cell_coords(s, cell, c);
+        for (int b = 0; b < s->nb; ++b) {
+            long i = spin_index(s, c, b);
+            if (mask & T_ZEE) for (int k = 0; k < 3; ++k) F[3*i+k] += s->mu[b] * ORC_MU_B * s->Bext[k];
+            if (mask & T_ANI) {
+                double p = dot3(s->Kax + 3*b, n + 3*i);
+                for (int k = 0; k < 3; ++k) F[3*i+k] += 2.0 * s->K[b] * p * s->Kax[3*b+k];
+            }
+        }
+        for (int p = 0; p < s->npairs; ++p) {
+            if (!shifted_cell(s, c, s->pt + 3*p, +1, cj)) continue;
+            long i = spin_index(s, c, s->pi[p]), j = spin_index(s, cj, s->pj[p]);
+            const double *D = s->pD + 3*p;
+            if (mask & T_EXC) for (int k = 0; k < 3; ++k) {
+                F[3*i+k] += s->pJ[p] * n[3*j+k];
+                F[3*j+k] += s->pJ[p] * n[3*i+k];
+            }
+            if (mask & T_DMI) {
+                double a[3], bb[3];
+                cross3(n + 3*j, D, a); cross3(n + 3*i, D, bb);
+                for (int k = 0; k < 3; ++k) { F[3*i+k] += a[k]; F[3*j+k] -= bb[k]; }
+            }
+        }
+        if (mask & T_QUAD) for (int q = 0; q < s->nquads; ++q) {
+            if (!shifted_cell(s, c, s->qt + 9*q + 0, +1, cj)) continue;
+            if (!shifted_cell(s, c, s->qt + 9*q + 3, +1, ck)) continue;
+            if (!shifted_cell(s, c, s->qt + 9*q + 6, +1, cl)) continue;
+            long i = spin_index(s, c,  s->qb[4*q+0]), j = spin_index(s, cj, s->qb[4*q+1]);
+            long k = spin_index(s, ck, s->qb[4*q+2]), l = spin_index(s, cl, s->qb[4*q+3]);
+            double dij = dot3(n + 3*i, n + 3*j), dkl = dot3(n + 3*k, n + 3*l), K = s->qK[q];
+            for (int x = 0; x < 3; ++x) {
+                double fi = K * dkl * n[3*j+x], fj = K * dkl * n[3*i+x];
+                double fk = K * dij * n[3*l+x], fl = K * dij * n[3*k+x];
+                F[3*i+x] += fi; F[3*j+x] += fj; F[3*k+x] += fk; F[3*l+x] += fl;
+            }
+        }
+    }
+    if ((mask & T_DDI) && s->ddi) {
+        double *Fd = (double *)calloc(3 * s->N, sizeof(double));
+        if (s->ddi_direct) orc_ddi_direct(s, n, Fd); else orc_ddi_fft(s, n, Fd);
+        for (long i = 0; i < 3 * s->N; ++i) F[i] += Fd[i];
+        free(Fd);
+    }
+}
+
+/* ------------------------------------------------------------------ gradient, gather form
+ * Same sums, regrouped per spin so that spins can be processed independently (OpenMP):
+ * a spin on basis atom b collects, for every list entry in which b appears, the partner's
+ * contribution.  For a pair (bi, bj, t): as "i" the partner is (cell + t, bj) with +D; as "j"
+ * the partner is (cell - t, bi) with -D.  A quadruplet anchored at cell c0 has its four
+ * members at c0, c0+tj, c0+tk, c0+tl; a spin in role r sits at c0 + t_r, so c0 = cell - t_r.
+ * A quadruplet with any member off an open edge does not exist (reading R20).             */
+static void gather_one(const orc_system *s, const double *n, long cell, int b, int mask, double F[3]) {
+    int c[3], c2[3], c0[3], cm[4][3];
+    static const int zero3[3] = {0, 0, 0};
+    cell_coords(s, cell, c);
+    const double *ni = n + 3 * spin_index(s, c, b);
+    F[0] = F[1] = F[2] = 0.0;
+    if (mask & T_ZEE) for (int k = 0; k < 3; ++k) F[k] += s->mu[b] * ORC_MU_B * s->Bext[k];
+    if (mask & T_ANI) {
+        double p = dot3(s->Kax + 3*b, ni);
+        for (int k = 0; k < 3; ++k) F[k] += 2.0 * s->K[b] * p * s->Kax[3*b+k];
+    }
+    if (mask & (T_EXC | T_DMI)) for (int p = 0; p < s->npairs; ++p) {
+        const double *D = s->pD + 3*p;
+        if (s->pi[p] == b && shifted_cell(s, c, s->pt + 3*p, +1, c2)) {
+            const double *nj = n + 3 * spin_index(s, c2, s->pj[p]);
+            if (mask & T_EXC) for (int k = 0; k < 3; ++k) F[k] += s->pJ[p] * nj[k];
+            if (mask & T_DMI) { double x[3]; cross3(nj, D, x); for (int k = 0; k < 3; ++k) F[k] += x[k]; }
+        }
+        if (s->pj[p] == b && shifted_cell(s, c, s->pt + 3*p, -1, c2)) {
+            const double *nj = n + 3 * spin_index(s, c2, s->pi[p]);
+            if (mask & T_EXC) for (int k = 0; k < 3; ++k) F[k] += s->pJ[p] * nj[k];
+            if (mask & T_DMI) { double x[3]; cross3(nj, D, x); for (int k = 0; k < 3; ++k) F[k] -= x[k]; }
+        }
+    }
+    if (mask & T_QUAD) for (int q = 0; q < s->nquads; ++q) {
+        for (int role = 0; role < 4; ++role) {
+            if (s->qb[4*q + role] != b) continue;
+            const int *tr = (role == 0) ? zero3 : s->qt + 9*q + 3*(role-1);
+            if (!shifted_cell(s, c, tr, -1, c0)) continue;
+            int ok = 1;
+            for (int m = 0; m < 4 && ok; ++m) {
+                const int *tm = (m == 0) ? zero3 : s->qt + 9*q + 3*(m-1);
+                ok = shifted_cell(s, c0, tm, +1, cm[m]);
+            }
+            if (!ok) continue;
+            /* the member that must come back to this very site (guards against open-edge aliasing) */
+            if (cm[role][0] != c[0] || cm[role][1] != c[1] || cm[role][2] != c[2]) continue;
+            const double *m0 = n + 3 * spin_index(s, cm[0], s->qb[4*q+0]);
+            const double *m1 = n + 3 * spin_index(s, cm[1], s->qb[4*q+1]);
+            const double *m2 = n + 3 * spin_index(s, cm[2], s->qb[4*q+2]);
+            const double *m3 = n + 3 * spin_index(s, cm[3], s->qb[4*q+3]);
+            double K = s->qK[q];
+            const double *partner; double w;
+            if (role == 0)      { partner = m1; w = dot3(m2, m3); }
+            else if (role == 1) { partner = m0; w = dot3(m2, m3); }
+            else if (role == 2) { partner = m3; w = dot3(m0, m1); }
+            else                { partner = m2; w = dot3(m0, m1); }
+            for (int k = 0; k < 3; ++k) F[k] += K * w * partner[k];
+        }
+    }
+}
+
+void orc_gradient(orc_system *s, const double *n, double *F, int mask) {
+    long N = s->N; int nb = s->nb;
+#pragma omp parallel for schedule(static) num_threads(s->nthreads)
+    for (long i = 0; i < N; ++i) gather_one(s, n, i / nb, (int)(i % nb), mask, F + 3*i);
+    if ((mask & T_DDI) && s->ddi) {
+        double *Fd = (double *)calloc(3 * N, sizeof(double));
+        if (s->ddi_direct) orc_ddi_direct(s, n, Fd); else orc_ddi_fft(s, n, Fd);
+        for (long i = 0; i < 3 * N; ++i) F[i] += Fd[i];
+        free(Fd);
+    }
+}
+
+/* ------------------------------------------------------------------ dipole-dipole, direct sum (:81, :89)
+ * F_i = mu_i C_dd sum_{j, images; r != 0} mu_j [3 r^ (n_j.r^) - n_j] / r^3 ,  r = r_j + image - r_i.
+ * Images: t_d in [-nimg_d, nimg_d] in periodic directions, 0 in open ones (reading R16);
+ * self images (i == j, t != 0) are included.                                              */
+void orc_ddi_direct(const orc_system *s, const double *n, double *F) {
+    long N = s->N; int nb = s->nb;
+    int lim[3]; for (int d = 0; d < 3; ++d) lim[d] = s->per[d] ? s->nimg[d] : 0;
+#pragma omp parallel for schedule(static) num_threads(s->nthreads)
+    for (long i = 0; i < N; ++i) {
+        int ci[3], cj[3]; cell_coords(s, i / nb, ci); int a = (int)(i % nb);
+        double acc[3] = {0, 0, 0};
+        for (long j = 0; j < N; ++j) {
+            cell_coords(s, j / nb, cj); int b = (int)(j % nb);
+            const double *nj = n + 3*j;
+            for (int t0 = -lim[0]; t0 <= lim[0]; ++t0)
+            for (int t1 = -lim[1]; t1 <= lim[1]; ++t1)
+            for (int t2 = -lim[2]; t2 <= lim[2]; ++t2) {
+                if (i == j && t0 == 0 && t1 == 0 && t2 == 0) continue;
+                double f[3] = { cj[0] - ci[0] + (double)t0 * s->nc[0] + s->basis[3*b+0] - s->basis[3*a+0],
+                                cj[1] - ci[1] + (double)t1 * s->nc[1] + s->basis[3*b+1] - s->basis[3*a+1],
+                                cj[2] - ci[2] + (double)t2 * s->nc[2] + s->basis[3*b+2] - s->basis[3*a+2] };
+                double r[3]; frac_to_cart(s, f, r);
+                double r2 = dot3(r, r), rn = sqrt(r2);
+                double rh[3] = { r[0]/rn, r[1]/rn, r[2]/rn };
+                double p = dot3(nj, rh), w = s->mu[b] / (r2 * rn);
+                for (int k = 0; k < 3; ++k) acc[k] += w * (3.0 * rh[k] * p - nj[k]);
+            }
+        }
+        for (int k = 0; k < 3; ++k) F[3*i+k] = s->mu[a] * ORC_C_DD * acc[k];
+    }
+}
+
+/* ------------------------------------------------------------------ own FFT (paper uses FFTW3, :87)
+ * In-place complex transform of length n, sign = -1 forward / +1 backward, unnormalised.
+ * Power-of-two lengths: textbook iterative radix-2 (bit reversal + butterflies, twiddles
+ * from cos/sin of the exact angle).  Any other length: the DFT sum written out.           */
+static void fft_line(double *re, double *im, int n, int sign) {
+    if (n <= 1) return;
+    if ((n & (n - 1)) == 0) {
+        for (int i = 1, j = 0; i < n; ++i) {
+            int bit = n >> 1;
+            for (; j & bit; bit >>= 1) j ^= bit;
+            j ^= bit;
+            if (i < j) { double t = re[i]; re[i] = re[j]; re[j] = t; t = im[i]; im[i] = im[j]; im[j] = t; }
+        }
+        for (int len = 2; len <= n; len <<= 1) {
+            int half = len >> 1;
+            for (int k = 0; k < half; ++k) {
+                double ang = sign * 2.0 * ORC_PI * (double)k / (double)len;
+                double wr = cos(ang), wi = sin(ang);
+                for (int i = k; i < n; i += len) {
+                    int j = i + half;
+                    double xr = re[j]*wr - im[j]*wi, xi = re[j]*wi + im[j]*wr;
+                    re[j] = re[i] - xr; im[j] = im[i] - xi;
+                    re[i] += xr; im[i] += xi;
+                }
+            }
+        }
+    } else {
+        double *or_ = (double *)malloc(2 * n * sizeof(double)), *oi = or_ + n;
+        for (int k = 0; k < n; ++k) {
+            double sr = 0, si = 0;
+            for (int j = 0; j < n; ++j) {
+                double ang = sign * 2.0 * ORC_PI * (double)(((long)k * j) % n) / (double)n;
+                double wr = cos(ang), wi = sin(ang);
+                sr += re[j]*wr - im[j]*wi; si += re[j]*wi + im[j]*wr;
+            }
+            or_[k] = sr; oi[k] = si;
+        }
+        memcpy(re, or_, n * sizeof(double)); memcpy(im, oi, n * sizeof(double));
+        free(or_);
+    }
+}
+/* 3-D transform of interleaved complex data z[2*(x + P0*(y + P1*zc))], one axis after the other */
+static void fft3d(double *z, const int P[3], int sign, int nthreads) {
+    long stride[3] = { 1, P[0], (long)P[0] * P[1] };
+    long Ptot = (long)P[0] * P[1] * P[2];
+    (void)nthreads;
+    for (int ax = 0; ax < 3; ++ax) {
+        int n = P[ax];
+        if (n == 1) continue;
+        long nlines = Ptot / n;
+#pragma omp parallel num_threads(nthreads)
+        {
+            double *re = (double *)malloc(2 * n * sizeof(double)), *im = re + n;
+#pragma omp for schedule(static)
+            for (long line = 0; line < nlines; ++line) {
+                /* base index of this line: enumerate the other two axes */
+                int a1 = (ax + 1) % 3, a2 = (ax + 2) % 3;
+                long i1 = line % P[a1], i2 = line / P[a1];
+                long base = i1 * stride[a1] + i2 * stride[a2];
+                for (int k = 0; k < n; ++k) { re[k] = z[2*(base + k*stride[ax])]; im[k] = z[2*(base + k*stride[ax]) + 1]; }
+                fft_line(re, im, n, sign);
+                for (int k = 0; k < n; ++k) { z[2*(base + k*stride[ax])] = re[k]; z[2*(base + k*stride[ax]) + 1] = im[k]; }
+            }
+            free(re);
+        }
+    }
+}
+/* exported for the FFT pins */
+void orc_fft3d(double *z, const int P[3], int sign) { fft3d(z, P, sign, 1); }
+
+/* ------------------------------------------------------------------ dipole-dipole by padded FFT (:81-87)
+ * One padded array per sublattice, one convolution per sublattice pair (:87).
+ *   P_d = 2 N_d if N_d > 1 else 1 (reading R17).
+ *   K_ab(Delta) = sum_images T(r), r = alat * ((Delta + t*N) + p_a - p_b) . bravais,
+ *   T(r) = (3 r^ r^T - 1)/r^3, stored at index Delta mod P_d for Delta in (-N_d, N_d);
+ *   Delta = (target cell) - (source cell).  T is even in r, so this equals T(r_j - r_i).
+ *   F_a(c) = mu_a C_dd sum_b sum_c' K_ab(c - c') mu_b n_b(c')
+ *          = mu_a C_dd IFFT[ sum_b K^_ab . FFT[mu_b n_b zero-padded] ](c).
+ * Six independent components xx, xy, xz, yy, yz, zz.                                       */
+static const int SYM_A[6] = {0, 0, 0, 1, 1, 2}, SYM_B[6] = {0, 1, 2, 1, 2, 2};
+
+static void ddi_prepare(orc_system *s) {
+    if (s->Khat) return;
+    for (int d = 0; d < 3; ++d) s->P[d] = (s->nc[d] > 1) ? 2 * s->nc[d] : 1;
+    s->Ptot = (long)s->P[0] * s->P[1] * s->P[2];
+    long Pt = s->Ptot; int nb = s->nb;
+    s->Khat = (double *)calloc((size_t)nb * nb * 6 * Pt * 2, sizeof(double));
+    int lim[3]; for (int d = 0; d < 3; ++d) lim[d] = s->per[d] ? s->nimg[d] : 0;
+    for (int a = 0; a < nb; ++a) for (int b = 0; b < nb; ++b) {
+        double *Kab = s->Khat + ((size_t)(a * nb + b) * 6) * Pt * 2;
+#pragma omp parallel for schedule(static) num_threads(s->nthreads)
+        for (long idx = 0; idx < Pt; ++idx) {
+            int g[3] = { (int)(idx % s->P[0]), (int)((idx / s->P[0]) % s->P[1]), (int)(idx / ((long)s->P[0] * s->P[1])) };
+            int Delta[3], skip = 0;
+            for (int d = 0; d < 3; ++d) {
+                if (s->P[d] == 1) { Delta[d] = 0; continue; }
+                if (g[d] == s->nc[d]) { skip = 1; break; }          /* index N_d stays zero */
+                Delta[d] = (g[d] < s->nc[d]) ? g[d] : g[d] - s->P[d];
+            }
+            if (skip) continue;
+            double acc[6] = {0, 0, 0, 0, 0, 0};
+            for (int t0 = -lim[0]; t0 <= lim[0]; ++t0)
+            for (int t1 = -lim[1]; t1 <= lim[1]; ++t1)
+            for (int t2 = -lim[2]; t2 <= lim[2]; ++t2) {
+                double f[3] = { Delta[0] + (double)t0 * s->nc[0] + s->basis[3*a+0] - s->basis[3*b+0],
+                                Delta[1] + (double)t1 * s->nc[1] + s->basis[3*a+1] - s->basis[3*b+1],
+                                Delta[2] + (double)t2 * s->nc[2] + s->basis[3*a+2] - s->basis[3*b+2] };
+                double r[3]; frac_to_cart(s, f, r);
+                double r2 = dot3(r, r);
+                if (r2 < 1e-20) continue;                             /* r = 0: the i == j term */
+                double rn = sqrt(r2), r3 = r2 * rn;
+                double rh[3] = { r[0]/rn, r[1]/rn, r[2]/rn };
+                for (int m = 0; m < 6; ++m)
+                    acc[m] += (3.0 * rh[SYM_A[m]] * rh[SYM_B[m]] - (SYM_A[m] == SYM_B[m] ? 1.0 : 0.0)) / r3;
+            }
+            for (int m = 0; m < 6; ++m) Kab[2 * ((size_t)m * Pt + idx)] = acc[m];
+        }
+        for (int m = 0; m < 6; ++m) fft3d(Kab + 2 * (size_t)m * Pt, s->P, -1, s->nthreads);
+    }
+}
+
+void orc_ddi_fft(orc_system *s, const double *n, double *F) {
+    ddi_prepare(s);
+    long Pt = s->Ptot; int nb = s->nb;
+    double *M = (double *)calloc((size_t)nb * 3 * Pt * 2, sizeof(double));
+    double *H = (double *)malloc((size_t)3 * Pt * 2 * sizeof(double));
+    int c[3];
+    for (long cell = 0; cell < s->ncell; ++cell) {
+        cell_coords(s, cell, c);
+        long pidx = c[0] + (long)s->P[0] * (c[1] + (long)s->P[1] * c[2]);
+        for (int b = 0; b < nb; ++b) for (int k = 0; k < 3; ++k)
+            M[2 * ((size_t)(b * 3 + k) * Pt + pidx)] = s->mu[b] * n[3 * spin_index(s, c, b) + k];
+    }
+    for (int b = 0; b < nb; ++b) for (int k = 0; k < 3; ++k) fft3d(M + 2 * (size_t)(b * 3 + k) * Pt, s->P, -1, s->nthreads);
+    for (int a = 0; a < nb; ++a) {
+        memset(H, 0, (size_t)3 * Pt * 2 * sizeof(double));
+        for (int b = 0; b < nb; ++b) {
+            const double *Kab = s->Khat + ((size_t)(a * nb + b) * 6) * Pt * 2;
+            const double *Mb = M + 2 * (size_t)(b * 3) * Pt;
+#pragma omp parallel for schedule(static) num_threads(s->nthreads)
+            for (long q = 0; q < Pt; ++q) {
+                /* full symmetric 3x3 from the six stored components */
+                static const int comp[3][3] = { {0, 1, 2}, {1, 3, 4}, {2, 4, 5} };
+                for (int al = 0; al < 3; ++al) {
+                    double hr = 0, hi = 0;
+                    for (int be = 0; be < 3; ++be) {
+                        double kr = Kab[2 * ((size_t)comp[al][be] * Pt + q)], ki = Kab[2 * ((size_t)comp[al][be] * Pt + q) + 1];
+                        double mr = Mb[2 * ((size_t)be * Pt + q)], mi = Mb[2 * ((size_t)be * Pt + q) + 1];
+                        hr += kr * mr - ki * mi; hi += kr * mi + ki * mr;
+                    }
+                    H[2 * ((size_t)al * Pt + q)] += hr; H[2 * ((size_t)al * Pt + q) + 1] += hi;
+                }
+            }
+        }
+        for (int k = 0; k < 3; ++k) fft3d(H + 2 * (size_t)k * Pt, s->P, +1, s->nthreads);
+        for (long cell = 0; cell < s->ncell; ++cell) {
+            cell_coords(s, cell, c);
+            long pidx = c[0] + (long)s->P[0] * (c[1] + (long)s->P[1] * c[2]);
+            for (int k = 0; k < 3; ++k)
+                F[3 * spin_index(s, c, a) + k] = s->mu[a] * ORC_C_DD * H[2 * ((size_t)k * Pt + pidx)] / (double)Pt;
+        }
+    }
+    free(M); free(H);
+}
+
+/* ------------------------------------------------------------------ Philox4x32-10 (reading R13)
+ * Salmon et al. counter-based generator: 10 rounds of
+ *   (c0,c1,c2,c3) <- (hi(M1*c2) ^ c1 ^ k0, lo(M1*c2), hi(M0*c0) ^ c3 ^ k1, lo(M0*c0)),
+ * key bumped by (W0, W1) between rounds.                                                  */
+void orc_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]) {
+    uint32_t c0 = ctr[0], c1 = ctr[1], c2 = ctr[2], c3 = ctr[3], k0 = key[0], k1 = key[1];
+    for (int r = 0; r < 10; ++r) {
+        if (r > 0) { k0 += 0x9E3779B9u; k1 += 0xBB67AE85u; }
+        uint64_t p0 = (uint64_t)0xD2511F53u * c0, p1 = (uint64_t)0xCD9E8D57u * c2;
+        uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ k0, n1 = (uint32_t)p1;
+        uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3 ^ k1, n3 = (uint32_t)p0;
+        c0 = n0; c1 = n1; c2 = n2; c3 = n3;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+/* uniform in (0,1) from 64 bits: top 53 bits plus one half, times 2^-53 */
+static inline double u01(uint32_t hi, uint32_t lo) {
+    uint64_t v = (((uint64_t)hi << 32) | lo) >> 11;
+    return ((double)v + 0.5) * (1.0 / 9007199254740992.0);
+}
+/* three standard normals for (seed, step, spin): key = seed, counter = (spin, block, step_lo, step_hi);
+ * Box-Muller; block 0 -> (xi_x, xi_y), block 1 -> xi_z.                                      */
+void orc_thermal_xi(uint64_t seed, uint64_t step, uint32_t spin, double xi[3]) {
+    uint32_t key[2] = { (uint32_t)seed, (uint32_t)(seed >> 32) }, x[4];
+    uint32_t c0[4] = { spin, 0u, (uint32_t)step, (uint32_t)(step >> 32) };
+    orc_philox4x32_10(c0, key, x);
+    double u1 = u01(x[0], x[1]), u2 = u01(x[2], x[3]);
+    double rad = sqrt(-2.0 * log(u1));
+    xi[0] = rad * cos(2.0 * ORC_PI * u2);
+    xi[1] = rad * sin(2.0 * ORC_PI * u2);
+    uint32_t c1[4] = { spin, 1u, (uint32_t)step, (uint32_t)(step >> 32) };
+    orc_philox4x32_10(c1, key, x);
+    u1 = u01(x[0], x[1]); u2 = u01(x[2], x[3]);
+    xi[2] = sqrt(-2.0 * log(u1)) * cos(2.0 * ORC_PI * u2);
+}
+/* Eq. 11 with the 1/sqrt(dt) of :160 (reading R10): sigma = sqrt(2 alpha k_B T mu / (gamma dt)), meV */
+double orc_thermal_sigma(const orc_system *s, int b) {
+    return sqrt(2.0 * s->alpha * ORC_K_B * s->T * s->mu[b] * ORC_MU_B / (ORC_GAMMA * s->dt));
+}
+
+/* ------------------------------------------------------------------ (j_e . grad) n on the lattice (reading R14)
+ * j^ is expanded in the Bravais vectors of the directions with more than one cell
+ * (least squares when there are fewer than three), j^ = sum_d c_d a_d (a_d in Angstrom), so that
+ * (j^.grad) n = sum_d c_d dn/dx_d with x_d the cell coordinate; dn/dx_d by central differences
+ * on the same sublattice, one-sided at an open edge.                                          */
+static void stt_coeffs(const orc_system *s, double cd[3]) {
+    int act[3], na = 0;
+    for (int d = 0; d < 3; ++d) { cd[d] = 0.0; if (s->nc[d] > 1) act[na++] = d; }
+    if (na == 0) return;
+    double G[3][3], rhs[3];
+    for (int p = 0; p < na; ++p) {
+        double ap[3]; for (int k = 0; k < 3; ++k) ap[k] = s->alat * s->brav[3*act[p]+k];
+        rhs[p] = dot3(ap, s->jdir);
+        for (int q = 0; q < na; ++q) {
+            double aq[3]; for (int k = 0; k < 3; ++k) aq[k] = s->alat * s->brav[3*act[q]+k];
+            G[p][q] = dot3(ap, aq);
+        }
+    }
+    /* solve the (na x na) normal equations G c = rhs by Gaussian elimination with pivoting */
+    for (int p = 0; p < na; ++p) {
+        int piv = p;
+        for (int r = p + 1; r < na; ++r) if (fabs(G[r][p]) > fabs(G[piv][p])) piv = r;
+        if (piv != p) { for (int q = 0; q < na; ++q) { double t = G[p][q]; G[p][q] = G[piv][q]; G[piv][q] = t; } double t = rhs[p]; rhs[p] = rhs[piv]; rhs[piv] = t; }
+        for (int r = p + 1; r < na; ++r) {
+            double f = G[r][p] / G[p][p];
+            for (int q = p; q < na; ++q) G[r][q] -= f * G[p][q];
+            rhs[r] -= f * rhs[p];
+        }
+    }
+    double sol[3];
+    for (int p = na - 1; p >= 0; --p) {
+        double v = rhs[p];
+        for (int q = p + 1; q < na; ++q) v -= G[p][q] * sol[q];
+        sol[p] = v / G[p][p];
+    }
+    for (int p = 0; p < na; ++p) cd[act[p]] = sol[p];
+}
+void orc_stt_gradient(orc_system *s, const double *n, double *sg) {
+    double cd[3]; stt_coeffs(s, cd);
+    long N = s->N; int nb = s->nb;
+#pragma omp parallel for schedule(static) num_threads(s->nthreads)
+    for (long i = 0; i < N; ++i) {
+        int c[3], cp[3], cm[3]; cell_coords(s, i / nb, c); int b = (int)(i % nb);
+        double acc[3] = {0, 0, 0};
+        for (int d = 0; d < 3; ++d) {
+            if (s->nc[d] <= 1 || cd[d] == 0.0) continue;
+            int e[3] = {0, 0, 0}; e[d] = 1;
+            int hp = shifted_cell(s, c, e, +1, cp), hm = shifted_cell(s, c, e, -1, cm);
+            const double *n0 = n + 3*i;
+            const double *np_ = hp ? n + 3 * spin_index(s, cp, b) : n0;
+            const double *nm_ = hm ? n + 3 * spin_index(s, cm, b) : n0;
+            double w = (hp && hm) ? 0.5 : ((hp || hm) ? 1.0 : 0.0);
+            for (int k = 0; k < 3; ++k) acc[k] += cd[d] * w * (np_[k] - nm_[k]);
+        }
+        for (int k = 0; k < 3; ++k) sg[3*i+k] = acc[k];
+    }
+}
+
+/* ------------------------------------------------------------------ Eq. 10 as dn/dt = n x A (B1)
+ * A = -gamma/((1+alpha^2) mu) [F + alpha n x F] + u/(1+alpha^2) [-(alpha-beta) s + (1+alpha beta) n x s]
+ * with F in meV (incl. thermal), mu = mu_s mu_B in meV/T, s = (j^.grad) n in 1/Angstrom, u in A/ps. */
+static inline void rot_field(const orc_system *s, int b, const double *n, const double *F, const double *sg, double *A) {
+    double nxF[3], nxs[3] = {0, 0, 0};
+    cross3(n, F, nxF);
+    double pre = -ORC_GAMMA / ((1.0 + s->alpha * s->alpha) * s->mu[b] * ORC_MU_B);
+    double us = s->u / (1.0 + s->alpha * s->alpha);
+    if (s->u != 0.0) cross3(n, sg, nxs);
+    for (int k = 0; k < 3; ++k) {
+        A[k] = pre * (F[k] + s->alpha * nxF[k]);
+        if (s->u != 0.0) A[k] += us * (-(s->alpha - s->beta) * sg[k] + (1.0 + s->alpha * s->beta) * nxs[k]);
+    }
+}
+/* R(A) n: exact flow of dn/dt = n x A = (-A) x n over dt, i.e. Rodrigues rotation about
+ * e = -A/|A| by theta = |A| dt (reading R7).                                                 */
+static inline void rotate(const double *A, double dt, const double *n, double *out) {
+    double a = sqrt(dot3(A, A));
+    if (a == 0.0) { out[0] = n[0]; out[1] = n[1]; out[2] = n[2]; return; }
+    double e[3] = { -A[0]/a, -A[1]/a, -A[2]/a }, th = a * dt, c = cos(th), sn = sin(th);
+    double exn[3]; cross3(e, n, exn);
+    double en = dot3(e, n);
+    for (int k = 0; k < 3; ++k) out[k] = n[k] * c + exn[k] * sn + e[k] * en * (1.0 - c);
+}
+
+/* full force incl. thermal term; Fth may be NULL */
+static void total_force(orc_system *s, const double *n, const double *Fth, double *F) {
+    orc_gradient(s, n, F, T_ALL);
+    if (Fth) for (long i = 0; i < 3 * s->N; ++i) F[i] += Fth[i];
+}
+
+/* One Depondt step (App. B, B5-B7): predictor with R(A), A^p at the predicted configuration
+ * with the same thermal field (reading R11), corrector R((A+A^p)/2) applied to n(t) (reading R8),
+ * then renormalisation (reading R19).                                                        */
+void orc_llg_step(orc_system *s) {
+    long N = s->N; int nb = s->nb;
+    double *F = (double *)malloc(3 * N * sizeof(double)), *A = (double *)malloc(3 * N * sizeof(double));
+    double *np_ = (double *)malloc(3 * N * sizeof(double)), *sg = (double *)calloc(3 * N, sizeof(double));
+    double *Fth = NULL;
+    if (s->T > 0.0) {
+        Fth = (double *)malloc(3 * N * sizeof(double));
+#pragma omp parallel for schedule(static) num_threads(s->nthreads)
+        for (long i = 0; i < N; ++i) {
+            double xi[3]; orc_thermal_xi(s->seed, s->step, (uint32_t)i, xi);
+            double sig = orc_thermal_sigma(s, (int)(i % nb));
+            for (int k = 0; k < 3; ++k) Fth[3*i+k] = sig * xi[k];
+        }
+    }
+    total_force(s, s->n, Fth, F);
+    if (s->u != 0.0) orc_stt_gradient(s, s->n, sg);
+#pragma omp parallel for schedule(static) num_threads(s->nthreads)
+    for (long i = 0; i < N; ++i) {
+        rot_field(s, (int)(i % nb), s->n + 3*i, F + 3*i, sg + 3*i, A + 3*i);
+        rotate(A + 3*i, s->dt, s->n + 3*i, np_ + 3*i);                       /* B5 */
+    }
+    total_force(s, np_, Fth, F);
+    if (s->u != 0.0) orc_stt_gradient(s, np_, sg);
+#pragma omp parallel for schedule(static) num_threads(s->nthreads)
+    for (long i = 0; i < N; ++i) {
+        double Ap[3], Ac[3], out[3];
+        rot_field(s, (int)(i % nb), np_ + 3*i, F + 3*i, sg + 3*i, Ap);
+        for (int k = 0; k < 3; ++k) Ac[k] = 0.5 * (A[3*i+k] + Ap[k]);         /* B6 */
+        rotate(Ac, s->dt, s->n + 3*i, out);                                   /* B7 */
+        double nrm = sqrt(dot3(out, out));
+        for (int k = 0; k < 3; ++k) s->n[3*i+k] = out[k] / nrm;
+    }
+    s->step += 1;
+    free(F); free(A); free(np_); free(sg); free(Fth);
+}
+void orc_llg_iterate(orc_system *s, long nsteps) { for (long k = 0; k < nsteps; ++k) orc_llg_step(s); }
+
+/* Heun's method, B3-B4 with f = n x A, renormalised every step.  Only used to pin Fig. 5's
+ * "Heun within 1e-6 / Depondt 3e-7" statement; no thermal field, no current.                */
+void orc_heun_step(orc_system *s) {
+    long N = s->N; int nb = s->nb;
+    double *F = (double *)malloc(3 * N * sizeof(double)), *f0 = (double *)malloc(3 * N * sizeof(double));
+    double *np_ = (double *)malloc(3 * N * sizeof(double)), *sg = (double *)calloc(3 * N, sizeof(double));
+    total_force(s, s->n, NULL, F);
+    for (long i = 0; i < N; ++i) {
+        double A[3]; rot_field(s, (int)(i % nb), s->n + 3*i, F + 3*i, sg + 3*i, A);
+        cross3(s->n + 3*i, A, f0 + 3*i);
+        for (int k = 0; k < 3; ++k) np_[3*i+k] = s->n[3*i+k] + s->dt * f0[3*i+k];
+    }
+    total_force(s, np_, NULL, F);
+    for (long i = 0; i < N; ++i) {
+        double A[3], f1[3], out[3];
+        rot_field(s, (int)(i % nb), np_ + 3*i, F + 3*i, sg + 3*i, A);
+        cross3(np_ + 3*i, A, f1);
+        for (int k = 0; k < 3; ++k) out[k] = s->n[3*i+k] + 0.5 * s->dt * (f0[3*i+k] + f1[k]);
+        double nrm = sqrt(dot3(out, out));
+        for (int k = 0; k < 3; ++k) s->n[3*i+k] = out[k] / nrm;
+    }
+    s->step += 1;
+    free(F); free(f0); free(np_); free(sg);
+}
+
+/* ------------------------------------------------------------------ what the boundary returns
+ * effective_field: deterministic F/(mu_s mu_B) in Tesla (reading R2).
+ * observables: M = (1/N) sum n_i (:131) and max_i |F_i - (F_i.n_i) n_i| in meV (reading R22). */
+void orc_effective_field(orc_system *s, double *B) {
+    orc_gradient(s, s->n, B, T_ALL);
+    for (long i = 0; i < s->N; ++i) {
+        double m = s->mu[i % s->nb] * ORC_MU_B;
+        for (int k = 0; k < 3; ++k) B[3*i+k] /= m;
+    }
+}
+void orc_observables(orc_system *s, double M[3], double *max_torque) {
+    double *F = (double *)malloc(3 * s->N * sizeof(double));
+    orc_gradient(s, s->n, F, T_ALL);
+    long double m[3] = {0, 0, 0}; double mt = 0.0;
+    for (long i = 0; i < s->N; ++i) {
+        const double *n = s->n + 3*i; double p = dot3(F + 3*i, n), t[3];
+        for (int k = 0; k < 3; ++k) { m[k] += n[k]; t[k] = F[3*i+k] - p * n[k]; }
+        double tn = sqrt(dot3(t, t));
+        if (tn > mt) mt = tn;
+    }
+    for (int k = 0; k < 3; ++k) M[k] = (double)(m[k] / (long double)s->N);
+    *max_torque = mt;
+    free(F);
+}
