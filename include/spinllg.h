@@ -1,0 +1,143 @@
+/*
+ * spinllg.h -- C-ABI boundary of the B200-native LLG hot path.
+ *
+ * One data-parallel path of "Spirit: Multifunctional Framework for Atomistic Spin Simulations"
+ * (arXiv 1901.11350; line numbers below are /root/reference/PAPER.md):
+ *
+ *     n  ->  F(n) = -dH/dn  (extended Heisenberg Hamiltonian, Eq. 1 :61-67 and Eq. 2 :75)
+ *        ->  Depondt predictor/corrector update of every spin (Eq. 10 :147-153, App. B B5-B7 :369-380)
+ *
+ * Every step of the path runs in hand-written CUDA kernels for sm_100a (cuFFT performs only the
+ * Fourier transforms of the dipolar convolution).  There is no CPU fallback: every call that needs the
+ * device returns SPIN_ERR_CUDA when no CUDA device is usable.
+ *
+ * Conventions
+ *   units       energy meV, field Tesla, moments mu_B, time fs at the API (ps inside), length Angstrom
+ *   constants   CODATA 2018: mu_B = 0.057883818060 meV/T, k_B = 0.08617333262 meV/K,
+ *               gamma = 0.176085963023 rad/(ps T), mu0 mu_B^2/(4 pi A^3) = 0.0536815112 meV
+ *   spin index  i = b + n_basis*(ia + Na*(ib + Nb*ic)), b the basis atom (fastest), (ia,ib,ic) the cell
+ *   arrays      "host" pointers are ordinary host memory owned by the caller; "device" pointers are
+ *               CUDA device memory owned by the caller.  All spin / field arrays at the boundary are
+ *               AoS: x0 y0 z0 x1 y1 z1 ... (3N doubles).  The internal layout is private.
+ *   ownership   the library owns all memory behind spin_system; setters copy, getters copy
+ *   errors      every function returns 0 (SPIN_OK) or a negative code; nothing throws across the ABI;
+ *               spin_last_error() gives a message for the last failure on the calling thread
+ *   ordering    setters may be called in any order; the device plan is (re)built lazily by the next
+ *               call that computes
+ *   streams     all device work of a system is enqueued on one CUDA stream (default: a private
+ *               non-blocking stream); spin_set_stream() rebinds it, e.g. to torch's current stream
+ */
+#ifndef SPINLLG_H
+#define SPINLLG_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct spin_system spin_system;
+
+enum {
+    SPIN_OK = 0,
+    SPIN_ERR_ARG = -1,        /* bad argument (null pointer, out-of-range index, self pair, ...) */
+    SPIN_ERR_STATE = -2,      /* call not valid in this state                                    */
+    SPIN_ERR_MEMORY = -3,     /* host or device allocation failed                                */
+    SPIN_ERR_CUDA = -4,       /* CUDA / cuFFT error, or no device                                */
+    SPIN_ERR_LIMIT = -5       /* interaction table larger than the kernels support               */
+};
+
+/* ---- geometry (PAPER.md:79 "Bravais vectors and basis cells with any given number of atoms"; :307 boundary
+ * conditions).  bravais: rows a, b, c in units of lattice_constant_A.  basis_frac: 3*n_basis fractional
+ * coordinates.  n_cells >= 1 each.  periodic: 0 = open, 1 = periodic per direction.  A 2-D lattice is
+ * n_cells[2] = 1 with periodic[2] = 0.  Initial state: all spins +z, mu_s = 1, no interactions.
+ * 1 <= n_basis <= 8, N = n_basis*prod(n_cells) < 2^31.                                                      */
+int spin_geometry_create(const double bravais[9], int n_basis, const double *basis_frac /*host*/,
+                         const int n_cells[3], const int periodic[3], double lattice_constant_A,
+                         spin_system **out);
+void spin_system_destroy(spin_system *sys);
+int64_t spin_system_nspins(const spin_system *sys);
+
+/* Bind the CUDA stream (a cudaStream_t passed as void*; NULL = back to the system's private stream).
+ * The legacy default stream cannot be captured into CUDA graphs and is not accepted. */
+int spin_set_stream(spin_system *sys, void *cuda_stream);
+
+/* ---- Hamiltonian, Eq. 1 (:61-67) and Eq. 2 (:75) ------------------------------------------------------- */
+/* magnetic moments mu_i per basis atom, in mu_B, > 0 (":59 m_i = mu_i n_i") */
+int hamiltonian_set_mu_s(spin_system *sys, const double *mu_s /*host, n_basis*/);
+/* Zeeman term -sum_i mu_i B.n_i: field magnitude in Tesla and direction (normalised internally) */
+int hamiltonian_set_field(spin_system *sys, double B_tesla, const double dir[3]);
+/* uniaxial anisotropy -sum_i K (K^.n_i)^2 with one axis per basis atom (":69 axes ... of the basis cell");
+ * n entries (basis_idx, K_meV, axis); atoms not listed get K = 0; a later call replaces the earlier one     */
+int hamiltonian_set_anisotropy(spin_system *sys, int n, const int *basis_idx, const double *K_meV,
+                               const double *axis /*host, 3n*/);
+/* unique pairs <ij> (":69 unique pairs", ":71 no limitation on number or distance"): pair p couples basis atom
+ * i_basis[p] in cell c with j_basis[p] in cell c + translation[p], with -J n_i.n_j - D.(n_i x n_j).
+ * Each bond is listed ONCE (either direction); D_ji = -D_ij is implied.  D_meV may be NULL (no DMI).
+ * Errors: index out of range, a pair of a site with itself (same basis atom, zero translation).
+ * Replaces any earlier explicit pair list (shell helpers below are kept separately and add up).             */
+int hamiltonian_set_pairs(spin_system *sys, int n_pairs, const int *i_basis, const int *j_basis,
+                          const int *translation /*host, 3*n_pairs*/, const double *J_meV,
+                          const double *D_meV /*host, 3*n_pairs or NULL*/);
+/* helper: exchange by neighbour shell; shell s (s = 0 nearest) gets J_meV[s] on all of its bonds.  The host
+ * neighbour finder only scans directions with n_cells > 1.                                                  */
+int hamiltonian_set_exchange_shells(spin_system *sys, int n_shells, const double *J_meV);
+/* helper: DMI by neighbour shell with a direction convention (the paper leaves D_ij to the user):
+ * chirality +1/-1: D_ij = +/- D r^_ij (bulk, Bloch);  +2/-2: D_ij = +/- D (z^ x r^_ij) (interfacial, Neel)    */
+int hamiltonian_set_dmi_shells(spin_system *sys, int n_shells, const double *D_meV, int chirality);
+/* quadruplets, Eq. 2: -K (n_i.n_j)(n_k.n_l); basis_ijkl: 4 basis atoms per quadruplet; translation_jkl: cell
+ * translations of j, k, l relative to i (9 ints per quadruplet).  Sites may repeat (4-spin-2-site, 3-site).  */
+int hamiltonian_set_quadruplets(spin_system *sys, int n, const int *basis_ijkl /*host, 4n*/,
+                                const int *translation_jkl /*host, 9n*/, const double *K_meV);
+/* dipole-dipole coupling through the zero-padded FFT convolution (:81-87).  n_periodic_images[d]: images
+ * t_d in [-n, n] summed in periodic direction d (ignored in open directions).                               */
+int hamiltonian_set_ddi(spin_system *sys, int enabled, const int n_periodic_images[3]);
+
+/* ---- state ---------------------------------------------------------------------------------------------- */
+/* spins are normalised on input; zero vectors are an error */
+int spins_set(spin_system *sys, const double *n_xyz /*host, 3N AoS*/);
+int spins_get(spin_system *sys, double *n_xyz /*host, 3N AoS*/);
+int spins_set_device(spin_system *sys, const double *n_xyz /*device, 3N AoS*/);
+int spins_get_device(spin_system *sys, double *n_xyz /*device, 3N AoS*/);
+
+/* ---- dynamics: Eq. 10 with the thermal field of Eq. 11 (:157-160), Depondt solver (App. B) --------------
+ * dt in fs; alpha Gilbert damping; T in Kelvin (0 = no noise); seed of the counter-based Philox4x32-10
+ * generator keyed by (seed; step, spin, block); u in Angstrom/ps along the unit vector j_dir; beta the
+ * non-adiabatic parameter.  Resets the step counter to 0.                                                   */
+int llg_configure(spin_system *sys, double dt_fs, double alpha, double T_kelvin, uint64_t seed,
+                  double u_A_per_ps, const double j_dir[3], double beta);
+/* advance n_steps Depondt steps; asynchronous on the system's stream.  The step counter persists, so
+ * llg_iterate(a); llg_iterate(b) reproduces llg_iterate(a+b) exactly.                                       */
+int llg_iterate(spin_system *sys, int64_t n_steps);
+int llg_get_step(const spin_system *sys, uint64_t *step);
+int llg_set_step(spin_system *sys, uint64_t step);
+/* wait for all work enqueued on the system's stream */
+int spin_synchronize(spin_system *sys);
+
+/* ---- observables ------------------------------------------------------------------------------------------
+ * effective_field: deterministic B_eff,i = -(1/(mu_i mu_B)) dH/dn_i in Tesla (:155), no noise, no current   */
+int effective_field(spin_system *sys, double *B_xyz /*host, 3N AoS*/);
+int effective_field_device(spin_system *sys, double *B_xyz /*device, 3N AoS*/);
+/* total energy and its terms (Zeeman, anisotropy, exchange, DMI, quadruplet, dipolar), meV; either may be NULL */
+int energy(spin_system *sys, double *E_total_meV, double E_terms_meV[6]);
+/* M = (1/N) sum_i n_i (:131) and max_i |F_i - (F_i.n_i) n_i| in meV                                        */
+int observables(spin_system *sys, double M[3], double *max_torque_meV);
+
+/* ---- introspection (measurement support) -------------------------------------------------------------- */
+/* number of kernel launches (own kernels) and cuFFT executions issued by this system so far */
+int spin_launch_counts(const spin_system *sys, int64_t *own_kernels, int64_t *cufft_execs);
+/* per-kernel device timing: when enabled, CUDA events bracket every launch of the step kernels; get returns the
+ * accumulated milliseconds and launch counts for kind = 0 predictor, 1 corrector, 2 ddi (all ddi stages).   */
+int spin_profile_enable(spin_system *sys, int enabled);
+int spin_profile_get(spin_system *sys, int kind, double *total_ms, int64_t *launches);
+/* execution options: use_graph (capture steps into a CUDA graph; default 1), store_A (1: predictor stores the
+ * rotation field A, 0: corrector recomputes it; default 0)                                                  */
+int spin_set_option(spin_system *sys, const char *name, int value);
+
+const char *spin_last_error(void);
+const char *spin_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SPINLLG_H */

@@ -1,0 +1,268 @@
+"""Thin ctypes binding of the C-ABI library (include/spinllg.h): argument marshalling only.
+
+Every step of the hot path runs inside libspinllg.so's CUDA kernels; this module only converts numpy arrays /
+torch device pointers to C pointers and raises SpinError on a non-zero return code.  There is no CPU fallback:
+if the library is missing it is built with nvcc, and if that fails the import of the library raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+from . import build as _build
+
+_LIB = None
+
+EXPORTS = [
+    "spin_geometry_create", "spin_system_destroy", "spin_system_nspins", "spin_set_stream",
+    "hamiltonian_set_mu_s", "hamiltonian_set_field", "hamiltonian_set_anisotropy", "hamiltonian_set_pairs",
+    "hamiltonian_set_exchange_shells", "hamiltonian_set_dmi_shells", "hamiltonian_set_quadruplets",
+    "hamiltonian_set_ddi", "spins_set", "spins_get", "spins_set_device", "spins_get_device",
+    "llg_configure", "llg_iterate", "llg_get_step", "llg_set_step", "spin_synchronize",
+    "effective_field", "effective_field_device", "energy", "observables",
+    "spin_launch_counts", "spin_profile_enable", "spin_profile_get", "spin_set_option",
+    "spin_last_error", "spin_version",
+]
+
+
+class SpinError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"spinllg error {code}: {msg}")
+        self.code = code
+
+
+def lib() -> C.CDLL:
+    """Load (building if stale) libspinllg.so and declare the prototypes of include/spinllg.h."""
+    global _LIB
+    if _LIB is not None:
+        return _LIB
+    path = _build.build()
+    if not os.path.exists(path):
+        raise ImportError("libspinllg.so is missing and could not be built; there is no CPU fallback")
+    L = C.CDLL(path)
+    dp, ip, vp = C.POINTER(C.c_double), C.POINTER(C.c_int), C.c_void_p
+    i64p = C.POINTER(C.c_int64)
+    proto = {
+        "spin_geometry_create": (C.c_int, [dp, C.c_int, dp, ip, ip, C.c_double, C.POINTER(vp)]),
+        "spin_system_destroy": (None, [vp]),
+        "spin_system_nspins": (C.c_int64, [vp]),
+        "spin_set_stream": (C.c_int, [vp, vp]),
+        "hamiltonian_set_mu_s": (C.c_int, [vp, dp]),
+        "hamiltonian_set_field": (C.c_int, [vp, C.c_double, dp]),
+        "hamiltonian_set_anisotropy": (C.c_int, [vp, C.c_int, ip, dp, dp]),
+        "hamiltonian_set_pairs": (C.c_int, [vp, C.c_int, ip, ip, ip, dp, dp]),
+        "hamiltonian_set_exchange_shells": (C.c_int, [vp, C.c_int, dp]),
+        "hamiltonian_set_dmi_shells": (C.c_int, [vp, C.c_int, dp, C.c_int]),
+        "hamiltonian_set_quadruplets": (C.c_int, [vp, C.c_int, ip, ip, dp]),
+        "hamiltonian_set_ddi": (C.c_int, [vp, C.c_int, ip]),
+        "spins_set": (C.c_int, [vp, dp]),
+        "spins_get": (C.c_int, [vp, dp]),
+        "spins_set_device": (C.c_int, [vp, vp]),
+        "spins_get_device": (C.c_int, [vp, vp]),
+        "llg_configure": (C.c_int, [vp, C.c_double, C.c_double, C.c_double, C.c_uint64, C.c_double, dp, C.c_double]),
+        "llg_iterate": (C.c_int, [vp, C.c_int64]),
+        "llg_get_step": (C.c_int, [vp, C.POINTER(C.c_uint64)]),
+        "llg_set_step": (C.c_int, [vp, C.c_uint64]),
+        "spin_synchronize": (C.c_int, [vp]),
+        "effective_field": (C.c_int, [vp, dp]),
+        "effective_field_device": (C.c_int, [vp, vp]),
+        "energy": (C.c_int, [vp, dp, dp]),
+        "observables": (C.c_int, [vp, dp, dp]),
+        "spin_launch_counts": (C.c_int, [vp, i64p, i64p]),
+        "spin_profile_enable": (C.c_int, [vp, C.c_int]),
+        "spin_profile_get": (C.c_int, [vp, C.c_int, dp, i64p]),
+        "spin_set_option": (C.c_int, [vp, C.c_char_p, C.c_int]),
+        "spin_last_error": (C.c_char_p, []),
+        "spin_version": (C.c_char_p, []),
+    }
+    for name, (res, args) in proto.items():
+        fn = getattr(L, name)          # AttributeError here = a symbol of spinllg.h is not exported
+        fn.restype = res
+        fn.argtypes = args
+    _LIB = L
+    return L
+
+
+def _check(rc):
+    if rc != 0:
+        raise SpinError(rc, lib().spin_last_error().decode())
+
+
+def _d(a):
+    a = np.ascontiguousarray(a, dtype=np.float64)
+    return a, a.ctypes.data_as(C.POINTER(C.c_double))
+
+
+def _i(a):
+    a = np.ascontiguousarray(a, dtype=np.int32)
+    return a, a.ctypes.data_as(C.POINTER(C.c_int))
+
+
+class SpinSystem:
+    """Python handle of a `spin_system*`; method names are the C-ABI names."""
+
+    def __init__(self, bravais, basis, n_cells, periodic, lattice_constant=1.0):
+        L = lib()
+        basis = np.atleast_2d(np.asarray(basis, float))
+        b_, bp = _d(np.asarray(bravais, float).reshape(9))
+        s_, sp = _d(basis.reshape(-1))
+        n_, npx = _i(n_cells)
+        p_, pp = _i(periodic)
+        h = C.c_void_p()
+        _check(L.spin_geometry_create(bp, basis.shape[0], sp, npx, pp, float(lattice_constant), C.byref(h)))
+        self._h = h
+        self.n_basis = basis.shape[0]
+        self.N = int(L.spin_system_nspins(h))
+
+    def close(self):
+        if getattr(self, "_h", None):
+            lib().spin_system_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    @classmethod
+    def from_workload(cls, w, use_shell_helpers=False, stream=None):
+        s = cls(w.bravais, w.basis, w.n_cells, w.periodic, w.lattice_constant)
+        if stream is not None:
+            s.spin_set_stream(stream)
+        s.hamiltonian_set_mu_s(w.mu_s)
+        s.hamiltonian_set_field(w.B, w.B_dir)
+        if w.aniso:
+            s.hamiltonian_set_anisotropy([a[0] for a in w.aniso], [a[1] for a in w.aniso], [a[2] for a in w.aniso])
+        if not use_shell_helpers:
+            s.hamiltonian_set_pairs(w.pair_i, w.pair_j, w.pair_t, w.pair_J, w.pair_D)
+        if len(w.quad_K):
+            s.hamiltonian_set_quadruplets(w.quad_b, w.quad_t, w.quad_K)
+        s.hamiltonian_set_ddi(w.ddi, w.ddi_images)
+        s.llg_configure(w.dt_fs, w.alpha, w.T, w.seed, w.u, w.j_dir, w.beta)
+        s.spins_set(w.initial_spins())
+        return s
+
+    # ---- C-ABI calls -----------------------------------------------------------------------------------
+    def spin_set_stream(self, stream):
+        """stream: int cudaStream_t handle (e.g. torch.cuda.current_stream().cuda_stream) or None."""
+        _check(lib().spin_set_stream(self._h, C.c_void_p(int(stream) if stream else None)))
+
+    def hamiltonian_set_mu_s(self, mu):
+        a, p = _d(np.broadcast_to(np.asarray(mu, float), (self.n_basis,)))
+        _check(lib().hamiltonian_set_mu_s(self._h, p))
+
+    def hamiltonian_set_field(self, B, direction):
+        a, p = _d(direction)
+        _check(lib().hamiltonian_set_field(self._h, float(B), p))
+
+    def hamiltonian_set_anisotropy(self, basis_idx, K, axis):
+        b, bp = _i(basis_idx)
+        k, kp = _d(K)
+        a, ap = _d(np.asarray(axis, float).reshape(-1))
+        _check(lib().hamiltonian_set_anisotropy(self._h, len(b), bp, kp, ap))
+
+    def hamiltonian_set_pairs(self, i, j, t, J, D=None):
+        i_, ip = _i(i)
+        j_, jp = _i(j)
+        t_, tp = _i(np.asarray(t).reshape(-1))
+        J_, Jp = _d(J)
+        Dp = None
+        if D is not None:
+            D_, Dp = _d(np.asarray(D, float).reshape(-1))
+        _check(lib().hamiltonian_set_pairs(self._h, len(i_), ip, jp, tp, Jp, Dp))
+
+    def hamiltonian_set_exchange_shells(self, J):
+        a, p = _d(J)
+        _check(lib().hamiltonian_set_exchange_shells(self._h, len(a), p))
+
+    def hamiltonian_set_dmi_shells(self, D, chirality):
+        a, p = _d(D)
+        _check(lib().hamiltonian_set_dmi_shells(self._h, len(a), p, int(chirality)))
+
+    def hamiltonian_set_quadruplets(self, basis_ijkl, trans_jkl, K):
+        b, bp = _i(np.asarray(basis_ijkl).reshape(-1))
+        t, tp = _i(np.asarray(trans_jkl).reshape(-1))
+        k, kp = _d(K)
+        _check(lib().hamiltonian_set_quadruplets(self._h, len(k), bp, tp, kp))
+
+    def hamiltonian_set_ddi(self, enabled, n_images=(0, 0, 0)):
+        n, p = _i(n_images)
+        _check(lib().hamiltonian_set_ddi(self._h, int(bool(enabled)), p))
+
+    def spins_set(self, n):
+        a, p = _d(np.asarray(n, float).reshape(-1))
+        if a.size != 3 * self.N:
+            raise ValueError("spins_set expects 3N doubles")
+        _check(lib().spins_set(self._h, p))
+
+    def spins_get(self, out=None):
+        out = np.empty((self.N, 3)) if out is None else out
+        _check(lib().spins_get(self._h, out.ctypes.data_as(C.POINTER(C.c_double))))
+        return out
+
+    def spins_set_device(self, dev_ptr):
+        _check(lib().spins_set_device(self._h, C.c_void_p(int(dev_ptr))))
+
+    def spins_get_device(self, dev_ptr):
+        _check(lib().spins_get_device(self._h, C.c_void_p(int(dev_ptr))))
+
+    def llg_configure(self, dt_fs, alpha, T=0.0, seed=0, u=0.0, j_dir=(1, 0, 0), beta=0.0):
+        j, jp = _d(j_dir)
+        _check(lib().llg_configure(self._h, float(dt_fs), float(alpha), float(T), int(seed), float(u), jp, float(beta)))
+
+    def llg_iterate(self, n_steps):
+        _check(lib().llg_iterate(self._h, int(n_steps)))
+
+    def llg_get_step(self):
+        v = C.c_uint64(0)
+        _check(lib().llg_get_step(self._h, C.byref(v)))
+        return int(v.value)
+
+    def llg_set_step(self, step):
+        _check(lib().llg_set_step(self._h, int(step)))
+
+    def spin_synchronize(self):
+        _check(lib().spin_synchronize(self._h))
+
+    def effective_field(self, out=None):
+        out = np.empty((self.N, 3)) if out is None else out
+        _check(lib().effective_field(self._h, out.ctypes.data_as(C.POINTER(C.c_double))))
+        return out
+
+    def effective_field_device(self, dev_ptr):
+        _check(lib().effective_field_device(self._h, C.c_void_p(int(dev_ptr))))
+
+    def energy(self):
+        tot = C.c_double(0.0)
+        terms = np.zeros(6)
+        _check(lib().energy(self._h, C.byref(tot), terms.ctypes.data_as(C.POINTER(C.c_double))))
+        return float(tot.value), terms
+
+    def observables(self):
+        M = np.zeros(3)
+        mt = C.c_double(0.0)
+        _check(lib().observables(self._h, M.ctypes.data_as(C.POINTER(C.c_double)), C.byref(mt)))
+        return M, float(mt.value)
+
+    def spin_launch_counts(self):
+        a, b = C.c_int64(0), C.c_int64(0)
+        _check(lib().spin_launch_counts(self._h, C.byref(a), C.byref(b)))
+        return int(a.value), int(b.value)
+
+    def spin_profile_enable(self, on=True):
+        _check(lib().spin_profile_enable(self._h, int(bool(on))))
+
+    def spin_profile_get(self, kind):
+        ms, n = C.c_double(0.0), C.c_int64(0)
+        _check(lib().spin_profile_get(self._h, int(kind), C.byref(ms), C.byref(n)))
+        return float(ms.value), int(n.value)
+
+    def spin_set_option(self, name, value):
+        _check(lib().spin_set_option(self._h, name.encode(), int(value)))
+
+
+def version() -> str:
+    return lib().spin_version().decode()

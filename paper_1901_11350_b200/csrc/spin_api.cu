@@ -1,0 +1,771 @@
+// spin_api.cu -- C-ABI entry points (include/spinllg.h), host planner and kernel launches.
+//
+// Host side of the path: geometry, the neighbour-shell finder, expansion of the unique pair / quadruplet lists into
+// per-basis-atom gather tables (forward + backward entries, D sign flipped backward), LLG prefactors,
+// and the launch sequence of one Depondt step (App. B :369-380):
+//     [DDI(n)] -> predictor -> [DDI(n^p)] -> corrector          (2 own kernels per step without DDI)
+// captured into a CUDA graph for launch-bound lattices.
+#include <math.h>
+#include <stdarg.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <algorithm>
+#include <map>
+
+#include "spin_kernels.cuh"
+
+using namespace spin;
+
+// ---------------------------------------------------------------------------------------------- errors
+static thread_local char g_err[512] = "";
+
+int spin::fail(int code, const char *fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+    return code;
+}
+extern "C" const char *spin_last_error(void) { return g_err; }
+extern "C" const char *spin_version(void) { return "spinllg-b200 0.1 (sm_100a, fp64)"; }
+
+#define REQUIRE(cond, ...)                                   \
+    do {                                                     \
+        if (!(cond)) return spin::fail(SPIN_ERR_ARG, __VA_ARGS__); \
+    } while (0)
+
+static void drop_graphs(spin_system *s) {
+    for (int k = 0; k < 2; ++k)
+        if (s->graph_exec[k]) { cudaGraphExecDestroy(s->graph_exec[k]); s->graph_exec[k] = nullptr; }
+    s->graph_steps = 0;
+}
+
+// ---------------------------------------------------------------------------------------------- brick shapes
+// 2-D lattices use 32x8x1 bricks, 3-D lattices 32x4x2 (256 threads either way).
+namespace {
+struct Launch { dim3 grid, block; bool flat; };
+
+Launch brick_launch(const spin_system *s) {
+    Launch L;
+    L.flat = s->nc[2] < 2;
+    const int BX = 32, BY = L.flat ? 8 : 4, BZ = L.flat ? 1 : 2;
+    const int nbx = (s->nc[0] + BX - 1) / BX, nby = (s->nc[1] + BY - 1) / BY, nbz = (s->nc[2] + BZ - 1) / BZ;
+    L.grid = dim3((unsigned)(nbx * nby * nbz), (unsigned)s->nb, 1);
+    L.block = dim3(256, 1, 1);
+    return L;
+}
+
+void cart(const spin_system *s, const double f[3], double r[3]) {
+    for (int k = 0; k < 3; ++k) r[k] = s->alat * (f[0] * s->brav[k] + f[1] * s->brav[3 + k] + f[2] * s->brav[6 + k]);
+}
+
+// translation reduced to the representative of smallest magnitude in a periodic direction
+int reduce_translation(int t, int n, int periodic) {
+    if (!periodic) return t;
+    int r = t % n;
+    if (r < 0) r += n;
+    if (2 * r > n) r -= n;
+    return r;
+}
+
+// ------------------------------------------------------------------------------------------ neighbour shells
+// All bonds (bi -> bj at translation t) sorted by length and grouped into shells; each bond once (the partner
+// direction (bj -> bi, -t) is the same bond).  Only directions with more than one cell are scanned.
+struct Bond { int bi, bj, t[3]; double r[3], len; };
+
+std::vector<std::vector<Bond>> find_shells(const spin_system *s, int n_shells) {
+    std::vector<std::vector<Bond>> shells;
+    for (int range = 2;; ++range) {
+        std::vector<Bond> all;
+        int lim[3];
+        for (int d = 0; d < 3; ++d) lim[d] = (s->nc[d] > 1) ? range : 0;
+        for (int bi = 0; bi < s->nb; ++bi)
+            for (int bj = 0; bj < s->nb; ++bj)
+                for (int t0 = -lim[0]; t0 <= lim[0]; ++t0)
+                    for (int t1 = -lim[1]; t1 <= lim[1]; ++t1)
+                        for (int t2 = -lim[2]; t2 <= lim[2]; ++t2) {
+                            if (bi == bj && t0 == 0 && t1 == 0 && t2 == 0) continue;
+                            // keep one representative of {(bi,bj,t), (bj,bi,-t)}
+                            const int key_a[5] = {bi, bj, t0, t1, t2}, key_b[5] = {bj, bi, -t0, -t1, -t2};
+                            if (std::lexicographical_compare(key_b, key_b + 5, key_a, key_a + 5)) continue;
+                            Bond b;
+                            b.bi = bi; b.bj = bj; b.t[0] = t0; b.t[1] = t1; b.t[2] = t2;
+                            const double f[3] = {t0 + s->basis[3 * bj] - s->basis[3 * bi], t1 + s->basis[3 * bj + 1] - s->basis[3 * bi + 1],
+                                                 t2 + s->basis[3 * bj + 2] - s->basis[3 * bi + 2]};
+                            cart(s, f, b.r);
+                            b.len = sqrt(b.r[0] * b.r[0] + b.r[1] * b.r[1] + b.r[2] * b.r[2]);
+                            all.push_back(b);
+                        }
+        std::stable_sort(all.begin(), all.end(), [](const Bond &x, const Bond &y) { return x.len < y.len; });
+        shells.clear();
+        const double tol = 1e-6 * s->alat;
+        for (const Bond &b : all) {
+            if (shells.empty() || b.len > shells.back().front().len + tol) shells.emplace_back();
+            shells.back().push_back(b);
+        }
+        // shells are complete only up to the radius the scan certainly covers
+        double rmin = 1e300;
+        for (int d = 0; d < 3; ++d) {
+            if (lim[d] == 0) continue;
+            // distance between lattice planes along direction d bounds what a scan of `range` cells covers
+            double a[3], b2[3], c[3];
+            const int d1 = (d + 1) % 3, d2 = (d + 2) % 3;
+            for (int k = 0; k < 3; ++k) { a[k] = s->brav[3 * d + k]; b2[k] = s->brav[3 * d1 + k]; c[k] = s->brav[3 * d2 + k]; }
+            double nrm[3] = {b2[1] * c[2] - b2[2] * c[1], b2[2] * c[0] - b2[0] * c[2], b2[0] * c[1] - b2[1] * c[0]};
+            const double nn = sqrt(nrm[0] * nrm[0] + nrm[1] * nrm[1] + nrm[2] * nrm[2]);
+            const double h = fabs(a[0] * nrm[0] + a[1] * nrm[1] + a[2] * nrm[2]) / nn * s->alat;
+            rmin = std::min(rmin, h * (range - 1));
+        }
+        int complete = 0;
+        for (auto &sh : shells) if (sh.front().len < rmin - tol) ++complete; else break;
+        if (complete >= n_shells || range > 12 || rmin == 1e300) {
+            shells.resize(std::min<size_t>(shells.size(), (size_t)n_shells));
+            return shells;
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------ plan
+int stt_coefficients(const spin_system *s, double cd[3]) {
+    // j^ = sum_d c_d a_d over the directions with more than one cell (least squares if fewer than three)
+    int act[3], na = 0;
+    for (int d = 0; d < 3; ++d) { cd[d] = 0.0; if (s->nc[d] > 1) act[na++] = d; }
+    if (na == 0) return 0;
+    double G[3][4];
+    for (int p = 0; p < na; ++p) {
+        double ap[3];
+        for (int k = 0; k < 3; ++k) ap[k] = s->alat * s->brav[3 * act[p] + k];
+        G[p][3] = ap[0] * s->jdir[0] + ap[1] * s->jdir[1] + ap[2] * s->jdir[2];
+        for (int q = 0; q < na; ++q) {
+            double aq[3];
+            for (int k = 0; k < 3; ++k) aq[k] = s->alat * s->brav[3 * act[q] + k];
+            G[p][q] = ap[0] * aq[0] + ap[1] * aq[1] + ap[2] * aq[2];
+        }
+    }
+    for (int p = 0; p < na; ++p) {          // Gauss-Jordan with partial pivoting on the normal equations
+        int piv = p;
+        for (int r = p + 1; r < na; ++r) if (fabs(G[r][p]) > fabs(G[piv][p])) piv = r;
+        if (fabs(G[piv][p]) < 1e-300) return -1;
+        if (piv != p) for (int q = 0; q < 4; ++q) std::swap(G[p][q], G[piv][q]);
+        for (int r = 0; r < na; ++r) {
+            if (r == p) continue;
+            const double f = G[r][p] / G[p][p];
+            for (int q = p; q < na; ++q) G[r][q] -= f * G[p][q];
+            G[r][3] -= f * G[p][3];
+        }
+    }
+    for (int p = 0; p < na; ++p) cd[act[p]] = G[p][3] / G[p][p];
+    return 0;
+}
+
+int build_plan(spin_system *s) {
+    DevicePlan &P = s->plan;
+    memset(&P, 0, sizeof(P));
+    P.Na = s->nc[0]; P.Nb = s->nc[1]; P.Nc = s->nc[2];
+    P.perA = s->per[0]; P.perB = s->per[1]; P.perC = s->per[2];
+    P.nb = s->nb; P.Ncell = (int)s->ncell; P.stride = s->stride;
+    const double a2 = 1.0 + s->alpha * s->alpha;
+    for (int b = 0; b < s->nb; ++b) {
+        const double m = s->mu[b] * MU_B;
+        for (int k = 0; k < 3; ++k) { P.zee[b][k] = m * s->Bmag * s->Bdir[k]; P.Kax[b][k] = s->Kax[3 * b + k]; }
+        P.K2[b] = 2.0 * s->K[b];
+        P.pre[b] = -GAMMA / (a2 * m);
+        P.sigma[b] = (s->T > 0.0) ? sqrt(2.0 * s->alpha * K_B * s->T * m / (GAMMA * s->dt_ps)) : 0.0;
+        P.inv_mu[b] = 1.0 / m;
+    }
+    P.alpha = s->alpha; P.dt = s->dt_ps; P.dt2 = s->dt_ps * s->dt_ps;
+    P.thermal_on = (s->T > 0.0) ? 1 : 0;
+    P.seed_lo = (uint32_t)s->seed; P.seed_hi = (uint32_t)(s->seed >> 32);
+    P.has_ddi = s->ddi_on ? 1 : 0;
+    P.stt_on = (s->u != 0.0) ? 1 : 0;
+    if (P.stt_on) {
+        if (stt_coefficients(s, P.stt_c) != 0) return spin::fail(SPIN_ERR_ARG, "current direction: singular lattice metric");
+        P.stt_s = -s->u * (s->alpha - s->beta) / a2;
+        P.stt_x = s->u * (1.0 + s->alpha * s->beta) / a2;
+        for (int d = 0; d < 3; ++d) if (P.stt_c[d] != 0.0) P.reach[d] = 1;
+    }
+    // ---- pair gather tables: every unique pair gives a forward entry for basis atom bi (+t, +D) and a backward
+    // entry for bj (-t, -D).  Order per atom: all forward entries in list order, then all backward entries.
+    std::vector<HostPair> all;
+    all.insert(all.end(), s->pairs_explicit.begin(), s->pairs_explicit.end());
+    all.insert(all.end(), s->pairs_exch_shells.begin(), s->pairs_exch_shells.end());
+    all.insert(all.end(), s->pairs_dmi_shells.begin(), s->pairs_dmi_shells.end());
+    const int Nd[3] = {s->nc[0], s->nc[1], s->nc[2]};
+    int ne = 0;
+    for (int b = 0; b < s->nb; ++b) {
+        P.pair_begin[b] = ne;
+        for (int dir = 0; dir < 2; ++dir)
+            for (const HostPair &p : all) {
+                if ((dir == 0 ? p.bi : p.bj) != b) continue;
+                const double sgn = dir == 0 ? 1.0 : -1.0;
+                PairEntry e;
+                memset(&e, 0, sizeof(e));
+                int t[3];
+                bool dead = false;
+                for (int d = 0; d < 3; ++d) {
+                    t[d] = reduce_translation((dir == 0 ? 1 : -1) * p.t[d], Nd[d], s->per[d]);
+                    if (!s->per[d] && abs(t[d]) >= Nd[d]) dead = true;      // never inside an open lattice
+                }
+                if (dead) continue;
+                e.da = t[0]; e.db = t[1]; e.dc = t[2];
+                e.bj = dir == 0 ? p.bj : p.bi;
+                e.lin = (e.bj - b) * (int)s->ncell + t[0] + Nd[0] * (t[1] + Nd[1] * t[2]);
+                e.J = p.J; e.Dx = sgn * p.D[0]; e.Dy = sgn * p.D[1]; e.Dz = sgn * p.D[2];
+                // merge with an existing entry on the same partner (e.g. exchange shells + DMI shells on one bond)
+                bool merged = false;
+                for (int q = P.pair_begin[b]; q < ne; ++q) {
+                    PairEntry &o = P.pairs[q];
+                    if (o.bj == e.bj && o.da == e.da && o.db == e.db && o.dc == e.dc) {
+                        o.J += e.J; o.Dx += e.Dx; o.Dy += e.Dy; o.Dz += e.Dz;
+                        merged = true;
+                        break;
+                    }
+                }
+                if (merged) continue;
+                if (ne >= SPIN_MAX_PAIR_ENTRIES)
+                    return spin::fail(SPIN_ERR_LIMIT, "pair table needs more than %d gather entries", SPIN_MAX_PAIR_ENTRIES);
+                P.pairs[ne++] = e;
+                for (int d = 0; d < 3; ++d) P.reach[d] = std::max(P.reach[d], abs(t[d]));
+            }
+    }
+    P.pair_begin[s->nb] = ne;
+    // ---- quadruplet role tables (Eq. 2): role r of quadruplet q for basis atom b = q.b[r]
+    int nq = 0;
+    for (int b = 0; b < s->nb; ++b) {
+        P.quad_begin[b] = nq;
+        for (const HostQuad &q : s->quads) {
+            int tm[4][3] = {{0, 0, 0}, {q.t[0], q.t[1], q.t[2]}, {q.t[3], q.t[4], q.t[5]}, {q.t[6], q.t[7], q.t[8]}};
+            for (int role = 0; role < 4; ++role) {
+                if (q.b[role] != b) continue;
+                // F_role += K (n_Q . n_R) n_P
+                const int Pm = role == 0 ? 1 : role == 1 ? 0 : role == 2 ? 3 : 2;
+                const int Qm = role < 2 ? 2 : 0, Rm = role < 2 ? 3 : 1;
+                const int mem[3] = {Pm, Qm, Rm};
+                QuadEntry e;
+                memset(&e, 0, sizeof(e));
+                bool dead = false;
+                for (int m = 0; m < 3; ++m) {
+                    for (int d = 0; d < 3; ++d) {
+                        const int t = reduce_translation(tm[mem[m]][d] - tm[role][d], Nd[d], s->per[d]);
+                        if (!s->per[d] && abs(t) >= Nd[d]) dead = true;
+                        e.d[m][d] = t;
+                        P.reach[d] = std::max(P.reach[d], abs(t));
+                    }
+                    e.b[m] = q.b[mem[m]];
+                    e.lin[m] = (e.b[m] - b) * (int)s->ncell + e.d[m][0] + Nd[0] * (e.d[m][1] + Nd[1] * e.d[m][2]);
+                }
+                if (dead) continue;      // some member can never be inside an open lattice
+                e.K = q.K;
+                if (nq >= SPIN_MAX_QUAD_ENTRIES)
+                    return spin::fail(SPIN_ERR_LIMIT, "quadruplet table needs more than %d role entries", SPIN_MAX_QUAD_ENTRIES);
+                P.quads[nq++] = e;
+            }
+        }
+    }
+    P.quad_begin[s->nb] = nq;
+    // an entry whose reduced translation equals the lattice size can only be interior-tested with a real margin
+    for (int d = 0; d < 3; ++d) if (P.reach[d] >= Nd[d]) P.reach[d] = Nd[d];   // never interior in that direction
+    return SPIN_OK;
+}
+
+int ensure_plan(spin_system *s) {
+    if (!s->plan_dirty) return SPIN_OK;
+    int rc = build_plan(s);
+    if (rc) return rc;
+    drop_graphs(s);
+    if (s->ddi_on) {
+        if (!s->d_fddi[0]) {
+            SPIN_CUDA(cudaMalloc(&s->d_fddi[0], (size_t)3 * s->stride * sizeof(double)));
+            SPIN_CUDA(cudaMalloc(&s->d_fddi[1], (size_t)3 * s->stride * sizeof(double)));
+        }
+        rc = ddi_prepare(s);
+        if (rc) return rc;
+    } else {
+        ddi_release(s);
+    }
+    s->plan_dirty = false;
+    return SPIN_OK;
+}
+
+// one Depondt step enqueued on the stream; step_add is added to the device step counter by the kernels
+template <int BX, int BY, int BZ>
+int enqueue_step_t(spin_system *s, const Launch &L, unsigned step_add) {
+    double *n = s->d_n[s->cur], *nout = s->d_n[s->cur ^ 1];
+    const bool prof = s->profile_on != 0;
+    if (s->ddi_on) {
+        if (prof) cudaEventRecord(s->ev0, s->stream);
+        int rc = ddi_field(s, n, s->d_fddi[0]);
+        if (rc) return rc;
+        if (prof) { cudaEventRecord(s->ev1, s->stream); cudaEventSynchronize(s->ev1); float ms; cudaEventElapsedTime(&ms, s->ev0, s->ev1); s->prof_ms[2] += ms; s->prof_n[2]++; }
+    }
+    if (prof) cudaEventRecord(s->ev0, s->stream);
+    if (s->opt_store_A)
+        predictor_kernel<BX, BY, BZ, true><<<L.grid, L.block, 0, s->stream>>>(s->plan, n, s->d_fddi[0], s->d_np, s->d_A, s->d_step, step_add);
+    else
+        predictor_kernel<BX, BY, BZ, false><<<L.grid, L.block, 0, s->stream>>>(s->plan, n, s->d_fddi[0], s->d_np, nullptr, s->d_step, step_add);
+    s->n_launch++;
+    if (prof) { cudaEventRecord(s->ev1, s->stream); cudaEventSynchronize(s->ev1); float ms; cudaEventElapsedTime(&ms, s->ev0, s->ev1); s->prof_ms[0] += ms; s->prof_n[0]++; }
+    if (s->ddi_on) {
+        if (prof) cudaEventRecord(s->ev0, s->stream);
+        int rc = ddi_field(s, s->d_np, s->d_fddi[1]);
+        if (rc) return rc;
+        if (prof) { cudaEventRecord(s->ev1, s->stream); cudaEventSynchronize(s->ev1); float ms; cudaEventElapsedTime(&ms, s->ev0, s->ev1); s->prof_ms[2] += ms; s->prof_n[2]++; }
+    }
+    if (prof) cudaEventRecord(s->ev0, s->stream);
+    if (s->opt_store_A)
+        corrector_kernel<BX, BY, BZ, true><<<L.grid, L.block, 0, s->stream>>>(s->plan, n, s->d_np, s->d_fddi[0], s->d_fddi[1], s->d_A, nout, s->d_step, step_add);
+    else
+        corrector_kernel<BX, BY, BZ, false><<<L.grid, L.block, 0, s->stream>>>(s->plan, n, s->d_np, s->d_fddi[0], s->d_fddi[1], nullptr, nout, s->d_step, step_add);
+    s->n_launch++;
+    if (prof) { cudaEventRecord(s->ev1, s->stream); cudaEventSynchronize(s->ev1); float ms; cudaEventElapsedTime(&ms, s->ev0, s->ev1); s->prof_ms[1] += ms; s->prof_n[1]++; }
+    s->cur ^= 1;
+    return SPIN_OK;
+}
+int enqueue_step(spin_system *s, unsigned step_add) {
+    const Launch L = brick_launch(s);
+    return L.flat ? enqueue_step_t<32, 8, 1>(s, L, step_add) : enqueue_step_t<32, 4, 2>(s, L, step_add);
+}
+
+// deterministic force of the current configuration into d_np (scratch), terms by mask
+int enqueue_force(spin_system *s, int mask, double *d_out) {
+    const Launch L = brick_launch(s);
+    double *n = s->d_n[s->cur];
+    if (s->ddi_on && (mask & T_DDI)) { int rc = ddi_field(s, n, s->d_fddi[0]); if (rc) return rc; }
+    if (L.flat) force_kernel<32, 8, 1><<<L.grid, L.block, 0, s->stream>>>(s->plan, n, s->d_fddi[0], mask, d_out);
+    else force_kernel<32, 4, 2><<<L.grid, L.block, 0, s->stream>>>(s->plan, n, s->d_fddi[0], mask, d_out);
+    s->n_launch++;
+    return SPIN_OK;
+}
+
+int reduce_all(spin_system *s, double out[N_RED]) {
+    const Launch L = brick_launch(s);
+    double *n = s->d_n[s->cur];
+    if (s->ddi_on) { int rc = ddi_field(s, n, s->d_fddi[0]); if (rc) return rc; }
+    const int nblocks = (int)(L.grid.x * L.grid.y);
+    if (L.flat) reduce_kernel<32, 8, 1><<<L.grid, L.block, 0, s->stream>>>(s->plan, n, s->d_fddi[0], s->d_partials);
+    else reduce_kernel<32, 4, 2><<<L.grid, L.block, 0, s->stream>>>(s->plan, n, s->d_fddi[0], s->d_partials);
+    reduce_final_kernel<<<1, 32 * N_RED, 0, s->stream>>>(s->d_partials, nblocks, s->d_result);
+    s->n_launch += 2;
+    SPIN_CUDA(cudaMemcpyAsync(out, s->d_result, N_RED * sizeof(double), cudaMemcpyDeviceToHost, s->stream));
+    SPIN_CUDA(cudaStreamSynchronize(s->stream));
+    SPIN_CUDA(cudaGetLastError());
+    return SPIN_OK;
+}
+
+}  // namespace
+
+// ---------------------------------------------------------------------------------------------- lifecycle
+extern "C" int spin_geometry_create(const double bravais[9], int n_basis, const double *basis_frac, const int n_cells[3],
+                                    const int periodic[3], double lattice_constant_A, spin_system **out) {
+    REQUIRE(bravais && basis_frac && n_cells && periodic && out, "null argument");
+    REQUIRE(n_basis >= 1 && n_basis <= SPIN_MAX_BASIS, "n_basis must be in [1, %d]", SPIN_MAX_BASIS);
+    REQUIRE(lattice_constant_A > 0.0, "lattice constant must be positive");
+    int64_t ncell = 1;
+    for (int d = 0; d < 3; ++d) { REQUIRE(n_cells[d] >= 1, "n_cells must be >= 1"); ncell *= n_cells[d]; }
+    REQUIRE(ncell * n_basis < (int64_t)2147483647 / 3, "lattice too large for 32-bit indexing");
+    const double *a = bravais, *b = bravais + 3, *c = bravais + 6;
+    const double vol = a[0] * (b[1] * c[2] - b[2] * c[1]) - a[1] * (b[0] * c[2] - b[2] * c[0]) + a[2] * (b[0] * c[1] - b[1] * c[0]);
+    REQUIRE(fabs(vol) > 1e-12, "bravais vectors are linearly dependent");
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1)
+        return spin::fail(SPIN_ERR_CUDA, "no CUDA device: this library has no CPU fallback");
+    spin_system *s = new spin_system();
+    memcpy(s->brav, bravais, sizeof(s->brav));
+    s->nb = n_basis;
+    s->basis.assign(basis_frac, basis_frac + 3 * n_basis);
+    for (int d = 0; d < 3; ++d) { s->nc[d] = n_cells[d]; s->per[d] = periodic[d] ? 1 : 0; }
+    s->alat = lattice_constant_A;
+    s->ncell = ncell; s->N = ncell * n_basis;
+    s->stride = (int)((s->N + 63) / 64 * 64);
+    s->mu.assign(n_basis, 1.0);
+    s->Bmag = 0.0; s->Bdir[0] = 0; s->Bdir[1] = 0; s->Bdir[2] = 1;
+    s->K.assign(n_basis, 0.0);
+    s->Kax.assign(3 * n_basis, 0.0);
+    for (int bb = 0; bb < n_basis; ++bb) s->Kax[3 * bb + 2] = 1.0;
+    s->ddi_on = 0; s->ddi_img[0] = s->ddi_img[1] = s->ddi_img[2] = 0;
+    s->dt_ps = 1e-3; s->alpha = 0.1; s->T = 0; s->u = 0; s->jdir[0] = 1; s->jdir[1] = 0; s->jdir[2] = 0; s->beta = 0;
+    s->seed = 0; s->step = 0;
+    s->stream = nullptr; s->own_stream = nullptr; s->cur = 0;
+    s->d_n[0] = s->d_n[1] = s->d_np = s->d_A = s->d_fddi[0] = s->d_fddi[1] = s->d_aos = s->d_partials = s->d_result = nullptr;
+    s->d_step = nullptr; s->ddi = nullptr; s->plan_dirty = true;
+    s->opt_graph = 1; s->opt_store_A = 0; s->graph_exec[0] = s->graph_exec[1] = nullptr; s->graph_steps = 0;
+    s->n_launch = s->n_fft = 0; s->profile_on = 0;
+    for (int k = 0; k < 3; ++k) { s->prof_ms[k] = 0; s->prof_n[k] = 0; }
+    s->ev0 = s->ev1 = nullptr;
+    const size_t bytes = (size_t)3 * s->stride * sizeof(double);
+    const Launch L = brick_launch(s);
+    cudaError_t e = cudaStreamCreateWithFlags(&s->own_stream, cudaStreamNonBlocking);
+    s->stream = s->own_stream;
+    if (e == cudaSuccess) e = cudaMalloc(&s->d_n[0], bytes);
+    if (e == cudaSuccess) e = cudaMalloc(&s->d_n[1], bytes);
+    if (e == cudaSuccess) e = cudaMalloc(&s->d_np, bytes);
+    if (e == cudaSuccess) e = cudaMalloc(&s->d_A, bytes);
+    if (e == cudaSuccess) e = cudaMalloc(&s->d_aos, (size_t)3 * s->N * sizeof(double) + sizeof(int));
+    if (e == cudaSuccess) e = cudaMalloc(&s->d_partials, (size_t)L.grid.x * L.grid.y * N_RED * sizeof(double));
+    if (e == cudaSuccess) e = cudaMalloc(&s->d_result, 16 * sizeof(double));
+    if (e == cudaSuccess) e = cudaMalloc(&s->d_step, sizeof(unsigned long long));
+    if (e == cudaSuccess) e = cudaMemset(s->d_step, 0, sizeof(unsigned long long));
+    if (e == cudaSuccess) e = cudaMemset(s->d_n[0], 0, bytes);
+    if (e == cudaSuccess) e = cudaMemset(s->d_n[1], 0, bytes);
+    if (e == cudaSuccess) e = cudaMemset(s->d_np, 0, bytes);
+    if (e == cudaSuccess) e = cudaEventCreate(&s->ev0);
+    if (e == cudaSuccess) e = cudaEventCreate(&s->ev1);
+    if (e == cudaSuccess) e = cudaDeviceSynchronize();
+    if (e != cudaSuccess) {
+        const int code = (e == cudaErrorMemoryAllocation) ? SPIN_ERR_MEMORY : SPIN_ERR_CUDA;
+        spin::fail(code, "device setup failed: %s", cudaGetErrorString(e));
+        spin_system_destroy(s);
+        return code;
+    }
+    // initial state: all spins +z
+    std::vector<double> z((size_t)3 * s->N, 0.0);
+    for (int64_t i = 0; i < s->N; ++i) z[3 * i + 2] = 1.0;
+    *out = s;
+    int rc = spins_set(s, z.data());
+    if (rc) { spin_system_destroy(s); *out = nullptr; return rc; }
+    return SPIN_OK;
+}
+
+extern "C" void spin_system_destroy(spin_system *s) {
+    if (!s) return;
+    drop_graphs(s);
+    if (s->own_stream) cudaStreamDestroy(s->own_stream);
+    ddi_release(s);
+    cudaFree(s->d_n[0]); cudaFree(s->d_n[1]); cudaFree(s->d_np); cudaFree(s->d_A); cudaFree(s->d_fddi[0]); cudaFree(s->d_fddi[1]);
+    cudaFree(s->d_aos); cudaFree(s->d_partials); cudaFree(s->d_result); cudaFree(s->d_step);
+    if (s->ev0) cudaEventDestroy(s->ev0);
+    if (s->ev1) cudaEventDestroy(s->ev1);
+    delete s;
+}
+
+extern "C" int64_t spin_system_nspins(const spin_system *s) { return s ? s->N : 0; }
+
+extern "C" int spin_set_stream(spin_system *s, void *stream) {
+    REQUIRE(s, "null system");
+    SPIN_CUDA(cudaStreamSynchronize(s->stream));
+    s->stream = stream ? (cudaStream_t)stream : s->own_stream;
+    drop_graphs(s);
+    if (s->ddi) s->plan_dirty = true;     // cuFFT plans are bound to a stream
+    return SPIN_OK;
+}
+
+// ---------------------------------------------------------------------------------------------- Hamiltonian setters
+extern "C" int hamiltonian_set_mu_s(spin_system *s, const double *mu) {
+    REQUIRE(s && mu, "null argument");
+    for (int b = 0; b < s->nb; ++b) REQUIRE(mu[b] > 0.0 && isfinite(mu[b]), "mu_s must be positive");
+    s->mu.assign(mu, mu + s->nb);
+    s->plan_dirty = true;
+    return SPIN_OK;
+}
+extern "C" int hamiltonian_set_field(spin_system *s, double B, const double dir[3]) {
+    REQUIRE(s && dir, "null argument");
+    const double n = sqrt(dir[0] * dir[0] + dir[1] * dir[1] + dir[2] * dir[2]);
+    REQUIRE(isfinite(B) && (n > 0.0 || B == 0.0), "field direction must be non-zero");
+    s->Bmag = B;
+    for (int k = 0; k < 3; ++k) s->Bdir[k] = n > 0.0 ? dir[k] / n : (k == 2 ? 1.0 : 0.0);
+    s->plan_dirty = true;
+    return SPIN_OK;
+}
+extern "C" int hamiltonian_set_anisotropy(spin_system *s, int n, const int *bidx, const double *K, const double *axis) {
+    REQUIRE(s && n >= 0 && (n == 0 || (bidx && K && axis)), "bad argument");
+    std::vector<double> Kn(s->nb, 0.0), ax(3 * s->nb, 0.0);
+    for (int b = 0; b < s->nb; ++b) ax[3 * b + 2] = 1.0;
+    for (int e = 0; e < n; ++e) {
+        REQUIRE(bidx[e] >= 0 && bidx[e] < s->nb, "anisotropy: basis index %d out of range", bidx[e]);
+        const double *a = axis + 3 * e;
+        const double nn = sqrt(a[0] * a[0] + a[1] * a[1] + a[2] * a[2]);
+        REQUIRE(nn > 0.0 && isfinite(K[e]), "anisotropy: zero axis or non-finite K");
+        Kn[bidx[e]] = K[e];
+        for (int k = 0; k < 3; ++k) ax[3 * bidx[e] + k] = a[k] / nn;
+    }
+    s->K = Kn; s->Kax = ax;
+    s->plan_dirty = true;
+    return SPIN_OK;
+}
+extern "C" int hamiltonian_set_pairs(spin_system *s, int np, const int *bi, const int *bj, const int *t, const double *J, const double *D) {
+    REQUIRE(s && np >= 0 && (np == 0 || (bi && bj && t && J)), "bad argument");
+    std::vector<HostPair> v;
+    std::map<std::vector<int>, int> seen;
+    for (int p = 0; p < np; ++p) {
+        REQUIRE(bi[p] >= 0 && bi[p] < s->nb && bj[p] >= 0 && bj[p] < s->nb, "pair %d: basis index out of range", p);
+        REQUIRE(!(bi[p] == bj[p] && t[3 * p] == 0 && t[3 * p + 1] == 0 && t[3 * p + 2] == 0), "pair %d couples a site with itself", p);
+        // the same bond listed in both directions would be double counting (":69 unique pairs")
+        std::vector<int> fwd = {bi[p], bj[p], t[3 * p], t[3 * p + 1], t[3 * p + 2]}, bwd = {bj[p], bi[p], -t[3 * p], -t[3 * p + 1], -t[3 * p + 2]};
+        REQUIRE(!seen.count(bwd) || fwd == bwd, "pair %d repeats pair %d in the opposite direction", p, seen.count(bwd) ? seen[bwd] : -1);
+        seen[fwd] = p;
+        HostPair h;
+        h.bi = bi[p]; h.bj = bj[p];
+        for (int k = 0; k < 3; ++k) { h.t[k] = t[3 * p + k]; h.D[k] = D ? D[3 * p + k] : 0.0; }
+        h.J = J[p];
+        REQUIRE(isfinite(h.J) && isfinite(h.D[0]) && isfinite(h.D[1]) && isfinite(h.D[2]), "pair %d: non-finite coupling", p);
+        v.push_back(h);
+    }
+    s->pairs_explicit.swap(v);
+    s->plan_dirty = true;
+    return SPIN_OK;
+}
+extern "C" int hamiltonian_set_exchange_shells(spin_system *s, int n_shells, const double *J) {
+    REQUIRE(s && n_shells >= 0 && (n_shells == 0 || J), "bad argument");
+    std::vector<HostPair> v;
+    if (n_shells > 0) {
+        auto shells = find_shells(s, n_shells);
+        REQUIRE((int)shells.size() == n_shells, "only %d neighbour shells exist on this lattice", (int)shells.size());
+        for (int k = 0; k < n_shells; ++k)
+            for (const Bond &b : shells[k]) {
+                HostPair h;
+                h.bi = b.bi; h.bj = b.bj; h.J = J[k];
+                for (int d = 0; d < 3; ++d) { h.t[d] = b.t[d]; h.D[d] = 0.0; }
+                v.push_back(h);
+            }
+    }
+    s->pairs_exch_shells.swap(v);
+    s->plan_dirty = true;
+    return SPIN_OK;
+}
+extern "C" int hamiltonian_set_dmi_shells(spin_system *s, int n_shells, const double *Dm, int chirality) {
+    REQUIRE(s && n_shells >= 0 && (n_shells == 0 || Dm), "bad argument");
+    REQUIRE(chirality == 1 || chirality == -1 || chirality == 2 || chirality == -2, "chirality must be +-1 (bulk) or +-2 (interfacial)");
+    std::vector<HostPair> v;
+    if (n_shells > 0) {
+        auto shells = find_shells(s, n_shells);
+        REQUIRE((int)shells.size() == n_shells, "only %d neighbour shells exist on this lattice", (int)shells.size());
+        for (int k = 0; k < n_shells; ++k)
+            for (const Bond &b : shells[k]) {
+                HostPair h;
+                h.bi = b.bi; h.bj = b.bj; h.J = 0.0;
+                const double rh[3] = {b.r[0] / b.len, b.r[1] / b.len, b.r[2] / b.len};
+                const double sg = chirality > 0 ? 1.0 : -1.0;
+                if (abs(chirality) == 1) { h.D[0] = sg * Dm[k] * rh[0]; h.D[1] = sg * Dm[k] * rh[1]; h.D[2] = sg * Dm[k] * rh[2]; }
+                else { h.D[0] = sg * Dm[k] * (-rh[1]); h.D[1] = sg * Dm[k] * rh[0]; h.D[2] = 0.0; }      // z x r
+                for (int d = 0; d < 3; ++d) h.t[d] = b.t[d];
+                v.push_back(h);
+            }
+    }
+    s->pairs_dmi_shells.swap(v);
+    s->plan_dirty = true;
+    return SPIN_OK;
+}
+extern "C" int hamiltonian_set_quadruplets(spin_system *s, int n, const int *b4, const int *t9, const double *K) {
+    REQUIRE(s && n >= 0 && (n == 0 || (b4 && t9 && K)), "bad argument");
+    std::vector<HostQuad> v;
+    for (int q = 0; q < n; ++q) {
+        HostQuad h;
+        for (int k = 0; k < 4; ++k) { h.b[k] = b4[4 * q + k]; REQUIRE(h.b[k] >= 0 && h.b[k] < s->nb, "quadruplet %d: basis index out of range", q); }
+        for (int k = 0; k < 9; ++k) h.t[k] = t9[9 * q + k];
+        h.K = K[q];
+        REQUIRE(isfinite(h.K), "quadruplet %d: non-finite K", q);
+        v.push_back(h);
+    }
+    s->quads.swap(v);
+    s->plan_dirty = true;
+    return SPIN_OK;
+}
+extern "C" int hamiltonian_set_ddi(spin_system *s, int enabled, const int img[3]) {
+    REQUIRE(s && (!enabled || img), "bad argument");
+    if (enabled) for (int d = 0; d < 3; ++d) REQUIRE(img[d] >= 0 && img[d] <= 1000, "n_periodic_images out of range");
+    s->ddi_on = enabled ? 1 : 0;
+    for (int d = 0; d < 3; ++d) s->ddi_img[d] = enabled ? img[d] : 0;
+    s->plan_dirty = true;
+    return SPIN_OK;
+}
+
+// ---------------------------------------------------------------------------------------------- state
+static int pack_from_device_aos(spin_system *s, const double *d_aos) {
+    int *bad = (int *)(s->d_aos + (size_t)3 * s->N);
+    SPIN_CUDA(cudaMemsetAsync(bad, 0, sizeof(int), s->stream));
+    const int nt = 256;
+    pack_kernel<<<(unsigned)((s->N + nt - 1) / nt), nt, 0, s->stream>>>(d_aos, s->d_n[s->cur], (int)s->N, s->nb, (int)s->ncell, s->stride, 1, bad);
+    s->n_launch++;
+    int h_bad = 0;
+    SPIN_CUDA(cudaMemcpyAsync(&h_bad, bad, sizeof(int), cudaMemcpyDeviceToHost, s->stream));
+    SPIN_CUDA(cudaStreamSynchronize(s->stream));
+    SPIN_CUDA(cudaGetLastError());
+    if (h_bad) return spin::fail(SPIN_ERR_ARG, "spins_set: zero or non-finite spin vector");
+    return SPIN_OK;
+}
+extern "C" int spins_set(spin_system *s, const double *n) {
+    REQUIRE(s && n, "null argument");
+    SPIN_CUDA(cudaMemcpyAsync(s->d_aos, n, (size_t)3 * s->N * sizeof(double), cudaMemcpyHostToDevice, s->stream));
+    return pack_from_device_aos(s, s->d_aos);
+}
+extern "C" int spins_set_device(spin_system *s, const double *n) {
+    REQUIRE(s && n, "null argument");
+    return pack_from_device_aos(s, n);
+}
+extern "C" int spins_get_device(spin_system *s, double *n) {
+    REQUIRE(s && n, "null argument");
+    const int nt = 256;
+    unpack_kernel<<<(unsigned)((s->N + nt - 1) / nt), nt, 0, s->stream>>>(s->d_n[s->cur], n, (int)s->N, s->nb, (int)s->ncell, s->stride, nullptr);
+    s->n_launch++;
+    SPIN_CUDA(cudaGetLastError());
+    return SPIN_OK;
+}
+extern "C" int spins_get(spin_system *s, double *n) {
+    REQUIRE(s && n, "null argument");
+    int rc = spins_get_device(s, s->d_aos);
+    if (rc) return rc;
+    SPIN_CUDA(cudaMemcpyAsync(n, s->d_aos, (size_t)3 * s->N * sizeof(double), cudaMemcpyDeviceToHost, s->stream));
+    SPIN_CUDA(cudaStreamSynchronize(s->stream));
+    return SPIN_OK;
+}
+
+// ---------------------------------------------------------------------------------------------- dynamics
+extern "C" int llg_configure(spin_system *s, double dt_fs, double alpha, double T, uint64_t seed, double u, const double jdir[3], double beta) {
+    REQUIRE(s, "null system");
+    REQUIRE(dt_fs > 0.0 && isfinite(dt_fs), "dt must be positive");
+    REQUIRE(alpha >= 0.0 && isfinite(alpha), "alpha must be >= 0");
+    REQUIRE(T >= 0.0 && isfinite(T), "T must be >= 0");
+    REQUIRE(isfinite(u) && isfinite(beta), "non-finite current parameters");
+    double j[3] = {1, 0, 0};
+    if (jdir) { j[0] = jdir[0]; j[1] = jdir[1]; j[2] = jdir[2]; }
+    const double nn = sqrt(j[0] * j[0] + j[1] * j[1] + j[2] * j[2]);
+    REQUIRE(nn > 0.0 || u == 0.0, "current direction must be non-zero");
+    s->dt_ps = dt_fs * 1e-3; s->alpha = alpha; s->T = T; s->seed = seed; s->u = u; s->beta = beta;
+    for (int k = 0; k < 3; ++k) s->jdir[k] = nn > 0.0 ? j[k] / nn : (k == 0 ? 1.0 : 0.0);
+    s->plan_dirty = true;
+    return llg_set_step(s, 0);
+}
+extern "C" int llg_get_step(const spin_system *s, uint64_t *step) {
+    REQUIRE(s && step, "null argument");
+    *step = s->step;
+    return SPIN_OK;
+}
+extern "C" int llg_set_step(spin_system *s, uint64_t step) {
+    REQUIRE(s, "null system");
+    s->step = step;
+    SPIN_CUDA(cudaStreamSynchronize(s->stream));
+    const unsigned long long v = step;
+    SPIN_CUDA(cudaMemcpy(s->d_step, &v, sizeof(v), cudaMemcpyHostToDevice));
+    return SPIN_OK;
+}
+
+extern "C" int llg_iterate(spin_system *s, int64_t n_steps) {
+    REQUIRE(s && n_steps >= 0, "bad argument");
+    int rc = ensure_plan(s);
+    if (rc) return rc;
+    int64_t done = 0;
+    // Launch-bound lattices: replay a captured graph of G steps (an even number, so the ping-pong buffers return to the
+    // same roles); the kernels read the step counter from device memory, the graph's last node advances it by G.
+    const bool graph_ok = s->opt_graph && !s->profile_on && !s->ddi_on;
+    const int G = 16;
+    if (graph_ok && n_steps >= G) {
+        cudaGraphExec_t &gexec = s->graph_exec[s->cur];
+        if (!gexec) {
+            cudaGraph_t graph = nullptr;
+            SPIN_CUDA(cudaStreamBeginCapture(s->stream, cudaStreamCaptureModeThreadLocal));
+            const int64_t launches_before = s->n_launch;
+            for (int k = 0; k < G && rc == SPIN_OK; ++k) rc = enqueue_step(s, (unsigned)k);
+            advance_step_kernel<<<1, 1, 0, s->stream>>>(s->d_step, (unsigned long long)G);
+            s->n_launch = launches_before;
+            cudaError_t e = cudaStreamEndCapture(s->stream, &graph);
+            if (rc) { if (graph) cudaGraphDestroy(graph); return rc; }
+            if (e != cudaSuccess) return spin::fail(SPIN_ERR_CUDA, "graph capture failed: %s", cudaGetErrorString(e));
+            e = cudaGraphInstantiate(&gexec, graph, 0);
+            cudaGraphDestroy(graph);
+            if (e != cudaSuccess) { gexec = nullptr; return spin::fail(SPIN_ERR_CUDA, "graph instantiate failed: %s", cudaGetErrorString(e)); }
+            s->graph_steps = G;
+        }
+        while (n_steps - done >= G) {
+            SPIN_CUDA(cudaGraphLaunch(gexec, s->stream));
+            s->n_launch += 2 * G + 1;
+            done += G;
+        }
+    }
+    const int64_t rest = n_steps - done;
+    for (int64_t k = 0; k < rest; ++k) {
+        rc = enqueue_step(s, (unsigned)k);
+        if (rc) return rc;
+    }
+    if (rest > 0) {
+        advance_step_kernel<<<1, 1, 0, s->stream>>>(s->d_step, (unsigned long long)rest);
+        s->n_launch++;
+    }
+    s->step += (uint64_t)n_steps;
+    SPIN_CUDA(cudaGetLastError());
+    return SPIN_OK;
+}
+
+extern "C" int spin_synchronize(spin_system *s) {
+    REQUIRE(s, "null system");
+    SPIN_CUDA(cudaStreamSynchronize(s->stream));
+    SPIN_CUDA(cudaGetLastError());
+    return SPIN_OK;
+}
+
+// ---------------------------------------------------------------------------------------------- observables
+extern "C" int effective_field_device(spin_system *s, double *B) {
+    REQUIRE(s && B, "null argument");
+    int rc = ensure_plan(s);
+    if (rc) return rc;
+    rc = enqueue_force(s, T_ALL, s->d_np);
+    if (rc) return rc;
+    // B = F / (mu_b mu_B), boundary order
+    double *d_scale = s->d_result + 8;
+    SPIN_CUDA(cudaMemcpyAsync(d_scale, s->plan.inv_mu, s->nb * sizeof(double), cudaMemcpyHostToDevice, s->stream));
+    const int nt = 256;
+    unpack_kernel<<<(unsigned)((s->N + nt - 1) / nt), nt, 0, s->stream>>>(s->d_np, B, (int)s->N, s->nb, (int)s->ncell, s->stride, d_scale);
+    s->n_launch++;
+    SPIN_CUDA(cudaGetLastError());
+    return SPIN_OK;
+}
+extern "C" int effective_field(spin_system *s, double *B) {
+    REQUIRE(s && B, "null argument");
+    int rc = effective_field_device(s, s->d_aos);
+    if (rc) return rc;
+    SPIN_CUDA(cudaMemcpyAsync(B, s->d_aos, (size_t)3 * s->N * sizeof(double), cudaMemcpyDeviceToHost, s->stream));
+    SPIN_CUDA(cudaStreamSynchronize(s->stream));
+    SPIN_CUDA(cudaGetLastError());
+    return SPIN_OK;
+}
+extern "C" int energy(spin_system *s, double *E_total, double E_terms[6]) {
+    REQUIRE(s, "null system");
+    int rc = ensure_plan(s);
+    if (rc) return rc;
+    double r[N_RED];
+    rc = reduce_all(s, r);
+    if (rc) return rc;
+    double tot = 0.0;
+    for (int k = 0; k < 6; ++k) { if (E_terms) E_terms[k] = r[k]; tot += r[k]; }
+    if (E_total) *E_total = tot;
+    return SPIN_OK;
+}
+extern "C" int observables(spin_system *s, double M[3], double *max_torque) {
+    REQUIRE(s, "null system");
+    int rc = ensure_plan(s);
+    if (rc) return rc;
+    double r[N_RED];
+    rc = reduce_all(s, r);
+    if (rc) return rc;
+    if (M) for (int k = 0; k < 3; ++k) M[k] = r[6 + k] / (double)s->N;
+    if (max_torque) *max_torque = r[9];
+    return SPIN_OK;
+}
+
+// ---------------------------------------------------------------------------------------------- introspection
+extern "C" int spin_launch_counts(const spin_system *s, int64_t *own, int64_t *fft) {
+    REQUIRE(s, "null system");
+    if (own) *own = s->n_launch;
+    if (fft) *fft = s->n_fft;
+    return SPIN_OK;
+}
+extern "C" int spin_profile_enable(spin_system *s, int on) {
+    REQUIRE(s, "null system");
+    s->profile_on = on ? 1 : 0;
+    for (int k = 0; k < 3; ++k) { s->prof_ms[k] = 0; s->prof_n[k] = 0; }
+    return SPIN_OK;
+}
+extern "C" int spin_profile_get(spin_system *s, int kind, double *ms, int64_t *n) {
+    REQUIRE(s && kind >= 0 && kind < 3, "bad argument");
+    if (ms) *ms = s->prof_ms[kind];
+    if (n) *n = s->prof_n[kind];
+    return SPIN_OK;
+}
+extern "C" int spin_set_option(spin_system *s, const char *name, int value) {
+    REQUIRE(s && name, "null argument");
+    if (!strcmp(name, "use_graph")) s->opt_graph = value ? 1 : 0;
+    else if (!strcmp(name, "store_A")) s->opt_store_A = value ? 1 : 0;
+    else return spin::fail(SPIN_ERR_ARG, "unknown option '%s'", name);
+    drop_graphs(s);
+    return SPIN_OK;
+}

@@ -1,0 +1,144 @@
+// spinllg_internal.h -- private definitions of the B200 LLG library (not part of the C-ABI).
+//
+// Layout in HBM: spins are kept structure-of-arrays and sublattice-major,
+//     n[comp * stride + b * Ncell + (ia + Na*(ib + Nb*ic))],   comp in {x,y,z}
+// so that a warp reads 32 consecutive doubles of one component of one sublattice (256 B, two full lines).
+// The boundary order (AoS, basis fastest; include/spinllg.h) is converted by pack/unpack kernels.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <cufft.h>
+#include <stdint.h>
+
+#include <string>
+#include <vector>
+
+#include "../../include/spinllg.h"
+
+#define SPIN_MAX_BASIS 8
+#define SPIN_MAX_PAIR_ENTRIES 160
+#define SPIN_MAX_QUAD_ENTRIES 32
+
+namespace spin {
+
+// CODATA 2018 (reading R5)
+constexpr double MU_B = 0.057883818060;    // meV / T
+constexpr double K_B = 0.08617333262;      // meV / K
+constexpr double GAMMA = 0.176085963023;   // rad / (ps T)
+constexpr double C_DD = 0.0536815112;      // meV, mu0 mu_B^2 / (4 pi Angstrom^3)
+
+enum TermMask { T_ZEE = 1, T_ANI = 2, T_EXC = 4, T_DMI = 8, T_QUAD = 16, T_DDI = 32, T_ALL = 63 };
+
+// One gather entry of a basis atom's pair table: the spin at cell c collects J n_j + n_j x D from the partner
+// on sublattice bj at cell c + (da,db,dc).  Backward entries carry -D and -t ("unique pairs").
+struct PairEntry {
+    int da, db, dc;      // partner cell translation, reduced to (-N_d, N_d) in periodic directions
+    int bj;              // partner sublattice
+    int lin;             // linear index offset valid when no coordinate wraps (interior bricks)
+    int pad_;
+    double J, Dx, Dy, Dz;
+};
+
+// One role of one quadruplet (Eq. 2): F += K (n_Q . n_R) n_P, the three other members given relative to this spin.
+struct QuadEntry {
+    int d[3][3];         // translations of P, Q, R relative to this spin
+    int b[3];            // their sublattices
+    int lin[3];
+    int pad_;
+    double K;
+};
+
+struct DevicePlan {
+    int Na, Nb, Nc;
+    int perA, perB, perC;
+    int nb;
+    int Ncell;
+    int stride;                              // component stride of the SoA arrays (doubles)
+    int reach[3];                            // max |translation| per direction over all entries (interior test)
+    int pair_begin[SPIN_MAX_BASIS + 1];
+    int quad_begin[SPIN_MAX_BASIS + 1];
+    double zee[SPIN_MAX_BASIS][3];           // mu_b mu_B B            (meV)
+    double K2[SPIN_MAX_BASIS];               // 2 K_b                  (meV)
+    double Kax[SPIN_MAX_BASIS][3];           // unit anisotropy axis
+    double pre[SPIN_MAX_BASIS];              // -gamma / ((1+alpha^2) mu_b mu_B)   (rad / (ps meV))
+    double sigma[SPIN_MAX_BASIS];            // thermal amplitude sqrt(2 alpha kB T mu / (gamma dt)) (meV)
+    double inv_mu[SPIN_MAX_BASIS];           // 1 / (mu_b mu_B)        (T / meV)
+    double alpha, dt, dt2;
+    int stt_on;
+    int has_ddi;
+    double stt_c[3];                         // j^ = sum_d stt_c[d] a_d   (1/Angstrom)
+    double stt_s, stt_x;                     // -u (alpha-beta)/(1+alpha^2),  u (1+alpha beta)/(1+alpha^2)
+    uint32_t seed_lo, seed_hi;
+    int thermal_on;
+    int pad_;
+    PairEntry pairs[SPIN_MAX_PAIR_ENTRIES];
+    QuadEntry quads[SPIN_MAX_QUAD_ENTRIES];
+};
+
+struct HostPair { int bi, bj, t[3]; double J, D[3]; };
+struct HostQuad { int b[4]; int t[9]; double K; };
+
+}  // namespace spin
+
+struct DdiState;   // spin_ddi.cu
+
+struct spin_system {
+    // ---- geometry
+    double brav[9];
+    int nb;
+    std::vector<double> basis;     // 3*nb fractional
+    int nc[3], per[3];
+    double alat;
+    int64_t ncell, N;
+    int stride;
+    // ---- Hamiltonian (host description)
+    std::vector<double> mu;        // nb
+    double Bmag, Bdir[3];
+    std::vector<double> K, Kax;    // nb, 3*nb
+    std::vector<spin::HostPair> pairs_explicit, pairs_exch_shells, pairs_dmi_shells;
+    std::vector<spin::HostQuad> quads;
+    int ddi_on, ddi_img[3];
+    // ---- LLG
+    double dt_ps, alpha, T, u, jdir[3], beta;
+    uint64_t seed, step;
+    // ---- device
+    cudaStream_t stream, own_stream;
+    double *d_n[2];                // ping-pong spin buffers (3*stride each)
+    int cur;
+    double *d_np;                  // predictor
+    double *d_A;                   // rotation field of the predictor stage (store_A option)
+    double *d_fddi[2];             // dipolar force of n and of n^p (3*stride each), only with DDI
+    double *d_aos;                 // staging buffer, boundary order (3N)
+    double *d_partials;            // reduction scratch
+    double *d_result;              // reduction result (16 doubles)
+    unsigned long long *d_step;    // device copy of the step counter (read by the kernels)
+    spin::DevicePlan plan;
+    bool plan_dirty;
+    DdiState *ddi;
+    // ---- execution options / bookkeeping
+    int opt_graph, opt_store_A;
+    cudaGraphExec_t graph_exec[2];   // one captured graph per ping-pong parity
+    int graph_steps;
+    int64_t n_launch, n_fft;
+    int profile_on;
+    double prof_ms[3];
+    int64_t prof_n[3];
+    cudaEvent_t ev0, ev1;
+};
+
+namespace spin {
+// shared error plumbing (spin_api.cu)
+int fail(int code, const char *fmt, ...);
+#define SPIN_CUDA(call)                                                                             \
+    do {                                                                                            \
+        cudaError_t e__ = (call);                                                                   \
+        if (e__ != cudaSuccess)                                                                     \
+            return spin::fail(SPIN_ERR_CUDA, "%s failed: %s (%s:%d)", #call, cudaGetErrorString(e__), \
+                              __FILE__, __LINE__);                                                  \
+    } while (0)
+
+// spin_ddi.cu
+int ddi_prepare(spin_system *s);                                   // (re)build tensor spectra and FFT plans
+int ddi_field(spin_system *s, const double *d_n, double *d_f);     // d_f (SoA, meV) = dipolar force of d_n
+void ddi_release(spin_system *s);
+}  // namespace spin

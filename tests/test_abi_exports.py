@@ -1,0 +1,58 @@
+"""CPU-only checks of the boundary: the C-ABI library builds, loads, and exports every symbol include/spinllg.h declares.
+No compute call is made here (there is no GPU in the build container)."""
+import ctypes
+import os
+import re
+
+import numpy as np
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def declared_functions():
+    text = open(os.path.join(ROOT, "include", "spinllg.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    names = re.findall(r"\b([a-z_0-9]+)\s*\(", text)
+    return sorted({n for n in names if n not in ("defined",)})
+
+
+def test_library_builds_and_exports_every_declared_symbol():
+    import paper_1901_11350_b200 as P
+    L = P.lib()
+    decl = declared_functions()
+    assert len(decl) >= 25
+    for name in decl:
+        assert hasattr(L, name), f"{name} declared in include/spinllg.h but not exported"
+    assert sorted(P.EXPORTS) == decl
+    assert "sm_100a" in P.version()
+
+
+def test_library_is_built_for_sm_100a():
+    import subprocess
+    import paper_1901_11350_b200.build as B
+    out = subprocess.run(["cuobjdump", "-lelf", B.build()], capture_output=True, text=True).stdout
+    assert "sm_100a" in out
+
+
+def test_no_cpu_fallback_without_device():
+    """Without a CUDA device the product must fail loudly, not compute on the CPU."""
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a GPU is present")
+    import paper_1901_11350_b200 as P
+    with pytest.raises(P.SpinError) as e:
+        P.SpinSystem(np.eye(3), [[0, 0, 0]], (4, 4, 1), (1, 1, 0))
+    assert e.value.code == -4 and "no CPU fallback" in str(e.value)
+
+
+def test_product_does_not_import_oracle():
+    pkg = os.path.join(ROOT, "paper_1901_11350_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                src = open(os.path.join(dirpath, f)).read()
+                assert not re.search(r"^\s*(from|import)\s+oracle\b", src, flags=re.M), f
+                assert "spin_oracle" not in src and "liboracle" not in src, f
+    osrc = open(os.path.join(ROOT, "oracle", "spin_oracle.c")).read() + open(os.path.join(ROOT, "oracle", "__init__.py")).read()
+    assert "paper_1901_11350_b200" not in osrc.replace("paper_1901_11350_b200/; only", "").replace("(paper_1901_11350_b200) never", "")

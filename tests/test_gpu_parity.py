@@ -1,0 +1,236 @@
+"""Parity of the CUDA path (through the C-ABI) against the CPU oracle, element by element on the same seeded inputs.
+
+Tolerances (BASELINE.json north_star; read as in DESIGN.md "Tolerances"):
+    fields    max|dB|  <= 1e-12 * max_i|B_i|
+    energies  |dE|     <= 1e-12 * sum_terms |E_term|
+    spins     max|dn|  <= 1e-9 after the configuration's steps, identical Philox noise
+"""
+import dataclasses
+
+import numpy as np
+import pytest
+
+import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+FIELD_RTOL = 1e-12
+ENERGY_RTOL = 1e-12
+SPIN_ATOL = 1e-9
+
+
+@pytest.fixture(scope="module")
+def P():
+    import paper_1901_11350_b200 as P
+    return P
+
+
+@pytest.fixture(scope="module")
+def O():
+    import oracle
+    return oracle
+
+
+def pair(P, O, w, **kw):
+    return P.SpinSystem.from_workload(w, **kw), O.OracleSystem.from_workload(w)
+
+
+def assert_fields_close(Bg, Bo):
+    scale = np.abs(Bo).max()
+    assert np.abs(Bg - Bo).max() <= FIELD_RTOL * scale, (np.abs(Bg - Bo).max(), scale)
+
+
+# replicas: ragged sizes (not multiples of the 32x8x1 / 32x4x2 bricks), several bricks per direction
+REPLICAS = {
+    1: (37, 19, 1),
+    2: (45, 33, 1),
+    3: (35, 9, 7),
+    4: (33, 17, 1),
+    5: (20, 12, 5),
+}
+
+
+@pytest.mark.parametrize("cfg", [1, 2, 3, 4, 5])
+def test_effective_field_and_energy_parity(P, O, cfg):
+    w = W.CONFIGS[cfg]().resized(REPLICAS[cfg])
+    g, o = pair(P, O, w)
+    assert_fields_close(g.effective_field(), o.effective_field())
+    Eg, Tg = g.energy()
+    To = o.energy_terms()
+    assert np.abs(Tg - To).max() <= ENERGY_RTOL * np.abs(To).sum(), (Tg, To)
+    assert abs(Eg - To.sum()) <= ENERGY_RTOL * np.abs(To).sum()
+    Mg, tg = g.observables()
+    Mo, to = o.observables()
+    assert np.abs(Mg - Mo).max() < 1e-14
+    assert abs(tg - to) <= 1e-12 * to
+
+
+@pytest.mark.parametrize("periodic", [(0, 0, 0), (1, 0, 1), (0, 1, 0)])
+@pytest.mark.parametrize("cfg", [2, 3, 4])
+def test_field_parity_open_and_mixed_boundaries(P, O, cfg, periodic):
+    w = W.CONFIGS[cfg]().resized(REPLICAS[cfg])
+    if w.n_cells[2] == 1:
+        periodic = (periodic[0], periodic[1], 0)
+    w = dataclasses.replace(w, periodic=periodic)
+    g, o = pair(P, O, w)
+    assert_fields_close(g.effective_field(), o.effective_field())
+    assert np.abs(g.energy()[1] - o.energy_terms()).max() <= ENERGY_RTOL * np.abs(o.energy_terms()).sum()
+
+
+@pytest.mark.parametrize("cells,periodic", [((1, 1, 1), (0, 0, 0)), ((1, 1, 1), (1, 1, 1)), ((2, 2, 2), (1, 1, 1)), ((40, 1, 1), (1, 0, 0)),
+                                            ((1, 1, 9), (0, 0, 1)), ((3, 2, 1), (1, 1, 0))])
+def test_degenerate_lattices(P, O, cells, periodic):
+    """Single cell, periodic self-wrap (N_d = 1, 2), chains along a and along c."""
+    w = dataclasses.replace(W.CONFIGS[3](), n_cells=cells, periodic=periodic)
+    g, o = pair(P, O, w)
+    assert_fields_close(g.effective_field(), o.effective_field())
+    g.llg_iterate(20); o.iterate(20)
+    assert np.abs(g.spins_get() - o.spins()).max() < 1e-13
+
+
+@pytest.mark.parametrize("cfg,steps", [(1, 1000), (2, 400), (3, 300), (4, 300), (5, 60)])
+def test_trajectory_parity_replicas(P, O, cfg, steps):
+    """Depondt trajectories on small replicas: 1e-9 max-abs after `steps` steps, thermal configs with identical noise."""
+    w = W.CONFIGS[cfg]().resized(REPLICAS[cfg], steps)
+    g, o = pair(P, O, w)
+    g.llg_iterate(steps); o.iterate(steps)
+    ng, no = g.spins_get(), o.spins()
+    assert np.abs(np.linalg.norm(ng, axis=1) - 1).max() < 4e-16
+    d = np.abs(ng - no).max()
+    print(f"cfg{cfg} replica {w.n_cells} steps={steps}: max|dn| = {d:.3e}")
+    assert d <= SPIN_ATOL
+    assert g.llg_get_step() == steps
+
+
+def test_cfg1_full_config(P, O):
+    """Config 1 exactly as BASELINE.json states it: 32x32, 1000 steps."""
+    w = W.config1()
+    g, o = pair(P, O, w)
+    g.llg_iterate(w.steps); o.iterate(w.steps)
+    d = np.abs(g.spins_get() - o.spins()).max()
+    print(f"cfg1 full: max|dn| = {d:.3e}")
+    assert d <= SPIN_ATOL
+    assert_fields_close(g.effective_field(), o.effective_field())
+
+
+def test_thermal_noise_is_identical_single_step(P, O):
+    """No Hamiltonian: one step is driven by the thermal field alone, so the update exposes xi_i directly.
+    Agreement at 1e-13 for every spin means the Philox counters, key, uniform mapping and Box-Muller match."""
+    w = dataclasses.replace(W.config2().resized((21, 13, 1)), B=0.0, aniso=[], pair_J=W.config2().pair_J * 0, pair_D=W.config2().pair_D * 0,
+                            T=300.0, seed=(0xDEADBEEF << 32) | 0x12345678)
+    g, o = pair(P, O, w)
+    g.llg_set_step((5 << 32) + 17); o.step = (5 << 32) + 17
+    g.llg_iterate(1); o.iterate(1)
+    moved = np.abs(o.spins() - w.initial_spins()).max()
+    assert moved > 1e-3
+    assert np.abs(g.spins_get() - o.spins()).max() < 1e-13
+
+
+def test_split_invariance_and_graph_equivalence(P, O):
+    """llg_iterate(a); llg_iterate(b) == llg_iterate(a+b) bit for bit; CUDA-graph replay == plain launches."""
+    w = W.config2().resized((40, 24, 1))
+    a = P.SpinSystem.from_workload(w)
+    b = P.SpinSystem.from_workload(w)
+    c = P.SpinSystem.from_workload(w)
+    c.spin_set_option("use_graph", 0)
+    a.llg_iterate(57)
+    b.llg_iterate(20); b.llg_iterate(17); b.llg_iterate(20)
+    c.llg_iterate(57)
+    na = a.spins_get()
+    assert np.array_equal(na, b.spins_get())
+    assert np.array_equal(na, c.spins_get())
+    assert a.llg_get_step() == b.llg_get_step() == c.llg_get_step() == 57
+
+
+@pytest.mark.parametrize("cfg", [2, 4])
+def test_store_A_option_matches_recompute(P, O, cfg):
+    w = W.CONFIGS[cfg]().resized(REPLICAS[cfg], 50)
+    a = P.SpinSystem.from_workload(w)
+    b = P.SpinSystem.from_workload(w)
+    b.spin_set_option("store_A", 1)
+    a.llg_iterate(50); b.llg_iterate(50)
+    assert np.abs(a.spins_get() - b.spins_get()).max() < 1e-13
+
+
+def test_shell_helpers_match_explicit_pairs(P, O):
+    """Host neighbour finder: exchange / DMI by shell == the explicit pair lists of the workloads."""
+    for cfg, J, D, chir in [(1, [1.0], [0.3], 2), (2, [1.0, -0.3, -0.1], [0.2], 2), (3, [1.0], [0.2], 1)]:
+        w = W.CONFIGS[cfg]().resized(REPLICAS[cfg])
+        a = P.SpinSystem.from_workload(w)
+        b = P.SpinSystem.from_workload(w, use_shell_helpers=True)
+        b.hamiltonian_set_exchange_shells(J)
+        b.hamiltonian_set_dmi_shells(D, chir)
+        Ba, Bb = a.effective_field(), b.effective_field()
+        assert np.abs(Ba - Bb).max() <= 1e-13 * np.abs(Ba).max(), cfg
+    # honeycomb: shell 0 = 3 inter-sublattice bonds, shell 1 = 6 intra-sublattice bonds per atom
+    w = W.config4().resized(REPLICAS[4])
+    a = P.SpinSystem.from_workload(w)
+    b = P.SpinSystem.from_workload(w, use_shell_helpers=True)
+    b.hamiltonian_set_exchange_shells([-2.0, 0.5])
+    b.hamiltonian_set_dmi_shells([0.1], 2)
+    assert np.abs(a.effective_field() - b.effective_field()).max() <= 1e-13 * np.abs(a.effective_field()).max()
+
+
+def test_ddi_parity_multibasis_and_monolayer(P, O):
+    """Dipolar force: asymmetric 2-atom basis, mixed boundaries, images; and the 1x1x1 periodic monolayer
+    whose lattice sum tends to 9.0336217 (the oracle pins that limit)."""
+    brav = np.array([[1, 0, 0], [0.5, 0.8, 0], [0.1, 0.2, 1.1]])
+    for basis, cells, per, img in [([[0, 0, 0], [0.31, 0.17, 0.23]], (6, 5, 3), (1, 0, 1), (1, 0, 2)),
+                                   ([[0, 0, 0]], (7, 6, 1), (1, 1, 0), (3, 3, 0)),
+                                   ([[0, 0, 0]], (1, 1, 1), (1, 1, 0), (50, 50, 0))]:
+        g = P.SpinSystem(brav, basis, cells, per, 1.3)
+        o = O.OracleSystem(brav, basis, cells, per, 1.3)
+        mu = np.linspace(1.0, 2.5, len(basis))
+        g.hamiltonian_set_mu_s(mu); o.set_mu_s(mu)
+        g.hamiltonian_set_ddi(True, img); o.set_ddi(True, img)
+        n = np.random.default_rng(3).standard_normal((g.N, 3))
+        n /= np.linalg.norm(n, axis=1, keepdims=True)
+        g.spins_set(n); o.set_spins(n)
+        assert_fields_close(g.effective_field(), o.effective_field())
+        Eg = g.energy()[1][5]
+        Eo = o.energy_terms()[5]
+        assert abs(Eg - Eo) <= 1e-12 * abs(Eo)
+        # and against the O(N^2) direct sum
+        Fd = o.ddi_field(n, direct=True) / (mu[np.arange(g.N) % len(basis)] * O.MU_B)[:, None]
+        assert np.abs(g.effective_field() - Fd).max() <= 1e-11 * np.abs(Fd).max()
+
+
+def test_error_codes(P):
+    s = P.SpinSystem(np.eye(3), [[0, 0, 0]], (4, 4, 1), (1, 1, 0))
+    with pytest.raises(P.SpinError) as e:
+        s.hamiltonian_set_pairs([0], [0], [[0, 0, 0]], [1.0])
+    assert e.value.code == -1
+    with pytest.raises(P.SpinError):
+        s.hamiltonian_set_pairs([0, 0], [0, 0], [[1, 0, 0], [-1, 0, 0]], [1.0, 1.0])     # same bond twice
+    with pytest.raises(P.SpinError):
+        s.hamiltonian_set_pairs([1], [0], [[1, 0, 0]], [1.0])
+    with pytest.raises(P.SpinError):
+        s.hamiltonian_set_mu_s([-1.0])
+    with pytest.raises(P.SpinError):
+        s.llg_configure(-1.0, 0.1)
+    with pytest.raises(P.SpinError):
+        s.spins_set(np.zeros((16, 3)))
+    with pytest.raises(P.SpinError):
+        P.SpinSystem(np.eye(3), [[0, 0, 0]], (0, 4, 1), (1, 1, 0))
+    with pytest.raises(P.SpinError):
+        P.SpinSystem(np.array([[1, 0, 0], [2, 0, 0], [0, 0, 1.0]]), [[0, 0, 0]], (4, 4, 1), (1, 1, 0))
+
+
+def test_device_pointer_io_with_torch_stream(P, O):
+    import torch
+    w = W.config1().resized((37, 19, 1))
+    st = torch.cuda.Stream()
+    g = P.SpinSystem.from_workload(w, stream=st.cuda_stream)
+    o = O.OracleSystem.from_workload(w)
+    n0 = torch.from_numpy(w.initial_spins()).cuda()
+    with torch.cuda.stream(st):
+        g.spins_set_device(n0.data_ptr())
+        g.llg_iterate(40)
+        out = torch.empty_like(n0)
+        g.spins_get_device(out.data_ptr())
+        B = torch.empty_like(n0)
+        g.effective_field_device(B.data_ptr())
+    st.synchronize()
+    o.iterate(40)
+    assert np.abs(out.cpu().numpy() - o.spins()).max() < 1e-12
+    assert_fields_close(B.cpu().numpy(), o.effective_field())
