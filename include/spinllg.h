@@ -133,6 +133,15 @@ int spin_profile_get(spin_system *sys, int kind, double *total_ms, int64_t *laun
 /* execution options: use_graph (capture steps into a CUDA graph; default 1), store_A (1: predictor stores the
  * rotation field A, 0: corrector recomputes it; default 0)                                                  */
 int spin_set_option(spin_system *sys, const char *name, int value);
+/* further option: use_jit (1: the two sweeps are specialised per system at run time with NVRTC -- lattice extents, gather
+ * tables and prefactors become compile-time constants; 0: table-driven kernels; default 1).
+ * spin_kernel_info writes "jit" or "generic: <why>" into buf: which sweep kernels the system is using.                 */
+int spin_kernel_info(spin_system *sys, char *buf, int len);
+/* the generated translation unit of the specialised sweeps (buf may be NULL); compile != 0 also compiles it for sm_100a
+ * (needs no device) and returns the cubin size.  Host-side planner check; works in planner-only mode
+ * (environment SPINLLG_PLANNER_ONLY=1 lets spin_geometry_create succeed without a device; every computing call then
+ * still fails with SPIN_ERR_CUDA).                                                                                    */
+int spin_jit_source(spin_system *sys, char *buf, int len, int compile, int64_t *cubin_bytes);
 
 const char *spin_last_error(void);
 const char *spin_version(void);

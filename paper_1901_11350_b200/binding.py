@@ -23,7 +23,7 @@ EXPORTS = [
     "llg_configure", "llg_iterate", "llg_get_step", "llg_set_step", "spin_synchronize",
     "effective_field", "effective_field_device", "energy", "observables",
     "spin_launch_counts", "spin_profile_enable", "spin_profile_get", "spin_set_option",
-    "spin_last_error", "spin_version",
+    "spin_kernel_info", "spin_jit_source", "spin_last_error", "spin_version",
 ]
 
 
@@ -74,6 +74,8 @@ def lib() -> C.CDLL:
         "spin_profile_enable": (C.c_int, [vp, C.c_int]),
         "spin_profile_get": (C.c_int, [vp, C.c_int, dp, i64p]),
         "spin_set_option": (C.c_int, [vp, C.c_char_p, C.c_int]),
+        "spin_kernel_info": (C.c_int, [vp, C.c_char_p, C.c_int]),
+        "spin_jit_source": (C.c_int, [vp, C.c_char_p, C.c_int, C.c_int, i64p]),
         "spin_last_error": (C.c_char_p, []),
         "spin_version": (C.c_char_p, []),
     }
@@ -128,7 +130,7 @@ class SpinSystem:
             pass
 
     @classmethod
-    def from_workload(cls, w, use_shell_helpers=False, stream=None):
+    def from_workload(cls, w, use_shell_helpers=False, stream=None, set_spins=True):
         s = cls(w.bravais, w.basis, w.n_cells, w.periodic, w.lattice_constant)
         if stream is not None:
             s.spin_set_stream(stream)
@@ -142,7 +144,8 @@ class SpinSystem:
             s.hamiltonian_set_quadruplets(w.quad_b, w.quad_t, w.quad_K)
         s.hamiltonian_set_ddi(w.ddi, w.ddi_images)
         s.llg_configure(w.dt_fs, w.alpha, w.T, w.seed, w.u, w.j_dir, w.beta)
-        s.spins_set(w.initial_spins())
+        if set_spins:
+            s.spins_set(w.initial_spins())
         return s
 
     # ---- C-ABI calls -----------------------------------------------------------------------------------
@@ -262,6 +265,17 @@ class SpinSystem:
 
     def spin_set_option(self, name, value):
         _check(lib().spin_set_option(self._h, name.encode(), int(value)))
+
+    def spin_kernel_info(self):
+        buf = C.create_string_buffer(1024)
+        _check(lib().spin_kernel_info(self._h, buf, 1024))
+        return buf.value.decode()
+
+    def spin_jit_source(self, compile=False):
+        buf = C.create_string_buffer(1 << 18)
+        nbytes = C.c_int64(0)
+        _check(lib().spin_jit_source(self._h, buf, 1 << 18, int(bool(compile)), C.byref(nbytes)))
+        return buf.value.decode(), int(nbytes.value)
 
 
 def version() -> str:

@@ -11,8 +11,8 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libspinllg.so")
-SOURCES = ["spin_api.cu", "spin_ddi.cu"]
-HEADERS = ["spinllg_internal.h", "spin_kernels.cuh", os.path.join("..", "..", "include", "spinllg.h")]
+SOURCES = ["spin_api.cu", "spin_ddi.cu", "spin_jit.cu"]
+HEADERS = ["spinllg_internal.h", "spin_kernels.cuh", "spin_device_math.cuh", "spin_jit_kernels.cuh", os.path.join("..", "..", "include", "spinllg.h")]
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
 
 
@@ -37,7 +37,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     cuda_lib = os.path.join(os.path.dirname(os.path.dirname(nvcc_path())), "lib64")
     cmd = [nvcc_path(), "-std=c++17", "-O3", "-lineinfo", *ARCH, "-Xcompiler", "-fPIC", "-shared",
            "-o", LIB, *[os.path.join(CSRC, f) for f in SOURCES],
-           "-lcufft", "-Xlinker", "-rpath", "-Xlinker", cuda_lib]
+           "-lcufft", "-lnvrtc", "-ldl", "-Xlinker", "-rpath", "-Xlinker", cuda_lib]
     if verbose:
         cmd.insert(1, "-Xptxas")
         cmd.insert(2, "-v")

@@ -269,7 +269,13 @@ int build_plan(spin_system *s) {
     return SPIN_OK;
 }
 
+#define NEED_DEVICE(s)                                                                                          \
+    do {                                                                                                        \
+        if (!(s)->has_device) return spin::fail(SPIN_ERR_CUDA, "no CUDA device: this library has no CPU fallback"); \
+    } while (0)
+
 int ensure_plan(spin_system *s) {
+    NEED_DEVICE(s);
     if (!s->plan_dirty) return SPIN_OK;
     int rc = build_plan(s);
     if (rc) return rc;
@@ -283,6 +289,15 @@ int ensure_plan(spin_system *s) {
         if (rc) return rc;
     } else {
         ddi_release(s);
+    }
+    // run-time specialised sweeps; on failure the table-driven kernels stay in use and the reason is kept
+    s->jit_note.clear();
+    if (s->opt_jit) {
+        rc = jit_prepare(s);
+        if (rc) { s->jit_note = spin_last_error(); jit_release(s); }
+    } else {
+        jit_release(s);
+        s->jit_note = "disabled by option use_jit=0";
     }
     s->plan_dirty = false;
     return SPIN_OK;
@@ -299,8 +314,10 @@ int enqueue_step_t(spin_system *s, const Launch &L, unsigned step_add) {
         if (rc) return rc;
         if (prof) { cudaEventRecord(s->ev1, s->stream); cudaEventSynchronize(s->ev1); float ms; cudaEventElapsedTime(&ms, s->ev0, s->ev1); s->prof_ms[2] += ms; s->prof_n[2]++; }
     }
+    const bool jit = jit_ready(s);
     if (prof) cudaEventRecord(s->ev0, s->stream);
-    if (s->opt_store_A)
+    if (jit) { int rc = jit_launch_predictor(s, L.grid, L.block, n, s->d_fddi[0], s->d_np, s->d_A, step_add); if (rc) return rc; }
+    else if (s->opt_store_A)
         predictor_kernel<BX, BY, BZ, true><<<L.grid, L.block, 0, s->stream>>>(s->plan, n, s->d_fddi[0], s->d_np, s->d_A, s->d_step, step_add);
     else
         predictor_kernel<BX, BY, BZ, false><<<L.grid, L.block, 0, s->stream>>>(s->plan, n, s->d_fddi[0], s->d_np, nullptr, s->d_step, step_add);
@@ -313,7 +330,8 @@ int enqueue_step_t(spin_system *s, const Launch &L, unsigned step_add) {
         if (prof) { cudaEventRecord(s->ev1, s->stream); cudaEventSynchronize(s->ev1); float ms; cudaEventElapsedTime(&ms, s->ev0, s->ev1); s->prof_ms[2] += ms; s->prof_n[2]++; }
     }
     if (prof) cudaEventRecord(s->ev0, s->stream);
-    if (s->opt_store_A)
+    if (jit) { int rc = jit_launch_corrector(s, L.grid, L.block, n, s->d_np, s->d_fddi[0], s->d_fddi[1], s->d_A, nout, step_add); if (rc) return rc; }
+    else if (s->opt_store_A)
         corrector_kernel<BX, BY, BZ, true><<<L.grid, L.block, 0, s->stream>>>(s->plan, n, s->d_np, s->d_fddi[0], s->d_fddi[1], s->d_A, nout, s->d_step, step_add);
     else
         corrector_kernel<BX, BY, BZ, false><<<L.grid, L.block, 0, s->stream>>>(s->plan, n, s->d_np, s->d_fddi[0], s->d_fddi[1], nullptr, nout, s->d_step, step_add);
@@ -368,9 +386,15 @@ extern "C" int spin_geometry_create(const double bravais[9], int n_basis, const 
     const double vol = a[0] * (b[1] * c[2] - b[2] * c[1]) - a[1] * (b[0] * c[2] - b[2] * c[0]) + a[2] * (b[0] * c[1] - b[1] * c[0]);
     REQUIRE(fabs(vol) > 1e-12, "bravais vectors are linearly dependent");
     int ndev = 0;
-    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1)
+    bool has_device = cudaGetDeviceCount(&ndev) == cudaSuccess && ndev >= 1;
+    // planner-only mode for the CPU test-suite (gather tables, generated kernel source); nothing can be computed in it
+    const char *plan_only = getenv("SPINLLG_PLANNER_ONLY");
+    if (!has_device && !(plan_only && plan_only[0] == '1'))
         return spin::fail(SPIN_ERR_CUDA, "no CUDA device: this library has no CPU fallback");
+    if (!has_device) cudaGetLastError();
     spin_system *s = new spin_system();
+    s->has_device = has_device;
+    s->jit = nullptr; s->opt_jit = 1;
     memcpy(s->brav, bravais, sizeof(s->brav));
     s->nb = n_basis;
     s->basis.assign(basis_frac, basis_frac + 3 * n_basis);
@@ -395,6 +419,7 @@ extern "C" int spin_geometry_create(const double bravais[9], int n_basis, const 
     s->ev0 = s->ev1 = nullptr;
     const size_t bytes = (size_t)3 * s->stride * sizeof(double);
     const Launch L = brick_launch(s);
+    if (!has_device) { *out = s; return SPIN_OK; }
     cudaError_t e = cudaStreamCreateWithFlags(&s->own_stream, cudaStreamNonBlocking);
     s->stream = s->own_stream;
     if (e == cudaSuccess) e = cudaMalloc(&s->d_n[0], bytes);
@@ -432,6 +457,7 @@ extern "C" void spin_system_destroy(spin_system *s) {
     drop_graphs(s);
     if (s->own_stream) cudaStreamDestroy(s->own_stream);
     ddi_release(s);
+    jit_release(s);
     cudaFree(s->d_n[0]); cudaFree(s->d_n[1]); cudaFree(s->d_np); cudaFree(s->d_A); cudaFree(s->d_fddi[0]); cudaFree(s->d_fddi[1]);
     cudaFree(s->d_aos); cudaFree(s->d_partials); cudaFree(s->d_result); cudaFree(s->d_step);
     if (s->ev0) cudaEventDestroy(s->ev0);
@@ -443,6 +469,7 @@ extern "C" int64_t spin_system_nspins(const spin_system *s) { return s ? s->N : 
 
 extern "C" int spin_set_stream(spin_system *s, void *stream) {
     REQUIRE(s, "null system");
+    NEED_DEVICE(s);
     SPIN_CUDA(cudaStreamSynchronize(s->stream));
     s->stream = stream ? (cudaStream_t)stream : s->own_stream;
     drop_graphs(s);
@@ -572,6 +599,7 @@ extern "C" int hamiltonian_set_ddi(spin_system *s, int enabled, const int img[3]
 
 // ---------------------------------------------------------------------------------------------- state
 static int pack_from_device_aos(spin_system *s, const double *d_aos) {
+    NEED_DEVICE(s);
     int *bad = (int *)(s->d_aos + (size_t)3 * s->N);
     SPIN_CUDA(cudaMemsetAsync(bad, 0, sizeof(int), s->stream));
     const int nt = 256;
@@ -586,6 +614,7 @@ static int pack_from_device_aos(spin_system *s, const double *d_aos) {
 }
 extern "C" int spins_set(spin_system *s, const double *n) {
     REQUIRE(s && n, "null argument");
+    NEED_DEVICE(s);
     SPIN_CUDA(cudaMemcpyAsync(s->d_aos, n, (size_t)3 * s->N * sizeof(double), cudaMemcpyHostToDevice, s->stream));
     return pack_from_device_aos(s, s->d_aos);
 }
@@ -595,6 +624,7 @@ extern "C" int spins_set_device(spin_system *s, const double *n) {
 }
 extern "C" int spins_get_device(spin_system *s, double *n) {
     REQUIRE(s && n, "null argument");
+    NEED_DEVICE(s);
     const int nt = 256;
     unpack_kernel<<<(unsigned)((s->N + nt - 1) / nt), nt, 0, s->stream>>>(s->d_n[s->cur], n, (int)s->N, s->nb, (int)s->ncell, s->stride, nullptr);
     s->n_launch++;
@@ -634,6 +664,7 @@ extern "C" int llg_get_step(const spin_system *s, uint64_t *step) {
 extern "C" int llg_set_step(spin_system *s, uint64_t step) {
     REQUIRE(s, "null system");
     s->step = step;
+    if (!s->has_device) return SPIN_OK;
     SPIN_CUDA(cudaStreamSynchronize(s->stream));
     const unsigned long long v = step;
     SPIN_CUDA(cudaMemcpy(s->d_step, &v, sizeof(v), cudaMemcpyHostToDevice));
@@ -688,6 +719,7 @@ extern "C" int llg_iterate(spin_system *s, int64_t n_steps) {
 
 extern "C" int spin_synchronize(spin_system *s) {
     REQUIRE(s, "null system");
+    NEED_DEVICE(s);
     SPIN_CUDA(cudaStreamSynchronize(s->stream));
     SPIN_CUDA(cudaGetLastError());
     return SPIN_OK;
@@ -764,8 +796,34 @@ extern "C" int spin_profile_get(spin_system *s, int kind, double *ms, int64_t *n
 extern "C" int spin_set_option(spin_system *s, const char *name, int value) {
     REQUIRE(s && name, "null argument");
     if (!strcmp(name, "use_graph")) s->opt_graph = value ? 1 : 0;
-    else if (!strcmp(name, "store_A")) s->opt_store_A = value ? 1 : 0;
+    else if (!strcmp(name, "store_A")) { s->opt_store_A = value ? 1 : 0; s->plan_dirty = true; }
+    else if (!strcmp(name, "use_jit")) { s->opt_jit = value ? 1 : 0; s->plan_dirty = true; }
     else return spin::fail(SPIN_ERR_ARG, "unknown option '%s'", name);
     drop_graphs(s);
+    return SPIN_OK;
+}
+
+// which sweep kernels are in use: "jit" (run-time specialised) or "generic: <reason>"
+extern "C" int spin_kernel_info(spin_system *s, char *buf, int len) {
+    REQUIRE(s && buf && len > 0, "bad argument");
+    if (s->has_device) { int rc = ensure_plan(s); if (rc) return rc; }
+    if (jit_ready(s)) snprintf(buf, (size_t)len, "jit");
+    else snprintf(buf, (size_t)len, "generic: %s", s->jit_note.c_str());
+    return SPIN_OK;
+}
+// the generated translation unit of the specialised sweeps; with compile != 0 it is also compiled with NVRTC (no device
+// needed) and the size of the cubin is returned in *cubin_bytes
+extern "C" int spin_jit_source(spin_system *s, char *buf, int len, int compile, int64_t *cubin_bytes) {
+    REQUIRE(s, "null system");
+    int rc = build_plan(s);
+    if (rc) return rc;
+    const std::string src = jit_source(s);
+    if (buf && len > 0) snprintf(buf, (size_t)len, "%s", src.c_str());
+    if (compile) {
+        std::string cubin, log;
+        rc = jit_compile(src, cubin, log);
+        if (rc) return rc;
+        if (cubin_bytes) *cubin_bytes = (int64_t)cubin.size();
+    }
     return SPIN_OK;
 }

@@ -1,0 +1,288 @@
+// spin_jit_kernels.cuh -- the two Depondt sweeps specialised per spin system (compiled at run time by NVRTC for sm_100a).
+//
+// The host planner (spin_jit.cu) prints the system as compile-time constants into `namespace spec` and then includes this
+// file.  Everything that the table-driven kernels (spin_kernels.cuh) look up at run time is a constant here:
+//   * lattice extents and boundary conditions  -> div/mod and periodic wrap by constants, open-edge tests only where needed
+//   * the gather table of every basis atom     -> fully unrolled, J and D folded into fma operands, zero D components dropped,
+//                                                 partner coordinates shared between entries by common-subexpression elimination
+//   * LLG prefactors, time step, noise amplitude
+// One thread per spin, bricks of BX x BY x BZ spins of one sublattice per block; no atomics, no shared memory.
+// Device-only: no host headers (NVRTC).  Formulas and paper citations: see spin_kernels.cuh / spin_device_math.cuh.
+//
+// namespace spec must define (all constexpr):
+//   int NA, NB, NC, NBASIS, NCELL, STRIDE, BX, BY, BZ;  bool PER_A, PER_B, PER_C, STORE_A, HAS_DDI, THERMAL_ON, STT_ON;
+//   int PAIR_BEGIN[NBASIS+1], P_DA[], P_DB[], P_DC[], P_BJ[];  double P_J[], P_DX[], P_DY[], P_DZ[];
+//   int QUAD_BEGIN[NBASIS+1], Q_D[][9], Q_B[][3];  double Q_K[];
+//   double ZEE[NBASIS][3], K2[NBASIS], KAX[NBASIS][3], PRE[NBASIS], SIGMA[NBASIS];
+//   double ALPHA, DT, DT2, STT_C[3], STT_S, STT_X;
+#pragma once
+
+#include "spin_device_math.cuh"
+
+namespace spinjit {
+
+typedef unsigned int u32;
+typedef unsigned long long u64;
+
+template <int V> struct Int { static constexpr int value = V; };
+
+template <int I, int END, class F>
+__device__ __forceinline__ void static_for(F &&f) {
+    if constexpr (I < END) {
+        f(Int<I>{});
+        static_for<I + 1, END>(f);
+    }
+}
+
+struct Coord { int ia, ib, ic; };
+
+// coordinate i shifted by the compile-time translation D along a direction with N cells.  Periodic: wrapped (|D| <= N/2 by
+// construction of the table).  Open: `ok` is cleared when the partner is off the edge and the own coordinate is returned.
+template <int D, int N, bool PER>
+__device__ __forceinline__ int shift(int i, bool &ok) {
+    if constexpr (D == 0) {
+        return i;
+    } else if constexpr (PER) {
+        int j = i + D;
+        if constexpr (D > 0) { if (j >= N) j -= N; } else { if (j < 0) j += N; }
+        return j;
+    } else {
+        const int j = i + D;
+        const bool in = (D > 0) ? (j < N) : (j >= 0);
+        ok = ok && in;
+        return in ? j : i;
+    }
+}
+
+template <int DA, int DB, int DC, int BJ>
+__device__ __forceinline__ int partner(const Coord &c, bool &ok) {
+    const int ja = shift<DA, spec::NA, spec::PER_A>(c.ia, ok);
+    const int jb = shift<DB, spec::NB, spec::PER_B>(c.ib, ok);
+    const int jc = shift<DC, spec::NC, spec::PER_C>(c.ic, ok);
+    return BJ * spec::NCELL + ja + spec::NA * jb + (spec::NA * spec::NB) * jc;
+}
+
+template <int DA, int DB, int DC>
+__host__ __device__ constexpr bool always_inside() {
+    return (DA == 0 || spec::PER_A) && (DB == 0 || spec::PER_B) && (DC == 0 || spec::PER_C);
+}
+
+__device__ __forceinline__ void load3(const double *p, int j, double (&v)[3]) {
+    v[0] = __ldg(p + j);
+    v[1] = __ldg(p + spec::STRIDE + j);
+    v[2] = __ldg(p + 2 * spec::STRIDE + j);
+}
+
+// F += (Zeeman + anisotropy + pairs + quadruplets) of basis atom B for NCONF configurations sharing the lattice
+template <int B, int NCONF>
+__device__ __forceinline__ void force(const double *const (&cfg)[NCONF], const Coord &c, const double (&own)[NCONF][3],
+                                      double (&F)[NCONF][3]) {
+#pragma unroll
+    for (int k = 0; k < NCONF; ++k) {
+        if constexpr (spec::ZEE[B][0] != 0.0) F[k][0] += spec::ZEE[B][0];
+        if constexpr (spec::ZEE[B][1] != 0.0) F[k][1] += spec::ZEE[B][1];
+        if constexpr (spec::ZEE[B][2] != 0.0) F[k][2] += spec::ZEE[B][2];
+        if constexpr (spec::K2[B] != 0.0) {
+            constexpr double kx = spec::KAX[B][0], ky = spec::KAX[B][1], kz = spec::KAX[B][2];
+            double p = 0.0;
+            if constexpr (kx != 0.0) p = fma(kx, own[k][0], p);
+            if constexpr (ky != 0.0) p = fma(ky, own[k][1], p);
+            if constexpr (kz != 0.0) p = fma(kz, own[k][2], p);
+            p *= spec::K2[B];
+            if constexpr (kx != 0.0) F[k][0] = fma(p, kx, F[k][0]);
+            if constexpr (ky != 0.0) F[k][1] = fma(p, ky, F[k][1]);
+            if constexpr (kz != 0.0) F[k][2] = fma(p, kz, F[k][2]);
+        }
+    }
+    static_for<spec::PAIR_BEGIN[B], spec::PAIR_BEGIN[B + 1]>([&](auto e) {
+        constexpr int E = decltype(e)::value;
+        constexpr int DA = spec::P_DA[E], DB = spec::P_DB[E], DC = spec::P_DC[E];
+        constexpr double J = spec::P_J[E], Dx = spec::P_DX[E], Dy = spec::P_DY[E], Dz = spec::P_DZ[E];
+        bool ok = true;
+        const int j = partner<DA, DB, DC, spec::P_BJ[E]>(c, ok);
+#pragma unroll
+        for (int k = 0; k < NCONF; ++k) {
+            double p[3];
+            load3(cfg[k], j, p);
+            if constexpr (!always_inside<DA, DB, DC>()) {
+                if (!ok) { p[0] = 0.0; p[1] = 0.0; p[2] = 0.0; }
+            }
+            // J n_j + n_j x D, zero components dropped at compile time
+            if constexpr (J != 0.0) { F[k][0] = fma(J, p[0], F[k][0]); F[k][1] = fma(J, p[1], F[k][1]); F[k][2] = fma(J, p[2], F[k][2]); }
+            if constexpr (Dz != 0.0) { F[k][0] = fma(p[1], Dz, F[k][0]); F[k][1] = fma(p[0], -Dz, F[k][1]); }
+            if constexpr (Dy != 0.0) { F[k][0] = fma(p[2], -Dy, F[k][0]); F[k][2] = fma(p[0], Dy, F[k][2]); }
+            if constexpr (Dx != 0.0) { F[k][1] = fma(p[2], Dx, F[k][1]); F[k][2] = fma(p[1], -Dx, F[k][2]); }
+        }
+    });
+    static_for<spec::QUAD_BEGIN[B], spec::QUAD_BEGIN[B + 1]>([&](auto e) {
+        constexpr int E = decltype(e)::value;
+        bool ok = true;
+        const int jp = partner<spec::Q_D[E][0], spec::Q_D[E][1], spec::Q_D[E][2], spec::Q_B[E][0]>(c, ok);
+        const int jq = partner<spec::Q_D[E][3], spec::Q_D[E][4], spec::Q_D[E][5], spec::Q_B[E][1]>(c, ok);
+        const int jr = partner<spec::Q_D[E][6], spec::Q_D[E][7], spec::Q_D[E][8], spec::Q_B[E][2]>(c, ok);
+        constexpr bool inside = always_inside<spec::Q_D[E][0], spec::Q_D[E][1], spec::Q_D[E][2]>() &&
+                                always_inside<spec::Q_D[E][3], spec::Q_D[E][4], spec::Q_D[E][5]>() &&
+                                always_inside<spec::Q_D[E][6], spec::Q_D[E][7], spec::Q_D[E][8]>();
+#pragma unroll
+        for (int k = 0; k < NCONF; ++k) {
+            double P[3], Q[3], R[3];
+            load3(cfg[k], jp, P); load3(cfg[k], jq, Q); load3(cfg[k], jr, R);
+            double w = spec::Q_K[E] * fma(Q[0], R[0], fma(Q[1], R[1], Q[2] * R[2]));
+            if constexpr (!inside) { if (!ok) w = 0.0; }
+            F[k][0] = fma(w, P[0], F[k][0]); F[k][1] = fma(w, P[1], F[k][1]); F[k][2] = fma(w, P[2], F[k][2]);
+        }
+    });
+}
+
+// (j^ . grad) n: central differences on the same sublattice, one-sided at open edges
+template <int B, int NCONF>
+__device__ __forceinline__ void stt_gradient(const double *const (&cfg)[NCONF], const Coord &c, const double (&own)[NCONF][3],
+                                             double (&sg)[NCONF][3]) {
+    static_for<0, 3>([&](auto dd) {
+        constexpr int D = decltype(dd)::value;
+        if constexpr (spec::STT_C[D] != 0.0) {
+            bool hp = true, hm = true;
+            const int jp = partner<(D == 0), (D == 1), (D == 2), B>(c, hp);
+            const int jm = partner<-(D == 0), -(D == 1), -(D == 2), B>(c, hm);
+            const double w = spec::STT_C[D] * ((hp && hm) ? 0.5 : ((hp || hm) ? 1.0 : 0.0));
+#pragma unroll
+            for (int k = 0; k < NCONF; ++k) {
+                double vp[3], vm[3];
+                load3(cfg[k], jp, vp); load3(cfg[k], jm, vm);      // off-edge partners alias the own site -> difference 0
+                sg[k][0] = fma(w, vp[0] - vm[0], sg[k][0]); sg[k][1] = fma(w, vp[1] - vm[1], sg[k][1]); sg[k][2] = fma(w, vp[2] - vm[2], sg[k][2]);
+            }
+        }
+    });
+}
+
+// A = pre [F + alpha n x F] + stt_s s + stt_x n x s   (Eq. 10 as dn/dt = n x A)
+template <int B>
+__device__ __forceinline__ void rotation_field(const double (&n)[3], const double (&F)[3], const double (&sg)[3], double (&A)[3]) {
+    constexpr double pre = spec::PRE[B], pa = spec::PRE[B] * spec::ALPHA;
+    const double cx = fma(n[1], F[2], -n[2] * F[1]), cy = fma(n[2], F[0], -n[0] * F[2]), cz = fma(n[0], F[1], -n[1] * F[0]);
+    A[0] = fma(pa, cx, pre * F[0]);
+    A[1] = fma(pa, cy, pre * F[1]);
+    A[2] = fma(pa, cz, pre * F[2]);
+    if constexpr (spec::STT_ON) {
+        const double sx = fma(n[1], sg[2], -n[2] * sg[1]), sy = fma(n[2], sg[0], -n[0] * sg[2]), sz = fma(n[0], sg[1], -n[1] * sg[0]);
+        A[0] += fma(spec::STT_X, sx, spec::STT_S * sg[0]);
+        A[1] += fma(spec::STT_X, sy, spec::STT_S * sg[1]);
+        A[2] += fma(spec::STT_X, sz, spec::STT_S * sg[2]);
+    }
+}
+
+__device__ __forceinline__ bool locate(Coord &c, int &idx, int b) {
+    constexpr int nbx = (spec::NA + spec::BX - 1) / spec::BX, nby = (spec::NB + spec::BY - 1) / spec::BY;
+    int brick = blockIdx.x;
+    const int bx = brick % nbx;
+    brick /= nbx;
+    const int by = brick % nby, bz = brick / nby;
+    const int t = threadIdx.x;
+    c.ia = bx * spec::BX + (t % spec::BX);
+    c.ib = by * spec::BY + (t / spec::BX) % spec::BY;
+    c.ic = bz * spec::BZ + t / (spec::BX * spec::BY);
+    idx = b * spec::NCELL + c.ia + spec::NA * c.ib + (spec::NA * spec::NB) * c.ic;
+    return (c.ia < spec::NA) && (c.ib < spec::NB) && (c.ic < spec::NC);
+}
+
+template <int B>
+__device__ __forceinline__ void thermal_force(const Coord &c, u64 step, u32 seed_lo, u32 seed_hi, double (&f)[3]) {
+    if constexpr (spec::THERMAL_ON) {
+        const u32 cell = (u32)(c.ia + spec::NA * c.ib + (spec::NA * spec::NB) * c.ic);
+        double xi[3];
+        spin::thermal_xi(seed_lo, seed_hi, step, (u32)B + (u32)spec::NBASIS * cell, xi);
+        f[0] = spec::SIGMA[B] * xi[0]; f[1] = spec::SIGMA[B] * xi[1]; f[2] = spec::SIGMA[B] * xi[2];
+    } else {
+        f[0] = 0.0; f[1] = 0.0; f[2] = 0.0;
+    }
+}
+
+template <int B>
+__device__ __forceinline__ void predictor_body(const double *__restrict__ n, const double *__restrict__ fddi, double *__restrict__ np,
+                                               double *__restrict__ Aout, u64 step, u32 seed_lo, u32 seed_hi) {
+    Coord c;
+    int idx;
+    if (!locate(c, idx, B)) return;
+    const double *const cfg[1] = {n};
+    double own[1][3], F[1][3], sg[1][3] = {{0.0, 0.0, 0.0}};
+    load3(n, idx, own[0]);
+    thermal_force<B>(c, step, seed_lo, seed_hi, F[0]);
+    force<B, 1>(cfg, c, own, F);
+    if constexpr (spec::HAS_DDI) { double d[3]; load3(fddi, idx, d); F[0][0] += d[0]; F[0][1] += d[1]; F[0][2] += d[2]; }
+    if constexpr (spec::STT_ON) stt_gradient<B, 1>(cfg, c, own, sg);
+    double A[3], out[3];
+    rotation_field<B>(own[0], F[0], sg[0], A);
+    spin::rodrigues(A, spec::DT, spec::DT2, own[0], out);
+    np[idx] = out[0]; np[spec::STRIDE + idx] = out[1]; np[2 * spec::STRIDE + idx] = out[2];
+    if constexpr (spec::STORE_A) { Aout[idx] = A[0]; Aout[spec::STRIDE + idx] = A[1]; Aout[2 * spec::STRIDE + idx] = A[2]; }
+}
+
+template <int B>
+__device__ __forceinline__ void corrector_body(const double *__restrict__ n, const double *__restrict__ np, const double *__restrict__ fddi_n,
+                                               const double *__restrict__ fddi_np, const double *__restrict__ Ain, double *__restrict__ nout,
+                                               u64 step, u32 seed_lo, u32 seed_hi) {
+    Coord c;
+    int idx;
+    if (!locate(c, idx, B)) return;
+    double th[3], A[3], Ap[3], n0[3];
+    thermal_force<B>(c, step, seed_lo, seed_hi, th);
+    load3(n, idx, n0);
+    if constexpr (spec::STORE_A) {
+        const double *const cfg[1] = {np};
+        double own[1][3], F[1][3] = {{th[0], th[1], th[2]}}, sg[1][3] = {{0.0, 0.0, 0.0}};
+        load3(np, idx, own[0]);
+        force<B, 1>(cfg, c, own, F);
+        if constexpr (spec::HAS_DDI) { double d[3]; load3(fddi_np, idx, d); F[0][0] += d[0]; F[0][1] += d[1]; F[0][2] += d[2]; }
+        if constexpr (spec::STT_ON) stt_gradient<B, 1>(cfg, c, own, sg);
+        rotation_field<B>(own[0], F[0], sg[0], Ap);
+        load3(Ain, idx, A);
+    } else {
+        const double *const cfg[2] = {n, np};
+        double own[2][3], F[2][3] = {{th[0], th[1], th[2]}, {th[0], th[1], th[2]}}, sg[2][3] = {{0.0, 0.0, 0.0}, {0.0, 0.0, 0.0}};
+        own[0][0] = n0[0]; own[0][1] = n0[1]; own[0][2] = n0[2];
+        load3(np, idx, own[1]);
+        force<B, 2>(cfg, c, own, F);
+        if constexpr (spec::HAS_DDI) {
+            double d[3];
+            load3(fddi_n, idx, d); F[0][0] += d[0]; F[0][1] += d[1]; F[0][2] += d[2];
+            load3(fddi_np, idx, d); F[1][0] += d[0]; F[1][1] += d[1]; F[1][2] += d[2];
+        }
+        if constexpr (spec::STT_ON) stt_gradient<B, 2>(cfg, c, own, sg);
+        rotation_field<B>(own[0], F[0], sg[0], A);
+        rotation_field<B>(own[1], F[1], sg[1], Ap);
+    }
+    const double Ac[3] = {0.5 * (A[0] + Ap[0]), 0.5 * (A[1] + Ap[1]), 0.5 * (A[2] + Ap[2])};
+    double out[3];
+    spin::rodrigues(Ac, spec::DT, spec::DT2, n0, out);
+    spin::renormalise(out);
+    nout[idx] = out[0]; nout[spec::STRIDE + idx] = out[1]; nout[2 * spec::STRIDE + idx] = out[2];
+}
+
+template <int B, class Fn>
+__device__ __forceinline__ void dispatch_basis(int b, Fn &&fn) {
+    if constexpr (B < spec::NBASIS) {
+        if (b == B) fn(Int<B>{});
+        else dispatch_basis<B + 1>(b, fn);
+    }
+}
+
+}  // namespace spinjit
+
+extern "C" __global__ void __launch_bounds__(spec::BX *spec::BY *spec::BZ)
+    jit_predictor(const double *__restrict__ n, const double *__restrict__ fddi, double *__restrict__ np, double *__restrict__ Aout,
+                  const unsigned long long *__restrict__ d_step, unsigned int step_add, unsigned int seed_lo, unsigned int seed_hi) {
+    const unsigned long long step = *d_step + step_add;
+    spinjit::dispatch_basis<0>((int)blockIdx.y, [&](auto b) {
+        spinjit::predictor_body<decltype(b)::value>(n, fddi, np, Aout, step, seed_lo, seed_hi);
+    });
+}
+
+extern "C" __global__ void __launch_bounds__(spec::BX *spec::BY *spec::BZ)
+    jit_corrector(const double *__restrict__ n, const double *__restrict__ np, const double *__restrict__ fddi_n,
+                  const double *__restrict__ fddi_np, const double *__restrict__ Ain, double *__restrict__ nout,
+                  const unsigned long long *__restrict__ d_step, unsigned int step_add, unsigned int seed_lo, unsigned int seed_hi) {
+    const unsigned long long step = *d_step + step_add;
+    spinjit::dispatch_basis<0>((int)blockIdx.y, [&](auto b) {
+        spinjit::corrector_body<decltype(b)::value>(n, np, fddi_n, fddi_np, Ain, nout, step, seed_lo, seed_hi);
+    });
+}

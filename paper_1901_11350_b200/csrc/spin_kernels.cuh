@@ -13,6 +13,7 @@
 #pragma once
 
 #include "spinllg_internal.h"
+#include "spin_device_math.cuh"
 
 namespace spin {
 
@@ -143,37 +144,6 @@ __device__ __forceinline__ void stt_gradient(const DevicePlan &P, const double *
 }
 
 // ---------------------------------------------------------------------------------------------------------
-// Philox4x32-10 (Salmon et al. 2011) and the thermal triple (R13): key = seed, counter =
-// (spin, block, step_lo, step_hi); uniforms from the top 53 of 64 bits (+1/2 ulp); Box-Muller.
-__device__ __forceinline__ void philox4x32_10(uint32_t &c0, uint32_t &c1, uint32_t &c2, uint32_t &c3, uint32_t k0, uint32_t k1) {
-#pragma unroll
-    for (int r = 0; r < 10; ++r) {
-        const uint32_t h0 = __umulhi(0xD2511F53u, c0), l0 = 0xD2511F53u * c0;
-        const uint32_t h1 = __umulhi(0xCD9E8D57u, c2), l1 = 0xCD9E8D57u * c2;
-        const uint32_t n0 = h1 ^ c1 ^ k0, n2 = h0 ^ c3 ^ k1;
-        c0 = n0; c1 = l1; c2 = n2; c3 = l0;
-        k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
-    }
-}
-__device__ __forceinline__ double uniform53(uint32_t hi, uint32_t lo) {
-    const unsigned long long v = (((unsigned long long)hi << 32) | lo) >> 11;
-    return ((double)v + 0.5) * (1.0 / 9007199254740992.0);
-}
-__device__ __forceinline__ void thermal_xi(uint32_t seed_lo, uint32_t seed_hi, unsigned long long step, uint32_t spin, double (&xi)[3]) {
-    uint32_t a0 = spin, a1 = 0u, a2 = (uint32_t)step, a3 = (uint32_t)(step >> 32);
-    philox4x32_10(a0, a1, a2, a3, seed_lo, seed_hi);
-    double sn, cs;
-    double rad = sqrt(-2.0 * log(uniform53(a0, a1)));
-    sincospi(2.0 * uniform53(a2, a3), &sn, &cs);
-    xi[0] = rad * cs;
-    xi[1] = rad * sn;
-    uint32_t b0 = spin, b1 = 1u, b2 = (uint32_t)step, b3 = (uint32_t)(step >> 32);
-    philox4x32_10(b0, b1, b2, b3, seed_lo, seed_hi);
-    rad = sqrt(-2.0 * log(uniform53(b0, b1)));
-    xi[2] = rad * cospi(2.0 * uniform53(b2, b3));
-}
-
-// ---------------------------------------------------------------------------------------------------------
 // Eq. 10 as dn/dt = n x A:  A = pre [F + alpha n x F] + stt_s s + stt_x n x s
 __device__ __forceinline__ void rotation_field(const DevicePlan &P, int b, const double (&n)[3], const double (&F)[3],
                                                const double (&sg)[3], double (&A)[3]) {
@@ -188,51 +158,6 @@ __device__ __forceinline__ void rotation_field(const DevicePlan &P, int b, const
         A[1] += P.stt_s * sg[1] + P.stt_x * sy;
         A[2] += P.stt_s * sg[2] + P.stt_x * sz;
     }
-}
-
-// R(A) n: Rodrigues rotation about -A/|A| by theta = |A| dt (exact flow of dn/dt = n x A for constant A).
-// Written without square root or division:  with x = theta^2,
-//     n' = n (1 - x q(x)) - (A x n) dt s(x) + A (A.n) dt^2 q(x),   s = sin(theta)/theta,  q = (1 - cos(theta))/theta^2
-// s and q are even power series in theta; for x < 1/4 their Taylor polynomials of degree 8 in x are exact to
-// < 1e-18; larger angles take the trigonometric branch.
-__device__ __forceinline__ void rodrigues(const double (&A)[3], double dt, double dt2, const double (&n)[3], double (&out)[3]) {
-    const double a2 = A[0] * A[0] + A[1] * A[1] + A[2] * A[2];
-    const double x = a2 * dt2;
-    double s, q;
-    if (x < 0.25) {
-        // s(x) = sum (-x)^k / (2k+1)!,  q(x) = sum (-x)^k / (2k+2)!
-        s = -1.0 / 355687428096000.0;                 // 1/17!
-        q = -1.0 / 6402373705728000.0;                // 1/18!
-        s = fma(s, x, 1.0 / 1307674368000.0);   q = fma(q, x, 1.0 / 20922789888000.0);   // 15!, 16!
-        s = fma(s, x, -1.0 / 6227020800.0);     q = fma(q, x, -1.0 / 87178291200.0);     // 13!, 14!
-        s = fma(s, x, 1.0 / 39916800.0);        q = fma(q, x, 1.0 / 479001600.0);        // 11!, 12!
-        s = fma(s, x, -1.0 / 362880.0);         q = fma(q, x, -1.0 / 3628800.0);         // 9!, 10!
-        s = fma(s, x, 1.0 / 5040.0);            q = fma(q, x, 1.0 / 40320.0);            // 7!, 8!
-        s = fma(s, x, -1.0 / 120.0);            q = fma(q, x, -1.0 / 720.0);             // 5!, 6!
-        s = fma(s, x, 1.0 / 6.0);               q = fma(q, x, 1.0 / 24.0);               // 3!, 4!
-        s = fma(s, -x, 1.0);                    q = fma(q, -x, 0.5);
-    } else {
-        const double th = sqrt(x);
-        double sn, cs;
-        sincos(th, &sn, &cs);
-        s = sn / th;
-        q = (1.0 - cs) / x;
-    }
-    const double c = fma(-x, q, 1.0);
-    const double ds = dt * s, an = (A[0] * n[0] + A[1] * n[1] + A[2] * n[2]) * dt2 * q;
-    const double cx = A[1] * n[2] - A[2] * n[1], cy = A[2] * n[0] - A[0] * n[2], cz = A[0] * n[1] - A[1] * n[0];
-    out[0] = n[0] * c - cx * ds + A[0] * an;
-    out[1] = n[1] * c - cy * ds + A[1] * an;
-    out[2] = n[2] * c - cz * ds + A[2] * an;
-}
-
-__device__ __forceinline__ void renormalise(double (&v)[3]) {
-    // |v|^2 = 1 + eps with eps ~ 1e-16 after a rotation of a unit vector: 1/sqrt(1+eps) by its series
-    const double eps = fma(v[0], v[0], fma(v[1], v[1], fma(v[2], v[2], -1.0)));
-    double sc;
-    if (fabs(eps) < 1e-5) sc = fma(eps, fma(eps, fma(eps, -0.3125, 0.375), -0.5), 1.0);
-    else sc = 1.0 / sqrt(1.0 + eps);
-    v[0] *= sc; v[1] *= sc; v[2] *= sc;
 }
 
 // ---------------------------------------------------------------------------------------------------------

@@ -81,6 +81,7 @@ struct HostQuad { int b[4]; int t[9]; double K; };
 }  // namespace spin
 
 struct DdiState;   // spin_ddi.cu
+struct JitState;   // spin_jit.cu
 
 struct spin_system {
     // ---- geometry
@@ -115,8 +116,11 @@ struct spin_system {
     spin::DevicePlan plan;
     bool plan_dirty;
     DdiState *ddi;
+    JitState *jit;                 // run-time specialised sweeps (null: table-driven kernels)
+    bool has_device;               // false only in the planner-only mode used by the CPU tests
+    std::string jit_note;          // why the specialised sweeps are not in use, if they are not
     // ---- execution options / bookkeeping
-    int opt_graph, opt_store_A;
+    int opt_graph, opt_store_A, opt_jit;
     cudaGraphExec_t graph_exec[2];   // one captured graph per ping-pong parity
     int graph_steps;
     int64_t n_launch, n_fft;
@@ -141,4 +145,16 @@ int fail(int code, const char *fmt, ...);
 int ddi_prepare(spin_system *s);                                   // (re)build tensor spectra and FFT plans
 int ddi_field(spin_system *s, const double *d_n, double *d_f);     // d_f (SoA, meV) = dipolar force of d_n
 void ddi_release(spin_system *s);
+
+// spin_jit.cu
+std::string jit_source(const spin_system *s);
+int jit_compile(const std::string &source, std::string &cubin, std::string &log);
+int jit_prepare(spin_system *s);
+void jit_release(spin_system *s);
+bool jit_ready(const spin_system *s);
+const char *jit_log(const spin_system *s);
+int jit_launch_predictor(spin_system *s, dim3 grid, dim3 block, const double *n, const double *fddi, double *np, double *Aout,
+                         unsigned step_add);
+int jit_launch_corrector(spin_system *s, dim3 grid, dim3 block, const double *n, const double *np, const double *fddi_n,
+                         const double *fddi_np, const double *Ain, double *nout, unsigned step_add);
 }  // namespace spin

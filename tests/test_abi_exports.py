@@ -56,3 +56,28 @@ def test_product_does_not_import_oracle():
                 assert "spin_oracle" not in src and "liboracle" not in src, f
     osrc = open(os.path.join(ROOT, "oracle", "spin_oracle.c")).read() + open(os.path.join(ROOT, "oracle", "__init__.py")).read()
     assert "paper_1901_11350_b200" not in osrc.replace("paper_1901_11350_b200/; only", "").replace("(paper_1901_11350_b200) never", "")
+
+
+@pytest.mark.parametrize("cfg", [1, 2, 3, 4, 5])
+def test_planner_generates_and_compiles_specialised_sweeps(cfg, monkeypatch):
+    """Host planner + NVRTC (no device needed): the gather tables of every config become a translation unit that compiles
+    for sm_100a.  Entry counts per spin as SURVEY 8(a) states them: 4 / 18 / 6 / 9 pairs + 4 quadruplet roles / 6."""
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("planner-only mode is for boxes without a GPU")
+    monkeypatch.setenv("SPINLLG_PLANNER_ONLY", "1")
+    import paper_1901_11350_b200 as P
+    import workloads as W
+    w = W.CONFIGS[cfg]()
+    s = P.SpinSystem.from_workload(w, set_spins=False)
+    src, nbytes = s.spin_jit_source(compile=True)
+    assert nbytes > 10000
+    begin = [int(x) for x in re.search(r"PAIR_BEGIN\[\d+\] = \{([^}]*)\}", src).group(1).split(",")]
+    qbegin = [int(x) for x in re.search(r"QUAD_BEGIN\[\d+\] = \{([^}]*)\}", src).group(1).split(",")]
+    expect_pairs = {1: [4], 2: [18], 3: [6], 4: [9, 9], 5: [6]}[cfg]
+    assert [b - a for a, b in zip(begin, begin[1:])] == expect_pairs
+    assert [b - a for a, b in zip(qbegin, qbegin[1:])] == ({4: [4, 4]}.get(cfg, [0] * w.n_basis))
+    # computing without a device still fails loudly
+    with pytest.raises(P.SpinError) as e:
+        s.llg_iterate(1)
+    assert e.value.code == -4

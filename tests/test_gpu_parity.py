@@ -234,3 +234,16 @@ def test_device_pointer_io_with_torch_stream(P, O):
     o.iterate(40)
     assert np.abs(out.cpu().numpy() - o.spins()).max() < 1e-12
     assert_fields_close(B.cpu().numpy(), o.effective_field())
+
+
+@pytest.mark.parametrize("cfg", [1, 2, 3, 4, 5])
+def test_specialised_and_table_driven_sweeps_agree(P, O, cfg):
+    """The NVRTC-specialised sweeps are the default path; the table-driven kernels (use_jit=0) must give the same trajectory."""
+    w = W.CONFIGS[cfg]().resized(REPLICAS[cfg], 30)
+    a = P.SpinSystem.from_workload(w)
+    b = P.SpinSystem.from_workload(w)
+    b.spin_set_option("use_jit", 0)
+    assert a.spin_kernel_info() == "jit", a.spin_kernel_info()
+    assert b.spin_kernel_info().startswith("generic")
+    a.llg_iterate(30); b.llg_iterate(30)
+    assert np.abs(a.spins_get() - b.spins_get()).max() < 1e-13
