@@ -159,12 +159,12 @@ int stt_coefficients(const spin_system *s, double cd[3]) {
     return 0;
 }
 
-int build_plan(spin_system *s) {
-    DevicePlan &P = s->plan;
+int build_plan(const spin_system *s, DevicePlan &P) {
     memset(&P, 0, sizeof(P));
+    int reach[3] = {0, 0, 0};
     P.Na = s->nc[0]; P.Nb = s->nc[1]; P.Nc = s->nc[2];
     P.perA = s->per[0]; P.perB = s->per[1]; P.perC = s->per[2];
-    P.nb = s->nb; P.Ncell = (int)s->ncell; P.stride = s->stride;
+    P.nb = s->nb; P.Ncell = (int)s->ncell;
     const double a2 = 1.0 + s->alpha * s->alpha;
     for (int b = 0; b < s->nb; ++b) {
         const double m = s->mu[b] * MU_B;
@@ -183,7 +183,7 @@ int build_plan(spin_system *s) {
         if (stt_coefficients(s, P.stt_c) != 0) return spin::fail(SPIN_ERR_ARG, "current direction: singular lattice metric");
         P.stt_s = -s->u * (s->alpha - s->beta) / a2;
         P.stt_x = s->u * (1.0 + s->alpha * s->beta) / a2;
-        for (int d = 0; d < 3; ++d) if (P.stt_c[d] != 0.0) P.reach[d] = 1;
+        for (int d = 0; d < 3; ++d) if (P.stt_c[d] != 0.0) reach[d] = 1;
     }
     // ---- pair gather tables: every unique pair gives a forward entry for basis atom bi (+t, +D) and a backward
     // entry for bj (-t, -D).  Order per atom: all forward entries in list order, then all backward entries.
@@ -210,7 +210,6 @@ int build_plan(spin_system *s) {
                 if (dead) continue;
                 e.da = t[0]; e.db = t[1]; e.dc = t[2];
                 e.bj = dir == 0 ? p.bj : p.bi;
-                e.lin = (e.bj - b) * (int)s->ncell + t[0] + Nd[0] * (t[1] + Nd[1] * t[2]);
                 e.J = p.J; e.Dx = sgn * p.D[0]; e.Dy = sgn * p.D[1]; e.Dz = sgn * p.D[2];
                 // merge with an existing entry on the same partner (e.g. exchange shells + DMI shells on one bond)
                 bool merged = false;
@@ -226,7 +225,7 @@ int build_plan(spin_system *s) {
                 if (ne >= SPIN_MAX_PAIR_ENTRIES)
                     return spin::fail(SPIN_ERR_LIMIT, "pair table needs more than %d gather entries", SPIN_MAX_PAIR_ENTRIES);
                 P.pairs[ne++] = e;
-                for (int d = 0; d < 3; ++d) P.reach[d] = std::max(P.reach[d], abs(t[d]));
+                for (int d = 0; d < 3; ++d) reach[d] = std::max(reach[d], abs(t[d]));
             }
     }
     P.pair_begin[s->nb] = ne;
@@ -250,12 +249,11 @@ int build_plan(spin_system *s) {
                         const int t = reduce_translation(tm[mem[m]][d] - tm[role][d], Nd[d], s->per[d]);
                         if (!s->per[d] && abs(t) >= Nd[d]) dead = true;
                         e.d[m][d] = t;
-                        P.reach[d] = std::max(P.reach[d], abs(t));
                     }
                     e.b[m] = q.b[mem[m]];
-                    e.lin[m] = (e.b[m] - b) * (int)s->ncell + e.d[m][0] + Nd[0] * (e.d[m][1] + Nd[1] * e.d[m][2]);
                 }
                 if (dead) continue;      // some member can never be inside an open lattice
+                for (int m = 0; m < 3; ++m) for (int d = 0; d < 3; ++d) reach[d] = std::max(reach[d], abs(e.d[m][d]));
                 e.K = q.K;
                 if (nq >= SPIN_MAX_QUAD_ENTRIES)
                     return spin::fail(SPIN_ERR_LIMIT, "quadruplet table needs more than %d role entries", SPIN_MAX_QUAD_ENTRIES);
@@ -264,9 +262,29 @@ int build_plan(spin_system *s) {
         }
     }
     P.quad_begin[s->nb] = nq;
-    // an entry whose reduced translation equals the lattice size can only be interior-tested with a real margin
-    for (int d = 0; d < 3; ++d) if (P.reach[d] >= Nd[d]) P.reach[d] = Nd[d];   // never interior in that direction
+    // ---- layout with ghost cells (spinllg_internal.h): ghost width = reach; rows start on 128-byte lines
+    P.rA = reach[0]; P.rB = reach[1]; P.rC = reach[2];
+    P.gA = (P.perA && P.rA > 0) ? 1 : 0; P.gB = (P.perB && P.rB > 0) ? 1 : 0; P.gC = (P.perC && P.rC > 0) ? 1 : 0;
+    P.LA = (P.rA + 15) / 16 * 16; P.LB = P.rB; P.LC = P.rC;
+    P.PA = P.LA + (P.Na + P.rA + 15) / 16 * 16; P.PB = P.Nb + 2 * P.rB; P.PC = P.Nc + 2 * P.rC;
+    const int64_t sub = (int64_t)3 * P.PA * P.PB * P.PC;
+    if (sub * s->nb >= (int64_t)2147483647) return spin::fail(SPIN_ERR_LIMIT, "padded lattice too large for 32-bit indexing");
+    P.sub = (int)sub;
+    auto lin = [&](int b, int bj, const int t[3]) { return (bj - b) * P.sub + (t[2] * P.PB + t[1]) * 3 * P.PA + t[0]; };
+    for (int b = 0; b < s->nb; ++b) {
+        for (int e = P.pair_begin[b]; e < P.pair_begin[b + 1]; ++e) {
+            const int t[3] = {P.pairs[e].da, P.pairs[e].db, P.pairs[e].dc};
+            P.pairs[e].lin = lin(b, P.pairs[e].bj, t);
+        }
+        for (int e = P.quad_begin[b]; e < P.quad_begin[b + 1]; ++e)
+            for (int m = 0; m < 3; ++m) P.quads[e].lin[m] = lin(b, P.quads[e].b[m], P.quads[e].d[m]);
+    }
     return SPIN_OK;
+}
+
+bool same_layout(const DevicePlan &a, const DevicePlan &b) {
+    return a.LA == b.LA && a.LB == b.LB && a.LC == b.LC && a.PA == b.PA && a.PB == b.PB && a.PC == b.PC && a.sub == b.sub &&
+           a.rA == b.rA && a.rB == b.rB && a.rC == b.rC && a.gA == b.gA && a.gB == b.gB && a.gC == b.gC;
 }
 
 #define NEED_DEVICE(s)                                                                                          \
@@ -274,17 +292,49 @@ int build_plan(spin_system *s) {
         if (!(s)->has_device) return spin::fail(SPIN_ERR_CUDA, "no CUDA device: this library has no CPU fallback"); \
     } while (0)
 
+// (re)allocate the per-spin arrays for the layout of `P`; the current configuration is carried over through the
+// boundary-order staging buffer when `keep` is set
+int allocate_arrays(spin_system *s, const DevicePlan &P, bool keep) {
+    const int nt = 256;
+    const unsigned nblk = (unsigned)((s->N + nt - 1) / nt);
+    if (keep) {
+        unpack_kernel<<<nblk, nt, 0, s->stream>>>(s->plan, s->d_n[s->cur], s->d_aos, (int)s->N, 0);
+        s->n_launch++;
+        SPIN_CUDA(cudaStreamSynchronize(s->stream));
+    }
+    double **arrs[] = {&s->d_n[0], &s->d_n[1], &s->d_np, &s->d_A, &s->d_fddi[0], &s->d_fddi[1]};
+    const size_t bytes = (size_t)s->nb * P.sub * sizeof(double);
+    for (double **a : arrs) {
+        if (*a) cudaFree(*a);
+        *a = nullptr;
+        cudaError_t e = cudaMalloc(a, bytes);
+        if (e != cudaSuccess) return spin::fail(SPIN_ERR_MEMORY, "device allocation of %zu bytes failed: %s", bytes, cudaGetErrorString(e));
+        SPIN_CUDA(cudaMemsetAsync(*a, 0, bytes, s->stream));      // ghost cells of open edges must read as zero forever
+    }
+    s->cur = 0;
+    if (keep) {
+        int *bad = (int *)(s->d_aos + (size_t)3 * s->N);
+        pack_kernel<<<nblk, nt, 0, s->stream>>>(P, s->d_aos, s->d_n[0], (int)s->N, 0, bad);
+        s->n_launch++;
+    }
+    SPIN_CUDA(cudaStreamSynchronize(s->stream));
+    SPIN_CUDA(cudaGetLastError());
+    return SPIN_OK;
+}
+
 int ensure_plan(spin_system *s) {
     NEED_DEVICE(s);
     if (!s->plan_dirty) return SPIN_OK;
-    int rc = build_plan(s);
+    DevicePlan P;
+    int rc = build_plan(s, P);
     if (rc) return rc;
     drop_graphs(s);
+    if (!s->d_n[0] || !same_layout(P, s->plan)) {
+        rc = allocate_arrays(s, P, s->d_n[0] != nullptr);
+        if (rc) return rc;
+    }
+    s->plan = P;
     if (s->ddi_on) {
-        if (!s->d_fddi[0]) {
-            SPIN_CUDA(cudaMalloc(&s->d_fddi[0], (size_t)3 * s->stride * sizeof(double)));
-            SPIN_CUDA(cudaMalloc(&s->d_fddi[1], (size_t)3 * s->stride * sizeof(double)));
-        }
         rc = ddi_prepare(s);
         if (rc) return rc;
     } else {
@@ -401,7 +451,6 @@ extern "C" int spin_geometry_create(const double bravais[9], int n_basis, const 
     for (int d = 0; d < 3; ++d) { s->nc[d] = n_cells[d]; s->per[d] = periodic[d] ? 1 : 0; }
     s->alat = lattice_constant_A;
     s->ncell = ncell; s->N = ncell * n_basis;
-    s->stride = (int)((s->N + 63) / 64 * 64);
     s->mu.assign(n_basis, 1.0);
     s->Bmag = 0.0; s->Bdir[0] = 0; s->Bdir[1] = 0; s->Bdir[2] = 1;
     s->K.assign(n_basis, 0.0);
@@ -417,23 +466,16 @@ extern "C" int spin_geometry_create(const double bravais[9], int n_basis, const 
     s->n_launch = s->n_fft = 0; s->profile_on = 0;
     for (int k = 0; k < 3; ++k) { s->prof_ms[k] = 0; s->prof_n[k] = 0; }
     s->ev0 = s->ev1 = nullptr;
-    const size_t bytes = (size_t)3 * s->stride * sizeof(double);
     const Launch L = brick_launch(s);
+    memset(&s->plan, 0, sizeof(s->plan));
     if (!has_device) { *out = s; return SPIN_OK; }
     cudaError_t e = cudaStreamCreateWithFlags(&s->own_stream, cudaStreamNonBlocking);
     s->stream = s->own_stream;
-    if (e == cudaSuccess) e = cudaMalloc(&s->d_n[0], bytes);
-    if (e == cudaSuccess) e = cudaMalloc(&s->d_n[1], bytes);
-    if (e == cudaSuccess) e = cudaMalloc(&s->d_np, bytes);
-    if (e == cudaSuccess) e = cudaMalloc(&s->d_A, bytes);
     if (e == cudaSuccess) e = cudaMalloc(&s->d_aos, (size_t)3 * s->N * sizeof(double) + sizeof(int));
     if (e == cudaSuccess) e = cudaMalloc(&s->d_partials, (size_t)L.grid.x * L.grid.y * N_RED * sizeof(double));
     if (e == cudaSuccess) e = cudaMalloc(&s->d_result, 16 * sizeof(double));
     if (e == cudaSuccess) e = cudaMalloc(&s->d_step, sizeof(unsigned long long));
     if (e == cudaSuccess) e = cudaMemset(s->d_step, 0, sizeof(unsigned long long));
-    if (e == cudaSuccess) e = cudaMemset(s->d_n[0], 0, bytes);
-    if (e == cudaSuccess) e = cudaMemset(s->d_n[1], 0, bytes);
-    if (e == cudaSuccess) e = cudaMemset(s->d_np, 0, bytes);
     if (e == cudaSuccess) e = cudaEventCreate(&s->ev0);
     if (e == cudaSuccess) e = cudaEventCreate(&s->ev1);
     if (e == cudaSuccess) e = cudaDeviceSynchronize();
@@ -447,7 +489,10 @@ extern "C" int spin_geometry_create(const double bravais[9], int n_basis, const 
     std::vector<double> z((size_t)3 * s->N, 0.0);
     for (int64_t i = 0; i < s->N; ++i) z[3 * i + 2] = 1.0;
     *out = s;
-    int rc = spins_set(s, z.data());
+    DevicePlan P0;                    // initial layout (no interactions yet: no ghost cells); the plan stays dirty
+    int rc = build_plan(s, P0);
+    if (rc == SPIN_OK) rc = allocate_arrays(s, P0, false);
+    if (rc == SPIN_OK) { s->plan = P0; rc = spins_set(s, z.data()); }
     if (rc) { spin_system_destroy(s); *out = nullptr; return rc; }
     return SPIN_OK;
 }
@@ -603,7 +648,7 @@ static int pack_from_device_aos(spin_system *s, const double *d_aos) {
     int *bad = (int *)(s->d_aos + (size_t)3 * s->N);
     SPIN_CUDA(cudaMemsetAsync(bad, 0, sizeof(int), s->stream));
     const int nt = 256;
-    pack_kernel<<<(unsigned)((s->N + nt - 1) / nt), nt, 0, s->stream>>>(d_aos, s->d_n[s->cur], (int)s->N, s->nb, (int)s->ncell, s->stride, 1, bad);
+    pack_kernel<<<(unsigned)((s->N + nt - 1) / nt), nt, 0, s->stream>>>(s->plan, d_aos, s->d_n[s->cur], (int)s->N, 1, bad);
     s->n_launch++;
     int h_bad = 0;
     SPIN_CUDA(cudaMemcpyAsync(&h_bad, bad, sizeof(int), cudaMemcpyDeviceToHost, s->stream));
@@ -626,7 +671,7 @@ extern "C" int spins_get_device(spin_system *s, double *n) {
     REQUIRE(s && n, "null argument");
     NEED_DEVICE(s);
     const int nt = 256;
-    unpack_kernel<<<(unsigned)((s->N + nt - 1) / nt), nt, 0, s->stream>>>(s->d_n[s->cur], n, (int)s->N, s->nb, (int)s->ncell, s->stride, nullptr);
+    unpack_kernel<<<(unsigned)((s->N + nt - 1) / nt), nt, 0, s->stream>>>(s->plan, s->d_n[s->cur], n, (int)s->N, 0);
     s->n_launch++;
     SPIN_CUDA(cudaGetLastError());
     return SPIN_OK;
@@ -733,10 +778,8 @@ extern "C" int effective_field_device(spin_system *s, double *B) {
     rc = enqueue_force(s, T_ALL, s->d_np);
     if (rc) return rc;
     // B = F / (mu_b mu_B), boundary order
-    double *d_scale = s->d_result + 8;
-    SPIN_CUDA(cudaMemcpyAsync(d_scale, s->plan.inv_mu, s->nb * sizeof(double), cudaMemcpyHostToDevice, s->stream));
     const int nt = 256;
-    unpack_kernel<<<(unsigned)((s->N + nt - 1) / nt), nt, 0, s->stream>>>(s->d_np, B, (int)s->N, s->nb, (int)s->ncell, s->stride, d_scale);
+    unpack_kernel<<<(unsigned)((s->N + nt - 1) / nt), nt, 0, s->stream>>>(s->plan, s->d_np, B, (int)s->N, 1);
     s->n_launch++;
     SPIN_CUDA(cudaGetLastError());
     return SPIN_OK;
@@ -815,7 +858,7 @@ extern "C" int spin_kernel_info(spin_system *s, char *buf, int len) {
 // needed) and the size of the cubin is returned in *cubin_bytes
 extern "C" int spin_jit_source(spin_system *s, char *buf, int len, int compile, int64_t *cubin_bytes) {
     REQUIRE(s, "null system");
-    int rc = build_plan(s);
+    int rc = build_plan(s, s->plan);
     if (rc) return rc;
     const std::string src = jit_source(s);
     if (buf && len > 0) snprintf(buf, (size_t)len, "%s", src.c_str());

@@ -75,16 +75,17 @@ __global__ void ddi_tensor_kernel(const __grid_constant__ DdiGeom G, int a, int 
 }
 
 // M_b padded <- mu_b n_b on the occupied corner (the rest of the array stays zero from allocation time)
-__global__ void ddi_scatter_kernel(const double *__restrict__ n, int stride, int Ncell, int Na, int Nb, int nb, int P0, int P1,
-                                   long long Ptot, const double *__restrict__ mu, double *__restrict__ Mpad) {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;   // internal index b*Ncell + cell
-    if (i >= nb * Ncell) return;
-    const int b = i / Ncell, cell = i - b * Ncell;
-    const int ia = cell % Na, ib = (cell / Na) % Nb, ic = cell / (Na * Nb);
+__global__ void ddi_scatter_kernel(const __grid_constant__ DevicePlan L, const double *__restrict__ n, int P0, int P1, long long Ptot,
+                                   const double *__restrict__ mu, double *__restrict__ Mpad) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;   // b*Ncell + cell, x fastest
+    if (i >= L.nb * L.Ncell) return;
+    const int b = i / L.Ncell, cell = i - b * L.Ncell;
+    const int ia = cell % L.Na, ib = (cell / L.Na) % L.Nb, ic = cell / (L.Na * L.Nb);
     const long long p = ia + (long long)P0 * (ib + (long long)P1 * ic);
+    const int j = b * L.sub + ((ic + L.LC) * L.PB + (ib + L.LB)) * (3 * L.PA) + (ia + L.LA);
     const double m = mu[b];
 #pragma unroll
-    for (int k = 0; k < 3; ++k) Mpad[(size_t)(b * 3 + k) * Ptot + p] = m * n[k * stride + i];
+    for (int k = 0; k < 3; ++k) Mpad[(size_t)(b * 3 + k) * Ptot + p] = m * n[j + k * L.PA];
 }
 
 // H^_a = sum_b K^_ab . M^_b  (symmetric 3x3 complex tensor from 6 stored components)
@@ -112,16 +113,17 @@ __global__ void ddi_contract_kernel(const cufftDoubleComplex *__restrict__ Khat,
 }
 
 // F_a(c) = mu_a C_dd / Ptot * H_a(c) on the occupied corner, written in the internal SoA layout
-__global__ void ddi_gather_kernel(const double *__restrict__ Hpad, int stride, int Ncell, int Na, int Nb, int nb, int P0, int P1,
-                                  long long Ptot, const double *__restrict__ mu, double scale, double *__restrict__ f) {
+__global__ void ddi_gather_kernel(const __grid_constant__ DevicePlan L, const double *__restrict__ Hpad, int P0, int P1, long long Ptot,
+                                  const double *__restrict__ mu, double scale, double *__restrict__ f) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= nb * Ncell) return;
-    const int b = i / Ncell, cell = i - b * Ncell;
-    const int ia = cell % Na, ib = (cell / Na) % Nb, ic = cell / (Na * Nb);
+    if (i >= L.nb * L.Ncell) return;
+    const int b = i / L.Ncell, cell = i - b * L.Ncell;
+    const int ia = cell % L.Na, ib = (cell / L.Na) % L.Nb, ic = cell / (L.Na * L.Nb);
     const long long p = ia + (long long)P0 * (ib + (long long)P1 * ic);
+    const int j = b * L.sub + ((ic + L.LC) * L.PB + (ib + L.LB)) * (3 * L.PA) + (ia + L.LA);
     const double m = mu[b] * scale;
 #pragma unroll
-    for (int k = 0; k < 3; ++k) f[k * stride + i] = m * Hpad[(size_t)(b * 3 + k) * Ptot + p];
+    for (int k = 0; k < 3; ++k) f[j + k * L.PA] = m * Hpad[(size_t)(b * 3 + k) * Ptot + p];
 }
 
 // rank-0 case (a single cell): the "transform" of one point is the point itself
@@ -213,8 +215,7 @@ int spin::ddi_field(spin_system *s, const double *d_n, double *d_f) {
     if (!d) return spin::fail(SPIN_ERR_STATE, "dipolar plan missing");
     const int nb = s->nb, Ncell = (int)s->ncell, nspin = nb * Ncell, nt = 256;
     const unsigned gs = (unsigned)((nspin + nt - 1) / nt);
-    ddi_scatter_kernel<<<gs, nt, 0, s->stream>>>(d_n, s->stride, Ncell, s->nc[0], s->nc[1], nb, d->P[0], d->P[1], (long long)d->Ptot,
-                                                  d->d_geom, d->d_Mpad);
+    ddi_scatter_kernel<<<gs, nt, 0, s->stream>>>(s->plan, d_n, d->P[0], d->P[1], (long long)d->Ptot, d->d_geom, d->d_Mpad);
     s->n_launch++;
     if (d->rank > 0) { SPIN_FFT(cufftExecD2Z(d->plan_r2c, d->d_Mpad, d->d_Mhat)); s->n_fft++; }
     else { real_to_complex_kernel<<<1, 32, 0, s->stream>>>(d->d_Mpad, d->d_Mhat, nb * 3); s->n_launch++; }
@@ -223,8 +224,8 @@ int spin::ddi_field(spin_system *s, const double *d_n, double *d_f) {
     s->n_launch++;
     if (d->rank > 0) { SPIN_FFT(cufftExecZ2D(d->plan_c2r, d->d_Hhat, d->d_Hpad)); s->n_fft++; }
     else { complex_to_real_kernel<<<1, 32, 0, s->stream>>>(d->d_Hhat, d->d_Hpad, nb * 3); s->n_launch++; }
-    ddi_gather_kernel<<<gs, nt, 0, s->stream>>>(d->d_Hpad, s->stride, Ncell, s->nc[0], s->nc[1], nb, d->P[0], d->P[1],
-                                                 (long long)d->Ptot, d->d_geom, C_DD / (double)d->Ptot, d_f);
+    ddi_gather_kernel<<<gs, nt, 0, s->stream>>>(s->plan, d->d_Hpad, d->P[0], d->P[1], (long long)d->Ptot, d->d_geom,
+                                                 C_DD / (double)d->Ptot, d_f);
     s->n_launch++;
     return SPIN_OK;
 }

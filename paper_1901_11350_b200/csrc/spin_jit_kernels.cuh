@@ -2,15 +2,17 @@
 //
 // The host planner (spin_jit.cu) prints the system as compile-time constants into `namespace spec` and then includes this
 // file.  Everything that the table-driven kernels (spin_kernels.cuh) look up at run time is a constant here:
-//   * lattice extents and boundary conditions  -> div/mod and periodic wrap by constants, open-edge tests only where needed
-//   * the gather table of every basis atom     -> fully unrolled, J and D folded into fma operands, zero D components dropped,
-//                                                 partner coordinates shared between entries by common-subexpression elimination
+//   * lattice extents, ghost-cell layout          -> div/mod by constants; every partner is `own address + immediate`
+//   * the gather table of every basis atom        -> fully unrolled, J and D folded into fma operands, zero D components dropped
 //   * LLG prefactors, time step, noise amplitude
+// Ghost cells (spinllg_internal.h "Layout") hold the periodic images or, at open edges, zeros, so the gather needs neither
+// wrap arithmetic nor edge tests; the writers of n^p and n(t+dt) also write the periodic images.
 // One thread per spin, bricks of BX x BY x BZ spins of one sublattice per block; no atomics, no shared memory.
 // Device-only: no host headers (NVRTC).  Formulas and paper citations: see spin_kernels.cuh / spin_device_math.cuh.
 //
 // namespace spec must define (all constexpr):
-//   int NA, NB, NC, NBASIS, NCELL, STRIDE, BX, BY, BZ;  bool PER_A, PER_B, PER_C, STORE_A, HAS_DDI, THERMAL_ON, STT_ON;
+//   int NA, NB, NC, NBASIS, BX, BY, BZ;  int LA, LB, LC, PA, PB, PC, SUB, RA, RB, RC;  bool GA, GB, GC, PER_A, PER_B, PER_C;
+//   bool STORE_A, HAS_DDI, THERMAL_ON, STT_ON;
 //   int PAIR_BEGIN[NBASIS+1], P_DA[], P_DB[], P_DC[], P_BJ[];  double P_J[], P_DX[], P_DY[], P_DZ[];
 //   int QUAD_BEGIN[NBASIS+1], Q_D[][9], Q_B[][3];  double Q_K[];
 //   double ZEE[NBASIS][3], K2[NBASIS], KAX[NBASIS][3], PRE[NBASIS], SIGMA[NBASIS];
@@ -36,47 +38,47 @@ __device__ __forceinline__ void static_for(F &&f) {
 
 struct Coord { int ia, ib, ic; };
 
-// coordinate i shifted by the compile-time translation D along a direction with N cells.  Periodic: wrapped (|D| <= N/2 by
-// construction of the table).  Open: `ok` is cleared when the partner is off the edge and the own coordinate is returned.
-template <int D, int N, bool PER>
-__device__ __forceinline__ int shift(int i, bool &ok) {
-    if constexpr (D == 0) {
-        return i;
-    } else if constexpr (PER) {
-        int j = i + D;
-        if constexpr (D > 0) { if (j >= N) j -= N; } else { if (j < 0) j += N; }
-        return j;
-    } else {
-        const int j = i + D;
-        const bool in = (D > 0) ? (j < N) : (j >= 0);
-        ok = ok && in;
-        return in ? j : i;
+constexpr int ROW = 3 * spec::PA;                 // doubles between consecutive lattice rows
+constexpr int PLANE = 3 * spec::PA * spec::PB;    // doubles between consecutive lattice planes
+
+// linear offset of the partner (sublattice BJ at translation DA, DB, DC) from a site of sublattice B
+template <int B, int BJ, int DA, int DB, int DC>
+__host__ __device__ constexpr int lin() {
+    return (BJ - B) * spec::SUB + DC * PLANE + DB * ROW + DA;
+}
+
+// q points at the x component of the own site; O is a compile-time offset in doubles
+template <int O>
+__device__ __forceinline__ void load3(const double *__restrict__ q, double (&v)[3]) {
+    v[0] = __ldg(q + O);
+    v[1] = __ldg(q + O + spec::PA);
+    v[2] = __ldg(q + O + 2 * spec::PA);
+}
+__device__ __forceinline__ void store3(double *__restrict__ q, const double (&v)[3]) {
+    q[0] = v[0]; q[spec::PA] = v[1]; q[2 * spec::PA] = v[2];
+}
+// a spin and its periodic images in the ghost layers (at most one image per direction)
+__device__ __forceinline__ void store_spin(double *__restrict__ q, const Coord &c, const double (&v)[3]) {
+    store3(q, v);
+    if constexpr (spec::GA || spec::GB || spec::GC) {
+        int sa = 0, sb = 0, sc = 0;
+        if constexpr (spec::GA) { if (c.ia < spec::RA) sa = spec::NA; else if (c.ia >= spec::NA - spec::RA) sa = -spec::NA; }
+        if constexpr (spec::GB) { if (c.ib < spec::RB) sb = spec::NB * ROW; else if (c.ib >= spec::NB - spec::RB) sb = -spec::NB * ROW; }
+        if constexpr (spec::GC) { if (c.ic < spec::RC) sc = spec::NC * PLANE; else if (c.ic >= spec::NC - spec::RC) sc = -spec::NC * PLANE; }
+        if (sa | sb | sc) {
+#pragma unroll
+            for (int m = 1; m < 8; ++m) {
+                if (((m & 1) && !sa) || ((m & 2) && !sb) || ((m & 4) && !sc)) continue;
+                store3(q + (((m & 1) ? sa : 0) + ((m & 2) ? sb : 0) + ((m & 4) ? sc : 0)), v);
+            }
+        }
     }
 }
 
-template <int DA, int DB, int DC, int BJ>
-__device__ __forceinline__ int partner(const Coord &c, bool &ok) {
-    const int ja = shift<DA, spec::NA, spec::PER_A>(c.ia, ok);
-    const int jb = shift<DB, spec::NB, spec::PER_B>(c.ib, ok);
-    const int jc = shift<DC, spec::NC, spec::PER_C>(c.ic, ok);
-    return BJ * spec::NCELL + ja + spec::NA * jb + (spec::NA * spec::NB) * jc;
-}
-
-template <int DA, int DB, int DC>
-__host__ __device__ constexpr bool always_inside() {
-    return (DA == 0 || spec::PER_A) && (DB == 0 || spec::PER_B) && (DC == 0 || spec::PER_C);
-}
-
-__device__ __forceinline__ void load3(const double *p, int j, double (&v)[3]) {
-    v[0] = __ldg(p + j);
-    v[1] = __ldg(p + spec::STRIDE + j);
-    v[2] = __ldg(p + 2 * spec::STRIDE + j);
-}
-
-// F += (Zeeman + anisotropy + pairs + quadruplets) of basis atom B for NCONF configurations sharing the lattice
+// F += (Zeeman + anisotropy + pairs + quadruplets) of basis atom B for NCONF configurations sharing the lattice;
+// cfg[k] points at the x component of the own site in configuration k
 template <int B, int NCONF>
-__device__ __forceinline__ void force(const double *const (&cfg)[NCONF], const Coord &c, const double (&own)[NCONF][3],
-                                      double (&F)[NCONF][3]) {
+__device__ __forceinline__ void force(const double *const (&cfg)[NCONF], const double (&own)[NCONF][3], double (&F)[NCONF][3]) {
 #pragma unroll
     for (int k = 0; k < NCONF; ++k) {
         if constexpr (spec::ZEE[B][0] != 0.0) F[k][0] += spec::ZEE[B][0];
@@ -96,17 +98,12 @@ __device__ __forceinline__ void force(const double *const (&cfg)[NCONF], const C
     }
     static_for<spec::PAIR_BEGIN[B], spec::PAIR_BEGIN[B + 1]>([&](auto e) {
         constexpr int E = decltype(e)::value;
-        constexpr int DA = spec::P_DA[E], DB = spec::P_DB[E], DC = spec::P_DC[E];
+        constexpr int O = lin<B, spec::P_BJ[E], spec::P_DA[E], spec::P_DB[E], spec::P_DC[E]>();
         constexpr double J = spec::P_J[E], Dx = spec::P_DX[E], Dy = spec::P_DY[E], Dz = spec::P_DZ[E];
-        bool ok = true;
-        const int j = partner<DA, DB, DC, spec::P_BJ[E]>(c, ok);
 #pragma unroll
         for (int k = 0; k < NCONF; ++k) {
             double p[3];
-            load3(cfg[k], j, p);
-            if constexpr (!always_inside<DA, DB, DC>()) {
-                if (!ok) { p[0] = 0.0; p[1] = 0.0; p[2] = 0.0; }
-            }
+            load3<O>(cfg[k], p);
             // J n_j + n_j x D, zero components dropped at compile time
             if constexpr (J != 0.0) { F[k][0] = fma(J, p[0], F[k][0]); F[k][1] = fma(J, p[1], F[k][1]); F[k][2] = fma(J, p[2], F[k][2]); }
             if constexpr (Dz != 0.0) { F[k][0] = fma(p[1], Dz, F[k][0]); F[k][1] = fma(p[0], -Dz, F[k][1]); }
@@ -116,39 +113,40 @@ __device__ __forceinline__ void force(const double *const (&cfg)[NCONF], const C
     });
     static_for<spec::QUAD_BEGIN[B], spec::QUAD_BEGIN[B + 1]>([&](auto e) {
         constexpr int E = decltype(e)::value;
-        bool ok = true;
-        const int jp = partner<spec::Q_D[E][0], spec::Q_D[E][1], spec::Q_D[E][2], spec::Q_B[E][0]>(c, ok);
-        const int jq = partner<spec::Q_D[E][3], spec::Q_D[E][4], spec::Q_D[E][5], spec::Q_B[E][1]>(c, ok);
-        const int jr = partner<spec::Q_D[E][6], spec::Q_D[E][7], spec::Q_D[E][8], spec::Q_B[E][2]>(c, ok);
-        constexpr bool inside = always_inside<spec::Q_D[E][0], spec::Q_D[E][1], spec::Q_D[E][2]>() &&
-                                always_inside<spec::Q_D[E][3], spec::Q_D[E][4], spec::Q_D[E][5]>() &&
-                                always_inside<spec::Q_D[E][6], spec::Q_D[E][7], spec::Q_D[E][8]>();
+        constexpr int OP = lin<B, spec::Q_B[E][0], spec::Q_D[E][0], spec::Q_D[E][1], spec::Q_D[E][2]>();
+        constexpr int OQ = lin<B, spec::Q_B[E][1], spec::Q_D[E][3], spec::Q_D[E][4], spec::Q_D[E][5]>();
+        constexpr int OR = lin<B, spec::Q_B[E][2], spec::Q_D[E][6], spec::Q_D[E][7], spec::Q_D[E][8]>();
 #pragma unroll
         for (int k = 0; k < NCONF; ++k) {
             double P[3], Q[3], R[3];
-            load3(cfg[k], jp, P); load3(cfg[k], jq, Q); load3(cfg[k], jr, R);
-            double w = spec::Q_K[E] * fma(Q[0], R[0], fma(Q[1], R[1], Q[2] * R[2]));
-            if constexpr (!inside) { if (!ok) w = 0.0; }
+            load3<OP>(cfg[k], P); load3<OQ>(cfg[k], Q); load3<OR>(cfg[k], R);
+            const double w = spec::Q_K[E] * fma(Q[0], R[0], fma(Q[1], R[1], Q[2] * R[2]));
             F[k][0] = fma(w, P[0], F[k][0]); F[k][1] = fma(w, P[1], F[k][1]); F[k][2] = fma(w, P[2], F[k][2]);
         }
     });
 }
 
 // (j^ . grad) n: central differences on the same sublattice, one-sided at open edges
-template <int B, int NCONF>
+template <int NCONF>
 __device__ __forceinline__ void stt_gradient(const double *const (&cfg)[NCONF], const Coord &c, const double (&own)[NCONF][3],
                                              double (&sg)[NCONF][3]) {
     static_for<0, 3>([&](auto dd) {
         constexpr int D = decltype(dd)::value;
         if constexpr (spec::STT_C[D] != 0.0) {
-            bool hp = true, hm = true;
-            const int jp = partner<(D == 0), (D == 1), (D == 2), B>(c, hp);
-            const int jm = partner<-(D == 0), -(D == 1), -(D == 2), B>(c, hm);
+            constexpr int STEP = D == 0 ? 1 : (D == 1 ? ROW : PLANE);
+            constexpr bool PER = D == 0 ? spec::PER_A : (D == 1 ? spec::PER_B : spec::PER_C);
+            constexpr int EXT = D == 0 ? spec::NA : (D == 1 ? spec::NB : spec::NC);
+            const int x = D == 0 ? c.ia : (D == 1 ? c.ib : c.ic);
+            const bool hp = PER || x + 1 < EXT, hm = PER || x > 0;
             const double w = spec::STT_C[D] * ((hp && hm) ? 0.5 : ((hp || hm) ? 1.0 : 0.0));
 #pragma unroll
             for (int k = 0; k < NCONF; ++k) {
                 double vp[3], vm[3];
-                load3(cfg[k], jp, vp); load3(cfg[k], jm, vm);      // off-edge partners alias the own site -> difference 0
+                load3<STEP>(cfg[k], vp); load3<-STEP>(cfg[k], vm);
+                if constexpr (!PER) {      // ghost cells of an open edge hold zeros: use the own spin for the one-sided difference
+                    if (!hp) { vp[0] = own[k][0]; vp[1] = own[k][1]; vp[2] = own[k][2]; }
+                    if (!hm) { vm[0] = own[k][0]; vm[1] = own[k][1]; vm[2] = own[k][2]; }
+                }
                 sg[k][0] = fma(w, vp[0] - vm[0], sg[k][0]); sg[k][1] = fma(w, vp[1] - vm[1], sg[k][1]); sg[k][2] = fma(w, vp[2] - vm[2], sg[k][2]);
             }
         }
@@ -171,7 +169,8 @@ __device__ __forceinline__ void rotation_field(const double (&n)[3], const doubl
     }
 }
 
-__device__ __forceinline__ bool locate(Coord &c, int &idx, int b) {
+template <int B>
+__device__ __forceinline__ bool locate(Coord &c, int &idx) {
     constexpr int nbx = (spec::NA + spec::BX - 1) / spec::BX, nby = (spec::NB + spec::BY - 1) / spec::BY;
     int brick = blockIdx.x;
     const int bx = brick % nbx;
@@ -181,7 +180,7 @@ __device__ __forceinline__ bool locate(Coord &c, int &idx, int b) {
     c.ia = bx * spec::BX + (t % spec::BX);
     c.ib = by * spec::BY + (t / spec::BX) % spec::BY;
     c.ic = bz * spec::BZ + t / (spec::BX * spec::BY);
-    idx = b * spec::NCELL + c.ia + spec::NA * c.ib + (spec::NA * spec::NB) * c.ic;
+    idx = B * spec::SUB + (c.ic + spec::LC) * PLANE + (c.ib + spec::LB) * ROW + (c.ia + spec::LA);
     return (c.ia < spec::NA) && (c.ib < spec::NB) && (c.ic < spec::NC);
 }
 
@@ -193,7 +192,7 @@ __device__ __forceinline__ void thermal_force(const Coord &c, u64 step, u32 seed
         spin::thermal_xi(seed_lo, seed_hi, step, (u32)B + (u32)spec::NBASIS * cell, xi);
         f[0] = spec::SIGMA[B] * xi[0]; f[1] = spec::SIGMA[B] * xi[1]; f[2] = spec::SIGMA[B] * xi[2];
     } else {
-        f[0] = 0.0; f[1] = 0.0; f[2] = 0.0;
+        f[0] = -0.0; f[1] = -0.0; f[2] = -0.0;      // additive identity that the compiler may fold away (x + -0.0 == x exactly)
     }
 }
 
@@ -202,19 +201,19 @@ __device__ __forceinline__ void predictor_body(const double *__restrict__ n, con
                                                double *__restrict__ Aout, u64 step, u32 seed_lo, u32 seed_hi) {
     Coord c;
     int idx;
-    if (!locate(c, idx, B)) return;
-    const double *const cfg[1] = {n};
+    if (!locate<B>(c, idx)) return;
+    const double *const cfg[1] = {n + idx};
     double own[1][3], F[1][3], sg[1][3] = {{0.0, 0.0, 0.0}};
-    load3(n, idx, own[0]);
+    load3<0>(cfg[0], own[0]);
     thermal_force<B>(c, step, seed_lo, seed_hi, F[0]);
-    force<B, 1>(cfg, c, own, F);
-    if constexpr (spec::HAS_DDI) { double d[3]; load3(fddi, idx, d); F[0][0] += d[0]; F[0][1] += d[1]; F[0][2] += d[2]; }
-    if constexpr (spec::STT_ON) stt_gradient<B, 1>(cfg, c, own, sg);
+    force<B, 1>(cfg, own, F);
+    if constexpr (spec::HAS_DDI) { double d[3]; load3<0>(fddi + idx, d); F[0][0] += d[0]; F[0][1] += d[1]; F[0][2] += d[2]; }
+    if constexpr (spec::STT_ON) stt_gradient<1>(cfg, c, own, sg);
     double A[3], out[3];
     rotation_field<B>(own[0], F[0], sg[0], A);
     spin::rodrigues(A, spec::DT, spec::DT2, own[0], out);
-    np[idx] = out[0]; np[spec::STRIDE + idx] = out[1]; np[2 * spec::STRIDE + idx] = out[2];
-    if constexpr (spec::STORE_A) { Aout[idx] = A[0]; Aout[spec::STRIDE + idx] = A[1]; Aout[2 * spec::STRIDE + idx] = A[2]; }
+    store_spin(np + idx, c, out);
+    if constexpr (spec::STORE_A) store3(Aout + idx, A);
 }
 
 template <int B>
@@ -223,31 +222,31 @@ __device__ __forceinline__ void corrector_body(const double *__restrict__ n, con
                                                u64 step, u32 seed_lo, u32 seed_hi) {
     Coord c;
     int idx;
-    if (!locate(c, idx, B)) return;
+    if (!locate<B>(c, idx)) return;
     double th[3], A[3], Ap[3], n0[3];
     thermal_force<B>(c, step, seed_lo, seed_hi, th);
-    load3(n, idx, n0);
+    load3<0>(n + idx, n0);
     if constexpr (spec::STORE_A) {
-        const double *const cfg[1] = {np};
+        const double *const cfg[1] = {np + idx};
         double own[1][3], F[1][3] = {{th[0], th[1], th[2]}}, sg[1][3] = {{0.0, 0.0, 0.0}};
-        load3(np, idx, own[0]);
-        force<B, 1>(cfg, c, own, F);
-        if constexpr (spec::HAS_DDI) { double d[3]; load3(fddi_np, idx, d); F[0][0] += d[0]; F[0][1] += d[1]; F[0][2] += d[2]; }
-        if constexpr (spec::STT_ON) stt_gradient<B, 1>(cfg, c, own, sg);
+        load3<0>(cfg[0], own[0]);
+        force<B, 1>(cfg, own, F);
+        if constexpr (spec::HAS_DDI) { double d[3]; load3<0>(fddi_np + idx, d); F[0][0] += d[0]; F[0][1] += d[1]; F[0][2] += d[2]; }
+        if constexpr (spec::STT_ON) stt_gradient<1>(cfg, c, own, sg);
         rotation_field<B>(own[0], F[0], sg[0], Ap);
-        load3(Ain, idx, A);
+        load3<0>(Ain + idx, A);
     } else {
-        const double *const cfg[2] = {n, np};
+        const double *const cfg[2] = {n + idx, np + idx};
         double own[2][3], F[2][3] = {{th[0], th[1], th[2]}, {th[0], th[1], th[2]}}, sg[2][3] = {{0.0, 0.0, 0.0}, {0.0, 0.0, 0.0}};
         own[0][0] = n0[0]; own[0][1] = n0[1]; own[0][2] = n0[2];
-        load3(np, idx, own[1]);
-        force<B, 2>(cfg, c, own, F);
+        load3<0>(cfg[1], own[1]);
+        force<B, 2>(cfg, own, F);
         if constexpr (spec::HAS_DDI) {
             double d[3];
-            load3(fddi_n, idx, d); F[0][0] += d[0]; F[0][1] += d[1]; F[0][2] += d[2];
-            load3(fddi_np, idx, d); F[1][0] += d[0]; F[1][1] += d[1]; F[1][2] += d[2];
+            load3<0>(fddi_n + idx, d); F[0][0] += d[0]; F[0][1] += d[1]; F[0][2] += d[2];
+            load3<0>(fddi_np + idx, d); F[1][0] += d[0]; F[1][1] += d[1]; F[1][2] += d[2];
         }
-        if constexpr (spec::STT_ON) stt_gradient<B, 2>(cfg, c, own, sg);
+        if constexpr (spec::STT_ON) stt_gradient<2>(cfg, c, own, sg);
         rotation_field<B>(own[0], F[0], sg[0], A);
         rotation_field<B>(own[1], F[1], sg[1], Ap);
     }
@@ -255,7 +254,7 @@ __device__ __forceinline__ void corrector_body(const double *__restrict__ n, con
     double out[3];
     spin::rodrigues(Ac, spec::DT, spec::DT2, n0, out);
     spin::renormalise(out);
-    nout[idx] = out[0]; nout[spec::STRIDE + idx] = out[1]; nout[2 * spec::STRIDE + idx] = out[2];
+    store_spin(nout + idx, c, out);
 }
 
 template <int B, class Fn>

@@ -1,9 +1,12 @@
-// spin_kernels.cuh -- device code of the LLG hot path (sm_100a, fp64).
+// spin_kernels.cuh -- table-driven device code of the LLG hot path (sm_100a, fp64).
 //
-// One thread per spin; each spin GATHERS its own pair / quadruplet contributions (no atomics).  Thread blocks
-// map to 3-D bricks of one sublattice so that the neighbours of a brick stay in L1/L2.  Interaction tables
-// travel as a __grid_constant__ kernel parameter (constant bank), periodic-image index arithmetic is done
-// in registers and skipped entirely for bricks that touch no boundary.
+// One thread per spin; each spin GATHERS its own pair / quadruplet contributions (no atomics).  Thread blocks map to
+// 3-D bricks of one sublattice.  Interaction tables travel as a __grid_constant__ kernel parameter (constant bank).
+// The spin arrays carry ghost cells (spinllg_internal.h "Layout"), so a partner is always at `own index + constant`:
+// no periodic-wrap arithmetic and no open-edge tests in the gather (ghosts of open edges hold zeros, which contribute
+// exactly nothing to J n_j + n_j x D or K (n_Q.n_R) n_P).  Writers of a spin array also write its periodic images.
+// These kernels serve every system; the two sweeps are normally replaced by their run-time specialised versions
+// (spin_jit_kernels.cuh), the reductions / force / pack kernels below are always the ones in use.
 //
 // Formulas (PAPER.md line numbers):
 //   force      F_i = -dH/dn_i of Eq. 1 (:61-67) and Eq. 2 (:75), ":155 B_eff = -dH/dn_i"
@@ -19,10 +22,13 @@ namespace spin {
 
 struct Site {
     int ia, ib, ic, b;
-    int idx;          // internal SoA index  b*Ncell + cell
+    int idx;          // index of the x component in the padded layout; y, z at +PA, +2 PA
     bool valid;
-    bool interior;    // the whole brick is at least `reach` away from every boundary
 };
+
+__device__ __forceinline__ int site_index(const DevicePlan &P, int b, int ia, int ib, int ic) {
+    return b * P.sub + ((ic + P.LC) * P.PB + (ib + P.LB)) * (3 * P.PA) + (ia + P.LA);
+}
 
 template <int BX, int BY, int BZ>
 __device__ __forceinline__ Site locate(const DevicePlan &P) {
@@ -33,42 +39,43 @@ __device__ __forceinline__ Site locate(const DevicePlan &P) {
     brick /= nbx;
     const int by = brick % nby, bz = brick / nby;
     const int t = threadIdx.x;
-    const int x0 = bx * BX, y0 = by * BY, z0 = bz * BZ;
-    s.ia = x0 + (t % BX);
-    s.ib = y0 + (t / BX) % BY;
-    s.ic = z0 + t / (BX * BY);
+    s.ia = bx * BX + (t % BX);
+    s.ib = by * BY + (t / BX) % BY;
+    s.ic = bz * BZ + t / (BX * BY);
     s.b = blockIdx.y;
     s.valid = (s.ia < P.Na) && (s.ib < P.Nb) && (s.ic < P.Nc);
-    s.idx = s.b * P.Ncell + s.ia + P.Na * (s.ib + P.Nb * s.ic);
-    s.interior = (x0 >= P.reach[0]) && (x0 + BX + P.reach[0] <= P.Na) && (y0 >= P.reach[1]) &&
-                 (y0 + BY + P.reach[1] <= P.Nb) && (z0 >= P.reach[2]) && (z0 + BZ + P.reach[2] <= P.Nc);
+    s.idx = site_index(P, s.b, s.ia, s.ib, s.ic);
     return s;
 }
 
-// partner index with boundary conditions; returns false when the partner falls off an open edge
-__device__ __forceinline__ bool partner(const DevicePlan &P, const Site &s, int da, int db, int dc, int bj, int lin,
-                                        int &idx) {
-    if (s.interior) {
-        idx = s.idx + lin;
-        return true;
+__device__ __forceinline__ void load3(const DevicePlan &P, const double *__restrict__ a, int idx, double (&v)[3]) {
+    v[0] = __ldg(a + idx); v[1] = __ldg(a + idx + P.PA); v[2] = __ldg(a + idx + 2 * P.PA);
+}
+__device__ __forceinline__ void store3(const DevicePlan &P, double *__restrict__ a, int idx, const double (&v)[3]) {
+    a[idx] = v[0]; a[idx + P.PA] = v[1]; a[idx + 2 * P.PA] = v[2];
+}
+// store a spin and its periodic images in the ghost layers (at most one image per direction)
+__device__ __forceinline__ void store_spin(const DevicePlan &P, double *__restrict__ a, int ia, int ib, int ic, int idx, const double (&v)[3]) {
+    store3(P, a, idx, v);
+    int sa = 0, sb = 0, sc = 0;
+    if (P.gA) { if (ia < P.rA) sa = P.Na; else if (ia >= P.Na - P.rA) sa = -P.Na; }
+    if (P.gB) { if (ib < P.rB) sb = P.Nb; else if (ib >= P.Nb - P.rB) sb = -P.Nb; }
+    if (P.gC) { if (ic < P.rC) sc = P.Nc; else if (ic >= P.Nc - P.rC) sc = -P.Nc; }
+    if (sa | sb | sc) {
+        for (int m = 1; m < 8; ++m) {
+            if (((m & 1) && !sa) || ((m & 2) && !sb) || ((m & 4) && !sc)) continue;
+            const int off = ((m & 1) ? sa : 0) + 3 * P.PA * (((m & 2) ? sb : 0) + P.PB * ((m & 4) ? sc : 0));
+            store3(P, a, idx + off, v);
+        }
     }
-    int ja = s.ia + da, jb = s.ib + db, jc = s.ic + dc;
-    bool ok = true;
-    if (ja < 0) { ja += P.Na; ok = ok && P.perA; } else if (ja >= P.Na) { ja -= P.Na; ok = ok && P.perA; }
-    if (jb < 0) { jb += P.Nb; ok = ok && P.perB; } else if (jb >= P.Nb) { jb -= P.Nb; ok = ok && P.perB; }
-    if (jc < 0) { jc += P.Nc; ok = ok && P.perC; } else if (jc >= P.Nc) { jc -= P.Nc; ok = ok && P.perC; }
-    idx = ok ? bj * P.Ncell + ja + P.Na * (jb + P.Nb * jc) : s.idx;
-    return ok;
 }
 
 // ---------------------------------------------------------------------------------------------------------
-// Short-range force of NCONF configurations that share the lattice (n and n^p in the corrector): the partner
-// index is computed once per table entry and used for every configuration.
-// cfg[c] points at the x component; y and z follow at +stride, +2*stride.
+// Short-range force of NCONF configurations that share the lattice (n and n^p in the corrector).
 template <int NCONF>
 __device__ __forceinline__ void short_range_force(const DevicePlan &P, const double *const (&cfg)[NCONF], const Site &s,
                                                   const double (&own)[NCONF][3], int mask, double (&F)[NCONF][3]) {
-    const int b = s.b, st = P.stride;
+    const int b = s.b;
     if (mask & T_ZEE) {
 #pragma unroll
         for (int c = 0; c < NCONF; ++c) { F[c][0] += P.zee[b][0]; F[c][1] += P.zee[b][1]; F[c][2] += P.zee[b][2]; }
@@ -83,36 +90,30 @@ __device__ __forceinline__ void short_range_force(const DevicePlan &P, const dou
     }
     if (mask & (T_EXC | T_DMI)) {
         const double wj = (mask & T_EXC) ? 1.0 : 0.0, wd = (mask & T_DMI) ? 1.0 : 0.0;
-        const bool all = (mask & T_EXC) && (mask & T_DMI);
         for (int e = P.pair_begin[b]; e < P.pair_begin[b + 1]; ++e) {
             const PairEntry &pe = P.pairs[e];
-            int j;
-            if (!partner(P, s, pe.da, pe.db, pe.dc, pe.bj, pe.lin, j)) continue;
-            const double J = all ? pe.J : wj * pe.J;
-            const double Dx = all ? pe.Dx : wd * pe.Dx, Dy = all ? pe.Dy : wd * pe.Dy, Dz = all ? pe.Dz : wd * pe.Dz;
+            const int j = s.idx + pe.lin;
+            const double J = wj * pe.J, Dx = wd * pe.Dx, Dy = wd * pe.Dy, Dz = wd * pe.Dz;
 #pragma unroll
             for (int c = 0; c < NCONF; ++c) {
-                const double px = __ldg(cfg[c] + j), py = __ldg(cfg[c] + st + j), pz = __ldg(cfg[c] + 2 * st + j);
+                double p[3];
+                load3(P, cfg[c], j, p);
                 // J n_j + n_j x D
-                F[c][0] += J * px + (py * Dz - pz * Dy);
-                F[c][1] += J * py + (pz * Dx - px * Dz);
-                F[c][2] += J * pz + (px * Dy - py * Dx);
+                F[c][0] += J * p[0] + (p[1] * Dz - p[2] * Dy);
+                F[c][1] += J * p[1] + (p[2] * Dx - p[0] * Dz);
+                F[c][2] += J * p[2] + (p[0] * Dy - p[1] * Dx);
             }
         }
     }
     if (mask & T_QUAD) {
         for (int e = P.quad_begin[b]; e < P.quad_begin[b + 1]; ++e) {
             const QuadEntry &q = P.quads[e];
-            int jp, jq, jr;
-            bool ok = partner(P, s, q.d[0][0], q.d[0][1], q.d[0][2], q.b[0], q.lin[0], jp);
-            ok = partner(P, s, q.d[1][0], q.d[1][1], q.d[1][2], q.b[1], q.lin[1], jq) && ok;
-            ok = partner(P, s, q.d[2][0], q.d[2][1], q.d[2][2], q.b[2], q.lin[2], jr) && ok;
-            if (!ok) continue;
 #pragma unroll
             for (int c = 0; c < NCONF; ++c) {
-                const double *x = cfg[c], *y = cfg[c] + st, *z = cfg[c] + 2 * st;
-                const double w = q.K * (__ldg(x + jq) * __ldg(x + jr) + __ldg(y + jq) * __ldg(y + jr) + __ldg(z + jq) * __ldg(z + jr));
-                F[c][0] += w * __ldg(x + jp); F[c][1] += w * __ldg(y + jp); F[c][2] += w * __ldg(z + jp);
+                double pp[3], pq[3], pr[3];
+                load3(P, cfg[c], s.idx + q.lin[0], pp); load3(P, cfg[c], s.idx + q.lin[1], pq); load3(P, cfg[c], s.idx + q.lin[2], pr);
+                const double w = q.K * (pq[0] * pr[0] + pq[1] * pr[1] + pq[2] * pr[2]);
+                F[c][0] += w * pp[0]; F[c][1] += w * pp[1]; F[c][2] += w * pp[2];
             }
         }
     }
@@ -122,23 +123,20 @@ __device__ __forceinline__ void short_range_force(const DevicePlan &P, const dou
 template <int NCONF>
 __device__ __forceinline__ void stt_gradient(const DevicePlan &P, const double *const (&cfg)[NCONF], const Site &s,
                                              const double (&own)[NCONF][3], double (&sg)[NCONF][3]) {
-    const int st = P.stride;
+    const int coord[3] = {s.ia, s.ib, s.ic}, ext[3] = {P.Na, P.Nb, P.Nc}, per[3] = {P.perA, P.perB, P.perC};
+    const int step[3] = {1, 3 * P.PA, 3 * P.PA * P.PB};
 #pragma unroll
     for (int d = 0; d < 3; ++d) {
         const double cd = P.stt_c[d];
         if (cd == 0.0) continue;
-        int jp, jm;
-        const bool hp = partner(P, s, d == 0, d == 1, d == 2, s.b, d == 0 ? 1 : (d == 1 ? P.Na : P.Na * P.Nb), jp);
-        const bool hm = partner(P, s, -(d == 0), -(d == 1), -(d == 2), s.b, d == 0 ? -1 : (d == 1 ? -P.Na : -P.Na * P.Nb), jm);
+        const bool hp = per[d] || coord[d] + 1 < ext[d], hm = per[d] || coord[d] > 0;
         const double w = cd * ((hp && hm) ? 0.5 : ((hp || hm) ? 1.0 : 0.0));
 #pragma unroll
         for (int c = 0; c < NCONF; ++c) {
-#pragma unroll
-            for (int k = 0; k < 3; ++k) {
-                const double vp = hp ? __ldg(cfg[c] + k * st + jp) : own[c][k];
-                const double vm = hm ? __ldg(cfg[c] + k * st + jm) : own[c][k];
-                sg[c][k] += w * (vp - vm);
-            }
+            double vp[3] = {own[c][0], own[c][1], own[c][2]}, vm[3] = {own[c][0], own[c][1], own[c][2]};
+            if (hp) load3(P, cfg[c], s.idx + step[d], vp);
+            if (hm) load3(P, cfg[c], s.idx - step[d], vm);
+            sg[c][0] += w * (vp[0] - vm[0]); sg[c][1] += w * (vp[1] - vm[1]); sg[c][2] += w * (vp[2] - vm[2]);
         }
     }
 }
@@ -160,6 +158,16 @@ __device__ __forceinline__ void rotation_field(const DevicePlan &P, int b, const
     }
 }
 
+__device__ __forceinline__ void thermal_force(const DevicePlan &P, const Site &s, unsigned long long step, double (&f)[3]) {
+    f[0] = 0.0; f[1] = 0.0; f[2] = 0.0;
+    if (P.thermal_on) {
+        const unsigned int cell = (unsigned int)(s.ia + P.Na * (s.ib + P.Nb * s.ic));
+        thermal_xi(P.seed_lo, P.seed_hi, step, (unsigned int)s.b + (unsigned int)P.nb * cell, f);
+        const double sg = P.sigma[s.b];
+        f[0] *= sg; f[1] *= sg; f[2] *= sg;
+    }
+}
+
 // ---------------------------------------------------------------------------------------------------------
 // Sweep 1 (B5): n -> n^p.  Reads n (own + gathered neighbours), optional dipolar force of n; writes n^p and,
 // with STORE_A, the rotation field A.
@@ -170,25 +178,18 @@ __global__ void __launch_bounds__(BX *BY *BZ)
                      unsigned int step_add) {
     const Site s = locate<BX, BY, BZ>(P);
     if (!s.valid) return;
-    const int st = P.stride;
     const double *const cfg[1] = {n};
-    const double own[1][3] = {{n[s.idx], n[st + s.idx], n[2 * st + s.idx]}};
-    double F[1][3] = {{0.0, 0.0, 0.0}};
+    double own[1][3], F[1][3], sg[1][3] = {{0.0, 0.0, 0.0}};
+    load3(P, n, s.idx, own[0]);
+    thermal_force(P, s, *d_step + step_add, F[0]);
     short_range_force<1>(P, cfg, s, own, T_ALL, F);
-    if (P.has_ddi) { F[0][0] += fddi[s.idx]; F[0][1] += fddi[st + s.idx]; F[0][2] += fddi[2 * st + s.idx]; }
-    if (P.thermal_on) {
-        double xi[3];
-        thermal_xi(P.seed_lo, P.seed_hi, *d_step + step_add, (uint32_t)(s.b + P.nb * (s.idx - s.b * P.Ncell)), xi);
-        const double sg = P.sigma[s.b];
-        F[0][0] += sg * xi[0]; F[0][1] += sg * xi[1]; F[0][2] += sg * xi[2];
-    }
-    double sg[1][3] = {{0.0, 0.0, 0.0}};
+    if (P.has_ddi) { double d[3]; load3(P, fddi, s.idx, d); F[0][0] += d[0]; F[0][1] += d[1]; F[0][2] += d[2]; }
     if (P.stt_on) stt_gradient<1>(P, cfg, s, own, sg);
     double A[3], out[3];
     rotation_field(P, s.b, own[0], F[0], sg[0], A);
     rodrigues(A, P.dt, P.dt2, own[0], out);
-    np[s.idx] = out[0]; np[st + s.idx] = out[1]; np[2 * st + s.idx] = out[2];
-    if (STORE_A) { Aout[s.idx] = A[0]; Aout[st + s.idx] = A[1]; Aout[2 * st + s.idx] = A[2]; }
+    store_spin(P, np, s.ia, s.ib, s.ic, s.idx, out);
+    if (STORE_A) store3(P, Aout, s.idx, A);
 }
 
 // Sweep 2 (B6, B7): A^p = A(n^p) with the same thermal field, A^c = (A + A^p)/2, n(t+dt) = R(A^c) n(t), renormalise.
@@ -200,35 +201,29 @@ __global__ void __launch_bounds__(BX *BY *BZ)
                      double *__restrict__ nout, const unsigned long long *__restrict__ d_step, unsigned int step_add) {
     const Site s = locate<BX, BY, BZ>(P);
     if (!s.valid) return;
-    const int st = P.stride;
-    double xi[3] = {0.0, 0.0, 0.0};
-    if (P.thermal_on) {
-        thermal_xi(P.seed_lo, P.seed_hi, *d_step + step_add, (uint32_t)(s.b + P.nb * (s.idx - s.b * P.Ncell)), xi);
-        const double sg = P.sigma[s.b];
-        xi[0] *= sg; xi[1] *= sg; xi[2] *= sg;
-    }
-    double A[3], Ap[3];
-    const double n0[3] = {n[s.idx], n[st + s.idx], n[2 * st + s.idx]};
+    double th[3], A[3], Ap[3], n0[3];
+    thermal_force(P, s, *d_step + step_add, th);
+    load3(P, n, s.idx, n0);
     if (STORE_A) {
         const double *const cfg[1] = {np};
-        const double own[1][3] = {{np[s.idx], np[st + s.idx], np[2 * st + s.idx]}};
-        double F[1][3] = {{xi[0], xi[1], xi[2]}};
+        double own[1][3], F[1][3] = {{th[0], th[1], th[2]}}, sg[1][3] = {{0.0, 0.0, 0.0}};
+        load3(P, np, s.idx, own[0]);
         short_range_force<1>(P, cfg, s, own, T_ALL, F);
-        if (P.has_ddi) { F[0][0] += fddi_np[s.idx]; F[0][1] += fddi_np[st + s.idx]; F[0][2] += fddi_np[2 * st + s.idx]; }
-        double sg[1][3] = {{0.0, 0.0, 0.0}};
+        if (P.has_ddi) { double d[3]; load3(P, fddi_np, s.idx, d); F[0][0] += d[0]; F[0][1] += d[1]; F[0][2] += d[2]; }
         if (P.stt_on) stt_gradient<1>(P, cfg, s, own, sg);
         rotation_field(P, s.b, own[0], F[0], sg[0], Ap);
-        A[0] = Ain[s.idx]; A[1] = Ain[st + s.idx]; A[2] = Ain[2 * st + s.idx];
+        load3(P, Ain, s.idx, A);
     } else {
         const double *const cfg[2] = {n, np};
-        const double own[2][3] = {{n0[0], n0[1], n0[2]}, {np[s.idx], np[st + s.idx], np[2 * st + s.idx]}};
-        double F[2][3] = {{xi[0], xi[1], xi[2]}, {xi[0], xi[1], xi[2]}};
+        double own[2][3], F[2][3] = {{th[0], th[1], th[2]}, {th[0], th[1], th[2]}}, sg[2][3] = {{0.0, 0.0, 0.0}, {0.0, 0.0, 0.0}};
+        own[0][0] = n0[0]; own[0][1] = n0[1]; own[0][2] = n0[2];
+        load3(P, np, s.idx, own[1]);
         short_range_force<2>(P, cfg, s, own, T_ALL, F);
         if (P.has_ddi) {
-            F[0][0] += fddi_n[s.idx]; F[0][1] += fddi_n[st + s.idx]; F[0][2] += fddi_n[2 * st + s.idx];
-            F[1][0] += fddi_np[s.idx]; F[1][1] += fddi_np[st + s.idx]; F[1][2] += fddi_np[2 * st + s.idx];
+            double d[3];
+            load3(P, fddi_n, s.idx, d); F[0][0] += d[0]; F[0][1] += d[1]; F[0][2] += d[2];
+            load3(P, fddi_np, s.idx, d); F[1][0] += d[0]; F[1][1] += d[1]; F[1][2] += d[2];
         }
-        double sg[2][3] = {{0.0, 0.0, 0.0}, {0.0, 0.0, 0.0}};
         if (P.stt_on) stt_gradient<2>(P, cfg, s, own, sg);
         rotation_field(P, s.b, own[0], F[0], sg[0], A);
         rotation_field(P, s.b, own[1], F[1], sg[1], Ap);
@@ -237,13 +232,20 @@ __global__ void __launch_bounds__(BX *BY *BZ)
     double out[3];
     rodrigues(Ac, P.dt, P.dt2, n0, out);
     renormalise(out);
-    nout[s.idx] = out[0]; nout[st + s.idx] = out[1]; nout[2 * st + s.idx] = out[2];
+    store_spin(P, nout, s.ia, s.ib, s.ic, s.idx, out);
 }
 
 // ---------------------------------------------------------------------------------------------------------
-// Boundary order (AoS, basis fastest) <-> internal order (SoA, sublattice-major)
-__global__ void pack_kernel(const double *__restrict__ aos, double *__restrict__ soa, int N, int nb, int Ncell, int stride, int normalise, int *bad) {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;   // boundary index
+// Boundary order (AoS, basis fastest) <-> internal padded layout.  One thread per spin in boundary order.
+__device__ __forceinline__ void boundary_to_site(const DevicePlan &P, int i, int &b, int &ia, int &ib, int &ic, int &idx) {
+    b = i % P.nb;
+    const int cell = i / P.nb;
+    ia = cell % P.Na; ib = (cell / P.Na) % P.Nb; ic = cell / (P.Na * P.Nb);
+    idx = site_index(P, b, ia, ib, ic);
+}
+__global__ void pack_kernel(const __grid_constant__ DevicePlan P, const double *__restrict__ aos, double *__restrict__ dst, int N,
+                            int normalise, int *bad) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= N) return;
     double v[3] = {aos[3 * (size_t)i], aos[3 * (size_t)i + 1], aos[3 * (size_t)i + 2]};
     if (normalise) {
@@ -251,32 +253,35 @@ __global__ void pack_kernel(const double *__restrict__ aos, double *__restrict__
         if (!(r2 > 0.0) || !isfinite(r2)) { atomicExch(bad, 1); v[0] = 0; v[1] = 0; v[2] = 1; }
         else { const double r = sqrt(r2); v[0] /= r; v[1] /= r; v[2] /= r; }
     }
-    const int b = i % nb, cell = i / nb, j = b * Ncell + cell;
-    soa[j] = v[0]; soa[stride + j] = v[1]; soa[2 * stride + j] = v[2];
+    int b, ia, ib, ic, idx;
+    boundary_to_site(P, i, b, ia, ib, ic, idx);
+    store_spin(P, dst, ia, ib, ic, idx, v);
 }
-__global__ void unpack_kernel(const double *__restrict__ soa, double *__restrict__ aos, int N, int nb, int Ncell, int stride,
-                              const double *__restrict__ scale /*per sublattice or null*/) {
+__global__ void unpack_kernel(const __grid_constant__ DevicePlan P, const double *__restrict__ src, double *__restrict__ aos, int N,
+                              int scale_by_inv_mu) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= N) return;
-    const int b = i % nb, cell = i / nb, j = b * Ncell + cell;
-    const double sc = scale ? scale[b] : 1.0;
-    aos[3 * (size_t)i] = sc * soa[j]; aos[3 * (size_t)i + 1] = sc * soa[stride + j]; aos[3 * (size_t)i + 2] = sc * soa[2 * stride + j];
+    int b, ia, ib, ic, idx;
+    boundary_to_site(P, i, b, ia, ib, ic, idx);
+    double v[3];
+    load3(P, src, idx, v);
+    const double sc = scale_by_inv_mu ? P.inv_mu[b] : 1.0;
+    aos[3 * (size_t)i] = sc * v[0]; aos[3 * (size_t)i + 1] = sc * v[1]; aos[3 * (size_t)i + 2] = sc * v[2];
 }
 
-// deterministic force F (meV, SoA) of the current configuration: all terms of the mask (+ dipolar array if given)
+// deterministic force F (meV, padded layout) of the current configuration: all terms of the mask (+ dipolar array if given)
 template <int BX, int BY, int BZ>
 __global__ void __launch_bounds__(BX *BY *BZ)
     force_kernel(const __grid_constant__ DevicePlan P, const double *__restrict__ n, const double *__restrict__ fddi, int mask,
                  double *__restrict__ Fout) {
     const Site s = locate<BX, BY, BZ>(P);
     if (!s.valid) return;
-    const int st = P.stride;
     const double *const cfg[1] = {n};
-    const double own[1][3] = {{n[s.idx], n[st + s.idx], n[2 * st + s.idx]}};
-    double F[1][3] = {{0.0, 0.0, 0.0}};
+    double own[1][3], F[1][3] = {{0.0, 0.0, 0.0}};
+    load3(P, n, s.idx, own[0]);
     short_range_force<1>(P, cfg, s, own, mask, F);
-    if ((mask & T_DDI) && P.has_ddi) { F[0][0] += fddi[s.idx]; F[0][1] += fddi[st + s.idx]; F[0][2] += fddi[2 * st + s.idx]; }
-    Fout[s.idx] = F[0][0]; Fout[st + s.idx] = F[0][1]; Fout[2 * st + s.idx] = F[0][2];
+    if ((mask & T_DDI) && P.has_ddi) { double d[3]; load3(P, fddi, s.idx, d); F[0][0] += d[0]; F[0][1] += d[1]; F[0][2] += d[2]; }
+    store3(P, Fout, s.idx, F[0]);
 }
 
 // ---------------------------------------------------------------------------------------------------------
@@ -307,9 +312,9 @@ __global__ void __launch_bounds__(BX *BY *BZ)
 #pragma unroll
     for (int k = 0; k < N_RED; ++k) v[k] = 0.0;
     if (s.valid) {
-        const int st = P.stride;
         const double *const cfg[1] = {n};
-        const double own[1][3] = {{n[s.idx], n[st + s.idx], n[2 * st + s.idx]}};
+        double own[1][3];
+        load3(P, n, s.idx, own[0]);
         double Ft[3] = {0.0, 0.0, 0.0};
         const int masks[5] = {T_ZEE, T_ANI, T_EXC, T_DMI, T_QUAD};
         const double inv_k[5] = {1.0, 0.5, 0.5, 0.5, 0.25};
@@ -321,9 +326,10 @@ __global__ void __launch_bounds__(BX *BY *BZ)
             Ft[0] += F[0][0]; Ft[1] += F[0][1]; Ft[2] += F[0][2];
         }
         if (P.has_ddi) {
-            const double fx = fddi[s.idx], fy = fddi[st + s.idx], fz = fddi[2 * st + s.idx];
-            v[5] = -0.5 * (own[0][0] * fx + own[0][1] * fy + own[0][2] * fz);
-            Ft[0] += fx; Ft[1] += fy; Ft[2] += fz;
+            double f[3];
+            load3(P, fddi, s.idx, f);
+            v[5] = -0.5 * (own[0][0] * f[0] + own[0][1] * f[1] + own[0][2] * f[2]);
+            Ft[0] += f[0]; Ft[1] += f[1]; Ft[2] += f[2];
         }
         v[6] = own[0][0]; v[7] = own[0][1]; v[8] = own[0][2];
         const double p = Ft[0] * own[0][0] + Ft[1] * own[0][1] + Ft[2] * own[0][2];

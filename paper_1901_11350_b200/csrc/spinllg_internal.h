@@ -1,8 +1,9 @@
 // spinllg_internal.h -- private definitions of the B200 LLG library (not part of the C-ABI).
 //
 // Layout in HBM: spins are kept structure-of-arrays and sublattice-major,
-//     n[comp * stride + b * Ncell + (ia + Na*(ib + Nb*ic))],   comp in {x,y,z}
-// so that a warp reads 32 consecutive doubles of one component of one sublattice (256 B, two full lines).
+//     n[b*sub + ((ic+LC)*PB + (ib+LB)) * 3*PA + comp*PA + (ia+LA)],   comp in {x,y,z}      (see DevicePlan)
+// so that a warp reads 32 consecutive doubles of one component of one lattice row (256 B, two full lines), the three
+// components of a row are adjacent, and ghost cells make every neighbour a constant offset from the own site.
 // The boundary order (AoS, basis fastest; include/spinllg.h) is converted by pack/unpack kernels.
 #pragma once
 
@@ -53,8 +54,17 @@ struct DevicePlan {
     int perA, perB, perC;
     int nb;
     int Ncell;
-    int stride;                              // component stride of the SoA arrays (doubles)
-    int reach[3];                            // max |translation| per direction over all entries (interior test)
+    // ---- Layout of every per-spin array (n, n^p, A, dipolar force), in doubles:
+    //   index(b, ia, ib, ic, comp) = b*sub + ((ic+LC)*PB + (ib+LB)) * 3*PA + comp*PA + (ia+LA)
+    // i.e. sublattice-major, then rows of the padded lattice, each row holding its x, y and z components as three
+    // consecutive runs of PA doubles (component offset PA*8 bytes: an immediate in the load instruction).
+    // rA/rB/rC ghost cells on each side hold the periodic images (gA/gB/gC = 1) or zeros (open edges).
+    // LA and PA are multiples of 16 doubles so that every run starts on a 128-byte line.
+    int LA, LB, LC;
+    int PA, PB, PC;
+    int sub;                                 // 3*PA*PB*PC
+    int rA, rB, rC;                          // ghost width = max |translation| per direction over all table entries
+    int gA, gB, gC;                          // periodic images to maintain in that direction
     int pair_begin[SPIN_MAX_BASIS + 1];
     int quad_begin[SPIN_MAX_BASIS + 1];
     double zee[SPIN_MAX_BASIS][3];           // mu_b mu_B B            (meV)
@@ -91,7 +101,6 @@ struct spin_system {
     int nc[3], per[3];
     double alat;
     int64_t ncell, N;
-    int stride;
     // ---- Hamiltonian (host description)
     std::vector<double> mu;        // nb
     double Bmag, Bdir[3];
@@ -104,11 +113,11 @@ struct spin_system {
     uint64_t seed, step;
     // ---- device
     cudaStream_t stream, own_stream;
-    double *d_n[2];                // ping-pong spin buffers (3*stride each)
+    double *d_n[2];                // ping-pong spin buffers (nb*sub doubles each)
     int cur;
     double *d_np;                  // predictor
     double *d_A;                   // rotation field of the predictor stage (store_A option)
-    double *d_fddi[2];             // dipolar force of n and of n^p (3*stride each), only with DDI
+    double *d_fddi[2];             // dipolar force of n and of n^p (nb*sub doubles each), only with DDI
     double *d_aos;                 // staging buffer, boundary order (3N)
     double *d_partials;            // reduction scratch
     double *d_result;              // reduction result (16 doubles)
