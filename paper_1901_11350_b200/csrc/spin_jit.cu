@@ -5,11 +5,14 @@
 // cubin is loaded through the runtime's library API.  The result is cached per system and rebuilt when the plan changes.
 // If NVRTC is unavailable or compilation fails the system keeps using the table-driven kernels and records why
 // (spin_kernel_info reports which path is active; nothing is silently computed on the CPU either way).
+#include <cuda.h>
 #include <dlfcn.h>
 #include <nvrtc.h>
+#include <stdlib.h>
 #include <stdio.h>
 #include <string.h>
 
+#include <algorithm>
 #include <sstream>
 #include <string>
 
@@ -17,11 +20,27 @@
 
 using namespace spin;
 
+// staging geometry of one TMA-fed sweep (spin_jit_tma.cuh): tile, ring depth, look-ahead, chunks along c
+struct TmaGeo {
+    int tbx, tby, ring, look, nzc, cz;
+    int narr;                 // arrays staged per plane (predictor 1, corrector 2)
+    size_t smem_bytes;
+    int items;
+};
+
 struct JitState {
     cudaLibrary_t lib;
     cudaKernel_t k_pred, k_corr;
     bool loaded;
     std::string source, log;
+    // TMA-fed plane-marching sweeps
+    bool tma;                 // generated and loaded
+    std::string tma_note;     // why not, if not
+    TmaGeo gp, gc;
+    cudaKernel_t k_pred_tma, k_corr_tma;
+    int grid_p, grid_c;
+    CUtensorMap tm_n[2];              // predictor: n[cur] with the predictor tile
+    CUtensorMap tm_cn[2], tm_cnp;     // corrector: n[cur], n^p with the corrector tile
 };
 
 namespace {
@@ -52,6 +71,72 @@ void emit_array(std::ostringstream &o, const char *type, const char *name, int n
 }
 
 }  // namespace
+
+namespace {
+
+int sm_count(const spin_system *s) {
+    int n = 148;
+    if (s->has_device) { int dev = 0; if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev); }
+    return n > 0 ? n : 148;
+}
+
+// Choose the staging geometry of one sweep.  Defaults: 32 x TBY tiles (TBY 8), look-ahead 3 planes; the number of chunks along
+// c is chosen so that the work items fill the resident CTAs evenly while the 2*rC extra planes per chunk stay cheap.
+// SPINLLG_TMA_P / SPINLLG_TMA_C = "tbx,tby,look,nzc" override (0 = default) for tuning.
+bool plan_tma_geo(const spin_system *s, int narr, const char *env, TmaGeo &g, std::string &why) {
+    const DevicePlan &P = s->plan;
+    int tbx = 32, tby = 8, look = 3, nzc = 0;
+    if (const char *e = getenv(env)) {
+        int v[4] = {0, 0, 0, 0};
+        sscanf(e, "%d,%d,%d,%d", &v[0], &v[1], &v[2], &v[3]);
+        if (v[0] > 0) tbx = v[0];
+        if (v[1] > 0) tby = v[1];
+        if (v[2] > 0) look = v[2];
+        if (v[3] > 0) nzc = v[3];
+    }
+    if (tbx % 2 || (tbx * tby) % 32 || tbx * tby > 1024) { why = "tile must have an even width and a multiple of 32 cells, at most 1024"; return false; }
+    g.tbx = tbx; g.tby = tby; g.look = look; g.ring = look + 2 * P.rC + 1; g.narr = narr;
+    const int wx = tbx + 2 * ((P.rA + 1) / 2 * 2), wy = tby + 2 * P.rB;      // rim along a rounded up to even (16-byte aligned box rows)
+    if (wx > 256 || wy > 256 || P.nb > 256) { why = "staged box exceeds the TMA box limit of 256 per dimension"; return false; }
+    const size_t arr = ((size_t)3 * wx * wy * P.nb + 15) / 16 * 16;
+    g.smem_bytes = (size_t)g.ring * narr * arr * 8 + (size_t)g.ring * 8;
+    if (g.smem_bytes > 220 * 1024) { why = "staging ring does not fit in shared memory"; return false; }
+    const int cols = ((P.Na + tbx - 1) / tbx) * ((P.Nb + tby - 1) / tby);
+    int per_sm = (int)std::min<size_t>((size_t)2048 / (tbx * tby), (size_t)(227 * 1024) / (g.smem_bytes + 1024));
+    if (per_sm < 1) per_sm = 1;
+    const int slots = sm_count(s) * per_sm;
+    if (nzc <= 0) {
+        double best = -1.0;
+        for (int k = 1; k <= P.Nc; ++k) {
+            const int cz = (P.Nc + k - 1) / k;
+            if ((k - 1) * cz >= P.Nc) continue;                           // an empty last chunk
+            const long items = (long)cols * k;
+            const long waves = (items + slots - 1) / slots;
+            const double util = (double)items / (double)(waves * slots);
+            const double eff = util * (double)P.Nc / ((double)k * (cz + 2 * P.rC));
+            if (eff > best + 1e-9) { best = eff; nzc = k; }
+        }
+    }
+    if (nzc > P.Nc) nzc = P.Nc;
+    g.nzc = nzc; g.cz = (P.Nc + nzc - 1) / nzc;
+    g.items = cols * nzc;
+    return true;
+}
+
+void emit_tma_geo(std::ostringstream &o, const char *name, const TmaGeo &g) {
+    o << "struct " << name << " { static constexpr int TBX = " << g.tbx << ", TBY = " << g.tby << ", RING = " << g.ring << ", LOOK = " << g.look
+      << ", NZC = " << g.nzc << ", CZ = " << g.cz << "; };\n";
+}
+
+}  // namespace
+
+// the staging geometry of both sweeps, or why the TMA-fed sweeps are not generated for this system
+static bool plan_tma(const spin_system *s, TmaGeo &gp, TmaGeo &gc, std::string &why) {
+    if (!s->opt_tma) { why = "disabled by option use_tma=0"; return false; }
+    if (s->opt_store_A) { why = "store_A=1 uses the brick kernels"; return false; }
+    if (s->opt_tma < 2 && s->N < 16384) { why = "lattice too small to fill persistent CTAs"; return false; }
+    return plan_tma_geo(s, 1, "SPINLLG_TMA_P", gp, why) && plan_tma_geo(s, 2, "SPINLLG_TMA_C", gc, why);
+}
 
 std::string spin::jit_source(const spin_system *s) {
     const DevicePlan &P = s->plan;
@@ -107,7 +192,12 @@ std::string spin::jit_source(const spin_system *s) {
     o << "constexpr double STT_C[3] = {" << hexd(P.stt_on ? P.stt_c[0] : 0.0) << ", " << hexd(P.stt_on ? P.stt_c[1] : 0.0) << ", "
       << hexd(P.stt_on ? P.stt_c[2] : 0.0) << "};\n";
     o << "constexpr double STT_S = " << hexd(P.stt_s) << ", STT_X = " << hexd(P.stt_x) << ";\n";
+    TmaGeo gp, gc;
+    std::string why;
+    const bool tma = plan_tma(s, gp, gc, why);
+    if (tma) { emit_tma_geo(o, "TmaP", gp); emit_tma_geo(o, "TmaC", gc); }
     o << "}  // namespace spec\n";
+    if (tma) o << "#define SPIN_TMA 1\n";
     o << "#include \"spin_jit_kernels.cuh\"\n";
     return o.str();
 }
@@ -149,12 +239,62 @@ void spin::jit_release(spin_system *s) {
     s->jit = nullptr;
 }
 
+// CUtensorMap of one per-spin array: dims (x: PA, comp: 3, y: PB, z: PC, sublattice: nb), box = one staged plane
+static int encode_plane_map(const spin_system *s, const TmaGeo &g, const double *base, CUtensorMap *tm) {
+    typedef CUresult (*encode_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *, const cuuint32_t *,
+                                  const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    static encode_fn encode = nullptr;
+    if (!encode) {
+        void *fn = nullptr;
+        cudaDriverEntryPointQueryResult qr;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qr) != cudaSuccess || !fn || qr != cudaDriverEntryPointSuccess)
+            return spin::fail(SPIN_ERR_CUDA, "cuTensorMapEncodeTiled is not available from this driver");
+        encode = (encode_fn)fn;
+    }
+    const DevicePlan &P = s->plan;
+    const cuuint64_t dims[5] = {(cuuint64_t)P.PA, 3, (cuuint64_t)P.PB, (cuuint64_t)P.PC, (cuuint64_t)P.nb};
+    const cuuint64_t strides[4] = {(cuuint64_t)P.PA * 8, (cuuint64_t)3 * P.PA * 8, (cuuint64_t)3 * P.PA * P.PB * 8, (cuuint64_t)P.sub * 8};
+    const cuuint32_t box[5] = {(cuuint32_t)(g.tbx + 2 * ((P.rA + 1) / 2 * 2)), 3, (cuuint32_t)(g.tby + 2 * P.rB), 1, (cuuint32_t)P.nb};
+    const cuuint32_t estr[5] = {1, 1, 1, 1, 1};
+    const CUresult r = encode(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 5, (void *)base, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                              CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return spin::fail(SPIN_ERR_CUDA, "cuTensorMapEncodeTiled failed with code %d", (int)r);
+    return SPIN_OK;
+}
+
+// kernels, launch geometry and tensor maps of the TMA-fed sweeps; on failure j->tma stays false and j->tma_note says why
+static void tma_prepare(spin_system *s, JitState *j) {
+    j->tma = false;
+    if (!plan_tma(s, j->gp, j->gc, j->tma_note)) return;
+    cudaError_t e = cudaLibraryGetKernel(&j->k_pred_tma, j->lib, "jit_predictor_tma");
+    if (e == cudaSuccess) e = cudaLibraryGetKernel(&j->k_corr_tma, j->lib, "jit_corrector_tma");
+    if (e == cudaSuccess) e = cudaFuncSetAttribute((const void *)j->k_pred_tma, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)j->gp.smem_bytes);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute((const void *)j->k_corr_tma, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)j->gc.smem_bytes);
+    int occ_p = 0, occ_c = 0;
+    if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_p, (const void *)j->k_pred_tma, j->gp.tbx * j->gp.tby, j->gp.smem_bytes);
+    if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_c, (const void *)j->k_corr_tma, j->gc.tbx * j->gc.tby, j->gc.smem_bytes);
+    if (e != cudaSuccess) { cudaGetLastError(); j->tma_note = std::string("TMA kernel setup failed: ") + cudaGetErrorString(e); return; }
+    if (occ_p < 1 || occ_c < 1) { j->tma_note = "TMA kernels do not fit on an SM"; return; }
+    const int sms = sm_count(s);
+    j->grid_p = std::min(j->gp.items, sms * occ_p);
+    j->grid_c = std::min(j->gc.items, sms * occ_c);
+    if (encode_plane_map(s, j->gp, s->d_n[0], &j->tm_n[0]) || encode_plane_map(s, j->gp, s->d_n[1], &j->tm_n[1]) ||
+        encode_plane_map(s, j->gc, s->d_n[0], &j->tm_cn[0]) || encode_plane_map(s, j->gc, s->d_n[1], &j->tm_cn[1]) ||
+        encode_plane_map(s, j->gc, s->d_np, &j->tm_cnp)) { j->tma_note = spin_last_error(); return; }
+    j->tma = true;
+    j->tma_note.clear();
+}
+
 int spin::jit_prepare(spin_system *s) {
     const std::string src = jit_source(s);
-    if (s->jit && s->jit->loaded && s->jit->source == src) return SPIN_OK;      // plan changed in ways the sweeps do not see
+    if (s->jit && s->jit->loaded && s->jit->source == src) {      // plan changed in ways the sweeps do not see
+        tma_prepare(s, s->jit);                                   // the arrays may have moved: tensor maps are rebuilt
+        return SPIN_OK;
+    }
     jit_release(s);
     JitState *j = new JitState();
     j->loaded = false;
+    j->tma = false;
     j->source = src;
     s->jit = j;
     std::string cubin;
@@ -166,6 +306,7 @@ int spin::jit_prepare(spin_system *s) {
     e = cudaLibraryGetKernel(&j->k_pred, j->lib, "jit_predictor");
     if (e == cudaSuccess) e = cudaLibraryGetKernel(&j->k_corr, j->lib, "jit_corrector");
     if (e != cudaSuccess) return spin::fail(SPIN_ERR_CUDA, "cudaLibraryGetKernel failed: %s", cudaGetErrorString(e));
+    tma_prepare(s, j);
     return SPIN_OK;
 }
 
@@ -187,6 +328,29 @@ int spin::jit_launch_corrector(spin_system *s, dim3 grid, dim3 block, const doub
     void *args[] = {(void *)&n, (void *)&np, (void *)&fddi_n, (void *)&fddi_np, (void *)&Ain, (void *)&nout, (void *)&d_step, (void *)&step_add,
                     (void *)&seed_lo, (void *)&seed_hi};
     SPIN_CUDA(cudaLaunchKernel((const void *)s->jit->k_corr, grid, block, args, 0, s->stream));
+    return SPIN_OK;
+}
+
+bool spin::jit_tma_ready(const spin_system *s) { return s->jit && s->jit->loaded && s->jit->tma; }
+const char *spin::jit_tma_note(const spin_system *s) { return s->jit ? s->jit->tma_note.c_str() : "specialised kernels not loaded"; }
+
+// the corrector stages n and n^p with its own tile: the maps are encoded per sweep geometry
+int spin::jit_launch_predictor_tma(spin_system *s, int cur, const double *fddi, double *np, unsigned step_add) {
+    JitState *j = s->jit;
+    unsigned seed_lo = s->plan.seed_lo, seed_hi = s->plan.seed_hi;
+    const unsigned long long *d_step = s->d_step;
+    void *args[] = {(void *)&j->tm_n[cur], (void *)&fddi, (void *)&np, (void *)&d_step, (void *)&step_add, (void *)&seed_lo, (void *)&seed_hi};
+    SPIN_CUDA(cudaLaunchKernel((const void *)j->k_pred_tma, dim3((unsigned)j->grid_p), dim3((unsigned)(j->gp.tbx * j->gp.tby)), args, j->gp.smem_bytes, s->stream));
+    return SPIN_OK;
+}
+
+int spin::jit_launch_corrector_tma(spin_system *s, int cur, const double *fddi_n, const double *fddi_np, double *nout, unsigned step_add) {
+    JitState *j = s->jit;
+    unsigned seed_lo = s->plan.seed_lo, seed_hi = s->plan.seed_hi;
+    const unsigned long long *d_step = s->d_step;
+    void *args[] = {(void *)&j->tm_cn[cur], (void *)&j->tm_cnp, (void *)&fddi_n, (void *)&fddi_np, (void *)&nout, (void *)&d_step, (void *)&step_add,
+                    (void *)&seed_lo, (void *)&seed_hi};
+    SPIN_CUDA(cudaLaunchKernel((const void *)j->k_corr_tma, dim3((unsigned)j->grid_c), dim3((unsigned)(j->gc.tbx * j->gc.tby)), args, j->gc.smem_bytes, s->stream));
     return SPIN_OK;
 }
 

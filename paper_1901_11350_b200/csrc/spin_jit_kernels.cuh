@@ -75,10 +75,19 @@ __device__ __forceinline__ void store_spin(double *__restrict__ q, const Coord &
     }
 }
 
-// F += (Zeeman + anisotropy + pairs + quadruplets) of basis atom B for NCONF configurations sharing the lattice;
-// cfg[k] points at the x component of the own site in configuration k
-template <int B, int NCONF>
-__device__ __forceinline__ void force(const double *const (&cfg)[NCONF], const double (&own)[NCONF][3], double (&F)[NCONF][3]) {
+// Site accessors: where the partner (sublattice BJ at translation DA, DB, DC) of a site of sublattice B is read from.
+// GlobalAcc: the ghost-cell arrays in global memory (own address + immediate); RingAcc (spin_jit_tma.cuh): the ring of lattice
+// planes that TMA stages in shared memory.
+template <int NCONF>
+struct GlobalAcc {
+    const double *cfg[NCONF];      // x component of the own site in configuration k
+    template <int B, int BJ, int DA, int DB, int DC>
+    __device__ __forceinline__ void load(int k, double (&v)[3]) const { load3<lin<B, BJ, DA, DB, DC>()>(cfg[k], v); }
+};
+
+// F += (Zeeman + anisotropy + pairs + quadruplets) of basis atom B for NCONF configurations sharing the lattice
+template <int B, int NCONF, class Acc>
+__device__ __forceinline__ void force(const Acc &cfg, const double (&own)[NCONF][3], double (&F)[NCONF][3]) {
 #pragma unroll
     for (int k = 0; k < NCONF; ++k) {
         if constexpr (spec::ZEE[B][0] != 0.0) F[k][0] += spec::ZEE[B][0];
@@ -98,12 +107,11 @@ __device__ __forceinline__ void force(const double *const (&cfg)[NCONF], const d
     }
     static_for<spec::PAIR_BEGIN[B], spec::PAIR_BEGIN[B + 1]>([&](auto e) {
         constexpr int E = decltype(e)::value;
-        constexpr int O = lin<B, spec::P_BJ[E], spec::P_DA[E], spec::P_DB[E], spec::P_DC[E]>();
         constexpr double J = spec::P_J[E], Dx = spec::P_DX[E], Dy = spec::P_DY[E], Dz = spec::P_DZ[E];
 #pragma unroll
         for (int k = 0; k < NCONF; ++k) {
             double p[3];
-            load3<O>(cfg[k], p);
+            cfg.template load<B, spec::P_BJ[E], spec::P_DA[E], spec::P_DB[E], spec::P_DC[E]>(k, p);
             // J n_j + n_j x D, zero components dropped at compile time
             if constexpr (J != 0.0) { F[k][0] = fma(J, p[0], F[k][0]); F[k][1] = fma(J, p[1], F[k][1]); F[k][2] = fma(J, p[2], F[k][2]); }
             if constexpr (Dz != 0.0) { F[k][0] = fma(p[1], Dz, F[k][0]); F[k][1] = fma(p[0], -Dz, F[k][1]); }
@@ -113,13 +121,12 @@ __device__ __forceinline__ void force(const double *const (&cfg)[NCONF], const d
     });
     static_for<spec::QUAD_BEGIN[B], spec::QUAD_BEGIN[B + 1]>([&](auto e) {
         constexpr int E = decltype(e)::value;
-        constexpr int OP = lin<B, spec::Q_B[E][0], spec::Q_D[E][0], spec::Q_D[E][1], spec::Q_D[E][2]>();
-        constexpr int OQ = lin<B, spec::Q_B[E][1], spec::Q_D[E][3], spec::Q_D[E][4], spec::Q_D[E][5]>();
-        constexpr int OR = lin<B, spec::Q_B[E][2], spec::Q_D[E][6], spec::Q_D[E][7], spec::Q_D[E][8]>();
 #pragma unroll
         for (int k = 0; k < NCONF; ++k) {
             double P[3], Q[3], R[3];
-            load3<OP>(cfg[k], P); load3<OQ>(cfg[k], Q); load3<OR>(cfg[k], R);
+            cfg.template load<B, spec::Q_B[E][0], spec::Q_D[E][0], spec::Q_D[E][1], spec::Q_D[E][2]>(k, P);
+            cfg.template load<B, spec::Q_B[E][1], spec::Q_D[E][3], spec::Q_D[E][4], spec::Q_D[E][5]>(k, Q);
+            cfg.template load<B, spec::Q_B[E][2], spec::Q_D[E][6], spec::Q_D[E][7], spec::Q_D[E][8]>(k, R);
             const double w = spec::Q_K[E] * fma(Q[0], R[0], fma(Q[1], R[1], Q[2] * R[2]));
             F[k][0] = fma(w, P[0], F[k][0]); F[k][1] = fma(w, P[1], F[k][1]); F[k][2] = fma(w, P[2], F[k][2]);
         }
@@ -127,13 +134,12 @@ __device__ __forceinline__ void force(const double *const (&cfg)[NCONF], const d
 }
 
 // (j^ . grad) n: central differences on the same sublattice, one-sided at open edges
-template <int NCONF>
-__device__ __forceinline__ void stt_gradient(const double *const (&cfg)[NCONF], const Coord &c, const double (&own)[NCONF][3],
-                                             double (&sg)[NCONF][3]) {
+template <int B, int NCONF, class Acc>
+__device__ __forceinline__ void stt_gradient(const Acc &cfg, const Coord &c, const double (&own)[NCONF][3], double (&sg)[NCONF][3]) {
     static_for<0, 3>([&](auto dd) {
         constexpr int D = decltype(dd)::value;
         if constexpr (spec::STT_C[D] != 0.0) {
-            constexpr int STEP = D == 0 ? 1 : (D == 1 ? ROW : PLANE);
+            constexpr int SA = D == 0 ? 1 : 0, SB = D == 1 ? 1 : 0, SC = D == 2 ? 1 : 0;
             constexpr bool PER = D == 0 ? spec::PER_A : (D == 1 ? spec::PER_B : spec::PER_C);
             constexpr int EXT = D == 0 ? spec::NA : (D == 1 ? spec::NB : spec::NC);
             const int x = D == 0 ? c.ia : (D == 1 ? c.ib : c.ic);
@@ -142,7 +148,7 @@ __device__ __forceinline__ void stt_gradient(const double *const (&cfg)[NCONF], 
 #pragma unroll
             for (int k = 0; k < NCONF; ++k) {
                 double vp[3], vm[3];
-                load3<STEP>(cfg[k], vp); load3<-STEP>(cfg[k], vm);
+                cfg.template load<B, B, SA, SB, SC>(k, vp); cfg.template load<B, B, -SA, -SB, -SC>(k, vm);
                 if constexpr (!PER) {      // ghost cells of an open edge hold zeros: use the own spin for the one-sided difference
                     if (!hp) { vp[0] = own[k][0]; vp[1] = own[k][1]; vp[2] = own[k][2]; }
                     if (!hm) { vm[0] = own[k][0]; vm[1] = own[k][1]; vm[2] = own[k][2]; }
@@ -202,13 +208,13 @@ __device__ __forceinline__ void predictor_body(const double *__restrict__ n, con
     Coord c;
     int idx;
     if (!locate<B>(c, idx)) return;
-    const double *const cfg[1] = {n + idx};
+    const GlobalAcc<1> cfg = {{n + idx}};
     double own[1][3], F[1][3], sg[1][3] = {{0.0, 0.0, 0.0}};
-    load3<0>(cfg[0], own[0]);
+    load3<0>(cfg.cfg[0], own[0]);
     thermal_force<B>(c, step, seed_lo, seed_hi, F[0]);
     force<B, 1>(cfg, own, F);
     if constexpr (spec::HAS_DDI) { double d[3]; load3<0>(fddi + idx, d); F[0][0] += d[0]; F[0][1] += d[1]; F[0][2] += d[2]; }
-    if constexpr (spec::STT_ON) stt_gradient<1>(cfg, c, own, sg);
+    if constexpr (spec::STT_ON) stt_gradient<B, 1>(cfg, c, own, sg);
     double A[3], out[3];
     rotation_field<B>(own[0], F[0], sg[0], A);
     spin::rodrigues(A, spec::DT, spec::DT2, own[0], out);
@@ -227,26 +233,26 @@ __device__ __forceinline__ void corrector_body(const double *__restrict__ n, con
     thermal_force<B>(c, step, seed_lo, seed_hi, th);
     load3<0>(n + idx, n0);
     if constexpr (spec::STORE_A) {
-        const double *const cfg[1] = {np + idx};
+        const GlobalAcc<1> cfg = {{np + idx}};
         double own[1][3], F[1][3] = {{th[0], th[1], th[2]}}, sg[1][3] = {{0.0, 0.0, 0.0}};
-        load3<0>(cfg[0], own[0]);
+        load3<0>(cfg.cfg[0], own[0]);
         force<B, 1>(cfg, own, F);
         if constexpr (spec::HAS_DDI) { double d[3]; load3<0>(fddi_np + idx, d); F[0][0] += d[0]; F[0][1] += d[1]; F[0][2] += d[2]; }
-        if constexpr (spec::STT_ON) stt_gradient<1>(cfg, c, own, sg);
+        if constexpr (spec::STT_ON) stt_gradient<B, 1>(cfg, c, own, sg);
         rotation_field<B>(own[0], F[0], sg[0], Ap);
         load3<0>(Ain + idx, A);
     } else {
-        const double *const cfg[2] = {n + idx, np + idx};
+        const GlobalAcc<2> cfg = {{n + idx, np + idx}};
         double own[2][3], F[2][3] = {{th[0], th[1], th[2]}, {th[0], th[1], th[2]}}, sg[2][3] = {{0.0, 0.0, 0.0}, {0.0, 0.0, 0.0}};
         own[0][0] = n0[0]; own[0][1] = n0[1]; own[0][2] = n0[2];
-        load3<0>(cfg[1], own[1]);
+        load3<0>(cfg.cfg[1], own[1]);
         force<B, 2>(cfg, own, F);
         if constexpr (spec::HAS_DDI) {
             double d[3];
             load3<0>(fddi_n + idx, d); F[0][0] += d[0]; F[0][1] += d[1]; F[0][2] += d[2];
             load3<0>(fddi_np + idx, d); F[1][0] += d[0]; F[1][1] += d[1]; F[1][2] += d[2];
         }
-        if constexpr (spec::STT_ON) stt_gradient<2>(cfg, c, own, sg);
+        if constexpr (spec::STT_ON) stt_gradient<B, 2>(cfg, c, own, sg);
         rotation_field<B>(own[0], F[0], sg[0], A);
         rotation_field<B>(own[1], F[1], sg[1], Ap);
     }
@@ -285,3 +291,7 @@ extern "C" __global__ void __launch_bounds__(spec::BX *spec::BY *spec::BZ)
         spinjit::corrector_body<decltype(b)::value>(n, np, fddi_n, fddi_np, Ain, nout, step, seed_lo, seed_hi);
     });
 }
+
+#ifdef SPIN_TMA
+#include "spin_jit_tma.cuh"
+#endif

@@ -243,7 +243,41 @@ def test_specialised_and_table_driven_sweeps_agree(P, O, cfg):
     a = P.SpinSystem.from_workload(w)
     b = P.SpinSystem.from_workload(w)
     b.spin_set_option("use_jit", 0)
-    assert a.spin_kernel_info() == "jit", a.spin_kernel_info()
+    assert a.spin_kernel_info().startswith("jit"), a.spin_kernel_info()
     assert b.spin_kernel_info().startswith("generic")
     a.llg_iterate(30); b.llg_iterate(30)
     assert np.abs(a.spins_get() - b.spins_get()).max() < 1e-13
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# TMA-fed plane-marching sweeps (csrc/spin_jit_tma.cuh): forced on for small replicas (use_tma=2), several items per CTA
+TMA_CASES = [
+    (1, (37, 19, 1), 200, None),
+    (2, (45, 33, 1), 200, None),
+    (3, (35, 9, 7), 200, None),
+    (3, (70, 37, 45), 20, "0,0,0,45"),       # 15 columns x 45 chunks = 675 items > resident CTAs: every CTA marches several items
+    (3, (70, 37, 45), 20, "0,16,2,3"),       # 32x16 tiles, look-ahead 2, 3 chunks of 15 planes
+    (4, (33, 17, 1), 200, None),
+    (5, (20, 12, 5), 30, None),
+]
+
+
+@pytest.mark.parametrize("cfg,cells,steps,geo", TMA_CASES)
+def test_tma_sweeps_match_oracle(P, O, cfg, cells, steps, geo, monkeypatch):
+    if geo:
+        monkeypatch.setenv("SPINLLG_TMA_P", geo)
+        monkeypatch.setenv("SPINLLG_TMA_C", geo)
+    w = W.CONFIGS[cfg]().resized(cells, steps)
+    g, o = pair(P, O, w)
+    g.spin_set_option("use_tma", 2)
+    assert g.spin_kernel_info() == "jit+tma", g.spin_kernel_info()
+    g.llg_iterate(steps); o.iterate(steps)
+    d = np.abs(g.spins_get() - o.spins()).max()
+    print(f"tma cfg{cfg} {cells} steps={steps}: max|dn| = {d:.3e}")
+    assert d <= SPIN_ATOL
+    # bit-identical to the brick kernels: same arithmetic, only the staging differs
+    b = P.SpinSystem.from_workload(w)
+    b.spin_set_option("use_tma", 0)
+    assert b.spin_kernel_info().startswith("jit (brick")
+    b.llg_iterate(steps)
+    assert np.array_equal(b.spins_get(), g.spins_get())
