@@ -135,8 +135,9 @@ int spin_profile_get(spin_system *sys, int kind, double *total_ms, int64_t *laun
 int spin_set_option(spin_system *sys, const char *name, int value);
 /* further option: use_jit (1: the two sweeps are specialised per system at run time with NVRTC -- lattice extents, gather
  * tables and prefactors become compile-time constants; 0: table-driven kernels; default 1).
- * use_tma (default 1): the specialised sweeps run as persistent kernels that stage lattice planes in shared memory with TMA
- * tensor copies (lattices of at least 16384 spins; 2 forces it for any size, 0 keeps the brick kernels).
+ * use_tma (default 0): 1 runs the specialised sweeps as persistent kernels that stage lattice planes in shared memory with TMA
+ * tensor copies (lattices of at least 16384 spins; 2 forces it for any size).  Measured slower than the brick kernels on
+ * cfg3, hence off by default.
  * spin_kernel_info writes "jit+tma", "jit (brick kernels: <why>)" or "generic: <why>" into buf: which sweep kernels are in use.  */
 int spin_kernel_info(spin_system *sys, char *buf, int len);
 /* the generated translation unit of the specialised sweeps (buf may be NULL); compile != 0 also compiles it for sm_100a

@@ -446,7 +446,7 @@ extern "C" int spin_geometry_create(const double bravais[9], int n_basis, const 
     if (!has_device) cudaGetLastError();
     spin_system *s = new spin_system();
     s->has_device = has_device;
-    s->jit = nullptr; s->opt_jit = 1; s->opt_tma = 1;
+    s->jit = nullptr; s->opt_jit = 1; s->opt_tma = 0;
     memcpy(s->brav, bravais, sizeof(s->brav));
     s->nb = n_basis;
     s->basis.assign(basis_frac, basis_frac + 3 * n_basis);

@@ -22,7 +22,7 @@ using namespace spin;
 
 // staging geometry of one TMA-fed sweep (spin_jit_tma.cuh): tile, ring depth, look-ahead, chunks along c
 struct TmaGeo {
-    int tbx, tby, ring, look, nzc, cz;
+    int tbx, tby, kz, ring, look, nzc, cz;
     int narr;                 // arrays staged per plane (predictor 1, corrector 2)
     size_t smem_bytes;
     int items;
@@ -82,27 +82,29 @@ int sm_count(const spin_system *s) {
 
 // Choose the staging geometry of one sweep.  Defaults: 32 x TBY tiles (TBY 8), look-ahead 3 planes; the number of chunks along
 // c is chosen so that the work items fill the resident CTAs evenly while the 2*rC extra planes per chunk stay cheap.
-// SPINLLG_TMA_P / SPINLLG_TMA_C = "tbx,tby,look,nzc" override (0 = default) for tuning.
+// SPINLLG_TMA_P / SPINLLG_TMA_C = "tbx,tby,look,nzc,kz" override (0 = default) for tuning.
 bool plan_tma_geo(const spin_system *s, int narr, const char *env, TmaGeo &g, std::string &why) {
     const DevicePlan &P = s->plan;
-    int tbx = 32, tby = 8, look = 3, nzc = 0;
+    int tbx = 32, tby = 8, look = 2, nzc = 0, kz = 2;
     if (const char *e = getenv(env)) {
-        int v[4] = {0, 0, 0, 0};
-        sscanf(e, "%d,%d,%d,%d", &v[0], &v[1], &v[2], &v[3]);
+        int v[5] = {0, 0, 0, 0, 0};
+        sscanf(e, "%d,%d,%d,%d,%d", &v[0], &v[1], &v[2], &v[3], &v[4]);
         if (v[0] > 0) tbx = v[0];
         if (v[1] > 0) tby = v[1];
         if (v[2] > 0) look = v[2];
         if (v[3] > 0) nzc = v[3];
+        if (v[4] > 0) kz = v[4];
     }
-    if (tbx % 2 || (tbx * tby) % 32 || tbx * tby > 1024) { why = "tile must have an even width and a multiple of 32 cells, at most 1024"; return false; }
-    g.tbx = tbx; g.tby = tby; g.look = look; g.ring = look + 2 * P.rC + 1; g.narr = narr;
+    look = (look + kz - 1) / kz * kz;
+    if (tbx % 2 || (tbx * tby) % 32 || tbx * tby * kz > 1024) { why = "tile must have an even width and a multiple of 32 cells, at most 1024 threads"; return false; }
+    g.tbx = tbx; g.tby = tby; g.kz = kz; g.look = look; g.ring = look + kz + 2 * P.rC; g.narr = narr;
     const int wx = tbx + 2 * ((P.rA + 1) / 2 * 2), wy = tby + 2 * P.rB;      // rim along a rounded up to even (16-byte aligned box rows)
     if (wx > 256 || wy > 256 || P.nb > 256) { why = "staged box exceeds the TMA box limit of 256 per dimension"; return false; }
     const size_t arr = ((size_t)3 * wx * wy * P.nb + 15) / 16 * 16;
     g.smem_bytes = (size_t)g.ring * narr * arr * 8 + (size_t)g.ring * 8;
     if (g.smem_bytes > 220 * 1024) { why = "staging ring does not fit in shared memory"; return false; }
     const int cols = ((P.Na + tbx - 1) / tbx) * ((P.Nb + tby - 1) / tby);
-    int per_sm = (int)std::min<size_t>((size_t)2048 / (tbx * tby), (size_t)(227 * 1024) / (g.smem_bytes + 1024));
+    int per_sm = (int)std::min<size_t>((size_t)2048 / (tbx * tby * kz), (size_t)(227 * 1024) / (g.smem_bytes + 1024));
     if (per_sm < 1) per_sm = 1;
     const int slots = sm_count(s) * per_sm;
     if (nzc <= 0) {
@@ -124,11 +126,28 @@ bool plan_tma_geo(const spin_system *s, int narr, const char *env, TmaGeo &g, st
 }
 
 void emit_tma_geo(std::ostringstream &o, const char *name, const TmaGeo &g) {
-    o << "struct " << name << " { static constexpr int TBX = " << g.tbx << ", TBY = " << g.tby << ", RING = " << g.ring << ", LOOK = " << g.look
+    o << "struct " << name << " { static constexpr int TBX = " << g.tbx << ", TBY = " << g.tby << ", KZ = " << g.kz << ", RING = " << g.ring << ", LOOK = " << g.look
       << ", NZC = " << g.nzc << ", CZ = " << g.cz << "; };\n";
 }
 
 }  // namespace
+
+// brick of the specialised brick kernels: BX x BY x BZ sites per block (SPINLLG_BRICK="bx,by,bz" overrides, for tuning)
+static void jit_brick(const spin_system *s, int b[3]) {
+    const bool flat = s->nc[2] < 2;
+    b[0] = 32; b[1] = flat ? 8 : 4; b[2] = flat ? 1 : 2;
+    if (const char *e = getenv("SPINLLG_BRICK")) {
+        int v[3] = {0, 0, 0};
+        sscanf(e, "%d,%d,%d", &v[0], &v[1], &v[2]);
+        if (v[0] > 0 && v[1] > 0 && v[2] > 0 && v[0] * v[1] * v[2] <= 1024 && (v[0] * v[1] * v[2]) % 32 == 0 && (!flat || v[2] == 1)) { b[0] = v[0]; b[1] = v[1]; b[2] = v[2]; }
+    }
+}
+static void jit_brick_launch(const spin_system *s, dim3 &grid, dim3 &block) {
+    int b[3];
+    jit_brick(s, b);
+    grid = dim3((unsigned)(((s->nc[0] + b[0] - 1) / b[0]) * ((s->nc[1] + b[1] - 1) / b[1]) * ((s->nc[2] + b[2] - 1) / b[2])), (unsigned)s->nb, 1);
+    block = dim3((unsigned)(b[0] * b[1] * b[2]), 1, 1);
+}
 
 // the staging geometry of both sweeps, or why the TMA-fed sweeps are not generated for this system
 static bool plan_tma(const spin_system *s, TmaGeo &gp, TmaGeo &gc, std::string &why) {
@@ -149,11 +168,17 @@ std::string spin::jit_source(const spin_system *s) {
       << ", SUB = " << P.sub << ", RA = " << P.rA << ", RB = " << P.rB << ", RC = " << P.rC << ";\n";
     o << "constexpr bool GA = " << (P.gA ? "true" : "false") << ", GB = " << (P.gB ? "true" : "false") << ", GC = "
       << (P.gC ? "true" : "false") << ";\n";
-    o << "constexpr int BX = 32, BY = " << (flat ? 8 : 4) << ", BZ = " << (flat ? 1 : 2) << ";\n";
+    int brick[3];
+    jit_brick(s, brick);
+    o << "constexpr int BX = " << brick[0] << ", BY = " << brick[1] << ", BZ = " << brick[2] << ";\n";
     o << "constexpr bool PER_A = " << (P.perA ? "true" : "false") << ", PER_B = " << (P.perB ? "true" : "false")
       << ", PER_C = " << (P.perC ? "true" : "false") << ";\n";
     o << "constexpr bool STORE_A = " << (s->opt_store_A ? "true" : "false") << ", HAS_DDI = " << (P.has_ddi ? "true" : "false")
       << ", THERMAL_ON = " << (P.thermal_on ? "true" : "false") << ", STT_ON = " << (P.stt_on ? "true" : "false") << ";\n";
+    // L2 prefetch distance of the brick kernels, in lattice planes (SPINLLG_PREFETCH overrides; 0 = off)
+    int pf = 0;
+    if (const char *e = getenv("SPINLLG_PREFETCH")) pf = atoi(e);
+    o << "constexpr int PF_PLANES = " << (flat ? 0 : pf) << ";\n";
     const int np = P.pair_begin[P.nb], nq = P.quad_begin[P.nb];
     emit_array<int>(o, "int", "PAIR_BEGIN", P.nb + 1, [&](int i) { return std::to_string(P.pair_begin[i]); });
     emit_array<int>(o, "int", "P_DA", np, [&](int i) { return std::to_string(P.pairs[i].da); });
@@ -192,12 +217,42 @@ std::string spin::jit_source(const spin_system *s) {
     o << "constexpr double STT_C[3] = {" << hexd(P.stt_on ? P.stt_c[0] : 0.0) << ", " << hexd(P.stt_on ? P.stt_c[1] : 0.0) << ", "
       << hexd(P.stt_on ? P.stt_c[2] : 0.0) << "};\n";
     o << "constexpr double STT_S = " << hexd(P.stt_s) << ", STT_X = " << hexd(P.stt_x) << ";\n";
+    // the same values in constant memory (operands of the fp64 instructions; spec:: decides at compile time what is zero)
+    o << "}  // namespace spec\nnamespace specc {\n";
+    auto emit_c = [&](const char *name, int n, auto &&get) {
+        o << "__constant__ double " << name << "[" << (n > 0 ? n : 1) << "] = {";
+        for (int i = 0; i < n; ++i) o << (i ? ", " : "") << hexd(get(i));
+        if (n == 0) o << "0.0";
+        o << "};\n";
+    };
+    auto emit_cb3 = [&](const char *name, const double (*v)[3]) {
+        o << "__constant__ double " << name << "[" << P.nb << "][3] = {";
+        for (int b = 0; b < P.nb; ++b) o << (b ? ", {" : "{") << hexd(v[b][0]) << ", " << hexd(v[b][1]) << ", " << hexd(v[b][2]) << "}";
+        o << "};\n";
+    };
+    emit_c("P_J", np, [&](int i) { return P.pairs[i].J; });
+    emit_c("P_DX", np, [&](int i) { return P.pairs[i].Dx; });
+    emit_c("P_DY", np, [&](int i) { return P.pairs[i].Dy; });
+    emit_c("P_DZ", np, [&](int i) { return P.pairs[i].Dz; });
+    emit_c("Q_K", nq, [&](int i) { return P.quads[i].K; });
+    emit_cb3("ZEE", P.zee);
+    emit_cb3("KAX", P.Kax);
+    emit_c("K2", P.nb, [&](int i) { return P.K2[i]; });
+    emit_c("PRE", P.nb, [&](int i) { return P.pre[i]; });
+    emit_c("PREA", P.nb, [&](int i) { return P.pre[i] * P.alpha; });
+    emit_c("SIGMA", P.nb, [&](int i) { return P.sigma[i]; });
+    emit_c("STT_C", 3, [&](int i) { return P.stt_on ? P.stt_c[i] : 0.0; });
+    o << "__constant__ double DT = " << hexd(P.dt) << ", DT2 = " << hexd(P.dt2) << ", HDT = " << hexd(0.5 * P.dt) << ", QDT2 = " << hexd(0.25 * P.dt2)
+      << ", STT_S = " << hexd(P.stt_s) << ", STT_X = " << hexd(P.stt_x) << ";\n";
+    o << "}  // namespace specc\nnamespace spec {\n";
     TmaGeo gp, gc;
     std::string why;
     const bool tma = plan_tma(s, gp, gc, why);
     if (tma) { emit_tma_geo(o, "TmaP", gp); emit_tma_geo(o, "TmaC", gc); }
     o << "}  // namespace spec\n";
     if (tma) o << "#define SPIN_TMA 1\n";
+    if (const char *e = getenv("SPINLLG_MINBLOCKS")) o << "#define SPIN_MINBLOCKS " << atoi(e) << "\n";
+    if (const char *e = getenv("SPINLLG_ABLATE")) o << "#define SPIN_ABLATE " << atoi(e) << "\n";
     o << "#include \"spin_jit_kernels.cuh\"\n";
     return o.str();
 }
@@ -271,8 +326,8 @@ static void tma_prepare(spin_system *s, JitState *j) {
     if (e == cudaSuccess) e = cudaFuncSetAttribute((const void *)j->k_pred_tma, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)j->gp.smem_bytes);
     if (e == cudaSuccess) e = cudaFuncSetAttribute((const void *)j->k_corr_tma, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)j->gc.smem_bytes);
     int occ_p = 0, occ_c = 0;
-    if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_p, (const void *)j->k_pred_tma, j->gp.tbx * j->gp.tby, j->gp.smem_bytes);
-    if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_c, (const void *)j->k_corr_tma, j->gc.tbx * j->gc.tby, j->gc.smem_bytes);
+    if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_p, (const void *)j->k_pred_tma, j->gp.tbx * j->gp.tby * j->gp.kz, j->gp.smem_bytes);
+    if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_c, (const void *)j->k_corr_tma, j->gc.tbx * j->gc.tby * j->gc.kz, j->gc.smem_bytes);
     if (e != cudaSuccess) { cudaGetLastError(); j->tma_note = std::string("TMA kernel setup failed: ") + cudaGetErrorString(e); return; }
     if (occ_p < 1 || occ_c < 1) { j->tma_note = "TMA kernels do not fit on an SM"; return; }
     const int sms = sm_count(s);
@@ -317,6 +372,7 @@ int spin::jit_launch_predictor(spin_system *s, dim3 grid, dim3 block, const doub
     unsigned seed_lo = s->plan.seed_lo, seed_hi = s->plan.seed_hi;
     const unsigned long long *d_step = s->d_step;
     void *args[] = {(void *)&n, (void *)&fddi, (void *)&np, (void *)&Aout, (void *)&d_step, (void *)&step_add, (void *)&seed_lo, (void *)&seed_hi};
+    jit_brick_launch(s, grid, block);
     SPIN_CUDA(cudaLaunchKernel((const void *)s->jit->k_pred, grid, block, args, 0, s->stream));
     return SPIN_OK;
 }
@@ -327,6 +383,7 @@ int spin::jit_launch_corrector(spin_system *s, dim3 grid, dim3 block, const doub
     const unsigned long long *d_step = s->d_step;
     void *args[] = {(void *)&n, (void *)&np, (void *)&fddi_n, (void *)&fddi_np, (void *)&Ain, (void *)&nout, (void *)&d_step, (void *)&step_add,
                     (void *)&seed_lo, (void *)&seed_hi};
+    jit_brick_launch(s, grid, block);
     SPIN_CUDA(cudaLaunchKernel((const void *)s->jit->k_corr, grid, block, args, 0, s->stream));
     return SPIN_OK;
 }
@@ -340,7 +397,7 @@ int spin::jit_launch_predictor_tma(spin_system *s, int cur, const double *fddi, 
     unsigned seed_lo = s->plan.seed_lo, seed_hi = s->plan.seed_hi;
     const unsigned long long *d_step = s->d_step;
     void *args[] = {(void *)&j->tm_n[cur], (void *)&fddi, (void *)&np, (void *)&d_step, (void *)&step_add, (void *)&seed_lo, (void *)&seed_hi};
-    SPIN_CUDA(cudaLaunchKernel((const void *)j->k_pred_tma, dim3((unsigned)j->grid_p), dim3((unsigned)(j->gp.tbx * j->gp.tby)), args, j->gp.smem_bytes, s->stream));
+    SPIN_CUDA(cudaLaunchKernel((const void *)j->k_pred_tma, dim3((unsigned)j->grid_p), dim3((unsigned)(j->gp.tbx * j->gp.tby * j->gp.kz)), args, j->gp.smem_bytes, s->stream));
     return SPIN_OK;
 }
 
@@ -350,7 +407,7 @@ int spin::jit_launch_corrector_tma(spin_system *s, int cur, const double *fddi_n
     const unsigned long long *d_step = s->d_step;
     void *args[] = {(void *)&j->tm_cn[cur], (void *)&j->tm_cnp, (void *)&fddi_n, (void *)&fddi_np, (void *)&nout, (void *)&d_step, (void *)&step_add,
                     (void *)&seed_lo, (void *)&seed_hi};
-    SPIN_CUDA(cudaLaunchKernel((const void *)j->k_corr_tma, dim3((unsigned)j->grid_c), dim3((unsigned)(j->gc.tbx * j->gc.tby)), args, j->gc.smem_bytes, s->stream));
+    SPIN_CUDA(cudaLaunchKernel((const void *)j->k_corr_tma, dim3((unsigned)j->grid_c), dim3((unsigned)(j->gc.tbx * j->gc.tby * j->gc.kz)), args, j->gc.smem_bytes, s->stream));
     return SPIN_OK;
 }
 

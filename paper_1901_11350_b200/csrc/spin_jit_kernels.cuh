@@ -19,6 +19,12 @@
 //   double ALPHA, DT, DT2, STT_C[3], STT_S, STT_X;
 #pragma once
 
+#ifndef SPIN_ABLATE
+#define SPIN_ABLATE 0
+#endif
+#ifndef SPIN_MINBLOCKS
+#define SPIN_MINBLOCKS 1
+#endif
 #include "spin_device_math.cuh"
 
 namespace spinjit {
@@ -61,11 +67,16 @@ __device__ __forceinline__ void store3(double *__restrict__ q, const double (&v)
 __device__ __forceinline__ void store_spin(double *__restrict__ q, const Coord &c, const double (&v)[3]) {
     store3(q, v);
     if constexpr (spec::GA || spec::GB || spec::GC) {
-        int sa = 0, sb = 0, sc = 0;
-        if constexpr (spec::GA) { if (c.ia < spec::RA) sa = spec::NA; else if (c.ia >= spec::NA - spec::RA) sa = -spec::NA; }
-        if constexpr (spec::GB) { if (c.ib < spec::RB) sb = spec::NB * ROW; else if (c.ib >= spec::NB - spec::RB) sb = -spec::NB * ROW; }
-        if constexpr (spec::GC) { if (c.ic < spec::RC) sc = spec::NC * PLANE; else if (c.ic >= spec::NC - spec::RC) sc = -spec::NC * PLANE; }
-        if (sa | sb | sc) {
+        // one unsigned compare per direction decides whether the site has any image at all (interior sites: nearly all)
+        bool edge = false;
+        if constexpr (spec::GA) { if constexpr (spec::NA > 2 * spec::RA) edge |= (unsigned)(c.ia - spec::RA) >= (unsigned)(spec::NA - 2 * spec::RA); else edge = true; }
+        if constexpr (spec::GB) { if constexpr (spec::NB > 2 * spec::RB) edge |= (unsigned)(c.ib - spec::RB) >= (unsigned)(spec::NB - 2 * spec::RB); else edge = true; }
+        if constexpr (spec::GC) { if constexpr (spec::NC > 2 * spec::RC) edge |= (unsigned)(c.ic - spec::RC) >= (unsigned)(spec::NC - 2 * spec::RC); else edge = true; }
+        if (edge) {
+            int sa = 0, sb = 0, sc = 0;
+            if constexpr (spec::GA) { if (c.ia < spec::RA) sa = spec::NA; else if (c.ia >= spec::NA - spec::RA) sa = -spec::NA; }
+            if constexpr (spec::GB) { if (c.ib < spec::RB) sb = spec::NB * ROW; else if (c.ib >= spec::NB - spec::RB) sb = -spec::NB * ROW; }
+            if constexpr (spec::GC) { if (c.ic < spec::RC) sc = spec::NC * PLANE; else if (c.ic >= spec::NC - spec::RC) sc = -spec::NC * PLANE; }
 #pragma unroll
             for (int m = 1; m < 8; ++m) {
                 if (((m & 1) && !sa) || ((m & 2) && !sb) || ((m & 4) && !sc)) continue;
@@ -90,19 +101,21 @@ template <int B, int NCONF, class Acc>
 __device__ __forceinline__ void force(const Acc &cfg, const double (&own)[NCONF][3], double (&F)[NCONF][3]) {
 #pragma unroll
     for (int k = 0; k < NCONF; ++k) {
-        if constexpr (spec::ZEE[B][0] != 0.0) F[k][0] += spec::ZEE[B][0];
-        if constexpr (spec::ZEE[B][1] != 0.0) F[k][1] += spec::ZEE[B][1];
-        if constexpr (spec::ZEE[B][2] != 0.0) F[k][2] += spec::ZEE[B][2];
+        // spec:: holds the values as constexpr (zero terms vanish at compile time); specc:: holds the same values in constant
+        // memory, from where an fp64 instruction reads them as an operand (a 64-bit immediate would cost two extra moves)
+        if constexpr (spec::ZEE[B][0] != 0.0) F[k][0] += specc::ZEE[B][0];
+        if constexpr (spec::ZEE[B][1] != 0.0) F[k][1] += specc::ZEE[B][1];
+        if constexpr (spec::ZEE[B][2] != 0.0) F[k][2] += specc::ZEE[B][2];
         if constexpr (spec::K2[B] != 0.0) {
-            constexpr double kx = spec::KAX[B][0], ky = spec::KAX[B][1], kz = spec::KAX[B][2];
+            constexpr bool hx = spec::KAX[B][0] != 0.0, hy = spec::KAX[B][1] != 0.0, hz = spec::KAX[B][2] != 0.0;
             double p = 0.0;
-            if constexpr (kx != 0.0) p = fma(kx, own[k][0], p);
-            if constexpr (ky != 0.0) p = fma(ky, own[k][1], p);
-            if constexpr (kz != 0.0) p = fma(kz, own[k][2], p);
-            p *= spec::K2[B];
-            if constexpr (kx != 0.0) F[k][0] = fma(p, kx, F[k][0]);
-            if constexpr (ky != 0.0) F[k][1] = fma(p, ky, F[k][1]);
-            if constexpr (kz != 0.0) F[k][2] = fma(p, kz, F[k][2]);
+            if constexpr (hx) p = fma(specc::KAX[B][0], own[k][0], p);
+            if constexpr (hy) p = fma(specc::KAX[B][1], own[k][1], p);
+            if constexpr (hz) p = fma(specc::KAX[B][2], own[k][2], p);
+            p *= specc::K2[B];
+            if constexpr (hx) F[k][0] = fma(p, specc::KAX[B][0], F[k][0]);
+            if constexpr (hy) F[k][1] = fma(p, specc::KAX[B][1], F[k][1]);
+            if constexpr (hz) F[k][2] = fma(p, specc::KAX[B][2], F[k][2]);
         }
     }
     static_for<spec::PAIR_BEGIN[B], spec::PAIR_BEGIN[B + 1]>([&](auto e) {
@@ -113,10 +126,10 @@ __device__ __forceinline__ void force(const Acc &cfg, const double (&own)[NCONF]
             double p[3];
             cfg.template load<B, spec::P_BJ[E], spec::P_DA[E], spec::P_DB[E], spec::P_DC[E]>(k, p);
             // J n_j + n_j x D, zero components dropped at compile time
-            if constexpr (J != 0.0) { F[k][0] = fma(J, p[0], F[k][0]); F[k][1] = fma(J, p[1], F[k][1]); F[k][2] = fma(J, p[2], F[k][2]); }
-            if constexpr (Dz != 0.0) { F[k][0] = fma(p[1], Dz, F[k][0]); F[k][1] = fma(p[0], -Dz, F[k][1]); }
-            if constexpr (Dy != 0.0) { F[k][0] = fma(p[2], -Dy, F[k][0]); F[k][2] = fma(p[0], Dy, F[k][2]); }
-            if constexpr (Dx != 0.0) { F[k][1] = fma(p[2], Dx, F[k][1]); F[k][2] = fma(p[1], -Dx, F[k][2]); }
+            if constexpr (J != 0.0) { const double j = specc::P_J[E]; F[k][0] = fma(j, p[0], F[k][0]); F[k][1] = fma(j, p[1], F[k][1]); F[k][2] = fma(j, p[2], F[k][2]); }
+            if constexpr (Dz != 0.0) { const double d = specc::P_DZ[E]; F[k][0] = fma(p[1], d, F[k][0]); F[k][1] = fma(p[0], -d, F[k][1]); }
+            if constexpr (Dy != 0.0) { const double d = specc::P_DY[E]; F[k][0] = fma(p[2], -d, F[k][0]); F[k][2] = fma(p[0], d, F[k][2]); }
+            if constexpr (Dx != 0.0) { const double d = specc::P_DX[E]; F[k][1] = fma(p[2], d, F[k][1]); F[k][2] = fma(p[1], -d, F[k][2]); }
         }
     });
     static_for<spec::QUAD_BEGIN[B], spec::QUAD_BEGIN[B + 1]>([&](auto e) {
@@ -127,7 +140,7 @@ __device__ __forceinline__ void force(const Acc &cfg, const double (&own)[NCONF]
             cfg.template load<B, spec::Q_B[E][0], spec::Q_D[E][0], spec::Q_D[E][1], spec::Q_D[E][2]>(k, P);
             cfg.template load<B, spec::Q_B[E][1], spec::Q_D[E][3], spec::Q_D[E][4], spec::Q_D[E][5]>(k, Q);
             cfg.template load<B, spec::Q_B[E][2], spec::Q_D[E][6], spec::Q_D[E][7], spec::Q_D[E][8]>(k, R);
-            const double w = spec::Q_K[E] * fma(Q[0], R[0], fma(Q[1], R[1], Q[2] * R[2]));
+            const double w = specc::Q_K[E] * fma(Q[0], R[0], fma(Q[1], R[1], Q[2] * R[2]));
             F[k][0] = fma(w, P[0], F[k][0]); F[k][1] = fma(w, P[1], F[k][1]); F[k][2] = fma(w, P[2], F[k][2]);
         }
     });
@@ -144,7 +157,7 @@ __device__ __forceinline__ void stt_gradient(const Acc &cfg, const Coord &c, con
             constexpr int EXT = D == 0 ? spec::NA : (D == 1 ? spec::NB : spec::NC);
             const int x = D == 0 ? c.ia : (D == 1 ? c.ib : c.ic);
             const bool hp = PER || x + 1 < EXT, hm = PER || x > 0;
-            const double w = spec::STT_C[D] * ((hp && hm) ? 0.5 : ((hp || hm) ? 1.0 : 0.0));
+            const double w = specc::STT_C[D] * ((hp && hm) ? 0.5 : ((hp || hm) ? 1.0 : 0.0));
 #pragma unroll
             for (int k = 0; k < NCONF; ++k) {
                 double vp[3], vm[3];
@@ -162,16 +175,16 @@ __device__ __forceinline__ void stt_gradient(const Acc &cfg, const Coord &c, con
 // A = pre [F + alpha n x F] + stt_s s + stt_x n x s   (Eq. 10 as dn/dt = n x A)
 template <int B>
 __device__ __forceinline__ void rotation_field(const double (&n)[3], const double (&F)[3], const double (&sg)[3], double (&A)[3]) {
-    constexpr double pre = spec::PRE[B], pa = spec::PRE[B] * spec::ALPHA;
+    const double pre = specc::PRE[B], pa = specc::PREA[B];
     const double cx = fma(n[1], F[2], -n[2] * F[1]), cy = fma(n[2], F[0], -n[0] * F[2]), cz = fma(n[0], F[1], -n[1] * F[0]);
     A[0] = fma(pa, cx, pre * F[0]);
     A[1] = fma(pa, cy, pre * F[1]);
     A[2] = fma(pa, cz, pre * F[2]);
     if constexpr (spec::STT_ON) {
         const double sx = fma(n[1], sg[2], -n[2] * sg[1]), sy = fma(n[2], sg[0], -n[0] * sg[2]), sz = fma(n[0], sg[1], -n[1] * sg[0]);
-        A[0] += fma(spec::STT_X, sx, spec::STT_S * sg[0]);
-        A[1] += fma(spec::STT_X, sy, spec::STT_S * sg[1]);
-        A[2] += fma(spec::STT_X, sz, spec::STT_S * sg[2]);
+        A[0] += fma(specc::STT_X, sx, specc::STT_S * sg[0]);
+        A[1] += fma(specc::STT_X, sy, specc::STT_S * sg[1]);
+        A[2] += fma(specc::STT_X, sz, specc::STT_S * sg[2]);
     }
 }
 
@@ -190,13 +203,26 @@ __device__ __forceinline__ bool locate(Coord &c, int &idx) {
     return (c.ia < spec::NA) && (c.ib < spec::NB) && (c.ic < spec::NC);
 }
 
+// L2 prefetch of the lines a later wave of blocks will read: spec::PF_PLANES lattice planes ahead of the own site (0 = off).
+// One lane per 128-byte line issues it (the rows start on line boundaries); no registers are tied up.
+__device__ __forceinline__ void prefetch_ahead(const double *__restrict__ q, const Coord &c) {
+    if constexpr (spec::PF_PLANES > 0) {
+        if ((c.ia & 15) == 0 && c.ic + spec::PF_PLANES < spec::NC) {
+            const double *t = q + spec::PF_PLANES * PLANE;
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(t));
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(t + spec::PA));
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(t + 2 * spec::PA));
+        }
+    }
+}
+
 template <int B>
 __device__ __forceinline__ void thermal_force(const Coord &c, u64 step, u32 seed_lo, u32 seed_hi, double (&f)[3]) {
     if constexpr (spec::THERMAL_ON) {
         const u32 cell = (u32)(c.ia + spec::NA * c.ib + (spec::NA * spec::NB) * c.ic);
         double xi[3];
         spin::thermal_xi(seed_lo, seed_hi, step, (u32)B + (u32)spec::NBASIS * cell, xi);
-        f[0] = spec::SIGMA[B] * xi[0]; f[1] = spec::SIGMA[B] * xi[1]; f[2] = spec::SIGMA[B] * xi[2];
+        f[0] = specc::SIGMA[B] * xi[0]; f[1] = specc::SIGMA[B] * xi[1]; f[2] = specc::SIGMA[B] * xi[2];
     } else {
         f[0] = -0.0; f[1] = -0.0; f[2] = -0.0;      // additive identity that the compiler may fold away (x + -0.0 == x exactly)
     }
@@ -208,16 +234,26 @@ __device__ __forceinline__ void predictor_body(const double *__restrict__ n, con
     Coord c;
     int idx;
     if (!locate<B>(c, idx)) return;
+    prefetch_ahead(n + idx, c);
     const GlobalAcc<1> cfg = {{n + idx}};
     double own[1][3], F[1][3], sg[1][3] = {{0.0, 0.0, 0.0}};
     load3<0>(cfg.cfg[0], own[0]);
     thermal_force<B>(c, step, seed_lo, seed_hi, F[0]);
+#if !(SPIN_ABLATE & 1)
     force<B, 1>(cfg, own, F);
+#endif
     if constexpr (spec::HAS_DDI) { double d[3]; load3<0>(fddi + idx, d); F[0][0] += d[0]; F[0][1] += d[1]; F[0][2] += d[2]; }
     if constexpr (spec::STT_ON) stt_gradient<B, 1>(cfg, c, own, sg);
     double A[3], out[3];
+#if SPIN_ABLATE & 4
+    out[0] = own[0][0] + F[0][0]; out[1] = own[0][1] + F[0][1]; out[2] = own[0][2] + F[0][2];
+#else
     rotation_field<B>(own[0], F[0], sg[0], A);
-    spin::rodrigues(A, spec::DT, spec::DT2, own[0], out);
+    spin::rodrigues(A, specc::DT, specc::DT2, own[0], out);
+#endif
+#if SPIN_ABLATE & 2
+    if (out[0] == 123.456)
+#endif
     store_spin(np + idx, c, out);
     if constexpr (spec::STORE_A) store3(Aout + idx, A);
 }
@@ -229,6 +265,8 @@ __device__ __forceinline__ void corrector_body(const double *__restrict__ n, con
     Coord c;
     int idx;
     if (!locate<B>(c, idx)) return;
+    prefetch_ahead(n + idx, c);
+    prefetch_ahead(np + idx, c);
     double th[3], A[3], Ap[3], n0[3];
     thermal_force<B>(c, step, seed_lo, seed_hi, th);
     load3<0>(n + idx, n0);
@@ -256,9 +294,10 @@ __device__ __forceinline__ void corrector_body(const double *__restrict__ n, con
         rotation_field<B>(own[0], F[0], sg[0], A);
         rotation_field<B>(own[1], F[1], sg[1], Ap);
     }
-    const double Ac[3] = {0.5 * (A[0] + Ap[0]), 0.5 * (A[1] + Ap[1]), 0.5 * (A[2] + Ap[2])};
+    // A^c = (A + A^p)/2: the factor 1/2 is folded into the time step (dt/2, dt^2/4 are exact scalings, the result is bit-identical)
+    const double Ac[3] = {A[0] + Ap[0], A[1] + Ap[1], A[2] + Ap[2]};
     double out[3];
-    spin::rodrigues(Ac, spec::DT, spec::DT2, n0, out);
+    spin::rodrigues(Ac, specc::HDT, specc::QDT2, n0, out);
     spin::renormalise(out);
     store_spin(nout + idx, c, out);
 }
@@ -273,7 +312,7 @@ __device__ __forceinline__ void dispatch_basis(int b, Fn &&fn) {
 
 }  // namespace spinjit
 
-extern "C" __global__ void __launch_bounds__(spec::BX *spec::BY *spec::BZ)
+extern "C" __global__ void __launch_bounds__(spec::BX *spec::BY *spec::BZ, SPIN_MINBLOCKS)
     jit_predictor(const double *__restrict__ n, const double *__restrict__ fddi, double *__restrict__ np, double *__restrict__ Aout,
                   const unsigned long long *__restrict__ d_step, unsigned int step_add, unsigned int seed_lo, unsigned int seed_hi) {
     const unsigned long long step = *d_step + step_add;
@@ -282,7 +321,7 @@ extern "C" __global__ void __launch_bounds__(spec::BX *spec::BY *spec::BZ)
     });
 }
 
-extern "C" __global__ void __launch_bounds__(spec::BX *spec::BY *spec::BZ)
+extern "C" __global__ void __launch_bounds__(spec::BX *spec::BY *spec::BZ, SPIN_MINBLOCKS)
     jit_corrector(const double *__restrict__ n, const double *__restrict__ np, const double *__restrict__ fddi_n,
                   const double *__restrict__ fddi_np, const double *__restrict__ Ain, double *__restrict__ nout,
                   const unsigned long long *__restrict__ d_step, unsigned int step_add, unsigned int seed_lo, unsigned int seed_hi) {

@@ -11,7 +11,7 @@
 // Results are written straight to global memory (coalesced rows, periodic images included, as in the brick kernels).
 // The arithmetic is the same code as the brick kernels (force<>, rotation_field<>, rodrigues): only the accessor differs.
 //
-// spec must also define: struct TmaP, struct TmaC, each with static constexpr int TBX, TBY, RING, LOOK, NZC, CZ.
+// spec must also define: struct TmaP, struct TmaC, each with static constexpr int TBX, TBY, KZ, RING, LOOK, NZC, CZ.
 #pragma once
 
 namespace spintma {
@@ -22,7 +22,7 @@ struct __align__(64) TensorMap { unsigned long long opaque[16]; };      // CUten
 // geometry of one sweep's staging; G (spec::TmaP for the predictor, spec::TmaC for the corrector) gives TBX, TBY, RING, LOOK, NZC, CZ
 template <class G>
 struct Geo {
-    static constexpr int TBX = G::TBX, TBY = G::TBY, RING = G::RING, LOOK = G::LOOK, NZC = G::NZC, CZ = G::CZ;
+    static constexpr int TBX = G::TBX, TBY = G::TBY, RING = G::RING, LOOK = G::LOOK, NZC = G::NZC, CZ = G::CZ, KZ = G::KZ;
     static constexpr int HX = (spec::RA + 1) / 2 * 2;                     // rim along a, even: TMA needs 16-byte aligned box rows in global memory
     static constexpr int WX = TBX + 2 * HX, WY = TBY + 2 * spec::RB;      // staged box: cells incl. the ghost rim
     static constexpr int SROW = 3 * WX;                                   // doubles between rows of a staged plane (x, y, z runs)
@@ -32,8 +32,8 @@ struct Geo {
     static constexpr int NTX = (spec::NA + TBX - 1) / TBX, NTY = (spec::NB + TBY - 1) / TBY;
     static constexpr int NITEMS = NTX * NTY * NZC;                        // work items: column x chunk
     static constexpr int PL = CZ + 2 * spec::RC;                          // planes staged per item
-    static constexpr int NTHREADS = TBX * TBY;
-    static_assert(RING >= LOOK + 2 * spec::RC + 1, "ring too small for the look-ahead");
+    static constexpr int NTHREADS = TBX * TBY * KZ;
+    static_assert(RING >= LOOK + KZ + 2 * spec::RC && LOOK % KZ == 0, "ring too small for the look-ahead");
     static_assert((WX * 8) % 16 == 0, "TMA box rows must be multiples of 16 bytes");
 };
 
@@ -99,10 +99,11 @@ __device__ __forceinline__ void issue(int q, const TensorMap *const (&tm)[NARR],
 }
 
 // The marching loop shared by both sweeps: body(c, acc) is called once per thread and computed plane with
-// acc.off[a][dz + RC] set for every staged array a.
+// acc.off[a][dz + RC] set for every staged array a.  KZ consecutive stream positions are computed per iteration, one per
+// group of TBX*TBY threads (more warps per staged byte); LOOK is a multiple of KZ, RING >= LOOK + KZ + 2 RC.
 template <class G, int NARR, class Body>
 __device__ __forceinline__ void march(const TensorMap *const (&tm)[NARR], Body &&body) {
-    constexpr int PL = Geo<G>::PL, ARR = Geo<G>::ARR, NITEMS = Geo<G>::NITEMS, SROW = Geo<G>::SROW;
+    constexpr int PL = Geo<G>::PL, ARR = Geo<G>::ARR, NITEMS = Geo<G>::NITEMS, SROW = Geo<G>::SROW, KZ = G::KZ, NT2 = G::TBX * G::TBY;
     u64 *bar_mem = (u64 *)(smem + G::RING * NARR * ARR);
     const u32 bars = smem_u32(bar_mem);
     const int tid = threadIdx.x;
@@ -115,28 +116,36 @@ __device__ __forceinline__ void march(const TensorMap *const (&tm)[NARR], Body &
     __syncthreads();
     if (tid == 0)
         for (int q = 0; q < G::LOOK && q < Q; ++q) issue<G, NARR>(q, tm, bars);
-    const int txi = tid % G::TBX, tyi = tid / G::TBX;
+    const int kz = tid / NT2, t2 = tid - kz * NT2;
+    const int txi = t2 % G::TBX, tyi = t2 / G::TBX;
     const int cell = (tyi + spec::RB) * SROW + (txi + Geo<G>::HX);
-    for (int q = 0; q < Q; ++q) {
-        if (tid == 0 && q + G::LOOK < Q) issue<G, NARR>(q + G::LOOK, tm, bars);     // its slot was released by the barrier below
-        mbar_wait(bars + 8u * (q % G::RING), (u32)((q / G::RING) & 1));
-        const int j = q / PL, p = q - j * PL;
-        if (p >= 2 * spec::RC) {                       // planes z-RC .. z+RC of this item are staged: compute plane z
-            const Item it = item_of<G>(j);
-            Coord c;
-            c.ia = it.x0 + txi; c.ib = it.y0 + tyi; c.ic = it.z0 + p - 2 * spec::RC;
-            if (c.ia < spec::NA && c.ib < spec::NB && c.ic < spec::NC) {
-                RingAcc<G, NARR> acc;
+    for (int q0 = 0; q0 < Q; q0 += KZ) {
+        if (tid == 0) {                                 // the slots of these positions were released by the barrier below
 #pragma unroll
-                for (int dz = -spec::RC; dz <= spec::RC; ++dz) {
-                    const int slot = (q - spec::RC + dz) % G::RING;
+            for (int k = 0; k < KZ; ++k)
+                if (q0 + G::LOOK + k < Q) issue<G, NARR>(q0 + G::LOOK + k, tm, bars);
+        }
+        const int q = q0 + kz;
+        if (q < Q) {
+            for (int k = 0; k <= kz; ++k) mbar_wait(bars + 8u * ((q0 + k) % G::RING), (u32)(((q0 + k) / G::RING) & 1));
+            const int j = q / PL, p = q - j * PL;
+            if (p >= 2 * spec::RC) {                   // planes z-RC .. z+RC of this item are staged: compute plane z
+                const Item it = item_of<G>(j);
+                Coord c;
+                c.ia = it.x0 + txi; c.ib = it.y0 + tyi; c.ic = it.z0 + p - 2 * spec::RC;
+                if (c.ia < spec::NA && c.ib < spec::NB && c.ic < spec::NC) {
+                    RingAcc<G, NARR> acc;
 #pragma unroll
-                    for (int a = 0; a < NARR; ++a) acc.off[a][dz + spec::RC] = (slot * NARR + a) * ARR + cell;
+                    for (int dz = -spec::RC; dz <= spec::RC; ++dz) {
+                        const int slot = (q - spec::RC + dz) % G::RING;
+#pragma unroll
+                        for (int a = 0; a < NARR; ++a) acc.off[a][dz + spec::RC] = (slot * NARR + a) * ARR + cell;
+                    }
+                    body(c, acc);
                 }
-                body(c, acc);
             }
         }
-        __syncthreads();                               // every thread is done with the oldest plane: its slot may be refilled
+        __syncthreads();                               // every thread is done with the oldest planes: their slots may be refilled
     }
 }
 
@@ -159,12 +168,21 @@ extern "C" __global__ void __launch_bounds__(spintma::Geo<spec::TmaP>::NTHREADS)
             double own[1][3], F[1][3], sg[1][3] = {{0.0, 0.0, 0.0}};
             acc.template load<B, B, 0, 0, 0>(0, own[0]);
             thermal_force<B>(c, step, seed_lo, seed_hi, F[0]);
+#if !(SPIN_ABLATE & 1)
             force<B, 1>(acc, own, F);
+#endif
             if constexpr (spec::HAS_DDI) { double d[3]; load3<0>(fddi + idx, d); F[0][0] += d[0]; F[0][1] += d[1]; F[0][2] += d[2]; }
             if constexpr (spec::STT_ON) stt_gradient<B, 1>(acc, c, own, sg);
             double A[3], out[3];
+#if SPIN_ABLATE & 4
+            out[0] = own[0][0] + F[0][0]; out[1] = own[0][1] + F[0][1]; out[2] = own[0][2] + F[0][2];
+#else
             rotation_field<B>(own[0], F[0], sg[0], A);
-            spin::rodrigues(A, spec::DT, spec::DT2, own[0], out);
+            spin::rodrigues(A, specc::DT, specc::DT2, own[0], out);
+#endif
+#if SPIN_ABLATE & 2
+            if (out[0] == 123.456)
+#endif
             store_spin(np + idx, c, out);
         });
     });
@@ -195,9 +213,9 @@ extern "C" __global__ void __launch_bounds__(spintma::Geo<spec::TmaC>::NTHREADS)
             if constexpr (spec::STT_ON) stt_gradient<B, 2>(acc, c, own, sg);
             rotation_field<B>(own[0], F[0], sg[0], A);
             rotation_field<B>(own[1], F[1], sg[1], Ap);
-            const double Ac[3] = {0.5 * (A[0] + Ap[0]), 0.5 * (A[1] + Ap[1]), 0.5 * (A[2] + Ap[2])};
+            const double Ac[3] = {A[0] + Ap[0], A[1] + Ap[1], A[2] + Ap[2]};      // the 1/2 is folded into dt (exact)
             double out[3];
-            spin::rodrigues(Ac, spec::DT, spec::DT2, own[0], out);
+            spin::rodrigues(Ac, specc::HDT, specc::QDT2, own[0], out);
             spin::renormalise(out);
             store_spin(nout + idx, c, out);
         });
