@@ -175,6 +175,8 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
+    from paper_1901_11350_b200 import replicas
+    w = replicas.replica_workload(w, rank)          # N > 1: independent replicas, one per rank (no data-path collective)
     stream = torch.cuda.Stream()
     n0 = w.initial_spins()
     sys_ = P.SpinSystem.from_workload(w, stream=stream.cuda_stream)
@@ -203,11 +205,8 @@ def main():
     ms = ev0.elapsed_time(ev1)
     l1, f1 = sys_.spin_launch_counts()
     clocks = sampler.stop() if rank == 0 else None
-    t = torch.tensor([ms], device="cuda", dtype=torch.float64)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms_max = float(t.item())
-    value = world * N * inner * args.steps / (ms_max * 1e-3)
+    ms_max = replicas.max_over_ranks(ms, device="cuda")
+    value = replicas.whole_job_rate(N, inner * args.steps, ms_max, world)
 
     # ---------------- end to end through host buffers (pinned), copies inside the timed region
     host_in = torch.from_numpy(n0.copy()).pin_memory()
@@ -225,10 +224,7 @@ def main():
     ee1.record(stream)
     barrier()
     e2e_ms = ee0.elapsed_time(ee1)      # events on the launching stream bracket copies + kernels; the host blocks on each copy
-    te = torch.tensor([e2e_ms], device="cuda", dtype=torch.float64)
-    if world > 1:
-        dist.all_reduce(te, op=dist.ReduceOp.MAX)
-    e2e_value = world * N * inner * e2e_steps / (float(te.item()) * 1e-3)
+    e2e_value = replicas.whole_job_rate(N, inner * e2e_steps, replicas.max_over_ranks(e2e_ms, device="cuda"), world)
 
     # ---------------- per-kernel split (events around every launch, plain launches) -> live duration of the dominant kernel
     sys_.spin_profile_enable(True)
@@ -254,12 +250,12 @@ def main():
             "config": {"workload": w.name, "spins": N, "llg_iterations_per_step": inner, "solver": "Depondt", "parallelism": f"replicas x{world}",
                        "l2": "state arrays n, n^p, n' = %.0f MB > 126 MB L2 (no flush needed)" % (3 * 24 * N / 1e6) if 72 * N > 126e6 else
                              "state %.1f MB is L2-resident; effective bandwidth reported" % (3 * 24 * N / 1e6),
-                       "store_A": args.store_A},
+                       "store_A": args.store_A, "kernels": sys_.spin_kernel_info()},
             "clocks": clocks,
             "e2e": {"value": e2e_value, "unit": "spin-updates/s", "h2d_bytes_per_step": int(host_in.numel() * 8), "d2h_bytes_per_step": int(host_out.numel() * 8),
                     "steps": e2e_steps},
             "gpu_launches": int(l1 - l0), "cufft_execs": int(f1 - f0),
-            "roofline": {"bound": "hbm", "kernel": "corrector_kernel", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+            "roofline": {"bound": "hbm", "kernel": "jit_corrector" if sys_.spin_kernel_info().startswith("jit") else "corrector_kernel", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                          "peak_source": peak_src, "traffic": committed_traffic(w.name),
                          "algorithmic_bytes_per_launch": ALG_BYTES_CORRECTOR * N, "launch_ms": corr_live_ms,
                          "kernel_share_of_step": per_iter["corrector"] / tot,

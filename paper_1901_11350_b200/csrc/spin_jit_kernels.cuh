@@ -22,8 +22,10 @@
 #ifndef SPIN_ABLATE
 #define SPIN_ABLATE 0
 #endif
-#ifndef SPIN_MINBLOCKS
-#define SPIN_MINBLOCKS 1
+#ifdef SPIN_MINBLOCKS
+#define SPIN_BOUNDS(t) __launch_bounds__(t, SPIN_MINBLOCKS)
+#else
+#define SPIN_BOUNDS(t) __launch_bounds__(t)
 #endif
 #include "spin_device_math.cuh"
 
@@ -312,7 +314,7 @@ __device__ __forceinline__ void dispatch_basis(int b, Fn &&fn) {
 
 }  // namespace spinjit
 
-extern "C" __global__ void __launch_bounds__(spec::BX *spec::BY *spec::BZ, SPIN_MINBLOCKS)
+extern "C" __global__ void SPIN_BOUNDS(spec::BX *spec::BY *spec::BZ)
     jit_predictor(const double *__restrict__ n, const double *__restrict__ fddi, double *__restrict__ np, double *__restrict__ Aout,
                   const unsigned long long *__restrict__ d_step, unsigned int step_add, unsigned int seed_lo, unsigned int seed_hi) {
     const unsigned long long step = *d_step + step_add;
@@ -321,7 +323,7 @@ extern "C" __global__ void __launch_bounds__(spec::BX *spec::BY *spec::BZ, SPIN_
     });
 }
 
-extern "C" __global__ void __launch_bounds__(spec::BX *spec::BY *spec::BZ, SPIN_MINBLOCKS)
+extern "C" __global__ void SPIN_BOUNDS(spec::BX *spec::BY *spec::BZ)
     jit_corrector(const double *__restrict__ n, const double *__restrict__ np, const double *__restrict__ fddi_n,
                   const double *__restrict__ fddi_np, const double *__restrict__ Ain, double *__restrict__ nout,
                   const unsigned long long *__restrict__ d_step, unsigned int step_add, unsigned int seed_lo, unsigned int seed_hi) {

@@ -281,3 +281,27 @@ def test_tma_sweeps_match_oracle(P, O, cfg, cells, steps, geo, monkeypatch):
     assert b.spin_kernel_info().startswith("jit (brick")
     b.llg_iterate(steps)
     assert np.array_equal(b.spins_get(), g.spins_get())
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# BASELINE.json's full sizes in the launch configuration bench.py times (specialised kernels, CUDA-graph replay of 16-step
+# batches).  The oracle computes the whole lattice for the field; trajectories run as many steps as it finishes in seconds.
+FULL_SIZE = [(2, 2000), (3, 48), (4, 200), (5, 4)]
+
+
+@pytest.mark.parametrize("cfg,steps", FULL_SIZE)
+def test_full_size_configs(P, O, cfg, steps):
+    w = W.CONFIGS[cfg]()
+    g, o = pair(P, O, w)
+    assert g.spin_kernel_info().startswith("jit"), g.spin_kernel_info()
+    Bg, Bo = g.effective_field(), o.effective_field()
+    assert_fields_close(Bg, Bo)
+    Eg, Tg = g.energy()
+    To = o.energy_terms()
+    assert np.abs(Tg - To).max() <= ENERGY_RTOL * np.abs(To).sum(), (Tg, To)
+    g.llg_iterate(steps); o.iterate(steps)
+    ng, no = g.spins_get(), o.spins()
+    d = np.abs(ng - no).max()
+    print(f"cfg{cfg} full size {w.n_cells} ({w.n_spins} spins) steps={steps}: max|dn| = {d:.3e}")
+    assert d <= SPIN_ATOL
+    assert np.abs(np.linalg.norm(ng, axis=1) - 1).max() < 4e-16
