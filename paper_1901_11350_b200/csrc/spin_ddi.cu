@@ -28,6 +28,13 @@ struct DdiState {
     cufftDoubleComplex *d_Mhat, *d_Hhat;   // [nb*3][Phalf]
     cufftDoubleComplex *d_Khat;            // [nb*nb][6][Phalf]
     double *d_geom;            // small device copy: bravais*alat (9), basis (3*nb), mu (nb)
+    // ---- slab path (thin films, one basis atom): cuFFT transforms the a-b planes only (2-D, batched over the occupied
+    // c-planes); the short transform along c, the tensor contraction and the inverse transform along c are one kernel.
+    bool slab;
+    int NZ, PZ;                // occupied planes, padded length along c (PZ = 2 NZ, or 1)
+    int64_t S2, R2;            // complex / real points of one a-b plane: P1*(P0/2+1), P1*P0
+    cufftHandle plan2_r2c, plan2_c2r;
+    double *d_Kre;             // [6][PZ][S2] real: the tensor spectrum is real for a single basis atom (the kernel is even)
 };
 
 namespace {
@@ -75,6 +82,7 @@ __global__ void ddi_tensor_kernel(const __grid_constant__ DdiGeom G, int a, int 
 }
 
 // M_b padded <- mu_b n_b on the occupied corner (the rest of the array stays zero from allocation time)
+// (Ptot = stride between components: the whole padded grid, or NZ a-b planes on the slab path)
 __global__ void ddi_scatter_kernel(const __grid_constant__ DevicePlan L, const double *__restrict__ n, int P0, int P1, long long Ptot,
                                    const double *__restrict__ mu, double *__restrict__ Mpad) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;   // b*Ncell + cell, x fastest
@@ -136,6 +144,66 @@ __global__ void complex_to_real_kernel(const cufftDoubleComplex *__restrict__ in
     if (i < n) out[i] = in[i].x;
 }
 
+// real part of a spectrum (slab path: the tensor spectrum of a single basis atom is real)
+__global__ void real_part_kernel(const cufftDoubleComplex *__restrict__ in, double *__restrict__ out, long long n) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) out[i] = in[i].x;
+}
+
+// twiddles exp(-2 pi i j / PZ), j < PZ <= 16
+__constant__ double DDI_WR[16], DDI_WI[16];
+
+// Slab path, one thread per in-plane wave vector q = (kx, ky):
+//   M^(kz) = sum_{z < NZ} M2(z) w^(kz z)          (pruned transform along c: planes z >= NZ are zero padding)
+//   H^(kz) = K^(kz) . M^(kz)                      (6-component real symmetric tensor)
+//   H2(z)  = sum_{kz < PZ} H^(kz) w^(-kz z),  z < NZ only
+// M2 / H2: [3][NZ][S2] complex (the 2-D spectra of the occupied planes); Kre: [6][PZ][S2].
+template <int NZ, int PZ>
+__global__ void __launch_bounds__(128) ddi_slab_contract_kernel(const double *__restrict__ Kre, const cufftDoubleComplex *__restrict__ M2,
+                                                                 cufftDoubleComplex *__restrict__ H2, long long S2) {
+    const long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (q >= S2) return;
+    double mr[3][NZ], mi[3][NZ], hr[3][NZ], hi[3][NZ];
+#pragma unroll
+    for (int c = 0; c < 3; ++c)
+#pragma unroll
+        for (int z = 0; z < NZ; ++z) {
+            const cufftDoubleComplex v = M2[(size_t)(c * NZ + z) * S2 + q];
+            mr[c][z] = v.x; mi[c][z] = v.y; hr[c][z] = 0.0; hi[c][z] = 0.0;
+        }
+#pragma unroll
+    for (int kz = 0; kz < PZ; ++kz) {
+        double Mr[3], Mi[3];
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            double ar = 0.0, ai = 0.0;
+#pragma unroll
+            for (int z = 0; z < NZ; ++z) {
+                const double wr = DDI_WR[(kz * z) % PZ], wi = DDI_WI[(kz * z) % PZ];
+                ar = fma(mr[c][z], wr, fma(-mi[c][z], wi, ar));
+                ai = fma(mr[c][z], wi, fma(mi[c][z], wr, ai));
+            }
+            Mr[c] = ar; Mi[c] = ai;
+        }
+        const size_t o = (size_t)kz * S2 + q, st = (size_t)PZ * S2;
+        const double kxx = Kre[o], kxy = Kre[st + o], kxz = Kre[2 * st + o], kyy = Kre[3 * st + o], kyz = Kre[4 * st + o], kzz = Kre[5 * st + o];
+        const double Hr[3] = {kxx * Mr[0] + kxy * Mr[1] + kxz * Mr[2], kxy * Mr[0] + kyy * Mr[1] + kyz * Mr[2], kxz * Mr[0] + kyz * Mr[1] + kzz * Mr[2]};
+        const double Hi[3] = {kxx * Mi[0] + kxy * Mi[1] + kxz * Mi[2], kxy * Mi[0] + kyy * Mi[1] + kyz * Mi[2], kxz * Mi[0] + kyz * Mi[1] + kzz * Mi[2]};
+#pragma unroll
+        for (int c = 0; c < 3; ++c)
+#pragma unroll
+            for (int z = 0; z < NZ; ++z) {
+                const double wr = DDI_WR[(kz * z) % PZ], wi = -DDI_WI[(kz * z) % PZ];      // conjugate twiddle
+                hr[c][z] = fma(Hr[c], wr, fma(-Hi[c], wi, hr[c][z]));
+                hi[c][z] = fma(Hr[c], wi, fma(Hi[c], wr, hi[c][z]));
+            }
+    }
+#pragma unroll
+    for (int c = 0; c < 3; ++c)
+#pragma unroll
+        for (int z = 0; z < NZ; ++z) H2[(size_t)(c * NZ + z) * S2 + q] = make_cuDoubleComplex(hr[c][z], hi[c][z]);
+}
+
 #define SPIN_FFT(call)                                                                                         \
     do {                                                                                                       \
         cufftResult r__ = (call);                                                                              \
@@ -149,6 +217,8 @@ void spin::ddi_release(spin_system *s) {
     DdiState *d = s->ddi;
     if (!d) return;
     if (d->have_plans) { cufftDestroy(d->plan_r2c); cufftDestroy(d->plan_c2r); }
+    if (d->slab) { cufftDestroy(d->plan2_r2c); cufftDestroy(d->plan2_c2r); }
+    cudaFree(d->d_Kre);
     cudaFree(d->d_Mpad); cudaFree(d->d_Hpad); cudaFree(d->d_Mhat); cudaFree(d->d_Hhat); cudaFree(d->d_Khat); cudaFree(d->d_geom);
     delete d;
     s->ddi = nullptr;
@@ -167,7 +237,13 @@ int spin::ddi_prepare(spin_system *s) {
     for (int k = 2; k >= 0; --k) if (d->P[k] > 1) d->fdims[d->rank++] = d->P[k];
     d->Phalf = d->Ptot;
     if (d->rank > 0) { const int inner = d->fdims[d->rank - 1]; d->Phalf = d->Ptot / inner * (inner / 2 + 1); }
-    const size_t nreal = (size_t)nb * 3 * d->Ptot, ncplx = (size_t)nb * 3 * d->Phalf;
+    // slab path: one basis atom, both in-plane directions padded, at most 8 planes (power of two) along c
+    d->NZ = s->nc[2]; d->PZ = d->P[2];
+    d->R2 = (int64_t)d->P[0] * d->P[1]; d->S2 = (int64_t)d->P[1] * (d->P[0] / 2 + 1);
+    const bool want_slab = s->opt_ddi_slab && nb == 1 && d->P[0] > 1 && d->P[1] > 1 &&
+                           (d->PZ == 1 || d->PZ == 2 || d->PZ == 4 || d->PZ == 8 || d->PZ == 16);
+    size_t nreal = (size_t)nb * 3 * d->Ptot, ncplx = (size_t)nb * 3 * d->Phalf;
+    if (want_slab) { nreal = (size_t)3 * d->NZ * d->R2; ncplx = (size_t)3 * d->NZ * d->S2; }
     SPIN_CUDA(cudaMalloc(&d->d_Mpad, nreal * sizeof(double)));
     SPIN_CUDA(cudaMalloc(&d->d_Hpad, nreal * sizeof(double)));
     SPIN_CUDA(cudaMalloc(&d->d_Mhat, ncplx * sizeof(cufftDoubleComplex)));
@@ -177,12 +253,28 @@ int spin::ddi_prepare(spin_system *s) {
     SPIN_CUDA(cudaMemsetAsync(d->d_Mpad, 0, nreal * sizeof(double), s->stream));
     SPIN_CUDA(cudaMemcpyAsync(d->d_geom, s->mu.data(), nb * sizeof(double), cudaMemcpyHostToDevice, s->stream));
     cufftHandle plan6 = 0;
+    if (want_slab) {
+        int dims2[2] = {d->P[1], d->P[0]};
+        SPIN_FFT(cufftPlanMany(&d->plan2_r2c, 2, dims2, nullptr, 1, 0, nullptr, 1, 0, CUFFT_D2Z, 3 * d->NZ));
+        d->slab = true;      // from here on ddi_release destroys the 2-D plans
+        SPIN_FFT(cufftPlanMany(&d->plan2_c2r, 2, dims2, nullptr, 1, 0, nullptr, 1, 0, CUFFT_Z2D, 3 * d->NZ));
+        SPIN_FFT(cufftSetStream(d->plan2_r2c, s->stream));
+        SPIN_FFT(cufftSetStream(d->plan2_c2r, s->stream));
+        double wr[16], wi[16];
+        for (int j = 0; j < 16; ++j) { wr[j] = cos(-2.0 * M_PI * j / d->PZ); wi[j] = sin(-2.0 * M_PI * j / d->PZ); }
+        // exact values at the multiples of a quarter turn
+        for (int j = 0; j < d->PZ; ++j) if ((4 * j) % d->PZ == 0) { const int k = (4 * j) / d->PZ; wr[j] = k == 0 ? 1 : k == 2 ? -1 : 0; wi[j] = k == 1 ? -1 : k == 3 ? 1 : 0; }
+        SPIN_CUDA(cudaMemcpyToSymbolAsync(DDI_WR, wr, sizeof(wr), 0, cudaMemcpyHostToDevice, s->stream));
+        SPIN_CUDA(cudaMemcpyToSymbolAsync(DDI_WI, wi, sizeof(wi), 0, cudaMemcpyHostToDevice, s->stream));
+    }
     if (d->rank > 0) {
-        SPIN_FFT(cufftPlanMany(&d->plan_r2c, d->rank, d->fdims, nullptr, 1, 0, nullptr, 1, 0, CUFFT_D2Z, nb * 3));
-        SPIN_FFT(cufftPlanMany(&d->plan_c2r, d->rank, d->fdims, nullptr, 1, 0, nullptr, 1, 0, CUFFT_Z2D, nb * 3));
-        d->have_plans = true;
-        SPIN_FFT(cufftSetStream(d->plan_r2c, s->stream));
-        SPIN_FFT(cufftSetStream(d->plan_c2r, s->stream));
+        if (!want_slab) {
+            SPIN_FFT(cufftPlanMany(&d->plan_r2c, d->rank, d->fdims, nullptr, 1, 0, nullptr, 1, 0, CUFFT_D2Z, nb * 3));
+            SPIN_FFT(cufftPlanMany(&d->plan_c2r, d->rank, d->fdims, nullptr, 1, 0, nullptr, 1, 0, CUFFT_Z2D, nb * 3));
+            d->have_plans = true;
+            SPIN_FFT(cufftSetStream(d->plan_r2c, s->stream));
+            SPIN_FFT(cufftSetStream(d->plan_c2r, s->stream));
+        }
         SPIN_FFT(cufftPlanMany(&plan6, d->rank, d->fdims, nullptr, 1, 0, nullptr, 1, 0, CUFFT_D2Z, 6));
         SPIN_FFT(cufftSetStream(plan6, s->stream));
     }
@@ -203,10 +295,17 @@ int spin::ddi_prepare(spin_system *s) {
             if (d->rank > 0) { SPIN_FFT(cufftExecD2Z(plan6, d_K6, dst)); s->n_fft++; }
             else { real_to_complex_kernel<<<1, 32, 0, s->stream>>>(d_K6, dst, 6); s->n_launch++; }
         }
+    if (want_slab) {       // keep the real part only (exactly real for one basis atom: K(-Delta) = K(Delta))
+        const long long nk = (long long)6 * d->Phalf;
+        SPIN_CUDA(cudaMalloc(&d->d_Kre, (size_t)nk * sizeof(double)));
+        real_part_kernel<<<(unsigned)((nk + 255) / 256), 256, 0, s->stream>>>(d->d_Khat, d->d_Kre, nk);
+        s->n_launch++;
+    }
     SPIN_CUDA(cudaStreamSynchronize(s->stream));
     SPIN_CUDA(cudaGetLastError());
     cudaFree(d_K6);
     if (plan6) cufftDestroy(plan6);
+    if (want_slab) { cudaFree(d->d_Khat); d->d_Khat = nullptr; }
     return SPIN_OK;
 }
 
@@ -215,6 +314,23 @@ int spin::ddi_field(spin_system *s, const double *d_n, double *d_f) {
     if (!d) return spin::fail(SPIN_ERR_STATE, "dipolar plan missing");
     const int nb = s->nb, Ncell = (int)s->ncell, nspin = nb * Ncell, nt = 256;
     const unsigned gs = (unsigned)((nspin + nt - 1) / nt);
+    if (d->slab) {
+        const long long cs = (long long)d->NZ * d->R2;        // stride between components: the occupied planes only
+        ddi_scatter_kernel<<<gs, nt, 0, s->stream>>>(s->plan, d_n, d->P[0], d->P[1], cs, d->d_geom, d->d_Mpad);
+        SPIN_FFT(cufftExecD2Z(d->plan2_r2c, d->d_Mpad, d->d_Mhat));
+        const unsigned gq = (unsigned)((d->S2 + 127) / 128);
+        switch (d->PZ) {
+            case 1: ddi_slab_contract_kernel<1, 1><<<gq, 128, 0, s->stream>>>(d->d_Kre, d->d_Mhat, d->d_Hhat, (long long)d->S2); break;
+            case 2: ddi_slab_contract_kernel<1, 2><<<gq, 128, 0, s->stream>>>(d->d_Kre, d->d_Mhat, d->d_Hhat, (long long)d->S2); break;
+            case 4: ddi_slab_contract_kernel<2, 4><<<gq, 128, 0, s->stream>>>(d->d_Kre, d->d_Mhat, d->d_Hhat, (long long)d->S2); break;
+            case 8: ddi_slab_contract_kernel<4, 8><<<gq, 128, 0, s->stream>>>(d->d_Kre, d->d_Mhat, d->d_Hhat, (long long)d->S2); break;
+            default: ddi_slab_contract_kernel<8, 16><<<gq, 128, 0, s->stream>>>(d->d_Kre, d->d_Mhat, d->d_Hhat, (long long)d->S2); break;
+        }
+        SPIN_FFT(cufftExecZ2D(d->plan2_c2r, d->d_Hhat, d->d_Hpad));
+        ddi_gather_kernel<<<gs, nt, 0, s->stream>>>(s->plan, d->d_Hpad, d->P[0], d->P[1], cs, d->d_geom, C_DD / (double)d->Ptot, d_f);
+        s->n_launch += 3; s->n_fft += 2;
+        return SPIN_OK;
+    }
     ddi_scatter_kernel<<<gs, nt, 0, s->stream>>>(s->plan, d_n, d->P[0], d->P[1], (long long)d->Ptot, d->d_geom, d->d_Mpad);
     s->n_launch++;
     if (d->rank > 0) { SPIN_FFT(cufftExecD2Z(d->plan_r2c, d->d_Mpad, d->d_Mhat)); s->n_fft++; }

@@ -305,3 +305,27 @@ def test_full_size_configs(P, O, cfg, steps):
     print(f"cfg{cfg} full size {w.n_cells} ({w.n_spins} spins) steps={steps}: max|dn| = {d:.3e}")
     assert d <= SPIN_ATOL
     assert np.abs(np.linalg.norm(ng, axis=1) - 1).max() < 4e-16
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# Dipolar slab path (csrc/spin_ddi.cu): 2-D cuFFT over the occupied planes + one kernel for the transform along c, the tensor
+# contraction and the inverse transform.  Taken for one basis atom and 1, 2, 4 or 8 planes; other shapes use the 3-D path.
+@pytest.mark.parametrize("cells,per,img", [((20, 12, 4), (1, 1, 0), (2, 2, 0)), ((16, 10, 8), (1, 1, 0), (1, 1, 0)), ((12, 9, 2), (0, 1, 0), (0, 2, 0)),
+                                            ((14, 11, 1), (1, 1, 0), (3, 3, 0)), ((10, 8, 4), (1, 0, 1), (1, 0, 1))])
+def test_ddi_slab_path_matches_oracle_and_3d_path(P, O, cells, per, img):
+    w = dataclasses.replace(W.config5().resized(cells, 20), periodic=per, ddi_images=img)
+    g, o = pair(P, O, w)
+    Bo = o.effective_field()
+    assert_fields_close(g.effective_field(), Bo)
+    assert abs(g.energy()[1][5] - o.energy_terms()[5]) <= 1e-12 * np.abs(o.energy_terms()).sum()
+    # the general 3-D path on the same system
+    h = P.SpinSystem.from_workload(w)
+    h.spin_set_option("ddi_slab", 0)
+    assert_fields_close(h.effective_field(), Bo)
+    # against the O(N^2) direct sum (dipolar part only: switch everything else off)
+    w0 = dataclasses.replace(w, pair_J=w.pair_J * 0, pair_D=w.pair_D * 0, B=0.0, aniso=[])
+    g0, o0 = pair(P, O, w0)
+    Fd = o0.ddi_field(direct=True) / (w.mu_s[0] * O.MU_B)
+    assert np.abs(g0.effective_field() - Fd).max() <= 1e-11 * np.abs(Fd).max()
+    g.llg_iterate(20); o.iterate(20)
+    assert np.abs(g.spins_get() - o.spins()).max() <= SPIN_ATOL
