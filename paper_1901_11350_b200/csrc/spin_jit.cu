@@ -175,6 +175,11 @@ std::string spin::jit_source(const spin_system *s) {
       << ", PER_C = " << (P.perC ? "true" : "false") << ";\n";
     o << "constexpr bool STORE_A = " << (s->opt_store_A ? "true" : "false") << ", HAS_DDI = " << (P.has_ddi ? "true" : "false")
       << ", THERMAL_ON = " << (P.thermal_on ? "true" : "false") << ", STT_ON = " << (P.stt_on ? "true" : "false") << ";\n";
+    {   // partners in the own lattice row by warp shuffle: measured slower than the L1 hits it replaces (66 -> 79 us per step on
+        // cfg3), so off unless SPINLLG_SHFL=1
+        const char *e = getenv("SPINLLG_SHFL");
+        o << "constexpr bool SHFL = " << ((e && atoi(e) != 0) ? "true" : "false") << ";\n";
+    }
     // L2 prefetch distance of the brick kernels, in lattice planes (SPINLLG_PREFETCH overrides; 0 = off)
     int pf = 0;
     if (const char *e = getenv("SPINLLG_PREFETCH")) pf = atoi(e);

@@ -91,11 +91,28 @@ __device__ __forceinline__ void store_spin(double *__restrict__ q, const Coord &
 // Site accessors: where the partner (sublattice BJ at translation DA, DB, DC) of a site of sublattice B is read from.
 // GlobalAcc: the ghost-cell arrays in global memory (own address + immediate); RingAcc (spin_jit_tma.cuh): the ring of lattice
 // planes that TMA stages in shared memory.
+// With spec::SHFL, partners in the own lattice row (same sublattice, translation along a only) come from the neighbouring
+// lanes' own spins by warp shuffle -- a brick row is one warp -- and only the lanes at the ends of the row (or next to a lane
+// outside the lattice) go to memory: 6 of the 21 vector loads of a nearest-neighbour stencil become single-lane loads.
 template <int NCONF>
 struct GlobalAcc {
     const double *cfg[NCONF];      // x component of the own site in configuration k
+    double own[NCONF][3];          // the own spin (shuffle source), set by the sweep body
+    unsigned mask;                 // lanes of this warp that hold a lattice site
+    int lane;
     template <int B, int BJ, int DA, int DB, int DC>
-    __device__ __forceinline__ void load(int k, double (&v)[3]) const { load3<lin<B, BJ, DA, DB, DC>()>(cfg[k], v); }
+    __device__ __forceinline__ void load(int k, double (&v)[3]) const {
+        if constexpr (spec::SHFL && BJ == B && DB == 0 && DC == 0 && DA != 0 && DA > -32 && DA < 32 && spec::BX % 32 == 0) {
+            const int src = lane + DA;
+            v[0] = __shfl_sync(mask, own[k][0], src & 31);
+            v[1] = __shfl_sync(mask, own[k][1], src & 31);
+            v[2] = __shfl_sync(mask, own[k][2], src & 31);
+            if (src < 0 || src > 31 || !((mask >> src) & 1u)) load3<lin<B, BJ, DA, DB, DC>()>(cfg[k], v);
+        } else {
+            load3<lin<B, BJ, DA, DB, DC>()>(cfg[k], v);
+        }
+    }
+    __device__ __forceinline__ void set_own(int k, const double (&o)[3]) { own[k][0] = o[0]; own[k][1] = o[1]; own[k][2] = o[2]; }
 };
 
 // F += (Zeeman + anisotropy + pairs + quadruplets) of basis atom B for NCONF configurations sharing the lattice
@@ -235,11 +252,15 @@ __device__ __forceinline__ void predictor_body(const double *__restrict__ n, con
                                                double *__restrict__ Aout, u64 step, u32 seed_lo, u32 seed_hi) {
     Coord c;
     int idx;
-    if (!locate<B>(c, idx)) return;
+    const bool valid = locate<B>(c, idx);
+    const unsigned mask = __ballot_sync(0xffffffffu, valid);
+    if (!valid) return;
     prefetch_ahead(n + idx, c);
-    const GlobalAcc<1> cfg = {{n + idx}};
+    GlobalAcc<1> cfg;
+    cfg.cfg[0] = n + idx; cfg.mask = mask; cfg.lane = (int)(threadIdx.x & 31u);
     double own[1][3], F[1][3], sg[1][3] = {{0.0, 0.0, 0.0}};
     load3<0>(cfg.cfg[0], own[0]);
+    cfg.set_own(0, own[0]);
     thermal_force<B>(c, step, seed_lo, seed_hi, F[0]);
 #if !(SPIN_ABLATE & 1)
     force<B, 1>(cfg, own, F);
@@ -266,26 +287,32 @@ __device__ __forceinline__ void corrector_body(const double *__restrict__ n, con
                                                u64 step, u32 seed_lo, u32 seed_hi) {
     Coord c;
     int idx;
-    if (!locate<B>(c, idx)) return;
+    const bool valid = locate<B>(c, idx);
+    const unsigned mask = __ballot_sync(0xffffffffu, valid);
+    if (!valid) return;
     prefetch_ahead(n + idx, c);
     prefetch_ahead(np + idx, c);
     double th[3], A[3], Ap[3], n0[3];
     thermal_force<B>(c, step, seed_lo, seed_hi, th);
     load3<0>(n + idx, n0);
     if constexpr (spec::STORE_A) {
-        const GlobalAcc<1> cfg = {{np + idx}};
+        GlobalAcc<1> cfg;
+        cfg.cfg[0] = np + idx; cfg.mask = mask; cfg.lane = (int)(threadIdx.x & 31u);
         double own[1][3], F[1][3] = {{th[0], th[1], th[2]}}, sg[1][3] = {{0.0, 0.0, 0.0}};
         load3<0>(cfg.cfg[0], own[0]);
+        cfg.set_own(0, own[0]);
         force<B, 1>(cfg, own, F);
         if constexpr (spec::HAS_DDI) { double d[3]; load3<0>(fddi_np + idx, d); F[0][0] += d[0]; F[0][1] += d[1]; F[0][2] += d[2]; }
         if constexpr (spec::STT_ON) stt_gradient<B, 1>(cfg, c, own, sg);
         rotation_field<B>(own[0], F[0], sg[0], Ap);
         load3<0>(Ain + idx, A);
     } else {
-        const GlobalAcc<2> cfg = {{n + idx, np + idx}};
+        GlobalAcc<2> cfg;
+        cfg.cfg[0] = n + idx; cfg.cfg[1] = np + idx; cfg.mask = mask; cfg.lane = (int)(threadIdx.x & 31u);
         double own[2][3], F[2][3] = {{th[0], th[1], th[2]}, {th[0], th[1], th[2]}}, sg[2][3] = {{0.0, 0.0, 0.0}, {0.0, 0.0, 0.0}};
         own[0][0] = n0[0]; own[0][1] = n0[1]; own[0][2] = n0[2];
         load3<0>(cfg.cfg[1], own[1]);
+        cfg.set_own(0, own[0]); cfg.set_own(1, own[1]);
         force<B, 2>(cfg, own, F);
         if constexpr (spec::HAS_DDI) {
             double d[3];
