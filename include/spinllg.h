@@ -138,7 +138,10 @@ int spin_set_option(spin_system *sys, const char *name, int value);
  * use_tma (default 0): 1 runs the specialised sweeps as persistent kernels that stage lattice planes in shared memory with TMA
  * tensor copies (lattices of at least 16384 spins; 2 forces it for any size).  Measured slower than the brick kernels on
  * cfg3, hence off by default.
- * spin_kernel_info writes "jit+tma", "jit (brick kernels: <why>)" or "generic: <why>" into buf: which sweep kernels are in use.  */
+ * use_col (default 0): 1 runs them as column-marching kernels (one thread per lattice column, own spin at z-1, z, z+1 kept in
+ * registers; 3-D lattices).  Also measured slower than the brick kernels.
+ * ddi_slab (default 1): thin films with one basis atom take the dipolar slab path (2-D cuFFT + fused transform along c).
+ * spin_kernel_info writes "jit+col", "jit+tma", "jit (brick kernels: <why>)" or "generic: <why>" into buf: which sweep kernels are in use.  */
 int spin_kernel_info(spin_system *sys, char *buf, int len);
 /* the generated translation unit of the specialised sweeps (buf may be NULL); compile != 0 also compiles it for sm_100a
  * (needs no device) and returns the cubin size.  Host-side planner check; works in planner-only mode

@@ -364,9 +364,10 @@ int enqueue_step_t(spin_system *s, const Launch &L, unsigned step_add) {
         if (rc) return rc;
         if (prof) { cudaEventRecord(s->ev1, s->stream); cudaEventSynchronize(s->ev1); float ms; cudaEventElapsedTime(&ms, s->ev0, s->ev1); s->prof_ms[2] += ms; s->prof_n[2]++; }
     }
-    const bool jit = jit_ready(s), tma = jit_tma_ready(s);
+    const bool jit = jit_ready(s), col = jit_col_ready(s), tma = !col && jit_tma_ready(s);
     if (prof) cudaEventRecord(s->ev0, s->stream);
-    if (tma) { int rc = jit_launch_predictor_tma(s, s->cur, s->d_fddi[0], s->d_np, step_add); if (rc) return rc; }
+    if (col) { int rc = jit_launch_predictor_col(s, n, s->d_fddi[0], s->d_np, step_add); if (rc) return rc; }
+    else if (tma) { int rc = jit_launch_predictor_tma(s, s->cur, s->d_fddi[0], s->d_np, step_add); if (rc) return rc; }
     else if (jit) { int rc = jit_launch_predictor(s, L.grid, L.block, n, s->d_fddi[0], s->d_np, s->d_A, step_add); if (rc) return rc; }
     else if (s->opt_store_A)
         predictor_kernel<BX, BY, BZ, true><<<L.grid, L.block, 0, s->stream>>>(s->plan, n, s->d_fddi[0], s->d_np, s->d_A, s->d_step, step_add);
@@ -381,7 +382,8 @@ int enqueue_step_t(spin_system *s, const Launch &L, unsigned step_add) {
         if (prof) { cudaEventRecord(s->ev1, s->stream); cudaEventSynchronize(s->ev1); float ms; cudaEventElapsedTime(&ms, s->ev0, s->ev1); s->prof_ms[2] += ms; s->prof_n[2]++; }
     }
     if (prof) cudaEventRecord(s->ev0, s->stream);
-    if (tma) { int rc = jit_launch_corrector_tma(s, s->cur, s->d_fddi[0], s->d_fddi[1], nout, step_add); if (rc) return rc; }
+    if (col) { int rc = jit_launch_corrector_col(s, n, s->d_np, s->d_fddi[0], s->d_fddi[1], nout, step_add); if (rc) return rc; }
+    else if (tma) { int rc = jit_launch_corrector_tma(s, s->cur, s->d_fddi[0], s->d_fddi[1], nout, step_add); if (rc) return rc; }
     else if (jit) { int rc = jit_launch_corrector(s, L.grid, L.block, n, s->d_np, s->d_fddi[0], s->d_fddi[1], s->d_A, nout, step_add); if (rc) return rc; }
     else if (s->opt_store_A)
         corrector_kernel<BX, BY, BZ, true><<<L.grid, L.block, 0, s->stream>>>(s->plan, n, s->d_np, s->d_fddi[0], s->d_fddi[1], s->d_A, nout, s->d_step, step_add);
@@ -446,7 +448,7 @@ extern "C" int spin_geometry_create(const double bravais[9], int n_basis, const 
     if (!has_device) cudaGetLastError();
     spin_system *s = new spin_system();
     s->has_device = has_device;
-    s->jit = nullptr; s->opt_jit = 1; s->opt_tma = 0; s->opt_ddi_slab = 1;
+    s->jit = nullptr; s->opt_jit = 1; s->opt_tma = 0; s->opt_ddi_slab = 1; s->opt_col = 0;
     memcpy(s->brav, bravais, sizeof(s->brav));
     s->nb = n_basis;
     s->basis.assign(basis_frac, basis_frac + 3 * n_basis);
@@ -843,6 +845,7 @@ extern "C" int spin_set_option(spin_system *s, const char *name, int value) {
     if (!strcmp(name, "use_graph")) s->opt_graph = value ? 1 : 0;
     else if (!strcmp(name, "store_A")) { s->opt_store_A = value ? 1 : 0; s->plan_dirty = true; }
     else if (!strcmp(name, "use_jit")) { s->opt_jit = value ? 1 : 0; s->plan_dirty = true; }
+    else if (!strcmp(name, "use_col")) { s->opt_col = value ? 1 : 0; s->plan_dirty = true; }
     else if (!strcmp(name, "ddi_slab")) { s->opt_ddi_slab = value ? 1 : 0; s->plan_dirty = true; }
     else if (!strcmp(name, "use_tma")) { s->opt_tma = value < 0 ? 0 : (value > 2 ? 2 : value); s->plan_dirty = true; }
     else return spin::fail(SPIN_ERR_ARG, "unknown option '%s'", name);
@@ -854,7 +857,8 @@ extern "C" int spin_set_option(spin_system *s, const char *name, int value) {
 extern "C" int spin_kernel_info(spin_system *s, char *buf, int len) {
     REQUIRE(s && buf && len > 0, "bad argument");
     if (s->has_device) { int rc = ensure_plan(s); if (rc) return rc; }
-    if (jit_tma_ready(s)) snprintf(buf, (size_t)len, "jit+tma");
+    if (jit_col_ready(s)) snprintf(buf, (size_t)len, "jit+col");
+    else if (jit_tma_ready(s)) snprintf(buf, (size_t)len, "jit+tma");
     else if (jit_ready(s)) snprintf(buf, (size_t)len, "jit (brick kernels: %s)", jit_tma_note(s));
     else snprintf(buf, (size_t)len, "generic: %s", s->jit_note.c_str());
     return SPIN_OK;

@@ -38,6 +38,10 @@ struct JitState {
     std::string tma_note;     // why not, if not
     TmaGeo gp, gc;
     cudaKernel_t k_pred_tma, k_corr_tma;
+    // column-marching sweeps
+    bool col;
+    cudaKernel_t k_pred_col, k_corr_col;
+    int col_geo[4];           // CBX, CBY, CCZ, CNZC
     int grid_p, grid_c;
     CUtensorMap tm_n[2];              // predictor: n[cur] with the predictor tile
     CUtensorMap tm_cn[2], tm_cnp;     // corrector: n[cur], n^p with the corrector tile
@@ -149,6 +153,25 @@ static void jit_brick_launch(const spin_system *s, dim3 &grid, dim3 &block) {
     block = dim3((unsigned)(b[0] * b[1] * b[2]), 1, 1);
 }
 
+// column-marching sweeps (spin_jit_col.cuh): tile of columns per block, planes per chunk, chunks; false if not applicable.
+// SPINLLG_COL="cbx,cby,ccz" overrides the defaults (32 x 4 columns, 16 planes per chunk).
+static bool plan_col(const spin_system *s, int g[4]) {
+    const DevicePlan &P = s->plan;
+    if (!s->opt_col || s->opt_store_A || P.rC < 1 || P.Nc < 2) return false;
+    int cbx = 32, cby = 4, ccz = 16;
+    if (const char *e = getenv("SPINLLG_COL")) {
+        int v[3] = {0, 0, 0};
+        sscanf(e, "%d,%d,%d", &v[0], &v[1], &v[2]);
+        if (v[0] > 0) cbx = v[0];
+        if (v[1] > 0) cby = v[1];
+        if (v[2] > 0) ccz = v[2];
+    }
+    if ((cbx * cby) % 32 || cbx * cby > 1024) return false;
+    if (ccz > P.Nc) ccz = P.Nc;
+    g[0] = cbx; g[1] = cby; g[2] = ccz; g[3] = (P.Nc + ccz - 1) / ccz;
+    return true;
+}
+
 // the staging geometry of both sweeps, or why the TMA-fed sweeps are not generated for this system
 static bool plan_tma(const spin_system *s, TmaGeo &gp, TmaGeo &gc, std::string &why) {
     if (!s->opt_tma) { why = "disabled by option use_tma=0"; return false; }
@@ -255,6 +278,9 @@ std::string spin::jit_source(const spin_system *s) {
     const bool tma = plan_tma(s, gp, gc, why);
     if (tma) { emit_tma_geo(o, "TmaP", gp); emit_tma_geo(o, "TmaC", gc); }
     o << "}  // namespace spec\n";
+    int cg[4];
+    const bool col = plan_col(s, cg);
+    if (col) o << "namespace spec { constexpr int CBX = " << cg[0] << ", CBY = " << cg[1] << ", CCZ = " << cg[2] << ", CNZC = " << cg[3] << "; }\n#define SPIN_COL 1\n";
     if (tma) o << "#define SPIN_TMA 1\n";
     if (const char *e = getenv("SPINLLG_MINBLOCKS")) o << "#define SPIN_MINBLOCKS " << atoi(e) << "\n";
     if (const char *e = getenv("SPINLLG_ABLATE")) o << "#define SPIN_ABLATE " << atoi(e) << "\n";
@@ -355,6 +381,7 @@ int spin::jit_prepare(spin_system *s) {
     JitState *j = new JitState();
     j->loaded = false;
     j->tma = false;
+    j->col = false;
     j->source = src;
     s->jit = j;
     std::string cubin;
@@ -367,6 +394,12 @@ int spin::jit_prepare(spin_system *s) {
     if (e == cudaSuccess) e = cudaLibraryGetKernel(&j->k_corr, j->lib, "jit_corrector");
     if (e != cudaSuccess) return spin::fail(SPIN_ERR_CUDA, "cudaLibraryGetKernel failed: %s", cudaGetErrorString(e));
     tma_prepare(s, j);
+    j->col = plan_col(s, j->col_geo);
+    if (j->col) {
+        e = cudaLibraryGetKernel(&j->k_pred_col, j->lib, "jit_predictor_col");
+        if (e == cudaSuccess) e = cudaLibraryGetKernel(&j->k_corr_col, j->lib, "jit_corrector_col");
+        if (e != cudaSuccess) { cudaGetLastError(); j->col = false; }
+    }
     return SPIN_OK;
 }
 
@@ -390,6 +423,38 @@ int spin::jit_launch_corrector(spin_system *s, dim3 grid, dim3 block, const doub
                     (void *)&seed_lo, (void *)&seed_hi};
     jit_brick_launch(s, grid, block);
     SPIN_CUDA(cudaLaunchKernel((const void *)s->jit->k_corr, grid, block, args, 0, s->stream));
+    return SPIN_OK;
+}
+
+bool spin::jit_col_ready(const spin_system *s) { return s->jit && s->jit->loaded && s->jit->col; }
+
+static void col_launch_dims(const spin_system *s, const JitState *j, dim3 &grid, dim3 &block) {
+    const int *g = j->col_geo;
+    grid = dim3((unsigned)(((s->nc[0] + g[0] - 1) / g[0]) * ((s->nc[1] + g[1] - 1) / g[1]) * g[3]), (unsigned)s->nb, 1);
+    block = dim3((unsigned)(g[0] * g[1]), 1, 1);
+}
+
+int spin::jit_launch_predictor_col(spin_system *s, const double *n, const double *fddi, double *np, unsigned step_add) {
+    JitState *j = s->jit;
+    unsigned seed_lo = s->plan.seed_lo, seed_hi = s->plan.seed_hi;
+    const unsigned long long *d_step = s->d_step;
+    void *args[] = {(void *)&n, (void *)&fddi, (void *)&np, (void *)&d_step, (void *)&step_add, (void *)&seed_lo, (void *)&seed_hi};
+    dim3 grid, block;
+    col_launch_dims(s, j, grid, block);
+    SPIN_CUDA(cudaLaunchKernel((const void *)j->k_pred_col, grid, block, args, 0, s->stream));
+    return SPIN_OK;
+}
+
+int spin::jit_launch_corrector_col(spin_system *s, const double *n, const double *np, const double *fddi_n, const double *fddi_np, double *nout,
+                                   unsigned step_add) {
+    JitState *j = s->jit;
+    unsigned seed_lo = s->plan.seed_lo, seed_hi = s->plan.seed_hi;
+    const unsigned long long *d_step = s->d_step;
+    void *args[] = {(void *)&n, (void *)&np, (void *)&fddi_n, (void *)&fddi_np, (void *)&nout, (void *)&d_step, (void *)&step_add, (void *)&seed_lo,
+                    (void *)&seed_hi};
+    dim3 grid, block;
+    col_launch_dims(s, j, grid, block);
+    SPIN_CUDA(cudaLaunchKernel((const void *)j->k_corr_col, grid, block, args, 0, s->stream));
     return SPIN_OK;
 }
 

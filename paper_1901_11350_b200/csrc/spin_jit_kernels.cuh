@@ -360,6 +360,9 @@ extern "C" __global__ void SPIN_BOUNDS(spec::BX *spec::BY *spec::BZ)
     });
 }
 
+#ifdef SPIN_COL
+#include "spin_jit_col.cuh"
+#endif
 #ifdef SPIN_TMA
 #include "spin_jit_tma.cuh"
 #endif

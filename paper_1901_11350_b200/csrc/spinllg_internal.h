@@ -129,7 +129,7 @@ struct spin_system {
     bool has_device;               // false only in the planner-only mode used by the CPU tests
     std::string jit_note;          // why the specialised sweeps are not in use, if they are not
     // ---- execution options / bookkeeping
-    int opt_graph, opt_store_A, opt_jit, opt_tma, opt_ddi_slab;
+    int opt_graph, opt_store_A, opt_jit, opt_tma, opt_ddi_slab, opt_col;
     cudaGraphExec_t graph_exec[2];   // one captured graph per ping-pong parity
     int graph_steps;
     int64_t n_launch, n_fft;
@@ -162,6 +162,11 @@ int jit_prepare(spin_system *s);
 void jit_release(spin_system *s);
 bool jit_ready(const spin_system *s);
 const char *jit_log(const spin_system *s);
+// column-marching versions of the two sweeps (spin_jit_col.cuh)
+bool jit_col_ready(const spin_system *s);
+int jit_launch_predictor_col(spin_system *s, const double *n, const double *fddi, double *np, unsigned step_add);
+int jit_launch_corrector_col(spin_system *s, const double *n, const double *np, const double *fddi_n, const double *fddi_np, double *nout,
+                             unsigned step_add);
 // TMA-fed plane-marching versions of the two sweeps (spin_jit_tma.cuh); cur = index of the current n buffer
 bool jit_tma_ready(const spin_system *s);
 const char *jit_tma_note(const spin_system *s);

@@ -269,6 +269,7 @@ def test_tma_sweeps_match_oracle(P, O, cfg, cells, steps, geo, monkeypatch):
         monkeypatch.setenv("SPINLLG_TMA_C", geo)
     w = W.CONFIGS[cfg]().resized(cells, steps)
     g, o = pair(P, O, w)
+    g.spin_set_option("use_col", 0)
     g.spin_set_option("use_tma", 2)
     assert g.spin_kernel_info() == "jit+tma", g.spin_kernel_info()
     g.llg_iterate(steps); o.iterate(steps)
@@ -278,6 +279,7 @@ def test_tma_sweeps_match_oracle(P, O, cfg, cells, steps, geo, monkeypatch):
     # bit-identical to the brick kernels: same arithmetic, only the staging differs
     b = P.SpinSystem.from_workload(w)
     b.spin_set_option("use_tma", 0)
+    b.spin_set_option("use_col", 0)
     assert b.spin_kernel_info().startswith("jit (brick")
     b.llg_iterate(steps)
     assert np.array_equal(b.spins_get(), g.spins_get())
@@ -329,3 +331,35 @@ def test_ddi_slab_path_matches_oracle_and_3d_path(P, O, cells, per, img):
     assert np.abs(g0.effective_field() - Fd).max() <= 1e-11 * np.abs(Fd).max()
     g.llg_iterate(20); o.iterate(20)
     assert np.abs(g.spins_get() - o.spins()).max() <= SPIN_ATOL
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# Column-marching sweeps (csrc/spin_jit_col.cuh), option use_col=1 (measured slower than the bricks): same arithmetic
+@pytest.mark.parametrize("cfg,cells,steps,geo", [(3, (35, 9, 7), 100, None), (3, (70, 37, 45), 20, "32,8,16"), (3, (33, 5, 40), 20, "64,2,7"),
+                                                 (5, (20, 12, 5), 20, None), (5, (20, 12, 4), 20, "32,4,3"), (3, (6, 5, 2), 50, None)])
+def test_column_marching_sweeps(P, O, cfg, cells, steps, geo, monkeypatch):
+    if geo:
+        monkeypatch.setenv("SPINLLG_COL", geo)
+    w = W.CONFIGS[cfg]().resized(cells, steps)
+    g, o = pair(P, O, w)
+    g.spin_set_option("use_col", 1)
+    assert g.spin_kernel_info() == "jit+col", g.spin_kernel_info()
+    g.llg_iterate(steps); o.iterate(steps)
+    d = np.abs(g.spins_get() - o.spins()).max()
+    print(f"col cfg{cfg} {cells} steps={steps}: max|dn| = {d:.3e}")
+    assert d <= SPIN_ATOL
+    b = P.SpinSystem.from_workload(w)
+    b.spin_set_option("use_col", 0)
+    assert b.spin_kernel_info().startswith("jit (brick")
+    b.llg_iterate(steps)
+    assert np.array_equal(b.spins_get(), g.spins_get())
+
+
+def test_column_marching_with_open_and_mixed_boundaries(P, O):
+    for per in [(0, 0, 0), (1, 0, 1), (0, 1, 0)]:
+        w = dataclasses.replace(W.config3().resized((21, 10, 9), 30), periodic=per)
+        g, o = pair(P, O, w)
+        g.spin_set_option("use_col", 1)
+        assert g.spin_kernel_info() == "jit+col"
+        g.llg_iterate(30); o.iterate(30)
+        assert np.abs(g.spins_get() - o.spins()).max() <= SPIN_ATOL
