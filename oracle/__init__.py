@@ -66,6 +66,7 @@ def lib():
         L.orc_llg_step.argtypes = [vp]
         L.orc_llg_iterate.argtypes = [vp, C.c_long]
         L.orc_heun_step.argtypes = [vp]
+        L.orc_set_solver.argtypes = [vp, C.c_int]
         L.orc_effective_field.argtypes = [vp, dp]
         L.orc_observables.argtypes = [vp, dp, dp]
         _lib = L
@@ -237,6 +238,10 @@ class OracleSystem:
 
     def iterate(self, n_steps):
         lib().orc_llg_iterate(self._h, int(n_steps))
+
+    def set_solver(self, solver):
+        """0 Depondt (App. B B5-B7), 1 Heun (B3-B4), 2 SIB semi-implicit midpoint (App. C)."""
+        lib().orc_set_solver(self._h, int(solver))
 
     def heun_step(self):
         lib().orc_heun_step(self._h)

@@ -13,8 +13,9 @@
  *   dipole-dipole     :81-89 direct sum / FFT convolution   -> orc_ddi_direct, orc_ddi_fft
  *   LLG explicit form Eq. 10 (:147-153)                     -> rot_field()
  *   thermal field     Eq. 11 (:157-160)                     -> orc_thermal_xi, sigma
- *   Depondt solver    App. B, B5-B7 (:369-380)              -> orc_llg_step
- *   Heun solver       App. B, B3-B4 (:355-367)              -> orc_heun_step (pin only)
+ *   Depondt solver    App. B, B5-B7 (:369-380)              -> orc_llg_step (solver 0)
+ *   Heun solver       App. B, B3-B4 (:355-367)              -> orc_llg_step (solver 1); orc_heun_step = the same written on its own (pin)
+ *   SIB solver        App. C, C5-C11 (:384-436)             -> orc_llg_step (solver 2), imp_update (Cramer's rule as printed)
  * Readings of silent / garbled passages are listed in DESIGN.md ("Readings") under the
  * same R-numbers as SURVEY.md 8(c).
  *
@@ -69,6 +70,7 @@ typedef struct orc_system {
     uint64_t seed, step;
     double *n;               /* 3N */
     int nthreads;
+    int solver;              /* 0 Depondt (App. B B5-B7), 1 Heun (B3-B4), 2 SIB semi-implicit midpoint (App. C) */
 } orc_system;
 
 /* ------------------------------------------------------------------ helpers */
@@ -198,6 +200,7 @@ void orc_llg_configure(orc_system *s, double dt_fs, double alpha, double T, uint
     for (int k = 0; k < 3; ++k) s->jdir[k] = (nrm > 0) ? jdir[k] / nrm : 0.0;
     s->step = 0;
 }
+void orc_set_solver(orc_system *s, int solver) { s->solver = solver; }
 uint64_t orc_get_step(const orc_system *s) { return s->step; }
 void orc_set_step(orc_system *s, uint64_t st) { s->step = st; }
 
@@ -730,9 +733,33 @@ static void total_force(orc_system *s, const double *n, const double *Fth, doubl
     if (Fth) for (long i = 0; i < 3 * s->N; ++i) F[i] += Fth[i];
 }
 
-/* One Depondt step (App. B, B5-B7): predictor with R(A), A^p at the predicted configuration
- * with the same thermal field (reading R11), corrector R((A+A^p)/2) applied to n(t) (reading R8),
- * then renormalisation (reading R19).                                                        */
+/* Semi-implicit midpoint update (App. C, C5-C10): solve M x = M^T n with M = I + skew(A'), A' = (dt/2) A,
+ * by Cramer's rule exactly as the paper writes it: a = M^T n = n + n x A' (C8), x_alpha = det(M^alpha)/det(M) (C9),
+ * M^alpha = M with column alpha replaced by a (C10).  The paper prints M with A; the factor dt/2 follows from C5
+ * (n^p - (dt/2) n^p x A = n + (dt/2) n x A), reading R25 in DESIGN.md.                                                */
+static double det3(const double m[3][3]) {
+    return m[0][0] * (m[1][1] * m[2][2] - m[1][2] * m[2][1]) - m[0][1] * (m[1][0] * m[2][2] - m[1][2] * m[2][0])
+         + m[0][2] * (m[1][0] * m[2][1] - m[1][1] * m[2][0]);
+}
+static inline void imp_update(const double *A, double dt, const double *n, double *out) {
+    double Ah[3] = { 0.5 * dt * A[0], 0.5 * dt * A[1], 0.5 * dt * A[2] };
+    double M[3][3] = { { 1.0, -Ah[2], Ah[1] }, { Ah[2], 1.0, -Ah[0] }, { -Ah[1], Ah[0], 1.0 } };      /* C7 */
+    double nxA[3]; cross3(n, Ah, nxA);
+    double a[3] = { n[0] + nxA[0], n[1] + nxA[1], n[2] + nxA[2] };                                   /* C8 */
+    double d = det3(M);
+    for (int al = 0; al < 3; ++al) {
+        double Ma[3][3];
+        for (int r = 0; r < 3; ++r) for (int c = 0; c < 3; ++c) Ma[r][c] = (c == al) ? a[r] : M[r][c];   /* C10 */
+        out[al] = det3(Ma) / d;                                                                       /* C9 */
+    }
+}
+
+/* One step of the selected solver.  All three are two-stage predictor/corrector schemes on dn/dt = n x A (B1) that share
+ * the thermal field of the step between the stages (reading R11):
+ *   Depondt (App. B, B5-B7): n^p = R(A) n; A^p = A(n^p); n <- R((A+A^p)/2) n(t) (reading R8); renormalise (R19).
+ *   Heun (B3-B4 with f = n x A): n^p = n + dt n x A; n <- n + dt/2 (n x A + n^p x A^p); renormalise every step.
+ *   SIB (App. C, C5, C11): n^p from the implicit-midpoint structure with A(n); n <- the same structure with A evaluated at
+ *        the midpoint configuration {(n_j + n_j^p)/2}; length is preserved by construction, no renormalisation.        */
 void orc_llg_step(orc_system *s) {
     long N = s->N; int nb = s->nb;
     double *F = (double *)malloc(3 * N * sizeof(double)), *A = (double *)malloc(3 * N * sizeof(double));
@@ -752,16 +779,31 @@ void orc_llg_step(orc_system *s) {
 #pragma omp parallel for schedule(static) num_threads(s->nthreads)
     for (long i = 0; i < N; ++i) {
         rot_field(s, (int)(i % nb), s->n + 3*i, F + 3*i, sg + 3*i, A + 3*i);
-        rotate(A + 3*i, s->dt, s->n + 3*i, np_ + 3*i);                       /* B5 */
+        if (s->solver == 0) rotate(A + 3*i, s->dt, s->n + 3*i, np_ + 3*i);                       /* B5 */
+        else if (s->solver == 1) {                                                               /* B3 */
+            double f0[3]; cross3(s->n + 3*i, A + 3*i, f0);
+            for (int k = 0; k < 3; ++k) np_[3*i+k] = s->n[3*i+k] + s->dt * f0[k];
+        } else imp_update(A + 3*i, s->dt, s->n + 3*i, np_ + 3*i);                                /* C5 */
     }
-    total_force(s, np_, Fth, F);
-    if (s->u != 0.0) orc_stt_gradient(s, np_, sg);
+    /* configuration the second field is evaluated at: n^p (B6), or the midpoint (n + n^p)/2 (C11) */
+    double *second = np_;
+    if (s->solver == 2) for (long i = 0; i < 3 * N; ++i) np_[i] = 0.5 * (s->n[i] + np_[i]);
+    total_force(s, second, Fth, F);
+    if (s->u != 0.0) orc_stt_gradient(s, second, sg);
 #pragma omp parallel for schedule(static) num_threads(s->nthreads)
     for (long i = 0; i < N; ++i) {
         double Ap[3], Ac[3], out[3];
-        rot_field(s, (int)(i % nb), np_ + 3*i, F + 3*i, sg + 3*i, Ap);
-        for (int k = 0; k < 3; ++k) Ac[k] = 0.5 * (A[3*i+k] + Ap[k]);         /* B6 */
-        rotate(Ac, s->dt, s->n + 3*i, out);                                   /* B7 */
+        rot_field(s, (int)(i % nb), second + 3*i, F + 3*i, sg + 3*i, Ap);
+        if (s->solver == 0) {
+            for (int k = 0; k < 3; ++k) Ac[k] = 0.5 * (A[3*i+k] + Ap[k]);     /* B6 */
+            rotate(Ac, s->dt, s->n + 3*i, out);                               /* B7 */
+        } else if (s->solver == 1) {                                          /* B4 */
+            double f0[3], f1[3]; cross3(s->n + 3*i, A + 3*i, f0); cross3(np_ + 3*i, Ap, f1);
+            for (int k = 0; k < 3; ++k) out[k] = s->n[3*i+k] + 0.5 * s->dt * (f0[k] + f1[k]);
+        } else {
+            imp_update(Ap, s->dt, s->n + 3*i, out);                           /* C11 */
+        }
+        if (s->solver == 2) { for (int k = 0; k < 3; ++k) s->n[3*i+k] = out[k]; continue; }
         double nrm = sqrt(dot3(out, out));
         for (int k = 0; k < 3; ++k) s->n[3*i+k] = out[k] / nrm;
     }

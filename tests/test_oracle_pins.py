@@ -79,7 +79,10 @@ def _larmor_error(dt_fs, alpha, method, t_ps=100.0, mu_s=2.0, B=1.0):
     gp = O.GAMMA / (1 + alpha * alpha)
     err, dev = 0.0, 0.0
     for k in range(int(round(t_ps / (dt_fs * 1e-3)))):
-        s.iterate(1) if method == "depondt" else s.heun_step()
+        if method == "heun_standalone":
+            s.heun_step()
+        else:
+            s.set_solver({"depondt": 0, "heun": 1, "sib": 2}[method]); s.iterate(1)
         t = (k + 1) * dt_fs * 1e-3
         nz = math.tanh(alpha * gp * B * t)
         ph = gp * B * t
@@ -108,6 +111,46 @@ def test_O2_larmor_mu_independent_and_heun_order():
     assert e1 == pytest.approx(e2, rel=1e-6)                        # reading R2: mu cancels
     eh, _ = _larmor_error(10.0, 0.1, "heun")
     assert e1 < eh < 10 * GOLD["larmor_heun_error_order"]["value"]
+    # the Heun branch of the general step (thermal field and current included) equals Heun written out on its own
+    assert _larmor_error(10.0, 0.1, "heun_standalone")[0] == eh
+
+
+def test_solvers_heun_and_sib_closed_forms():
+    """Heun (App. B, B3-B4) and the semi-implicit midpoint solver SIB (App. C, C5-C11) against what mathematics fixes:
+    second order on the damped Larmor problem of Eq. 12; SIB keeps |n| = 1 without renormalisation; and for alpha = 0 in a
+    constant field both SIB stages see the same A, so one step is the Cayley rotation about the field by exactly
+    2 atan(gamma B dt / 2) -- which pins the dt/2 in the skew matrix (reading R25) and the sense of rotation."""
+    for m in ("heun", "sib"):
+        e, dev = _larmor_error(10.0, 0.1, m, t_ps=20.0)
+        eh, _ = _larmor_error(5.0, 0.1, m, t_ps=20.0)
+        assert e / eh == pytest.approx(4.0, rel=0.15), (m, e, eh)
+        assert e < 2e-5 and dev < 1e-14, (m, e, dev)
+    s = OracleSystem(np.eye(3), [[0, 0, 0]], (1, 1, 1), (0, 0, 0))
+    B, dt_fs, steps = 3.0, 50.0, 40
+    s.set_mu_s([2.0]); s.set_field(B, (0, 0, 1)); s.llg_configure(dt_fs, 0.0); s.set_solver(2)
+    n0 = np.array([0.6, 0.0, 0.8])
+    s.set_spins([n0]); s.iterate(steps)
+    ph = steps * 2.0 * math.atan(O.GAMMA * B * dt_fs * 1e-3 / 2.0)       # Eq. 12 sense: phi grows with +gamma B t
+    ex = np.array([0.6 * math.cos(ph), 0.6 * math.sin(ph), 0.8])
+    assert np.abs(s.spins()[0] - ex).max() < 1e-14
+    # no hidden renormalisation: a non-unit start keeps its length
+    s.set_spins([1.5 * n0]); s.iterate(7)
+    assert abs(np.linalg.norm(s.spins()[0]) - 1.5) < 1e-14
+
+
+@pytest.mark.parametrize("solver", [1, 2])
+def test_solvers_energy_decreases_and_split_invariance(solver):
+    """alpha > 0, T = 0: the energy must not increase (Heun, SIB); with noise, iterate(a) + iterate(b) == iterate(a+b)."""
+    w = small(3, (6, 6, 6))
+    s = OracleSystem.from_workload(w); s.set_solver(solver)
+    E = [s.energy()]
+    for _ in range(6):
+        s.iterate(50); E.append(s.energy())
+    assert all(b <= a + 1e-10 * abs(a) for a, b in zip(E, E[1:])), E
+    w2 = small(2, (8, 8, 1))
+    a = OracleSystem.from_workload(w2); a.set_solver(solver); a.iterate(30)
+    b = OracleSystem.from_workload(w2); b.set_solver(solver); b.iterate(11); b.iterate(19)
+    assert np.array_equal(a.spins(), b.spins())
 
 
 # ------------------------------------------------------------------ O3 gradient vs finite differences
