@@ -106,7 +106,16 @@ int spins_get_device(spin_system *sys, double *n_xyz /*device, 3N AoS*/);
  * non-adiabatic parameter.  Resets the step counter to 0.                                                   */
 int llg_configure(spin_system *sys, double dt_fs, double alpha, double T_kelvin, uint64_t seed,
                   double u_A_per_ps, const double j_dir[3], double beta);
-/* advance n_steps Depondt steps; asynchronous on the system's stream.  The step counter persists, so
+/* Solver of the LLG equation written as dn/dt = n x A (B1, :349).  All are two-stage predictor/corrector schemes over the same
+ * two field sweeps and share the thermal field of the step between the stages:
+ *   SPIN_SOLVER_DEPONDT  App. B, B5-B7 (:369-380): rotations R(A), renormalised                       (default)
+ *   SPIN_SOLVER_HEUN     App. B, B3-B4 (:355-367): n + dt/2 (n x A + n^p x A^p), renormalised every step
+ *   SPIN_SOLVER_SIB      App. C, C5-C11 (:384-436): semi-implicit midpoint; field of the corrector at {(n_j + n_j^p)/2};
+ *                        preserves |n_i| by construction (no renormalisation)
+ * Heun and SIB run in the run-time specialised kernels only (SPIN_ERR_STATE from llg_iterate if those are unavailable). */
+enum { SPIN_SOLVER_DEPONDT = 0, SPIN_SOLVER_HEUN = 1, SPIN_SOLVER_SIB = 2 };
+int llg_set_solver(spin_system *sys, int solver);
+/* advance n_steps steps of the selected solver (Depondt unless llg_set_solver chose another); asynchronous on the system's stream.  The step counter persists, so
  * llg_iterate(a); llg_iterate(b) reproduces llg_iterate(a+b) exactly.                                       */
 int llg_iterate(spin_system *sys, int64_t n_steps);
 int llg_get_step(const spin_system *sys, uint64_t *step);

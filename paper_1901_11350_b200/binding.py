@@ -20,7 +20,7 @@ EXPORTS = [
     "hamiltonian_set_mu_s", "hamiltonian_set_field", "hamiltonian_set_anisotropy", "hamiltonian_set_pairs",
     "hamiltonian_set_exchange_shells", "hamiltonian_set_dmi_shells", "hamiltonian_set_quadruplets",
     "hamiltonian_set_ddi", "spins_set", "spins_get", "spins_set_device", "spins_get_device",
-    "llg_configure", "llg_iterate", "llg_get_step", "llg_set_step", "spin_synchronize",
+    "llg_configure", "llg_set_solver", "llg_iterate", "llg_get_step", "llg_set_step", "spin_synchronize",
     "effective_field", "effective_field_device", "energy", "observables",
     "spin_launch_counts", "spin_profile_enable", "spin_profile_get", "spin_set_option",
     "spin_kernel_info", "spin_jit_source", "spin_last_error", "spin_version",
@@ -62,6 +62,7 @@ def lib() -> C.CDLL:
         "spins_set_device": (C.c_int, [vp, vp]),
         "spins_get_device": (C.c_int, [vp, vp]),
         "llg_configure": (C.c_int, [vp, C.c_double, C.c_double, C.c_double, C.c_uint64, C.c_double, dp, C.c_double]),
+        "llg_set_solver": (C.c_int, [vp, C.c_int]),
         "llg_iterate": (C.c_int, [vp, C.c_int64]),
         "llg_get_step": (C.c_int, [vp, C.POINTER(C.c_uint64)]),
         "llg_set_step": (C.c_int, [vp, C.c_uint64]),
@@ -215,6 +216,10 @@ class SpinSystem:
     def llg_configure(self, dt_fs, alpha, T=0.0, seed=0, u=0.0, j_dir=(1, 0, 0), beta=0.0):
         j, jp = _d(j_dir)
         _check(lib().llg_configure(self._h, float(dt_fs), float(alpha), float(T), int(seed), float(u), jp, float(beta)))
+
+    def llg_set_solver(self, solver):
+        """0 Depondt, 1 Heun, 2 SIB (include/spinllg.h SPIN_SOLVER_*)."""
+        _check(lib().llg_set_solver(self._h, int(solver)))
 
     def llg_iterate(self, n_steps):
         _check(lib().llg_iterate(self._h, int(n_steps)))

@@ -462,7 +462,7 @@ extern "C" int spin_geometry_create(const double bravais[9], int n_basis, const 
     for (int bb = 0; bb < n_basis; ++bb) s->Kax[3 * bb + 2] = 1.0;
     s->ddi_on = 0; s->ddi_img[0] = s->ddi_img[1] = s->ddi_img[2] = 0;
     s->dt_ps = 1e-3; s->alpha = 0.1; s->T = 0; s->u = 0; s->jdir[0] = 1; s->jdir[1] = 0; s->jdir[2] = 0; s->beta = 0;
-    s->seed = 0; s->step = 0;
+    s->seed = 0; s->step = 0; s->solver = SPIN_SOLVER_DEPONDT;
     s->stream = nullptr; s->own_stream = nullptr; s->cur = 0;
     s->d_n[0] = s->d_n[1] = s->d_np = s->d_A = s->d_fddi[0] = s->d_fddi[1] = s->d_aos = s->d_partials = s->d_result = nullptr;
     s->d_step = nullptr; s->ddi = nullptr; s->plan_dirty = true;
@@ -705,6 +705,12 @@ extern "C" int llg_configure(spin_system *s, double dt_fs, double alpha, double 
     s->plan_dirty = true;
     return llg_set_step(s, 0);
 }
+extern "C" int llg_set_solver(spin_system *s, int solver) {
+    REQUIRE(s, "null system");
+    REQUIRE(solver == SPIN_SOLVER_DEPONDT || solver == SPIN_SOLVER_HEUN || solver == SPIN_SOLVER_SIB, "unknown solver %d", solver);
+    if (s->solver != solver) { s->solver = solver; s->plan_dirty = true; drop_graphs(s); }
+    return SPIN_OK;
+}
 extern "C" int llg_get_step(const spin_system *s, uint64_t *step) {
     REQUIRE(s && step, "null argument");
     *step = s->step;
@@ -724,6 +730,8 @@ extern "C" int llg_iterate(spin_system *s, int64_t n_steps) {
     REQUIRE(s && n_steps >= 0, "bad argument");
     int rc = ensure_plan(s);
     if (rc) return rc;
+    if (s->solver != SPIN_SOLVER_DEPONDT && !jit_ready(s))
+        return spin::fail(SPIN_ERR_STATE, "the Heun and SIB solvers need the run-time specialised kernels (%s)", s->jit_note.c_str());
     int64_t done = 0;
     // Launch-bound lattices: replay a captured graph of G steps (an even number, so the ping-pong buffers return to the
     // same roles); the kernels read the step counter from device memory, the graph's last node advances it by G.

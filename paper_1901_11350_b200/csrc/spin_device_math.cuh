@@ -75,6 +75,31 @@ __device__ __forceinline__ void rodrigues(const double (&A)[3], double dt, doubl
     out[2] = n[2] * c - cz * ds + A[2] * an;
 }
 
+// Implicit-midpoint structure of the SIB solver (App. C, C5-C10): x + A' x x = n + n x A' with A' = (dt/2) A.
+// The paper solves the 3x3 system by Cramer's rule; its closed form is x = [a + A'(a.A') - A' x a] / (1 + |A'|^2), a = n + n x A'
+// (dot the equation with A' for x.A' = a.A', cross it with A' and eliminate A' x x).  |x| = |n| exactly (Cayley transform).
+__device__ __forceinline__ void imp_update(const double (&A)[3], double hdt, const double (&n)[3], double (&out)[3]) {
+    const double Ah[3] = {hdt * A[0], hdt * A[1], hdt * A[2]};
+    const double a[3] = {n[0] + (n[1] * Ah[2] - n[2] * Ah[1]), n[1] + (n[2] * Ah[0] - n[0] * Ah[2]), n[2] + (n[0] * Ah[1] - n[1] * Ah[0])};
+    const double aA = a[0] * Ah[0] + a[1] * Ah[1] + a[2] * Ah[2];
+    const double inv = 1.0 / (1.0 + (Ah[0] * Ah[0] + Ah[1] * Ah[1] + Ah[2] * Ah[2]));
+    out[0] = (a[0] + Ah[0] * aA - (Ah[1] * a[2] - Ah[2] * a[1])) * inv;
+    out[1] = (a[1] + Ah[1] * aA - (Ah[2] * a[0] - Ah[0] * a[2])) * inv;
+    out[2] = (a[2] + Ah[2] * aA - (Ah[0] * a[1] - Ah[1] * a[0])) * inv;
+}
+
+// Heun (App. B, B3-B4) with f = n x A:  f(n, A) added to `acc` with weight w
+__device__ __forceinline__ void heun_add(const double (&n)[3], const double (&A)[3], double w, double (&acc)[3]) {
+    acc[0] = fma(w, n[1] * A[2] - n[2] * A[1], acc[0]);
+    acc[1] = fma(w, n[2] * A[0] - n[0] * A[2], acc[1]);
+    acc[2] = fma(w, n[0] * A[1] - n[1] * A[0], acc[2]);
+}
+
+__device__ __forceinline__ void renormalise_general(double (&v)[3]) {      // Heun: |v| is not close to 1 to rounding
+    const double sc = 1.0 / sqrt(v[0] * v[0] + v[1] * v[1] + v[2] * v[2]);
+    v[0] *= sc; v[1] *= sc; v[2] *= sc;
+}
+
 __device__ __forceinline__ void renormalise(double (&v)[3]) {
     // |v|^2 = 1 + eps with eps ~ 1e-16 after a rotation of a unit vector: 1/sqrt(1+eps) by its series
     const double eps = fma(v[0], v[0], fma(v[1], v[1], fma(v[2], v[2], -1.0)));

@@ -157,7 +157,7 @@ static void jit_brick_launch(const spin_system *s, dim3 &grid, dim3 &block) {
 // SPINLLG_COL="cbx,cby,ccz" overrides the defaults (32 x 4 columns, 16 planes per chunk).
 static bool plan_col(const spin_system *s, int g[4]) {
     const DevicePlan &P = s->plan;
-    if (!s->opt_col || s->opt_store_A || P.rC < 1 || P.Nc < 2) return false;
+    if (!s->opt_col || s->opt_store_A || s->solver != 0 || P.rC < 1 || P.Nc < 2) return false;
     int cbx = 32, cby = 4, ccz = 16;
     if (const char *e = getenv("SPINLLG_COL")) {
         int v[3] = {0, 0, 0};
@@ -175,6 +175,7 @@ static bool plan_col(const spin_system *s, int g[4]) {
 // the staging geometry of both sweeps, or why the TMA-fed sweeps are not generated for this system
 static bool plan_tma(const spin_system *s, TmaGeo &gp, TmaGeo &gc, std::string &why) {
     if (!s->opt_tma) { why = "disabled by option use_tma=0"; return false; }
+    if (s->solver != 0) { why = "Depondt solver only"; return false; }
     if (s->opt_store_A) { why = "store_A=1 uses the brick kernels"; return false; }
     if (s->opt_tma < 2 && s->N < 16384) { why = "lattice too small to fill persistent CTAs"; return false; }
     return plan_tma_geo(s, 1, "SPINLLG_TMA_P", gp, why) && plan_tma_geo(s, 2, "SPINLLG_TMA_C", gc, why);
@@ -196,7 +197,8 @@ std::string spin::jit_source(const spin_system *s) {
     o << "constexpr int BX = " << brick[0] << ", BY = " << brick[1] << ", BZ = " << brick[2] << ";\n";
     o << "constexpr bool PER_A = " << (P.perA ? "true" : "false") << ", PER_B = " << (P.perB ? "true" : "false")
       << ", PER_C = " << (P.perC ? "true" : "false") << ";\n";
-    o << "constexpr bool STORE_A = " << (s->opt_store_A ? "true" : "false") << ", HAS_DDI = " << (P.has_ddi ? "true" : "false")
+    o << "constexpr int SOLVER = " << s->solver << ";      // 0 Depondt, 1 Heun, 2 SIB\n";
+    o << "constexpr bool STORE_A = " << ((s->opt_store_A && s->solver == 0) ? "true" : "false") << ", HAS_DDI = " << (P.has_ddi ? "true" : "false")
       << ", THERMAL_ON = " << (P.thermal_on ? "true" : "false") << ", STT_ON = " << (P.stt_on ? "true" : "false") << ";\n";
     {   // partners in the own lattice row by warp shuffle: measured slower than the L1 hits it replaces (66 -> 79 us per step on
         // cfg3), so off unless SPINLLG_SHFL=1

@@ -115,6 +115,18 @@ struct GlobalAcc {
     __device__ __forceinline__ void set_own(int k, const double (&o)[3]) { own[k][0] = o[0]; own[k][1] = o[1]; own[k][2] = o[2]; }
 };
 
+// SIB corrector (C11): the field is evaluated at the midpoint configuration {(n_j + n_j^p)/2}
+struct MidAcc {
+    const double *a, *b;           // own site in n and in n^p
+    template <int B, int BJ, int DA, int DB, int DC>
+    __device__ __forceinline__ void load(int, double (&v)[3]) const {
+        double u[3], w[3];
+        load3<lin<B, BJ, DA, DB, DC>()>(a, u);
+        load3<lin<B, BJ, DA, DB, DC>()>(b, w);
+        v[0] = 0.5 * (u[0] + w[0]); v[1] = 0.5 * (u[1] + w[1]); v[2] = 0.5 * (u[2] + w[2]);
+    }
+};
+
 // F += (Zeeman + anisotropy + pairs + quadruplets) of basis atom B for NCONF configurations sharing the lattice
 template <int B, int NCONF, class Acc>
 __device__ __forceinline__ void force(const Acc &cfg, const double (&own)[NCONF][3], double (&F)[NCONF][3]) {
@@ -272,7 +284,9 @@ __device__ __forceinline__ void predictor_body(const double *__restrict__ n, con
     out[0] = own[0][0] + F[0][0]; out[1] = own[0][1] + F[0][1]; out[2] = own[0][2] + F[0][2];
 #else
     rotation_field<B>(own[0], F[0], sg[0], A);
-    spin::rodrigues(A, specc::DT, specc::DT2, own[0], out);
+    if constexpr (spec::SOLVER == 0) spin::rodrigues(A, specc::DT, specc::DT2, own[0], out);                 // B5
+    else if constexpr (spec::SOLVER == 1) { out[0] = own[0][0]; out[1] = own[0][1]; out[2] = own[0][2]; spin::heun_add(own[0], A, specc::DT, out); }   // B3
+    else spin::imp_update(A, specc::HDT, own[0], out);                                                        // C5
 #endif
 #if SPIN_ABLATE & 2
     if (out[0] == 123.456)
@@ -295,6 +309,25 @@ __device__ __forceinline__ void corrector_body(const double *__restrict__ n, con
     double th[3], A[3], Ap[3], n0[3];
     thermal_force<B>(c, step, seed_lo, seed_hi, th);
     load3<0>(n + idx, n0);
+    if constexpr (spec::SOLVER == 2) {
+        // SIB corrector (C11): A at the midpoint configuration, the implicit-midpoint structure applied to n(t); A(n) is not needed
+        const MidAcc cfg = {n + idx, np + idx};
+        double own[1][3], F[1][3] = {{th[0], th[1], th[2]}}, sg[1][3] = {{0.0, 0.0, 0.0}};
+        cfg.load<B, B, 0, 0, 0>(0, own[0]);
+        force<B, 1>(cfg, own, F);
+        if constexpr (spec::HAS_DDI) {      // the dipolar force is linear in the configuration: its value at the midpoint is the mean
+            double d[3], e[3];
+            load3<0>(fddi_n + idx, d); load3<0>(fddi_np + idx, e);
+            F[0][0] += 0.5 * (d[0] + e[0]); F[0][1] += 0.5 * (d[1] + e[1]); F[0][2] += 0.5 * (d[2] + e[2]);
+        }
+        if constexpr (spec::STT_ON) stt_gradient<B, 1>(cfg, c, own, sg);
+        rotation_field<B>(own[0], F[0], sg[0], Ap);
+        double out[3];
+        spin::imp_update(Ap, specc::HDT, n0, out);
+        store_spin(nout + idx, c, out);
+        return;
+    }
+    double np0[3] = {0.0, 0.0, 0.0};
     if constexpr (spec::STORE_A) {
         GlobalAcc<1> cfg;
         cfg.cfg[0] = np + idx; cfg.mask = mask; cfg.lane = (int)(threadIdx.x & 31u);
@@ -312,6 +345,7 @@ __device__ __forceinline__ void corrector_body(const double *__restrict__ n, con
         double own[2][3], F[2][3] = {{th[0], th[1], th[2]}, {th[0], th[1], th[2]}}, sg[2][3] = {{0.0, 0.0, 0.0}, {0.0, 0.0, 0.0}};
         own[0][0] = n0[0]; own[0][1] = n0[1]; own[0][2] = n0[2];
         load3<0>(cfg.cfg[1], own[1]);
+        np0[0] = own[1][0]; np0[1] = own[1][1]; np0[2] = own[1][2];
         cfg.set_own(0, own[0]); cfg.set_own(1, own[1]);
         force<B, 2>(cfg, own, F);
         if constexpr (spec::HAS_DDI) {
@@ -323,11 +357,19 @@ __device__ __forceinline__ void corrector_body(const double *__restrict__ n, con
         rotation_field<B>(own[0], F[0], sg[0], A);
         rotation_field<B>(own[1], F[1], sg[1], Ap);
     }
-    // A^c = (A + A^p)/2: the factor 1/2 is folded into the time step (dt/2, dt^2/4 are exact scalings, the result is bit-identical)
-    const double Ac[3] = {A[0] + Ap[0], A[1] + Ap[1], A[2] + Ap[2]};
     double out[3];
-    spin::rodrigues(Ac, specc::HDT, specc::QDT2, n0, out);
-    spin::renormalise(out);
+    if constexpr (spec::SOLVER == 1) {
+        // Heun corrector (B4): n + dt/2 (n x A + n^p x A^p), renormalised every step
+        out[0] = n0[0]; out[1] = n0[1]; out[2] = n0[2];
+        spin::heun_add(n0, A, specc::HDT, out);
+        spin::heun_add(np0, Ap, specc::HDT, out);
+        spin::renormalise_general(out);
+    } else {
+        // A^c = (A + A^p)/2: the factor 1/2 is folded into the time step (dt/2, dt^2/4 are exact scalings, the result is bit-identical)
+        const double Ac[3] = {A[0] + Ap[0], A[1] + Ap[1], A[2] + Ap[2]};
+        spin::rodrigues(Ac, specc::HDT, specc::QDT2, n0, out);
+        spin::renormalise(out);
+    }
     store_spin(nout + idx, c, out);
 }
 

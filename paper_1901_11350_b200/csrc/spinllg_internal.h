@@ -111,6 +111,7 @@ struct spin_system {
     // ---- LLG
     double dt_ps, alpha, T, u, jdir[3], beta;
     uint64_t seed, step;
+    int solver;                    // SPIN_SOLVER_*
     // ---- device
     cudaStream_t stream, own_stream;
     double *d_n[2];                // ping-pong spin buffers (nb*sub doubles each)

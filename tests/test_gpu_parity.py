@@ -363,3 +363,33 @@ def test_column_marching_with_open_and_mixed_boundaries(P, O):
         assert g.spin_kernel_info() == "jit+col"
         g.llg_iterate(30); o.iterate(30)
         assert np.abs(g.spins_get() - o.spins()).max() <= SPIN_ATOL
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# Other solvers on the same two field sweeps: Heun (App. B B3-B4) and SIB (App. C C5-C11)
+@pytest.mark.parametrize("solver", [1, 2])
+@pytest.mark.parametrize("cfg,steps", [(1, 300), (2, 200), (3, 150), (4, 150), (5, 30)])
+def test_heun_and_sib_trajectory_parity(P, O, cfg, steps, solver):
+    w = W.CONFIGS[cfg]().resized(REPLICAS[cfg], steps)
+    g, o = pair(P, O, w)
+    g.llg_set_solver(solver); o.set_solver(solver)
+    g.llg_iterate(steps); o.iterate(steps)
+    ng, no = g.spins_get(), o.spins()
+    d = np.abs(ng - no).max()
+    print(f"solver {solver} cfg{cfg} replica steps={steps}: max|dn| = {d:.3e}")
+    assert d <= SPIN_ATOL
+    assert np.abs(np.linalg.norm(ng, axis=1) - 1).max() < (1e-12 if solver == 2 else 4e-16)      # SIB: preserved, not renormalised
+    # a different solver gives a different trajectory (the option is not ignored)
+    h = P.SpinSystem.from_workload(w); h.llg_iterate(steps)
+    assert np.abs(h.spins_get() - ng).max() > 1e-12
+
+
+def test_solver_needs_specialised_kernels(P):
+    s = P.SpinSystem.from_workload(W.config1().resized((8, 8, 1), 4))
+    s.spin_set_option("use_jit", 0)
+    s.llg_set_solver(2)
+    with pytest.raises(P.SpinError) as e:
+        s.llg_iterate(1)
+    assert e.value.code == -2
+    with pytest.raises(P.SpinError):
+        s.llg_set_solver(7)
