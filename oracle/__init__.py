@@ -67,6 +67,10 @@ def lib():
         L.orc_llg_iterate.argtypes = [vp, C.c_long]
         L.orc_heun_step.argtypes = [vp]
         L.orc_set_solver.argtypes = [vp, C.c_int]
+        L.orc_topological_charge.argtypes = [vp, dp]
+        L.orc_topological_charge.restype = C.c_double
+        L.orc_spherical_area.argtypes = [dp, dp, dp]
+        L.orc_spherical_area.restype = C.c_double
         L.orc_effective_field.argtypes = [vp, dp]
         L.orc_observables.argtypes = [vp, dp, dp]
         _lib = L
@@ -239,12 +243,22 @@ class OracleSystem:
     def iterate(self, n_steps):
         lib().orc_llg_iterate(self._h, int(n_steps))
 
+    def topological_charge(self, n=None):
+        """Q of App. A summed over the a-b planes (one basis atom)."""
+        a, p = _d(self.spins() if n is None else n)
+        return float(lib().orc_topological_charge(self._h, p))
+
     def set_solver(self, solver):
         """0 Depondt (App. B B5-B7), 1 Heun (B3-B4), 2 SIB semi-implicit midpoint (App. C)."""
         lib().orc_set_solver(self._h, int(solver))
 
     def heun_step(self):
         lib().orc_heun_step(self._h)
+
+
+def spherical_area(ni, nj, nk):
+    (a, pa), (b, pb), (c, pc) = _d(ni), _d(nj), _d(nk)
+    return float(lib().orc_spherical_area(pa, pb, pc))
 
 
 def philox4x32_10(counter, key):

@@ -15,6 +15,7 @@
  *   thermal field     Eq. 11 (:157-160)                     -> orc_thermal_xi, sigma
  *   Depondt solver    App. B, B5-B7 (:369-380)              -> orc_llg_step (solver 0)
  *   Heun solver       App. B, B3-B4 (:355-367)              -> orc_llg_step (solver 1); orc_heun_step = the same written on its own (pin)
+ *   topological charge App. A, A1-A2 (:317-343)             -> orc_topological_charge, orc_spherical_area
  *   SIB solver        App. C, C5-C11 (:384-436)             -> orc_llg_step (solver 2), imp_update (Cramer's rule as printed)
  * Readings of silent / garbled passages are listed in DESIGN.md ("Readings") under the
  * same R-numbers as SURVEY.md 8(c).
@@ -835,6 +836,46 @@ void orc_heun_step(orc_system *s) {
     }
     s->step += 1;
     free(F); free(f0); free(np_); free(sg);
+}
+
+/* ------------------------------------------------------------------ topological charge, App. A (:317-343)
+ * Q = (1/4 pi) sum_l A_l (A1) over the elementary triangles l of every a-b plane, A_l the signed area of the spherical
+ * triangle (n_i, n_j, n_k):  cos(A_l/2) = (1 + ni.nj + ni.nk + nj.nk) / sqrt(2 (1+ni.nj)(1+nj.nk)(1+nk.ni))  (A2),
+ * sign(A_l) = sign[n_i . (n_j x n_k)] (the extracted text prints "n_i . (n_i x n_k)", which is identically zero: garbled,
+ * reading R26).  Triangles: each cell (ia, ib) gives (r, r+a, r+a+b) and (r, r+a+b, r+b), counter-clockwise about +z
+ * when (a x b).z > 0 (the order is mirrored otherwise, :331).  One basis atom.  A triangle with a corner outside an open
+ * edge is skipped; periodic directions wrap (":343 only defined with periodical boundary conditions").               */
+static double spherical_area(const double *ni, const double *nj, const double *nk) {
+    double ij = dot3(ni, nj), ik = dot3(ni, nk), jk = dot3(nj, nk);
+    double den = sqrt(2.0 * (1.0 + ij) * (1.0 + jk) * (1.0 + ik));
+    if (den == 0.0) return 0.0;                        /* exceptional configuration (A3): not defined, counted as 0 */
+    double c = (1.0 + ij + ik + jk) / den;
+    if (c > 1.0) c = 1.0;
+    if (c < -1.0) c = -1.0;
+    double A = 2.0 * acos(c), jxk[3];
+    cross3(nj, nk, jxk);
+    double t = dot3(ni, jxk);
+    return t > 0.0 ? A : (t < 0.0 ? -A : 0.0);
+}
+double orc_spherical_area(const double *ni, const double *nj, const double *nk) { return spherical_area(ni, nj, nk); }
+double orc_topological_charge(const orc_system *s, const double *n) {
+    if (s->nb != 1) return NAN;
+    const double *a = s->brav, *b = s->brav + 3;
+    int ccw = (a[0] * b[1] - a[1] * b[0]) > 0.0;
+    long double sum = 0.0L;
+    for (int ic = 0; ic < s->nc[2]; ++ic)
+        for (int ib = 0; ib < s->nc[1]; ++ib)
+            for (int ia = 0; ia < s->nc[0]; ++ia) {
+                int ia1 = ia + 1, ib1 = ib + 1;
+                if (ia1 == s->nc[0]) { if (!s->per[0]) continue; ia1 = 0; }
+                if (ib1 == s->nc[1]) { if (!s->per[1]) continue; ib1 = 0; }
+                int c00[3] = {ia, ib, ic}, c10[3] = {ia1, ib, ic}, c11[3] = {ia1, ib1, ic}, c01[3] = {ia, ib1, ic};
+                const double *n00 = n + 3 * cell_index(s, c00), *n10 = n + 3 * cell_index(s, c10);
+                const double *n11 = n + 3 * cell_index(s, c11), *n01 = n + 3 * cell_index(s, c01);
+                if (ccw) sum += spherical_area(n00, n10, n11) + spherical_area(n00, n11, n01);
+                else     sum += spherical_area(n00, n11, n10) + spherical_area(n00, n01, n11);
+            }
+    return (double)(sum / (4.0L * (long double)ORC_PI));
 }
 
 /* ------------------------------------------------------------------ what the boundary returns

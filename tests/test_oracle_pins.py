@@ -511,3 +511,50 @@ def test_workload_pair_lists_are_complete_shells(cfg, expected):
             dist = round(dist, 9)
             assert count[dist] == z == brute[dist], (cfg, b, dist, count, brute.get(dist))
         assert set(count) == {round(k, 9) for k in expected}
+
+
+# ------------------------------------------------------------------ topological charge, App. A
+def _girard_area(a, b, c):
+    """Spherical excess (Girard): area = alpha + beta + gamma - pi from the corner angles -- independent of Eq. A2."""
+    def corner(p, q, r):
+        u = np.cross(p, q); v = np.cross(p, r)
+        return math.acos(np.clip(np.dot(u, v) / (np.linalg.norm(u) * np.linalg.norm(v)), -1, 1))
+    return corner(a, b, c) + corner(b, c, a) + corner(c, a, b) - math.pi
+
+
+def test_topological_charge_spherical_triangle_area():
+    """Eq. A2: one octant of the sphere has area 4 pi / 8; orientation gives the sign; random triangles
+    agree with Girard's spherical excess."""
+    x, y, z = np.eye(3)
+    assert O.spherical_area(x, y, z) == pytest.approx(math.pi / 2, abs=1e-15)
+    assert O.spherical_area(x, z, y) == pytest.approx(-math.pi / 2, abs=1e-15)
+    rng = np.random.default_rng(11)
+    for _ in range(200):
+        t = rng.standard_normal((3, 3)); t /= np.linalg.norm(t, axis=1, keepdims=True)
+        sgn = np.sign(np.dot(t[0], np.cross(t[1], t[2])))
+        assert O.spherical_area(*t) == pytest.approx(sgn * _girard_area(*t), abs=1e-9)
+
+
+@pytest.mark.parametrize("cfg,cells", [(1, (40, 40, 1)), (2, (36, 36, 1))])
+def test_topological_charge_of_textures(cfg, cells):
+    """Q = -1 for a skyrmion in a +z background, +1 for the antiskyrmion, 0 for the ferromagnet, additive,
+    odd under n -> -n; an integer to rounding on a periodic lattice (Berg-Luescher)."""
+    w = small(cfg, cells)
+    s = OracleSystem.from_workload(w)
+    fm = np.tile([0.0, 0.0, 1.0], (w.n_spins, 1))
+    assert s.topological_charge(fm) == 0.0
+    pos = w.positions()
+    ctr = pos[:, :2].mean(axis=0)
+    sk = W.skyrmion_spins(w, 9.0)
+    assert s.topological_charge(sk) == pytest.approx(-1.0, abs=1e-12)
+    anti = sk * np.array([1.0, -1.0, 1.0])
+    assert s.topological_charge(anti) == pytest.approx(+1.0, abs=1e-12)
+    assert s.topological_charge(-sk) == pytest.approx(+1.0, abs=1e-12)
+    two = W.skyrmion_spins(w, 6.0, centre=ctr - [8.0, 0.0])
+    other = W.skyrmion_spins(w, 6.0, centre=ctr + [8.0, 0.0])
+    inside = np.linalg.norm(pos[:, :2] - (ctr + [8.0, 0.0]), axis=1) < 6.0
+    two[inside] = other[inside]
+    assert s.topological_charge(two) == pytest.approx(-2.0, abs=1e-12)
+    # a random configuration on a periodic lattice still has an integer charge
+    q = s.topological_charge(rand_spins(w.n_spins, 5))
+    assert abs(q - round(q)) < 1e-9
