@@ -132,6 +132,11 @@ int energy(spin_system *sys, double *E_total_meV, double E_terms_meV[6]);
 /* M = (1/N) sum_i n_i (:131) and max_i |F_i - (F_i.n_i) n_i| in meV                                        */
 int observables(spin_system *sys, double M[3], double *max_torque_meV);
 
+/* topological charge of App. A (:317-343), Eqs. A1-A2: Q = (1/4 pi) sum of the signed spherical-triangle areas over the two
+ * elementary triangles (r, r+a, r+a+b), (r, r+a+b, r+b) of every cell, counter-clockwise about +z, summed over the a-b planes.
+ * One basis atom (SPIN_ERR_ARG otherwise).  Periodic directions wrap; triangles leaving an open edge are skipped (:343).  */
+int topological_charge(spin_system *sys, double *Q);
+
 /* ---- introspection (measurement support) -------------------------------------------------------------- */
 /* number of kernel launches (own kernels) and cuFFT executions issued by this system so far */
 int spin_launch_counts(const spin_system *sys, int64_t *own_kernels, int64_t *cufft_execs);

@@ -21,7 +21,7 @@ EXPORTS = [
     "hamiltonian_set_exchange_shells", "hamiltonian_set_dmi_shells", "hamiltonian_set_quadruplets",
     "hamiltonian_set_ddi", "spins_set", "spins_get", "spins_set_device", "spins_get_device",
     "llg_configure", "llg_set_solver", "llg_iterate", "llg_get_step", "llg_set_step", "spin_synchronize",
-    "effective_field", "effective_field_device", "energy", "observables",
+    "effective_field", "effective_field_device", "energy", "observables", "topological_charge",
     "spin_launch_counts", "spin_profile_enable", "spin_profile_get", "spin_set_option",
     "spin_kernel_info", "spin_jit_source", "spin_last_error", "spin_version",
 ]
@@ -71,6 +71,7 @@ def lib() -> C.CDLL:
         "effective_field_device": (C.c_int, [vp, vp]),
         "energy": (C.c_int, [vp, dp, dp]),
         "observables": (C.c_int, [vp, dp, dp]),
+        "topological_charge": (C.c_int, [vp, dp]),
         "spin_launch_counts": (C.c_int, [vp, i64p, i64p]),
         "spin_profile_enable": (C.c_int, [vp, C.c_int]),
         "spin_profile_get": (C.c_int, [vp, C.c_int, dp, i64p]),
@@ -216,6 +217,11 @@ class SpinSystem:
     def llg_configure(self, dt_fs, alpha, T=0.0, seed=0, u=0.0, j_dir=(1, 0, 0), beta=0.0):
         j, jp = _d(j_dir)
         _check(lib().llg_configure(self._h, float(dt_fs), float(alpha), float(T), int(seed), float(u), jp, float(beta)))
+
+    def topological_charge(self):
+        q = C.c_double(0.0)
+        _check(lib().topological_charge(self._h, C.byref(q)))
+        return float(q.value)
 
     def llg_set_solver(self, solver):
         """0 Depondt, 1 Heun, 2 SIB (include/spinllg.h SPIN_SOLVER_*)."""

@@ -829,6 +829,27 @@ extern "C" int observables(spin_system *s, double M[3], double *max_torque) {
     return SPIN_OK;
 }
 
+// Q of App. A summed over the a-b planes; one basis atom
+extern "C" int topological_charge(spin_system *s, double *Q) {
+    REQUIRE(s && Q, "null argument");
+    REQUIRE(s->nb == 1, "the topological charge is defined for one basis atom (triangulation of a Bravais lattice)");
+    int rc = ensure_plan(s);
+    if (rc) return rc;
+    const int nblk = (int)((s->ncell + 255) / 256);
+    const int ccw = (s->brav[0] * s->brav[4] - s->brav[1] * s->brav[3]) > 0.0 ? 1 : 0;
+    double *d_part = nullptr;
+    SPIN_CUDA(cudaMalloc(&d_part, (size_t)nblk * sizeof(double)));
+    topo_kernel<<<nblk, 256, 0, s->stream>>>(s->plan, s->d_n[s->cur], ccw, d_part);
+    topo_final_kernel<<<1, 32, 0, s->stream>>>(d_part, nblk, s->d_result);
+    s->n_launch += 2;
+    cudaError_t e = cudaMemcpyAsync(Q, s->d_result, sizeof(double), cudaMemcpyDeviceToHost, s->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s->stream);
+    cudaFree(d_part);
+    if (e != cudaSuccess) return spin::fail(SPIN_ERR_CUDA, "topological_charge: %s", cudaGetErrorString(e));
+    SPIN_CUDA(cudaGetLastError());
+    return SPIN_OK;
+}
+
 // ---------------------------------------------------------------------------------------------- introspection
 extern "C" int spin_launch_counts(const spin_system *s, int64_t *own, int64_t *fft) {
     REQUIRE(s, "null system");

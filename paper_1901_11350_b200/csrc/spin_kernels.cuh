@@ -364,6 +364,52 @@ __global__ void reduce_final_kernel(const double *__restrict__ partials, int nbl
     if (lane == 0) out[k] = r;
 }
 
+// Topological charge, App. A: Q = (1/4 pi) sum_l A_l over the two elementary triangles of every cell of every
+// a-b plane; A_l = signed area of the spherical triangle (n_i, n_j, n_k), evaluated as 2 atan2(n_i.(n_j x n_k), 1 + n_i.n_j +
+// n_j.n_k + n_k.n_i) -- the same angle as Eq. A2 with its sign rule, without the square root and the acos near +-1.
+__device__ __forceinline__ double spherical_area(const double (&a)[3], const double (&b)[3], const double (&c)[3]) {
+    const double t = a[0] * (b[1] * c[2] - b[2] * c[1]) + a[1] * (b[2] * c[0] - b[0] * c[2]) + a[2] * (b[0] * c[1] - b[1] * c[0]);
+    const double d = 1.0 + (a[0] * b[0] + a[1] * b[1] + a[2] * b[2]) + (b[0] * c[0] + b[1] * c[1] + b[2] * c[2]) + (c[0] * a[0] + c[1] * a[1] + c[2] * a[2]);
+    return (t == 0.0) ? 0.0 : 2.0 * atan2(t, d);
+}
+// one thread per cell (one basis atom); partial sums per block, folded by topo_final_kernel in a fixed order
+__global__ void __launch_bounds__(256) topo_kernel(const __grid_constant__ DevicePlan P, const double *__restrict__ n, int ccw,
+                                                   double *__restrict__ partials) {
+    __shared__ double sh[8];
+    const int cell = blockIdx.x * 256 + threadIdx.x;
+    double v = 0.0;
+    if (cell < P.Ncell) {
+        const int ia = cell % P.Na, ib = (cell / P.Na) % P.Nb, ic = cell / (P.Na * P.Nb);
+        int ia1 = ia + 1, ib1 = ib + 1;
+        bool ok = true;
+        if (ia1 == P.Na) { if (P.perA) ia1 = 0; else ok = false; }
+        if (ib1 == P.Nb) { if (P.perB) ib1 = 0; else ok = false; }
+        if (ok) {
+            double n00[3], n10[3], n11[3], n01[3];
+            load3(P, n, site_index(P, 0, ia, ib, ic), n00);
+            load3(P, n, site_index(P, 0, ia1, ib, ic), n10);
+            load3(P, n, site_index(P, 0, ia1, ib1, ic), n11);
+            load3(P, n, site_index(P, 0, ia, ib1, ic), n01);
+            v = ccw ? spherical_area(n00, n10, n11) + spherical_area(n00, n11, n01)
+                    : spherical_area(n00, n11, n10) + spherical_area(n00, n01, n11);
+        }
+    }
+    v = warp_sum(v);
+    if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = v;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double r = sh[0];
+        for (int i = 1; i < 8; ++i) r += sh[i];
+        partials[blockIdx.x] = r;
+    }
+}
+__global__ void topo_final_kernel(const double *__restrict__ partials, int nblocks, double *__restrict__ out) {
+    double r = 0.0;
+    for (int i = threadIdx.x; i < nblocks; i += 32) r += partials[i];
+    r = warp_sum(r);
+    if (threadIdx.x == 0) out[0] = r * (1.0 / (4.0 * 3.14159265358979323846));
+}
+
 __global__ void advance_step_kernel(unsigned long long *d_step, unsigned long long add) { *d_step += add; }
 
 }  // namespace spin

@@ -393,3 +393,26 @@ def test_solver_needs_specialised_kernels(P):
     assert e.value.code == -2
     with pytest.raises(P.SpinError):
         s.llg_set_solver(7)
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# Topological charge reduction (App. A)
+@pytest.mark.parametrize("cfg,cells,per", [(1, (40, 37, 1), (1, 1, 0)), (2, (36, 36, 1), (1, 1, 0)), (1, (33, 20, 1), (0, 1, 0)), (3, (20, 18, 5), (1, 1, 1))])
+def test_topological_charge_parity(P, O, cfg, cells, per):
+    """Tolerance 1e-7 absolute: the oracle evaluates Eq. A2 as printed, A = 2 acos(c), whose condition number 1/sin(A/2) turns an
+    ulp of c into ~1e-8..1e-10 per small triangle; the kernel uses the atan2 form of the same angle (exact to ulps).  Any real
+    mistake moves Q by a triangle area (>= 1e-3) or an integer."""
+    w = dataclasses.replace(W.CONFIGS[cfg]().resized(cells, 10), periodic=per)
+    g, o = pair(P, O, w)
+    for n in (W.skyrmion_spins(w, 8.0), w.initial_spins()):
+        g.spins_set(n); o.set_spins(n)
+        qg, qo = g.topological_charge(), o.topological_charge()
+        assert abs(qg - qo) <= 1e-7, (qg, qo)
+    g.spins_set(W.skyrmion_spins(w, 8.0))
+    if per[0] and per[1]:
+        assert g.topological_charge() == pytest.approx(-1.0 * cells[2], abs=1e-10)
+    g.llg_iterate(10); o.set_spins(g.spins_get())
+    assert abs(g.topological_charge() - o.topological_charge()) <= 1e-7
+    two = P.SpinSystem.from_workload(W.config4().resized((8, 8, 1), 1))
+    with pytest.raises(P.SpinError):
+        two.topological_charge()
