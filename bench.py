@@ -3,7 +3,7 @@
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 3] [--inner 100]
 
-One bench "step" = one `llg_iterate(inner)` call = `inner` Depondt iterations (each: field of every spin at n,
+One bench "step" = one `llg_iterate(inner)` call = `inner` (default 128) Depondt iterations (each: field of every spin at n,
 predictor, field at n^p, corrector; all rows of SURVEY 8(a)) over the whole lattice.  Workload at N=1: configs[2] of
 BASELINE.json, the 3-D simple cubic 128^3 lattice (2,097,152 spins) the headline metric is quoted on.
     value   whole-job spin-updates/s, state resident in HBM, CUDA events on the launching stream, max over ranks
@@ -146,7 +146,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=3, help="BASELINE.json config number (1-5); default 3 = 128^3 headline")
-    ap.add_argument("--inner", type=int, default=100, help="LLG iterations per bench step")
+    ap.add_argument("--inner", type=int, default=128, help="LLG iterations per bench step (a multiple of the 16-step CUDA graph)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--store-A", type=int, default=0)
     args = ap.parse_args()
