@@ -184,7 +184,7 @@ static bool plan_tma(const spin_system *s, TmaGeo &gp, TmaGeo &gc, std::string &
 std::string spin::jit_source(const spin_system *s) {
     const DevicePlan &P = s->plan;
     std::ostringstream o;
-    const bool flat = s->nc[2] < 2;
+    
     o << "// generated by spin_jit.cu -- one spin system as compile-time constants\n";
     o << "namespace spec {\n";
     o << "constexpr int NA = " << P.Na << ", NB = " << P.Nb << ", NC = " << P.Nc << ", NBASIS = " << P.nb << ";\n";
@@ -200,15 +200,6 @@ std::string spin::jit_source(const spin_system *s) {
     o << "constexpr int SOLVER = " << s->solver << ";      // 0 Depondt, 1 Heun, 2 SIB\n";
     o << "constexpr bool STORE_A = " << ((s->opt_store_A && s->solver == 0) ? "true" : "false") << ", HAS_DDI = " << (P.has_ddi ? "true" : "false")
       << ", THERMAL_ON = " << (P.thermal_on ? "true" : "false") << ", STT_ON = " << (P.stt_on ? "true" : "false") << ";\n";
-    {   // partners in the own lattice row by warp shuffle: measured slower than the L1 hits it replaces (66 -> 79 us per step on
-        // cfg3), so off unless SPINLLG_SHFL=1
-        const char *e = getenv("SPINLLG_SHFL");
-        o << "constexpr bool SHFL = " << ((e && atoi(e) != 0) ? "true" : "false") << ";\n";
-    }
-    // L2 prefetch distance of the brick kernels, in lattice planes (SPINLLG_PREFETCH overrides; 0 = off)
-    int pf = 0;
-    if (const char *e = getenv("SPINLLG_PREFETCH")) pf = atoi(e);
-    o << "constexpr int PF_PLANES = " << (flat ? 0 : pf) << ";\n";
     const int np = P.pair_begin[P.nb], nq = P.quad_begin[P.nb];
     emit_array<int>(o, "int", "PAIR_BEGIN", P.nb + 1, [&](int i) { return std::to_string(P.pair_begin[i]); });
     emit_array<int>(o, "int", "P_DA", np, [&](int i) { return std::to_string(P.pairs[i].da); });
@@ -284,8 +275,6 @@ std::string spin::jit_source(const spin_system *s) {
     const bool col = plan_col(s, cg);
     if (col) o << "namespace spec { constexpr int CBX = " << cg[0] << ", CBY = " << cg[1] << ", CCZ = " << cg[2] << ", CNZC = " << cg[3] << "; }\n#define SPIN_COL 1\n";
     if (tma) o << "#define SPIN_TMA 1\n";
-    if (const char *e = getenv("SPINLLG_MINBLOCKS")) o << "#define SPIN_MINBLOCKS " << atoi(e) << "\n";
-    if (const char *e = getenv("SPINLLG_ABLATE")) o << "#define SPIN_ABLATE " << atoi(e) << "\n";
     o << "#include \"spin_jit_kernels.cuh\"\n";
     return o.str();
 }

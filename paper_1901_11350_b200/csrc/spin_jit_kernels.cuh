@@ -19,14 +19,7 @@
 //   double ALPHA, DT, DT2, STT_C[3], STT_S, STT_X;
 #pragma once
 
-#ifndef SPIN_ABLATE
-#define SPIN_ABLATE 0
-#endif
-#ifdef SPIN_MINBLOCKS
-#define SPIN_BOUNDS(t) __launch_bounds__(t, SPIN_MINBLOCKS)
-#else
 #define SPIN_BOUNDS(t) __launch_bounds__(t)
-#endif
 #include "spin_device_math.cuh"
 
 namespace spinjit {
@@ -91,28 +84,11 @@ __device__ __forceinline__ void store_spin(double *__restrict__ q, const Coord &
 // Site accessors: where the partner (sublattice BJ at translation DA, DB, DC) of a site of sublattice B is read from.
 // GlobalAcc: the ghost-cell arrays in global memory (own address + immediate); RingAcc (spin_jit_tma.cuh): the ring of lattice
 // planes that TMA stages in shared memory.
-// With spec::SHFL, partners in the own lattice row (same sublattice, translation along a only) come from the neighbouring
-// lanes' own spins by warp shuffle -- a brick row is one warp -- and only the lanes at the ends of the row (or next to a lane
-// outside the lattice) go to memory: 6 of the 21 vector loads of a nearest-neighbour stencil become single-lane loads.
 template <int NCONF>
 struct GlobalAcc {
     const double *cfg[NCONF];      // x component of the own site in configuration k
-    double own[NCONF][3];          // the own spin (shuffle source), set by the sweep body
-    unsigned mask;                 // lanes of this warp that hold a lattice site
-    int lane;
     template <int B, int BJ, int DA, int DB, int DC>
-    __device__ __forceinline__ void load(int k, double (&v)[3]) const {
-        if constexpr (spec::SHFL && BJ == B && DB == 0 && DC == 0 && DA != 0 && DA > -32 && DA < 32 && spec::BX % 32 == 0) {
-            const int src = lane + DA;
-            v[0] = __shfl_sync(mask, own[k][0], src & 31);
-            v[1] = __shfl_sync(mask, own[k][1], src & 31);
-            v[2] = __shfl_sync(mask, own[k][2], src & 31);
-            if (src < 0 || src > 31 || !((mask >> src) & 1u)) load3<lin<B, BJ, DA, DB, DC>()>(cfg[k], v);
-        } else {
-            load3<lin<B, BJ, DA, DB, DC>()>(cfg[k], v);
-        }
-    }
-    __device__ __forceinline__ void set_own(int k, const double (&o)[3]) { own[k][0] = o[0]; own[k][1] = o[1]; own[k][2] = o[2]; }
+    __device__ __forceinline__ void load(int k, double (&v)[3]) const { load3<lin<B, BJ, DA, DB, DC>()>(cfg[k], v); }
 };
 
 // SIB corrector (C11): the field is evaluated at the midpoint configuration {(n_j + n_j^p)/2}
@@ -234,19 +210,6 @@ __device__ __forceinline__ bool locate(Coord &c, int &idx) {
     return (c.ia < spec::NA) && (c.ib < spec::NB) && (c.ic < spec::NC);
 }
 
-// L2 prefetch of the lines a later wave of blocks will read: spec::PF_PLANES lattice planes ahead of the own site (0 = off).
-// One lane per 128-byte line issues it (the rows start on line boundaries); no registers are tied up.
-__device__ __forceinline__ void prefetch_ahead(const double *__restrict__ q, const Coord &c) {
-    if constexpr (spec::PF_PLANES > 0) {
-        if ((c.ia & 15) == 0 && c.ic + spec::PF_PLANES < spec::NC) {
-            const double *t = q + spec::PF_PLANES * PLANE;
-            asm volatile("prefetch.global.L2 [%0];" ::"l"(t));
-            asm volatile("prefetch.global.L2 [%0];" ::"l"(t + spec::PA));
-            asm volatile("prefetch.global.L2 [%0];" ::"l"(t + 2 * spec::PA));
-        }
-    }
-}
-
 template <int B>
 __device__ __forceinline__ void thermal_force(const Coord &c, u64 step, u32 seed_lo, u32 seed_hi, double (&f)[3]) {
     if constexpr (spec::THERMAL_ON) {
@@ -264,33 +227,20 @@ __device__ __forceinline__ void predictor_body(const double *__restrict__ n, con
                                                double *__restrict__ Aout, u64 step, u32 seed_lo, u32 seed_hi) {
     Coord c;
     int idx;
-    const bool valid = locate<B>(c, idx);
-    const unsigned mask = __ballot_sync(0xffffffffu, valid);
-    if (!valid) return;
-    prefetch_ahead(n + idx, c);
+    if (!locate<B>(c, idx)) return;
     GlobalAcc<1> cfg;
-    cfg.cfg[0] = n + idx; cfg.mask = mask; cfg.lane = (int)(threadIdx.x & 31u);
+    cfg.cfg[0] = n + idx;
     double own[1][3], F[1][3], sg[1][3] = {{0.0, 0.0, 0.0}};
     load3<0>(cfg.cfg[0], own[0]);
-    cfg.set_own(0, own[0]);
     thermal_force<B>(c, step, seed_lo, seed_hi, F[0]);
-#if !(SPIN_ABLATE & 1)
     force<B, 1>(cfg, own, F);
-#endif
     if constexpr (spec::HAS_DDI) { double d[3]; load3<0>(fddi + idx, d); F[0][0] += d[0]; F[0][1] += d[1]; F[0][2] += d[2]; }
     if constexpr (spec::STT_ON) stt_gradient<B, 1>(cfg, c, own, sg);
     double A[3], out[3];
-#if SPIN_ABLATE & 4
-    out[0] = own[0][0] + F[0][0]; out[1] = own[0][1] + F[0][1]; out[2] = own[0][2] + F[0][2];
-#else
     rotation_field<B>(own[0], F[0], sg[0], A);
     if constexpr (spec::SOLVER == 0) spin::rodrigues(A, specc::DT, specc::DT2, own[0], out);                 // B5
     else if constexpr (spec::SOLVER == 1) { out[0] = own[0][0]; out[1] = own[0][1]; out[2] = own[0][2]; spin::heun_add(own[0], A, specc::DT, out); }   // B3
     else spin::imp_update(A, specc::HDT, own[0], out);                                                        // C5
-#endif
-#if SPIN_ABLATE & 2
-    if (out[0] == 123.456)
-#endif
     store_spin(np + idx, c, out);
     if constexpr (spec::STORE_A) store3(Aout + idx, A);
 }
@@ -301,11 +251,7 @@ __device__ __forceinline__ void corrector_body(const double *__restrict__ n, con
                                                u64 step, u32 seed_lo, u32 seed_hi) {
     Coord c;
     int idx;
-    const bool valid = locate<B>(c, idx);
-    const unsigned mask = __ballot_sync(0xffffffffu, valid);
-    if (!valid) return;
-    prefetch_ahead(n + idx, c);
-    prefetch_ahead(np + idx, c);
+    if (!locate<B>(c, idx)) return;
     double th[3], A[3], Ap[3], n0[3];
     thermal_force<B>(c, step, seed_lo, seed_hi, th);
     load3<0>(n + idx, n0);
@@ -330,10 +276,9 @@ __device__ __forceinline__ void corrector_body(const double *__restrict__ n, con
     double np0[3] = {0.0, 0.0, 0.0};
     if constexpr (spec::STORE_A) {
         GlobalAcc<1> cfg;
-        cfg.cfg[0] = np + idx; cfg.mask = mask; cfg.lane = (int)(threadIdx.x & 31u);
+        cfg.cfg[0] = np + idx;
         double own[1][3], F[1][3] = {{th[0], th[1], th[2]}}, sg[1][3] = {{0.0, 0.0, 0.0}};
         load3<0>(cfg.cfg[0], own[0]);
-        cfg.set_own(0, own[0]);
         force<B, 1>(cfg, own, F);
         if constexpr (spec::HAS_DDI) { double d[3]; load3<0>(fddi_np + idx, d); F[0][0] += d[0]; F[0][1] += d[1]; F[0][2] += d[2]; }
         if constexpr (spec::STT_ON) stt_gradient<B, 1>(cfg, c, own, sg);
@@ -341,12 +286,11 @@ __device__ __forceinline__ void corrector_body(const double *__restrict__ n, con
         load3<0>(Ain + idx, A);
     } else {
         GlobalAcc<2> cfg;
-        cfg.cfg[0] = n + idx; cfg.cfg[1] = np + idx; cfg.mask = mask; cfg.lane = (int)(threadIdx.x & 31u);
+        cfg.cfg[0] = n + idx; cfg.cfg[1] = np + idx;
         double own[2][3], F[2][3] = {{th[0], th[1], th[2]}, {th[0], th[1], th[2]}}, sg[2][3] = {{0.0, 0.0, 0.0}, {0.0, 0.0, 0.0}};
         own[0][0] = n0[0]; own[0][1] = n0[1]; own[0][2] = n0[2];
         load3<0>(cfg.cfg[1], own[1]);
         np0[0] = own[1][0]; np0[1] = own[1][1]; np0[2] = own[1][2];
-        cfg.set_own(0, own[0]); cfg.set_own(1, own[1]);
         force<B, 2>(cfg, own, F);
         if constexpr (spec::HAS_DDI) {
             double d[3];

@@ -168,21 +168,12 @@ extern "C" __global__ void __launch_bounds__(spintma::Geo<spec::TmaP>::NTHREADS)
             double own[1][3], F[1][3], sg[1][3] = {{0.0, 0.0, 0.0}};
             acc.template load<B, B, 0, 0, 0>(0, own[0]);
             thermal_force<B>(c, step, seed_lo, seed_hi, F[0]);
-#if !(SPIN_ABLATE & 1)
             force<B, 1>(acc, own, F);
-#endif
             if constexpr (spec::HAS_DDI) { double d[3]; load3<0>(fddi + idx, d); F[0][0] += d[0]; F[0][1] += d[1]; F[0][2] += d[2]; }
             if constexpr (spec::STT_ON) stt_gradient<B, 1>(acc, c, own, sg);
             double A[3], out[3];
-#if SPIN_ABLATE & 4
-            out[0] = own[0][0] + F[0][0]; out[1] = own[0][1] + F[0][1]; out[2] = own[0][2] + F[0][2];
-#else
             rotation_field<B>(own[0], F[0], sg[0], A);
             spin::rodrigues(A, specc::DT, specc::DT2, own[0], out);
-#endif
-#if SPIN_ABLATE & 2
-            if (out[0] == 123.456)
-#endif
             store_spin(np + idx, c, out);
         });
     });
