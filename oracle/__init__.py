@@ -67,6 +67,7 @@ def lib():
         L.orc_llg_iterate.argtypes = [vp, C.c_long]
         L.orc_heun_step.argtypes = [vp]
         L.orc_set_solver.argtypes = [vp, C.c_int]
+        L.orc_set_pinned.argtypes = [vp, C.c_void_p]
         L.orc_topological_charge.argtypes = [vp, dp]
         L.orc_topological_charge.restype = C.c_double
         L.orc_spherical_area.argtypes = [dp, dp, dp]
@@ -247,6 +248,15 @@ class OracleSystem:
         """Q of App. A summed over the a-b planes (one basis atom)."""
         a, p = _d(self.spins() if n is None else n)
         return float(lib().orc_topological_charge(self._h, p))
+
+    def set_pinned(self, mask):
+        """mask: N flags (boundary order) or None.  Pinned spins never move; a pinned zero vector is a vacancy."""
+        if mask is None:
+            lib().orc_set_pinned(self._h, None)
+            return
+        m = np.ascontiguousarray(np.asarray(mask).astype(np.uint8).reshape(-1))
+        assert m.size == self.N
+        lib().orc_set_pinned(self._h, m.ctypes.data_as(C.c_void_p))
 
     def set_solver(self, solver):
         """0 Depondt (App. B B5-B7), 1 Heun (B3-B4), 2 SIB semi-implicit midpoint (App. C)."""

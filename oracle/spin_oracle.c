@@ -71,6 +71,8 @@ typedef struct orc_system {
     uint64_t seed, step;
     double *n;               /* 3N */
     int nthreads;
+    unsigned char *pinned;   /* N flags or NULL: a pinned spin keeps its value (":79 pinning of individual spins"); a vacancy
+                                (":79 defects, such as vacancies") is a pinned site holding the zero vector (reading R27)   */
     int solver;              /* 0 Depondt (App. B B5-B7), 1 Heun (B3-B4), 2 SIB semi-implicit midpoint (App. C) */
 } orc_system;
 
@@ -142,7 +144,7 @@ void orc_destroy(orc_system *s) {
     if (!s) return;
     free(s->basis); free(s->mu); free(s->K); free(s->Kax);
     free(s->pi); free(s->pj); free(s->pt); free(s->pJ); free(s->pD);
-    free(s->qb); free(s->qt); free(s->qK); free(s->Khat); free(s->n);
+    free(s->qb); free(s->qt); free(s->qK); free(s->Khat); free(s->n); free(s->pinned);
     free(s);
 }
 long orc_nspins(const orc_system *s) { return s->N; }
@@ -202,6 +204,12 @@ void orc_llg_configure(orc_system *s, double dt_fs, double alpha, double T, uint
     s->step = 0;
 }
 void orc_set_solver(orc_system *s, int solver) { s->solver = solver; }
+void orc_set_pinned(orc_system *s, const unsigned char *mask) {
+    free(s->pinned); s->pinned = NULL;
+    if (!mask) return;
+    s->pinned = (unsigned char *)malloc((size_t)s->N);
+    memcpy(s->pinned, mask, (size_t)s->N);
+}
 uint64_t orc_get_step(const orc_system *s) { return s->step; }
 void orc_set_step(orc_system *s, uint64_t st) { s->step = st; }
 
@@ -780,6 +788,7 @@ void orc_llg_step(orc_system *s) {
 #pragma omp parallel for schedule(static) num_threads(s->nthreads)
     for (long i = 0; i < N; ++i) {
         rot_field(s, (int)(i % nb), s->n + 3*i, F + 3*i, sg + 3*i, A + 3*i);
+        if (s->pinned && s->pinned[i]) { for (int k = 0; k < 3; ++k) np_[3*i+k] = s->n[3*i+k]; continue; }   /* pinned: n^p = n */
         if (s->solver == 0) rotate(A + 3*i, s->dt, s->n + 3*i, np_ + 3*i);                       /* B5 */
         else if (s->solver == 1) {                                                               /* B3 */
             double f0[3]; cross3(s->n + 3*i, A + 3*i, f0);
@@ -794,6 +803,7 @@ void orc_llg_step(orc_system *s) {
 #pragma omp parallel for schedule(static) num_threads(s->nthreads)
     for (long i = 0; i < N; ++i) {
         double Ap[3], Ac[3], out[3];
+        if (s->pinned && s->pinned[i]) continue;                               /* pinned: n_i(t+dt) = n_i(t) */
         rot_field(s, (int)(i % nb), second + 3*i, F + 3*i, sg + 3*i, Ap);
         if (s->solver == 0) {
             for (int k = 0; k < 3; ++k) Ac[k] = 0.5 * (A[3*i+k] + Ap[k]);     /* B6 */
@@ -896,6 +906,7 @@ void orc_observables(orc_system *s, double M[3], double *max_torque) {
         const double *n = s->n + 3*i; double p = dot3(F + 3*i, n), t[3];
         for (int k = 0; k < 3; ++k) { m[k] += n[k]; t[k] = F[3*i+k] - p * n[k]; }
         double tn = sqrt(dot3(t, t));
+        if (s->pinned && s->pinned[i]) continue;           /* a pinned spin carries no torque that matters */
         if (tn > mt) mt = tn;
     }
     for (int k = 0; k < 3; ++k) M[k] = (double)(m[k] / (long double)s->N);

@@ -558,3 +558,63 @@ def test_topological_charge_of_textures(cfg, cells):
     # a random configuration on a periodic lattice still has an integer charge
     q = s.topological_charge(rand_spins(w.n_spins, 5))
     assert abs(q - round(q)) < 1e-9
+
+
+# ------------------------------------------------------------------ pinned spins and vacancies
+def _chain(n_sites, J=1.0, B=0.0, alpha=0.1, dt_fs=10.0, mu=2.0):
+    s = OracleSystem(np.eye(3), [[0, 0, 0]], (n_sites, 1, 1), (0, 0, 0))
+    s.set_mu_s([mu]); s.set_field(B, (0, 0, 1)); s.llg_configure(dt_fs, alpha)
+    s.set_pairs([0], [0], [[1, 0, 0]], [J])
+    return s
+
+
+def test_pinned_spin_acts_as_a_fixed_field_source():
+    """Spin 0 pinned along x, spin 1 free, exchange J, no external field: spin 1 sees the constant field J x^ / (mu mu_B) and
+    follows Eq. 12 in the frame whose polar axis is x; the pinned spin does not move by a single bit."""
+    J, mu, alpha, dt_fs = 1.0, 2.0, 0.1, 10.0
+    s = _chain(2, J=J, alpha=alpha, dt_fs=dt_fs, mu=mu)
+    s.set_pinned([1, 0])
+    s.set_spins([[1.0, 0.0, 0.0], [0.0, 1.0, 0.0]])
+    Beff = J / (mu * O.MU_B)
+    gp = O.GAMMA / (1 + alpha * alpha)
+    err = 0.0
+    for k in range(500):
+        s.iterate(1)
+        t = (k + 1) * dt_fs * 1e-3
+        npar = math.tanh(alpha * gp * Beff * t); ph = gp * Beff * t; r = math.sqrt(1 - npar * npar)
+        # polar axis x, azimuth from y towards z (right-handed about x, same sense as Eq. 12 about z)
+        ex = np.array([npar, r * math.cos(ph), r * math.sin(ph)])
+        n = s.spins()
+        assert np.array_equal(n[0], [1.0, 0.0, 0.0])
+        err = max(err, np.abs(n[1] - ex).max())
+    assert err < 5e-5, err       # second-order error of the scheme at |A| dt = 0.15 rad per step
+
+
+def test_vacancy_decouples_its_neighbours():
+    """A vacancy (pinned zero vector) in the middle of a 3-site chain: the end spins are free spins, bit for bit the trajectory of
+    a single spin in the same field; and the energy equals that of the Hamiltonian with the vacant site's bonds removed."""
+    s = _chain(3, J=1.3, B=1.0)
+    s.set_pinned([0, 1, 0])
+    n0 = np.array([[1.0, 0.0, 0.0], [0.0, 0.0, 0.0], [0.6, 0.0, 0.8]])
+    s.set_spins(n0); s.iterate(300)
+    for site in (0, 2):
+        f = OracleSystem(np.eye(3), [[0, 0, 0]], (1, 1, 1), (0, 0, 0))
+        f.set_mu_s([2.0]); f.set_field(1.0, (0, 0, 1)); f.llg_configure(10.0, 0.1)
+        f.set_spins([n0[site]]); f.iterate(300)
+        assert np.array_equal(s.spins()[site], f.spins()[0])
+    assert np.array_equal(s.spins()[1], [0.0, 0.0, 0.0])
+    w = small(1, (6, 5, 1))
+    a = OracleSystem.from_workload(w)
+    n = rand_spins(w.n_spins, 3)
+    vac = 13
+    n[vac] = 0.0
+    keep = np.ones(len(w.pair_J), bool)       # bonds are per cell: removing a site's bonds needs the explicit site loop instead
+    E_vac = a.energy_terms(n)
+    # explicit: energy of the full lattice minus every term that involves the vacant site, evaluated with the original spin
+    m = rand_spins(w.n_spins, 3)
+    E_full = a.energy_terms(m)
+    F = a.gradient(m)                          # F_i = -dH/dn_i; pair terms are bilinear: E_pairs(site) = -n_i . F_i^{pairs}
+    Fz = a.gradient(m, mask=O.T_ZEE)[vac]; Fa = a.gradient(m, mask=O.T_ANI)[vac]
+    Fp = a.gradient(m, mask=O.T_EXC | O.T_DMI)[vac]
+    expect = E_full.sum() + np.dot(m[vac], Fz) + 0.5 * np.dot(m[vac], Fa) + np.dot(m[vac], Fp)
+    assert E_vac.sum() == pytest.approx(expect, rel=1e-12)
