@@ -100,6 +100,13 @@ int spins_get(spin_system *sys, double *n_xyz /*host, 3N AoS*/);
 int spins_set_device(spin_system *sys, const double *n_xyz /*device, 3N AoS*/);
 int spins_get_device(spin_system *sys, double *n_xyz /*device, 3N AoS*/);
 
+/* Pinning and vacancies (:79 "pinning of individual spins or a set of spins", "defects, such as vacancies").  mask: N flags in
+ * boundary index order, non-zero = pinned; NULL removes all pins.  A pinned spin is never updated by llg_iterate but acts on its
+ * neighbours as usual.  A vacancy is a pinned site holding the zero vector: spins_set accepts a zero vector on pinned sites only;
+ * such a site contributes nothing to any field or energy.  Pinned sites are excluded from the max-torque observable.
+ * Call before spins_set if the configuration contains vacancies.                                                              */
+int spins_set_pinned(spin_system *sys, const unsigned char *mask /*host, N*/);
+
 /* ---- dynamics: Eq. 10 with the thermal field of Eq. 11 (:157-160), Depondt solver (App. B) --------------
  * dt in fs; alpha Gilbert damping; T in Kelvin (0 = no noise); seed of the counter-based Philox4x32-10
  * generator keyed by (seed; step, spin, block); u in Angstrom/ps along the unit vector j_dir; beta the

@@ -19,7 +19,7 @@ EXPORTS = [
     "spin_geometry_create", "spin_system_destroy", "spin_system_nspins", "spin_set_stream",
     "hamiltonian_set_mu_s", "hamiltonian_set_field", "hamiltonian_set_anisotropy", "hamiltonian_set_pairs",
     "hamiltonian_set_exchange_shells", "hamiltonian_set_dmi_shells", "hamiltonian_set_quadruplets",
-    "hamiltonian_set_ddi", "spins_set", "spins_get", "spins_set_device", "spins_get_device",
+    "hamiltonian_set_ddi", "spins_set_pinned", "spins_set", "spins_get", "spins_set_device", "spins_get_device",
     "llg_configure", "llg_set_solver", "llg_iterate", "llg_get_step", "llg_set_step", "spin_synchronize",
     "effective_field", "effective_field_device", "energy", "observables", "topological_charge",
     "spin_launch_counts", "spin_profile_enable", "spin_profile_get", "spin_set_option",
@@ -63,6 +63,7 @@ def lib() -> C.CDLL:
         "spins_get_device": (C.c_int, [vp, vp]),
         "llg_configure": (C.c_int, [vp, C.c_double, C.c_double, C.c_double, C.c_uint64, C.c_double, dp, C.c_double]),
         "llg_set_solver": (C.c_int, [vp, C.c_int]),
+        "spins_set_pinned": (C.c_int, [vp, C.c_void_p]),
         "llg_iterate": (C.c_int, [vp, C.c_int64]),
         "llg_get_step": (C.c_int, [vp, C.POINTER(C.c_uint64)]),
         "llg_set_step": (C.c_int, [vp, C.c_uint64]),
@@ -217,6 +218,16 @@ class SpinSystem:
     def llg_configure(self, dt_fs, alpha, T=0.0, seed=0, u=0.0, j_dir=(1, 0, 0), beta=0.0):
         j, jp = _d(j_dir)
         _check(lib().llg_configure(self._h, float(dt_fs), float(alpha), float(T), int(seed), float(u), jp, float(beta)))
+
+    def spins_set_pinned(self, mask):
+        """mask: N flags (boundary order) or None.  Pinned spins never move; a pinned zero vector is a vacancy."""
+        if mask is None:
+            _check(lib().spins_set_pinned(self._h, None))
+            return
+        m = np.ascontiguousarray(np.asarray(mask).astype(np.uint8).reshape(-1))
+        if m.size != self.N:
+            raise ValueError("mask must have N entries")
+        _check(lib().spins_set_pinned(self._h, m.ctypes.data_as(C.c_void_p)))
 
     def topological_charge(self):
         q = C.c_double(0.0)

@@ -178,6 +178,7 @@ int build_plan(const spin_system *s, DevicePlan &P) {
     P.thermal_on = (s->T > 0.0) ? 1 : 0;
     P.seed_lo = (uint32_t)s->seed; P.seed_hi = (uint32_t)(s->seed >> 32);
     P.has_ddi = s->ddi_on ? 1 : 0;
+    P.pin = s->d_pin;
     P.stt_on = (s->u != 0.0) ? 1 : 0;
     if (P.stt_on) {
         if (stt_coefficients(s, P.stt_c) != 0) return spin::fail(SPIN_ERR_ARG, "current direction: singular lattice metric");
@@ -465,7 +466,7 @@ extern "C" int spin_geometry_create(const double bravais[9], int n_basis, const 
     s->seed = 0; s->step = 0; s->solver = SPIN_SOLVER_DEPONDT;
     s->stream = nullptr; s->own_stream = nullptr; s->cur = 0;
     s->d_n[0] = s->d_n[1] = s->d_np = s->d_A = s->d_fddi[0] = s->d_fddi[1] = s->d_aos = s->d_partials = s->d_result = nullptr;
-    s->d_step = nullptr; s->ddi = nullptr; s->plan_dirty = true;
+    s->d_step = nullptr; s->d_pin = nullptr; s->ddi = nullptr; s->plan_dirty = true;
     s->opt_graph = 1; s->opt_store_A = 0; s->graph_exec[0] = s->graph_exec[1] = nullptr; s->graph_steps = 0;
     s->n_launch = s->n_fft = 0; s->profile_on = 0;
     for (int k = 0; k < 3; ++k) { s->prof_ms[k] = 0; s->prof_n[k] = 0; }
@@ -508,6 +509,7 @@ extern "C" void spin_system_destroy(spin_system *s) {
     ddi_release(s);
     jit_release(s);
     cudaFree(s->d_n[0]); cudaFree(s->d_n[1]); cudaFree(s->d_np); cudaFree(s->d_A); cudaFree(s->d_fddi[0]); cudaFree(s->d_fddi[1]);
+    cudaFree(s->d_pin);
     cudaFree(s->d_aos); cudaFree(s->d_partials); cudaFree(s->d_result); cudaFree(s->d_step);
     if (s->ev0) cudaEventDestroy(s->ev0);
     if (s->ev1) cudaEventDestroy(s->ev1);
@@ -659,6 +661,25 @@ static int pack_from_device_aos(spin_system *s, const double *d_aos) {
     SPIN_CUDA(cudaStreamSynchronize(s->stream));
     SPIN_CUDA(cudaGetLastError());
     if (h_bad) return spin::fail(SPIN_ERR_ARG, "spins_set: zero or non-finite spin vector");
+    return SPIN_OK;
+}
+// pinned spins: flags in boundary order; null clears.  A pinned site may hold the zero vector (a vacancy).
+extern "C" int spins_set_pinned(spin_system *s, const unsigned char *mask) {
+    REQUIRE(s, "null system");
+    NEED_DEVICE(s);
+    SPIN_CUDA(cudaStreamSynchronize(s->stream));
+    if (!mask) {
+        if (s->d_pin) { cudaFree(s->d_pin); s->d_pin = nullptr; }
+    } else {
+        if (!s->d_pin) {
+            cudaError_t e = cudaMalloc(&s->d_pin, (size_t)s->N);
+            if (e != cudaSuccess) { s->d_pin = nullptr; return spin::fail(SPIN_ERR_MEMORY, "device allocation of %lld bytes failed", (long long)s->N); }
+        }
+        SPIN_CUDA(cudaMemcpy(s->d_pin, mask, (size_t)s->N, cudaMemcpyHostToDevice));
+    }
+    s->plan.pin = s->d_pin;       // pack_kernel reads it before the next plan build
+    s->plan_dirty = true;
+    drop_graphs(s);
     return SPIN_OK;
 }
 extern "C" int spins_set(spin_system *s, const double *n) {

@@ -157,7 +157,7 @@ static void jit_brick_launch(const spin_system *s, dim3 &grid, dim3 &block) {
 // SPINLLG_COL="cbx,cby,ccz" overrides the defaults (32 x 4 columns, 16 planes per chunk).
 static bool plan_col(const spin_system *s, int g[4]) {
     const DevicePlan &P = s->plan;
-    if (!s->opt_col || s->opt_store_A || s->solver != 0 || P.rC < 1 || P.Nc < 2) return false;
+    if (!s->opt_col || s->opt_store_A || s->solver != 0 || s->d_pin || P.rC < 1 || P.Nc < 2) return false;
     int cbx = 32, cby = 4, ccz = 16;
     if (const char *e = getenv("SPINLLG_COL")) {
         int v[3] = {0, 0, 0};
@@ -176,6 +176,7 @@ static bool plan_col(const spin_system *s, int g[4]) {
 static bool plan_tma(const spin_system *s, TmaGeo &gp, TmaGeo &gc, std::string &why) {
     if (!s->opt_tma) { why = "disabled by option use_tma=0"; return false; }
     if (s->solver != 0) { why = "Depondt solver only"; return false; }
+    if (s->d_pin) { why = "pinned spins use the brick kernels"; return false; }
     if (s->opt_store_A) { why = "store_A=1 uses the brick kernels"; return false; }
     if (s->opt_tma < 2 && s->N < 16384) { why = "lattice too small to fill persistent CTAs"; return false; }
     return plan_tma_geo(s, 1, "SPINLLG_TMA_P", gp, why) && plan_tma_geo(s, 2, "SPINLLG_TMA_C", gc, why);
@@ -197,6 +198,7 @@ std::string spin::jit_source(const spin_system *s) {
     o << "constexpr int BX = " << brick[0] << ", BY = " << brick[1] << ", BZ = " << brick[2] << ";\n";
     o << "constexpr bool PER_A = " << (P.perA ? "true" : "false") << ", PER_B = " << (P.perB ? "true" : "false")
       << ", PER_C = " << (P.perC ? "true" : "false") << ";\n";
+    o << "constexpr bool HAS_PIN = " << (s->d_pin ? "true" : "false") << ";\n";
     o << "constexpr int SOLVER = " << s->solver << ";      // 0 Depondt, 1 Heun, 2 SIB\n";
     o << "constexpr bool STORE_A = " << ((s->opt_store_A && s->solver == 0) ? "true" : "false") << ", HAS_DDI = " << (P.has_ddi ? "true" : "false")
       << ", THERMAL_ON = " << (P.thermal_on ? "true" : "false") << ", STT_ON = " << (P.stt_on ? "true" : "false") << ";\n";
@@ -400,7 +402,9 @@ int spin::jit_launch_predictor(spin_system *s, dim3 grid, dim3 block, const doub
                                unsigned step_add) {
     unsigned seed_lo = s->plan.seed_lo, seed_hi = s->plan.seed_hi;
     const unsigned long long *d_step = s->d_step;
-    void *args[] = {(void *)&n, (void *)&fddi, (void *)&np, (void *)&Aout, (void *)&d_step, (void *)&step_add, (void *)&seed_lo, (void *)&seed_hi};
+    const unsigned char *pin = s->d_pin;
+    void *args[] = {(void *)&n, (void *)&fddi, (void *)&np, (void *)&Aout, (void *)&d_step, (void *)&step_add, (void *)&seed_lo, (void *)&seed_hi,
+                    (void *)&pin};
     jit_brick_launch(s, grid, block);
     SPIN_CUDA(cudaLaunchKernel((const void *)s->jit->k_pred, grid, block, args, 0, s->stream));
     return SPIN_OK;
@@ -409,9 +413,10 @@ int spin::jit_launch_predictor(spin_system *s, dim3 grid, dim3 block, const doub
 int spin::jit_launch_corrector(spin_system *s, dim3 grid, dim3 block, const double *n, const double *np, const double *fddi_n,
                                const double *fddi_np, const double *Ain, double *nout, unsigned step_add) {
     unsigned seed_lo = s->plan.seed_lo, seed_hi = s->plan.seed_hi;
+    const unsigned char *pin = s->d_pin;
     const unsigned long long *d_step = s->d_step;
     void *args[] = {(void *)&n, (void *)&np, (void *)&fddi_n, (void *)&fddi_np, (void *)&Ain, (void *)&nout, (void *)&d_step, (void *)&step_add,
-                    (void *)&seed_lo, (void *)&seed_hi};
+                    (void *)&seed_lo, (void *)&seed_hi, (void *)&pin};
     jit_brick_launch(s, grid, block);
     SPIN_CUDA(cudaLaunchKernel((const void *)s->jit->k_corr, grid, block, args, 0, s->stream));
     return SPIN_OK;

@@ -222,9 +222,16 @@ __device__ __forceinline__ void thermal_force(const Coord &c, u64 step, u32 seed
     }
 }
 
+// pinned spins: flags in boundary order b + NBASIS * cell; a pinned spin is copied, never updated
+template <int B>
+__device__ __forceinline__ bool is_pinned(const unsigned char *__restrict__ pin, const Coord &c) {
+    if constexpr (spec::HAS_PIN) return pin[B + spec::NBASIS * (c.ia + spec::NA * (c.ib + spec::NB * c.ic))] != 0;
+    else return false;
+}
+
 template <int B>
 __device__ __forceinline__ void predictor_body(const double *__restrict__ n, const double *__restrict__ fddi, double *__restrict__ np,
-                                               double *__restrict__ Aout, u64 step, u32 seed_lo, u32 seed_hi) {
+                                               double *__restrict__ Aout, u64 step, u32 seed_lo, u32 seed_hi, const unsigned char *__restrict__ pin) {
     Coord c;
     int idx;
     if (!locate<B>(c, idx)) return;
@@ -232,6 +239,7 @@ __device__ __forceinline__ void predictor_body(const double *__restrict__ n, con
     cfg.cfg[0] = n + idx;
     double own[1][3], F[1][3], sg[1][3] = {{0.0, 0.0, 0.0}};
     load3<0>(cfg.cfg[0], own[0]);
+    if (is_pinned<B>(pin, c)) { store_spin(np + idx, c, own[0]); return; }
     thermal_force<B>(c, step, seed_lo, seed_hi, F[0]);
     force<B, 1>(cfg, own, F);
     if constexpr (spec::HAS_DDI) { double d[3]; load3<0>(fddi + idx, d); F[0][0] += d[0]; F[0][1] += d[1]; F[0][2] += d[2]; }
@@ -248,13 +256,14 @@ __device__ __forceinline__ void predictor_body(const double *__restrict__ n, con
 template <int B>
 __device__ __forceinline__ void corrector_body(const double *__restrict__ n, const double *__restrict__ np, const double *__restrict__ fddi_n,
                                                const double *__restrict__ fddi_np, const double *__restrict__ Ain, double *__restrict__ nout,
-                                               u64 step, u32 seed_lo, u32 seed_hi) {
+                                               u64 step, u32 seed_lo, u32 seed_hi, const unsigned char *__restrict__ pin) {
     Coord c;
     int idx;
     if (!locate<B>(c, idx)) return;
     double th[3], A[3], Ap[3], n0[3];
-    thermal_force<B>(c, step, seed_lo, seed_hi, th);
     load3<0>(n + idx, n0);
+    if (is_pinned<B>(pin, c)) { store_spin(nout + idx, c, n0); return; }
+    thermal_force<B>(c, step, seed_lo, seed_hi, th);
     if constexpr (spec::SOLVER == 2) {
         // SIB corrector (C11): A at the midpoint configuration, the implicit-midpoint structure applied to n(t); A(n) is not needed
         const MidAcc cfg = {n + idx, np + idx};
@@ -329,20 +338,22 @@ __device__ __forceinline__ void dispatch_basis(int b, Fn &&fn) {
 
 extern "C" __global__ void SPIN_BOUNDS(spec::BX *spec::BY *spec::BZ)
     jit_predictor(const double *__restrict__ n, const double *__restrict__ fddi, double *__restrict__ np, double *__restrict__ Aout,
-                  const unsigned long long *__restrict__ d_step, unsigned int step_add, unsigned int seed_lo, unsigned int seed_hi) {
+                  const unsigned long long *__restrict__ d_step, unsigned int step_add, unsigned int seed_lo, unsigned int seed_hi,
+                  const unsigned char *__restrict__ pin) {
     const unsigned long long step = *d_step + step_add;
     spinjit::dispatch_basis<0>((int)blockIdx.y, [&](auto b) {
-        spinjit::predictor_body<decltype(b)::value>(n, fddi, np, Aout, step, seed_lo, seed_hi);
+        spinjit::predictor_body<decltype(b)::value>(n, fddi, np, Aout, step, seed_lo, seed_hi, pin);
     });
 }
 
 extern "C" __global__ void SPIN_BOUNDS(spec::BX *spec::BY *spec::BZ)
     jit_corrector(const double *__restrict__ n, const double *__restrict__ np, const double *__restrict__ fddi_n,
                   const double *__restrict__ fddi_np, const double *__restrict__ Ain, double *__restrict__ nout,
-                  const unsigned long long *__restrict__ d_step, unsigned int step_add, unsigned int seed_lo, unsigned int seed_hi) {
+                  const unsigned long long *__restrict__ d_step, unsigned int step_add, unsigned int seed_lo, unsigned int seed_hi,
+                  const unsigned char *__restrict__ pin) {
     const unsigned long long step = *d_step + step_add;
     spinjit::dispatch_basis<0>((int)blockIdx.y, [&](auto b) {
-        spinjit::corrector_body<decltype(b)::value>(n, np, fddi_n, fddi_np, Ain, nout, step, seed_lo, seed_hi);
+        spinjit::corrector_body<decltype(b)::value>(n, np, fddi_n, fddi_np, Ain, nout, step, seed_lo, seed_hi, pin);
     });
 }
 

@@ -168,6 +168,10 @@ __device__ __forceinline__ void thermal_force(const DevicePlan &P, const Site &s
     }
 }
 
+__device__ __forceinline__ bool pinned(const DevicePlan &P, const Site &s) {
+    return P.pin != nullptr && P.pin[s.b + P.nb * (s.ia + P.Na * (s.ib + P.Nb * s.ic))] != 0;
+}
+
 // ---------------------------------------------------------------------------------------------------------
 // Sweep 1 (B5): n -> n^p.  Reads n (own + gathered neighbours), optional dipolar force of n; writes n^p and,
 // with STORE_A, the rotation field A.
@@ -181,6 +185,7 @@ __global__ void __launch_bounds__(BX *BY *BZ)
     const double *const cfg[1] = {n};
     double own[1][3], F[1][3], sg[1][3] = {{0.0, 0.0, 0.0}};
     load3(P, n, s.idx, own[0]);
+    if (pinned(P, s)) { store_spin(P, np, s.ia, s.ib, s.ic, s.idx, own[0]); return; }      // pinned: n^p = n
     thermal_force(P, s, *d_step + step_add, F[0]);
     short_range_force<1>(P, cfg, s, own, T_ALL, F);
     if (P.has_ddi) { double d[3]; load3(P, fddi, s.idx, d); F[0][0] += d[0]; F[0][1] += d[1]; F[0][2] += d[2]; }
@@ -202,8 +207,9 @@ __global__ void __launch_bounds__(BX *BY *BZ)
     const Site s = locate<BX, BY, BZ>(P);
     if (!s.valid) return;
     double th[3], A[3], Ap[3], n0[3];
-    thermal_force(P, s, *d_step + step_add, th);
     load3(P, n, s.idx, n0);
+    if (pinned(P, s)) { store_spin(P, nout, s.ia, s.ib, s.ic, s.idx, n0); return; }        // pinned: n(t+dt) = n(t)
+    thermal_force(P, s, *d_step + step_add, th);
     if (STORE_A) {
         const double *const cfg[1] = {np};
         double own[1][3], F[1][3] = {{th[0], th[1], th[2]}}, sg[1][3] = {{0.0, 0.0, 0.0}};
@@ -250,7 +256,8 @@ __global__ void pack_kernel(const __grid_constant__ DevicePlan P, const double *
     double v[3] = {aos[3 * (size_t)i], aos[3 * (size_t)i + 1], aos[3 * (size_t)i + 2]};
     if (normalise) {
         const double r2 = v[0] * v[0] + v[1] * v[1] + v[2] * v[2];
-        if (!(r2 > 0.0) || !isfinite(r2)) { atomicExch(bad, 1); v[0] = 0; v[1] = 0; v[2] = 1; }
+        if (r2 == 0.0 && P.pin != nullptr && P.pin[i] != 0) { /* a vacancy: pinned zero vector, kept as it is */ }
+        else if (!(r2 > 0.0) || !isfinite(r2)) { atomicExch(bad, 1); v[0] = 0; v[1] = 0; v[2] = 1; }
         else { const double r = sqrt(r2); v[0] /= r; v[1] /= r; v[2] /= r; }
     }
     int b, ia, ib, ic, idx;
@@ -334,7 +341,7 @@ __global__ void __launch_bounds__(BX *BY *BZ)
         v[6] = own[0][0]; v[7] = own[0][1]; v[8] = own[0][2];
         const double p = Ft[0] * own[0][0] + Ft[1] * own[0][1] + Ft[2] * own[0][2];
         const double tx = Ft[0] - p * own[0][0], ty = Ft[1] - p * own[0][1], tz = Ft[2] - p * own[0][2];
-        v[9] = sqrt(tx * tx + ty * ty + tz * tz);
+        v[9] = pinned(P, s) ? 0.0 : sqrt(tx * tx + ty * ty + tz * tz);      // a pinned spin carries no torque that matters
     }
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
 #pragma unroll

@@ -81,6 +81,7 @@ struct DevicePlan {
     uint32_t seed_lo, seed_hi;
     int thermal_on;
     int pad_;
+    const unsigned char *pin;                // N flags in boundary order (b + nb*cell) or null: pinned spins are never updated
     PairEntry pairs[SPIN_MAX_PAIR_ENTRIES];
     QuadEntry quads[SPIN_MAX_QUAD_ENTRIES];
 };
@@ -123,6 +124,7 @@ struct spin_system {
     double *d_partials;            // reduction scratch
     double *d_result;              // reduction result (16 doubles)
     unsigned long long *d_step;    // device copy of the step counter (read by the kernels)
+    unsigned char *d_pin;          // pinned-spin flags (boundary order), null if none
     spin::DevicePlan plan;
     bool plan_dirty;
     DdiState *ddi;

@@ -416,3 +416,42 @@ def test_topological_charge_parity(P, O, cfg, cells, per):
     two = P.SpinSystem.from_workload(W.config4().resized((8, 8, 1), 1))
     with pytest.raises(P.SpinError):
         two.topological_charge()
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# Pinned spins and vacancies
+@pytest.mark.parametrize("use_jit", [1, 0])
+@pytest.mark.parametrize("cfg,steps", [(1, 200), (2, 100), (3, 100), (4, 100), (5, 20)])
+def test_pinned_spins_and_vacancies(P, O, cfg, steps, use_jit):
+    w = W.CONFIGS[cfg]().resized(REPLICAS[cfg], steps)
+    rng = np.random.default_rng(100 + cfg)
+    mask = (rng.random(w.n_spins) < 0.15).astype(np.uint8)
+    vac = (rng.random(w.n_spins) < 0.3) & (mask == 1)          # about a third of the pinned sites are vacancies
+    n0 = w.initial_spins().copy()
+    n0[vac] = 0.0
+    g = P.SpinSystem.from_workload(w, set_spins=False)
+    o = O.OracleSystem.from_workload(w)
+    g.spin_set_option("use_jit", use_jit)
+    g.spins_set_pinned(mask); o.set_pinned(mask)
+    g.spins_set(n0); o.set_spins(n0)
+    assert_fields_close(g.effective_field(), o.effective_field())
+    To = o.energy_terms()
+    assert np.abs(g.energy()[1] - To).max() <= ENERGY_RTOL * np.abs(To).sum()
+    assert abs(g.observables()[1] - o.observables()[1]) <= 1e-12 * o.observables()[1]
+    start = g.spins_get()                                        # spins_set normalises: the reference for "unchanged" is what it stored
+    assert np.array_equal(start[vac], np.zeros((int(vac.sum()), 3)))
+    g.llg_iterate(steps); o.iterate(steps)
+    ng = g.spins_get()
+    assert np.array_equal(ng[mask == 1], start[mask == 1])       # pinned spins and vacancies do not move by a bit
+    assert np.abs(ng - o.spins()).max() <= SPIN_ATOL
+    assert np.abs(ng[mask == 0] - n0[mask == 0]).max() > 1e-3     # the others do
+    if use_jit:
+        for solver in (1, 2):
+            g.spins_set(n0); o.set_spins(n0)
+            g.llg_set_solver(solver); o.set_solver(solver)
+            g.llg_iterate(30); o.iterate(30)
+            assert np.abs(g.spins_get() - o.spins()).max() <= SPIN_ATOL
+    # a zero vector on an unpinned site is still an error; clearing the mask restores normal behaviour
+    g.spins_set_pinned(None)
+    with pytest.raises(P.SpinError):
+        g.spins_set(n0)
