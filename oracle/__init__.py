@@ -68,6 +68,8 @@ def lib():
         L.orc_heun_step.argtypes = [vp]
         L.orc_set_solver.argtypes = [vp, C.c_int]
         L.orc_set_pinned.argtypes = [vp, C.c_void_p]
+        L.orc_vp_iterate.argtypes = [vp, C.c_long, C.c_double, C.c_double]
+        L.orc_vp_reset.argtypes = [vp]
         L.orc_topological_charge.argtypes = [vp, dp]
         L.orc_topological_charge.restype = C.c_double
         L.orc_spherical_area.argtypes = [dp, dp, dp]
@@ -248,6 +250,13 @@ class OracleSystem:
         """Q of App. A summed over the a-b planes (one basis atom)."""
         a, p = _d(self.spins() if n is None else n)
         return float(lib().orc_topological_charge(self._h, p))
+
+    def vp_iterate(self, n_iter, dt, mass=1.0):
+        """Velocity-projection minimiser, App. D; velocity and previous force persist between calls (vp_reset clears them)."""
+        lib().orc_vp_iterate(self._h, int(n_iter), float(dt), float(mass))
+
+    def vp_reset(self):
+        lib().orc_vp_reset(self._h)
 
     def set_pinned(self, mask):
         """mask: N flags (boundary order) or None.  Pinned spins never move; a pinned zero vector is a vacancy."""

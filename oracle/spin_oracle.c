@@ -15,6 +15,7 @@
  *   thermal field     Eq. 11 (:157-160)                     -> orc_thermal_xi, sigma
  *   Depondt solver    App. B, B5-B7 (:369-380)              -> orc_llg_step (solver 0)
  *   Heun solver       App. B, B3-B4 (:355-367)              -> orc_llg_step (solver 1); orc_heun_step = the same written on its own (pin)
+ *   velocity projection App. D, D1-D5 (:438-463)            -> orc_vp_iterate
  *   topological charge App. A, A1-A2 (:317-343)             -> orc_topological_charge, orc_spherical_area
  *   SIB solver        App. C, C5-C11 (:384-436)             -> orc_llg_step (solver 2), imp_update (Cramer's rule as printed)
  * Readings of silent / garbled passages are listed in DESIGN.md ("Readings") under the
@@ -73,6 +74,7 @@ typedef struct orc_system {
     int nthreads;
     unsigned char *pinned;   /* N flags or NULL: a pinned spin keeps its value (":79 pinning of individual spins"); a vacancy
                                 (":79 defects, such as vacancies") is a pinned site holding the zero vector (reading R27)   */
+    double *vp_v, *vp_F;     /* velocity-projection minimiser (App. D): velocity and force of the previous iteration, or NULL  */
     int solver;              /* 0 Depondt (App. B B5-B7), 1 Heun (B3-B4), 2 SIB semi-implicit midpoint (App. C) */
 } orc_system;
 
@@ -144,7 +146,7 @@ void orc_destroy(orc_system *s) {
     if (!s) return;
     free(s->basis); free(s->mu); free(s->K); free(s->Kax);
     free(s->pi); free(s->pj); free(s->pt); free(s->pJ); free(s->pD);
-    free(s->qb); free(s->qt); free(s->qK); free(s->Khat); free(s->n); free(s->pinned);
+    free(s->qb); free(s->qt); free(s->qK); free(s->Khat); free(s->n); free(s->pinned); free(s->vp_v); free(s->vp_F);
     free(s);
 }
 long orc_nspins(const orc_system *s) { return s->N; }
@@ -846,6 +848,49 @@ void orc_heun_step(orc_system *s) {
     }
     s->step += 1;
     free(F); free(f0); free(np_); free(sg);
+}
+
+/* ------------------------------------------------------------------ velocity-projection minimiser, App. D (:438-463)
+ * "Pretend that the spins are massive particles moving on the surfaces of spheres", force F_i = -dH/dn_i (D4).  One iteration,
+ * in the order the appendix lists the equations (reading R28: the paper does not say where in the step the force is evaluated):
+ *     F(t+dt) = F(x(t))                                  force of the current configuration            (D4)
+ *     v <- v + dt/(2m) (F(t) + F(t+dt))                  velocity increment                             (D2)
+ *     v <- (v.F) F/|F|^2 if v.F > 0 else 0               projection, dot products over all 3N components (D3)
+ *     x <- x + dt v + dt^2/(2m) F                        position increment                             (D1)
+ *     x_i <- x_i/|x_i|                                   renormalisation                                (D5)
+ * The first iteration starts from v = 0 and F(t) = F(t+dt).  Pinned spins do not move and carry no force.            */
+void orc_vp_reset(orc_system *s) { free(s->vp_v); free(s->vp_F); s->vp_v = NULL; s->vp_F = NULL; }
+void orc_vp_iterate(orc_system *s, long n_iter, double dt, double mass) {
+    long N = s->N;
+    double *F = (double *)malloc(3 * N * sizeof(double));
+    for (long it = 0; it < n_iter; ++it) {
+        orc_gradient(s, s->n, F, T_ALL);
+        if (s->pinned) for (long i = 0; i < N; ++i) if (s->pinned[i]) { F[3*i] = 0; F[3*i+1] = 0; F[3*i+2] = 0; }
+        if (!s->vp_v) {
+            s->vp_v = (double *)calloc(3 * N, sizeof(double));
+            s->vp_F = (double *)malloc(3 * N * sizeof(double));
+            memcpy(s->vp_F, F, 3 * N * sizeof(double));
+        }
+        long double vF = 0.0L, FF = 0.0L;
+        for (long i = 0; i < 3 * N; ++i) {
+            s->vp_v[i] += 0.5 * dt / mass * (s->vp_F[i] + F[i]);                          /* D2 */
+            vF += (long double)s->vp_v[i] * F[i];
+            FF += (long double)F[i] * F[i];
+        }
+        double ratio = (vF > 0.0L && FF > 0.0L) ? (double)(vF / FF) : 0.0;                /* D3 */
+        for (long i = 0; i < N; ++i) {
+            if (s->pinned && s->pinned[i]) { for (int k = 0; k < 3; ++k) s->vp_v[3*i+k] = 0.0; continue; }
+            double x[3];
+            for (int k = 0; k < 3; ++k) {
+                s->vp_v[3*i+k] = ratio * F[3*i+k];
+                x[k] = s->n[3*i+k] + dt * s->vp_v[3*i+k] + 0.5 * dt * dt / mass * F[3*i+k];   /* D1 */
+            }
+            double nrm = sqrt(dot3(x, x));
+            for (int k = 0; k < 3; ++k) s->n[3*i+k] = x[k] / nrm;                          /* D5 */
+        }
+        memcpy(s->vp_F, F, 3 * N * sizeof(double));
+    }
+    free(F);
 }
 
 /* ------------------------------------------------------------------ topological charge, App. A (:317-343)

@@ -3,6 +3,7 @@
 None of these tests touches the CUDA path.  Each pin is chosen so that a plausible mistake in the oracle
 (dropped term, wrong sign or index, transposed operand, wrong unit) fails at least one of them.
 """
+import dataclasses
 import json
 import math
 import os
@@ -618,3 +619,38 @@ def test_vacancy_decouples_its_neighbours():
     Fp = a.gradient(m, mask=O.T_EXC | O.T_DMI)[vac]
     expect = E_full.sum() + np.dot(m[vac], Fz) + 0.5 * np.dot(m[vac], Fa) + np.dot(m[vac], Fp)
     assert E_vac.sum() == pytest.approx(expect, rel=1e-12)
+
+
+# ------------------------------------------------------------------ velocity-projection minimiser, App. D
+def test_vp_constant_force_closed_form():
+    """One spin in a field: F = mu mu_B B z^ is constant, so D1-D3 give v_k = k dt F / m (always parallel to F,
+    the projection changes nothing) and the k-th iteration displaces by (k + 1/2) dt^2 F / m before the renormalisation (D5).
+    Pins the 1/(2m) factors, the momentum accumulation and the order of D2 -> D3 -> D1."""
+    mu, B, dt, m = 2.0, 1.5, 0.05, 0.7
+    s = OracleSystem(np.eye(3), [[0, 0, 0]], (1, 1, 1), (0, 0, 0))
+    s.set_mu_s([mu]); s.set_field(B, (0, 0, 1))
+    x = np.array([0.8, 0.0, 0.6]); s.set_spins([x])
+    F = np.array([0.0, 0.0, mu * O.MU_B * B])
+    for k in range(1, 12):
+        s.vp_iterate(1, dt, m)
+        x = x + (k + 0.5) * dt * dt / m * F
+        x /= np.linalg.norm(x)
+        assert np.abs(s.spins()[0] - x).max() < 1e-15, k
+
+
+def test_vp_stops_on_overshoot_and_finds_the_ferromagnet():
+    """D3: when v.F <= 0 the velocity is dropped, so the energy of a ferromagnet in a field goes down to the closed form
+    E = -N (mu mu_B B + z J / 2) (D4: F = -dH/dn, a wrong sign would climb) from a random start."""
+    w = dataclasses.replace(small(1, (8, 8, 1)), pair_D=small(1, (8, 8, 1)).pair_D * 0, aniso=[])    # K = 0: -z is not metastable
+    s = OracleSystem.from_workload(w)
+    E0 = s.energy()
+    s.vp_iterate(4000, 0.1, 1.0)
+    N = w.n_spins
+    Efm = -N * (w.mu_s[0] * O.MU_B * w.B + 0.5 * 4 * 1.0)
+    assert s.energy() < E0
+    assert s.energy() == pytest.approx(Efm, rel=1e-10)
+    assert np.abs(s.spins() - [0, 0, 1]).max() < 1e-6
+    # split calls continue the same trajectory (velocity and previous force persist)
+    a = OracleSystem.from_workload(w); a.vp_iterate(30, 0.1)
+    b = OracleSystem.from_workload(w); b.vp_iterate(13, 0.1); b.vp_iterate(17, 0.1)
+    assert np.array_equal(a.spins(), b.spins())
