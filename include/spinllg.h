@@ -127,6 +127,13 @@ int llg_set_solver(spin_system *sys, int solver);
 int llg_iterate(spin_system *sys, int64_t n_steps);
 int llg_get_step(const spin_system *sys, uint64_t *step);
 int llg_set_step(spin_system *sys, uint64_t step);
+/* Velocity-projection minimiser, App. D (:438-463), Eqs. D1-D5 with the force F_i = -dH/dn_i in meV (D4): per iteration the force
+ * of the current configuration, v <- v + dt/(2m)(F_old + F) (D2), the projection of v on F over all 3N components (D3), x <- x +
+ * dt v + dt^2/(2m) F (D1), renormalisation (D5).  dt and mass are the pseudo-time step and mass of that fictitious dynamics (dt^2/m
+ * in 1/meV).  Velocity and previous force persist between calls; spins_set*, llg_iterate, any setter or minimise_vp_reset clear them.
+ * Pinned spins do not move and carry no force.  Asynchronous on the system's stream.                                            */
+int minimise_vp(spin_system *sys, int64_t n_iterations, double dt, double mass);
+int minimise_vp_reset(spin_system *sys);
 /* wait for all work enqueued on the system's stream */
 int spin_synchronize(spin_system *sys);
 

@@ -20,7 +20,7 @@ EXPORTS = [
     "hamiltonian_set_mu_s", "hamiltonian_set_field", "hamiltonian_set_anisotropy", "hamiltonian_set_pairs",
     "hamiltonian_set_exchange_shells", "hamiltonian_set_dmi_shells", "hamiltonian_set_quadruplets",
     "hamiltonian_set_ddi", "spins_set_pinned", "spins_set", "spins_get", "spins_set_device", "spins_get_device",
-    "llg_configure", "llg_set_solver", "llg_iterate", "llg_get_step", "llg_set_step", "spin_synchronize",
+    "llg_configure", "llg_set_solver", "minimise_vp", "minimise_vp_reset", "llg_iterate", "llg_get_step", "llg_set_step", "spin_synchronize",
     "effective_field", "effective_field_device", "energy", "observables", "topological_charge",
     "spin_launch_counts", "spin_profile_enable", "spin_profile_get", "spin_set_option",
     "spin_kernel_info", "spin_jit_source", "spin_last_error", "spin_version",
@@ -64,6 +64,8 @@ def lib() -> C.CDLL:
         "llg_configure": (C.c_int, [vp, C.c_double, C.c_double, C.c_double, C.c_uint64, C.c_double, dp, C.c_double]),
         "llg_set_solver": (C.c_int, [vp, C.c_int]),
         "spins_set_pinned": (C.c_int, [vp, C.c_void_p]),
+        "minimise_vp": (C.c_int, [vp, C.c_int64, C.c_double, C.c_double]),
+        "minimise_vp_reset": (C.c_int, [vp]),
         "llg_iterate": (C.c_int, [vp, C.c_int64]),
         "llg_get_step": (C.c_int, [vp, C.POINTER(C.c_uint64)]),
         "llg_set_step": (C.c_int, [vp, C.c_uint64]),
@@ -218,6 +220,12 @@ class SpinSystem:
     def llg_configure(self, dt_fs, alpha, T=0.0, seed=0, u=0.0, j_dir=(1, 0, 0), beta=0.0):
         j, jp = _d(j_dir)
         _check(lib().llg_configure(self._h, float(dt_fs), float(alpha), float(T), int(seed), float(u), jp, float(beta)))
+
+    def minimise_vp(self, n_iterations, dt, mass=1.0):
+        _check(lib().minimise_vp(self._h, int(n_iterations), float(dt), float(mass)))
+
+    def minimise_vp_reset(self):
+        _check(lib().minimise_vp_reset(self._h))
 
     def spins_set_pinned(self, mask):
         """mask: N flags (boundary order) or None.  Pinned spins never move; a pinned zero vector is a vacancy."""

@@ -326,6 +326,7 @@ int allocate_arrays(spin_system *s, const DevicePlan &P, bool keep) {
 int ensure_plan(spin_system *s) {
     NEED_DEVICE(s);
     if (!s->plan_dirty) return SPIN_OK;
+    s->vp_active = false;
     DevicePlan P;
     int rc = build_plan(s, P);
     if (rc) return rc;
@@ -466,6 +467,7 @@ extern "C" int spin_geometry_create(const double bravais[9], int n_basis, const 
     s->seed = 0; s->step = 0; s->solver = SPIN_SOLVER_DEPONDT;
     s->stream = nullptr; s->own_stream = nullptr; s->cur = 0;
     s->d_n[0] = s->d_n[1] = s->d_np = s->d_A = s->d_fddi[0] = s->d_fddi[1] = s->d_aos = s->d_partials = s->d_result = nullptr;
+    s->d_vp = nullptr; s->vp_active = false; s->vp_cur = 0;
     s->d_step = nullptr; s->d_pin = nullptr; s->ddi = nullptr; s->plan_dirty = true;
     s->opt_graph = 1; s->opt_store_A = 0; s->graph_exec[0] = s->graph_exec[1] = nullptr; s->graph_steps = 0;
     s->n_launch = s->n_fft = 0; s->profile_on = 0;
@@ -479,6 +481,7 @@ extern "C" int spin_geometry_create(const double bravais[9], int n_basis, const 
     if (e == cudaSuccess) e = cudaMalloc(&s->d_aos, (size_t)3 * s->N * sizeof(double) + sizeof(int));
     if (e == cudaSuccess) e = cudaMalloc(&s->d_partials, (size_t)L.grid.x * L.grid.y * N_RED * sizeof(double));
     if (e == cudaSuccess) e = cudaMalloc(&s->d_result, 16 * sizeof(double));
+    if (e == cudaSuccess) e = cudaMalloc(&s->d_vp, 4 * sizeof(double));
     if (e == cudaSuccess) e = cudaMalloc(&s->d_step, sizeof(unsigned long long));
     if (e == cudaSuccess) e = cudaMemset(s->d_step, 0, sizeof(unsigned long long));
     if (e == cudaSuccess) e = cudaEventCreate(&s->ev0);
@@ -509,7 +512,7 @@ extern "C" void spin_system_destroy(spin_system *s) {
     ddi_release(s);
     jit_release(s);
     cudaFree(s->d_n[0]); cudaFree(s->d_n[1]); cudaFree(s->d_np); cudaFree(s->d_A); cudaFree(s->d_fddi[0]); cudaFree(s->d_fddi[1]);
-    cudaFree(s->d_pin);
+    cudaFree(s->d_pin); cudaFree(s->d_vp);
     cudaFree(s->d_aos); cudaFree(s->d_partials); cudaFree(s->d_result); cudaFree(s->d_step);
     if (s->ev0) cudaEventDestroy(s->ev0);
     if (s->ev1) cudaEventDestroy(s->ev1);
@@ -651,6 +654,7 @@ extern "C" int hamiltonian_set_ddi(spin_system *s, int enabled, const int img[3]
 // ---------------------------------------------------------------------------------------------- state
 static int pack_from_device_aos(spin_system *s, const double *d_aos) {
     NEED_DEVICE(s);
+    s->vp_active = false;
     int *bad = (int *)(s->d_aos + (size_t)3 * s->N);
     SPIN_CUDA(cudaMemsetAsync(bad, 0, sizeof(int), s->stream));
     const int nt = 256;
@@ -751,6 +755,7 @@ extern "C" int llg_iterate(spin_system *s, int64_t n_steps) {
     REQUIRE(s && n_steps >= 0, "bad argument");
     int rc = ensure_plan(s);
     if (rc) return rc;
+    s->vp_active = false;
     if (s->solver != SPIN_SOLVER_DEPONDT && !jit_ready(s))
         return spin::fail(SPIN_ERR_STATE, "the Heun and SIB solvers need the run-time specialised kernels (%s)", s->jit_note.c_str());
     int64_t done = 0;
@@ -847,6 +852,43 @@ extern "C" int observables(spin_system *s, double M[3], double *max_torque) {
     if (rc) return rc;
     if (M) for (int k = 0; k < 3; ++k) M[k] = r[6 + k] / (double)s->N;
     if (max_torque) *max_torque = r[9];
+    return SPIN_OK;
+}
+
+// Velocity-projection minimiser (App. D): 3 own launches per iteration (+ the dipolar field)
+extern "C" int minimise_vp(spin_system *s, int64_t n_iter, double dt, double mass) {
+    REQUIRE(s && n_iter >= 0, "bad argument");
+    REQUIRE(dt > 0.0 && isfinite(dt) && mass > 0.0 && isfinite(mass), "dt and mass must be positive");
+    int rc = ensure_plan(s);
+    if (rc) return rc;
+    const Launch L = brick_launch(s);
+    const int nblocks = (int)(L.grid.x * L.grid.y);
+    double *Fbuf[2] = {s->d_A, s->d_fddi[1]};
+    if (!s->vp_active) {
+        SPIN_CUDA(cudaMemsetAsync(s->d_vp, 0, 4 * sizeof(double), s->stream));
+        SPIN_CUDA(cudaMemsetAsync(Fbuf[0], 0, (size_t)s->nb * s->plan.sub * sizeof(double), s->stream));
+        s->vp_cur = 0;
+        s->vp_active = true;
+    }
+    double *n = s->d_n[s->cur];
+    const double c = 0.5 * dt / mass, h = 0.5 * dt * dt / mass;
+    for (int64_t it = 0; it < n_iter; ++it) {
+        if (s->ddi_on) { rc = ddi_field(s, n, s->d_fddi[0]); if (rc) return rc; }
+        double *Fold = Fbuf[s->vp_cur], *Fnew = Fbuf[s->vp_cur ^ 1];
+        if (L.flat) vp_force_kernel<32, 8, 1><<<L.grid, L.block, 0, s->stream>>>(s->plan, n, s->d_fddi[0], Fold, Fnew, s->d_partials);
+        else vp_force_kernel<32, 4, 2><<<L.grid, L.block, 0, s->stream>>>(s->plan, n, s->d_fddi[0], Fold, Fnew, s->d_partials);
+        vp_final_kernel<<<1, 32, 0, s->stream>>>(s->d_partials, nblocks, c, s->d_vp);
+        if (L.flat) vp_update_kernel<32, 8, 1><<<L.grid, L.block, 0, s->stream>>>(s->plan, n, Fnew, s->d_vp, dt, h);
+        else vp_update_kernel<32, 4, 2><<<L.grid, L.block, 0, s->stream>>>(s->plan, n, Fnew, s->d_vp, dt, h);
+        s->n_launch += 3;
+        s->vp_cur ^= 1;
+    }
+    SPIN_CUDA(cudaGetLastError());
+    return SPIN_OK;
+}
+extern "C" int minimise_vp_reset(spin_system *s) {
+    REQUIRE(s, "null system");
+    s->vp_active = false;
     return SPIN_OK;
 }
 

@@ -371,6 +371,74 @@ __global__ void reduce_final_kernel(const double *__restrict__ partials, int nbl
     if (lane == 0) out[k] = r;
 }
 
+// ---------------------------------------------------------------------------------------------------------
+// Velocity-projection minimiser, App. D.  After the projection D3 the velocity is a multiple of the force,
+// v = r F, so the 3N-dimensional velocity never needs to be stored: with c = dt/(2m),
+//     v.F' = (r + c) F.F' + c F'.F'        (v + c (F + F') dotted with the new force F')
+//     r'   = v.F' / F'.F' if v.F' > 0 else 0                                              (D3)
+//     x   <- x + (dt r' + dt^2/(2m)) F',  renormalised                                    (D1, D5)
+// vp_force_kernel: F' of every spin (pinned spins: 0) and the per-block partial sums of F.F' and F'.F'.
+template <int BX, int BY, int BZ>
+__global__ void __launch_bounds__(BX *BY *BZ)
+    vp_force_kernel(const __grid_constant__ DevicePlan P, const double *__restrict__ n, const double *__restrict__ fddi,
+                    const double *__restrict__ Fold, double *__restrict__ Fnew, double *__restrict__ partials) {
+    constexpr int NW = BX * BY * BZ / 32;
+    __shared__ double sh[2][NW];
+    const Site s = locate<BX, BY, BZ>(P);
+    double a = 0.0, b = 0.0;
+    if (s.valid) {
+        const double *const cfg[1] = {n};
+        double own[1][3], F[1][3] = {{0.0, 0.0, 0.0}};
+        load3(P, n, s.idx, own[0]);
+        if (!pinned(P, s)) {
+            short_range_force<1>(P, cfg, s, own, T_ALL, F);
+            if (P.has_ddi) { double d[3]; load3(P, fddi, s.idx, d); F[0][0] += d[0]; F[0][1] += d[1]; F[0][2] += d[2]; }
+        }
+        double fo[3];
+        load3(P, Fold, s.idx, fo);
+        store3(P, Fnew, s.idx, F[0]);
+        a = fo[0] * F[0][0] + fo[1] * F[0][1] + fo[2] * F[0][2];
+        b = F[0][0] * F[0][0] + F[0][1] * F[0][1] + F[0][2] * F[0][2];
+    }
+    a = warp_sum(a); b = warp_sum(b);
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    if (lane == 0) { sh[0][w] = a; sh[1][w] = b; }
+    __syncthreads();
+    if (threadIdx.x < 2) {
+        double r = sh[threadIdx.x][0];
+        for (int i = 1; i < NW; ++i) r += sh[threadIdx.x][i];
+        partials[(size_t)(blockIdx.y * gridDim.x + blockIdx.x) * 2 + threadIdx.x] = r;
+    }
+}
+// one warp folds the partials in a fixed order and advances the scalar state: st[0] = r, st[1] = 1 after the first iteration
+__global__ void vp_final_kernel(const double *__restrict__ partials, int nblocks, double c, double *__restrict__ st) {
+    double a = 0.0, b = 0.0;
+    for (int i = threadIdx.x; i < nblocks; i += 32) { a += partials[2 * (size_t)i]; b += partials[2 * (size_t)i + 1]; }
+    a = warp_sum(a); b = warp_sum(b);
+    if (threadIdx.x == 0) {
+        double r = st[0];
+        if (st[1] == 0.0) { a = b; r = 0.0; st[1] = 1.0; }      // first iteration: v = 0 and F(t) = F(t+dt)
+        const double vF = (r + c) * a + c * b;
+        st[0] = (vF > 0.0 && b > 0.0) ? vF / b : 0.0;
+        st[2] = b;                                               // |F|^2, for convergence checks
+    }
+}
+template <int BX, int BY, int BZ>
+__global__ void __launch_bounds__(BX *BY *BZ)
+    vp_update_kernel(const __grid_constant__ DevicePlan P, double *__restrict__ n, const double *__restrict__ F, const double *__restrict__ st,
+                     double dt, double half_dt2_over_m) {
+    const Site s = locate<BX, BY, BZ>(P);
+    if (!s.valid || pinned(P, s)) return;
+    double x[3], f[3];
+    load3(P, n, s.idx, x);
+    load3(P, F, s.idx, f);
+    const double w = fma(dt, st[0], half_dt2_over_m);
+    x[0] = fma(w, f[0], x[0]); x[1] = fma(w, f[1], x[1]); x[2] = fma(w, f[2], x[2]);
+    const double sc = 1.0 / sqrt(x[0] * x[0] + x[1] * x[1] + x[2] * x[2]);
+    x[0] *= sc; x[1] *= sc; x[2] *= sc;
+    store_spin(P, n, s.ia, s.ib, s.ic, s.idx, x);
+}
+
 // Topological charge, App. A: Q = (1/4 pi) sum_l A_l over the two elementary triangles of every cell of every
 // a-b plane; A_l = signed area of the spherical triangle (n_i, n_j, n_k), evaluated as 2 atan2(n_i.(n_j x n_k), 1 + n_i.n_j +
 // n_j.n_k + n_k.n_i) -- the same angle as Eq. A2 with its sign rule, without the square root and the acos near +-1.

@@ -125,6 +125,9 @@ struct spin_system {
     double *d_result;              // reduction result (16 doubles)
     unsigned long long *d_step;    // device copy of the step counter (read by the kernels)
     unsigned char *d_pin;          // pinned-spin flags (boundary order), null if none
+    double *d_vp;                  // velocity-projection state: ratio r, started flag, |F|^2
+    bool vp_active;                // d_A holds the force of the previous VP iteration
+    int vp_cur;                    // which of {d_A, d_fddi[1]} holds it
     spin::DevicePlan plan;
     bool plan_dirty;
     DdiState *ddi;

@@ -455,3 +455,41 @@ def test_pinned_spins_and_vacancies(P, O, cfg, steps, use_jit):
     g.spins_set_pinned(None)
     with pytest.raises(P.SpinError):
         g.spins_set(n0)
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# Velocity-projection minimiser (App. D)
+@pytest.mark.parametrize("cfg,iters", [(1, 300), (2, 200), (3, 200), (4, 200), (5, 40)])
+def test_velocity_projection_parity(P, O, cfg, iters):
+    w = W.CONFIGS[cfg]().resized(REPLICAS[cfg], 1)
+    g, o = pair(P, O, w)
+    E0 = g.energy()[0]
+    g.minimise_vp(iters, 0.05, 1.0); o.vp_iterate(iters, 0.05, 1.0)
+    ng, no = g.spins_get(), o.spins()
+    d = np.abs(ng - no).max()
+    print(f"vp cfg{cfg} iters={iters}: max|dn| = {d:.3e}, E {E0:.6f} -> {g.energy()[0]:.6f}")
+    assert d <= SPIN_ATOL
+    assert g.energy()[0] < E0
+    assert np.abs(np.linalg.norm(ng, axis=1) - 1).max() < 4e-16
+    # split calls continue the same trajectory; an LLG step or spins_set in between restarts from v = 0
+    a = P.SpinSystem.from_workload(w); a.minimise_vp(17, 0.05); a.minimise_vp(iters - 17, 0.05)
+    assert np.array_equal(a.spins_get(), ng)
+    b = P.SpinSystem.from_workload(w); b.minimise_vp(17, 0.05); b.minimise_vp_reset(); b.minimise_vp(iters - 17, 0.05)
+    assert not np.array_equal(b.spins_get(), ng)
+
+
+def test_velocity_projection_with_pinned_spins_and_convergence(P, O):
+    w = dataclasses.replace(W.config1().resized((24, 16, 1), 1), pair_D=W.config1().pair_D * 0, aniso=[])
+    mask = np.zeros(w.n_spins, np.uint8); mask[::7] = 1
+    g = P.SpinSystem.from_workload(w); o = O.OracleSystem.from_workload(w)
+    g.spins_set_pinned(mask); o.set_pinned(mask)
+    start = g.spins_get()
+    g.minimise_vp(150, 0.1); o.vp_iterate(150, 0.1)
+    assert np.abs(g.spins_get() - o.spins()).max() <= SPIN_ATOL
+    assert np.array_equal(g.spins_get()[mask == 1], start[mask == 1])
+    # without pins: the ferromagnet in a field, closed-form ground-state energy -N (mu mu_B B + z J / 2)
+    h = P.SpinSystem.from_workload(w)
+    h.minimise_vp(4000, 0.1)
+    Efm = -w.n_spins * (w.mu_s[0] * O.MU_B * w.B + 2.0)
+    assert h.energy()[0] == pytest.approx(Efm, rel=1e-10)
+    assert h.observables()[1] < 1e-6
