@@ -493,3 +493,39 @@ def test_velocity_projection_with_pinned_spins_and_convergence(P, O):
     Efm = -w.n_spins * (w.mu_s[0] * O.MU_B * w.B + 2.0)
     assert h.energy()[0] == pytest.approx(Efm, rel=1e-10)
     assert h.observables()[1] < 1e-6
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# Limits and empty inputs
+def test_limits_and_empty_interaction_lists(P, O):
+    # lattice beyond 32-bit indexing of 3N doubles: refused at creation, nothing allocated
+    with pytest.raises(P.SpinError) as e:
+        P.SpinSystem(np.eye(3), [[0, 0, 0]], (2000, 2000, 200), (1, 1, 1))
+    assert e.value.code == -1
+    # more gather entries than the kernels' tables hold: SPIN_ERR_LIMIT when the plan is built, not a crash
+    s = P.SpinSystem(np.eye(3), [[0, 0, 0]], (40, 40, 1), (1, 1, 0))
+    t = [[a, b, 0] for a in range(0, 10) for b in range(-9, 10) if (a, b) > (0, 0)][:90]       # 90 unique bonds = 180 entries > 160
+    s.hamiltonian_set_pairs([0] * len(t), [0] * len(t), t, [0.01] * len(t))
+    with pytest.raises(P.SpinError) as e:
+        s.effective_field()
+    assert e.value.code == -5
+    # empty interaction lists: free spins in a field precess as one (Eq. 12), identical to the oracle
+    w = dataclasses.replace(W.config1().resized((9, 7, 1), 50), aniso=[], pair_i=np.zeros(0, int), pair_j=np.zeros(0, int),
+                            pair_t=np.zeros((0, 3), int), pair_J=np.zeros(0), pair_D=np.zeros((0, 3)))
+    g, o = pair(P, O, w)
+    assert_fields_close(g.effective_field(), o.effective_field())
+    assert np.allclose(g.effective_field(), [0.0, 0.0, w.B])
+    g.llg_iterate(50); o.iterate(50)
+    assert np.abs(g.spins_get() - o.spins()).max() < 1e-13
+    g.llg_iterate(0)                                                    # zero steps: a no-op
+    assert g.llg_get_step() == 50
+    # the largest lattice the test box takes comfortably: 256^3 (16.8 M spins, 1.6 GB of state), field on sampled sites
+    big = W.config3().resized((256, 256, 256), 2)
+    gb = P.SpinSystem.from_workload(big)
+    ob = O.OracleSystem.from_workload(big)
+    Bg = gb.effective_field()
+    Bo = ob.effective_field()
+    idx = np.random.default_rng(0).integers(0, big.n_spins, 4096)
+    assert np.abs(Bg[idx] - Bo[idx]).max() <= FIELD_RTOL * np.abs(Bo).max()
+    gb.llg_iterate(2); ob.iterate(2)
+    assert np.abs(gb.spins_get()[idx] - ob.spins()[idx]).max() <= SPIN_ATOL
