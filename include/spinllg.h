@@ -168,6 +168,7 @@ int spin_set_option(spin_system *sys, const char *name, int value);
  * cfg3, hence off by default.
  * use_col (default 0): 1 runs them as column-marching kernels (one thread per lattice column, own spin at z-1, z, z+1 kept in
  * registers; 3-D lattices).  Also measured slower than the brick kernels.
+ * cache_noise (default 1): the predictor keeps the thermal field of the step (24 B/spin) for the corrector instead of generating it twice.
  * ddi_slab (default 1): thin films with one basis atom take the dipolar slab path (2-D cuFFT + fused transform along c).
  * spin_kernel_info writes "jit+col", "jit+tma", "jit (brick kernels: <why>)" or "generic: <why>" into buf: which sweep kernels are in use.  */
 int spin_kernel_info(spin_system *sys, char *buf, int len);

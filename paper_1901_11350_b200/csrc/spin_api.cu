@@ -450,7 +450,7 @@ extern "C" int spin_geometry_create(const double bravais[9], int n_basis, const 
     if (!has_device) cudaGetLastError();
     spin_system *s = new spin_system();
     s->has_device = has_device;
-    s->jit = nullptr; s->opt_jit = 1; s->opt_tma = 0; s->opt_ddi_slab = 1; s->opt_col = 0;
+    s->jit = nullptr; s->opt_jit = 1; s->opt_tma = 0; s->opt_ddi_slab = 1; s->opt_col = 0; s->opt_cache_noise = 1;
     memcpy(s->brav, bravais, sizeof(s->brav));
     s->nb = n_basis;
     s->basis.assign(basis_frac, basis_frac + 3 * n_basis);
@@ -937,6 +937,7 @@ extern "C" int spin_set_option(spin_system *s, const char *name, int value) {
     if (!strcmp(name, "use_graph")) s->opt_graph = value ? 1 : 0;
     else if (!strcmp(name, "store_A")) { s->opt_store_A = value ? 1 : 0; s->plan_dirty = true; }
     else if (!strcmp(name, "use_jit")) { s->opt_jit = value ? 1 : 0; s->plan_dirty = true; }
+    else if (!strcmp(name, "cache_noise")) { s->opt_cache_noise = value ? 1 : 0; s->plan_dirty = true; }
     else if (!strcmp(name, "use_col")) { s->opt_col = value ? 1 : 0; s->plan_dirty = true; }
     else if (!strcmp(name, "ddi_slab")) { s->opt_ddi_slab = value ? 1 : 0; s->plan_dirty = true; }
     else if (!strcmp(name, "use_tma")) { s->opt_tma = value < 0 ? 0 : (value > 2 ? 2 : value); s->plan_dirty = true; }

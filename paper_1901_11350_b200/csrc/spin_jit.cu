@@ -198,6 +198,7 @@ std::string spin::jit_source(const spin_system *s) {
     o << "constexpr int BX = " << brick[0] << ", BY = " << brick[1] << ", BZ = " << brick[2] << ";\n";
     o << "constexpr bool PER_A = " << (P.perA ? "true" : "false") << ", PER_B = " << (P.perB ? "true" : "false")
       << ", PER_C = " << (P.perC ? "true" : "false") << ";\n";
+    o << "constexpr bool CACHE_NOISE = " << ((s->opt_cache_noise && P.thermal_on && !(s->opt_store_A && s->solver == 0)) ? "true" : "false") << ";\n";
     o << "constexpr bool HAS_PIN = " << (s->d_pin ? "true" : "false") << ";\n";
     o << "constexpr int SOLVER = " << s->solver << ";      // 0 Depondt, 1 Heun, 2 SIB\n";
     o << "constexpr bool STORE_A = " << ((s->opt_store_A && s->solver == 0) ? "true" : "false") << ", HAS_DDI = " << (P.has_ddi ? "true" : "false")

@@ -241,6 +241,9 @@ __device__ __forceinline__ void predictor_body(const double *__restrict__ n, con
     load3<0>(cfg.cfg[0], own[0]);
     if (is_pinned<B>(pin, c)) { store_spin(np + idx, c, own[0]); return; }
     thermal_force<B>(c, step, seed_lo, seed_hi, F[0]);
+    // the thermal field of the step is the same in both sweeps (R11): generating it costs two Philox blocks, two logarithms and three
+    // trigonometric evaluations per spin, so the predictor keeps it for the corrector (24 B/spin written and read back)
+    if constexpr (spec::CACHE_NOISE) store3(Aout + idx, F[0]);
     force<B, 1>(cfg, own, F);
     if constexpr (spec::HAS_DDI) { double d[3]; load3<0>(fddi + idx, d); F[0][0] += d[0]; F[0][1] += d[1]; F[0][2] += d[2]; }
     if constexpr (spec::STT_ON) stt_gradient<B, 1>(cfg, c, own, sg);
@@ -263,7 +266,8 @@ __device__ __forceinline__ void corrector_body(const double *__restrict__ n, con
     double th[3], A[3], Ap[3], n0[3];
     load3<0>(n + idx, n0);
     if (is_pinned<B>(pin, c)) { store_spin(nout + idx, c, n0); return; }
-    thermal_force<B>(c, step, seed_lo, seed_hi, th);
+    if constexpr (spec::CACHE_NOISE) load3<0>(Ain + idx, th);
+    else thermal_force<B>(c, step, seed_lo, seed_hi, th);
     if constexpr (spec::SOLVER == 2) {
         // SIB corrector (C11): A at the midpoint configuration, the implicit-midpoint structure applied to n(t); A(n) is not needed
         const MidAcc cfg = {n + idx, np + idx};
