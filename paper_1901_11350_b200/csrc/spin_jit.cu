@@ -38,6 +38,10 @@ struct JitState {
     std::string tma_note;     // why not, if not
     TmaGeo gp, gc;
     cudaKernel_t k_pred_tma, k_corr_tma;
+    // all steps in one cooperative launch (launch-bound lattices)
+    bool coop;
+    cudaKernel_t k_coop;
+    int coop_grid;
     // column-marching sweeps
     bool col;
     cudaKernel_t k_pred_col, k_corr_col;
@@ -376,6 +380,7 @@ int spin::jit_prepare(spin_system *s) {
     j->loaded = false;
     j->tma = false;
     j->col = false;
+    j->coop = false;
     j->source = src;
     s->jit = j;
     std::string cubin;
@@ -388,6 +393,22 @@ int spin::jit_prepare(spin_system *s) {
     if (e == cudaSuccess) e = cudaLibraryGetKernel(&j->k_corr, j->lib, "jit_corrector");
     if (e != cudaSuccess) return spin::fail(SPIN_ERR_CUDA, "cudaLibraryGetKernel failed: %s", cudaGetErrorString(e));
     tma_prepare(s, j);
+    j->coop = false;
+    if (s->opt_coop && !s->ddi_on) {
+        int dev = 0, can = 0, occ = 0;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&can, cudaDevAttrCooperativeLaunch, dev);
+        dim3 grid, block;
+        jit_brick_launch(s, grid, block);
+        cudaError_t ce = cudaLibraryGetKernel(&j->k_coop, j->lib, "jit_steps_coop");
+        if (ce == cudaSuccess) ce = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, (const void *)j->k_coop, (int)block.x, 0);
+        if (ce == cudaSuccess && can && occ > 0) {
+            j->coop_grid = std::min((int)(grid.x * grid.y), occ * sm_count(s));
+            j->coop = true;
+        } else {
+            cudaGetLastError();
+        }
+    }
     j->col = plan_col(s, j->col_geo);
     if (j->col) {
         e = cudaLibraryGetKernel(&j->k_pred_col, j->lib, "jit_predictor_col");
@@ -420,6 +441,25 @@ int spin::jit_launch_corrector(spin_system *s, dim3 grid, dim3 block, const doub
                     (void *)&seed_lo, (void *)&seed_hi, (void *)&pin};
     jit_brick_launch(s, grid, block);
     SPIN_CUDA(cudaLaunchKernel((const void *)s->jit->k_corr, grid, block, args, 0, s->stream));
+    return SPIN_OK;
+}
+
+bool spin::jit_coop_ready(const spin_system *s) { return s->jit && s->jit->loaded && s->jit->coop; }
+
+// nsteps Depondt/Heun/SIB steps in one cooperative launch; reads n from d_n[cur], leaves the result in d_n[cur ^ (nsteps & 1)]
+int spin::jit_launch_steps_coop(spin_system *s, unsigned nsteps) {
+    JitState *j = s->jit;
+    unsigned seed_lo = s->plan.seed_lo, seed_hi = s->plan.seed_hi;
+    const unsigned long long *d_step = s->d_step;
+    double *n0 = s->d_n[s->cur], *n1 = s->d_n[s->cur ^ 1], *np = s->d_np, *aux = s->d_A;
+    const unsigned char *pin = s->d_pin;
+    unsigned int *bar = s->d_bar;
+    SPIN_CUDA(cudaMemsetAsync(bar, 0, sizeof(unsigned int), s->stream));
+    void *args[] = {(void *)&n0, (void *)&n1, (void *)&np, (void *)&aux, (void *)&d_step, (void *)&nsteps, (void *)&seed_lo, (void *)&seed_hi,
+                    (void *)&pin, (void *)&bar};
+    dim3 grid, block;
+    jit_brick_launch(s, grid, block);
+    SPIN_CUDA(cudaLaunchCooperativeKernel((const void *)j->k_coop, dim3((unsigned)j->coop_grid), block, args, 0, s->stream));
     return SPIN_OK;
 }
 

@@ -49,11 +49,16 @@ __host__ __device__ constexpr int lin() {
 }
 
 // q points at the x component of the own site; O is a compile-time offset in doubles
-template <int O>
+// CG = true: coherent L1-cached loads (ld.global.ca) for the cooperative kernel, in which other blocks rewrite the arrays between
+// grid barriers -- the acquire fence of the barrier invalidates L1, after which weak loads must observe the released stores; the
+// non-coherent read-only path (ld.global.nc, __ldg) is only legal for data nobody writes during the kernel
+template <int O, bool CG = false>
 __device__ __forceinline__ void load3(const double *__restrict__ q, double (&v)[3]) {
-    v[0] = __ldg(q + O);
-    v[1] = __ldg(q + O + spec::PA);
-    v[2] = __ldg(q + O + 2 * spec::PA);
+    if constexpr (CG) {
+        v[0] = __ldca(q + O); v[1] = __ldca(q + O + spec::PA); v[2] = __ldca(q + O + 2 * spec::PA);
+    } else {
+        v[0] = __ldg(q + O); v[1] = __ldg(q + O + spec::PA); v[2] = __ldg(q + O + 2 * spec::PA);
+    }
 }
 __device__ __forceinline__ void store3(double *__restrict__ q, const double (&v)[3]) {
     q[0] = v[0]; q[spec::PA] = v[1]; q[2 * spec::PA] = v[2];
@@ -84,21 +89,22 @@ __device__ __forceinline__ void store_spin(double *__restrict__ q, const Coord &
 // Site accessors: where the partner (sublattice BJ at translation DA, DB, DC) of a site of sublattice B is read from.
 // GlobalAcc: the ghost-cell arrays in global memory (own address + immediate); RingAcc (spin_jit_tma.cuh): the ring of lattice
 // planes that TMA stages in shared memory.
-template <int NCONF>
+template <int NCONF, bool CG = false>
 struct GlobalAcc {
     const double *cfg[NCONF];      // x component of the own site in configuration k
     template <int B, int BJ, int DA, int DB, int DC>
-    __device__ __forceinline__ void load(int k, double (&v)[3]) const { load3<lin<B, BJ, DA, DB, DC>()>(cfg[k], v); }
+    __device__ __forceinline__ void load(int k, double (&v)[3]) const { load3<lin<B, BJ, DA, DB, DC>(), CG>(cfg[k], v); }
 };
 
 // SIB corrector (C11): the field is evaluated at the midpoint configuration {(n_j + n_j^p)/2}
+template <bool CG = false>
 struct MidAcc {
     const double *a, *b;           // own site in n and in n^p
     template <int B, int BJ, int DA, int DB, int DC>
     __device__ __forceinline__ void load(int, double (&v)[3]) const {
         double u[3], w[3];
-        load3<lin<B, BJ, DA, DB, DC>()>(a, u);
-        load3<lin<B, BJ, DA, DB, DC>()>(b, w);
+        load3<lin<B, BJ, DA, DB, DC>(), CG>(a, u);
+        load3<lin<B, BJ, DA, DB, DC>(), CG>(b, w);
         v[0] = 0.5 * (u[0] + w[0]); v[1] = 0.5 * (u[1] + w[1]); v[2] = 0.5 * (u[2] + w[2]);
     }
 };
@@ -196,9 +202,8 @@ __device__ __forceinline__ void rotation_field(const double (&n)[3], const doubl
 }
 
 template <int B>
-__device__ __forceinline__ bool locate(Coord &c, int &idx) {
+__device__ __forceinline__ bool locate(Coord &c, int &idx, int brick) {
     constexpr int nbx = (spec::NA + spec::BX - 1) / spec::BX, nby = (spec::NB + spec::BY - 1) / spec::BY;
-    int brick = blockIdx.x;
     const int bx = brick % nbx;
     brick /= nbx;
     const int by = brick % nby, bz = brick / nby;
@@ -216,7 +221,8 @@ __device__ __forceinline__ void thermal_force(const Coord &c, u64 step, u32 seed
         const u32 cell = (u32)(c.ia + spec::NA * c.ib + (spec::NA * spec::NB) * c.ic);
         double xi[3];
         spin::thermal_xi(seed_lo, seed_hi, step, (u32)B + (u32)spec::NBASIS * cell, xi);
-        f[0] = specc::SIGMA[B] * xi[0]; f[1] = specc::SIGMA[B] * xi[1]; f[2] = specc::SIGMA[B] * xi[2];
+        // rounded products (never contracted into a following add): the cached and the regenerated thermal field are the same bits
+        f[0] = __dmul_rn(specc::SIGMA[B], xi[0]); f[1] = __dmul_rn(specc::SIGMA[B], xi[1]); f[2] = __dmul_rn(specc::SIGMA[B], xi[2]);
     } else {
         f[0] = -0.0; f[1] = -0.0; f[2] = -0.0;      // additive identity that the compiler may fold away (x + -0.0 == x exactly)
     }
@@ -229,23 +235,23 @@ __device__ __forceinline__ bool is_pinned(const unsigned char *__restrict__ pin,
     else return false;
 }
 
-template <int B>
+template <int B, bool CG = false>
 __device__ __forceinline__ void predictor_body(const double *__restrict__ n, const double *__restrict__ fddi, double *__restrict__ np,
-                                               double *__restrict__ Aout, u64 step, u32 seed_lo, u32 seed_hi, const unsigned char *__restrict__ pin) {
+                                               double *__restrict__ Aout, u64 step, u32 seed_lo, u32 seed_hi, const unsigned char *__restrict__ pin, int brick) {
     Coord c;
     int idx;
-    if (!locate<B>(c, idx)) return;
-    GlobalAcc<1> cfg;
+    if (!locate<B>(c, idx, brick)) return;
+    GlobalAcc<1, CG> cfg;
     cfg.cfg[0] = n + idx;
     double own[1][3], F[1][3], sg[1][3] = {{0.0, 0.0, 0.0}};
-    load3<0>(cfg.cfg[0], own[0]);
+    load3<0, CG>(cfg.cfg[0], own[0]);
     if (is_pinned<B>(pin, c)) { store_spin(np + idx, c, own[0]); return; }
     thermal_force<B>(c, step, seed_lo, seed_hi, F[0]);
     // the thermal field of the step is the same in both sweeps (R11): generating it costs two Philox blocks, two logarithms and three
     // trigonometric evaluations per spin, so the predictor keeps it for the corrector (24 B/spin written and read back)
     if constexpr (spec::CACHE_NOISE) store3(Aout + idx, F[0]);
     force<B, 1>(cfg, own, F);
-    if constexpr (spec::HAS_DDI) { double d[3]; load3<0>(fddi + idx, d); F[0][0] += d[0]; F[0][1] += d[1]; F[0][2] += d[2]; }
+    if constexpr (spec::HAS_DDI) { double d[3]; load3<0, CG>(fddi + idx, d); F[0][0] += d[0]; F[0][1] += d[1]; F[0][2] += d[2]; }
     if constexpr (spec::STT_ON) stt_gradient<B, 1>(cfg, c, own, sg);
     double A[3], out[3];
     rotation_field<B>(own[0], F[0], sg[0], A);
@@ -256,27 +262,27 @@ __device__ __forceinline__ void predictor_body(const double *__restrict__ n, con
     if constexpr (spec::STORE_A) store3(Aout + idx, A);
 }
 
-template <int B>
+template <int B, bool CG = false>
 __device__ __forceinline__ void corrector_body(const double *__restrict__ n, const double *__restrict__ np, const double *__restrict__ fddi_n,
                                                const double *__restrict__ fddi_np, const double *__restrict__ Ain, double *__restrict__ nout,
-                                               u64 step, u32 seed_lo, u32 seed_hi, const unsigned char *__restrict__ pin) {
+                                               u64 step, u32 seed_lo, u32 seed_hi, const unsigned char *__restrict__ pin, int brick) {
     Coord c;
     int idx;
-    if (!locate<B>(c, idx)) return;
+    if (!locate<B>(c, idx, brick)) return;
     double th[3], A[3], Ap[3], n0[3];
-    load3<0>(n + idx, n0);
+    load3<0, CG>(n + idx, n0);
     if (is_pinned<B>(pin, c)) { store_spin(nout + idx, c, n0); return; }
-    if constexpr (spec::CACHE_NOISE) load3<0>(Ain + idx, th);
+    if constexpr (spec::CACHE_NOISE) load3<0, CG>(Ain + idx, th);
     else thermal_force<B>(c, step, seed_lo, seed_hi, th);
     if constexpr (spec::SOLVER == 2) {
         // SIB corrector (C11): A at the midpoint configuration, the implicit-midpoint structure applied to n(t); A(n) is not needed
-        const MidAcc cfg = {n + idx, np + idx};
+        const MidAcc<CG> cfg = {n + idx, np + idx};
         double own[1][3], F[1][3] = {{th[0], th[1], th[2]}}, sg[1][3] = {{0.0, 0.0, 0.0}};
-        cfg.load<B, B, 0, 0, 0>(0, own[0]);
+        cfg.template load<B, B, 0, 0, 0>(0, own[0]);
         force<B, 1>(cfg, own, F);
         if constexpr (spec::HAS_DDI) {      // the dipolar force is linear in the configuration: its value at the midpoint is the mean
             double d[3], e[3];
-            load3<0>(fddi_n + idx, d); load3<0>(fddi_np + idx, e);
+            load3<0, CG>(fddi_n + idx, d); load3<0, CG>(fddi_np + idx, e);
             F[0][0] += 0.5 * (d[0] + e[0]); F[0][1] += 0.5 * (d[1] + e[1]); F[0][2] += 0.5 * (d[2] + e[2]);
         }
         if constexpr (spec::STT_ON) stt_gradient<B, 1>(cfg, c, own, sg);
@@ -288,27 +294,27 @@ __device__ __forceinline__ void corrector_body(const double *__restrict__ n, con
     }
     double np0[3] = {0.0, 0.0, 0.0};
     if constexpr (spec::STORE_A) {
-        GlobalAcc<1> cfg;
+        GlobalAcc<1, CG> cfg;
         cfg.cfg[0] = np + idx;
         double own[1][3], F[1][3] = {{th[0], th[1], th[2]}}, sg[1][3] = {{0.0, 0.0, 0.0}};
-        load3<0>(cfg.cfg[0], own[0]);
+        load3<0, CG>(cfg.cfg[0], own[0]);
         force<B, 1>(cfg, own, F);
-        if constexpr (spec::HAS_DDI) { double d[3]; load3<0>(fddi_np + idx, d); F[0][0] += d[0]; F[0][1] += d[1]; F[0][2] += d[2]; }
+        if constexpr (spec::HAS_DDI) { double d[3]; load3<0, CG>(fddi_np + idx, d); F[0][0] += d[0]; F[0][1] += d[1]; F[0][2] += d[2]; }
         if constexpr (spec::STT_ON) stt_gradient<B, 1>(cfg, c, own, sg);
         rotation_field<B>(own[0], F[0], sg[0], Ap);
-        load3<0>(Ain + idx, A);
+        load3<0, CG>(Ain + idx, A);
     } else {
-        GlobalAcc<2> cfg;
+        GlobalAcc<2, CG> cfg;
         cfg.cfg[0] = n + idx; cfg.cfg[1] = np + idx;
         double own[2][3], F[2][3] = {{th[0], th[1], th[2]}, {th[0], th[1], th[2]}}, sg[2][3] = {{0.0, 0.0, 0.0}, {0.0, 0.0, 0.0}};
         own[0][0] = n0[0]; own[0][1] = n0[1]; own[0][2] = n0[2];
-        load3<0>(cfg.cfg[1], own[1]);
+        load3<0, CG>(cfg.cfg[1], own[1]);
         np0[0] = own[1][0]; np0[1] = own[1][1]; np0[2] = own[1][2];
         force<B, 2>(cfg, own, F);
         if constexpr (spec::HAS_DDI) {
             double d[3];
-            load3<0>(fddi_n + idx, d); F[0][0] += d[0]; F[0][1] += d[1]; F[0][2] += d[2];
-            load3<0>(fddi_np + idx, d); F[1][0] += d[0]; F[1][1] += d[1]; F[1][2] += d[2];
+            load3<0, CG>(fddi_n + idx, d); F[0][0] += d[0]; F[0][1] += d[1]; F[0][2] += d[2];
+            load3<0, CG>(fddi_np + idx, d); F[1][0] += d[0]; F[1][1] += d[1]; F[1][2] += d[2];
         }
         if constexpr (spec::STT_ON) stt_gradient<B, 2>(cfg, c, own, sg);
         rotation_field<B>(own[0], F[0], sg[0], A);
@@ -346,7 +352,7 @@ extern "C" __global__ void SPIN_BOUNDS(spec::BX *spec::BY *spec::BZ)
                   const unsigned char *__restrict__ pin) {
     const unsigned long long step = *d_step + step_add;
     spinjit::dispatch_basis<0>((int)blockIdx.y, [&](auto b) {
-        spinjit::predictor_body<decltype(b)::value>(n, fddi, np, Aout, step, seed_lo, seed_hi, pin);
+        spinjit::predictor_body<decltype(b)::value>(n, fddi, np, Aout, step, seed_lo, seed_hi, pin, (int)blockIdx.x);
     });
 }
 
@@ -357,8 +363,57 @@ extern "C" __global__ void SPIN_BOUNDS(spec::BX *spec::BY *spec::BZ)
                   const unsigned char *__restrict__ pin) {
     const unsigned long long step = *d_step + step_add;
     spinjit::dispatch_basis<0>((int)blockIdx.y, [&](auto b) {
-        spinjit::corrector_body<decltype(b)::value>(n, np, fddi_n, fddi_np, Ain, nout, step, seed_lo, seed_hi, pin);
+        spinjit::corrector_body<decltype(b)::value>(n, np, fddi_n, fddi_np, Ain, nout, step, seed_lo, seed_hi, pin, (int)blockIdx.x);
     });
+}
+
+// ---------------------------------------------------------------------------------------------------------------------------
+// Launch-bound lattices ("limited by the overhead of CUDA kernel launches"): ALL steps of an llg_iterate call in ONE
+// cooperative launch.  Every block walks its share of the bricks, predictor sweep -> grid barrier -> corrector sweep -> grid
+// barrier, ping-ponging between the two n buffers; the arrays are read with coherent loads (not the read-only path) because other blocks
+// rewrite them between barriers.  The barrier is a monotone arrival counter in global memory (release: fence + atomic add; acquire: polling
+// load + fence); a lost arrival traps instead of hanging the device.  All blocks are co-resident (cooperative launch).
+namespace spinjit {
+__device__ __forceinline__ void grid_barrier(unsigned int *bar, unsigned int nblocks, unsigned int &target) {
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        target += nblocks;
+        __threadfence();
+        atomicAdd(bar, 1u);
+        unsigned int seen = 0, polls = 0;
+        do {
+            asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(seen) : "l"(bar) : "memory");
+            if (++polls > (1u << 28)) __trap();
+        } while (seen < target);
+        __threadfence();
+    }
+    __syncthreads();
+}
+}  // namespace spinjit
+
+extern "C" __global__ void SPIN_BOUNDS(spec::BX *spec::BY *spec::BZ)
+    jit_steps_coop(double *__restrict__ n0, double *__restrict__ n1, double *__restrict__ np, double *__restrict__ aux,
+                   const unsigned long long *__restrict__ d_step, unsigned int nsteps, unsigned int seed_lo, unsigned int seed_hi,
+                   const unsigned char *__restrict__ pin, unsigned int *bar) {
+    using namespace spinjit;
+    constexpr int NBRICKS = ((spec::NA + spec::BX - 1) / spec::BX) * ((spec::NB + spec::BY - 1) / spec::BY) * ((spec::NC + spec::BZ - 1) / spec::BZ);
+    unsigned int target = 0;
+    const unsigned long long step0 = *d_step;
+    for (unsigned int k = 0; k < nsteps; ++k) {
+        const double *n = (k & 1u) ? n1 : n0;
+        double *nout = (k & 1u) ? n0 : n1;
+        const unsigned long long step = step0 + k;
+        for (int item = blockIdx.x; item < NBRICKS * spec::NBASIS; item += gridDim.x)
+            dispatch_basis<0>(item / NBRICKS, [&](auto b) {
+                predictor_body<decltype(b)::value, true>(n, nullptr, np, aux, step, seed_lo, seed_hi, pin, item % NBRICKS);
+            });
+        grid_barrier(bar, gridDim.x, target);
+        for (int item = blockIdx.x; item < NBRICKS * spec::NBASIS; item += gridDim.x)
+            dispatch_basis<0>(item / NBRICKS, [&](auto b) {
+                corrector_body<decltype(b)::value, true>(n, np, nullptr, nullptr, aux, nout, step, seed_lo, seed_hi, pin, item % NBRICKS);
+            });
+        grid_barrier(bar, gridDim.x, target);
+    }
 }
 
 #ifdef SPIN_COL

@@ -19,6 +19,7 @@
 #define SPIN_MAX_BASIS 8
 #define SPIN_MAX_PAIR_ENTRIES 160
 #define SPIN_MAX_QUAD_ENTRIES 32
+#define SPIN_COOP_MAX_SPINS 4096      // largest lattice that takes the cooperative all-steps kernel by default
 
 namespace spin {
 
@@ -125,6 +126,7 @@ struct spin_system {
     double *d_result;              // reduction result (16 doubles)
     unsigned long long *d_step;    // device copy of the step counter (read by the kernels)
     unsigned char *d_pin;          // pinned-spin flags (boundary order), null if none
+    unsigned int *d_bar;           // arrival counter of the cooperative kernel's grid barrier
     double *d_vp;                  // velocity-projection state: ratio r, started flag, |F|^2
     bool vp_active;                // d_A holds the force of the previous VP iteration
     int vp_cur;                    // which of {d_A, d_fddi[1]} holds it
@@ -135,7 +137,7 @@ struct spin_system {
     bool has_device;               // false only in the planner-only mode used by the CPU tests
     std::string jit_note;          // why the specialised sweeps are not in use, if they are not
     // ---- execution options / bookkeeping
-    int opt_graph, opt_store_A, opt_jit, opt_tma, opt_ddi_slab, opt_col, opt_cache_noise;
+    int opt_graph, opt_store_A, opt_jit, opt_tma, opt_ddi_slab, opt_col, opt_cache_noise, opt_coop;
     cudaGraphExec_t graph_exec[2];   // one captured graph per ping-pong parity
     int graph_steps;
     int64_t n_launch, n_fft;
@@ -168,6 +170,9 @@ int jit_prepare(spin_system *s);
 void jit_release(spin_system *s);
 bool jit_ready(const spin_system *s);
 const char *jit_log(const spin_system *s);
+// all steps of an llg_iterate call in one cooperative launch (jit_steps_coop)
+bool jit_coop_ready(const spin_system *s);
+int jit_launch_steps_coop(spin_system *s, unsigned nsteps);
 // column-marching versions of the two sweeps (spin_jit_col.cuh)
 bool jit_col_ready(const spin_system *s);
 int jit_launch_predictor_col(spin_system *s, const double *n, const double *fddi, double *np, unsigned step_add);

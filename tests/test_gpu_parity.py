@@ -133,6 +133,8 @@ def test_split_invariance_and_graph_equivalence(P, O):
     b = P.SpinSystem.from_workload(w)
     c = P.SpinSystem.from_workload(w)
     c.spin_set_option("use_graph", 0)
+    for s_ in (a, b, c):
+        s_.spin_set_option("use_coop", 0)          # this test is about the two-launches-per-step path: graphs vs plain launches
     a.llg_iterate(57)
     b.llg_iterate(20); b.llg_iterate(17); b.llg_iterate(20)
     c.llg_iterate(57)
@@ -140,6 +142,12 @@ def test_split_invariance_and_graph_equivalence(P, O):
     assert np.array_equal(na, b.spins_get())
     assert np.array_equal(na, c.spins_get())
     assert a.llg_get_step() == b.llg_get_step() == c.llg_get_step() == 57
+    # the cooperative all-steps-in-one-launch kernel (default for small lattices): same bits, split-invariant, odd and even counts
+    d = P.SpinSystem.from_workload(w)
+    assert d.spin_kernel_info() == "jit+coop", d.spin_kernel_info()      # 960 spins: taken by default
+    d.llg_iterate(20); d.llg_iterate(17); d.llg_iterate(20)
+    assert np.array_equal(na, d.spins_get())
+    assert d.llg_get_step() == 57
 
 
 @pytest.mark.parametrize("cfg", [2, 4])
@@ -270,6 +278,7 @@ def test_tma_sweeps_match_oracle(P, O, cfg, cells, steps, geo, monkeypatch):
     w = W.CONFIGS[cfg]().resized(cells, steps)
     g, o = pair(P, O, w)
     g.spin_set_option("use_col", 0)
+    g.spin_set_option("use_coop", 0)
     g.spin_set_option("use_tma", 2)
     assert g.spin_kernel_info() == "jit+tma", g.spin_kernel_info()
     g.llg_iterate(steps); o.iterate(steps)
@@ -280,6 +289,7 @@ def test_tma_sweeps_match_oracle(P, O, cfg, cells, steps, geo, monkeypatch):
     b = P.SpinSystem.from_workload(w)
     b.spin_set_option("use_tma", 0)
     b.spin_set_option("use_col", 0)
+    b.spin_set_option("use_coop", 0)
     assert b.spin_kernel_info().startswith("jit (brick")
     b.llg_iterate(steps)
     assert np.array_equal(b.spins_get(), g.spins_get())
@@ -343,6 +353,7 @@ def test_column_marching_sweeps(P, O, cfg, cells, steps, geo, monkeypatch):
     w = W.CONFIGS[cfg]().resized(cells, steps)
     g, o = pair(P, O, w)
     g.spin_set_option("use_col", 1)
+    g.spin_set_option("use_coop", 0)
     assert g.spin_kernel_info() == "jit+col", g.spin_kernel_info()
     g.llg_iterate(steps); o.iterate(steps)
     d = np.abs(g.spins_get() - o.spins()).max()
@@ -350,6 +361,7 @@ def test_column_marching_sweeps(P, O, cfg, cells, steps, geo, monkeypatch):
     assert d <= SPIN_ATOL
     b = P.SpinSystem.from_workload(w)
     b.spin_set_option("use_col", 0)
+    b.spin_set_option("use_coop", 0)
     assert b.spin_kernel_info().startswith("jit (brick")
     b.llg_iterate(steps)
     assert np.array_equal(b.spins_get(), g.spins_get())
@@ -360,6 +372,7 @@ def test_column_marching_with_open_and_mixed_boundaries(P, O):
         w = dataclasses.replace(W.config3().resized((21, 10, 9), 30), periodic=per)
         g, o = pair(P, O, w)
         g.spin_set_option("use_col", 1)
+        g.spin_set_option("use_coop", 0)
         assert g.spin_kernel_info() == "jit+col"
         g.llg_iterate(30); o.iterate(30)
         assert np.abs(g.spins_get() - o.spins()).max() <= SPIN_ATOL
@@ -529,3 +542,26 @@ def test_limits_and_empty_interaction_lists(P, O):
     assert np.abs(Bg[idx] - Bo[idx]).max() <= FIELD_RTOL * np.abs(Bo).max()
     gb.llg_iterate(2); ob.iterate(2)
     assert np.abs(gb.spins_get()[idx] - ob.spins()[idx]).max() <= SPIN_ATOL
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# Cooperative all-steps kernel (jit_steps_coop): bit-identical to the two-launch path for every solver, with noise, pins, 2 sublattices
+@pytest.mark.parametrize("cfg,cells,steps", [(1, (32, 32, 1), 1000), (2, (45, 33, 1), 101), (3, (35, 9, 7), 100), (4, (33, 17, 1), 100), (2, (256, 256, 1), 64)])
+def test_cooperative_kernel_matches_two_launch_path(P, O, cfg, cells, steps):
+    w = W.CONFIGS[cfg]().resized(cells, steps)
+    mask = (np.random.default_rng(cfg).random(w.n_spins) < 0.1).astype(np.uint8)
+    for solver in (0, 1, 2):
+        a = P.SpinSystem.from_workload(w); b = P.SpinSystem.from_workload(w)
+        for s_ in (a, b):
+            s_.llg_set_solver(solver); s_.spins_set_pinned(mask if solver == 1 else None)
+        a.spin_set_option("use_coop", 2)
+        b.spin_set_option("use_coop", 0)
+        assert a.spin_kernel_info() == "jit+coop" and b.spin_kernel_info().startswith("jit (brick"), (a.spin_kernel_info(), b.spin_kernel_info())
+        a.llg_iterate(steps); b.llg_iterate(steps)
+        assert np.array_equal(a.spins_get(), b.spins_get()), solver
+    o = O.OracleSystem.from_workload(w)
+    g = P.SpinSystem.from_workload(w)
+    g.spin_set_option("use_coop", 2)
+    n_o = min(steps, 200)
+    g.llg_iterate(n_o); o.iterate(n_o)
+    assert np.abs(g.spins_get() - o.spins()).max() <= SPIN_ATOL
