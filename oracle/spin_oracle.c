@@ -17,6 +17,7 @@
  *   Heun solver       App. B, B3-B4 (:355-367)              -> orc_llg_step (solver 1); orc_heun_step = the same written on its own (pin)
  *   velocity projection App. D, D1-D5 (:438-463)            -> orc_vp_iterate
  *   topological charge App. A, A1-A2 (:317-343)             -> orc_topological_charge, orc_spherical_area
+ *   RK4 solver        :168 (named only; textbook tableau)   -> orc_llg_step (solver 3), orc_rk4_step
  *   SIB solver        App. C, C5-C11 (:384-436)             -> orc_llg_step (solver 2), imp_update (Cramer's rule as printed)
  * Readings of silent / garbled passages are listed in DESIGN.md ("Readings") under the
  * same R-numbers as SURVEY.md 8(c).
@@ -75,7 +76,7 @@ typedef struct orc_system {
     unsigned char *pinned;   /* N flags or NULL: a pinned spin keeps its value (":79 pinning of individual spins"); a vacancy
                                 (":79 defects, such as vacancies") is a pinned site holding the zero vector (reading R27)   */
     double *vp_v, *vp_F;     /* velocity-projection minimiser (App. D): velocity and force of the previous iteration, or NULL  */
-    int solver;              /* 0 Depondt (App. B B5-B7), 1 Heun (B3-B4), 2 SIB semi-implicit midpoint (App. C) */
+    int solver;              /* 0 Depondt (App. B B5-B7), 1 Heun (B3-B4), 2 SIB semi-implicit midpoint (App. C), 3 RK4 (:168) */
 } orc_system;
 
 /* ------------------------------------------------------------------ helpers */
@@ -771,7 +772,9 @@ static inline void imp_update(const double *A, double dt, const double *n, doubl
  *   Heun (B3-B4 with f = n x A): n^p = n + dt n x A; n <- n + dt/2 (n x A + n^p x A^p); renormalise every step.
  *   SIB (App. C, C5, C11): n^p from the implicit-midpoint structure with A(n); n <- the same structure with A evaluated at
  *        the midpoint configuration {(n_j + n_j^p)/2}; length is preserved by construction, no renormalisation.        */
+static void orc_rk4_step(orc_system *s);
 void orc_llg_step(orc_system *s) {
+    if (s->solver == 3) { orc_rk4_step(s); return; }
     long N = s->N; int nb = s->nb;
     double *F = (double *)malloc(3 * N * sizeof(double)), *A = (double *)malloc(3 * N * sizeof(double));
     double *np_ = (double *)malloc(3 * N * sizeof(double)), *sg = (double *)calloc(3 * N, sizeof(double));
@@ -822,6 +825,46 @@ void orc_llg_step(orc_system *s) {
     }
     s->step += 1;
     free(F); free(A); free(np_); free(sg); free(Fth);
+}
+/* Classical 4th-order Runge-Kutta on dn/dt = f(n) = n x A(n) (B1), "a 4th order Runge-Kutta solver" (:168; no formulas in the
+ * paper, so the textbook tableau): k1 = f(n), k2 = f(n + dt/2 k1), k3 = f(n + dt/2 k2), k4 = f(n + dt k3),
+ * n <- n + dt/6 (k1 + 2 k2 + 2 k3 + k4), renormalised every step ("all [Runge-Kutta methods] have this property", :367).
+ * The stage configurations are not renormalised; the thermal field of the step is the same in all four stages (R11).    */
+static void orc_rk4_step(orc_system *s) {
+    long N = s->N; int nb = s->nb;
+    double *F = (double *)malloc(3 * N * sizeof(double)), *y = (double *)malloc(3 * N * sizeof(double));
+    double *acc = (double *)calloc(3 * N, sizeof(double)), *sg = (double *)calloc(3 * N, sizeof(double)), *Fth = NULL;
+    if (s->T > 0.0) {
+        Fth = (double *)malloc(3 * N * sizeof(double));
+        for (long i = 0; i < N; ++i) {
+            double xi[3]; orc_thermal_xi(s->seed, s->step, (uint32_t)i, xi);
+            double sig = orc_thermal_sigma(s, (int)(i % nb));
+            for (int k = 0; k < 3; ++k) Fth[3*i+k] = sig * xi[k];
+        }
+    }
+    const double cnext[4] = { 0.5, 0.5, 1.0, 0.0 }, wacc[4] = { 1.0, 2.0, 2.0, 1.0 };
+    memcpy(y, s->n, 3 * N * sizeof(double));
+    for (int st = 0; st < 4; ++st) {
+        total_force(s, y, Fth, F);
+        if (s->u != 0.0) orc_stt_gradient(s, y, sg);
+        for (long i = 0; i < N; ++i) {
+            double A[3], k[3];
+            rot_field(s, (int)(i % nb), y + 3*i, F + 3*i, sg + 3*i, A);
+            cross3(y + 3*i, A, k);
+            for (int c = 0; c < 3; ++c) acc[3*i+c] += wacc[st] * k[c];
+            if (s->pinned && s->pinned[i]) continue;
+            if (st < 3) for (int c = 0; c < 3; ++c) y[3*i+c] = s->n[3*i+c] + cnext[st] * s->dt * k[c];
+        }
+    }
+    for (long i = 0; i < N; ++i) {
+        if (s->pinned && s->pinned[i]) continue;
+        double out[3];
+        for (int c = 0; c < 3; ++c) out[c] = s->n[3*i+c] + s->dt / 6.0 * acc[3*i+c];
+        double nrm = sqrt(dot3(out, out));
+        for (int c = 0; c < 3; ++c) s->n[3*i+c] = out[c] / nrm;
+    }
+    s->step += 1;
+    free(F); free(y); free(acc); free(sg); free(Fth);
 }
 void orc_llg_iterate(orc_system *s, long nsteps) { for (long k = 0; k < nsteps; ++k) orc_llg_step(s); }
 

@@ -83,7 +83,7 @@ def _larmor_error(dt_fs, alpha, method, t_ps=100.0, mu_s=2.0, B=1.0):
         if method == "heun_standalone":
             s.heun_step()
         else:
-            s.set_solver({"depondt": 0, "heun": 1, "sib": 2}[method]); s.iterate(1)
+            s.set_solver({"depondt": 0, "heun": 1, "sib": 2, "rk4": 3}[method]); s.iterate(1)
         t = (k + 1) * dt_fs * 1e-3
         nz = math.tanh(alpha * gp * B * t)
         ph = gp * B * t
@@ -139,7 +139,17 @@ def test_solvers_heun_and_sib_closed_forms():
     assert abs(np.linalg.norm(s.spins()[0]) - 1.5) < 1e-14
 
 
-@pytest.mark.parametrize("solver", [1, 2])
+def test_solver_rk4_is_fourth_order():
+    """"A 4th order Runge-Kutta solver": on the damped Larmor problem of Eq. 12 the error falls by 2^4 when the step
+    is halved, and at dt = 10 fs it is orders below Heun's 1e-6 and Depondt's 3e-7 (:166)."""
+    e1, dev = _larmor_error(40.0, 0.1, "rk4", t_ps=20.0)
+    e2, _ = _larmor_error(20.0, 0.1, "rk4", t_ps=20.0)
+    assert e1 / e2 == pytest.approx(16.0, rel=0.15), (e1, e2)
+    e10, _ = _larmor_error(10.0, 0.1, "rk4", t_ps=20.0)
+    assert e10 < 1e-10 and dev < 5e-16, (e10, dev)
+
+
+@pytest.mark.parametrize("solver", [1, 2, 3])
 def test_solvers_energy_decreases_and_split_invariance(solver):
     """alpha > 0, T = 0: the energy must not increase (Heun, SIB); with noise, iterate(a) + iterate(b) == iterate(a+b)."""
     w = small(3, (6, 6, 6))
