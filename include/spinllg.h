@@ -119,8 +119,9 @@ int llg_configure(spin_system *sys, double dt_fs, double alpha, double T_kelvin,
  *   SPIN_SOLVER_HEUN     App. B, B3-B4 (:355-367): n + dt/2 (n x A + n^p x A^p), renormalised every step
  *   SPIN_SOLVER_SIB      App. C, C5-C11 (:384-436): semi-implicit midpoint; field of the corrector at {(n_j + n_j^p)/2};
  *                        preserves |n_i| by construction (no renormalisation)
- * Heun and SIB run in the run-time specialised kernels only (SPIN_ERR_STATE from llg_iterate if those are unavailable). */
-enum { SPIN_SOLVER_DEPONDT = 0, SPIN_SOLVER_HEUN = 1, SPIN_SOLVER_SIB = 2 };
+ *   SPIN_SOLVER_RK4      classical 4th-order Runge-Kutta (:168, named only): four field sweeps per step, renormalised every step
+ * Heun, SIB and RK4 run in the run-time specialised kernels only (SPIN_ERR_STATE from llg_iterate if those are unavailable). */
+enum { SPIN_SOLVER_DEPONDT = 0, SPIN_SOLVER_HEUN = 1, SPIN_SOLVER_SIB = 2, SPIN_SOLVER_RK4 = 3 };
 int llg_set_solver(spin_system *sys, int solver);
 /* advance n_steps steps of the selected solver (Depondt unless llg_set_solver chose another); asynchronous on the system's stream.  The step counter persists, so
  * llg_iterate(a); llg_iterate(b) reproduces llg_iterate(a+b) exactly.                                       */

@@ -30,7 +30,7 @@ struct TmaGeo {
 
 struct JitState {
     cudaLibrary_t lib;
-    cudaKernel_t k_pred, k_corr;
+    cudaKernel_t k_pred, k_corr, k_rk4;
     bool loaded;
     std::string source, log;
     // TMA-fed plane-marching sweeps
@@ -204,7 +204,7 @@ std::string spin::jit_source(const spin_system *s) {
       << ", PER_C = " << (P.perC ? "true" : "false") << ";\n";
     o << "constexpr bool CACHE_NOISE = " << ((s->opt_cache_noise && P.thermal_on && !(s->opt_store_A && s->solver == 0)) ? "true" : "false") << ";\n";
     o << "constexpr bool HAS_PIN = " << (s->d_pin ? "true" : "false") << ";\n";
-    o << "constexpr int SOLVER = " << s->solver << ";      // 0 Depondt, 1 Heun, 2 SIB\n";
+    o << "constexpr int SOLVER = " << s->solver << ";      // 0 Depondt, 1 Heun, 2 SIB, 3 RK4 (own stage kernel)\n";
     o << "constexpr bool STORE_A = " << ((s->opt_store_A && s->solver == 0) ? "true" : "false") << ", HAS_DDI = " << (P.has_ddi ? "true" : "false")
       << ", THERMAL_ON = " << (P.thermal_on ? "true" : "false") << ", STT_ON = " << (P.stt_on ? "true" : "false") << ";\n";
     const int np = P.pair_begin[P.nb], nq = P.quad_begin[P.nb];
@@ -391,10 +391,11 @@ int spin::jit_prepare(spin_system *s) {
     j->loaded = true;
     e = cudaLibraryGetKernel(&j->k_pred, j->lib, "jit_predictor");
     if (e == cudaSuccess) e = cudaLibraryGetKernel(&j->k_corr, j->lib, "jit_corrector");
+    if (e == cudaSuccess) e = cudaLibraryGetKernel(&j->k_rk4, j->lib, "jit_rk4_stage");
     if (e != cudaSuccess) return spin::fail(SPIN_ERR_CUDA, "cudaLibraryGetKernel failed: %s", cudaGetErrorString(e));
     tma_prepare(s, j);
     j->coop = false;
-    if (s->opt_coop && !s->ddi_on) {
+    if (s->opt_coop && !s->ddi_on && s->solver != SPIN_SOLVER_RK4) {
         int dev = 0, can = 0, occ = 0;
         cudaGetDevice(&dev);
         cudaDeviceGetAttribute(&can, cudaDevAttrCooperativeLaunch, dev);
@@ -441,6 +442,19 @@ int spin::jit_launch_corrector(spin_system *s, dim3 grid, dim3 block, const doub
                     (void *)&seed_lo, (void *)&seed_hi, (void *)&pin};
     jit_brick_launch(s, grid, block);
     SPIN_CUDA(cudaLaunchKernel((const void *)s->jit->k_corr, grid, block, args, 0, s->stream));
+    return SPIN_OK;
+}
+
+int spin::jit_launch_rk4_stage(spin_system *s, const double *base, const double *y, double *ynext, double *acc, double *noise,
+                                const double *fddi, int stage, unsigned step_add) {
+    unsigned seed_lo = s->plan.seed_lo, seed_hi = s->plan.seed_hi;
+    const unsigned long long *d_step = s->d_step;
+    const unsigned char *pin = s->d_pin;
+    void *args[] = {(void *)&base, (void *)&y, (void *)&ynext, (void *)&acc, (void *)&noise, (void *)&fddi, (void *)&stage, (void *)&d_step,
+                    (void *)&step_add, (void *)&seed_lo, (void *)&seed_hi, (void *)&pin};
+    dim3 grid, block;
+    jit_brick_launch(s, grid, block);
+    SPIN_CUDA(cudaLaunchKernel((const void *)s->jit->k_rk4, grid, block, args, 0, s->stream));
     return SPIN_OK;
 }
 

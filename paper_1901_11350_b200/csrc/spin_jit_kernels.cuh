@@ -336,6 +336,51 @@ __device__ __forceinline__ void corrector_body(const double *__restrict__ n, con
     store_spin(nout + idx, c, out);
 }
 
+// One stage of the classical 4th-order Runge-Kutta solver on dn/dt = f(n) = n x A(n):
+//   k = f(y);  stage 0: acc = k, y' = n + dt/2 k;  1: acc += 2k, y' = n + dt/2 k;  2: acc += 2k, y' = n + dt k;
+//   stage 3: n(t+dt) = n + dt/6 (acc + k), renormalised.  Stage configurations are not renormalised; one thermal field per step.
+template <int B>
+__device__ __forceinline__ void rk4_stage_body(const double *__restrict__ base, const double *__restrict__ y, double *__restrict__ ynext,
+                                               double *__restrict__ acc, double *__restrict__ noise, const double *__restrict__ fddi, int stage,
+                                               u64 step, u32 seed_lo, u32 seed_hi, const unsigned char *__restrict__ pin, int brick) {
+    Coord c;
+    int idx;
+    if (!locate<B>(c, idx, brick)) return;
+    double n0[3];
+    load3<0>(base + idx, n0);
+    if (is_pinned<B>(pin, c)) { store_spin(ynext + idx, c, n0); return; }
+    GlobalAcc<1> cfg;
+    cfg.cfg[0] = y + idx;
+    double own[1][3], F[1][3], sg[1][3] = {{0.0, 0.0, 0.0}};
+    load3<0>(cfg.cfg[0], own[0]);
+    if constexpr (spec::THERMAL_ON && !spec::HAS_DDI) {      // generated once per step, kept for the other three stages
+        if (stage == 0) { thermal_force<B>(c, step, seed_lo, seed_hi, F[0]); store3(noise + idx, F[0]); }
+        else load3<0>(noise + idx, F[0]);
+    } else {
+        thermal_force<B>(c, step, seed_lo, seed_hi, F[0]);
+    }
+    force<B, 1>(cfg, own, F);
+    if constexpr (spec::HAS_DDI) { double d[3]; load3<0>(fddi + idx, d); F[0][0] += d[0]; F[0][1] += d[1]; F[0][2] += d[2]; }
+    if constexpr (spec::STT_ON) stt_gradient<B, 1>(cfg, c, own, sg);
+    double A[3], k[3] = {0.0, 0.0, 0.0};
+    rotation_field<B>(own[0], F[0], sg[0], A);
+    spin::heun_add(own[0], A, 1.0, k);                      // k = y x A
+    double a[3] = {0.0, 0.0, 0.0};
+    if (stage > 0) load3<0>(acc + idx, a);
+    double out[3];
+    if (stage < 3) {
+        const double w = stage == 0 ? 1.0 : 2.0, h = stage == 2 ? specc::DT : specc::HDT;
+        a[0] = fma(w, k[0], a[0]); a[1] = fma(w, k[1], a[1]); a[2] = fma(w, k[2], a[2]);
+        store3(acc + idx, a);
+        out[0] = fma(h, k[0], n0[0]); out[1] = fma(h, k[1], n0[1]); out[2] = fma(h, k[2], n0[2]);
+    } else {
+        const double h = specc::DT / 6.0;
+        out[0] = fma(h, a[0] + k[0], n0[0]); out[1] = fma(h, a[1] + k[1], n0[1]); out[2] = fma(h, a[2] + k[2], n0[2]);
+        spin::renormalise_general(out);
+    }
+    store_spin(ynext + idx, c, out);
+}
+
 template <int B, class Fn>
 __device__ __forceinline__ void dispatch_basis(int b, Fn &&fn) {
     if constexpr (B < spec::NBASIS) {
@@ -364,6 +409,16 @@ extern "C" __global__ void SPIN_BOUNDS(spec::BX *spec::BY *spec::BZ)
     const unsigned long long step = *d_step + step_add;
     spinjit::dispatch_basis<0>((int)blockIdx.y, [&](auto b) {
         spinjit::corrector_body<decltype(b)::value>(n, np, fddi_n, fddi_np, Ain, nout, step, seed_lo, seed_hi, pin, (int)blockIdx.x);
+    });
+}
+
+extern "C" __global__ void SPIN_BOUNDS(spec::BX *spec::BY *spec::BZ)
+    jit_rk4_stage(const double *__restrict__ base, const double *__restrict__ y, double *__restrict__ ynext, double *__restrict__ acc,
+                  double *__restrict__ noise, const double *__restrict__ fddi, int stage, const unsigned long long *__restrict__ d_step,
+                  unsigned int step_add, unsigned int seed_lo, unsigned int seed_hi, const unsigned char *__restrict__ pin) {
+    const unsigned long long step = *d_step + step_add;
+    spinjit::dispatch_basis<0>((int)blockIdx.y, [&](auto b) {
+        spinjit::rk4_stage_body<decltype(b)::value>(base, y, ynext, acc, noise, fddi, stage, step, seed_lo, seed_hi, pin, (int)blockIdx.x);
     });
 }
 

@@ -170,6 +170,9 @@ int jit_prepare(spin_system *s);
 void jit_release(spin_system *s);
 bool jit_ready(const spin_system *s);
 const char *jit_log(const spin_system *s);
+// one stage of the RK4 solver (jit_rk4_stage)
+int jit_launch_rk4_stage(spin_system *s, const double *base, const double *y, double *ynext, double *acc, double *noise, const double *fddi,
+                         int stage, unsigned step_add);
 // all steps of an llg_iterate call in one cooperative launch (jit_steps_coop)
 bool jit_coop_ready(const spin_system *s);
 int jit_launch_steps_coop(spin_system *s, unsigned nsteps);

@@ -379,8 +379,8 @@ def test_column_marching_with_open_and_mixed_boundaries(P, O):
 
 
 # ---------------------------------------------------------------------------------------------------------------------
-# Other solvers on the same two field sweeps: Heun (App. B B3-B4) and SIB (App. C C5-C11)
-@pytest.mark.parametrize("solver", [1, 2])
+# Other solvers on the same field sweeps: Heun (App. B B3-B4), SIB (App. C C5-C11), RK4 (:168; solver 3)
+@pytest.mark.parametrize("solver", [1, 2, 3])
 @pytest.mark.parametrize("cfg,steps", [(1, 300), (2, 200), (3, 150), (4, 150), (5, 30)])
 def test_heun_and_sib_trajectory_parity(P, O, cfg, steps, solver):
     w = W.CONFIGS[cfg]().resized(REPLICAS[cfg], steps)
@@ -459,7 +459,7 @@ def test_pinned_spins_and_vacancies(P, O, cfg, steps, use_jit):
     assert np.abs(ng - o.spins()).max() <= SPIN_ATOL
     assert np.abs(ng[mask == 0] - n0[mask == 0]).max() > 1e-3     # the others do
     if use_jit:
-        for solver in (1, 2):
+        for solver in (1, 2, 3):
             g.spins_set(n0); o.set_spins(n0)
             g.llg_set_solver(solver); o.set_solver(solver)
             g.llg_iterate(30); o.iterate(30)
