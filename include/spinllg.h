@@ -169,12 +169,14 @@ int spin_set_option(spin_system *sys, const char *name, int value);
  * cfg3, hence off by default.
  * use_col (default 0): 1 runs them as column-marching kernels (one thread per lattice column, own spin at z-1, z, z+1 kept in
  * registers; 3-D lattices).  Also measured slower than the brick kernels.
+ * use_fused (default 0): 1 runs the Depondt step in one pass (predictor for tile + rim into shared memory, corrector from it; 48 B
+ * per spin-update of HBM traffic; lattices of at least 16384 spins, 2 forces it).  Measured slower than the brick kernels on cfg3.
  * use_coop (default 1): lattices of up to 4096 spins without dipolar coupling run ALL steps of an llg_iterate call in one
  * cooperative launch (grid barrier between the sweeps) instead of two launches per step; 2 forces it for any size (slower
  * beyond about 10^4 spins), 0 switches it off.
  * cache_noise (default 1): the predictor keeps the thermal field of the step (24 B/spin) for the corrector instead of generating it twice.
  * ddi_slab (default 1): thin films with one basis atom take the dipolar slab path (2-D cuFFT + fused transform along c).
- * spin_kernel_info writes "jit+coop", "jit+col", "jit+tma", "jit (brick kernels: <why>)" or "generic: <why>" into buf: which sweep kernels are in use.  */
+ * spin_kernel_info writes "jit+fused", "jit+coop", "jit+col", "jit+tma", "jit (brick kernels: <why>)" or "generic: <why>" into buf: which sweep kernels are in use.  */
 int spin_kernel_info(spin_system *sys, char *buf, int len);
 /* the generated translation unit of the specialised sweeps (buf may be NULL); compile != 0 also compiles it for sm_100a
  * (needs no device) and returns the cubin size.  Host-side planner check; works in planner-only mode

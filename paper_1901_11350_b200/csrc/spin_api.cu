@@ -374,6 +374,15 @@ int enqueue_step_t(spin_system *s, const Launch &L, unsigned step_add) {
         return SPIN_OK;
     }
     const bool prof = s->profile_on != 0;
+    if (jit_fused_ready(s)) {          // one pass: predictor into shared memory, corrector from it
+        if (prof) cudaEventRecord(s->ev0, s->stream);
+        int rc = jit_launch_fused(s, n, nout, step_add);
+        if (rc) return rc;
+        s->n_launch++;
+        if (prof) { cudaEventRecord(s->ev1, s->stream); cudaEventSynchronize(s->ev1); float ms; cudaEventElapsedTime(&ms, s->ev0, s->ev1); s->prof_ms[1] += ms; s->prof_n[1]++; }
+        s->cur ^= 1;
+        return SPIN_OK;
+    }
     if (s->ddi_on) {
         if (prof) cudaEventRecord(s->ev0, s->stream);
         int rc = ddi_field(s, n, s->d_fddi[0]);
@@ -464,7 +473,7 @@ extern "C" int spin_geometry_create(const double bravais[9], int n_basis, const 
     if (!has_device) cudaGetLastError();
     spin_system *s = new spin_system();
     s->has_device = has_device;
-    s->jit = nullptr; s->opt_jit = 1; s->opt_tma = 0; s->opt_ddi_slab = 1; s->opt_col = 0; s->opt_cache_noise = 1; s->opt_coop = 1; s->d_bar = nullptr;
+    s->jit = nullptr; s->opt_jit = 1; s->opt_tma = 0; s->opt_ddi_slab = 1; s->opt_col = 0; s->opt_cache_noise = 1; s->opt_coop = 1; s->opt_fused = 0; s->d_bar = nullptr;
     memcpy(s->brav, bravais, sizeof(s->brav));
     s->nb = n_basis;
     s->basis.assign(basis_frac, basis_frac + 3 * n_basis);
@@ -779,7 +788,8 @@ extern "C" int llg_iterate(spin_system *s, int64_t n_steps) {
     // (a grid barrier costs about as much as a launch inside a CUDA graph, and it empties L1), so the limit is low; option
     // use_coop = 2 forces it for any lattice without dipolar coupling.
     const int64_t COOP_CHUNK = 8192;
-    if (s->opt_coop && !s->profile_on && !s->ddi_on && (s->N <= SPIN_COOP_MAX_SPINS || s->opt_coop == 2) && jit_coop_ready(s) && n_steps > 0) {
+    if (s->opt_coop && !s->profile_on && !s->ddi_on && (s->N <= SPIN_COOP_MAX_SPINS || s->opt_coop == 2) && jit_coop_ready(s) && !jit_fused_ready(s) &&
+        n_steps > 0) {
         while (done < n_steps) {
             const unsigned chunk = (unsigned)std::min<int64_t>(COOP_CHUNK, n_steps - done);
             rc = jit_launch_steps_coop(s, chunk);
@@ -816,7 +826,7 @@ extern "C" int llg_iterate(spin_system *s, int64_t n_steps) {
         }
         while (n_steps - done >= G) {
             SPIN_CUDA(cudaGraphLaunch(gexec, s->stream));
-            s->n_launch += (s->solver == SPIN_SOLVER_RK4 ? 4 : 2) * G + 1;
+            s->n_launch += (s->solver == SPIN_SOLVER_RK4 ? 4 : (jit_fused_ready(s) ? 1 : 2)) * G + 1;
             done += G;
         }
     }
@@ -971,6 +981,7 @@ extern "C" int spin_set_option(spin_system *s, const char *name, int value) {
     if (!strcmp(name, "use_graph")) s->opt_graph = value ? 1 : 0;
     else if (!strcmp(name, "store_A")) { s->opt_store_A = value ? 1 : 0; s->plan_dirty = true; }
     else if (!strcmp(name, "use_jit")) { s->opt_jit = value ? 1 : 0; s->plan_dirty = true; }
+    else if (!strcmp(name, "use_fused")) { s->opt_fused = value < 0 ? 0 : (value > 2 ? 2 : value); s->plan_dirty = true; }
     else if (!strcmp(name, "use_coop")) { s->opt_coop = value < 0 ? 0 : (value > 2 ? 2 : value); s->plan_dirty = true; }
     else if (!strcmp(name, "cache_noise")) { s->opt_cache_noise = value ? 1 : 0; s->plan_dirty = true; }
     else if (!strcmp(name, "use_col")) { s->opt_col = value ? 1 : 0; s->plan_dirty = true; }
@@ -985,7 +996,8 @@ extern "C" int spin_set_option(spin_system *s, const char *name, int value) {
 extern "C" int spin_kernel_info(spin_system *s, char *buf, int len) {
     REQUIRE(s && buf && len > 0, "bad argument");
     if (s->has_device) { int rc = ensure_plan(s); if (rc) return rc; }
-    if (jit_coop_ready(s) && s->opt_coop && !s->ddi_on && (s->N <= SPIN_COOP_MAX_SPINS || s->opt_coop == 2)) snprintf(buf, (size_t)len, "jit+coop");
+    if (jit_fused_ready(s)) snprintf(buf, (size_t)len, "jit+fused");
+    else if (jit_coop_ready(s) && s->opt_coop && !s->ddi_on && (s->N <= SPIN_COOP_MAX_SPINS || s->opt_coop == 2)) snprintf(buf, (size_t)len, "jit+coop");
     else if (jit_col_ready(s)) snprintf(buf, (size_t)len, "jit+col");
     else if (jit_tma_ready(s)) snprintf(buf, (size_t)len, "jit+tma");
     else if (jit_ready(s)) snprintf(buf, (size_t)len, "jit (brick kernels: %s)", jit_tma_note(s));

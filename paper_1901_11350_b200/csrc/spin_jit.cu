@@ -38,6 +38,11 @@ struct JitState {
     std::string tma_note;     // why not, if not
     TmaGeo gp, gc;
     cudaKernel_t k_pred_tma, k_corr_tma;
+    // one-pass Depondt step (spin_jit_fused.cuh)
+    bool fused;
+    cudaKernel_t k_fused;
+    int fused_geo[4];         // FTX, FTY, FTZ, FNT
+    size_t fused_smem;
     // all steps in one cooperative launch (launch-bound lattices)
     bool coop;
     cudaKernel_t k_coop;
@@ -155,6 +160,29 @@ static void jit_brick_launch(const spin_system *s, dim3 &grid, dim3 &block) {
     jit_brick(s, b);
     grid = dim3((unsigned)(((s->nc[0] + b[0] - 1) / b[0]) * ((s->nc[1] + b[1] - 1) / b[1]) * ((s->nc[2] + b[2] - 1) / b[2])), (unsigned)s->nb, 1);
     block = dim3((unsigned)(b[0] * b[1] * b[2]), 1, 1);
+}
+
+// one-pass Depondt step (spin_jit_fused.cuh): tile and threads per block, shared-memory bytes; false if not applicable.
+// SPINLLG_FUSED="ftx,fty,ftz,threads" overrides the defaults (32 x 8 x 8 cells, 512 threads; flat lattices 32 x 16 x 1).
+static bool plan_fused(const spin_system *s, int g[4], size_t &smem) {
+    const DevicePlan &P = s->plan;
+    if (!s->opt_fused || s->solver != 0 || s->ddi_on || s->opt_store_A) return false;
+    if (s->opt_fused < 2 && s->N < 16384) return false;
+    const bool flat = P.Nc < 2;
+    int v[4] = {32, flat ? 16 : 8, flat ? 1 : 8, 512};
+    if (const char *e = getenv("SPINLLG_FUSED")) {
+        int u[4] = {0, 0, 0, 0};
+        sscanf(e, "%d,%d,%d,%d", &u[0], &u[1], &u[2], &u[3]);
+        for (int k = 0; k < 4; ++k) if (u[k] > 0) v[k] = u[k];
+    }
+    if (v[2] > P.Nc) v[2] = P.Nc;
+    if (v[3] % 32 || v[3] > 1024) return false;
+    const size_t np = (size_t)3 * (v[0] + 2 * P.rA) * (v[1] + 2 * P.rB) * (v[2] + 2 * P.rC) * P.nb;
+    const size_t a = (size_t)3 * v[0] * v[1] * v[2] * P.nb;
+    smem = (np + a * (P.thermal_on ? 2 : 1)) * sizeof(double);
+    if (smem > 220 * 1024) return false;
+    for (int k = 0; k < 4; ++k) g[k] = v[k];
+    return true;
 }
 
 // column-marching sweeps (spin_jit_col.cuh): tile of columns per block, planes per chunk, chunks; false if not applicable.
@@ -278,6 +306,10 @@ std::string spin::jit_source(const spin_system *s) {
     const bool tma = plan_tma(s, gp, gc, why);
     if (tma) { emit_tma_geo(o, "TmaP", gp); emit_tma_geo(o, "TmaC", gc); }
     o << "}  // namespace spec\n";
+    int fg[4];
+    size_t fsmem = 0;
+    if (plan_fused(s, fg, fsmem))
+        o << "namespace spec { constexpr int FTX = " << fg[0] << ", FTY = " << fg[1] << ", FTZ = " << fg[2] << ", FNT = " << fg[3] << "; }\n#define SPIN_FUSED 1\n";
     int cg[4];
     const bool col = plan_col(s, cg);
     if (col) o << "namespace spec { constexpr int CBX = " << cg[0] << ", CBY = " << cg[1] << ", CCZ = " << cg[2] << ", CNZC = " << cg[3] << "; }\n#define SPIN_COL 1\n";
@@ -381,6 +413,7 @@ int spin::jit_prepare(spin_system *s) {
     j->tma = false;
     j->col = false;
     j->coop = false;
+    j->fused = false;
     j->source = src;
     s->jit = j;
     std::string cubin;
@@ -394,6 +427,12 @@ int spin::jit_prepare(spin_system *s) {
     if (e == cudaSuccess) e = cudaLibraryGetKernel(&j->k_rk4, j->lib, "jit_rk4_stage");
     if (e != cudaSuccess) return spin::fail(SPIN_ERR_CUDA, "cudaLibraryGetKernel failed: %s", cudaGetErrorString(e));
     tma_prepare(s, j);
+    j->fused = plan_fused(s, j->fused_geo, j->fused_smem);
+    if (j->fused) {
+        cudaError_t fe = cudaLibraryGetKernel(&j->k_fused, j->lib, "jit_depondt_fused");
+        if (fe == cudaSuccess) fe = cudaFuncSetAttribute((const void *)j->k_fused, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)j->fused_smem);
+        if (fe != cudaSuccess) { cudaGetLastError(); j->fused = false; }
+    }
     j->coop = false;
     if (s->opt_coop && !s->ddi_on && s->solver != SPIN_SOLVER_RK4) {
         int dev = 0, can = 0, occ = 0;
@@ -455,6 +494,20 @@ int spin::jit_launch_rk4_stage(spin_system *s, const double *base, const double 
     dim3 grid, block;
     jit_brick_launch(s, grid, block);
     SPIN_CUDA(cudaLaunchKernel((const void *)s->jit->k_rk4, grid, block, args, 0, s->stream));
+    return SPIN_OK;
+}
+
+bool spin::jit_fused_ready(const spin_system *s) { return s->jit && s->jit->loaded && s->jit->fused; }
+
+int spin::jit_launch_fused(spin_system *s, const double *n, double *nout, unsigned step_add) {
+    JitState *j = s->jit;
+    unsigned seed_lo = s->plan.seed_lo, seed_hi = s->plan.seed_hi;
+    const unsigned long long *d_step = s->d_step;
+    const unsigned char *pin = s->d_pin;
+    void *args[] = {(void *)&n, (void *)&nout, (void *)&d_step, (void *)&step_add, (void *)&seed_lo, (void *)&seed_hi, (void *)&pin};
+    const int *g = j->fused_geo;
+    const unsigned tiles = (unsigned)(((s->nc[0] + g[0] - 1) / g[0]) * ((s->nc[1] + g[1] - 1) / g[1]) * ((s->nc[2] + g[2] - 1) / g[2]));
+    SPIN_CUDA(cudaLaunchKernel((const void *)j->k_fused, dim3(tiles), dim3((unsigned)g[3]), args, j->fused_smem, s->stream));
     return SPIN_OK;
 }
 

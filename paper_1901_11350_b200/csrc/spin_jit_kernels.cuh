@@ -471,6 +471,9 @@ extern "C" __global__ void SPIN_BOUNDS(spec::BX *spec::BY *spec::BZ)
     }
 }
 
+#ifdef SPIN_FUSED
+#include "spin_jit_fused.cuh"
+#endif
 #ifdef SPIN_COL
 #include "spin_jit_col.cuh"
 #endif

@@ -137,7 +137,7 @@ struct spin_system {
     bool has_device;               // false only in the planner-only mode used by the CPU tests
     std::string jit_note;          // why the specialised sweeps are not in use, if they are not
     // ---- execution options / bookkeeping
-    int opt_graph, opt_store_A, opt_jit, opt_tma, opt_ddi_slab, opt_col, opt_cache_noise, opt_coop;
+    int opt_graph, opt_store_A, opt_jit, opt_tma, opt_ddi_slab, opt_col, opt_cache_noise, opt_coop, opt_fused;
     cudaGraphExec_t graph_exec[2];   // one captured graph per ping-pong parity
     int graph_steps;
     int64_t n_launch, n_fft;
@@ -170,6 +170,9 @@ int jit_prepare(spin_system *s);
 void jit_release(spin_system *s);
 bool jit_ready(const spin_system *s);
 const char *jit_log(const spin_system *s);
+// one-pass Depondt step (jit_depondt_fused)
+bool jit_fused_ready(const spin_system *s);
+int jit_launch_fused(spin_system *s, const double *n, double *nout, unsigned step_add);
 // one stage of the RK4 solver (jit_rk4_stage)
 int jit_launch_rk4_stage(spin_system *s, const double *base, const double *y, double *ynext, double *acc, double *noise, const double *fddi,
                          int stage, unsigned step_add);

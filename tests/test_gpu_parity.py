@@ -565,3 +565,40 @@ def test_cooperative_kernel_matches_two_launch_path(P, O, cfg, cells, steps):
     n_o = min(steps, 200)
     g.llg_iterate(n_o); o.iterate(n_o)
     assert np.abs(g.spins_get() - o.spins()).max() <= SPIN_ATOL
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# One-pass Depondt step (csrc/spin_jit_fused.cuh): predictor for tile + rim into shared memory, corrector from it
+FUSED_CASES = [
+    (1, (37, 19, 1), 100, None, (1, 1, 0)),
+    (2, (45, 33, 1), 100, None, (1, 1, 0)),          # reach 2, thermal field kept in shared memory
+    (3, (35, 9, 7), 100, None, (1, 1, 1)),
+    (3, (70, 37, 45), 20, "32,8,8,512", (1, 1, 1)),
+    (3, (70, 37, 45), 20, "16,4,4,256", (0, 1, 0)),  # small tiles, open and periodic edges mixed
+    (3, (33, 5, 40), 20, "32,4,16,1024", (1, 0, 1)),
+    (4, (33, 17, 1), 100, None, (1, 1, 0)),          # two sublattices, quadruplets, current
+    (4, (33, 17, 1), 50, "32,8,1,256", (0, 0, 0)),
+    (3, (2, 2, 2), 30, None, (1, 1, 1)),             # the rim wraps onto the tile itself
+]
+
+
+@pytest.mark.parametrize("cfg,cells,steps,geo,per", FUSED_CASES)
+def test_one_pass_step_matches_two_sweep_kernels(P, O, cfg, cells, steps, geo, per, monkeypatch):
+    if geo:
+        monkeypatch.setenv("SPINLLG_FUSED", geo)
+    w = dataclasses.replace(W.CONFIGS[cfg]().resized(cells, steps), periodic=per)
+    mask = (np.random.default_rng(7).random(w.n_spins) < 0.05).astype(np.uint8)
+    g, o = pair(P, O, w)
+    g.spin_set_option("use_fused", 2)
+    g.spins_set_pinned(mask); o.set_pinned(mask)
+    assert g.spin_kernel_info() == "jit+fused", g.spin_kernel_info()
+    g.llg_iterate(steps); o.iterate(steps)
+    d = np.abs(g.spins_get() - o.spins()).max()
+    print(f"fused cfg{cfg} {cells} steps={steps}: max|dn| = {d:.3e}")
+    assert d <= SPIN_ATOL
+    b = P.SpinSystem.from_workload(w)
+    b.spin_set_option("use_coop", 0)
+    b.spins_set_pinned(mask)
+    assert b.spin_kernel_info().startswith("jit (brick")
+    b.llg_iterate(steps)
+    assert np.array_equal(b.spins_get(), g.spins_get())          # same arithmetic, bit for bit
