@@ -50,8 +50,10 @@ __constant__ double ROD_S[9] = {1.0, -1.0 / 6.0, 1.0 / 120.0, -1.0 / 5040.0, 1.0
 __constant__ double ROD_Q[9] = {0.5, -1.0 / 24.0, 1.0 / 720.0, -1.0 / 40320.0, 1.0 / 3628800.0, -1.0 / 479001600.0, 1.0 / 87178291200.0,
                                 -1.0 / 20922789888000.0, 1.0 / 6402373705728000.0};                     // (-1)^k / (2k+2)!
 __device__ __forceinline__ void rodrigues(const double (&A)[3], double dt, double dt2, const double (&n)[3], double (&out)[3]) {
-    const double a2 = A[0] * A[0] + A[1] * A[1] + A[2] * A[2];
-    const double x = a2 * dt2;
+    // every product and sum below is written out (fma / __dmul_rn): the compiler has no freedom to contract differently in different
+    // kernels, so all sweep variants give the same bits
+    const double a2 = fma(A[0], A[0], fma(A[1], A[1], __dmul_rn(A[2], A[2])));
+    const double x = __dmul_rn(a2, dt2);
     double s, q;
     if (x < 0x1p-10) {
         s = fma(fma(fma(fma(ROD_S[4], x, ROD_S[3]), x, ROD_S[2]), x, ROD_S[1]), x, ROD_S[0]);
@@ -68,35 +70,37 @@ __device__ __forceinline__ void rodrigues(const double (&A)[3], double dt, doubl
         q = (1.0 - cs) / x;
     }
     const double c = fma(-x, q, 1.0);
-    const double ds = dt * s, an = (A[0] * n[0] + A[1] * n[1] + A[2] * n[2]) * dt2 * q;
-    const double cx = A[1] * n[2] - A[2] * n[1], cy = A[2] * n[0] - A[0] * n[2], cz = A[0] * n[1] - A[1] * n[0];
-    out[0] = n[0] * c - cx * ds + A[0] * an;
-    out[1] = n[1] * c - cy * ds + A[1] * an;
-    out[2] = n[2] * c - cz * ds + A[2] * an;
+    const double ds = __dmul_rn(dt, s);
+    const double an = __dmul_rn(__dmul_rn(fma(A[0], n[0], fma(A[1], n[1], __dmul_rn(A[2], n[2]))), dt2), q);
+    const double cx = fma(A[1], n[2], -__dmul_rn(A[2], n[1])), cy = fma(A[2], n[0], -__dmul_rn(A[0], n[2])), cz = fma(A[0], n[1], -__dmul_rn(A[1], n[0]));
+    out[0] = fma(A[0], an, fma(-cx, ds, __dmul_rn(n[0], c)));
+    out[1] = fma(A[1], an, fma(-cy, ds, __dmul_rn(n[1], c)));
+    out[2] = fma(A[2], an, fma(-cz, ds, __dmul_rn(n[2], c)));
 }
 
 // Implicit-midpoint structure of the SIB solver (App. C, C5-C10): x + A' x x = n + n x A' with A' = (dt/2) A.
 // The paper solves the 3x3 system by Cramer's rule; its closed form is x = [a + A'(a.A') - A' x a] / (1 + |A'|^2), a = n + n x A'
 // (dot the equation with A' for x.A' = a.A', cross it with A' and eliminate A' x x).  |x| = |n| exactly (Cayley transform).
 __device__ __forceinline__ void imp_update(const double (&A)[3], double hdt, const double (&n)[3], double (&out)[3]) {
-    const double Ah[3] = {hdt * A[0], hdt * A[1], hdt * A[2]};
-    const double a[3] = {n[0] + (n[1] * Ah[2] - n[2] * Ah[1]), n[1] + (n[2] * Ah[0] - n[0] * Ah[2]), n[2] + (n[0] * Ah[1] - n[1] * Ah[0])};
-    const double aA = a[0] * Ah[0] + a[1] * Ah[1] + a[2] * Ah[2];
-    const double inv = 1.0 / (1.0 + (Ah[0] * Ah[0] + Ah[1] * Ah[1] + Ah[2] * Ah[2]));
-    out[0] = (a[0] + Ah[0] * aA - (Ah[1] * a[2] - Ah[2] * a[1])) * inv;
-    out[1] = (a[1] + Ah[1] * aA - (Ah[2] * a[0] - Ah[0] * a[2])) * inv;
-    out[2] = (a[2] + Ah[2] * aA - (Ah[0] * a[1] - Ah[1] * a[0])) * inv;
+    const double Ah[3] = {__dmul_rn(hdt, A[0]), __dmul_rn(hdt, A[1]), __dmul_rn(hdt, A[2])};
+    const double a[3] = {n[0] + fma(n[1], Ah[2], -__dmul_rn(n[2], Ah[1])), n[1] + fma(n[2], Ah[0], -__dmul_rn(n[0], Ah[2])),
+                         n[2] + fma(n[0], Ah[1], -__dmul_rn(n[1], Ah[0]))};
+    const double aA = fma(a[0], Ah[0], fma(a[1], Ah[1], __dmul_rn(a[2], Ah[2])));
+    const double inv = 1.0 / (1.0 + fma(Ah[0], Ah[0], fma(Ah[1], Ah[1], __dmul_rn(Ah[2], Ah[2]))));
+    out[0] = __dmul_rn(fma(Ah[0], aA, a[0]) - fma(Ah[1], a[2], -__dmul_rn(Ah[2], a[1])), inv);
+    out[1] = __dmul_rn(fma(Ah[1], aA, a[1]) - fma(Ah[2], a[0], -__dmul_rn(Ah[0], a[2])), inv);
+    out[2] = __dmul_rn(fma(Ah[2], aA, a[2]) - fma(Ah[0], a[1], -__dmul_rn(Ah[1], a[0])), inv);
 }
 
 // Heun (App. B, B3-B4) with f = n x A:  f(n, A) added to `acc` with weight w
 __device__ __forceinline__ void heun_add(const double (&n)[3], const double (&A)[3], double w, double (&acc)[3]) {
-    acc[0] = fma(w, n[1] * A[2] - n[2] * A[1], acc[0]);
-    acc[1] = fma(w, n[2] * A[0] - n[0] * A[2], acc[1]);
-    acc[2] = fma(w, n[0] * A[1] - n[1] * A[0], acc[2]);
+    acc[0] = fma(w, fma(n[1], A[2], -__dmul_rn(n[2], A[1])), acc[0]);
+    acc[1] = fma(w, fma(n[2], A[0], -__dmul_rn(n[0], A[2])), acc[1]);
+    acc[2] = fma(w, fma(n[0], A[1], -__dmul_rn(n[1], A[0])), acc[2]);
 }
 
 __device__ __forceinline__ void renormalise_general(double (&v)[3]) {      // Heun: |v| is not close to 1 to rounding
-    const double sc = 1.0 / sqrt(v[0] * v[0] + v[1] * v[1] + v[2] * v[2]);
+    const double sc = 1.0 / sqrt(fma(v[0], v[0], fma(v[1], v[1], __dmul_rn(v[2], v[2]))));
     v[0] *= sc; v[1] *= sc; v[2] *= sc;
 }
 

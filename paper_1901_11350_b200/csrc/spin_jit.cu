@@ -231,6 +231,10 @@ std::string spin::jit_source(const spin_system *s) {
     o << "constexpr bool PER_A = " << (P.perA ? "true" : "false") << ", PER_B = " << (P.perB ? "true" : "false")
       << ", PER_C = " << (P.perC ? "true" : "false") << ";\n";
     o << "constexpr bool CACHE_NOISE = " << ((s->opt_cache_noise && P.thermal_on && !(s->opt_store_A && s->solver == 0)) ? "true" : "false") << ";\n";
+    {   // corrector: the fields of n and of n^p one after the other (40 registers, 1.5 % faster on cfg3) or interleaved (48)
+        const char *e = getenv("SPINLLG_SPLIT");
+        o << "constexpr bool SPLIT_CORR = " << ((e && atoi(e) == 0) ? "false" : "true") << ";\n";
+    }
     o << "constexpr bool HAS_PIN = " << (s->d_pin ? "true" : "false") << ";\n";
     o << "constexpr int SOLVER = " << s->solver << ";      // 0 Depondt, 1 Heun, 2 SIB, 3 RK4 (own stage kernel)\n";
     o << "constexpr bool STORE_A = " << ((s->opt_store_A && s->solver == 0) ? "true" : "false") << ", HAS_DDI = " << (P.has_ddi ? "true" : "false")

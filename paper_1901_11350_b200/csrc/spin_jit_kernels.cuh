@@ -303,6 +303,28 @@ __device__ __forceinline__ void corrector_body(const double *__restrict__ n, con
         if constexpr (spec::STT_ON) stt_gradient<B, 1>(cfg, c, own, sg);
         rotation_field<B>(own[0], F[0], sg[0], Ap);
         load3<0, CG>(Ain + idx, A);
+    } else if constexpr (spec::SPLIT_CORR) {
+        // the two fields one after the other (fewer live registers, more resident warps) instead of interleaved
+        {
+            GlobalAcc<1, CG> cfg;
+            cfg.cfg[0] = n + idx;
+            double own[1][3] = {{n0[0], n0[1], n0[2]}}, F[1][3] = {{th[0], th[1], th[2]}}, sg[1][3] = {{0.0, 0.0, 0.0}};
+            force<B, 1>(cfg, own, F);
+            if constexpr (spec::HAS_DDI) { double d[3]; load3<0, CG>(fddi_n + idx, d); F[0][0] += d[0]; F[0][1] += d[1]; F[0][2] += d[2]; }
+            if constexpr (spec::STT_ON) stt_gradient<B, 1>(cfg, c, own, sg);
+            rotation_field<B>(own[0], F[0], sg[0], A);
+        }
+        {
+            GlobalAcc<1, CG> cfg;
+            cfg.cfg[0] = np + idx;
+            double own[1][3], F[1][3] = {{th[0], th[1], th[2]}}, sg[1][3] = {{0.0, 0.0, 0.0}};
+            load3<0, CG>(cfg.cfg[0], own[0]);
+            np0[0] = own[0][0]; np0[1] = own[0][1]; np0[2] = own[0][2];
+            force<B, 1>(cfg, own, F);
+            if constexpr (spec::HAS_DDI) { double d[3]; load3<0, CG>(fddi_np + idx, d); F[0][0] += d[0]; F[0][1] += d[1]; F[0][2] += d[2]; }
+            if constexpr (spec::STT_ON) stt_gradient<B, 1>(cfg, c, own, sg);
+            rotation_field<B>(own[0], F[0], sg[0], Ap);
+        }
     } else {
         GlobalAcc<2, CG> cfg;
         cfg.cfg[0] = n + idx; cfg.cfg[1] = np + idx;

@@ -602,3 +602,19 @@ def test_one_pass_step_matches_two_sweep_kernels(P, O, cfg, cells, steps, geo, p
     assert b.spin_kernel_info().startswith("jit (brick")
     b.llg_iterate(steps)
     assert np.array_equal(b.spins_get(), g.spins_get())          # same arithmetic, bit for bit
+
+
+def test_checkpoint_resume(P, O):
+    """SURVEY section 5 "checkpoint / resume": spins_get + llg_get_step, then spins_set + llg_set_step on a fresh system, continues
+    the same trajectory (the noise is keyed by the step counter).  spins_set renormalises, so agreement is to rounding, not bitwise."""
+    w = W.config2().resized((40, 24, 1))
+    a = P.SpinSystem.from_workload(w); a.llg_iterate(50)
+    b = P.SpinSystem.from_workload(w); b.llg_iterate(30)
+    snap, step = b.spins_get(), b.llg_get_step()
+    c = P.SpinSystem.from_workload(w)
+    c.spins_set(snap); c.llg_set_step(step); c.llg_iterate(20)
+    assert c.llg_get_step() == 50
+    assert np.abs(c.spins_get() - a.spins_get()).max() < 1e-12
+    d = P.SpinSystem.from_workload(w)
+    d.spins_set(snap); d.llg_iterate(20)                          # wrong step counter: different noise, different trajectory
+    assert np.abs(d.spins_get() - a.spins_get()).max() > 1e-6
