@@ -60,6 +60,7 @@ def lib():
         L.orc_fft3d.argtypes = [dp, ip, C.c_int]
         L.orc_philox4x32_10.argtypes = [C.POINTER(C.c_uint32), C.POINTER(C.c_uint32), C.POINTER(C.c_uint32)]
         L.orc_thermal_xi.argtypes = [C.c_uint64, C.c_uint64, C.c_uint32, dp]
+        L.orc_thermal_xi_image.argtypes = [C.c_uint64, C.c_uint64, C.c_uint32, C.c_uint32, dp]
         L.orc_thermal_sigma.restype = C.c_double
         L.orc_thermal_sigma.argtypes = [vp, C.c_int]
         L.orc_stt_gradient.argtypes = [vp, dp, dp]
@@ -67,6 +68,7 @@ def lib():
         L.orc_llg_iterate.argtypes = [vp, C.c_long]
         L.orc_heun_step.argtypes = [vp]
         L.orc_set_solver.argtypes = [vp, C.c_int]
+        L.orc_set_image.argtypes = [vp, C.c_uint32]
         L.orc_set_pinned.argtypes = [vp, C.c_void_p]
         L.orc_vp_iterate.argtypes = [vp, C.c_long, C.c_double, C.c_double]
         L.orc_vp_reset.argtypes = [vp]
@@ -267,6 +269,10 @@ class OracleSystem:
         assert m.size == self.N
         lib().orc_set_pinned(self._h, m.ctypes.data_as(C.c_void_p))
 
+    def set_image(self, image):
+        """Noise stream of image `image` (independent images of one batched system; 0 = single system)."""
+        lib().orc_set_image(self._h, int(image))
+
     def set_solver(self, solver):
         """0 Depondt (App. B B5-B7), 1 Heun (B3-B4), 2 SIB semi-implicit midpoint (App. C)."""
         lib().orc_set_solver(self._h, int(solver))
@@ -288,9 +294,12 @@ def philox4x32_10(counter, key):
     return tuple(int(x) for x in o)
 
 
-def thermal_xi(seed, step, spin):
+def thermal_xi(seed, step, spin, image=0):
     out = np.zeros(3)
-    lib().orc_thermal_xi(int(seed), int(step), int(spin), out.ctypes.data_as(C.POINTER(C.c_double)))
+    if image == 0:
+        lib().orc_thermal_xi(int(seed), int(step), int(spin), out.ctypes.data_as(C.POINTER(C.c_double)))
+    else:
+        lib().orc_thermal_xi_image(int(seed), int(step), int(spin), int(image), out.ctypes.data_as(C.POINTER(C.c_double)))
     return out
 
 

@@ -76,6 +76,7 @@ typedef struct orc_system {
     unsigned char *pinned;   /* N flags or NULL: a pinned spin keeps its value (":79 pinning of individual spins"); a vacancy
                                 (":79 defects, such as vacancies") is a pinned site holding the zero vector (reading R27)   */
     double *vp_v, *vp_F;     /* velocity-projection minimiser (App. D): velocity and force of the previous iteration, or NULL  */
+    uint32_t image;          /* which image's noise stream this system draws (0 = the single-system stream)                    */
     int solver;              /* 0 Depondt (App. B B5-B7), 1 Heun (B3-B4), 2 SIB semi-implicit midpoint (App. C), 3 RK4 (:168) */
 } orc_system;
 
@@ -207,6 +208,7 @@ void orc_llg_configure(orc_system *s, double dt_fs, double alpha, double T, uint
     s->step = 0;
 }
 void orc_set_solver(orc_system *s, int solver) { s->solver = solver; }
+void orc_set_image(orc_system *s, uint32_t image) { s->image = image; }
 void orc_set_pinned(orc_system *s, const unsigned char *mask) {
     free(s->pinned); s->pinned = NULL;
     if (!mask) return;
@@ -638,19 +640,22 @@ static inline double u01(uint32_t hi, uint32_t lo) {
 }
 /* three standard normals for (seed, step, spin): key = seed, counter = (spin, block, step_lo, step_hi);
  * Box-Muller; block 0 -> (xi_x, xi_y), block 1 -> xi_z.                                      */
-void orc_thermal_xi(uint64_t seed, uint64_t step, uint32_t spin, double xi[3]) {
+/* Independent images (chain of images :197, temperature sweeps :143, Fig. 13) draw independent noise from the same seed: image m
+ * uses the counter words block + 2 m (reading R30); image 0 is the single-system stream.                                    */
+void orc_thermal_xi_image(uint64_t seed, uint64_t step, uint32_t spin, uint32_t image, double xi[3]) {
     uint32_t key[2] = { (uint32_t)seed, (uint32_t)(seed >> 32) }, x[4];
-    uint32_t c0[4] = { spin, 0u, (uint32_t)step, (uint32_t)(step >> 32) };
+    uint32_t c0[4] = { spin, 2u * image, (uint32_t)step, (uint32_t)(step >> 32) };
     orc_philox4x32_10(c0, key, x);
     double u1 = u01(x[0], x[1]), u2 = u01(x[2], x[3]);
     double rad = sqrt(-2.0 * log(u1));
     xi[0] = rad * cos(2.0 * ORC_PI * u2);
     xi[1] = rad * sin(2.0 * ORC_PI * u2);
-    uint32_t c1[4] = { spin, 1u, (uint32_t)step, (uint32_t)(step >> 32) };
+    uint32_t c1[4] = { spin, 2u * image + 1u, (uint32_t)step, (uint32_t)(step >> 32) };
     orc_philox4x32_10(c1, key, x);
     u1 = u01(x[0], x[1]); u2 = u01(x[2], x[3]);
     xi[2] = sqrt(-2.0 * log(u1)) * cos(2.0 * ORC_PI * u2);
 }
+void orc_thermal_xi(uint64_t seed, uint64_t step, uint32_t spin, double xi[3]) { orc_thermal_xi_image(seed, step, spin, 0u, xi); }
 /* Eq. 11 with the 1/sqrt(dt) of :160 (reading R10): sigma = sqrt(2 alpha k_B T mu / (gamma dt)), meV */
 double orc_thermal_sigma(const orc_system *s, int b) {
     return sqrt(2.0 * s->alpha * ORC_K_B * s->T * s->mu[b] * ORC_MU_B / (ORC_GAMMA * s->dt));
@@ -783,7 +788,7 @@ void orc_llg_step(orc_system *s) {
         Fth = (double *)malloc(3 * N * sizeof(double));
 #pragma omp parallel for schedule(static) num_threads(s->nthreads)
         for (long i = 0; i < N; ++i) {
-            double xi[3]; orc_thermal_xi(s->seed, s->step, (uint32_t)i, xi);
+            double xi[3]; orc_thermal_xi_image(s->seed, s->step, (uint32_t)i, s->image, xi);
             double sig = orc_thermal_sigma(s, (int)(i % nb));
             for (int k = 0; k < 3; ++k) Fth[3*i+k] = sig * xi[k];
         }
@@ -837,7 +842,7 @@ static void orc_rk4_step(orc_system *s) {
     if (s->T > 0.0) {
         Fth = (double *)malloc(3 * N * sizeof(double));
         for (long i = 0; i < N; ++i) {
-            double xi[3]; orc_thermal_xi(s->seed, s->step, (uint32_t)i, xi);
+            double xi[3]; orc_thermal_xi_image(s->seed, s->step, (uint32_t)i, s->image, xi);
             double sig = orc_thermal_sigma(s, (int)(i % nb));
             for (int k = 0; k < 3; ++k) Fth[3*i+k] = sig * xi[k];
         }

@@ -618,3 +618,28 @@ def test_checkpoint_resume(P, O):
     d = P.SpinSystem.from_workload(w)
     d.spins_set(snap); d.llg_iterate(20)                          # wrong step counter: different noise, different trajectory
     assert np.abs(d.spins_get() - a.spins_get()).max() > 1e-6
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# BASELINE.json's full sizes AND full step counts (north_star: "spin configurations after each config's step count within 1e-9").
+# The oracle needs minutes of host time for these, so they only run with SPINLLG_FULL_STEPS=1; the residuals measured on the B200 box
+# are recorded in DESIGN.md section 3.  cfg5's 1000 steps (2000 padded-FFT dipolar evaluations in the oracle) are run for 100 steps.
+import os as _os
+FULL_STEPS = [(1, 1000), (2, 10000), (3, 2000), (4, 5000), (5, 100)]
+
+
+@pytest.mark.skipif(_os.environ.get("SPINLLG_FULL_STEPS") != "1", reason="minutes of oracle time; set SPINLLG_FULL_STEPS=1")
+@pytest.mark.parametrize("cfg,steps", FULL_STEPS)
+def test_full_size_full_step_count(P, O, cfg, steps):
+    import time
+    w = W.CONFIGS[cfg]()
+    g, o = pair(P, O, w)
+    t0 = time.perf_counter()
+    g.llg_iterate(steps); g.spin_synchronize()
+    t1 = time.perf_counter()
+    o.iterate(steps)
+    t2 = time.perf_counter()
+    ng, no = g.spins_get(), o.spins()
+    d = np.abs(ng - no).max()
+    print(f"FULL cfg{cfg} {w.n_cells} steps={steps}: max|dn| = {d:.3e}  (GPU {t1 - t0:.2f} s, oracle {t2 - t1:.1f} s on {o.threads} threads)")
+    assert d <= SPIN_ATOL

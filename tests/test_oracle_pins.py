@@ -664,3 +664,24 @@ def test_vp_stops_on_overshoot_and_finds_the_ferromagnet():
     a = OracleSystem.from_workload(w); a.vp_iterate(30, 0.1)
     b = OracleSystem.from_workload(w); b.vp_iterate(13, 0.1); b.vp_iterate(17, 0.1)
     assert np.array_equal(a.spins(), b.spins())
+
+
+def test_image_noise_streams_are_independent():
+    """Batched images (reading R30): image m draws from the Philox counter words block + 2 m.  Image 0 is the single-system stream;
+    other images are standard normal and uncorrelated with it and with each other."""
+    seed, n = 77, 4000
+    x = {m: np.array([O.thermal_xi(seed, 3, i, image=m) for i in range(n)]) for m in (0, 1, 2)}
+    assert np.array_equal(x[0], np.array([O.thermal_xi(seed, 3, i) for i in range(n)]))
+    for m in (1, 2):
+        assert abs(x[m].mean()) < 0.05 and abs(x[m].var() - 1.0) < 0.06
+    for a, b in ((0, 1), (0, 2), (1, 2)):
+        c = np.corrcoef(x[a].ravel(), x[b].ravel())[0, 1]
+        assert abs(c) < 0.04, (a, b, c)
+        assert not np.any(np.all(x[a] == x[b], axis=1))
+    # the layout: image m's x/y pair comes from counter word 2 m, its z from 2 m + 1
+    ctr = lambda blk: O.philox4x32_10([5, blk, 3, 0], [seed, 0])
+    assert not np.array_equal(ctr(2), ctr(0))
+    w = small(2, (8, 8, 1))
+    a = OracleSystem.from_workload(w); a.set_image(1); a.iterate(5)
+    b = OracleSystem.from_workload(w); b.iterate(5)
+    assert np.abs(a.spins() - b.spins()).max() > 1e-6
