@@ -100,6 +100,16 @@ int spins_get(spin_system *sys, double *n_xyz /*host, 3N AoS*/);
 int spins_set_device(spin_system *sys, const double *n_xyz /*device, 3N AoS*/);
 int spins_get_device(spin_system *sys, double *n_xyz /*device, 3N AoS*/);
 
+/* ---- batched images (":197 chain of images", temperature sweeps of Fig. 13): n_images independent configurations of the same lattice
+ * and Hamiltonian advance in the same launches (the sweeps take the image from the third grid dimension).  New images start as
+ * copies of image 0.  Image m draws its thermal noise from the Philox counter words block + 2 m, at its own temperature if
+ * llg_set_image_temperatures gives one (host array of n_images Kelvin values; needs T > 0 in llg_configure; NULL: all at T).
+ * spin_select_image chooses the image that spins_set/get[_device], effective_field, energy, observables and topological_charge
+ * address (default 0).  Two-stage solvers only; minimise_vp and the RK4 solver work on a single image (SPIN_ERR_STATE).     */
+int spin_set_images(spin_system *sys, int n_images);
+int spin_select_image(spin_system *sys, int image);
+int llg_set_image_temperatures(spin_system *sys, const double *T_kelvin /*host, n_images, or NULL*/);
+
 /* Pinning and vacancies (:79 "pinning of individual spins or a set of spins", "defects, such as vacancies").  mask: N flags in
  * boundary index order, non-zero = pinned; NULL removes all pins.  A pinned spin is never updated by llg_iterate but acts on its
  * neighbours as usual.  A vacancy is a pinned site holding the zero vector: spins_set accepts a zero vector on pinned sites only;

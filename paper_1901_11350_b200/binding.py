@@ -19,7 +19,7 @@ EXPORTS = [
     "spin_geometry_create", "spin_system_destroy", "spin_system_nspins", "spin_set_stream",
     "hamiltonian_set_mu_s", "hamiltonian_set_field", "hamiltonian_set_anisotropy", "hamiltonian_set_pairs",
     "hamiltonian_set_exchange_shells", "hamiltonian_set_dmi_shells", "hamiltonian_set_quadruplets",
-    "hamiltonian_set_ddi", "spins_set_pinned", "spins_set", "spins_get", "spins_set_device", "spins_get_device",
+    "hamiltonian_set_ddi", "spin_set_images", "spin_select_image", "llg_set_image_temperatures", "spins_set_pinned", "spins_set", "spins_get", "spins_set_device", "spins_get_device",
     "llg_configure", "llg_set_solver", "minimise_vp", "minimise_vp_reset", "llg_iterate", "llg_get_step", "llg_set_step", "spin_synchronize",
     "effective_field", "effective_field_device", "energy", "observables", "topological_charge",
     "spin_launch_counts", "spin_profile_enable", "spin_profile_get", "spin_set_option",
@@ -64,6 +64,9 @@ def lib() -> C.CDLL:
         "llg_configure": (C.c_int, [vp, C.c_double, C.c_double, C.c_double, C.c_uint64, C.c_double, dp, C.c_double]),
         "llg_set_solver": (C.c_int, [vp, C.c_int]),
         "spins_set_pinned": (C.c_int, [vp, C.c_void_p]),
+        "spin_set_images": (C.c_int, [vp, C.c_int]),
+        "spin_select_image": (C.c_int, [vp, C.c_int]),
+        "llg_set_image_temperatures": (C.c_int, [vp, dp]),
         "minimise_vp": (C.c_int, [vp, C.c_int64, C.c_double, C.c_double]),
         "minimise_vp_reset": (C.c_int, [vp]),
         "llg_iterate": (C.c_int, [vp, C.c_int64]),
@@ -220,6 +223,19 @@ class SpinSystem:
     def llg_configure(self, dt_fs, alpha, T=0.0, seed=0, u=0.0, j_dir=(1, 0, 0), beta=0.0):
         j, jp = _d(j_dir)
         _check(lib().llg_configure(self._h, float(dt_fs), float(alpha), float(T), int(seed), float(u), jp, float(beta)))
+
+    def spin_set_images(self, n_images):
+        _check(lib().spin_set_images(self._h, int(n_images)))
+
+    def spin_select_image(self, image):
+        _check(lib().spin_select_image(self._h, int(image)))
+
+    def llg_set_image_temperatures(self, T):
+        if T is None:
+            _check(lib().llg_set_image_temperatures(self._h, None))
+            return
+        a = np.ascontiguousarray(np.asarray(T, dtype=np.float64).reshape(-1))
+        _check(lib().llg_set_image_temperatures(self._h, a.ctypes.data_as(C.POINTER(C.c_double))))
 
     def minimise_vp(self, n_iterations, dt, mass=1.0):
         _check(lib().minimise_vp(self._h, int(n_iterations), float(dt), float(mass)))

@@ -293,18 +293,24 @@ bool same_layout(const DevicePlan &a, const DevicePlan &b) {
         if (!(s)->has_device) return spin::fail(SPIN_ERR_CUDA, "no CUDA device: this library has no CPU fallback"); \
     } while (0)
 
-// (re)allocate the per-spin arrays for the layout of `P`; the current configuration is carried over through the
+// offset (in doubles) of the selected image in every per-spin array
+inline size_t img_off(const spin_system *s) { return (size_t)s->img_sel * (size_t)s->nb * (size_t)s->plan.sub; }
+
+// (re)allocate the per-spin arrays for the layout of `P`; the current configurations (all images) are carried over through a
 // boundary-order staging buffer when `keep` is set
 int allocate_arrays(spin_system *s, const DevicePlan &P, bool keep) {
     const int nt = 256;
     const unsigned nblk = (unsigned)((s->N + nt - 1) / nt);
+    double *stage = s->d_aos;
     if (keep) {
-        unpack_kernel<<<nblk, nt, 0, s->stream>>>(s->plan, s->d_n[s->cur], s->d_aos, (int)s->N, 0);
-        s->n_launch++;
+        if (s->n_img > 1) SPIN_CUDA(cudaMalloc(&stage, (size_t)s->n_img * 3 * s->N * sizeof(double)));
+        for (int k = 0; k < s->n_img; ++k)
+            unpack_kernel<<<nblk, nt, 0, s->stream>>>(s->plan, s->d_n[s->cur] + (size_t)k * s->nb * s->plan.sub, stage + (size_t)k * 3 * s->N, (int)s->N, 0);
+        s->n_launch += s->n_img;
         SPIN_CUDA(cudaStreamSynchronize(s->stream));
     }
     double **arrs[] = {&s->d_n[0], &s->d_n[1], &s->d_np, &s->d_A, &s->d_fddi[0], &s->d_fddi[1]};
-    const size_t bytes = (size_t)s->nb * P.sub * sizeof(double);
+    const size_t bytes = (size_t)s->n_img * s->nb * P.sub * sizeof(double);
     for (double **a : arrs) {
         if (*a) cudaFree(*a);
         *a = nullptr;
@@ -315,10 +321,12 @@ int allocate_arrays(spin_system *s, const DevicePlan &P, bool keep) {
     s->cur = 0;
     if (keep) {
         int *bad = (int *)(s->d_aos + (size_t)3 * s->N);
-        pack_kernel<<<nblk, nt, 0, s->stream>>>(P, s->d_aos, s->d_n[0], (int)s->N, 0, bad);
-        s->n_launch++;
+        for (int k = 0; k < s->n_img; ++k)
+            pack_kernel<<<nblk, nt, 0, s->stream>>>(P, stage + (size_t)k * 3 * s->N, s->d_n[0] + (size_t)k * s->nb * P.sub, (int)s->N, 0, bad);
+        s->n_launch += s->n_img;
     }
     SPIN_CUDA(cudaStreamSynchronize(s->stream));
+    if (stage != s->d_aos) cudaFree(stage);
     SPIN_CUDA(cudaGetLastError());
     return SPIN_OK;
 }
@@ -383,9 +391,11 @@ int enqueue_step_t(spin_system *s, const Launch &L, unsigned step_add) {
         s->cur ^= 1;
         return SPIN_OK;
     }
+    const size_t istr = (size_t)s->nb * s->plan.sub;       // image stride
     if (s->ddi_on) {
         if (prof) cudaEventRecord(s->ev0, s->stream);
-        int rc = ddi_field(s, n, s->d_fddi[0]);
+        int rc = SPIN_OK;
+        for (int k = 0; k < s->n_img && rc == SPIN_OK; ++k) rc = ddi_field(s, n + k * istr, s->d_fddi[0] + k * istr);
         if (rc) return rc;
         if (prof) { cudaEventRecord(s->ev1, s->stream); cudaEventSynchronize(s->ev1); float ms; cudaEventElapsedTime(&ms, s->ev0, s->ev1); s->prof_ms[2] += ms; s->prof_n[2]++; }
     }
@@ -402,7 +412,8 @@ int enqueue_step_t(spin_system *s, const Launch &L, unsigned step_add) {
     if (prof) { cudaEventRecord(s->ev1, s->stream); cudaEventSynchronize(s->ev1); float ms; cudaEventElapsedTime(&ms, s->ev0, s->ev1); s->prof_ms[0] += ms; s->prof_n[0]++; }
     if (s->ddi_on) {
         if (prof) cudaEventRecord(s->ev0, s->stream);
-        int rc = ddi_field(s, s->d_np, s->d_fddi[1]);
+        int rc = SPIN_OK;
+        for (int k = 0; k < s->n_img && rc == SPIN_OK; ++k) rc = ddi_field(s, s->d_np + k * istr, s->d_fddi[1] + k * istr);
         if (rc) return rc;
         if (prof) { cudaEventRecord(s->ev1, s->stream); cudaEventSynchronize(s->ev1); float ms; cudaEventElapsedTime(&ms, s->ev0, s->ev1); s->prof_ms[2] += ms; s->prof_n[2]++; }
     }
@@ -427,7 +438,7 @@ int enqueue_step(spin_system *s, unsigned step_add) {
 // deterministic force of the current configuration into d_np (scratch), terms by mask
 int enqueue_force(spin_system *s, int mask, double *d_out) {
     const Launch L = brick_launch(s);
-    double *n = s->d_n[s->cur];
+    double *n = s->d_n[s->cur] + img_off(s);
     if (s->ddi_on && (mask & T_DDI)) { int rc = ddi_field(s, n, s->d_fddi[0]); if (rc) return rc; }
     if (L.flat) force_kernel<32, 8, 1><<<L.grid, L.block, 0, s->stream>>>(s->plan, n, s->d_fddi[0], mask, d_out);
     else force_kernel<32, 4, 2><<<L.grid, L.block, 0, s->stream>>>(s->plan, n, s->d_fddi[0], mask, d_out);
@@ -437,7 +448,7 @@ int enqueue_force(spin_system *s, int mask, double *d_out) {
 
 int reduce_all(spin_system *s, double out[N_RED]) {
     const Launch L = brick_launch(s);
-    double *n = s->d_n[s->cur];
+    double *n = s->d_n[s->cur] + img_off(s);
     if (s->ddi_on) { int rc = ddi_field(s, n, s->d_fddi[0]); if (rc) return rc; }
     const int nblocks = (int)(L.grid.x * L.grid.y);
     if (L.flat) reduce_kernel<32, 8, 1><<<L.grid, L.block, 0, s->stream>>>(s->plan, n, s->d_fddi[0], s->d_partials);
@@ -474,6 +485,7 @@ extern "C" int spin_geometry_create(const double bravais[9], int n_basis, const 
     spin_system *s = new spin_system();
     s->has_device = has_device;
     s->jit = nullptr; s->opt_jit = 1; s->opt_tma = 0; s->opt_ddi_slab = 1; s->opt_col = 0; s->opt_cache_noise = 1; s->opt_coop = 1; s->opt_fused = 0; s->d_bar = nullptr;
+    s->n_img = 1; s->img_sel = 0; s->d_img_sigma = nullptr;
     memcpy(s->brav, bravais, sizeof(s->brav));
     s->nb = n_basis;
     s->basis.assign(basis_frac, basis_frac + 3 * n_basis);
@@ -536,7 +548,7 @@ extern "C" void spin_system_destroy(spin_system *s) {
     ddi_release(s);
     jit_release(s);
     cudaFree(s->d_n[0]); cudaFree(s->d_n[1]); cudaFree(s->d_np); cudaFree(s->d_A); cudaFree(s->d_fddi[0]); cudaFree(s->d_fddi[1]);
-    cudaFree(s->d_pin); cudaFree(s->d_vp); cudaFree(s->d_bar);
+    cudaFree(s->d_pin); cudaFree(s->d_vp); cudaFree(s->d_bar); cudaFree(s->d_img_sigma);
     cudaFree(s->d_aos); cudaFree(s->d_partials); cudaFree(s->d_result); cudaFree(s->d_step);
     if (s->ev0) cudaEventDestroy(s->ev0);
     if (s->ev1) cudaEventDestroy(s->ev1);
@@ -682,7 +694,7 @@ static int pack_from_device_aos(spin_system *s, const double *d_aos) {
     int *bad = (int *)(s->d_aos + (size_t)3 * s->N);
     SPIN_CUDA(cudaMemsetAsync(bad, 0, sizeof(int), s->stream));
     const int nt = 256;
-    pack_kernel<<<(unsigned)((s->N + nt - 1) / nt), nt, 0, s->stream>>>(s->plan, d_aos, s->d_n[s->cur], (int)s->N, 1, bad);
+    pack_kernel<<<(unsigned)((s->N + nt - 1) / nt), nt, 0, s->stream>>>(s->plan, d_aos, s->d_n[s->cur] + img_off(s), (int)s->N, 1, bad);
     s->n_launch++;
     int h_bad = 0;
     SPIN_CUDA(cudaMemcpyAsync(&h_bad, bad, sizeof(int), cudaMemcpyDeviceToHost, s->stream));
@@ -691,6 +703,56 @@ static int pack_from_device_aos(spin_system *s, const double *d_aos) {
     if (h_bad) return spin::fail(SPIN_ERR_ARG, "spins_set: zero or non-finite spin vector");
     return SPIN_OK;
 }
+// ---- batched images
+extern "C" int spin_set_images(spin_system *s, int n_images) {
+    REQUIRE(s && n_images >= 1 && n_images <= 65535, "n_images must be in [1, 65535]");
+    NEED_DEVICE(s);
+    if (n_images == s->n_img) return SPIN_OK;
+    int rc = ensure_plan(s);                  // settle the layout first
+    if (rc) return rc;
+    SPIN_CUDA(cudaStreamSynchronize(s->stream));
+    const size_t istr = (size_t)s->nb * s->plan.sub, ibytes = istr * sizeof(double);
+    const int n_old = s->n_img, n_keep = std::min(n_old, n_images);
+    double *old = nullptr;
+    SPIN_CUDA(cudaMalloc(&old, (size_t)n_old * ibytes));
+    SPIN_CUDA(cudaMemcpy(old, s->d_n[s->cur], (size_t)n_old * ibytes, cudaMemcpyDeviceToDevice));
+    s->n_img = n_images;
+    s->img_sel = 0;
+    rc = allocate_arrays(s, s->plan, false);
+    if (rc == SPIN_OK) {
+        cudaError_t e = cudaMemcpy(s->d_n[0], old, (size_t)n_keep * ibytes, cudaMemcpyDeviceToDevice);
+        for (int k = n_keep; k < n_images && e == cudaSuccess; ++k)      // new images start as copies of image 0
+            e = cudaMemcpy(s->d_n[0] + (size_t)k * istr, old, ibytes, cudaMemcpyDeviceToDevice);
+        if (e != cudaSuccess) rc = spin::fail(SPIN_ERR_CUDA, "spin_set_images: %s", cudaGetErrorString(e));
+    }
+    cudaFree(old);
+    if (s->d_img_sigma) { cudaFree(s->d_img_sigma); s->d_img_sigma = nullptr; }
+    s->plan_dirty = true;                     // kernels variants and dipolar buffers depend on the image count
+    drop_graphs(s);
+    return rc;
+}
+extern "C" int spin_select_image(spin_system *s, int image) {
+    REQUIRE(s && image >= 0 && image < s->n_img, "image index out of range");
+    s->img_sel = image;
+    return SPIN_OK;
+}
+extern "C" int llg_set_image_temperatures(spin_system *s, const double *T_kelvin) {
+    REQUIRE(s, "null system");
+    NEED_DEVICE(s);
+    SPIN_CUDA(cudaStreamSynchronize(s->stream));
+    if (!T_kelvin) { if (s->d_img_sigma) { cudaFree(s->d_img_sigma); s->d_img_sigma = nullptr; } drop_graphs(s); return SPIN_OK; }
+    REQUIRE(s->T > 0.0, "llg_configure must set a positive reference temperature first");
+    std::vector<double> sc((size_t)s->n_img);
+    for (int k = 0; k < s->n_img; ++k) {
+        REQUIRE(T_kelvin[k] >= 0.0 && isfinite(T_kelvin[k]), "image %d: temperature must be >= 0", k);
+        sc[(size_t)k] = sqrt(T_kelvin[k] / s->T);
+    }
+    if (!s->d_img_sigma) SPIN_CUDA(cudaMalloc(&s->d_img_sigma, (size_t)s->n_img * sizeof(double)));
+    SPIN_CUDA(cudaMemcpy(s->d_img_sigma, sc.data(), (size_t)s->n_img * sizeof(double), cudaMemcpyHostToDevice));
+    drop_graphs(s);                           // captured launches hold the old pointer
+    return SPIN_OK;
+}
+
 // pinned spins: flags in boundary order; null clears.  A pinned site may hold the zero vector (a vacancy).
 extern "C" int spins_set_pinned(spin_system *s, const unsigned char *mask) {
     REQUIRE(s, "null system");
@@ -724,7 +786,7 @@ extern "C" int spins_get_device(spin_system *s, double *n) {
     REQUIRE(s && n, "null argument");
     NEED_DEVICE(s);
     const int nt = 256;
-    unpack_kernel<<<(unsigned)((s->N + nt - 1) / nt), nt, 0, s->stream>>>(s->plan, s->d_n[s->cur], n, (int)s->N, 0);
+    unpack_kernel<<<(unsigned)((s->N + nt - 1) / nt), nt, 0, s->stream>>>(s->plan, s->d_n[s->cur] + img_off(s), n, (int)s->N, 0);
     s->n_launch++;
     SPIN_CUDA(cudaGetLastError());
     return SPIN_OK;
@@ -780,6 +842,8 @@ extern "C" int llg_iterate(spin_system *s, int64_t n_steps) {
     int rc = ensure_plan(s);
     if (rc) return rc;
     s->vp_active = false;
+    if (s->n_img > 1 && (!jit_ready(s) || s->solver == SPIN_SOLVER_RK4))
+        return spin::fail(SPIN_ERR_STATE, "batched images need the run-time specialised kernels and a two-stage solver (%s)", s->jit_note.c_str());
     if (s->solver != SPIN_SOLVER_DEPONDT && !jit_ready(s))
         return spin::fail(SPIN_ERR_STATE, "the Heun, SIB and RK4 solvers need the run-time specialised kernels (%s)", s->jit_note.c_str());
     int64_t done = 0;
@@ -903,6 +967,7 @@ extern "C" int observables(spin_system *s, double M[3], double *max_torque) {
 extern "C" int minimise_vp(spin_system *s, int64_t n_iter, double dt, double mass) {
     REQUIRE(s && n_iter >= 0, "bad argument");
     REQUIRE(dt > 0.0 && isfinite(dt) && mass > 0.0 && isfinite(mass), "dt and mass must be positive");
+    if (s->n_img > 1) return spin::fail(SPIN_ERR_STATE, "minimise_vp works on a single image");
     int rc = ensure_plan(s);
     if (rc) return rc;
     const Launch L = brick_launch(s);
@@ -946,7 +1011,7 @@ extern "C" int topological_charge(spin_system *s, double *Q) {
     const int ccw = (s->brav[0] * s->brav[4] - s->brav[1] * s->brav[3]) > 0.0 ? 1 : 0;
     double *d_part = nullptr;
     SPIN_CUDA(cudaMalloc(&d_part, (size_t)nblk * sizeof(double)));
-    topo_kernel<<<nblk, 256, 0, s->stream>>>(s->plan, s->d_n[s->cur], ccw, d_part);
+    topo_kernel<<<nblk, 256, 0, s->stream>>>(s->plan, s->d_n[s->cur] + img_off(s), ccw, d_part);
     topo_final_kernel<<<1, 32, 0, s->stream>>>(d_part, nblk, s->d_result);
     s->n_launch += 2;
     cudaError_t e = cudaMemcpyAsync(Q, s->d_result, sizeof(double), cudaMemcpyDeviceToHost, s->stream);

@@ -24,15 +24,17 @@ __device__ __forceinline__ double uniform53(unsigned int hi, unsigned int lo) {
     const unsigned long long v = (((unsigned long long)hi << 32) | lo) >> 11;
     return ((double)v + 0.5) * (1.0 / 9007199254740992.0);
 }
-__device__ __forceinline__ void thermal_xi(unsigned int seed_lo, unsigned int seed_hi, unsigned long long step, unsigned int spin, double (&xi)[3]) {
-    unsigned int a0 = spin, a1 = 0u, a2 = (unsigned int)step, a3 = (unsigned int)(step >> 32);
+// image m of a batched system draws from the counter words block + 2 m (R30); image 0 is the single-system stream
+__device__ __forceinline__ void thermal_xi(unsigned int seed_lo, unsigned int seed_hi, unsigned long long step, unsigned int spin, double (&xi)[3],
+                                           unsigned int image = 0u) {
+    unsigned int a0 = spin, a1 = 2u * image, a2 = (unsigned int)step, a3 = (unsigned int)(step >> 32);
     philox4x32_10(a0, a1, a2, a3, seed_lo, seed_hi);
     double sn, cs;
     double rad = sqrt(-2.0 * log(uniform53(a0, a1)));
     sincospi(2.0 * uniform53(a2, a3), &sn, &cs);
     xi[0] = rad * cs;
     xi[1] = rad * sn;
-    unsigned int b0 = spin, b1 = 1u, b2 = (unsigned int)step, b3 = (unsigned int)(step >> 32);
+    unsigned int b0 = spin, b1 = 2u * image + 1u, b2 = (unsigned int)step, b3 = (unsigned int)(step >> 32);
     philox4x32_10(b0, b1, b2, b3, seed_lo, seed_hi);
     rad = sqrt(-2.0 * log(uniform53(b0, b1)));
     xi[2] = rad * cospi(2.0 * uniform53(b2, b3));

@@ -166,7 +166,7 @@ static void jit_brick_launch(const spin_system *s, dim3 &grid, dim3 &block) {
 // SPINLLG_FUSED="ftx,fty,ftz,threads" overrides the defaults (32 x 8 x 8 cells, 512 threads; flat lattices 32 x 16 x 1).
 static bool plan_fused(const spin_system *s, int g[4], size_t &smem) {
     const DevicePlan &P = s->plan;
-    if (!s->opt_fused || s->solver != 0 || s->ddi_on || s->opt_store_A) return false;
+    if (!s->opt_fused || s->solver != 0 || s->ddi_on || s->opt_store_A || s->n_img > 1) return false;
     if (s->opt_fused < 2 && s->N < 16384) return false;
     const bool flat = P.Nc < 2;
     int v[4] = {32, flat ? 16 : 8, flat ? 1 : 8, 512};
@@ -189,7 +189,7 @@ static bool plan_fused(const spin_system *s, int g[4], size_t &smem) {
 // SPINLLG_COL="cbx,cby,ccz" overrides the defaults (32 x 4 columns, 16 planes per chunk).
 static bool plan_col(const spin_system *s, int g[4]) {
     const DevicePlan &P = s->plan;
-    if (!s->opt_col || s->opt_store_A || s->solver != 0 || s->d_pin || P.rC < 1 || P.Nc < 2) return false;
+    if (!s->opt_col || s->opt_store_A || s->solver != 0 || s->d_pin || s->n_img > 1 || P.rC < 1 || P.Nc < 2) return false;
     int cbx = 32, cby = 4, ccz = 16;
     if (const char *e = getenv("SPINLLG_COL")) {
         int v[3] = {0, 0, 0};
@@ -209,6 +209,7 @@ static bool plan_tma(const spin_system *s, TmaGeo &gp, TmaGeo &gc, std::string &
     if (!s->opt_tma) { why = "disabled by option use_tma=0"; return false; }
     if (s->solver != 0) { why = "Depondt solver only"; return false; }
     if (s->d_pin) { why = "pinned spins use the brick kernels"; return false; }
+    if (s->n_img > 1) { why = "batched images use the brick kernels"; return false; }
     if (s->opt_store_A) { why = "store_A=1 uses the brick kernels"; return false; }
     if (s->opt_tma < 2 && s->N < 16384) { why = "lattice too small to fill persistent CTAs"; return false; }
     return plan_tma_geo(s, 1, "SPINLLG_TMA_P", gp, why) && plan_tma_geo(s, 2, "SPINLLG_TMA_C", gc, why);
@@ -405,10 +406,43 @@ static void tma_prepare(spin_system *s, JitState *j) {
     j->tma_note.clear();
 }
 
+// which variants of the sweeps this system can use (depends on options, solver, pins, image count -- not only on the source)
+static void variants_prepare(spin_system *s, JitState *j) {
+    tma_prepare(s, j);
+    j->fused = plan_fused(s, j->fused_geo, j->fused_smem);
+    if (j->fused) {
+        cudaError_t fe = cudaLibraryGetKernel(&j->k_fused, j->lib, "jit_depondt_fused");
+        if (fe == cudaSuccess) fe = cudaFuncSetAttribute((const void *)j->k_fused, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)j->fused_smem);
+        if (fe != cudaSuccess) { cudaGetLastError(); j->fused = false; }
+    }
+    j->coop = false;
+    if (s->opt_coop && !s->ddi_on && s->solver != SPIN_SOLVER_RK4 && s->n_img == 1) {
+        int dev = 0, can = 0, occ = 0;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&can, cudaDevAttrCooperativeLaunch, dev);
+        dim3 grid, block;
+        jit_brick_launch(s, grid, block);
+        cudaError_t ce = cudaLibraryGetKernel(&j->k_coop, j->lib, "jit_steps_coop");
+        if (ce == cudaSuccess) ce = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, (const void *)j->k_coop, (int)block.x, 0);
+        if (ce == cudaSuccess && can && occ > 0) {
+            j->coop_grid = std::min((int)(grid.x * grid.y), occ * sm_count(s));
+            j->coop = true;
+        } else {
+            cudaGetLastError();
+        }
+    }
+    j->col = plan_col(s, j->col_geo);
+    if (j->col) {
+        cudaError_t e = cudaLibraryGetKernel(&j->k_pred_col, j->lib, "jit_predictor_col");
+        if (e == cudaSuccess) e = cudaLibraryGetKernel(&j->k_corr_col, j->lib, "jit_corrector_col");
+        if (e != cudaSuccess) { cudaGetLastError(); j->col = false; }
+    }
+}
+
 int spin::jit_prepare(spin_system *s) {
     const std::string src = jit_source(s);
     if (s->jit && s->jit->loaded && s->jit->source == src) {      // plan changed in ways the sweeps do not see
-        tma_prepare(s, s->jit);                                   // the arrays may have moved: tensor maps are rebuilt
+        variants_prepare(s, s->jit);                              // the arrays may have moved, options may have changed
         return SPIN_OK;
     }
     jit_release(s);
@@ -430,35 +464,7 @@ int spin::jit_prepare(spin_system *s) {
     if (e == cudaSuccess) e = cudaLibraryGetKernel(&j->k_corr, j->lib, "jit_corrector");
     if (e == cudaSuccess) e = cudaLibraryGetKernel(&j->k_rk4, j->lib, "jit_rk4_stage");
     if (e != cudaSuccess) return spin::fail(SPIN_ERR_CUDA, "cudaLibraryGetKernel failed: %s", cudaGetErrorString(e));
-    tma_prepare(s, j);
-    j->fused = plan_fused(s, j->fused_geo, j->fused_smem);
-    if (j->fused) {
-        cudaError_t fe = cudaLibraryGetKernel(&j->k_fused, j->lib, "jit_depondt_fused");
-        if (fe == cudaSuccess) fe = cudaFuncSetAttribute((const void *)j->k_fused, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)j->fused_smem);
-        if (fe != cudaSuccess) { cudaGetLastError(); j->fused = false; }
-    }
-    j->coop = false;
-    if (s->opt_coop && !s->ddi_on && s->solver != SPIN_SOLVER_RK4) {
-        int dev = 0, can = 0, occ = 0;
-        cudaGetDevice(&dev);
-        cudaDeviceGetAttribute(&can, cudaDevAttrCooperativeLaunch, dev);
-        dim3 grid, block;
-        jit_brick_launch(s, grid, block);
-        cudaError_t ce = cudaLibraryGetKernel(&j->k_coop, j->lib, "jit_steps_coop");
-        if (ce == cudaSuccess) ce = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, (const void *)j->k_coop, (int)block.x, 0);
-        if (ce == cudaSuccess && can && occ > 0) {
-            j->coop_grid = std::min((int)(grid.x * grid.y), occ * sm_count(s));
-            j->coop = true;
-        } else {
-            cudaGetLastError();
-        }
-    }
-    j->col = plan_col(s, j->col_geo);
-    if (j->col) {
-        e = cudaLibraryGetKernel(&j->k_pred_col, j->lib, "jit_predictor_col");
-        if (e == cudaSuccess) e = cudaLibraryGetKernel(&j->k_corr_col, j->lib, "jit_corrector_col");
-        if (e != cudaSuccess) { cudaGetLastError(); j->col = false; }
-    }
+    variants_prepare(s, j);
     return SPIN_OK;
 }
 
@@ -469,9 +475,11 @@ int spin::jit_launch_predictor(spin_system *s, dim3 grid, dim3 block, const doub
     unsigned seed_lo = s->plan.seed_lo, seed_hi = s->plan.seed_hi;
     const unsigned long long *d_step = s->d_step;
     const unsigned char *pin = s->d_pin;
+    const double *img_sigma = s->d_img_sigma;
     void *args[] = {(void *)&n, (void *)&fddi, (void *)&np, (void *)&Aout, (void *)&d_step, (void *)&step_add, (void *)&seed_lo, (void *)&seed_hi,
-                    (void *)&pin};
+                    (void *)&pin, (void *)&img_sigma};
     jit_brick_launch(s, grid, block);
+    grid.z = (unsigned)s->n_img;
     SPIN_CUDA(cudaLaunchKernel((const void *)s->jit->k_pred, grid, block, args, 0, s->stream));
     return SPIN_OK;
 }
@@ -480,10 +488,12 @@ int spin::jit_launch_corrector(spin_system *s, dim3 grid, dim3 block, const doub
                                const double *fddi_np, const double *Ain, double *nout, unsigned step_add) {
     unsigned seed_lo = s->plan.seed_lo, seed_hi = s->plan.seed_hi;
     const unsigned char *pin = s->d_pin;
+    const double *img_sigma = s->d_img_sigma;
     const unsigned long long *d_step = s->d_step;
     void *args[] = {(void *)&n, (void *)&np, (void *)&fddi_n, (void *)&fddi_np, (void *)&Ain, (void *)&nout, (void *)&d_step, (void *)&step_add,
-                    (void *)&seed_lo, (void *)&seed_hi, (void *)&pin};
+                    (void *)&seed_lo, (void *)&seed_hi, (void *)&pin, (void *)&img_sigma};
     jit_brick_launch(s, grid, block);
+    grid.z = (unsigned)s->n_img;
     SPIN_CUDA(cudaLaunchKernel((const void *)s->jit->k_corr, grid, block, args, 0, s->stream));
     return SPIN_OK;
 }

@@ -215,14 +215,17 @@ __device__ __forceinline__ bool locate(Coord &c, int &idx, int brick) {
     return (c.ia < spec::NA) && (c.ib < spec::NB) && (c.ic < spec::NC);
 }
 
+// image / sigma_scale: batched images draw independent noise, each at its own temperature (sigma ~ sqrt(T)); 0 / 1.0 otherwise
 template <int B>
-__device__ __forceinline__ void thermal_force(const Coord &c, u64 step, u32 seed_lo, u32 seed_hi, double (&f)[3]) {
+__device__ __forceinline__ void thermal_force(const Coord &c, u64 step, u32 seed_lo, u32 seed_hi, double (&f)[3], u32 image = 0u,
+                                              double sigma_scale = 1.0) {
     if constexpr (spec::THERMAL_ON) {
         const u32 cell = (u32)(c.ia + spec::NA * c.ib + (spec::NA * spec::NB) * c.ic);
         double xi[3];
-        spin::thermal_xi(seed_lo, seed_hi, step, (u32)B + (u32)spec::NBASIS * cell, xi);
+        spin::thermal_xi(seed_lo, seed_hi, step, (u32)B + (u32)spec::NBASIS * cell, xi, image);
+        const double sg = __dmul_rn(specc::SIGMA[B], sigma_scale);
         // rounded products (never contracted into a following add): the cached and the regenerated thermal field are the same bits
-        f[0] = __dmul_rn(specc::SIGMA[B], xi[0]); f[1] = __dmul_rn(specc::SIGMA[B], xi[1]); f[2] = __dmul_rn(specc::SIGMA[B], xi[2]);
+        f[0] = __dmul_rn(sg, xi[0]); f[1] = __dmul_rn(sg, xi[1]); f[2] = __dmul_rn(sg, xi[2]);
     } else {
         f[0] = -0.0; f[1] = -0.0; f[2] = -0.0;      // additive identity that the compiler may fold away (x + -0.0 == x exactly)
     }
@@ -237,7 +240,8 @@ __device__ __forceinline__ bool is_pinned(const unsigned char *__restrict__ pin,
 
 template <int B, bool CG = false>
 __device__ __forceinline__ void predictor_body(const double *__restrict__ n, const double *__restrict__ fddi, double *__restrict__ np,
-                                               double *__restrict__ Aout, u64 step, u32 seed_lo, u32 seed_hi, const unsigned char *__restrict__ pin, int brick) {
+                                               double *__restrict__ Aout, u64 step, u32 seed_lo, u32 seed_hi, const unsigned char *__restrict__ pin, int brick,
+                                               u32 image = 0u, double sigma_scale = 1.0) {
     Coord c;
     int idx;
     if (!locate<B>(c, idx, brick)) return;
@@ -246,7 +250,7 @@ __device__ __forceinline__ void predictor_body(const double *__restrict__ n, con
     double own[1][3], F[1][3], sg[1][3] = {{0.0, 0.0, 0.0}};
     load3<0, CG>(cfg.cfg[0], own[0]);
     if (is_pinned<B>(pin, c)) { store_spin(np + idx, c, own[0]); return; }
-    thermal_force<B>(c, step, seed_lo, seed_hi, F[0]);
+    thermal_force<B>(c, step, seed_lo, seed_hi, F[0], image, sigma_scale);
     // the thermal field of the step is the same in both sweeps (R11): generating it costs two Philox blocks, two logarithms and three
     // trigonometric evaluations per spin, so the predictor keeps it for the corrector (24 B/spin written and read back)
     if constexpr (spec::CACHE_NOISE) store3(Aout + idx, F[0]);
@@ -265,7 +269,8 @@ __device__ __forceinline__ void predictor_body(const double *__restrict__ n, con
 template <int B, bool CG = false>
 __device__ __forceinline__ void corrector_body(const double *__restrict__ n, const double *__restrict__ np, const double *__restrict__ fddi_n,
                                                const double *__restrict__ fddi_np, const double *__restrict__ Ain, double *__restrict__ nout,
-                                               u64 step, u32 seed_lo, u32 seed_hi, const unsigned char *__restrict__ pin, int brick) {
+                                               u64 step, u32 seed_lo, u32 seed_hi, const unsigned char *__restrict__ pin, int brick, u32 image = 0u,
+                                               double sigma_scale = 1.0) {
     Coord c;
     int idx;
     if (!locate<B>(c, idx, brick)) return;
@@ -273,7 +278,7 @@ __device__ __forceinline__ void corrector_body(const double *__restrict__ n, con
     load3<0, CG>(n + idx, n0);
     if (is_pinned<B>(pin, c)) { store_spin(nout + idx, c, n0); return; }
     if constexpr (spec::CACHE_NOISE) load3<0, CG>(Ain + idx, th);
-    else thermal_force<B>(c, step, seed_lo, seed_hi, th);
+    else thermal_force<B>(c, step, seed_lo, seed_hi, th, image, sigma_scale);
     if constexpr (spec::SOLVER == 2) {
         // SIB corrector (C11): A at the midpoint configuration, the implicit-midpoint structure applied to n(t); A(n) is not needed
         const MidAcc<CG> cfg = {n + idx, np + idx};
@@ -416,10 +421,14 @@ __device__ __forceinline__ void dispatch_basis(int b, Fn &&fn) {
 extern "C" __global__ void SPIN_BOUNDS(spec::BX *spec::BY *spec::BZ)
     jit_predictor(const double *__restrict__ n, const double *__restrict__ fddi, double *__restrict__ np, double *__restrict__ Aout,
                   const unsigned long long *__restrict__ d_step, unsigned int step_add, unsigned int seed_lo, unsigned int seed_hi,
-                  const unsigned char *__restrict__ pin) {
+                  const unsigned char *__restrict__ pin, const double *__restrict__ img_sigma) {
     const unsigned long long step = *d_step + step_add;
+    // batched images: blockIdx.z selects the image; every per-spin array holds the images one after the other
+    const unsigned int image = blockIdx.z;
+    const size_t off = (size_t)image * ((size_t)spec::NBASIS * spec::SUB);
+    const double scale = img_sigma ? img_sigma[image] : 1.0;
     spinjit::dispatch_basis<0>((int)blockIdx.y, [&](auto b) {
-        spinjit::predictor_body<decltype(b)::value>(n, fddi, np, Aout, step, seed_lo, seed_hi, pin, (int)blockIdx.x);
+        spinjit::predictor_body<decltype(b)::value>(n + off, fddi + off, np + off, Aout + off, step, seed_lo, seed_hi, pin, (int)blockIdx.x, image, scale);
     });
 }
 
@@ -427,10 +436,14 @@ extern "C" __global__ void SPIN_BOUNDS(spec::BX *spec::BY *spec::BZ)
     jit_corrector(const double *__restrict__ n, const double *__restrict__ np, const double *__restrict__ fddi_n,
                   const double *__restrict__ fddi_np, const double *__restrict__ Ain, double *__restrict__ nout,
                   const unsigned long long *__restrict__ d_step, unsigned int step_add, unsigned int seed_lo, unsigned int seed_hi,
-                  const unsigned char *__restrict__ pin) {
+                  const unsigned char *__restrict__ pin, const double *__restrict__ img_sigma) {
     const unsigned long long step = *d_step + step_add;
+    const unsigned int image = blockIdx.z;
+    const size_t off = (size_t)image * ((size_t)spec::NBASIS * spec::SUB);
+    const double scale = img_sigma ? img_sigma[image] : 1.0;
     spinjit::dispatch_basis<0>((int)blockIdx.y, [&](auto b) {
-        spinjit::corrector_body<decltype(b)::value>(n, np, fddi_n, fddi_np, Ain, nout, step, seed_lo, seed_hi, pin, (int)blockIdx.x);
+        spinjit::corrector_body<decltype(b)::value>(n + off, np + off, fddi_n + off, fddi_np + off, Ain + off, nout + off, step, seed_lo, seed_hi, pin,
+                                                    (int)blockIdx.x, image, scale);
     });
 }
 

@@ -126,6 +126,10 @@ struct spin_system {
     double *d_result;              // reduction result (16 doubles)
     unsigned long long *d_step;    // device copy of the step counter (read by the kernels)
     unsigned char *d_pin;          // pinned-spin flags (boundary order), null if none
+    // ---- batched images: n_img independent configurations of the same lattice and Hamiltonian; every per-spin array holds them
+    // one after the other (stride nb * plan.sub doubles); the sweeps take the image from blockIdx.z
+    int n_img, img_sel;            // number of images; image that spins_set/get, effective_field, energy, ... address
+    double *d_img_sigma;           // per-image factor on the thermal amplitude, sqrt(T_image / T), or null (all 1)
     unsigned int *d_bar;           // arrival counter of the cooperative kernel's grid barrier
     double *d_vp;                  // velocity-projection state: ratio r, started flag, |F|^2
     bool vp_active;                // d_A holds the force of the previous VP iteration

@@ -643,3 +643,54 @@ def test_full_size_full_step_count(P, O, cfg, steps):
     d = np.abs(ng - no).max()
     print(f"FULL cfg{cfg} {w.n_cells} steps={steps}: max|dn| = {d:.3e}  (GPU {t1 - t0:.2f} s, oracle {t2 - t1:.1f} s on {o.threads} threads)")
     assert d <= SPIN_ATOL
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# Batched images: independent configurations advanced in the same launches
+@pytest.mark.parametrize("cfg,cells,steps", [(1, (37, 19, 1), 100), (2, (45, 33, 1), 100), (4, (33, 17, 1), 60), (5, (20, 12, 5), 10), (3, (35, 9, 7), 60)])
+def test_batched_images_match_independent_oracles(P, O, cfg, cells, steps):
+    w = W.CONFIGS[cfg]().resized(cells, steps)
+    n_img = 5
+    g = P.SpinSystem.from_workload(w)
+    g.spin_set_images(n_img)
+    temps = [w.T * f for f in (1.0, 0.25, 2.0, 0.0, 1.5)] if w.T > 0 else None
+    if temps:
+        g.llg_set_image_temperatures(temps)
+    starts = []
+    for m in range(n_img):
+        n0 = dataclasses.replace(w, seed=w.seed + 17 * m).initial_spins()
+        g.spin_select_image(m); g.spins_set(n0)
+        starts.append(n0)
+    oracles = []
+    for m in range(n_img):
+        wm = dataclasses.replace(w, T=temps[m]) if temps else w
+        o = O.OracleSystem.from_workload(wm); o.set_image(m); o.set_spins(starts[m])
+        oracles.append(o)
+    # fields and energies of every image before the run
+    for m in range(n_img):
+        g.spin_select_image(m)
+        assert_fields_close(g.effective_field(), oracles[m].effective_field())
+        To = oracles[m].energy_terms()
+        assert np.abs(g.energy()[1] - To).max() <= ENERGY_RTOL * np.abs(To).sum()
+    g.llg_iterate(steps)
+    worst = 0.0
+    for m in range(n_img):
+        oracles[m].iterate(steps)
+        g.spin_select_image(m)
+        worst = max(worst, np.abs(g.spins_get() - oracles[m].spins()).max())
+    print(f"images cfg{cfg}: worst max|dn| over {n_img} images = {worst:.3e}")
+    assert worst <= SPIN_ATOL
+    # image 0 of a batched run == the single-image run, bit for bit (when it runs at the reference temperature)
+    single = P.SpinSystem.from_workload(w); single.spin_set_option("use_coop", 0); single.spins_set(starts[0]); single.llg_iterate(steps)
+    g.spin_select_image(0)
+    assert np.array_equal(g.spins_get(), single.spins_get())
+    # shrinking keeps the first images, growing copies image 0
+    g.spin_select_image(1); keep1 = g.spins_get()
+    g.spin_set_images(2)
+    g.spin_select_image(1); assert np.array_equal(g.spins_get(), keep1)
+    g.spin_set_images(3)
+    g.spin_select_image(2); n2 = g.spins_get(); g.spin_select_image(0); assert np.array_equal(n2, g.spins_get())
+    with pytest.raises(P.SpinError):
+        g.spin_select_image(3)
+    with pytest.raises(P.SpinError):
+        g.minimise_vp(1, 0.1)
