@@ -694,3 +694,32 @@ def test_batched_images_match_independent_oracles(P, O, cfg, cells, steps):
         g.spin_select_image(3)
     with pytest.raises(P.SpinError):
         g.minimise_vp(1, 0.1)
+
+
+def test_stochastic_llg_temperature_sweep_orders_below_tc(P):
+    """Physics check of the thermal field on a coupled system (App. E, Fig. 13), with one image per temperature:
+    simple cubic ferromagnet, J = 1 meV, T_c = 1.44 J/k_B = 16.71 K (:139).  Time-averaged |M| falls monotonically with T, is
+    ordered well below T_c and disordered well above it (16^3 spins: the transition is rounded, so only the two sides are pinned)."""
+    w = dataclasses.replace(W.config3().resized((16, 16, 16), 1), pair_D=W.config3().pair_D * 0, B=0.0, T=10.0, alpha=0.5, dt_fs=5.0, seed=11)
+    temps = [4.0, 8.0, 12.0, 15.0, 18.0, 22.0, 30.0]
+    g = P.SpinSystem.from_workload(w)
+    g.spin_set_images(len(temps))
+    g.llg_set_image_temperatures(temps)
+    up = np.tile([0.0, 0.0, 1.0], (w.n_spins, 1))
+    for m in range(len(temps)):
+        g.spin_select_image(m); g.spins_set(up)
+    g.llg_iterate(6000)                                   # thermalise
+    acc = np.zeros(len(temps))
+    nsamp = 40
+    for _ in range(nsamp):
+        g.llg_iterate(150)
+        for m in range(len(temps)):
+            g.spin_select_image(m)
+            acc[m] += np.linalg.norm(g.observables()[0])
+    Mabs = acc / nsamp
+    print("T:", temps, "<|M|>:", np.round(Mabs, 3))
+    assert np.all(np.diff(Mabs) < 0.02)                   # monotone within sampling noise
+    assert Mabs[0] > 0.85 and Mabs[1] > 0.7               # ordered at T_c/4 and T_c/2
+    assert Mabs[-1] < 0.2 and Mabs[-2] < 0.3              # disordered at 1.3 T_c and 1.8 T_c
+    # spin-wave theory at low T: 1 - <|M|> grows linearly with T (classical spins): the 4 K and 8 K points give the same slope +-25 %
+    assert (1 - Mabs[1]) / (1 - Mabs[0]) == pytest.approx(2.0, rel=0.3)
