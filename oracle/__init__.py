@@ -69,6 +69,10 @@ def lib():
         L.orc_heun_step.argtypes = [vp]
         L.orc_set_solver.argtypes = [vp, C.c_int]
         L.orc_set_image.argtypes = [vp, C.c_uint32]
+        L.orc_gneb_forces.argtypes = [vp, C.c_int, dp, C.c_double, C.c_int, dp, dp, dp]
+        L.orc_gneb_iterate.argtypes = [vp, C.c_int, dp, C.c_long, C.c_double, C.c_double, C.c_int]
+        L.orc_geodesic_distance.argtypes = [vp, dp, dp]
+        L.orc_geodesic_distance.restype = C.c_double
         L.orc_set_pinned.argtypes = [vp, C.c_void_p]
         L.orc_vp_iterate.argtypes = [vp, C.c_long, C.c_double, C.c_double]
         L.orc_vp_reset.argtypes = [vp]
@@ -268,6 +272,23 @@ class OracleSystem:
         m = np.ascontiguousarray(np.asarray(mask).astype(np.uint8).reshape(-1))
         assert m.size == self.N
         lib().orc_set_pinned(self._h, m.ctypes.data_as(C.c_void_p))
+
+    def gneb_forces(self, chain, kappa=1.0, climbing=-1):
+        """chain: (M, N, 3).  Returns (F (M, N, 3), E (M,), l (M,) with l[nu] = geodesic distance nu -> nu+1)."""
+        ch = np.ascontiguousarray(np.asarray(chain, float)); M = ch.shape[0]
+        F = np.zeros_like(ch); E = np.zeros(M); l = np.zeros(M)
+        P = lambda a: a.ctypes.data_as(C.POINTER(C.c_double))
+        lib().orc_gneb_forces(self._h, M, P(ch), float(kappa), int(climbing), P(F), P(E), P(l))
+        return F, E, l
+
+    def gneb_iterate(self, chain, n_iter, step, kappa=1.0, climbing=-1):
+        ch = np.ascontiguousarray(np.asarray(chain, float)).copy(); M = ch.shape[0]
+        lib().orc_gneb_iterate(self._h, M, ch.ctypes.data_as(C.POINTER(C.c_double)), int(n_iter), float(step), float(kappa), int(climbing))
+        return ch
+
+    def geodesic_distance(self, a, b):
+        (x, px), (y, py) = _d(a), _d(b)
+        return float(lib().orc_geodesic_distance(self._h, px, py))
 
     def set_image(self, image):
         """Noise stream of image `image` (independent images of one batched system; 0 = single system)."""

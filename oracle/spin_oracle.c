@@ -15,6 +15,7 @@
  *   thermal field     Eq. 11 (:157-160)                     -> orc_thermal_xi, sigma
  *   Depondt solver    App. B, B5-B7 (:369-380)              -> orc_llg_step (solver 0)
  *   Heun solver       App. B, B3-B4 (:355-367)              -> orc_llg_step (solver 1); orc_heun_step = the same written on its own (pin)
+ *   GNEB forces       III.D Eqs. 14-17 (:193-216), App. F   -> orc_gneb_forces, orc_gneb_iterate, orc_geodesic_distance
  *   velocity projection App. D, D1-D5 (:438-463)            -> orc_vp_iterate
  *   topological charge App. A, A1-A2 (:317-343)             -> orc_topological_charge, orc_spherical_area
  *   RK4 solver        :168 (named only; textbook tableau)   -> orc_llg_step (solver 3), orc_rk4_step
@@ -937,6 +938,95 @@ void orc_vp_iterate(orc_system *s, long n_iter, double dt, double mass) {
             for (int k = 0; k < 3; ++k) s->n[3*i+k] = x[k] / nrm;                          /* D5 */
         }
         memcpy(s->vp_F, F, 3 * N * sizeof(double));
+    }
+    free(F);
+}
+
+/* ------------------------------------------------------------------ geodesic nudged elastic band, III.D (:193-216) and App. F
+ * A chain of M images (configurations) of the same system; chain[nu] points at 3N doubles.  One call computes, for every
+ * interior image, the total force of Eq. 14, F = F^S + F^E (3N-dimensional vectors):
+ *   tangent      "the definitions given in Ref. 55" (:212; Henkelman-Jonsson): tau+ = n_{nu+1} - n_nu, tau- = n_nu - n_{nu-1};
+ *                tau = tau+ if E_{nu+1} > E_nu > E_{nu-1}; tau- if E_{nu+1} < E_nu < E_{nu-1}; otherwise the mix
+ *                tau+ dEmax + tau- dEmin (E_{nu+1} > E_{nu-1}) or tau+ dEmin + tau- dEmax, dEmax/min = max/min |E_{nu+-1} - E_nu|;
+ *                then projected on the tangent space of the image, spin by spin (F1), and normalised in 3N dimensions
+ *   distance     l_{nu,mu}: geodesic, sqrt(sum_i angle(n_{nu,i}, n_{mu,i})^2) (:477 "the great-circle distance")
+ *   spring       F^S = kappa (l_{nu,nu+1} - l_{nu-1,nu}) tau (Eq. 15; the printed order of the two lengths would push an image
+ *                towards its nearer neighbour and bunch the chain up -- reading R31; kappa = 1 in the paper)
+ *   gradient     F^E = -grad E + (grad E . tau) tau (Eq. 16); climbing image: F^S = 0, F^E = -grad E + 2 (grad E . tau) tau (Eq. 17);
+ *                the total is projected on the tangent space spin by spin (F2)
+ * End images get zero force.  E_out[nu] receives the energies, l_out[nu] = l_{nu,nu+1}.  F_out: M x 3N.                  */
+static double geodesic_distance(long N, const double *a, const double *b) {
+    long double s2 = 0.0L;
+    for (long i = 0; i < N; ++i) {
+        double c[3]; cross3(a + 3*i, b + 3*i, c);
+        double ang = atan2(sqrt(dot3(c, c)), dot3(a + 3*i, b + 3*i));
+        s2 += (long double)ang * ang;
+    }
+    return (double)sqrtl(s2);
+}
+double orc_geodesic_distance(const orc_system *s, const double *a, const double *b) { return geodesic_distance(s->N, a, b); }
+void orc_gneb_forces(orc_system *s, int M, const double *chain, double kappa, int climbing, double *F_out, double *E_out, double *l_out) {
+    long N = s->N;
+    double *E = (double *)malloc(M * sizeof(double)), *l = (double *)calloc(M, sizeof(double));
+    double *G = (double *)malloc(3 * N * sizeof(double)), *tau = (double *)malloc(3 * N * sizeof(double));
+    for (int nu = 0; nu < M; ++nu) {
+        double Et[6]; orc_energy(s, chain + (size_t)nu * 3 * N, Et);
+        E[nu] = Et[0] + Et[1] + Et[2] + Et[3] + Et[4] + Et[5];
+        if (nu + 1 < M) l[nu] = geodesic_distance(N, chain + (size_t)nu * 3 * N, chain + (size_t)(nu + 1) * 3 * N);
+    }
+    memset(F_out, 0, (size_t)M * 3 * N * sizeof(double));
+    for (int nu = 1; nu + 1 < M; ++nu) {
+        const double *n = chain + (size_t)nu * 3 * N, *np_ = chain + (size_t)(nu + 1) * 3 * N, *nm = chain + (size_t)(nu - 1) * 3 * N;
+        double wp, wm;                                    /* tau = wp tau+ + wm tau- */
+        if (E[nu + 1] > E[nu] && E[nu] > E[nu - 1]) { wp = 1.0; wm = 0.0; }
+        else if (E[nu + 1] < E[nu] && E[nu] < E[nu - 1]) { wp = 0.0; wm = 1.0; }
+        else {
+            double dp = fabs(E[nu + 1] - E[nu]), dm = fabs(E[nu - 1] - E[nu]);
+            double dmax = dp > dm ? dp : dm, dmin = dp > dm ? dm : dp;
+            if (E[nu + 1] > E[nu - 1]) { wp = dmax; wm = dmin; } else { wp = dmin; wm = dmax; }
+            if (wp == 0.0 && wm == 0.0) { wp = 1.0; wm = 1.0; }      /* flat energy: the central difference */
+        }
+        long double t2 = 0.0L;
+        for (long i = 0; i < N; ++i) {
+            double t[3];
+            for (int k = 0; k < 3; ++k) t[k] = wp * (np_[3*i+k] - n[3*i+k]) + wm * (n[3*i+k] - nm[3*i+k]);
+            double p = dot3(t, n + 3*i);
+            for (int k = 0; k < 3; ++k) { tau[3*i+k] = t[k] - p * n[3*i+k]; t2 += (long double)tau[3*i+k] * tau[3*i+k]; }   /* F1 */
+        }
+        double tn = (double)sqrtl(t2);
+        for (long i = 0; i < 3 * N; ++i) tau[i] = tn > 0.0 ? tau[i] / tn : 0.0;
+        orc_gradient(s, n, G, T_ALL);                     /* G = -grad E */
+        if (s->pinned) for (long i = 0; i < N; ++i) if (s->pinned[i]) { G[3*i] = 0; G[3*i+1] = 0; G[3*i+2] = 0; }
+        long double gt = 0.0L;
+        for (long i = 0; i < 3 * N; ++i) gt += (long double)G[i] * tau[i];
+        double *F = F_out + (size_t)nu * 3 * N;
+        double cs = (nu == climbing) ? 0.0 : kappa * (l[nu] - l[nu - 1]);       /* Eq. 15 / 17 */
+        double ce = (nu == climbing) ? 2.0 * (double)gt : (double)gt;           /* Eq. 16 / 17: G - (G.tau) tau */
+        for (long i = 0; i < N; ++i) {
+            double f[3];
+            for (int k = 0; k < 3; ++k) f[k] = G[3*i+k] - ce * tau[3*i+k] + cs * tau[3*i+k];
+            double p = dot3(f, n + 3*i);
+            for (int k = 0; k < 3; ++k) F[3*i+k] = (s->pinned && s->pinned[i]) ? 0.0 : f[k] - p * n[3*i+k];             /* F2 */
+        }
+    }
+    if (E_out) memcpy(E_out, E, M * sizeof(double));
+    if (l_out) memcpy(l_out, l, M * sizeof(double));
+    free(E); free(l); free(G); free(tau);
+}
+/* one relaxation step of the chain: x <- x + step F, renormalised (plain steepest descent; the paper does not fix the optimiser) */
+void orc_gneb_iterate(orc_system *s, int M, double *chain, long n_iter, double step, double kappa, int climbing) {
+    long N = s->N;
+    double *F = (double *)malloc((size_t)M * 3 * N * sizeof(double));
+    for (long it = 0; it < n_iter; ++it) {
+        orc_gneb_forces(s, M, chain, kappa, climbing, F, NULL, NULL);
+        for (int nu = 1; nu + 1 < M; ++nu)
+            for (long i = 0; i < N; ++i) {
+                double *x = chain + (size_t)nu * 3 * N + 3 * i, *f = F + (size_t)nu * 3 * N + 3 * i, y[3];
+                if (s->pinned && s->pinned[i]) continue;
+                for (int k = 0; k < 3; ++k) y[k] = x[k] + step * f[k];
+                double nrm = sqrt(dot3(y, y));
+                for (int k = 0; k < 3; ++k) x[k] = y[k] / nrm;
+            }
     }
     free(F);
 }

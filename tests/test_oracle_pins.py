@@ -685,3 +685,70 @@ def test_image_noise_streams_are_independent():
     a = OracleSystem.from_workload(w); a.set_image(1); a.iterate(5)
     b = OracleSystem.from_workload(w); b.iterate(5)
     assert np.abs(a.spins() - b.spins()).max() > 1e-6
+
+
+# ------------------------------------------------------------------ GNEB forces (III.D Eqs. 14-17, App. F)
+def _single_spin(K=0.0, B=0.0):
+    s = OracleSystem(np.eye(3), [[0, 0, 0]], (1, 1, 1), (0, 0, 0))
+    s.set_mu_s([2.0]); s.set_field(B, (0, 0, 1))
+    if K:
+        s.set_anisotropy([0], [K], [[0, 0, 1]])
+    return s
+
+
+def _meridian(thetas, phi=0.3):
+    return np.array([[[math.sin(t) * math.cos(phi), math.sin(t) * math.sin(phi), math.cos(t)]] for t in thetas])
+
+
+def test_gneb_geodesic_distance_and_force_geometry():
+    """l is the great-circle distance, in 3N dimensions the root of the summed squared angles; F^E is orthogonal to the
+    tangent (Eq. 16), every force lies in the tangent space of its image (F2), end images get none."""
+    s = _single_spin(K=0.7, B=0.4)
+    a, b = _meridian([0.2])[0], _meridian([1.3])[0]
+    assert s.geodesic_distance(a, b) == pytest.approx(1.1, abs=1e-14)
+    w = small(1, (5, 4, 1))
+    o = OracleSystem.from_workload(w)
+    x, y = rand_spins(w.n_spins, 1), rand_spins(w.n_spins, 2)
+    ang = np.arccos(np.clip((x * y).sum(1), -1, 1))
+    assert o.geodesic_distance(x, y) == pytest.approx(math.sqrt((ang ** 2).sum()), rel=1e-12)
+    chain = np.array([rand_spins(w.n_spins, 10 + k) for k in range(5)])
+    F, E, l = o.gneb_forces(chain, kappa=0.0)
+    assert np.all(F[0] == 0) and np.all(F[-1] == 0)
+    for nu in (1, 2, 3):
+        assert np.abs((F[nu] * chain[nu]).sum(1)).max() < 1e-13                   # tangent to every spin
+        assert E[nu] == pytest.approx(o.energy(chain[nu]), rel=1e-14)
+    # pure spring force (no Hamiltonian): parallel to the tangent, i.e. to the projected central difference when E is flat
+    free = _single_spin()
+    ch = _meridian([0.1, 0.5, 1.6])
+    Fs, _, ls = free.gneb_forces(ch, kappa=2.0)
+    t = ch[2, 0] - ch[0, 0]; t -= np.dot(t, ch[1, 0]) * ch[1, 0]; t /= np.linalg.norm(t)
+    assert np.allclose(Fs[1, 0], 2.0 * (ls[1] - ls[0]) * t, atol=1e-14)             # towards the farther neighbour (reading R31)
+    assert ls[0] == pytest.approx(0.4, abs=1e-14) and ls[1] == pytest.approx(1.1, abs=1e-14)
+
+
+def test_gneb_springs_make_the_chain_equidistant():
+    """Eq. 15 "gives an equidistant distribution of images": on a flat energy surface unevenly spaced images relax to
+    equal geodesic spacing.  With the two lengths in the printed order the chain bunches up instead (reading R31)."""
+    free = _single_spin()
+    ch = _meridian([0.1, 0.2, 0.35, 1.9, 2.4])
+    out = free.gneb_iterate(ch, 400, 0.2, kappa=1.0)
+    l = [free.geodesic_distance(out[k], out[k + 1]) for k in range(4)]
+    assert max(l) - min(l) < 1e-6 and sum(l) == pytest.approx(2.3, abs=1e-9)
+
+
+def test_gneb_climbing_image_finds_the_anisotropy_barrier():
+    """One spin with easy axis z: the minimum-energy path from +z to -z is a meridian, the saddle is on the equator and the barrier
+    is exactly K (E = -K n_z^2).  The climbing image (Eq. 17) converges onto it."""
+    K = 0.8
+    s = _single_spin(K=K)
+    ch = _meridian(np.linspace(0.02, math.pi - 0.02, 9) + np.array([0, .05, -.04, .06, .1, -.03, .02, -.05, 0]))
+    ch[0, 0] = [0, 0, 1]; ch[-1, 0] = [0, 0, -1]
+    out = s.gneb_iterate(ch, 300, 0.2, kappa=1.0)
+    _, E, _ = s.gneb_forces(out)
+    ci = int(np.argmax(E))
+    out = s.gneb_iterate(out, 600, 0.2, kappa=1.0, climbing=ci)
+    F, E, l = s.gneb_forces(out, climbing=ci)
+    assert E[ci] - E[0] == pytest.approx(K, abs=1e-10)
+    assert abs(out[ci, 0, 2]) < 1e-6
+    assert np.abs(F).max() < 1e-6
+    assert max(l[:3]) - min(l[:3]) < 1e-3
