@@ -110,6 +110,16 @@ int spin_set_images(spin_system *sys, int n_images);
 int spin_select_image(spin_system *sys, int image);
 int llg_set_image_temperatures(spin_system *sys, const double *T_kelvin /*host, n_images, or NULL*/);
 
+/* Geodesic nudged elastic band on the batched images (III.D Eqs. 14-17 :193-216, App. F :475-489): the images are a chain, image 0
+ * and image n_images-1 its fixed ends.  Per interior image: tangent by the definitions of Ref. 55 (energy-weighted forward/backward
+ * differences), projected on the tangent space spin by spin (F1) and normalised in 3N dimensions; spring force kappa (l_{nu,nu+1} -
+ * l_{nu-1,nu}) tau with geodesic distances l (Eq. 15); gradient force -grad E + (grad E . tau) tau (Eq. 16); for the climbing image
+ * (index, or -1 for none) no spring and -grad E + 2 (grad E . tau) tau (Eq. 17); the total projected per spin (F2).
+ * gneb_forces returns F (host, n_images x 3N AoS, zero for the ends), the energies and l[nu] = l_{nu,nu+1}; any may be NULL.
+ * gneb_iterate relaxes the chain: x <- x + step F, renormalised, n_iterations times (step in 1/meV).  Blocking calls.        */
+int gneb_forces(spin_system *sys, double kappa, int climbing_image, double *F_xyz, double *E_meV, double *l_geodesic);
+int gneb_iterate(spin_system *sys, int64_t n_iterations, double step, double kappa, int climbing_image);
+
 /* Pinning and vacancies (:79 "pinning of individual spins or a set of spins", "defects, such as vacancies").  mask: N flags in
  * boundary index order, non-zero = pinned; NULL removes all pins.  A pinned spin is never updated by llg_iterate but acts on its
  * neighbours as usual.  A vacancy is a pinned site holding the zero vector: spins_set accepts a zero vector on pinned sites only;

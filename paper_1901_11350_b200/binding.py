@@ -19,7 +19,7 @@ EXPORTS = [
     "spin_geometry_create", "spin_system_destroy", "spin_system_nspins", "spin_set_stream",
     "hamiltonian_set_mu_s", "hamiltonian_set_field", "hamiltonian_set_anisotropy", "hamiltonian_set_pairs",
     "hamiltonian_set_exchange_shells", "hamiltonian_set_dmi_shells", "hamiltonian_set_quadruplets",
-    "hamiltonian_set_ddi", "spin_set_images", "spin_select_image", "llg_set_image_temperatures", "spins_set_pinned", "spins_set", "spins_get", "spins_set_device", "spins_get_device",
+    "hamiltonian_set_ddi", "spin_set_images", "spin_select_image", "llg_set_image_temperatures", "gneb_forces", "gneb_iterate", "spins_set_pinned", "spins_set", "spins_get", "spins_set_device", "spins_get_device",
     "llg_configure", "llg_set_solver", "minimise_vp", "minimise_vp_reset", "llg_iterate", "llg_get_step", "llg_set_step", "spin_synchronize",
     "effective_field", "effective_field_device", "energy", "observables", "topological_charge",
     "spin_launch_counts", "spin_profile_enable", "spin_profile_get", "spin_set_option",
@@ -65,6 +65,8 @@ def lib() -> C.CDLL:
         "llg_set_solver": (C.c_int, [vp, C.c_int]),
         "spins_set_pinned": (C.c_int, [vp, C.c_void_p]),
         "spin_set_images": (C.c_int, [vp, C.c_int]),
+        "gneb_forces": (C.c_int, [vp, C.c_double, C.c_int, dp, dp, dp]),
+        "gneb_iterate": (C.c_int, [vp, C.c_int64, C.c_double, C.c_double, C.c_int]),
         "spin_select_image": (C.c_int, [vp, C.c_int]),
         "llg_set_image_temperatures": (C.c_int, [vp, dp]),
         "minimise_vp": (C.c_int, [vp, C.c_int64, C.c_double, C.c_double]),
@@ -125,6 +127,7 @@ class SpinSystem:
         self._h = h
         self.n_basis = basis.shape[0]
         self.N = int(L.spin_system_nspins(h))
+        self.n_images = 1
 
     def close(self):
         if getattr(self, "_h", None):
@@ -224,7 +227,19 @@ class SpinSystem:
         j, jp = _d(j_dir)
         _check(lib().llg_configure(self._h, float(dt_fs), float(alpha), float(T), int(seed), float(u), jp, float(beta)))
 
+    def gneb_forces(self, kappa=1.0, climbing=-1):
+        """Returns (F (M, N, 3), E (M,), l (M,)) of the chain held in the batched images."""
+        M = self.n_images
+        F = np.zeros((M, self.N, 3)); E = np.zeros(M); l = np.zeros(M)
+        P_ = lambda a: a.ctypes.data_as(C.POINTER(C.c_double))
+        _check(lib().gneb_forces(self._h, float(kappa), int(climbing), P_(F), P_(E), P_(l)))
+        return F, E, l
+
+    def gneb_iterate(self, n_iterations, step, kappa=1.0, climbing=-1):
+        _check(lib().gneb_iterate(self._h, int(n_iterations), float(step), float(kappa), int(climbing)))
+
     def spin_set_images(self, n_images):
+        self.n_images = int(n_images)
         _check(lib().spin_set_images(self._h, int(n_images)))
 
     def spin_select_image(self, image):

@@ -1001,6 +1001,89 @@ extern "C" int minimise_vp_reset(spin_system *s) {
     return SPIN_OK;
 }
 
+// ---- GNEB on the batched images (III.D, App. F): images 0 and n_img-1 are the fixed ends of the chain
+namespace {
+int gneb_run(spin_system *s, int64_t n_iter, double step, double kappa, int climbing, bool want_outputs, double *F_host, double *E_host, double *l_host) {
+    const int M = s->n_img;
+    const Launch L = brick_launch(s);
+    const int nblocks = (int)(L.grid.x * L.grid.y);
+    const size_t istr = (size_t)s->nb * s->plan.sub;
+    double *d_part = nullptr, *d_sc = nullptr, *d_E = nullptr;
+    SPIN_CUDA(cudaMalloc(&d_part, (size_t)M * nblocks * 3 * sizeof(double)));
+    SPIN_CUDA(cudaMalloc(&d_sc, (size_t)M * 3 * sizeof(double)));
+    SPIN_CUDA(cudaMalloc(&d_E, (size_t)M * sizeof(double)));
+    std::vector<double> E((size_t)M);
+    const int sel = s->img_sel;
+    int rc = SPIN_OK;
+    dim3 grid(L.grid.x, L.grid.y, (unsigned)M);
+    double *n_all = s->d_n[s->cur], *G_all = s->d_np, *tau_all = s->d_A;
+    for (int64_t it = 0; it < n_iter && rc == SPIN_OK; ++it) {
+        for (int nu = 0; nu < M && rc == SPIN_OK; ++nu) {          // energy and force of every image
+            s->img_sel = nu;
+            double r[N_RED];
+            rc = reduce_all(s, r);
+            E[(size_t)nu] = r[0] + r[1] + r[2] + r[3] + r[4] + r[5];
+            if (rc == SPIN_OK) rc = enqueue_force(s, T_ALL, G_all + nu * istr);
+        }
+        if (rc) break;
+        cudaMemcpyAsync(d_E, E.data(), (size_t)M * sizeof(double), cudaMemcpyHostToDevice, s->stream);
+        const double st = want_outputs ? 0.0 : step;
+        if (L.flat) {
+            gneb_tangent_kernel<32, 8, 1><<<grid, L.block, 0, s->stream>>>(s->plan, n_all, G_all, d_E, M, istr, tau_all, d_part);
+            gneb_final_kernel<<<M, 32, 0, s->stream>>>(d_part, nblocks, d_sc);
+            gneb_assemble_kernel<32, 8, 1><<<grid, L.block, 0, s->stream>>>(s->plan, n_all, G_all, tau_all, d_sc, M, istr, kappa, climbing, st);
+        } else {
+            gneb_tangent_kernel<32, 4, 2><<<grid, L.block, 0, s->stream>>>(s->plan, n_all, G_all, d_E, M, istr, tau_all, d_part);
+            gneb_final_kernel<<<M, 32, 0, s->stream>>>(d_part, nblocks, d_sc);
+            gneb_assemble_kernel<32, 4, 2><<<grid, L.block, 0, s->stream>>>(s->plan, n_all, G_all, tau_all, d_sc, M, istr, kappa, climbing, st);
+        }
+        s->n_launch += 3;
+        cudaError_t e = cudaStreamSynchronize(s->stream);        // E (host vector) is reused by the next iteration
+        if (e != cudaSuccess) rc = spin::fail(SPIN_ERR_CUDA, "gneb: %s", cudaGetErrorString(e));
+    }
+    if (rc == SPIN_OK && want_outputs) {
+        if (E_host) memcpy(E_host, E.data(), (size_t)M * sizeof(double));
+        if (l_host) {
+            std::vector<double> sc((size_t)3 * M);
+            cudaMemcpy(sc.data(), d_sc, sc.size() * sizeof(double), cudaMemcpyDeviceToHost);
+            for (int nu = 0; nu < M; ++nu) l_host[nu] = sc[(size_t)3 * nu + 2];
+        }
+        if (F_host) {
+            const int nt = 256;
+            for (int nu = 0; nu < M; ++nu) {
+                unpack_kernel<<<(unsigned)((s->N + nt - 1) / nt), nt, 0, s->stream>>>(s->plan, G_all + nu * istr, s->d_aos, (int)s->N, 0);
+                s->n_launch++;
+                cudaMemcpyAsync(F_host + (size_t)nu * 3 * s->N, s->d_aos, (size_t)3 * s->N * sizeof(double), cudaMemcpyDeviceToHost, s->stream);
+                cudaStreamSynchronize(s->stream);
+            }
+        }
+    }
+    s->img_sel = sel;
+    cudaFree(d_part); cudaFree(d_sc); cudaFree(d_E);
+    if (rc == SPIN_OK && cudaGetLastError() != cudaSuccess) rc = spin::fail(SPIN_ERR_CUDA, "gneb: kernel launch failed");
+    return rc;
+}
+}  // namespace
+
+extern "C" int gneb_forces(spin_system *s, double kappa, int climbing_image, double *F_xyz, double *E_meV, double *l_geodesic) {
+    REQUIRE(s, "null system");
+    REQUIRE(s->n_img >= 3, "a chain needs at least 3 images (spin_set_images)");
+    REQUIRE(climbing_image < s->n_img, "climbing image out of range");
+    int rc = ensure_plan(s);
+    if (rc) return rc;
+    s->vp_active = false;
+    return gneb_run(s, 1, 0.0, kappa, climbing_image, true, F_xyz, E_meV, l_geodesic);
+}
+extern "C" int gneb_iterate(spin_system *s, int64_t n_iterations, double step, double kappa, int climbing_image) {
+    REQUIRE(s && n_iterations >= 0 && step > 0.0 && isfinite(step), "bad argument");
+    REQUIRE(s->n_img >= 3, "a chain needs at least 3 images (spin_set_images)");
+    REQUIRE(climbing_image < s->n_img, "climbing image out of range");
+    int rc = ensure_plan(s);
+    if (rc) return rc;
+    s->vp_active = false;
+    return gneb_run(s, n_iterations, step, kappa, climbing_image, false, nullptr, nullptr, nullptr);
+}
+
 // Q of App. A summed over the a-b planes; one basis atom
 extern "C" int topological_charge(spin_system *s, double *Q) {
     REQUIRE(s && Q, "null argument");

@@ -439,6 +439,110 @@ __global__ void __launch_bounds__(BX *BY *BZ)
     store_spin(P, n, s.ia, s.ib, s.ic, s.idx, x);
 }
 
+// ---------------------------------------------------------------------------------------------------------
+// Geodesic nudged elastic band, III.D Eqs. 14-17 and App. F, on a batch of images (blockIdx.z = image nu).
+// gneb_tangent_kernel: raw tangent of every interior image (Henkelman-Jonsson weights from the energies, projected on the tangent
+// space spin by spin, F1) and per-block partial sums of |tau|^2, G.tau (G = -grad E of the image) and of the squared angle to the
+// next image (geodesic distance).  gneb_final_kernel folds them in a fixed order.  gneb_assemble_kernel builds
+// F = G - c_E tau^ + c_S tau^ with c_E = (G.tau^) (twice that for the climbing image), c_S = kappa (l_{nu,nu+1} - l_{nu-1,nu}) (0 for the
+// climbing image), projects it (F2), stores it over G and, if step > 0, moves the image: x <- x + step F, renormalised.
+template <int BX, int BY, int BZ>
+__global__ void __launch_bounds__(BX *BY *BZ)
+    gneb_tangent_kernel(const __grid_constant__ DevicePlan P, const double *__restrict__ n_all, const double *__restrict__ G_all,
+                        const double *__restrict__ E, int M, size_t istr, double *__restrict__ tau_all, double *__restrict__ partials) {
+    constexpr int NW = BX * BY * BZ / 32;
+    __shared__ double sh[3][NW];
+    const int nu = blockIdx.z;
+    const Site s = locate<BX, BY, BZ>(P);
+    double t2 = 0.0, gt = 0.0, a2 = 0.0;
+    if (s.valid) {
+        double x[3], xp[3];
+        load3(P, n_all + nu * istr, s.idx, x);
+        if (nu + 1 < M) {
+            load3(P, n_all + (nu + 1) * istr, s.idx, xp);
+            const double cx = x[1] * xp[2] - x[2] * xp[1], cy = x[2] * xp[0] - x[0] * xp[2], cz = x[0] * xp[1] - x[1] * xp[0];
+            const double ang = atan2(sqrt(cx * cx + cy * cy + cz * cz), x[0] * xp[0] + x[1] * xp[1] + x[2] * xp[2]);
+            a2 = ang * ang;
+        }
+        if (nu > 0 && nu + 1 < M) {
+            double xm[3], g[3];
+            load3(P, n_all + (nu - 1) * istr, s.idx, xm);
+            double wp, wm;
+            const double Ep = E[nu + 1], E0 = E[nu], Em = E[nu - 1];
+            if (Ep > E0 && E0 > Em) { wp = 1.0; wm = 0.0; }
+            else if (Ep < E0 && E0 < Em) { wp = 0.0; wm = 1.0; }
+            else {
+                const double dp = fabs(Ep - E0), dm = fabs(Em - E0), dmax = fmax(dp, dm), dmin = fmin(dp, dm);
+                if (Ep > Em) { wp = dmax; wm = dmin; } else { wp = dmin; wm = dmax; }
+                if (wp == 0.0 && wm == 0.0) { wp = 1.0; wm = 1.0; }
+            }
+            double t[3] = {wp * (xp[0] - x[0]) + wm * (x[0] - xm[0]), wp * (xp[1] - x[1]) + wm * (x[1] - xm[1]), wp * (xp[2] - x[2]) + wm * (x[2] - xm[2])};
+            const double p = t[0] * x[0] + t[1] * x[1] + t[2] * x[2];
+            t[0] -= p * x[0]; t[1] -= p * x[1]; t[2] -= p * x[2];
+            store3(P, tau_all + nu * istr, s.idx, t);
+            load3(P, G_all + nu * istr, s.idx, g);
+            if (pinned(P, s)) { g[0] = 0.0; g[1] = 0.0; g[2] = 0.0; }
+            t2 = t[0] * t[0] + t[1] * t[1] + t[2] * t[2];
+            gt = g[0] * t[0] + g[1] * t[1] + g[2] * t[2];
+        }
+    }
+    t2 = warp_sum(t2); gt = warp_sum(gt); a2 = warp_sum(a2);
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    if (lane == 0) { sh[0][w] = t2; sh[1][w] = gt; sh[2][w] = a2; }
+    __syncthreads();
+    if (threadIdx.x < 3) {
+        double r = sh[threadIdx.x][0];
+        for (int i = 1; i < NW; ++i) r += sh[threadIdx.x][i];
+        const size_t nblocks = (size_t)gridDim.x * gridDim.y;
+        partials[((size_t)nu * nblocks + (size_t)blockIdx.y * gridDim.x + blockIdx.x) * 3 + threadIdx.x] = r;
+    }
+}
+// one warp per image: sc[nu] = {|tau|, G.tau^, l_{nu,nu+1}}
+__global__ void gneb_final_kernel(const double *__restrict__ partials, int nblocks, double *__restrict__ sc) {
+    const int nu = blockIdx.x;
+    double v[3] = {0.0, 0.0, 0.0};
+    for (int i = threadIdx.x; i < nblocks; i += 32)
+        for (int k = 0; k < 3; ++k) v[k] += partials[((size_t)nu * nblocks + i) * 3 + k];
+    for (int k = 0; k < 3; ++k) v[k] = warp_sum(v[k]);
+    if (threadIdx.x == 0) {
+        const double tn = sqrt(v[0]);
+        sc[3 * nu + 0] = tn;
+        sc[3 * nu + 1] = tn > 0.0 ? v[1] / tn : 0.0;
+        sc[3 * nu + 2] = sqrt(v[2]);
+    }
+}
+template <int BX, int BY, int BZ>
+__global__ void __launch_bounds__(BX *BY *BZ)
+    gneb_assemble_kernel(const __grid_constant__ DevicePlan P, double *__restrict__ n_all, double *__restrict__ G_all,
+                         const double *__restrict__ tau_all, const double *__restrict__ sc, int M, size_t istr, double kappa, int climbing,
+                         double step) {
+    const int nu = blockIdx.z;
+    const Site s = locate<BX, BY, BZ>(P);
+    if (!s.valid) return;
+    double f[3] = {0.0, 0.0, 0.0};
+    const bool interior = nu > 0 && nu + 1 < M;
+    if (interior && !pinned(P, s)) {
+        double x[3], g[3], t[3];
+        load3(P, n_all + nu * istr, s.idx, x);
+        load3(P, G_all + nu * istr, s.idx, g);
+        load3(P, tau_all + nu * istr, s.idx, t);
+        const double tn = sc[3 * nu], inv = tn > 0.0 ? 1.0 / tn : 0.0;
+        t[0] *= inv; t[1] *= inv; t[2] *= inv;
+        const double cs = (nu == climbing) ? 0.0 : kappa * (sc[3 * nu + 2] - sc[3 * (nu - 1) + 2]);
+        const double ce = (nu == climbing) ? 2.0 * sc[3 * nu + 1] : sc[3 * nu + 1];
+        f[0] = g[0] - ce * t[0] + cs * t[0]; f[1] = g[1] - ce * t[1] + cs * t[1]; f[2] = g[2] - ce * t[2] + cs * t[2];
+        const double p = f[0] * x[0] + f[1] * x[1] + f[2] * x[2];
+        f[0] -= p * x[0]; f[1] -= p * x[1]; f[2] -= p * x[2];
+        if (step > 0.0) {
+            x[0] += step * f[0]; x[1] += step * f[1]; x[2] += step * f[2];
+            const double r = 1.0 / sqrt(x[0] * x[0] + x[1] * x[1] + x[2] * x[2]);
+            x[0] *= r; x[1] *= r; x[2] *= r;
+            store_spin(P, n_all + nu * istr, s.ia, s.ib, s.ic, s.idx, x);
+        }
+    }
+    store3(P, G_all + nu * istr, s.idx, f);
+}
+
 // Topological charge, App. A: Q = (1/4 pi) sum_l A_l over the two elementary triangles of every cell of every
 // a-b plane; A_l = signed area of the spherical triangle (n_i, n_j, n_k), evaluated as 2 atan2(n_i.(n_j x n_k), 1 + n_i.n_j +
 // n_j.n_k + n_k.n_i) -- the same angle as Eq. A2 with its sign rule, without the square root and the acos near +-1.

@@ -723,3 +723,64 @@ def test_stochastic_llg_temperature_sweep_orders_below_tc(P):
     assert Mabs[-1] < 0.2 and Mabs[-2] < 0.3              # disordered at 1.3 T_c and 1.8 T_c
     # spin-wave theory at low T: 1 - <|M|> grows linearly with T (classical spins): the 4 K and 8 K points give the same slope +-25 %
     assert (1 - Mabs[1]) / (1 - Mabs[0]) == pytest.approx(2.0, rel=0.3)
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# GNEB forces on the batched images (III.D Eqs. 14-17, App. F)
+@pytest.mark.parametrize("cfg,cells", [(1, (13, 9, 1)), (3, (9, 5, 6)), (4, (9, 7, 1)), (5, (8, 6, 4))])
+def test_gneb_forces_and_relaxation_parity(P, O, cfg, cells):
+    w = dataclasses.replace(W.CONFIGS[cfg]().resized(cells, 1), T=0.0)
+    M = 6
+    # a chain between two random configurations: normalised linear interpolation plus a little noise
+    a, b = w.initial_spins(), dataclasses.replace(w, seed=w.seed + 5).initial_spins()
+    rng = np.random.default_rng(3)
+    chain = []
+    for k in range(M):
+        x = (1 - k / (M - 1)) * a + (k / (M - 1)) * b + 0.05 * rng.standard_normal(a.shape)
+        chain.append(x / np.linalg.norm(x, axis=1, keepdims=True))
+    chain = np.array(chain)
+    g = P.SpinSystem.from_workload(w); o = O.OracleSystem.from_workload(w)
+    g.spin_set_images(M)
+    for k in range(M):
+        g.spin_select_image(k); g.spins_set(chain[k])
+    for climbing in (-1, 3):
+        Fg, Eg, lg = g.gneb_forces(kappa=0.7, climbing=climbing)
+        Fo, Eo, lo = o.gneb_forces(chain, kappa=0.7, climbing=climbing)
+        assert np.abs(Eg - Eo).max() <= 1e-12 * np.abs(Eo).max()
+        assert np.abs(lg[:-1] - lo[:-1]).max() <= 1e-12 * lo.max()
+        assert np.abs(Fg - Fo).max() <= 1e-11 * np.abs(Fo).max(), (climbing, np.abs(Fg - Fo).max(), np.abs(Fo).max())
+        assert np.all(Fg[0] == 0) and np.all(Fg[-1] == 0)
+    g.gneb_iterate(25, 0.02, kappa=0.7, climbing=-1)
+    out = o.gneb_iterate(chain, 25, 0.02, kappa=0.7, climbing=-1)
+    worst = 0.0
+    for k in range(M):
+        g.spin_select_image(k)
+        worst = max(worst, np.abs(g.spins_get() - out[k]).max())
+    print(f"gneb cfg{cfg}: worst max|dn| after 25 iterations = {worst:.3e}")
+    assert worst <= SPIN_ATOL
+    _, E1, _ = g.gneb_forces(kappa=0.7)
+    assert E1[1:-1].sum() < Eo[1:-1].sum()                   # the interior images moved downhill
+
+
+def test_gneb_climbing_image_finds_the_anisotropy_barrier_on_the_gpu(P):
+    """Same closed form as the oracle pin: one spin, easy axis z, barrier exactly K, saddle on the equator."""
+    K = 0.8
+    s = P.SpinSystem(np.eye(3), [[0, 0, 0]], (1, 1, 1), (0, 0, 0))
+    s.hamiltonian_set_mu_s([2.0]); s.hamiltonian_set_anisotropy([0], [K], [[0, 0, 1]])
+    th = np.linspace(0.02, np.pi - 0.02, 9) + np.array([0, .05, -.04, .06, .1, -.03, .02, -.05, 0])
+    s.spin_set_images(9)
+    for k, t in enumerate(th):
+        v = [np.sin(t) * np.cos(0.3), np.sin(t) * np.sin(0.3), np.cos(t)]
+        if k == 0: v = [0, 0, 1]
+        if k == 8: v = [0, 0, -1]
+        s.spin_select_image(k); s.spins_set([v])
+    s.gneb_iterate(300, 0.2, kappa=1.0)
+    _, E, _ = s.gneb_forces()
+    ci = int(np.argmax(E))
+    s.gneb_iterate(600, 0.2, kappa=1.0, climbing=ci)
+    F, E, l = s.gneb_forces(climbing=ci)
+    assert E[ci] - E[0] == pytest.approx(K, abs=1e-10)
+    s.spin_select_image(ci)
+    assert abs(s.spins_get()[0, 2]) < 1e-6 and np.abs(F).max() < 1e-6
+    with pytest.raises(P.SpinError):
+        P.SpinSystem.from_workload(W.config1().resized((4, 4, 1), 1)).gneb_iterate(1, 0.1)      # no chain
