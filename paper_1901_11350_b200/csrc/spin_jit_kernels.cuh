@@ -424,9 +424,9 @@ extern "C" __global__ void SPIN_BOUNDS(spec::BX *spec::BY *spec::BZ)
                   const unsigned char *__restrict__ pin, const double *__restrict__ img_sigma) {
     const unsigned long long step = *d_step + step_add;
     // batched images: blockIdx.z selects the image; every per-spin array holds the images one after the other
-    const unsigned int image = blockIdx.z;
-    const size_t off = (size_t)image * ((size_t)spec::NBASIS * spec::SUB);
-    const double scale = img_sigma ? img_sigma[image] : 1.0;
+    const unsigned int image = spec::MULTI_IMAGE ? blockIdx.z : 0u;
+    const size_t off = spec::MULTI_IMAGE ? (size_t)image * ((size_t)spec::NBASIS * spec::SUB) : (size_t)0;
+    const double scale = (spec::MULTI_IMAGE && img_sigma) ? img_sigma[image] : 1.0;
     spinjit::dispatch_basis<0>((int)blockIdx.y, [&](auto b) {
         spinjit::predictor_body<decltype(b)::value>(n + off, fddi + off, np + off, Aout + off, step, seed_lo, seed_hi, pin, (int)blockIdx.x, image, scale);
     });
@@ -438,9 +438,9 @@ extern "C" __global__ void SPIN_BOUNDS(spec::BX *spec::BY *spec::BZ)
                   const unsigned long long *__restrict__ d_step, unsigned int step_add, unsigned int seed_lo, unsigned int seed_hi,
                   const unsigned char *__restrict__ pin, const double *__restrict__ img_sigma) {
     const unsigned long long step = *d_step + step_add;
-    const unsigned int image = blockIdx.z;
-    const size_t off = (size_t)image * ((size_t)spec::NBASIS * spec::SUB);
-    const double scale = img_sigma ? img_sigma[image] : 1.0;
+    const unsigned int image = spec::MULTI_IMAGE ? blockIdx.z : 0u;
+    const size_t off = spec::MULTI_IMAGE ? (size_t)image * ((size_t)spec::NBASIS * spec::SUB) : (size_t)0;
+    const double scale = (spec::MULTI_IMAGE && img_sigma) ? img_sigma[image] : 1.0;
     spinjit::dispatch_basis<0>((int)blockIdx.y, [&](auto b) {
         spinjit::corrector_body<decltype(b)::value>(n + off, np + off, fddi_n + off, fddi_np + off, Ain + off, nout + off, step, seed_lo, seed_hi, pin,
                                                     (int)blockIdx.x, image, scale);
