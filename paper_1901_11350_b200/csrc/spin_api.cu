@@ -852,7 +852,7 @@ extern "C" int llg_iterate(spin_system *s, int64_t n_steps) {
     // (a grid barrier costs about as much as a launch inside a CUDA graph, and it empties L1), so the limit is low; option
     // use_coop = 2 forces it for any lattice without dipolar coupling.
     const int64_t COOP_CHUNK = 8192;
-    if (s->opt_coop && !s->profile_on && !s->ddi_on && (s->N <= SPIN_COOP_MAX_SPINS || s->opt_coop == 2) && jit_coop_ready(s) && !jit_fused_ready(s) &&
+    if (s->opt_coop && !s->profile_on && !s->ddi_on && (s->N <= SPIN_COOP_MAX_SPINS || s->opt_coop >= 2) && jit_coop_ready(s) && !jit_fused_ready(s) &&
         n_steps > 0) {
         while (done < n_steps) {
             const unsigned chunk = (unsigned)std::min<int64_t>(COOP_CHUNK, n_steps - done);
@@ -1130,7 +1130,7 @@ extern "C" int spin_set_option(spin_system *s, const char *name, int value) {
     else if (!strcmp(name, "store_A")) { s->opt_store_A = value ? 1 : 0; s->plan_dirty = true; }
     else if (!strcmp(name, "use_jit")) { s->opt_jit = value ? 1 : 0; s->plan_dirty = true; }
     else if (!strcmp(name, "use_fused")) { s->opt_fused = value < 0 ? 0 : (value > 2 ? 2 : value); s->plan_dirty = true; }
-    else if (!strcmp(name, "use_coop")) { s->opt_coop = value < 0 ? 0 : (value > 2 ? 2 : value); s->plan_dirty = true; }
+    else if (!strcmp(name, "use_coop")) { s->opt_coop = value < 0 ? 0 : (value > 3 ? 3 : value); s->plan_dirty = true; }
     else if (!strcmp(name, "cache_noise")) { s->opt_cache_noise = value ? 1 : 0; s->plan_dirty = true; }
     else if (!strcmp(name, "use_col")) { s->opt_col = value ? 1 : 0; s->plan_dirty = true; }
     else if (!strcmp(name, "ddi_slab")) { s->opt_ddi_slab = value ? 1 : 0; s->plan_dirty = true; }
@@ -1145,7 +1145,7 @@ extern "C" int spin_kernel_info(spin_system *s, char *buf, int len) {
     REQUIRE(s && buf && len > 0, "bad argument");
     if (s->has_device) { int rc = ensure_plan(s); if (rc) return rc; }
     if (jit_fused_ready(s)) snprintf(buf, (size_t)len, "jit+fused");
-    else if (jit_coop_ready(s) && s->opt_coop && !s->ddi_on && (s->N <= SPIN_COOP_MAX_SPINS || s->opt_coop == 2)) snprintf(buf, (size_t)len, "jit+coop");
+    else if (jit_coop_ready(s) && s->opt_coop && !s->ddi_on && (s->N <= SPIN_COOP_MAX_SPINS || s->opt_coop >= 2)) snprintf(buf, (size_t)len, jit_cluster_ready(s) ? "jit+cluster" : "jit+coop");
     else if (jit_col_ready(s)) snprintf(buf, (size_t)len, "jit+col");
     else if (jit_tma_ready(s)) snprintf(buf, (size_t)len, "jit+tma");
     else if (jit_ready(s)) snprintf(buf, (size_t)len, "jit (brick kernels: %s)", jit_tma_note(s));

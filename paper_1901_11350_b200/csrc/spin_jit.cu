@@ -47,6 +47,8 @@ struct JitState {
     bool coop;
     cudaKernel_t k_coop;
     int coop_grid;
+    bool cluster;             // the whole lattice is one thread-block cluster (<= 16 bricks): hardware barrier instead of the grid barrier
+    cudaKernel_t k_cluster;
     // column-marching sweeps
     bool col;
     cudaKernel_t k_pred_col, k_corr_col;
@@ -417,6 +419,7 @@ static void variants_prepare(spin_system *s, JitState *j) {
         if (fe != cudaSuccess) { cudaGetLastError(); j->fused = false; }
     }
     j->coop = false;
+    j->cluster = false;
     if (s->opt_coop && !s->ddi_on && s->solver != SPIN_SOLVER_RK4 && s->n_img == 1) {
         int dev = 0, can = 0, occ = 0;
         cudaGetDevice(&dev);
@@ -430,6 +433,26 @@ static void variants_prepare(spin_system *s, JitState *j) {
             j->coop = true;
         } else {
             cudaGetLastError();
+        }
+        // one cluster for the whole lattice: up to 8 blocks is portable, up to 16 needs the non-portable opt-in
+        j->cluster = false;
+        const int items = (int)(grid.x * grid.y);
+        if (j->coop && s->opt_coop != 3 && items <= 16) {
+            cudaError_t ke = cudaLibraryGetKernel(&j->k_cluster, j->lib, "jit_steps_cluster");
+            if (ke == cudaSuccess && items > 8) ke = cudaFuncSetAttribute((const void *)j->k_cluster, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+            if (ke == cudaSuccess) {
+                cudaLaunchConfig_t cfg;
+                memset(&cfg, 0, sizeof(cfg));
+                cfg.gridDim = dim3((unsigned)items); cfg.blockDim = block;
+                cudaLaunchAttribute at;
+                at.id = cudaLaunchAttributeClusterDimension;
+                at.val.clusterDim.x = (unsigned)items; at.val.clusterDim.y = 1; at.val.clusterDim.z = 1;
+                cfg.attrs = &at; cfg.numAttrs = 1;
+                int nclusters = 0;
+                ke = cudaOccupancyMaxActiveClusters(&nclusters, (const void *)j->k_cluster, &cfg);
+                if (ke == cudaSuccess && nclusters >= 1) j->cluster = true;
+            }
+            if (ke != cudaSuccess) cudaGetLastError();
         }
     }
     j->col = plan_col(s, j->col_geo);
@@ -527,6 +550,7 @@ int spin::jit_launch_fused(spin_system *s, const double *n, double *nout, unsign
 }
 
 bool spin::jit_coop_ready(const spin_system *s) { return s->jit && s->jit->loaded && s->jit->coop; }
+bool spin::jit_cluster_ready(const spin_system *s) { return jit_coop_ready(s) && s->jit->cluster; }
 
 // nsteps Depondt/Heun/SIB steps in one cooperative launch; reads n from d_n[cur], leaves the result in d_n[cur ^ (nsteps & 1)]
 int spin::jit_launch_steps_coop(spin_system *s, unsigned nsteps) {
@@ -536,11 +560,24 @@ int spin::jit_launch_steps_coop(spin_system *s, unsigned nsteps) {
     double *n0 = s->d_n[s->cur], *n1 = s->d_n[s->cur ^ 1], *np = s->d_np, *aux = s->d_A;
     const unsigned char *pin = s->d_pin;
     unsigned int *bar = s->d_bar;
+    dim3 grid, block;
+    jit_brick_launch(s, grid, block);
+    if (j->cluster) {
+        void *cargs[] = {(void *)&n0, (void *)&n1, (void *)&np, (void *)&aux, (void *)&d_step, (void *)&nsteps, (void *)&seed_lo, (void *)&seed_hi, (void *)&pin};
+        const unsigned items = grid.x * grid.y;
+        cudaLaunchConfig_t cfg;
+        memset(&cfg, 0, sizeof(cfg));
+        cfg.gridDim = dim3(items); cfg.blockDim = block; cfg.stream = s->stream;
+        cudaLaunchAttribute at;
+        at.id = cudaLaunchAttributeClusterDimension;
+        at.val.clusterDim.x = items; at.val.clusterDim.y = 1; at.val.clusterDim.z = 1;
+        cfg.attrs = &at; cfg.numAttrs = 1;
+        SPIN_CUDA(cudaLaunchKernelExC(&cfg, (const void *)j->k_cluster, cargs));
+        return SPIN_OK;
+    }
     SPIN_CUDA(cudaMemsetAsync(bar, 0, sizeof(unsigned int), s->stream));
     void *args[] = {(void *)&n0, (void *)&n1, (void *)&np, (void *)&aux, (void *)&d_step, (void *)&nsteps, (void *)&seed_lo, (void *)&seed_hi,
                     (void *)&pin, (void *)&bar};
-    dim3 grid, block;
-    jit_brick_launch(s, grid, block);
     SPIN_CUDA(cudaLaunchCooperativeKernel((const void *)j->k_coop, dim3((unsigned)j->coop_grid), block, args, 0, s->stream));
     return SPIN_OK;
 }

@@ -481,29 +481,51 @@ __device__ __forceinline__ void grid_barrier(unsigned int *bar, unsigned int nbl
 }
 }  // namespace spinjit
 
-extern "C" __global__ void SPIN_BOUNDS(spec::BX *spec::BY *spec::BZ)
-    jit_steps_coop(double *__restrict__ n0, double *__restrict__ n1, double *__restrict__ np, double *__restrict__ aux,
-                   const unsigned long long *__restrict__ d_step, unsigned int nsteps, unsigned int seed_lo, unsigned int seed_hi,
-                   const unsigned char *__restrict__ pin, unsigned int *bar) {
-    using namespace spinjit;
+namespace spinjit {
+// hardware barrier of a thread-block cluster: every thread of every block arrives (release) and waits (acquire); cluster scope orders
+// the global-memory traffic of the blocks just like the grid barrier above, at a fraction of its latency
+__device__ __forceinline__ void cluster_barrier() {
+    asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
+    asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+
+template <class Barrier>
+__device__ __forceinline__ void all_steps(double *__restrict__ n0, double *__restrict__ n1, double *__restrict__ np, double *__restrict__ aux,
+                                          u64 step0, unsigned int nsteps, u32 seed_lo, u32 seed_hi, const unsigned char *__restrict__ pin,
+                                          Barrier &&barrier) {
     constexpr int NBRICKS = ((spec::NA + spec::BX - 1) / spec::BX) * ((spec::NB + spec::BY - 1) / spec::BY) * ((spec::NC + spec::BZ - 1) / spec::BZ);
-    unsigned int target = 0;
-    const unsigned long long step0 = *d_step;
     for (unsigned int k = 0; k < nsteps; ++k) {
         const double *n = (k & 1u) ? n1 : n0;
         double *nout = (k & 1u) ? n0 : n1;
-        const unsigned long long step = step0 + k;
+        const u64 step = step0 + k;
         for (int item = blockIdx.x; item < NBRICKS * spec::NBASIS; item += gridDim.x)
             dispatch_basis<0>(item / NBRICKS, [&](auto b) {
                 predictor_body<decltype(b)::value, true>(n, nullptr, np, aux, step, seed_lo, seed_hi, pin, item % NBRICKS);
             });
-        grid_barrier(bar, gridDim.x, target);
+        barrier();
         for (int item = blockIdx.x; item < NBRICKS * spec::NBASIS; item += gridDim.x)
             dispatch_basis<0>(item / NBRICKS, [&](auto b) {
                 corrector_body<decltype(b)::value, true>(n, np, nullptr, nullptr, aux, nout, step, seed_lo, seed_hi, pin, item % NBRICKS);
             });
-        grid_barrier(bar, gridDim.x, target);
+        barrier();
     }
+}
+}  // namespace spinjit
+
+extern "C" __global__ void SPIN_BOUNDS(spec::BX *spec::BY *spec::BZ)
+    jit_steps_coop(double *__restrict__ n0, double *__restrict__ n1, double *__restrict__ np, double *__restrict__ aux,
+                   const unsigned long long *__restrict__ d_step, unsigned int nsteps, unsigned int seed_lo, unsigned int seed_hi,
+                   const unsigned char *__restrict__ pin, unsigned int *bar) {
+    unsigned int target = 0;
+    spinjit::all_steps(n0, n1, np, aux, *d_step, nsteps, seed_lo, seed_hi, pin, [&]() { spinjit::grid_barrier(bar, gridDim.x, target); });
+}
+
+// the same for lattices of at most 16 bricks: the whole grid is ONE thread-block cluster and the barrier is the cluster's hardware barrier
+extern "C" __global__ void SPIN_BOUNDS(spec::BX *spec::BY *spec::BZ)
+    jit_steps_cluster(double *__restrict__ n0, double *__restrict__ n1, double *__restrict__ np, double *__restrict__ aux,
+                      const unsigned long long *__restrict__ d_step, unsigned int nsteps, unsigned int seed_lo, unsigned int seed_hi,
+                      const unsigned char *__restrict__ pin) {
+    spinjit::all_steps(n0, n1, np, aux, *d_step, nsteps, seed_lo, seed_hi, pin, []() { spinjit::cluster_barrier(); });
 }
 
 #ifdef SPIN_FUSED

@@ -182,6 +182,7 @@ int jit_launch_rk4_stage(spin_system *s, const double *base, const double *y, do
                          int stage, unsigned step_add);
 // all steps of an llg_iterate call in one cooperative launch (jit_steps_coop)
 bool jit_coop_ready(const spin_system *s);
+bool jit_cluster_ready(const spin_system *s);
 int jit_launch_steps_coop(spin_system *s, unsigned nsteps);
 // column-marching versions of the two sweeps (spin_jit_col.cuh)
 bool jit_col_ready(const spin_system *s);

@@ -144,7 +144,7 @@ def test_split_invariance_and_graph_equivalence(P, O):
     assert a.llg_get_step() == b.llg_get_step() == c.llg_get_step() == 57
     # the cooperative all-steps-in-one-launch kernel (default for small lattices): same bits, split-invariant, odd and even counts
     d = P.SpinSystem.from_workload(w)
-    assert d.spin_kernel_info() == "jit+coop", d.spin_kernel_info()      # 960 spins: taken by default
+    assert d.spin_kernel_info() in ("jit+coop", "jit+cluster"), d.spin_kernel_info()      # 960 spins: taken by default
     d.llg_iterate(20); d.llg_iterate(17); d.llg_iterate(20)
     assert np.array_equal(na, d.spins_get())
     assert d.llg_get_step() == 57
@@ -556,7 +556,7 @@ def test_cooperative_kernel_matches_two_launch_path(P, O, cfg, cells, steps):
             s_.llg_set_solver(solver); s_.spins_set_pinned(mask if solver == 1 else None)
         a.spin_set_option("use_coop", 2)
         b.spin_set_option("use_coop", 0)
-        assert a.spin_kernel_info() == "jit+coop" and b.spin_kernel_info().startswith("jit (brick"), (a.spin_kernel_info(), b.spin_kernel_info())
+        assert a.spin_kernel_info() in ("jit+coop", "jit+cluster") and b.spin_kernel_info().startswith("jit (brick"), (a.spin_kernel_info(), b.spin_kernel_info())
         a.llg_iterate(steps); b.llg_iterate(steps)
         assert np.array_equal(a.spins_get(), b.spins_get()), solver
     o = O.OracleSystem.from_workload(w)
@@ -784,3 +784,18 @@ def test_gneb_climbing_image_finds_the_anisotropy_barrier_on_the_gpu(P):
     assert abs(s.spins_get()[0, 2]) < 1e-6 and np.abs(F).max() < 1e-6
     with pytest.raises(P.SpinError):
         P.SpinSystem.from_workload(W.config1().resized((4, 4, 1), 1)).gneb_iterate(1, 0.1)      # no chain
+
+
+def test_cluster_barrier_kernel_matches_grid_barrier_and_two_launch_paths(P, O):
+    """Lattices of at most 16 bricks run as ONE thread-block cluster (hardware barrier); use_coop = 3 keeps the grid barrier."""
+    for cfg, cells, steps in [(1, (32, 32, 1), 1000), (2, (64, 40, 1), 300), (3, (32, 8, 6), 200), (4, (33, 17, 1), 150)]:
+        w = W.CONFIGS[cfg]().resized(cells, steps)
+        res = {}
+        for name, opt in (("cluster", 1), ("coop", 3), ("brick", 0)):
+            g = P.SpinSystem.from_workload(w)
+            g.spin_set_option("use_coop", opt)
+            info = g.spin_kernel_info()
+            assert info == {"cluster": "jit+cluster", "coop": "jit+coop"}.get(name, info) or name == "brick", (name, info)
+            g.llg_iterate(steps // 2); g.llg_iterate(steps - steps // 2)
+            res[name] = g.spins_get()
+        assert np.array_equal(res["cluster"], res["brick"]) and np.array_equal(res["coop"], res["brick"]), cfg
