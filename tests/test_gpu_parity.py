@@ -799,3 +799,63 @@ def test_cluster_barrier_kernel_matches_grid_barrier_and_two_launch_paths(P, O):
             g.llg_iterate(steps // 2); g.llg_iterate(steps - steps // 2)
             res[name] = g.spins_get()
         assert np.array_equal(res["cluster"], res["brick"]) and np.array_equal(res["coop"], res["brick"]), cfg
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# Randomised lattices: arbitrary Bravais vectors, 1-3 basis atoms, pairs up to two cells away (arbitrary J, D), quadruplets, mixed
+# boundaries, anisotropy per atom, current, noise, pins, every solver -- specialised kernels, table-driven kernels and oracle must agree
+@pytest.mark.parametrize("seed", range(16))
+def test_randomised_systems(P, O, seed):
+    rng = np.random.default_rng(1000 + seed)
+    nb = int(rng.integers(1, 4))
+    cells = tuple(int(x) for x in rng.integers(1, [38, 14, 7]))
+    per = tuple(int(x) for x in rng.integers(0, 2, 3))
+    brav = np.eye(3) + 0.25 * rng.standard_normal((3, 3))
+    basis = np.vstack([[0, 0, 0], rng.random((nb - 1, 3))]) if nb > 1 else np.zeros((1, 3))
+    npairs = int(rng.integers(1, 9))
+    seen, pi, pj, pt = set(), [], [], []
+    while len(pi) < npairs:
+        i, j = int(rng.integers(0, nb)), int(rng.integers(0, nb))
+        t = tuple(int(x) for x in rng.integers(-2, 3, 3))
+        t = tuple(0 if cells[d] == 1 and not per[d] else t[d] for d in range(3))
+        if (i == j and t == (0, 0, 0)) or (i, j, t) in seen or (j, i, tuple(-x for x in t)) in seen:
+            continue
+        seen.add((i, j, t)); pi.append(i); pj.append(j); pt.append(t)
+    nq = int(rng.integers(0, 3))
+    qb = rng.integers(0, nb, (nq, 4)); qt = rng.integers(-1, 2, (nq, 9))
+    for d in range(3):
+        if cells[d] == 1 and not per[d]:
+            qt[:, d::3] = 0
+    T = float(rng.choice([0.0, 30.0])); u = float(rng.choice([0.0, 0.2]))
+    def build(cls):
+        s = cls(brav, basis, cells, per, 1.1)
+        (s.hamiltonian_set_mu_s if cls is P.SpinSystem else s.set_mu_s)(1.0 + rng_mu)
+        (s.hamiltonian_set_field if cls is P.SpinSystem else s.set_field)(0.7, Bdir)
+        (s.hamiltonian_set_anisotropy if cls is P.SpinSystem else s.set_anisotropy)(list(range(nb)), Kv, Kax)
+        (s.hamiltonian_set_pairs if cls is P.SpinSystem else s.set_pairs)(pi, pj, pt, Jv, Dv)
+        if nq:
+            (s.hamiltonian_set_quadruplets if cls is P.SpinSystem else s.set_quadruplets)(qb, qt, Kq)
+        s.llg_configure(1.5, 0.2, T, 99 + seed, u, jdir, 0.05)
+        return s
+    rng_mu = rng.random(nb); Bdir = rng.standard_normal(3); Kv = 0.3 * rng.standard_normal(nb); Kax = rng.standard_normal((nb, 3))
+    Jv = rng.standard_normal(npairs); Dv = 0.4 * rng.standard_normal((npairs, 3)); Kq = 0.3 * rng.standard_normal(nq); jdir = rng.standard_normal(3)
+    g, h, o = build(P.SpinSystem), build(P.SpinSystem), build(O.OracleSystem)
+    h.spin_set_option("use_jit", 0)
+    N = g.N
+    n0 = rng.standard_normal((N, 3)); n0 /= np.linalg.norm(n0, axis=1, keepdims=True)
+    mask = (rng.random(N) < 0.1).astype(np.uint8)
+    for s_ in (g, h):
+        s_.spins_set_pinned(mask); s_.spins_set(n0)
+    o.set_pinned(mask); o.set_spins(n0)
+    Bo = o.effective_field()
+    assert_fields_close(g.effective_field(), Bo)
+    To = o.energy_terms()
+    assert np.abs(g.energy()[1] - To).max() <= ENERGY_RTOL * max(np.abs(To).sum(), 1e-300)
+    solver = int(rng.integers(0, 4))
+    g.llg_set_solver(solver); o.set_solver(solver)
+    g.llg_iterate(25); o.iterate(25)
+    d = np.abs(g.spins_get() - o.spins()).max()
+    assert d <= SPIN_ATOL, (seed, nb, cells, per, solver, d)
+    h.llg_iterate(25)                                    # table-driven Depondt
+    if solver == 0:
+        assert np.abs(h.spins_get() - o.spins()).max() <= SPIN_ATOL
