@@ -238,6 +238,10 @@ std::string spin::jit_source(const spin_system *s) {
         const char *e = getenv("SPINLLG_SPLIT");
         o << "constexpr bool SPLIT_CORR = " << ((e && atoi(e) == 0) ? "false" : "true") << ";\n";
     }
+    {   // corrector bricks in reverse order (L2 reuse of what the predictor touched last): 68.1 -> 65.3 us per step on cfg3
+        const char *e = getenv("SPINLLG_REVERSE");
+        o << "constexpr bool REVERSE_CORR = " << ((e && atoi(e) == 0) ? "false" : "true") << ";\n";
+    }
     o << "constexpr bool MULTI_IMAGE = " << (s->n_img > 1 ? "true" : "false") << ";\n";
     o << "constexpr bool HAS_PIN = " << (s->d_pin ? "true" : "false") << ";\n";
     o << "constexpr int SOLVER = " << s->solver << ";      // 0 Depondt, 1 Heun, 2 SIB, 3 RK4 (own stage kernel)\n";

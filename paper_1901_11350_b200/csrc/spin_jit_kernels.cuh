@@ -442,8 +442,11 @@ extern "C" __global__ void SPIN_BOUNDS(spec::BX *spec::BY *spec::BZ)
     const size_t off = spec::MULTI_IMAGE ? (size_t)image * ((size_t)spec::NBASIS * spec::SUB) : (size_t)0;
     const double scale = (spec::MULTI_IMAGE && img_sigma) ? img_sigma[image] : 1.0;
     spinjit::dispatch_basis<0>((int)blockIdx.y, [&](auto b) {
+        // The corrector walks the bricks in the opposite order to the predictor: what the predictor touched last (the tail of n and of
+        // n^p) is still in the 126 MB L2 and is read first; it ends at brick 0, where the next predictor starts.
+        const int brick = spec::REVERSE_CORR ? (int)(gridDim.x - 1u - blockIdx.x) : (int)blockIdx.x;
         spinjit::corrector_body<decltype(b)::value>(n + off, np + off, fddi_n + off, fddi_np + off, Ain + off, nout + off, step, seed_lo, seed_hi, pin,
-                                                    (int)blockIdx.x, image, scale);
+                                                    brick, image, scale);
     });
 }
 
