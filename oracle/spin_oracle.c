@@ -62,7 +62,9 @@ typedef struct orc_system {
     long ncell, N;
     double *mu;              /* nb, mu_B                                           */
     double Bext[3];          /* Tesla                                              */
-    double *K, *Kax;         /* nb, 3*nb (unit axes)                               */
+    double *K, *Kax;         /* legacy single-axis view (first entry per atom); the sums run over the entry list below */
+    int nani; int *ab; double *aK, *aax;   /* anisotropy entries: basis atom, K, unit axis -- "sum_i sum_j K_j (K^_j . n_i)^2" (Eq. 1 :61)
+                                              has a sum over axes j: an atom may carry several (reading R3, extended)             */
     int npairs; int *pi, *pj, *pt; double *pJ, *pD;
     int nquads; int *qb, *qt; double *qK;
     int ddi, nimg[3];
@@ -147,7 +149,7 @@ orc_system *orc_create(const double brav[9], int nb, const double *basis, const 
 }
 void orc_destroy(orc_system *s) {
     if (!s) return;
-    free(s->basis); free(s->mu); free(s->K); free(s->Kax);
+    free(s->basis); free(s->mu); free(s->K); free(s->Kax); free(s->ab); free(s->aK); free(s->aax);
     free(s->pi); free(s->pj); free(s->pt); free(s->pJ); free(s->pD);
     free(s->qb); free(s->qt); free(s->qK); free(s->Khat); free(s->n); free(s->pinned); free(s->vp_v); free(s->vp_F);
     free(s);
@@ -168,12 +170,13 @@ void orc_set_field(orc_system *s, double B, const double dir[3]) {
     for (int k = 0; k < 3; ++k) s->Bext[k] = (nrm > 0) ? B * dir[k] / nrm : 0.0;
 }
 void orc_set_anisotropy(orc_system *s, int n, const int *bidx, const double *K, const double *axis) {
-    for (int b = 0; b < s->nb; ++b) s->K[b] = 0.0;
+    free(s->ab); free(s->aK); free(s->aax);
+    s->nani = n;
+    s->ab = (int *)malloc((n + 1) * sizeof(int)); s->aK = (double *)malloc((n + 1) * sizeof(double)); s->aax = (double *)malloc(3 * (n + 1) * sizeof(double));
     for (int e = 0; e < n; ++e) {
-        int b = bidx[e];
         double nrm = sqrt(dot3(axis + 3*e, axis + 3*e));
-        s->K[b] = K[e];
-        for (int k = 0; k < 3; ++k) s->Kax[3*b+k] = axis[3*e+k] / nrm;
+        s->ab[e] = bidx[e]; s->aK[e] = K[e];
+        for (int k = 0; k < 3; ++k) s->aax[3*e+k] = axis[3*e+k] / nrm;
     }
 }
 void orc_set_pairs(orc_system *s, int np, const int *pi, const int *pj, const int *pt,
@@ -235,8 +238,10 @@ void orc_energy(orc_system *s, const double *n, double E[6]) {
         for (int b = 0; b < s->nb; ++b) {
             const double *ni = n + 3 * spin_index(s, c, b);
             ez -= (long double)(s->mu[b] * ORC_MU_B * dot3(s->Bext, ni));
-            double p = dot3(s->Kax + 3*b, ni);
-            ea -= (long double)(s->K[b] * p * p);
+            for (int e = 0; e < s->nani; ++e) if (s->ab[e] == b) {
+                double p = dot3(s->aax + 3*e, ni);
+                ea -= (long double)(s->aK[e] * p * p);
+            }
         }
         for (int p = 0; p < s->npairs; ++p) {
             if (!shifted_cell(s, c, s->pt + 3*p, +1, cj)) continue;
@@ -310,9 +315,9 @@ void orc_gradient_scatter(orc_system *s, const double *n, double *F, int mask) {
         for (int b = 0; b < s->nb; ++b) {
             long i = spin_index(s, c, b);
             if (mask & T_ZEE) for (int k = 0; k < 3; ++k) F[3*i+k] += s->mu[b] * ORC_MU_B * s->Bext[k];
-            if (mask & T_ANI) {
-                double p = dot3(s->Kax + 3*b, n + 3*i);
-                for (int k = 0; k < 3; ++k) F[3*i+k] += 2.0 * s->K[b] * p * s->Kax[3*b+k];
+            if (mask & T_ANI) for (int e = 0; e < s->nani; ++e) if (s->ab[e] == b) {
+                double p = dot3(s->aax + 3*e, n + 3*i);
+                for (int k = 0; k < 3; ++k) F[3*i+k] += 2.0 * s->aK[e] * p * s->aax[3*e+k];
             }
         }
         for (int p = 0; p < s->npairs; ++p) {
@@ -365,9 +370,9 @@ static void gather_one(const orc_system *s, const double *n, long cell, int b, i
     const double *ni = n + 3 * spin_index(s, c, b);
     F[0] = F[1] = F[2] = 0.0;
     if (mask & T_ZEE) for (int k = 0; k < 3; ++k) F[k] += s->mu[b] * ORC_MU_B * s->Bext[k];
-    if (mask & T_ANI) {
-        double p = dot3(s->Kax + 3*b, ni);
-        for (int k = 0; k < 3; ++k) F[k] += 2.0 * s->K[b] * p * s->Kax[3*b+k];
+    if (mask & T_ANI) for (int e = 0; e < s->nani; ++e) if (s->ab[e] == b) {
+        double p = dot3(s->aax + 3*e, ni);
+        for (int k = 0; k < 3; ++k) F[k] += 2.0 * s->aK[e] * p * s->aax[3*e+k];
     }
     if (mask & (T_EXC | T_DMI)) for (int p = 0; p < s->npairs; ++p) {
         const double *D = s->pD + 3*p;

@@ -752,3 +752,21 @@ def test_gneb_climbing_image_finds_the_anisotropy_barrier():
     assert abs(out[ci, 0, 2]) < 1e-6
     assert np.abs(F).max() < 1e-6
     assert max(l[:3]) - min(l[:3]) < 1e-3
+
+
+def test_several_anisotropy_axes_per_atom():
+    """Eq. 1 sums the anisotropy over axes j as well as over spins: -sum_i sum_j K_j (K^_j . n_i)^2.  Two axes on one atom:
+    the closed form of the biaxial energy (the form of Eq. 13, :187), the gradient against finite differences, and the equivalence of
+    two equal axes with one of double strength."""
+    s = OracleSystem(np.eye(3), [[0, 0, 0]], (3, 2, 1), (0, 0, 0))
+    s.set_mu_s([2.0])
+    K1, K2 = 0.7, -0.3
+    s.set_anisotropy([0, 0], [K1, K2], [[1, 0, 0], [0, 2, 0]])
+    n = rand_spins(6, 4)
+    assert s.energy_terms(n)[1] == pytest.approx(-(K1 * n[:, 0] ** 2 + K2 * n[:, 1] ** 2).sum(), rel=1e-14)
+    F = s.gradient(n)
+    assert np.allclose(F, np.stack([2 * K1 * n[:, 0], 2 * K2 * n[:, 1], 0 * n[:, 2]], axis=1), atol=1e-15)
+    _fd_check(s, n, [0, 3, 5])
+    a = OracleSystem(np.eye(3), [[0, 0, 0]], (3, 2, 1), (0, 0, 0)); a.set_anisotropy([0, 0], [0.2, 0.2], [[0, 0, 1], [0, 0, 1]])
+    b = OracleSystem(np.eye(3), [[0, 0, 0]], (3, 2, 1), (0, 0, 0)); b.set_anisotropy([0], [0.4], [[0, 0, 1]])
+    assert a.energy(n) == pytest.approx(b.energy(n), rel=1e-15)
