@@ -67,8 +67,9 @@ int spin_set_stream(spin_system *sys, void *cuda_stream);
 int hamiltonian_set_mu_s(spin_system *sys, const double *mu_s /*host, n_basis*/);
 /* Zeeman term -sum_i mu_i B.n_i: field magnitude in Tesla and direction (normalised internally) */
 int hamiltonian_set_field(spin_system *sys, double B_tesla, const double dir[3]);
-/* uniaxial anisotropy -sum_i K (K^.n_i)^2 with one axis per basis atom (":69 axes ... of the basis cell");
- * n entries (basis_idx, K_meV, axis); atoms not listed get K = 0; a later call replaces the earlier one     */
+/* uniaxial anisotropy -sum_i sum_j K_j (K^_j.n_i)^2 (Eq. 1 :61, ":69 axes ... of the basis cell"): n entries (basis_idx, K_meV, axis);
+ * a basis atom may be listed several times (several axes j, e.g. the biaxial Hamiltonian of Eq. 13 :187), atoms not listed
+ * have none; a later call replaces the earlier one; at most 16 entries in total                                              */
 int hamiltonian_set_anisotropy(spin_system *sys, int n, const int *basis_idx, const double *K_meV,
                                const double *axis /*host, 3n*/);
 /* unique pairs <ij> (":69 unique pairs", ":71 no limitation on number or distance"): pair p couples basis atom

@@ -168,11 +168,23 @@ int build_plan(const spin_system *s, DevicePlan &P) {
     const double a2 = 1.0 + s->alpha * s->alpha;
     for (int b = 0; b < s->nb; ++b) {
         const double m = s->mu[b] * MU_B;
-        for (int k = 0; k < 3; ++k) { P.zee[b][k] = m * s->Bmag * s->Bdir[k]; P.Kax[b][k] = s->Kax[3 * b + k]; }
-        P.K2[b] = 2.0 * s->K[b];
+        for (int k = 0; k < 3; ++k) P.zee[b][k] = m * s->Bmag * s->Bdir[k];
         P.pre[b] = -GAMMA / (a2 * m);
         P.sigma[b] = (s->T > 0.0) ? sqrt(2.0 * s->alpha * K_B * s->T * m / (GAMMA * s->dt_ps)) : 0.0;
         P.inv_mu[b] = 1.0 / m;
+    }
+    {   // anisotropy entries grouped by basis atom, list order kept within an atom
+        int na = 0;
+        for (int b = 0; b < s->nb; ++b) {
+            P.ani_begin[b] = na;
+            for (size_t e = 0; e < s->ani_b.size(); ++e) {
+                if (s->ani_b[e] != b) continue;
+                P.K2[na] = 2.0 * s->K[e];
+                for (int k = 0; k < 3; ++k) P.Kax[na][k] = s->Kax[3 * e + k];
+                ++na;
+            }
+        }
+        P.ani_begin[s->nb] = na;
     }
     P.alpha = s->alpha; P.dt = s->dt_ps; P.dt2 = s->dt_ps * s->dt_ps;
     P.thermal_on = (s->T > 0.0) ? 1 : 0;
@@ -494,9 +506,7 @@ extern "C" int spin_geometry_create(const double bravais[9], int n_basis, const 
     s->ncell = ncell; s->N = ncell * n_basis;
     s->mu.assign(n_basis, 1.0);
     s->Bmag = 0.0; s->Bdir[0] = 0; s->Bdir[1] = 0; s->Bdir[2] = 1;
-    s->K.assign(n_basis, 0.0);
-    s->Kax.assign(3 * n_basis, 0.0);
-    for (int bb = 0; bb < n_basis; ++bb) s->Kax[3 * bb + 2] = 1.0;
+    s->ani_b.clear(); s->K.clear(); s->Kax.clear();
     s->ddi_on = 0; s->ddi_img[0] = s->ddi_img[1] = s->ddi_img[2] = 0;
     s->dt_ps = 1e-3; s->alpha = 0.1; s->T = 0; s->u = 0; s->jdir[0] = 1; s->jdir[1] = 0; s->jdir[2] = 0; s->beta = 0;
     s->seed = 0; s->step = 0; s->solver = SPIN_SOLVER_DEPONDT;
@@ -586,17 +596,19 @@ extern "C" int hamiltonian_set_field(spin_system *s, double B, const double dir[
 }
 extern "C" int hamiltonian_set_anisotropy(spin_system *s, int n, const int *bidx, const double *K, const double *axis) {
     REQUIRE(s && n >= 0 && (n == 0 || (bidx && K && axis)), "bad argument");
-    std::vector<double> Kn(s->nb, 0.0), ax(3 * s->nb, 0.0);
-    for (int b = 0; b < s->nb; ++b) ax[3 * b + 2] = 1.0;
+    REQUIRE(n <= SPIN_MAX_ANI_ENTRIES, "at most %d anisotropy axes in total", SPIN_MAX_ANI_ENTRIES);
+    std::vector<int> ab;
+    std::vector<double> Kn, ax;
     for (int e = 0; e < n; ++e) {
         REQUIRE(bidx[e] >= 0 && bidx[e] < s->nb, "anisotropy: basis index %d out of range", bidx[e]);
         const double *a = axis + 3 * e;
         const double nn = sqrt(a[0] * a[0] + a[1] * a[1] + a[2] * a[2]);
         REQUIRE(nn > 0.0 && isfinite(K[e]), "anisotropy: zero axis or non-finite K");
-        Kn[bidx[e]] = K[e];
-        for (int k = 0; k < 3; ++k) ax[3 * bidx[e] + k] = a[k] / nn;
+        ab.push_back(bidx[e]);
+        Kn.push_back(K[e]);
+        for (int k = 0; k < 3; ++k) ax.push_back(a[k] / nn);
     }
-    s->K = Kn; s->Kax = ax;
+    s->ani_b = ab; s->K = Kn; s->Kax = ax;
     s->plan_dirty = true;
     return SPIN_OK;
 }

@@ -277,8 +277,13 @@ std::string spin::jit_source(const spin_system *s) {
         o << "};\n";
     };
     emit_b3("ZEE", P.zee);
-    emit_b3("KAX", P.Kax);
-    emit_array<double>(o, "double", "K2", P.nb, [&](int i) { return hexd(P.K2[i]); });
+    const int na = P.ani_begin[P.nb];
+    emit_array<int>(o, "int", "ANI_BEGIN", P.nb + 1, [&](int i) { return std::to_string(P.ani_begin[i]); });
+    o << "constexpr double KAX[" << (na ? na : 1) << "][3] = {";
+    for (int e = 0; e < na; ++e) o << (e ? ", {" : "{") << hexd(P.Kax[e][0]) << ", " << hexd(P.Kax[e][1]) << ", " << hexd(P.Kax[e][2]) << "}";
+    if (!na) o << "{0.0, 0.0, 0.0}";
+    o << "};\n";
+    emit_array<double>(o, "double", "K2", na, [&](int i) { return hexd(P.K2[i]); });
     emit_array<double>(o, "double", "PRE", P.nb, [&](int i) { return hexd(P.pre[i]); });
     emit_array<double>(o, "double", "SIGMA", P.nb, [&](int i) { return hexd(P.sigma[i]); });
     o << "constexpr double ALPHA = " << hexd(P.alpha) << ", DT = " << hexd(P.dt) << ", DT2 = " << hexd(P.dt2) << ";\n";
@@ -304,8 +309,11 @@ std::string spin::jit_source(const spin_system *s) {
     emit_c("P_DZ", np, [&](int i) { return P.pairs[i].Dz; });
     emit_c("Q_K", nq, [&](int i) { return P.quads[i].K; });
     emit_cb3("ZEE", P.zee);
-    emit_cb3("KAX", P.Kax);
-    emit_c("K2", P.nb, [&](int i) { return P.K2[i]; });
+    o << "__constant__ double KAX[" << (na ? na : 1) << "][3] = {";
+    for (int e = 0; e < na; ++e) o << (e ? ", {" : "{") << hexd(P.Kax[e][0]) << ", " << hexd(P.Kax[e][1]) << ", " << hexd(P.Kax[e][2]) << "}";
+    if (!na) o << "{0.0, 0.0, 0.0}";
+    o << "};\n";
+    emit_c("K2", na, [&](int i) { return P.K2[i]; });
     emit_c("PRE", P.nb, [&](int i) { return P.pre[i]; });
     emit_c("PREA", P.nb, [&](int i) { return P.pre[i] * P.alpha; });
     emit_c("SIGMA", P.nb, [&](int i) { return P.sigma[i]; });

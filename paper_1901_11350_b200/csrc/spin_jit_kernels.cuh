@@ -15,7 +15,7 @@
 //   bool STORE_A, HAS_DDI, THERMAL_ON, STT_ON;
 //   int PAIR_BEGIN[NBASIS+1], P_DA[], P_DB[], P_DC[], P_BJ[];  double P_J[], P_DX[], P_DY[], P_DZ[];
 //   int QUAD_BEGIN[NBASIS+1], Q_D[][9], Q_B[][3];  double Q_K[];
-//   double ZEE[NBASIS][3], K2[NBASIS], KAX[NBASIS][3], PRE[NBASIS], SIGMA[NBASIS];
+//   int ANI_BEGIN[NBASIS+1];  double ZEE[NBASIS][3], K2[n_ani], KAX[n_ani][3], PRE[NBASIS], SIGMA[NBASIS];
 //   double ALPHA, DT, DT2, STT_C[3], STT_S, STT_X;
 #pragma once
 
@@ -119,17 +119,20 @@ __device__ __forceinline__ void force(const Acc &cfg, const double (&own)[NCONF]
         if constexpr (spec::ZEE[B][0] != 0.0) F[k][0] += specc::ZEE[B][0];
         if constexpr (spec::ZEE[B][1] != 0.0) F[k][1] += specc::ZEE[B][1];
         if constexpr (spec::ZEE[B][2] != 0.0) F[k][2] += specc::ZEE[B][2];
-        if constexpr (spec::K2[B] != 0.0) {
-            constexpr bool hx = spec::KAX[B][0] != 0.0, hy = spec::KAX[B][1] != 0.0, hz = spec::KAX[B][2] != 0.0;
-            double p = 0.0;
-            if constexpr (hx) p = fma(specc::KAX[B][0], own[k][0], p);
-            if constexpr (hy) p = fma(specc::KAX[B][1], own[k][1], p);
-            if constexpr (hz) p = fma(specc::KAX[B][2], own[k][2], p);
-            p *= specc::K2[B];
-            if constexpr (hx) F[k][0] = fma(p, specc::KAX[B][0], F[k][0]);
-            if constexpr (hy) F[k][1] = fma(p, specc::KAX[B][1], F[k][1]);
-            if constexpr (hz) F[k][2] = fma(p, specc::KAX[B][2], F[k][2]);
-        }
+        static_for<spec::ANI_BEGIN[B], spec::ANI_BEGIN[B + 1]>([&](auto ae) {      // every anisotropy axis of this atom (Eq. 1 sums over axes)
+            constexpr int A = decltype(ae)::value;
+            if constexpr (spec::K2[A] != 0.0) {
+                constexpr bool hx = spec::KAX[A][0] != 0.0, hy = spec::KAX[A][1] != 0.0, hz = spec::KAX[A][2] != 0.0;
+                double p = 0.0;
+                if constexpr (hx) p = fma(specc::KAX[A][0], own[k][0], p);
+                if constexpr (hy) p = fma(specc::KAX[A][1], own[k][1], p);
+                if constexpr (hz) p = fma(specc::KAX[A][2], own[k][2], p);
+                p *= specc::K2[A];
+                if constexpr (hx) F[k][0] = fma(p, specc::KAX[A][0], F[k][0]);
+                if constexpr (hy) F[k][1] = fma(p, specc::KAX[A][1], F[k][1]);
+                if constexpr (hz) F[k][2] = fma(p, specc::KAX[A][2], F[k][2]);
+            }
+        });
     }
     static_for<spec::PAIR_BEGIN[B], spec::PAIR_BEGIN[B + 1]>([&](auto e) {
         constexpr int E = decltype(e)::value;

@@ -80,12 +80,14 @@ __device__ __forceinline__ void short_range_force(const DevicePlan &P, const dou
 #pragma unroll
         for (int c = 0; c < NCONF; ++c) { F[c][0] += P.zee[b][0]; F[c][1] += P.zee[b][1]; F[c][2] += P.zee[b][2]; }
     }
-    if ((mask & T_ANI) && P.K2[b] != 0.0) {
-        const double kx = P.Kax[b][0], ky = P.Kax[b][1], kz = P.Kax[b][2], k2 = P.K2[b];
+    if (mask & T_ANI) {
+        for (int e = P.ani_begin[b]; e < P.ani_begin[b + 1]; ++e) {
+            const double kx = P.Kax[e][0], ky = P.Kax[e][1], kz = P.Kax[e][2], k2 = P.K2[e];
 #pragma unroll
-        for (int c = 0; c < NCONF; ++c) {
-            const double p = k2 * (kx * own[c][0] + ky * own[c][1] + kz * own[c][2]);
-            F[c][0] += p * kx; F[c][1] += p * ky; F[c][2] += p * kz;
+            for (int c = 0; c < NCONF; ++c) {
+                const double p = k2 * (kx * own[c][0] + ky * own[c][1] + kz * own[c][2]);
+                F[c][0] += p * kx; F[c][1] += p * ky; F[c][2] += p * kz;
+            }
         }
     }
     if (mask & (T_EXC | T_DMI)) {

@@ -19,6 +19,7 @@
 #define SPIN_MAX_BASIS 8
 #define SPIN_MAX_PAIR_ENTRIES 160
 #define SPIN_MAX_QUAD_ENTRIES 32
+#define SPIN_MAX_ANI_ENTRIES 16      // anisotropy axes over all basis atoms
 #define SPIN_COOP_MAX_SPINS 4096      // largest lattice that takes the cooperative all-steps kernel by default
 
 namespace spin {
@@ -69,8 +70,9 @@ struct DevicePlan {
     int pair_begin[SPIN_MAX_BASIS + 1];
     int quad_begin[SPIN_MAX_BASIS + 1];
     double zee[SPIN_MAX_BASIS][3];           // mu_b mu_B B            (meV)
-    double K2[SPIN_MAX_BASIS];               // 2 K_b                  (meV)
-    double Kax[SPIN_MAX_BASIS][3];           // unit anisotropy axis
+    int ani_begin[SPIN_MAX_BASIS + 1];       // anisotropy entries of basis atom b: [ani_begin[b], ani_begin[b+1])  (Eq. 1 sums over axes)
+    double K2[SPIN_MAX_ANI_ENTRIES];         // 2 K of the entry       (meV)
+    double Kax[SPIN_MAX_ANI_ENTRIES][3];     // its unit axis
     double pre[SPIN_MAX_BASIS];              // -gamma / ((1+alpha^2) mu_b mu_B)   (rad / (ps meV))
     double sigma[SPIN_MAX_BASIS];            // thermal amplitude sqrt(2 alpha kB T mu / (gamma dt)) (meV)
     double inv_mu[SPIN_MAX_BASIS];           // 1 / (mu_b mu_B)        (T / meV)
@@ -106,7 +108,8 @@ struct spin_system {
     // ---- Hamiltonian (host description)
     std::vector<double> mu;        // nb
     double Bmag, Bdir[3];
-    std::vector<double> K, Kax;    // nb, 3*nb
+    std::vector<int> ani_b;        // anisotropy entries: basis atom,
+    std::vector<double> K, Kax;    // strength, unit axis (3 per entry)
     std::vector<spin::HostPair> pairs_explicit, pairs_exch_shells, pairs_dmi_shells;
     std::vector<spin::HostQuad> quads;
     int ddi_on, ddi_img[3];

@@ -831,13 +831,14 @@ def test_randomised_systems(P, O, seed):
         s = cls(brav, basis, cells, per, 1.1)
         (s.hamiltonian_set_mu_s if cls is P.SpinSystem else s.set_mu_s)(1.0 + rng_mu)
         (s.hamiltonian_set_field if cls is P.SpinSystem else s.set_field)(0.7, Bdir)
-        (s.hamiltonian_set_anisotropy if cls is P.SpinSystem else s.set_anisotropy)(list(range(nb)), Kv, Kax)
+        (s.hamiltonian_set_anisotropy if cls is P.SpinSystem else s.set_anisotropy)(ani_b, Kv, Kax)
         (s.hamiltonian_set_pairs if cls is P.SpinSystem else s.set_pairs)(pi, pj, pt, Jv, Dv)
         if nq:
             (s.hamiltonian_set_quadruplets if cls is P.SpinSystem else s.set_quadruplets)(qb, qt, Kq)
         s.llg_configure(1.5, 0.2, T, 99 + seed, u, jdir, 0.05)
         return s
-    rng_mu = rng.random(nb); Bdir = rng.standard_normal(3); Kv = 0.3 * rng.standard_normal(nb); Kax = rng.standard_normal((nb, 3))
+    ani_b = [int(x) for x in rng.integers(0, nb, int(rng.integers(0, 2 * nb + 1)))]        # 0..2 nb axes, several per atom allowed (Eq. 1)
+    rng_mu = rng.random(nb); Bdir = rng.standard_normal(3); Kv = 0.3 * rng.standard_normal(len(ani_b)); Kax = rng.standard_normal((len(ani_b), 3))
     Jv = rng.standard_normal(npairs); Dv = 0.4 * rng.standard_normal((npairs, 3)); Kq = 0.3 * rng.standard_normal(nq); jdir = rng.standard_normal(3)
     g, h, o = build(P.SpinSystem), build(P.SpinSystem), build(O.OracleSystem)
     h.spin_set_option("use_jit", 0)
@@ -859,3 +860,25 @@ def test_randomised_systems(P, O, seed):
     h.llg_iterate(25)                                    # table-driven Depondt
     if solver == 0:
         assert np.abs(h.spins_get() - o.spins()).max() <= SPIN_ATOL
+
+
+def test_biaxial_anisotropy_several_axes_per_atom(P, O):
+    """Eq. 1's sum over axes: the biaxial chain Hamiltonian of Eq. 13, -K1 n_x^2 + K2 n_y^2 - J n_i.n_j, with pinned ends."""
+    brav = np.eye(3)
+    g = P.SpinSystem(brav, [[0, 0, 0]], (48, 1, 1), (0, 0, 0)); o = O.OracleSystem(brav, [[0, 0, 0]], (48, 1, 1), (0, 0, 0))
+    for s_, pre in ((g, "hamiltonian_set_"), (o, "set_")):
+        getattr(s_, pre + "mu_s")([2.0])
+        getattr(s_, pre + "anisotropy")([0, 0], [0.5, -0.2], [[1, 0, 0], [0, 1, 0]])
+        getattr(s_, pre + "pairs")([0], [0], [[1, 0, 0]], [1.0])
+        s_.llg_configure(2.0, 0.1, 0.0, 0, 0.3, (1, 0, 0), 0.02)
+    w1 = dataclasses.replace(W.config1().resized((48, 1, 1), 1), periodic=(0, 0, 0))
+    n0 = W.domain_wall_spins(w1, width=4.0)
+    mask = np.zeros(48, np.uint8); mask[0] = mask[-1] = 1
+    g.spins_set_pinned(mask); o.set_pinned(mask)
+    g.spins_set(n0); o.set_spins(n0)
+    assert_fields_close(g.effective_field(), o.effective_field())
+    assert np.abs(g.energy()[1] - o.energy_terms()).max() <= ENERGY_RTOL * np.abs(o.energy_terms()).sum()
+    g.llg_iterate(400); o.iterate(400)
+    assert np.abs(g.spins_get() - o.spins()).max() <= SPIN_ATOL
+    with pytest.raises(P.SpinError):
+        g.hamiltonian_set_anisotropy([0] * 17, [0.1] * 17, [[0, 0, 1]] * 17)
