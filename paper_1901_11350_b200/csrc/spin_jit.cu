@@ -13,6 +13,8 @@
 #include <string.h>
 
 #include <algorithm>
+#include <map>
+#include <mutex>
 #include <sstream>
 #include <string>
 
@@ -339,7 +341,19 @@ std::string spin::jit_source(const spin_system *s) {
 }
 
 // compile `source` for sm_100a; on success the cubin is returned in `cubin`
+// process-wide cache of compiled translation units: systems with the same plan (replicas, option toggles that do not change the
+// source, test fixtures) share one NVRTC compilation
+namespace {
+std::mutex g_cache_mutex;
+std::map<std::string, std::string> g_cubin_cache;
+}
+
 int spin::jit_compile(const std::string &source, std::string &cubin, std::string &log) {
+    {
+        std::lock_guard<std::mutex> lock(g_cache_mutex);
+        auto it = g_cubin_cache.find(source);
+        if (it != g_cubin_cache.end() && !getenv("SPINLLG_JIT_DUMP")) { cubin = it->second; log.clear(); return SPIN_OK; }
+    }
     nvrtcProgram prog;
     if (nvrtcCreateProgram(&prog, source.c_str(), "spin_jit_spec.cu", 0, nullptr, nullptr) != NVRTC_SUCCESS)
         return spin::fail(SPIN_ERR_CUDA, "nvrtcCreateProgram failed");
@@ -359,6 +373,11 @@ int spin::jit_compile(const std::string &source, std::string &cubin, std::string
     cubin.assign(nc, '\0');
     nvrtcGetCUBIN(prog, &cubin[0]);
     nvrtcDestroyProgram(&prog);
+    {
+        std::lock_guard<std::mutex> lock(g_cache_mutex);
+        if (g_cubin_cache.size() >= 64) g_cubin_cache.clear();
+        g_cubin_cache[source] = cubin;
+    }
     if (const char *dump = getenv("SPINLLG_JIT_DUMP")) {       // developer aid: <dump>.cu / <dump>.cubin for cuobjdump -sass
         const std::string base(dump);
         if (FILE *f = fopen((base + ".cu").c_str(), "w")) { fwrite(source.data(), 1, source.size(), f); fclose(f); }
