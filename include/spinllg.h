@@ -198,7 +198,7 @@ int spin_set_option(spin_system *sys, const char *name, int value);
  * barrier, 0 switches it off.
  * cache_noise (default 1): the predictor keeps the thermal field of the step (24 B/spin) for the corrector instead of generating it twice.
  * ddi_slab (default 1): thin films with one basis atom take the dipolar slab path (2-D cuFFT + fused transform along c).
- * spin_kernel_info writes "jit+fused", "jit+cluster", "jit+coop", "jit+col", "jit+tma", "jit (brick kernels: <why>)" or "generic: <why>" into buf: which sweep kernels are in use.  */
+ * spin_kernel_info writes "jit+fused", "jit+cluster", "jit+coop", "jit+col", "jit+tma", "jit (brick sweeps)" or "generic: <why>" into buf: which sweep kernels are in use.  */
 int spin_kernel_info(spin_system *sys, char *buf, int len);
 /* the generated translation unit of the specialised sweeps (buf may be NULL); compile != 0 also compiles it for sm_100a
  * (needs no device) and returns the cubin size.  Host-side planner check; works in planner-only mode

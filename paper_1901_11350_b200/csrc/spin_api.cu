@@ -1160,7 +1160,7 @@ extern "C" int spin_kernel_info(spin_system *s, char *buf, int len) {
     else if (jit_coop_ready(s) && s->opt_coop && !s->ddi_on && (s->N <= SPIN_COOP_MAX_SPINS || s->opt_coop >= 2)) snprintf(buf, (size_t)len, jit_cluster_ready(s) ? "jit+cluster" : "jit+coop");
     else if (jit_col_ready(s)) snprintf(buf, (size_t)len, "jit+col");
     else if (jit_tma_ready(s)) snprintf(buf, (size_t)len, "jit+tma");
-    else if (jit_ready(s)) snprintf(buf, (size_t)len, "jit (brick kernels: %s)", jit_tma_note(s));
+    else if (jit_ready(s)) snprintf(buf, (size_t)len, "jit (brick sweeps)");
     else snprintf(buf, (size_t)len, "generic: %s", s->jit_note.c_str());
     return SPIN_OK;
 }
