@@ -69,6 +69,7 @@ def lib():
         L.orc_heun_step.argtypes = [vp]
         L.orc_set_solver.argtypes = [vp, C.c_int]
         L.orc_set_image.argtypes = [vp, C.c_uint32]
+        L.orc_set_damping_only.argtypes = [vp, C.c_int]
         L.orc_gneb_forces.argtypes = [vp, C.c_int, dp, C.c_double, C.c_int, dp, dp, dp]
         L.orc_gneb_iterate.argtypes = [vp, C.c_int, dp, C.c_long, C.c_double, C.c_double, C.c_int]
         L.orc_geodesic_distance.argtypes = [vp, dp, dp]
@@ -289,6 +290,10 @@ class OracleSystem:
     def geodesic_distance(self, a, b):
         (x, px), (y, py) = _d(a), _d(b)
         return float(lib().orc_geodesic_distance(self._h, px, py))
+
+    def set_damping_only(self, on):
+        """Drop the precession term of Eq. 10: the LLG solvers then minimise the energy."""
+        lib().orc_set_damping_only(self._h, int(bool(on)))
 
     def set_image(self, image):
         """Noise stream of image `image` (independent images of one batched system; 0 = single system)."""

@@ -80,6 +80,7 @@ typedef struct orc_system {
                                 (":79 defects, such as vacancies") is a pinned site holding the zero vector (reading R27)   */
     double *vp_v, *vp_F;     /* velocity-projection minimiser (App. D): velocity and force of the previous iteration, or NULL  */
     uint32_t image;          /* which image's noise stream this system draws (0 = the single-system stream)                    */
+    int damping_only;        /* 1: the precession term of Eq. 10 is dropped (:168), the solvers become minimisers                */
     int solver;              /* 0 Depondt (App. B B5-B7), 1 Heun (B3-B4), 2 SIB semi-implicit midpoint (App. C), 3 RK4 (:168) */
 } orc_system;
 
@@ -213,6 +214,7 @@ void orc_llg_configure(orc_system *s, double dt_fs, double alpha, double T, uint
 }
 void orc_set_solver(orc_system *s, int solver) { s->solver = solver; }
 void orc_set_image(orc_system *s, uint32_t image) { s->image = image; }
+void orc_set_damping_only(orc_system *s, int on) { s->damping_only = on ? 1 : 0; }
 void orc_set_pinned(orc_system *s, const unsigned char *mask) {
     free(s->pinned); s->pinned = NULL;
     if (!mask) return;
@@ -735,7 +737,8 @@ static inline void rot_field(const orc_system *s, int b, const double *n, const 
     double us = s->u / (1.0 + s->alpha * s->alpha);
     if (s->u != 0.0) cross3(n, sg, nxs);
     for (int k = 0; k < 3; ++k) {
-        A[k] = pre * (F[k] + s->alpha * nxF[k]);
+        /* ":168 these methods can also be used for energy minimization by considering only the damping part of the LLG equation" */
+        A[k] = pre * ((s->damping_only ? 0.0 : F[k]) + s->alpha * nxF[k]);
         if (s->u != 0.0) A[k] += us * (-(s->alpha - s->beta) * sg[k] + (1.0 + s->alpha * s->beta) * nxs[k]);
     }
 }

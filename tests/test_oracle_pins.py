@@ -770,3 +770,28 @@ def test_several_anisotropy_axes_per_atom():
     a = OracleSystem(np.eye(3), [[0, 0, 0]], (3, 2, 1), (0, 0, 0)); a.set_anisotropy([0, 0], [0.2, 0.2], [[0, 0, 1], [0, 0, 1]])
     b = OracleSystem(np.eye(3), [[0, 0, 0]], (3, 2, 1), (0, 0, 0)); b.set_anisotropy([0], [0.4], [[0, 0, 1]])
     assert a.energy(n) == pytest.approx(b.energy(n), rel=1e-15)
+
+
+def test_damping_only_dynamics_closed_form():
+    """"considering only the damping part of the LLG equation".  One spin in a field: without the precession term the
+    azimuth stays put and n_z follows the same tanh as in Eq. 12 (:178), n_z(t) = tanh(alpha gamma' B t + atanh n_z0)."""
+    alpha, B, dt_fs = 0.3, 2.0, 5.0
+    for solver in (0, 1, 2, 3):
+        s = OracleSystem(np.eye(3), [[0, 0, 0]], (1, 1, 1), (0, 0, 0))
+        s.set_mu_s([2.0]); s.set_field(B, (0, 0, 1)); s.llg_configure(dt_fs, alpha); s.set_solver(solver); s.set_damping_only(True)
+        n0 = np.array([0.6 * math.cos(0.7), 0.6 * math.sin(0.7), -0.8])
+        s.set_spins([n0])
+        gp = O.GAMMA / (1 + alpha * alpha)
+        for k in range(1, 401):
+            s.iterate(1)
+            n = s.spins()[0]
+            nz = math.tanh(alpha * gp * B * k * dt_fs * 1e-3 + math.atanh(-0.8))
+            assert abs(n[2] - nz) < 2e-6, (solver, k, n[2], nz)
+            assert abs(math.atan2(n[1], n[0]) - 0.7) < 1e-12
+    # a coupled system runs downhill
+    w = small(1, (8, 8, 1))
+    c = OracleSystem.from_workload(w); c.set_damping_only(True)
+    E = [c.energy()]
+    for _ in range(5):
+        c.iterate(100); E.append(c.energy())
+    assert all(b < a for a, b in zip(E, E[1:]))
