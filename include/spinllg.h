@@ -144,6 +144,9 @@ int llg_configure(spin_system *sys, double dt_fs, double alpha, double T_kelvin,
  * Heun, SIB and RK4 run in the run-time specialised kernels only (SPIN_ERR_STATE from llg_iterate if those are unavailable). */
 enum { SPIN_SOLVER_DEPONDT = 0, SPIN_SOLVER_HEUN = 1, SPIN_SOLVER_SIB = 2, SPIN_SOLVER_RK4 = 3 };
 int llg_set_solver(spin_system *sys, int solver);
+/* ":168 These methods can also be used for energy minimization by considering only the damping part of the LLG equation": with
+ * enabled != 0 the precession term -gamma/((1+alpha^2) mu) F of the rotation field is dropped and only the damping term remains. */
+int llg_set_damping_only(spin_system *sys, int enabled);
 /* advance n_steps steps of the selected solver (Depondt unless llg_set_solver chose another); asynchronous on the system's stream.  The step counter persists, so
  * llg_iterate(a); llg_iterate(b) reproduces llg_iterate(a+b) exactly.                                       */
 int llg_iterate(spin_system *sys, int64_t n_steps);

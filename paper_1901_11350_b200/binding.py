@@ -20,7 +20,7 @@ EXPORTS = [
     "hamiltonian_set_mu_s", "hamiltonian_set_field", "hamiltonian_set_anisotropy", "hamiltonian_set_pairs",
     "hamiltonian_set_exchange_shells", "hamiltonian_set_dmi_shells", "hamiltonian_set_quadruplets",
     "hamiltonian_set_ddi", "spin_set_images", "spin_select_image", "llg_set_image_temperatures", "gneb_forces", "gneb_iterate", "spins_set_pinned", "spins_set", "spins_get", "spins_set_device", "spins_get_device",
-    "llg_configure", "llg_set_solver", "minimise_vp", "minimise_vp_reset", "llg_iterate", "llg_get_step", "llg_set_step", "spin_synchronize",
+    "llg_configure", "llg_set_solver", "llg_set_damping_only", "minimise_vp", "minimise_vp_reset", "llg_iterate", "llg_get_step", "llg_set_step", "spin_synchronize",
     "effective_field", "effective_field_device", "energy", "observables", "topological_charge",
     "spin_launch_counts", "spin_profile_enable", "spin_profile_get", "spin_set_option",
     "spin_kernel_info", "spin_jit_source", "spin_last_error", "spin_version",
@@ -63,6 +63,7 @@ def lib() -> C.CDLL:
         "spins_get_device": (C.c_int, [vp, vp]),
         "llg_configure": (C.c_int, [vp, C.c_double, C.c_double, C.c_double, C.c_uint64, C.c_double, dp, C.c_double]),
         "llg_set_solver": (C.c_int, [vp, C.c_int]),
+        "llg_set_damping_only": (C.c_int, [vp, C.c_int]),
         "spins_set_pinned": (C.c_int, [vp, C.c_void_p]),
         "spin_set_images": (C.c_int, [vp, C.c_int]),
         "gneb_forces": (C.c_int, [vp, C.c_double, C.c_int, dp, dp, dp]),
@@ -272,6 +273,9 @@ class SpinSystem:
         q = C.c_double(0.0)
         _check(lib().topological_charge(self._h, C.byref(q)))
         return float(q.value)
+
+    def llg_set_damping_only(self, enabled):
+        _check(lib().llg_set_damping_only(self._h, int(bool(enabled))))
 
     def llg_set_solver(self, solver):
         """0 Depondt, 1 Heun, 2 SIB (include/spinllg.h SPIN_SOLVER_*)."""

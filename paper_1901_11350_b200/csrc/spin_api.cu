@@ -190,6 +190,7 @@ int build_plan(const spin_system *s, DevicePlan &P) {
     P.thermal_on = (s->T > 0.0) ? 1 : 0;
     P.seed_lo = (uint32_t)s->seed; P.seed_hi = (uint32_t)(s->seed >> 32);
     P.has_ddi = s->ddi_on ? 1 : 0;
+    P.damping_only = s->damping_only;
     P.pin = s->d_pin;
     P.stt_on = (s->u != 0.0) ? 1 : 0;
     if (P.stt_on) {
@@ -509,7 +510,7 @@ extern "C" int spin_geometry_create(const double bravais[9], int n_basis, const 
     s->ani_b.clear(); s->K.clear(); s->Kax.clear();
     s->ddi_on = 0; s->ddi_img[0] = s->ddi_img[1] = s->ddi_img[2] = 0;
     s->dt_ps = 1e-3; s->alpha = 0.1; s->T = 0; s->u = 0; s->jdir[0] = 1; s->jdir[1] = 0; s->jdir[2] = 0; s->beta = 0;
-    s->seed = 0; s->step = 0; s->solver = SPIN_SOLVER_DEPONDT;
+    s->seed = 0; s->step = 0; s->solver = SPIN_SOLVER_DEPONDT; s->damping_only = 0;
     s->stream = nullptr; s->own_stream = nullptr; s->cur = 0;
     s->d_n[0] = s->d_n[1] = s->d_np = s->d_A = s->d_fddi[0] = s->d_fddi[1] = s->d_aos = s->d_partials = s->d_result = nullptr;
     s->d_vp = nullptr; s->vp_active = false; s->vp_cur = 0;
@@ -832,6 +833,11 @@ extern "C" int llg_set_solver(spin_system *s, int solver) {
     REQUIRE(s, "null system");
     REQUIRE(solver == SPIN_SOLVER_DEPONDT || solver == SPIN_SOLVER_HEUN || solver == SPIN_SOLVER_SIB || solver == SPIN_SOLVER_RK4, "unknown solver %d", solver);
     if (s->solver != solver) { s->solver = solver; s->plan_dirty = true; drop_graphs(s); }
+    return SPIN_OK;
+}
+extern "C" int llg_set_damping_only(spin_system *s, int enabled) {
+    REQUIRE(s, "null system");
+    if (s->damping_only != (enabled ? 1 : 0)) { s->damping_only = enabled ? 1 : 0; s->plan_dirty = true; drop_graphs(s); }
     return SPIN_OK;
 }
 extern "C" int llg_get_step(const spin_system *s, uint64_t *step) {

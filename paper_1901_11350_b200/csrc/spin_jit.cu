@@ -245,6 +245,7 @@ std::string spin::jit_source(const spin_system *s) {
         o << "constexpr bool REVERSE_CORR = " << ((e && atoi(e) == 0) ? "false" : "true") << ";\n";
     }
     o << "constexpr bool MULTI_IMAGE = " << (s->n_img > 1 ? "true" : "false") << ";\n";
+    o << "constexpr bool DAMPING_ONLY = " << (s->damping_only ? "true" : "false") << ";\n";
     o << "constexpr bool HAS_PIN = " << (s->d_pin ? "true" : "false") << ";\n";
     o << "constexpr int SOLVER = " << s->solver << ";      // 0 Depondt, 1 Heun, 2 SIB, 3 RK4 (own stage kernel)\n";
     o << "constexpr bool STORE_A = " << ((s->opt_store_A && s->solver == 0) ? "true" : "false") << ", HAS_DDI = " << (P.has_ddi ? "true" : "false")

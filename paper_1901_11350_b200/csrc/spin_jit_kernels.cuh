@@ -193,9 +193,13 @@ template <int B>
 __device__ __forceinline__ void rotation_field(const double (&n)[3], const double (&F)[3], const double (&sg)[3], double (&A)[3]) {
     const double pre = specc::PRE[B], pa = specc::PREA[B];
     const double cx = fma(n[1], F[2], -n[2] * F[1]), cy = fma(n[2], F[0], -n[0] * F[2]), cz = fma(n[0], F[1], -n[1] * F[0]);
-    A[0] = fma(pa, cx, pre * F[0]);
-    A[1] = fma(pa, cy, pre * F[1]);
-    A[2] = fma(pa, cz, pre * F[2]);
+    if constexpr (spec::DAMPING_ONLY) {      // :168 "only the damping part of the LLG equation": the solvers become minimisers
+        A[0] = pa * cx; A[1] = pa * cy; A[2] = pa * cz;
+    } else {
+        A[0] = fma(pa, cx, pre * F[0]);
+        A[1] = fma(pa, cy, pre * F[1]);
+        A[2] = fma(pa, cz, pre * F[2]);
+    }
     if constexpr (spec::STT_ON) {
         const double sx = fma(n[1], sg[2], -n[2] * sg[1]), sy = fma(n[2], sg[0], -n[0] * sg[2]), sz = fma(n[0], sg[1], -n[1] * sg[0]);
         A[0] += fma(specc::STT_X, sx, specc::STT_S * sg[0]);

@@ -149,9 +149,10 @@ __device__ __forceinline__ void rotation_field(const DevicePlan &P, int b, const
                                                const double (&sg)[3], double (&A)[3]) {
     const double pre = P.pre[b], al = P.alpha;
     const double cx = n[1] * F[2] - n[2] * F[1], cy = n[2] * F[0] - n[0] * F[2], cz = n[0] * F[1] - n[1] * F[0];
-    A[0] = pre * (F[0] + al * cx);
-    A[1] = pre * (F[1] + al * cy);
-    A[2] = pre * (F[2] + al * cz);
+    const double pr = P.damping_only ? 0.0 : 1.0;      // :168 "only the damping part of the LLG equation"
+    A[0] = pre * (pr * F[0] + al * cx);
+    A[1] = pre * (pr * F[1] + al * cy);
+    A[2] = pre * (pr * F[2] + al * cz);
     if (P.stt_on) {
         const double sx = n[1] * sg[2] - n[2] * sg[1], sy = n[2] * sg[0] - n[0] * sg[2], sz = n[0] * sg[1] - n[1] * sg[0];
         A[0] += P.stt_s * sg[0] + P.stt_x * sx;

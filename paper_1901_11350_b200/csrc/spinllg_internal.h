@@ -83,7 +83,7 @@ struct DevicePlan {
     double stt_s, stt_x;                     // -u (alpha-beta)/(1+alpha^2),  u (1+alpha beta)/(1+alpha^2)
     uint32_t seed_lo, seed_hi;
     int thermal_on;
-    int pad_;
+    int damping_only;                        // 1: the precession term of Eq. 10 is dropped (:168)
     const unsigned char *pin;                // N flags in boundary order (b + nb*cell) or null: pinned spins are never updated
     PairEntry pairs[SPIN_MAX_PAIR_ENTRIES];
     QuadEntry quads[SPIN_MAX_QUAD_ENTRIES];
@@ -117,6 +117,7 @@ struct spin_system {
     double dt_ps, alpha, T, u, jdir[3], beta;
     uint64_t seed, step;
     int solver;                    // SPIN_SOLVER_*
+    int damping_only;              // drop the precession term (minimisation with the LLG solvers, :168)
     // ---- device
     cudaStream_t stream, own_stream;
     double *d_n[2];                // ping-pong spin buffers (nb*sub doubles each)

@@ -882,3 +882,21 @@ def test_biaxial_anisotropy_several_axes_per_atom(P, O):
     assert np.abs(g.spins_get() - o.spins()).max() <= SPIN_ATOL
     with pytest.raises(P.SpinError):
         g.hamiltonian_set_anisotropy([0] * 17, [0.1] * 17, [[0, 0, 1]] * 17)
+
+
+@pytest.mark.parametrize("cfg", [1, 3, 4])
+def test_damping_only_minimisation_parity(P, O, cfg):
+    """the LLG solvers as minimisers (precession term dropped); specialised and table-driven kernels against the oracle."""
+    w = dataclasses.replace(W.CONFIGS[cfg]().resized(REPLICAS[cfg], 1), T=0.0)
+    for use_jit, solver in ((1, 0), (1, 2), (0, 0)):
+        g, o = pair(P, O, w)
+        g.spin_set_option("use_jit", use_jit)
+        g.llg_set_solver(solver); o.set_solver(solver)
+        g.llg_set_damping_only(1); o.set_damping_only(True)
+        E0 = g.energy()[0]
+        g.llg_iterate(150); o.iterate(150)
+        assert np.abs(g.spins_get() - o.spins()).max() <= SPIN_ATOL
+        assert g.energy()[0] < E0
+        g.llg_set_damping_only(0); o.set_damping_only(False)
+        g.llg_iterate(20); o.iterate(20)
+        assert np.abs(g.spins_get() - o.spins()).max() <= SPIN_ATOL
