@@ -795,3 +795,29 @@ def test_damping_only_dynamics_closed_form():
     for _ in range(5):
         c.iterate(100); E.append(c.energy())
     assert all(b < a for a, b in zip(E, E[1:]))
+
+
+def test_current_driven_domain_wall_moves_at_beta_over_alpha_u():
+    """The experiment of Fig. 6: head-to-head wall in a chain along x with the biaxial Hamiltonian of Eq. 13 and the
+    end spins pinned.  Below the Walker breakdown the wall moves steadily ("linear fits" of Fig. 6) at the Zhang-Li / Thiaville (Ref. 53)
+    velocity v = (beta / alpha) u -- which pins both current terms of Eq. 10 for beta != alpha (O11 only covers beta = alpha), several
+    anisotropy axes per atom and pinning together.  Lattice discreteness and the approach to the steady state leave 2 %."""
+    N, alpha, beta, u = 240, 0.1, 0.2, 0.02
+    s = OracleSystem(np.eye(3), [[0, 0, 0]], (N, 1, 1), (0, 0, 0))
+    s.set_mu_s([2.0])
+    s.set_anisotropy([0, 0], [0.05, -0.03], [[1, 0, 0], [0, 1, 0]])        # easy axis x, hard axis y
+    s.set_pairs([0], [0], [[1, 0, 0]], [1.0])
+    s.llg_configure(10.0, alpha, 0.0, 0, u, (1, 0, 0), beta)
+    x = np.arange(N)
+    w = math.sqrt(1.0 / (2 * 0.05))
+    n0 = np.stack([-np.tanh((x - N / 2) / w), np.zeros(N), 1.0 / np.cosh((x - N / 2) / w)], axis=1)
+    n0 /= np.linalg.norm(n0, axis=1, keepdims=True)
+    mask = np.zeros(N, np.uint8); mask[0] = mask[-1] = 1
+    s.set_pinned(mask); s.set_spins(n0)
+    ts, xs = [], []
+    for k in range(160):
+        s.iterate(500)
+        ts.append((k + 1) * 5.0); xs.append(0.5 * (N + s.spins()[:, 0].sum()))      # wall position from sum n_x
+    v = np.polyfit(ts[120:], xs[120:], 1)[0]
+    assert v == pytest.approx(beta / alpha * u, rel=0.04), v
+    assert np.array_equal(s.spins()[0], n0[0]) and np.array_equal(s.spins()[-1], n0[-1])
