@@ -900,3 +900,16 @@ def test_damping_only_minimisation_parity(P, O, cfg):
         g.llg_set_damping_only(0); o.set_damping_only(False)
         g.llg_iterate(20); o.iterate(20)
         assert np.abs(g.spins_get() - o.spins()).max() <= SPIN_ATOL
+
+
+@pytest.mark.parametrize("B,branch", [(1.0, "degree-4 series"), (30.0, "degree-8 series"), (120.0, "trigonometric")])
+def test_rodrigues_branches(P, O, B, branch):
+    """The three evaluation branches of R(A) n (csrc/spin_device_math.cuh): |A| dt = gamma B dt = 0.009, 0.26 and 1.06 rad per step."""
+    w = dataclasses.replace(W.config3().resized((9, 5, 4), 1), B=B, dt_fs=50.0, alpha=0.1, pair_J=W.config3().pair_J * 0.01, pair_D=W.config3().pair_D * 0.01)
+    x = (0.176085963023 * B * 0.05) ** 2
+    assert {"degree-4 series": x < 2 ** -10, "degree-8 series": 2 ** -10 <= x < 0.25, "trigonometric": x >= 0.25}[branch]
+    for use_jit in (1, 0):
+        g, o = pair(P, O, w)
+        g.spin_set_option("use_jit", use_jit)
+        g.llg_iterate(60); o.iterate(60)
+        assert np.abs(g.spins_get() - o.spins()).max() < 1e-12, (branch, use_jit)
