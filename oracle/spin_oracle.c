@@ -27,11 +27,15 @@
  * Spin index (same as the C-ABI boundary): i = b + n_basis*(ia + Na*(ib + Nb*ic)).
  * Spins are stored AoS: n[3*i + {0,1,2}].
  *
- * Parity pins (tests/test_oracle_*.py): FM closed form, Larmor Eq. 12 with the paper's
- * printed 3e-7 error, finite differences, Euler identity, brute-force DDI, two-dipole and
- * monolayer closed forms, spin-spiral closed form, Langevin <n_z>, Philox known answers.
- * "parity unpinned" (convention only): DMI chirality sign of the helper
- * conventions (R15), DDI image count (R16), periodic self-wrap (R21), max-torque norm (R22).
+ * Parity pins (tests/test_oracle_pins.py): FM closed form, Larmor Eq. 12 with the paper's printed 3e-7 error, finite differences,
+ * Euler identity, brute-force DDI, two-dipole and monolayer closed forms, spin-spiral closed form, Langevin <n_z>, Philox known
+ * answers; Heun / SIB / RK4: convergence orders 2 / 2 / 4 on Eq. 12 and the exact Cayley rotation 2 atan(gamma B dt / 2); damping-only
+ * dynamics: tanh at fixed azimuth; velocity projection: (k + 1/2) dt^2 F / m and the FM ground state; pinned spins: Eq. 12 about the
+ * pinned neighbour; vacancies: decoupled neighbours; several anisotropy axes: biaxial closed form; topological charge: octant area,
+ * Girard's excess, Q = -1 / +1 / 0 / -2; GNEB: geodesic distance, force geometry, equidistant relaxation, barrier = K with a climbing
+ * image; image noise streams: moments and cross-correlations; current-driven wall of Fig. 6: velocity (beta / alpha) u.
+ * "parity unpinned" (convention only): DMI chirality sign of the helper conventions (R15), DDI image count (R16),
+ * periodic self-wrap (R21), max-torque norm (R22), the optimiser of the GNEB chain (steepest descent, R31).
  *
  * Build: gcc -O2 -ffp-contract=off -fopenmp -shared -fPIC (see oracle/build.py).
  */
