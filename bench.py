@@ -239,6 +239,7 @@ def main():
     ms_per_iter = ms_max / (inner * args.steps)
     corr_live_ms = ms_per_iter * per_iter["corrector"] / tot            # share from the profiled pass x live time per iteration
     peak, peak_src = measured_peaks()
+    fp64_tflops = sys_.spin_measure_fp64_tflops()       # the ALU ceiling: the path sits near the fp64 ridge (about 5 flop/B)
     achieved = ALG_BYTES_CORRECTOR * N / (corr_live_ms * 1e-3) / 1e9
     step_gbs = ALG_BYTES_STEP * N / (ms_per_iter * 1e-3) / 1e9
 
@@ -260,7 +261,10 @@ def main():
                          "algorithmic_bytes_per_launch": ALG_BYTES_CORRECTOR * N, "launch_ms": corr_live_ms,
                          "kernel_share_of_step": per_iter["corrector"] / tot,
                          "step_effective_gbs": step_gbs, "step_frac_of_peak": step_gbs / peak, "step_frac_of_8000": step_gbs / 8000.0,
-                         "profiled_ms": per_iter},
+                         "profiled_ms": per_iter,
+                         # fp64 instructions per spin-update counted by ncu on cfg3 (profiles/r1e): 77 + 130 warp instructions of 32 lanes
+                         "fp64_peak_tflops_measured": fp64_tflops,
+                         "fp64_frac_cfg3_count": (2.0 * 207 * N / (ms_per_iter * 1e-3) / 1e12) / fp64_tflops if w.name.startswith("cfg3") else None},
         }
         if world == 1 and not args.no_cpu_baseline:
             v, cores, sample = oracle_rate(w)

@@ -183,6 +183,8 @@ int spin_launch_counts(const spin_system *sys, int64_t *own_kernels, int64_t *cu
  * accumulated milliseconds and launch counts for kind = 0 predictor, 1 corrector, 2 ddi (all ddi stages).   */
 int spin_profile_enable(spin_system *sys, int enabled);
 int spin_profile_get(spin_system *sys, int kind, double *total_ms, int64_t *launches);
+/* measured fp64 FMA throughput of this device in TFLOP/s (register-only kernel, best of 5): the ALU ceiling next to the HBM one */
+int spin_measure_fp64_tflops(spin_system *sys, double *tflops);
 /* execution options: use_graph (capture steps into a CUDA graph; default 1), store_A (1: predictor stores the
  * rotation field A, 0: corrector recomputes it; default 0)                                                  */
 int spin_set_option(spin_system *sys, const char *name, int value);

@@ -22,7 +22,7 @@ EXPORTS = [
     "hamiltonian_set_ddi", "spin_set_images", "spin_select_image", "llg_set_image_temperatures", "gneb_forces", "gneb_iterate", "spins_set_pinned", "spins_set", "spins_get", "spins_set_device", "spins_get_device",
     "llg_configure", "llg_set_solver", "llg_set_damping_only", "minimise_vp", "minimise_vp_reset", "llg_iterate", "llg_get_step", "llg_set_step", "spin_synchronize",
     "effective_field", "effective_field_device", "energy", "observables", "topological_charge",
-    "spin_launch_counts", "spin_profile_enable", "spin_profile_get", "spin_set_option",
+    "spin_launch_counts", "spin_measure_fp64_tflops", "spin_profile_enable", "spin_profile_get", "spin_set_option",
     "spin_kernel_info", "spin_jit_source", "spin_last_error", "spin_version",
 ]
 
@@ -65,6 +65,7 @@ def lib() -> C.CDLL:
         "llg_set_solver": (C.c_int, [vp, C.c_int]),
         "llg_set_damping_only": (C.c_int, [vp, C.c_int]),
         "spins_set_pinned": (C.c_int, [vp, C.c_void_p]),
+        "spin_measure_fp64_tflops": (C.c_int, [vp, dp]),
         "spin_set_images": (C.c_int, [vp, C.c_int]),
         "gneb_forces": (C.c_int, [vp, C.c_double, C.c_int, dp, dp, dp]),
         "gneb_iterate": (C.c_int, [vp, C.c_int64, C.c_double, C.c_double, C.c_int]),
@@ -252,6 +253,11 @@ class SpinSystem:
             return
         a = np.ascontiguousarray(np.asarray(T, dtype=np.float64).reshape(-1))
         _check(lib().llg_set_image_temperatures(self._h, a.ctypes.data_as(C.POINTER(C.c_double))))
+
+    def spin_measure_fp64_tflops(self):
+        v = C.c_double(0.0)
+        _check(lib().spin_measure_fp64_tflops(self._h, C.byref(v)))
+        return float(v.value)
 
     def minimise_vp(self, n_iterations, dt, mass=1.0):
         _check(lib().minimise_vp(self._h, int(n_iterations), float(dt), float(mass)))

@@ -1130,6 +1130,29 @@ extern "C" int spin_launch_counts(const spin_system *s, int64_t *own, int64_t *f
     if (fft) *fft = s->n_fft;
     return SPIN_OK;
 }
+// measured fp64 FMA throughput of the device in TFLOP/s (2 flops per fma), best of 5 launches of a register-only kernel
+extern "C" int spin_measure_fp64_tflops(spin_system *s, double *tflops) {
+    REQUIRE(s && tflops, "null argument");
+    NEED_DEVICE(s);
+    int dev = 0, sms = 148;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    const int iters = 1 << 14, blocks = sms * 16;
+    double best = 0.0;
+    for (int rep = 0; rep < 6; ++rep) {
+        SPIN_CUDA(cudaEventRecord(s->ev0, s->stream));
+        fp64_rate_kernel<<<blocks, 256, 0, s->stream>>>(s->d_result, iters, 0.999999, 1e-9);
+        SPIN_CUDA(cudaEventRecord(s->ev1, s->stream));
+        SPIN_CUDA(cudaEventSynchronize(s->ev1));
+        float ms = 0.f;
+        SPIN_CUDA(cudaEventElapsedTime(&ms, s->ev0, s->ev1));
+        const double tf = 2.0 * 8.0 * (double)iters * 256.0 * blocks / (ms * 1e-3) / 1e12;
+        if (rep > 0 && tf > best) best = tf;
+    }
+    s->n_launch += 6;
+    *tflops = best;
+    return SPIN_OK;
+}
 extern "C" int spin_profile_enable(spin_system *s, int on) {
     REQUIRE(s, "null system");
     s->profile_on = on ? 1 : 0;

@@ -592,6 +592,17 @@ __global__ void topo_final_kernel(const double *__restrict__ partials, int nbloc
     if (threadIdx.x == 0) out[0] = r * (1.0 / (4.0 * 3.14159265358979323846));
 }
 
+// fp64 FMA rate of the device (measurement support): 8 independent dependent chains per thread, 2 flops per fma
+__global__ void __launch_bounds__(256) fp64_rate_kernel(double *out, int iters, double a, double b) {
+    double x0 = threadIdx.x, x1 = x0 + 1, x2 = x0 + 2, x3 = x0 + 3, x4 = x0 + 4, x5 = x0 + 5, x6 = x0 + 6, x7 = x0 + 7;
+    for (int i = 0; i < iters; ++i) {
+        x0 = fma(x0, a, b); x1 = fma(x1, a, b); x2 = fma(x2, a, b); x3 = fma(x3, a, b);
+        x4 = fma(x4, a, b); x5 = fma(x5, a, b); x6 = fma(x6, a, b); x7 = fma(x7, a, b);
+    }
+    const double r = x0 + x1 + x2 + x3 + x4 + x5 + x6 + x7;
+    if (r == 123.456) out[0] = r;          // never true: keeps the chains alive
+}
+
 __global__ void advance_step_kernel(unsigned long long *d_step, unsigned long long add) { *d_step += add; }
 
 }  // namespace spin
