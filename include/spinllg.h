@@ -95,7 +95,7 @@ int hamiltonian_set_quadruplets(spin_system *sys, int n, const int *basis_ijkl /
 int hamiltonian_set_ddi(spin_system *sys, int enabled, const int n_periodic_images[3]);
 
 /* ---- state ---------------------------------------------------------------------------------------------- */
-/* spins are normalised on input; zero vectors are an error */
+/* spins are normalised on input; a zero vector is an error except on a pinned site (a vacancy, see spins_set_pinned) */
 int spins_set(spin_system *sys, const double *n_xyz /*host, 3N AoS*/);
 int spins_get(spin_system *sys, double *n_xyz /*host, 3N AoS*/);
 int spins_set_device(spin_system *sys, const double *n_xyz /*device, 3N AoS*/);
