@@ -459,15 +459,22 @@ int enqueue_force(spin_system *s, int mask, double *d_out) {
     return SPIN_OK;
 }
 
-int reduce_all(spin_system *s, double out[N_RED]) {
+// the N_RED reductions of the selected image into d_out (device), no synchronisation
+int enqueue_reduce(spin_system *s, double *d_out) {
     const Launch L = brick_launch(s);
     double *n = s->d_n[s->cur] + img_off(s);
     if (s->ddi_on) { int rc = ddi_field(s, n, s->d_fddi[0]); if (rc) return rc; }
     const int nblocks = (int)(L.grid.x * L.grid.y);
     if (L.flat) reduce_kernel<32, 8, 1><<<L.grid, L.block, 0, s->stream>>>(s->plan, n, s->d_fddi[0], s->d_partials);
     else reduce_kernel<32, 4, 2><<<L.grid, L.block, 0, s->stream>>>(s->plan, n, s->d_fddi[0], s->d_partials);
-    reduce_final_kernel<<<1, 32 * N_RED, 0, s->stream>>>(s->d_partials, nblocks, s->d_result);
+    reduce_final_kernel<<<1, 32 * N_RED, 0, s->stream>>>(s->d_partials, nblocks, d_out);
     s->n_launch += 2;
+    return SPIN_OK;
+}
+
+int reduce_all(spin_system *s, double out[N_RED]) {
+    int rc = enqueue_reduce(s, s->d_result);
+    if (rc) return rc;
     SPIN_CUDA(cudaMemcpyAsync(out, s->d_result, N_RED * sizeof(double), cudaMemcpyDeviceToHost, s->stream));
     SPIN_CUDA(cudaStreamSynchronize(s->stream));
     SPIN_CUDA(cudaGetLastError());
@@ -1030,7 +1037,8 @@ int gneb_run(spin_system *s, int64_t n_iter, double step, double kappa, int clim
     SPIN_CUDA(cudaMalloc(&d_part, (size_t)M * nblocks * 3 * sizeof(double)));
     SPIN_CUDA(cudaMalloc(&d_sc, (size_t)M * 3 * sizeof(double)));
     SPIN_CUDA(cudaMalloc(&d_E, (size_t)M * sizeof(double)));
-    std::vector<double> E((size_t)M);
+    double *d_red = nullptr;                     // N_RED reductions per image; the energies never leave the device during the relaxation
+    SPIN_CUDA(cudaMalloc(&d_red, (size_t)M * 16 * sizeof(double)));
     const int sel = s->img_sel;
     int rc = SPIN_OK;
     dim3 grid(L.grid.x, L.grid.y, (unsigned)M);
@@ -1038,13 +1046,12 @@ int gneb_run(spin_system *s, int64_t n_iter, double step, double kappa, int clim
     for (int64_t it = 0; it < n_iter && rc == SPIN_OK; ++it) {
         for (int nu = 0; nu < M && rc == SPIN_OK; ++nu) {          // energy and force of every image
             s->img_sel = nu;
-            double r[N_RED];
-            rc = reduce_all(s, r);
-            E[(size_t)nu] = r[0] + r[1] + r[2] + r[3] + r[4] + r[5];
+            rc = enqueue_reduce(s, d_red + 16 * nu);
             if (rc == SPIN_OK) rc = enqueue_force(s, T_ALL, G_all + nu * istr);
         }
         if (rc) break;
-        cudaMemcpyAsync(d_E, E.data(), (size_t)M * sizeof(double), cudaMemcpyHostToDevice, s->stream);
+        gneb_energy_kernel<<<1, 64, 0, s->stream>>>(d_red, M, d_E);
+        s->n_launch++;
         const double st = want_outputs ? 0.0 : step;
         if (L.flat) {
             gneb_tangent_kernel<32, 8, 1><<<grid, L.block, 0, s->stream>>>(s->plan, n_all, G_all, d_E, M, istr, tau_all, d_part);
@@ -1056,11 +1063,13 @@ int gneb_run(spin_system *s, int64_t n_iter, double step, double kappa, int clim
             gneb_assemble_kernel<32, 4, 2><<<grid, L.block, 0, s->stream>>>(s->plan, n_all, G_all, tau_all, d_sc, M, istr, kappa, climbing, st);
         }
         s->n_launch += 3;
-        cudaError_t e = cudaStreamSynchronize(s->stream);        // E (host vector) is reused by the next iteration
+    }
+    if (rc == SPIN_OK) {
+        cudaError_t e = cudaStreamSynchronize(s->stream);
         if (e != cudaSuccess) rc = spin::fail(SPIN_ERR_CUDA, "gneb: %s", cudaGetErrorString(e));
     }
     if (rc == SPIN_OK && want_outputs) {
-        if (E_host) memcpy(E_host, E.data(), (size_t)M * sizeof(double));
+        if (E_host) cudaMemcpy(E_host, d_E, (size_t)M * sizeof(double), cudaMemcpyDeviceToHost);
         if (l_host) {
             std::vector<double> sc((size_t)3 * M);
             cudaMemcpy(sc.data(), d_sc, sc.size() * sizeof(double), cudaMemcpyDeviceToHost);
@@ -1077,7 +1086,7 @@ int gneb_run(spin_system *s, int64_t n_iter, double step, double kappa, int clim
         }
     }
     s->img_sel = sel;
-    cudaFree(d_part); cudaFree(d_sc); cudaFree(d_E);
+    cudaFree(d_part); cudaFree(d_sc); cudaFree(d_E); cudaFree(d_red);
     if (rc == SPIN_OK && cudaGetLastError() != cudaSuccess) rc = spin::fail(SPIN_ERR_CUDA, "gneb: kernel launch failed");
     return rc;
 }

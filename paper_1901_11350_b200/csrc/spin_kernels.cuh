@@ -500,6 +500,13 @@ __global__ void __launch_bounds__(BX *BY *BZ)
         partials[((size_t)nu * nblocks + (size_t)blockIdx.y * gridDim.x + blockIdx.x) * 3 + threadIdx.x] = r;
     }
 }
+// total energy of every image from its six terms (red: 16 doubles per image, the output of reduce_final_kernel)
+__global__ void gneb_energy_kernel(const double *__restrict__ red, int M, double *__restrict__ E) {
+    for (int nu = threadIdx.x; nu < M; nu += blockDim.x) {
+        const double *r = red + 16 * nu;
+        E[nu] = r[0] + r[1] + r[2] + r[3] + r[4] + r[5];
+    }
+}
 // one warp per image: sc[nu] = {|tau|, G.tau^, l_{nu,nu+1}}
 __global__ void gneb_final_kernel(const double *__restrict__ partials, int nblocks, double *__restrict__ sc) {
     const int nu = blockIdx.x;
