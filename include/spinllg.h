@@ -195,6 +195,8 @@ int spin_set_option(spin_system *sys, const char *name, int value);
  * cfg3, hence off by default.
  * use_col (default 0): 1 runs them as column-marching kernels (one thread per lattice column, own spin at z-1, z, z+1 kept in
  * registers; 3-D lattices).  Also measured slower than the brick kernels.
+ * use_pair (default 0): 1 runs them with two sites (ia, ia+1) per thread and 128-bit loads and stores (even Na; Depondt solver, no
+ * pinned spins, one image); 26 % fewer instructions and fewer L1 wavefronts, measured equal (predictor) or slower (corrector).
  * use_fused (default 0): 1 runs the Depondt step in one pass (predictor for tile + rim into shared memory, corrector from it; 48 B
  * per spin-update of HBM traffic; lattices of at least 16384 spins, 2 forces it).  Measured slower than the brick kernels on cfg3.
  * use_coop (default 1): lattices of up to 4096 spins without dipolar coupling run ALL steps of an llg_iterate call in one launch

@@ -412,9 +412,10 @@ int enqueue_step_t(spin_system *s, const Launch &L, unsigned step_add) {
         if (rc) return rc;
         if (prof) { cudaEventRecord(s->ev1, s->stream); cudaEventSynchronize(s->ev1); float ms; cudaEventElapsedTime(&ms, s->ev0, s->ev1); s->prof_ms[2] += ms; s->prof_n[2]++; }
     }
-    const bool jit = jit_ready(s), col = jit_col_ready(s), tma = !col && jit_tma_ready(s);
+    const bool jit = jit_ready(s), pair = jit_pair_ready(s), col = !pair && jit_col_ready(s), tma = !pair && !col && jit_tma_ready(s);
     if (prof) cudaEventRecord(s->ev0, s->stream);
-    if (col) { int rc = jit_launch_predictor_col(s, n, s->d_fddi[0], s->d_np, step_add); if (rc) return rc; }
+    if (pair) { int rc = jit_launch_predictor_pair(s, n, s->d_fddi[0], s->d_np, step_add); if (rc) return rc; }
+    else if (col) { int rc = jit_launch_predictor_col(s, n, s->d_fddi[0], s->d_np, step_add); if (rc) return rc; }
     else if (tma) { int rc = jit_launch_predictor_tma(s, s->cur, s->d_fddi[0], s->d_np, step_add); if (rc) return rc; }
     else if (jit) { int rc = jit_launch_predictor(s, L.grid, L.block, n, s->d_fddi[0], s->d_np, s->d_A, step_add); if (rc) return rc; }
     else if (s->opt_store_A)
@@ -431,7 +432,8 @@ int enqueue_step_t(spin_system *s, const Launch &L, unsigned step_add) {
         if (prof) { cudaEventRecord(s->ev1, s->stream); cudaEventSynchronize(s->ev1); float ms; cudaEventElapsedTime(&ms, s->ev0, s->ev1); s->prof_ms[2] += ms; s->prof_n[2]++; }
     }
     if (prof) cudaEventRecord(s->ev0, s->stream);
-    if (col) { int rc = jit_launch_corrector_col(s, n, s->d_np, s->d_fddi[0], s->d_fddi[1], nout, step_add); if (rc) return rc; }
+    if (pair) { int rc = jit_launch_corrector_pair(s, n, s->d_np, s->d_fddi[0], s->d_fddi[1], nout, step_add); if (rc) return rc; }
+    else if (col) { int rc = jit_launch_corrector_col(s, n, s->d_np, s->d_fddi[0], s->d_fddi[1], nout, step_add); if (rc) return rc; }
     else if (tma) { int rc = jit_launch_corrector_tma(s, s->cur, s->d_fddi[0], s->d_fddi[1], nout, step_add); if (rc) return rc; }
     else if (jit) { int rc = jit_launch_corrector(s, L.grid, L.block, n, s->d_np, s->d_fddi[0], s->d_fddi[1], s->d_A, nout, step_add); if (rc) return rc; }
     else if (s->opt_store_A)
@@ -504,7 +506,7 @@ extern "C" int spin_geometry_create(const double bravais[9], int n_basis, const 
     if (!has_device) cudaGetLastError();
     spin_system *s = new spin_system();
     s->has_device = has_device;
-    s->jit = nullptr; s->opt_jit = 1; s->opt_tma = 0; s->opt_ddi_slab = 1; s->opt_col = 0; s->opt_cache_noise = 1; s->opt_coop = 1; s->opt_fused = 0; s->d_bar = nullptr;
+    s->jit = nullptr; s->opt_jit = 1; s->opt_tma = 0; s->opt_ddi_slab = 1; s->opt_col = 0; s->opt_pair = 0; s->opt_cache_noise = 1; s->opt_coop = 1; s->opt_fused = 0; s->d_bar = nullptr;
     s->n_img = 1; s->img_sel = 0; s->d_img_sigma = nullptr;
     memcpy(s->brav, bravais, sizeof(s->brav));
     s->nb = n_basis;
@@ -1182,6 +1184,7 @@ extern "C" int spin_set_option(spin_system *s, const char *name, int value) {
     else if (!strcmp(name, "use_fused")) { s->opt_fused = value < 0 ? 0 : (value > 2 ? 2 : value); s->plan_dirty = true; }
     else if (!strcmp(name, "use_coop")) { s->opt_coop = value < 0 ? 0 : (value > 3 ? 3 : value); s->plan_dirty = true; }
     else if (!strcmp(name, "cache_noise")) { s->opt_cache_noise = value ? 1 : 0; s->plan_dirty = true; }
+    else if (!strcmp(name, "use_pair")) { s->opt_pair = value ? 1 : 0; s->plan_dirty = true; }
     else if (!strcmp(name, "use_col")) { s->opt_col = value ? 1 : 0; s->plan_dirty = true; }
     else if (!strcmp(name, "ddi_slab")) { s->opt_ddi_slab = value ? 1 : 0; s->plan_dirty = true; }
     else if (!strcmp(name, "use_tma")) { s->opt_tma = value < 0 ? 0 : (value > 2 ? 2 : value); s->plan_dirty = true; }
@@ -1196,6 +1199,7 @@ extern "C" int spin_kernel_info(spin_system *s, char *buf, int len) {
     if (s->has_device) { int rc = ensure_plan(s); if (rc) return rc; }
     if (jit_fused_ready(s)) snprintf(buf, (size_t)len, "jit+fused");
     else if (jit_coop_ready(s) && s->opt_coop && !s->ddi_on && (s->N <= SPIN_COOP_MAX_SPINS || s->opt_coop >= 2)) snprintf(buf, (size_t)len, jit_cluster_ready(s) ? "jit+cluster" : "jit+coop");
+    else if (jit_pair_ready(s)) snprintf(buf, (size_t)len, "jit+pair");
     else if (jit_col_ready(s)) snprintf(buf, (size_t)len, "jit+col");
     else if (jit_tma_ready(s)) snprintf(buf, (size_t)len, "jit+tma");
     else if (jit_ready(s)) snprintf(buf, (size_t)len, "jit (brick sweeps)");

@@ -55,6 +55,10 @@ struct JitState {
     bool col;
     cudaKernel_t k_pred_col, k_corr_col;
     int col_geo[4];           // CBX, CBY, CCZ, CNZC
+    // two sites per thread, 128-bit accesses (spin_jit_pair.cuh)
+    bool pair;
+    cudaKernel_t k_pred_pair, k_corr_pair;
+    int pair_geo[3];          // VBX, VBY, VBZ
     int grid_p, grid_c;
     CUtensorMap tm_n[2];              // predictor: n[cur] with the predictor tile
     CUtensorMap tm_cn[2], tm_cnp;     // corrector: n[cur], n^p with the corrector tile
@@ -208,6 +212,26 @@ static bool plan_col(const spin_system *s, int g[4]) {
     return true;
 }
 
+// two sites per thread (spin_jit_pair.cuh): brick of sites per block; false if not applicable (odd rows, options the variant does not
+// carry).  SPINLLG_PAIR="vbx,vby,vbz" overrides the default brick (32 x 4 x 2 sites = 128 threads).
+static bool plan_pair(const spin_system *s, int g[3]) {
+    const DevicePlan &P = s->plan;
+    if (!s->opt_pair || s->opt_store_A || s->solver != 0 || s->d_pin || s->n_img > 1) return false;
+    if (P.Na % 2 || P.LA % 2 || P.PA % 2 || P.sub % 2) return false;
+    int v[3] = {32, 4, 2};
+    if (const char *e = getenv("SPINLLG_PAIR")) {
+        int w[3] = {0, 0, 0};
+        sscanf(e, "%d,%d,%d", &w[0], &w[1], &w[2]);
+        for (int k = 0; k < 3; ++k) if (w[k] > 0) v[k] = w[k];
+    }
+    if (P.Nc == 1) { v[1] *= v[2]; v[2] = 1; }
+    while (v[0] > 2 && v[0] / 2 >= P.Na) { v[0] /= 2; v[1] *= 2; }      // short rows: same threads, more rows per block
+    const int threads = v[0] / 2 * v[1] * v[2];
+    if (v[0] % 2 || threads % 32 || threads > 1024) return false;
+    g[0] = v[0]; g[1] = v[1]; g[2] = v[2];
+    return true;
+}
+
 // the staging geometry of both sweeps, or why the TMA-fed sweeps are not generated for this system
 static bool plan_tma(const spin_system *s, TmaGeo &gp, TmaGeo &gc, std::string &why) {
     if (!s->opt_tma) { why = "disabled by option use_tma=0"; return false; }
@@ -336,6 +360,8 @@ std::string spin::jit_source(const spin_system *s) {
     int cg[4];
     const bool col = plan_col(s, cg);
     if (col) o << "namespace spec { constexpr int CBX = " << cg[0] << ", CBY = " << cg[1] << ", CCZ = " << cg[2] << ", CNZC = " << cg[3] << "; }\n#define SPIN_COL 1\n";
+    int pg[3];
+    if (plan_pair(s, pg)) o << "namespace spec { constexpr int VBX = " << pg[0] << ", VBY = " << pg[1] << ", VBZ = " << pg[2] << "; }\n#define SPIN_PAIR 1\n";
     if (tma) o << "#define SPIN_TMA 1\n";
     o << "#include \"spin_jit_kernels.cuh\"\n";
     return o.str();
@@ -493,6 +519,12 @@ static void variants_prepare(spin_system *s, JitState *j) {
         if (e == cudaSuccess) e = cudaLibraryGetKernel(&j->k_corr_col, j->lib, "jit_corrector_col");
         if (e != cudaSuccess) { cudaGetLastError(); j->col = false; }
     }
+    j->pair = plan_pair(s, j->pair_geo);
+    if (j->pair) {
+        cudaError_t e = cudaLibraryGetKernel(&j->k_pred_pair, j->lib, "jit_predictor_pair");
+        if (e == cudaSuccess) e = cudaLibraryGetKernel(&j->k_corr_pair, j->lib, "jit_corrector_pair");
+        if (e != cudaSuccess) { cudaGetLastError(); j->pair = false; }
+    }
 }
 
 int spin::jit_prepare(spin_system *s) {
@@ -506,6 +538,7 @@ int spin::jit_prepare(spin_system *s) {
     j->loaded = false;
     j->tma = false;
     j->col = false;
+    j->pair = false;
     j->coop = false;
     j->fused = false;
     j->source = src;
@@ -643,6 +676,38 @@ int spin::jit_launch_corrector_col(spin_system *s, const double *n, const double
     dim3 grid, block;
     col_launch_dims(s, j, grid, block);
     SPIN_CUDA(cudaLaunchKernel((const void *)j->k_corr_col, grid, block, args, 0, s->stream));
+    return SPIN_OK;
+}
+
+bool spin::jit_pair_ready(const spin_system *s) { return s->jit && s->jit->loaded && s->jit->pair; }
+
+static void pair_launch_dims(const spin_system *s, const JitState *j, dim3 &grid, dim3 &block) {
+    const int *g = j->pair_geo;
+    grid = dim3((unsigned)(((s->nc[0] + g[0] - 1) / g[0]) * ((s->nc[1] + g[1] - 1) / g[1]) * ((s->nc[2] + g[2] - 1) / g[2])), (unsigned)s->nb, 1);
+    block = dim3((unsigned)(g[0] / 2 * g[1] * g[2]), 1, 1);
+}
+
+int spin::jit_launch_predictor_pair(spin_system *s, const double *n, const double *fddi, double *np, unsigned step_add) {
+    JitState *j = s->jit;
+    unsigned seed_lo = s->plan.seed_lo, seed_hi = s->plan.seed_hi;
+    const unsigned long long *d_step = s->d_step;
+    void *args[] = {(void *)&n, (void *)&fddi, (void *)&np, (void *)&d_step, (void *)&step_add, (void *)&seed_lo, (void *)&seed_hi};
+    dim3 grid, block;
+    pair_launch_dims(s, j, grid, block);
+    SPIN_CUDA(cudaLaunchKernel((const void *)j->k_pred_pair, grid, block, args, 0, s->stream));
+    return SPIN_OK;
+}
+
+int spin::jit_launch_corrector_pair(spin_system *s, const double *n, const double *np, const double *fddi_n, const double *fddi_np, double *nout,
+                                    unsigned step_add) {
+    JitState *j = s->jit;
+    unsigned seed_lo = s->plan.seed_lo, seed_hi = s->plan.seed_hi;
+    const unsigned long long *d_step = s->d_step;
+    void *args[] = {(void *)&n, (void *)&np, (void *)&fddi_n, (void *)&fddi_np, (void *)&nout, (void *)&d_step, (void *)&step_add, (void *)&seed_lo,
+                    (void *)&seed_hi};
+    dim3 grid, block;
+    pair_launch_dims(s, j, grid, block);
+    SPIN_CUDA(cudaLaunchKernel((const void *)j->k_corr_pair, grid, block, args, 0, s->stream));
     return SPIN_OK;
 }
 

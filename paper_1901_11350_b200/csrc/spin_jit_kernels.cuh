@@ -63,9 +63,8 @@ __device__ __forceinline__ void load3(const double *__restrict__ q, double (&v)[
 __device__ __forceinline__ void store3(double *__restrict__ q, const double (&v)[3]) {
     q[0] = v[0]; q[spec::PA] = v[1]; q[2 * spec::PA] = v[2];
 }
-// a spin and its periodic images in the ghost layers (at most one image per direction)
-__device__ __forceinline__ void store_spin(double *__restrict__ q, const Coord &c, const double (&v)[3]) {
-    store3(q, v);
+// the periodic images of a spin in the ghost layers (at most one image per direction)
+__device__ __forceinline__ void store_images(double *__restrict__ q, const Coord &c, const double (&v)[3]) {
     if constexpr (spec::GA || spec::GB || spec::GC) {
         // one unsigned compare per direction decides whether the site has any image at all (interior sites: nearly all)
         bool edge = false;
@@ -84,6 +83,10 @@ __device__ __forceinline__ void store_spin(double *__restrict__ q, const Coord &
             }
         }
     }
+}
+__device__ __forceinline__ void store_spin(double *__restrict__ q, const Coord &c, const double (&v)[3]) {
+    store3(q, v);
+    store_images(q, c, v);
 }
 
 // Site accessors: where the partner (sublattice BJ at translation DA, DB, DC) of a site of sublattice B is read from.
@@ -543,6 +546,9 @@ extern "C" __global__ void SPIN_BOUNDS(spec::BX *spec::BY *spec::BZ)
 #endif
 #ifdef SPIN_COL
 #include "spin_jit_col.cuh"
+#endif
+#ifdef SPIN_PAIR
+#include "spin_jit_pair.cuh"
 #endif
 #ifdef SPIN_TMA
 #include "spin_jit_tma.cuh"

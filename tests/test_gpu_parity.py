@@ -379,6 +379,49 @@ def test_column_marching_with_open_and_mixed_boundaries(P, O):
 
 
 # ---------------------------------------------------------------------------------------------------------------------
+# Two sites per thread with 128-bit accesses (csrc/spin_jit_pair.cuh), option use_pair=1: same arithmetic, bit-identical
+@pytest.mark.parametrize("cfg,cells,steps,geo", [(1, (34, 9, 1), 100, None), (2, (70, 33, 1), 100, None), (3, (36, 9, 7), 60, None),
+                                                 (3, (70, 37, 11), 20, "64,2,2"), (3, (2, 5, 3), 50, None), (4, (34, 17, 1), 100, None),
+                                                 (5, (20, 12, 5), 20, None), (5, (20, 12, 4), 20, "16,4,4")])
+def test_pair_sweeps(P, O, cfg, cells, steps, geo, monkeypatch):
+    if geo:
+        monkeypatch.setenv("SPINLLG_PAIR", geo)
+    w = W.CONFIGS[cfg]().resized(cells, steps)
+    g, o = pair(P, O, w)
+    g.spin_set_option("use_pair", 1)
+    g.spin_set_option("use_coop", 0)
+    assert g.spin_kernel_info() == "jit+pair", g.spin_kernel_info()
+    g.llg_iterate(steps); o.iterate(steps)
+    d = np.abs(g.spins_get() - o.spins()).max()
+    print(f"pair cfg{cfg} {cells} steps={steps}: max|dn| = {d:.3e}")
+    assert d <= SPIN_ATOL
+    b = P.SpinSystem.from_workload(w)
+    b.spin_set_option("use_coop", 0)
+    assert b.spin_kernel_info().startswith("jit (brick")
+    b.llg_iterate(steps)
+    assert np.array_equal(b.spins_get(), g.spins_get())
+
+
+def test_pair_sweeps_boundaries_and_fallback(P, O):
+    for per in [(0, 0, 0), (1, 0, 1), (0, 1, 0)]:
+        w = dataclasses.replace(W.config3().resized((22, 10, 9), 30), periodic=per)
+        g, o = pair(P, O, w)
+        g.spin_set_option("use_pair", 1)
+        g.spin_set_option("use_coop", 0)
+        assert g.spin_kernel_info() == "jit+pair"
+        g.llg_iterate(30); o.iterate(30)
+        assert np.abs(g.spins_get() - o.spins()).max() <= SPIN_ATOL
+    # an odd row length cannot be paired: the option is ignored, the brick sweeps run
+    w = W.config3().resized((21, 10, 9), 10)
+    g, o = pair(P, O, w)
+    g.spin_set_option("use_pair", 1)
+    g.spin_set_option("use_coop", 0)
+    assert g.spin_kernel_info().startswith("jit (brick"), g.spin_kernel_info()
+    g.llg_iterate(10); o.iterate(10)
+    assert np.abs(g.spins_get() - o.spins()).max() <= SPIN_ATOL
+
+
+# ---------------------------------------------------------------------------------------------------------------------
 # Other solvers on the same field sweeps: Heun (App. B B3-B4), SIB (App. C C5-C11), RK4 (:168; solver 3)
 @pytest.mark.parametrize("solver", [1, 2, 3])
 @pytest.mark.parametrize("cfg,steps", [(1, 300), (2, 200), (3, 150), (4, 150), (5, 30)])
