@@ -149,6 +149,7 @@ def main():
     ap.add_argument("--inner", type=int, default=128, help="LLG iterations per bench step (a multiple of the 16-step CUDA graph)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--store-A", type=int, default=0)
+    ap.add_argument("--option", action="append", default=[], metavar="NAME=VALUE", help="spin_set_option pass-through (e.g. use_pdl=0) for A/B runs")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     w = W.CONFIGS[args.config]()
@@ -181,6 +182,9 @@ def main():
     n0 = w.initial_spins()
     sys_ = P.SpinSystem.from_workload(w, stream=stream.cuda_stream)
     sys_.spin_set_option("store_A", args.store_A)
+    for kv in args.option:
+        name, value = kv.split("=")
+        sys_.spin_set_option(name, int(value))
     N = sys_.N
     inner = args.inner
 

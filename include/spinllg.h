@@ -203,6 +203,10 @@ int spin_set_option(spin_system *sys, const char *name, int value);
  * instead of two launches per step: as one thread-block cluster with its hardware barrier between the sweeps (up to 16 bricks), else
  * as a cooperative launch with a grid barrier; 2 forces the path for any size (slower beyond about 10^4 spins), 3 forces the grid
  * barrier, 0 switches it off.
+ * use_pdl (default -1 = automatic): programmatic dependent launch of the two brick sweeps -- each sweep is launched with programmatic
+ * stream serialisation and waits inside the kernel (griddepcontrol.wait) for the previous kernel, so its launch latency and block ramp
+ * overlap the tail of the one before; 1 releases the dependents at entry (the automatic choice for lattices of many waves of blocks),
+ * 2 at the end of each block, 0 switches it off (the automatic choice for lattices of about one wave).  The order of all memory accesses, and with it every result bit, is unchanged.
  * cache_noise (default 1): the predictor keeps the thermal field of the step (24 B/spin) for the corrector instead of generating it twice.
  * ddi_slab (default 1): thin films with one basis atom take the dipolar slab path (2-D cuFFT + fused transform along c).
  * spin_kernel_info writes "jit+fused", "jit+cluster", "jit+coop", "jit+col", "jit+tma", "jit (brick sweeps)" or "generic: <why>" into buf: which sweep kernels are in use.  */

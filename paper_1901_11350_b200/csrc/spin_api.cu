@@ -506,7 +506,7 @@ extern "C" int spin_geometry_create(const double bravais[9], int n_basis, const 
     if (!has_device) cudaGetLastError();
     spin_system *s = new spin_system();
     s->has_device = has_device;
-    s->jit = nullptr; s->opt_jit = 1; s->opt_tma = 0; s->opt_ddi_slab = 1; s->opt_col = 0; s->opt_pair = 0; s->opt_cache_noise = 1; s->opt_coop = 1; s->opt_fused = 0; s->d_bar = nullptr;
+    s->jit = nullptr; s->opt_jit = 1; s->opt_tma = 0; s->opt_ddi_slab = 1; s->opt_col = 0; s->opt_pair = 0; s->opt_pdl = -1; s->opt_cache_noise = 1; s->opt_coop = 1; s->opt_fused = 0; s->d_bar = nullptr;
     s->n_img = 1; s->img_sel = 0; s->d_img_sigma = nullptr;
     memcpy(s->brav, bravais, sizeof(s->brav));
     s->nb = n_basis;
@@ -1184,6 +1184,7 @@ extern "C" int spin_set_option(spin_system *s, const char *name, int value) {
     else if (!strcmp(name, "use_fused")) { s->opt_fused = value < 0 ? 0 : (value > 2 ? 2 : value); s->plan_dirty = true; }
     else if (!strcmp(name, "use_coop")) { s->opt_coop = value < 0 ? 0 : (value > 3 ? 3 : value); s->plan_dirty = true; }
     else if (!strcmp(name, "cache_noise")) { s->opt_cache_noise = value ? 1 : 0; s->plan_dirty = true; }
+    else if (!strcmp(name, "use_pdl")) { s->opt_pdl = value > 2 ? -1 : value < 0 ? -1 : value; s->plan_dirty = true; }
     else if (!strcmp(name, "use_pair")) { s->opt_pair = value ? 1 : 0; s->plan_dirty = true; }
     else if (!strcmp(name, "use_col")) { s->opt_col = value ? 1 : 0; s->plan_dirty = true; }
     else if (!strcmp(name, "ddi_slab")) { s->opt_ddi_slab = value ? 1 : 0; s->plan_dirty = true; }

@@ -163,6 +163,18 @@ static void jit_brick(const spin_system *s, int b[3]) {
         if (v[0] > 0 && v[1] > 0 && v[2] > 0 && v[0] * v[1] * v[2] <= 1024 && (v[0] * v[1] * v[2]) % 32 == 0 && (!flat || v[2] == 1)) { b[0] = v[0]; b[1] = v[1]; b[2] = v[2]; }
     }
 }
+static void jit_brick_launch(const spin_system *s, dim3 &grid, dim3 &block);
+// programmatic dependent launch of the brick sweeps: 0 off, 1 dependents released at entry, 2 at the end of each block.
+// Measured (profiles/r1g_README.md): sweeps of many waves gain 1-3 % from 1 and lose with 2.  Sweeps of about one wave lose with 1 (the
+// next sweep's blocks are placed while this one's still hold their SMs, unevenly); with 2 they gain 14 % when the kernels were compiled
+// by NVRTC 12.9 and lose 4 % with NVRTC 12.8 (the one a process that imported torch has loaded), so the automatic choice leaves them alone.
+static int pdl_mode(const spin_system *s) {
+    if (s->opt_pdl >= 0) return s->opt_pdl;
+    dim3 grid, block;
+    jit_brick_launch(s, grid, block);
+    const long blocks = (long)grid.x * grid.y * s->n_img;
+    return blocks <= 6L * sm_count(s) ? 0 : 1;
+}
 static void jit_brick_launch(const spin_system *s, dim3 &grid, dim3 &block) {
     int b[3];
     jit_brick(s, b);
@@ -268,6 +280,8 @@ std::string spin::jit_source(const spin_system *s) {
         const char *e = getenv("SPINLLG_REVERSE");
         o << "constexpr bool REVERSE_CORR = " << ((e && atoi(e) == 0) ? "false" : "true") << ";\n";
     }
+    // programmatic dependent launch: the sweeps release their dependents at once and wait for their prerequisites in the kernel
+    o << "constexpr int PDL = " << pdl_mode(s) << ";      // 0 off, 1 dependents released at entry, 2 at the end of the block\n";
     o << "constexpr bool MULTI_IMAGE = " << (s->n_img > 1 ? "true" : "false") << ";\n";
     o << "constexpr bool DAMPING_ONLY = " << (s->damping_only ? "true" : "false") << ";\n";
     o << "constexpr bool HAS_PIN = " << (s->d_pin ? "true" : "false") << ";\n";
@@ -559,6 +573,21 @@ int spin::jit_prepare(spin_system *s) {
 
 bool spin::jit_ready(const spin_system *s) { return s->jit && s->jit->loaded; }
 
+// a brick sweep, launched with programmatic stream serialisation when the kernels were generated with spec::PDL (they then execute
+// griddepcontrol.wait before their first dependent access): the blocks of the sweep become resident while the previous kernel drains
+static cudaError_t launch_sweep(const spin_system *s, cudaKernel_t k, dim3 grid, dim3 block, void **args) {
+    if (!pdl_mode(s)) return cudaLaunchKernel((const void *)k, grid, block, args, 0, s->stream);
+    cudaLaunchConfig_t cfg;
+    memset(&cfg, 0, sizeof(cfg));
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.stream = s->stream;
+    cudaLaunchAttribute at;
+    memset(&at, 0, sizeof(at));
+    at.id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at.val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = &at; cfg.numAttrs = 1;
+    return cudaLaunchKernelExC(&cfg, (const void *)k, args);
+}
+
 int spin::jit_launch_predictor(spin_system *s, dim3 grid, dim3 block, const double *n, const double *fddi, double *np, double *Aout,
                                unsigned step_add) {
     unsigned seed_lo = s->plan.seed_lo, seed_hi = s->plan.seed_hi;
@@ -569,7 +598,7 @@ int spin::jit_launch_predictor(spin_system *s, dim3 grid, dim3 block, const doub
                     (void *)&pin, (void *)&img_sigma};
     jit_brick_launch(s, grid, block);
     grid.z = (unsigned)s->n_img;
-    SPIN_CUDA(cudaLaunchKernel((const void *)s->jit->k_pred, grid, block, args, 0, s->stream));
+    SPIN_CUDA(launch_sweep(s, s->jit->k_pred, grid, block, args));
     return SPIN_OK;
 }
 
@@ -583,7 +612,7 @@ int spin::jit_launch_corrector(spin_system *s, dim3 grid, dim3 block, const doub
                     (void *)&seed_lo, (void *)&seed_hi, (void *)&pin, (void *)&img_sigma};
     jit_brick_launch(s, grid, block);
     grid.z = (unsigned)s->n_img;
-    SPIN_CUDA(cudaLaunchKernel((const void *)s->jit->k_corr, grid, block, args, 0, s->stream));
+    SPIN_CUDA(launch_sweep(s, s->jit->k_corr, grid, block, args));
     return SPIN_OK;
 }
 

@@ -248,6 +248,18 @@ __device__ __forceinline__ bool is_pinned(const unsigned char *__restrict__ pin,
     else return false;
 }
 
+// Programmatic dependent launch (spec::PDL; the host then launches the sweep with programmatic stream serialisation): let the next
+// kernel of the stream become resident as soon as every block of this one has started, and wait here -- before the first access to
+// anything another kernel writes -- until the previous kernel has completed and its stores are visible.  Semantics of the stream
+// order are unchanged; the launch latency and the block ramp of each sweep overlap the tail of the one before.
+__device__ __forceinline__ void pdl_entry() {
+    if constexpr (spec::PDL == 1) asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    if constexpr (spec::PDL != 0) asm volatile("griddepcontrol.wait;" ::: "memory");
+}
+__device__ __forceinline__ void pdl_exit() {
+    if constexpr (spec::PDL == 2) asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+}
+
 template <int B, bool CG = false>
 __device__ __forceinline__ void predictor_body(const double *__restrict__ n, const double *__restrict__ fddi, double *__restrict__ np,
                                                double *__restrict__ Aout, u64 step, u32 seed_lo, u32 seed_hi, const unsigned char *__restrict__ pin, int brick,
@@ -432,6 +444,7 @@ extern "C" __global__ void SPIN_BOUNDS(spec::BX *spec::BY *spec::BZ)
     jit_predictor(const double *__restrict__ n, const double *__restrict__ fddi, double *__restrict__ np, double *__restrict__ Aout,
                   const unsigned long long *__restrict__ d_step, unsigned int step_add, unsigned int seed_lo, unsigned int seed_hi,
                   const unsigned char *__restrict__ pin, const double *__restrict__ img_sigma) {
+    spinjit::pdl_entry();
     const unsigned long long step = *d_step + step_add;
     // batched images: blockIdx.z selects the image; every per-spin array holds the images one after the other
     const unsigned int image = spec::MULTI_IMAGE ? blockIdx.z : 0u;
@@ -440,6 +453,7 @@ extern "C" __global__ void SPIN_BOUNDS(spec::BX *spec::BY *spec::BZ)
     spinjit::dispatch_basis<0>((int)blockIdx.y, [&](auto b) {
         spinjit::predictor_body<decltype(b)::value>(n + off, fddi + off, np + off, Aout + off, step, seed_lo, seed_hi, pin, (int)blockIdx.x, image, scale);
     });
+    spinjit::pdl_exit();
 }
 
 extern "C" __global__ void SPIN_BOUNDS(spec::BX *spec::BY *spec::BZ)
@@ -447,6 +461,7 @@ extern "C" __global__ void SPIN_BOUNDS(spec::BX *spec::BY *spec::BZ)
                   const double *__restrict__ fddi_np, const double *__restrict__ Ain, double *__restrict__ nout,
                   const unsigned long long *__restrict__ d_step, unsigned int step_add, unsigned int seed_lo, unsigned int seed_hi,
                   const unsigned char *__restrict__ pin, const double *__restrict__ img_sigma) {
+    spinjit::pdl_entry();
     const unsigned long long step = *d_step + step_add;
     const unsigned int image = spec::MULTI_IMAGE ? blockIdx.z : 0u;
     const size_t off = spec::MULTI_IMAGE ? (size_t)image * ((size_t)spec::NBASIS * spec::SUB) : (size_t)0;
@@ -458,6 +473,7 @@ extern "C" __global__ void SPIN_BOUNDS(spec::BX *spec::BY *spec::BZ)
         spinjit::corrector_body<decltype(b)::value>(n + off, np + off, fddi_n + off, fddi_np + off, Ain + off, nout + off, step, seed_lo, seed_hi, pin,
                                                     brick, image, scale);
     });
+    spinjit::pdl_exit();
 }
 
 extern "C" __global__ void SPIN_BOUNDS(spec::BX *spec::BY *spec::BZ)

@@ -145,7 +145,7 @@ struct spin_system {
     bool has_device;               // false only in the planner-only mode used by the CPU tests
     std::string jit_note;          // why the specialised sweeps are not in use, if they are not
     // ---- execution options / bookkeeping
-    int opt_graph, opt_store_A, opt_jit, opt_tma, opt_ddi_slab, opt_col, opt_pair, opt_cache_noise, opt_coop, opt_fused;
+    int opt_graph, opt_store_A, opt_jit, opt_tma, opt_ddi_slab, opt_col, opt_pair, opt_pdl, opt_cache_noise, opt_coop, opt_fused;
     cudaGraphExec_t graph_exec[2];   // one captured graph per ping-pong parity
     int graph_steps;
     int64_t n_launch, n_fft;

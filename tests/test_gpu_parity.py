@@ -379,6 +379,28 @@ def test_column_marching_with_open_and_mixed_boundaries(P, O):
 
 
 # ---------------------------------------------------------------------------------------------------------------------
+# Programmatic dependent launch of the brick sweeps (option use_pdl): only the launch overlap changes, never a result bit
+@pytest.mark.parametrize("cfg,cells,steps", [(1, (34, 9, 1), 100), (2, (70, 33, 1), 100), (3, (36, 19, 7), 60), (4, (34, 17, 1), 100),
+                                             (5, (20, 12, 4), 20)])
+def test_programmatic_dependent_launch_is_bit_identical(P, O, cfg, cells, steps):
+    w = W.CONFIGS[cfg]().resized(cells, steps)
+    out = []
+    for mode in (0, 1, 2, -1):
+        g = P.SpinSystem.from_workload(w)
+        g.spin_set_option("use_pdl", mode)
+        g.spin_set_option("use_coop", 0)
+        assert g.spin_kernel_info().startswith("jit (brick"), g.spin_kernel_info()
+        g.llg_iterate(steps // 2); g.llg_iterate(steps - steps // 2)      # graph replays and the eager remainder
+        out.append(g.spins_get())
+        g.close()
+    for k in (1, 2, 3):
+        assert np.array_equal(out[0], out[k]), k
+    o = O.OracleSystem.from_workload(w)
+    o.iterate(steps)
+    assert np.abs(out[0] - o.spins()).max() <= SPIN_ATOL
+
+
+# ---------------------------------------------------------------------------------------------------------------------
 # Two sites per thread with 128-bit accesses (csrc/spin_jit_pair.cuh), option use_pair=1: same arithmetic, bit-identical
 @pytest.mark.parametrize("cfg,cells,steps,geo", [(1, (34, 9, 1), 100, None), (2, (70, 33, 1), 100, None), (3, (36, 9, 7), 60, None),
                                                  (3, (70, 37, 11), 20, "64,2,2"), (3, (2, 5, 3), 50, None), (4, (34, 17, 1), 100, None),
