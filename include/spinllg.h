@@ -209,8 +209,12 @@ int spin_set_option(spin_system *sys, const char *name, int value);
  * 2 at the end of each block, 0 switches it off (the automatic choice for lattices of about one wave).  The order of all memory accesses, and with it every result bit, is unchanged.
  * cache_noise (default 1): the predictor keeps the thermal field of the step (24 B/spin) for the corrector instead of generating it twice.
  * ddi_slab (default 1): thin films with one basis atom take the dipolar slab path (2-D cuFFT + fused transform along c).
- * spin_kernel_info writes "jit+fused", "jit+cluster", "jit+coop", "jit+col", "jit+tma", "jit (brick sweeps)" or "generic: <why>" into buf: which sweep kernels are in use.  */
+ * spin_kernel_info writes "jit+fused", "jit+cluster", "jit+coop", "jit+pair", "jit+col", "jit+tma", "jit (brick sweeps)" or "generic: <why>" into buf: which sweep kernels are in use.  */
 int spin_kernel_info(spin_system *sys, char *buf, int len);
+/* The run-time compiler of the specialised sweeps, e.g. "12.9 (/usr/local/cuda/lib64/libnvrtc.so.12)".  NVRTC is bound at run time by
+ * path -- $SPINLLG_NVRTC, then the toolkit the library was built with, then the loader's libnvrtc.so.12 -- so that a different NVRTC
+ * already loaded into the process (torch ships 12.8) does not change the generated kernels.  No device needed.  */
+int spin_jit_compiler_info(char *buf, int len);
 /* the generated translation unit of the specialised sweeps (buf may be NULL); compile != 0 also compiles it for sm_100a
  * (needs no device) and returns the cubin size.  Host-side planner check; works in planner-only mode
  * (environment SPINLLG_PLANNER_ONLY=1 lets spin_geometry_create succeed without a device; every computing call then

@@ -5,6 +5,6 @@
 
 The package never imports `oracle` (the CPU checker) and has no CPU fallback.
 """
-from .binding import EXPORTS, SpinError, SpinSystem, lib, version
+from .binding import EXPORTS, SpinError, SpinSystem, lib, spin_jit_compiler_info, version
 
-__all__ = ["SpinSystem", "SpinError", "lib", "version", "EXPORTS"]
+__all__ = ["SpinSystem", "SpinError", "lib", "version", "spin_jit_compiler_info", "EXPORTS"]

@@ -37,7 +37,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     cuda_lib = os.path.join(os.path.dirname(os.path.dirname(nvcc_path())), "lib64")
     cmd = [nvcc_path(), "-std=c++17", "-O3", "-lineinfo", *ARCH, "-Xcompiler", "-fPIC", "-shared",
            "-o", LIB, *[os.path.join(CSRC, f) for f in SOURCES],
-           "-lcufft", "-lnvrtc", "-ldl", "-Xlinker", "-rpath", "-Xlinker", cuda_lib]
+           "-DSPIN_NVRTC_PATH=\"%s\"" % os.path.join(cuda_lib, "libnvrtc.so.12"), "-lcufft", "-ldl", "-Xlinker", "-rpath", "-Xlinker", cuda_lib]
     if verbose:
         cmd.insert(1, "-Xptxas")
         cmd.insert(2, "-v")

@@ -1207,6 +1207,11 @@ extern "C" int spin_kernel_info(spin_system *s, char *buf, int len) {
     else snprintf(buf, (size_t)len, "generic: %s", s->jit_note.c_str());
     return SPIN_OK;
 }
+extern "C" int spin_jit_compiler_info(char *buf, int len) {
+    REQUIRE(buf && len > 0, "bad argument");
+    snprintf(buf, (size_t)len, "%s", jit_compiler_info().c_str());
+    return SPIN_OK;
+}
 // the generated translation unit of the specialised sweeps; with compile != 0 it is also compiled with NVRTC (no device
 // needed) and the size of the cubin is returned in *cubin_bytes
 extern "C" int spin_jit_source(spin_system *s, char *buf, int len, int compile, int64_t *cubin_bytes) {

@@ -10,10 +10,12 @@
 #include <nvrtc.h>
 #include <stdlib.h>
 #include <stdio.h>
+#include <stddef.h>
 #include <string.h>
 
 #include <algorithm>
 #include <map>
+#include <vector>
 #include <mutex>
 #include <sstream>
 #include <string>
@@ -166,14 +168,16 @@ static void jit_brick(const spin_system *s, int b[3]) {
 static void jit_brick_launch(const spin_system *s, dim3 &grid, dim3 &block);
 // programmatic dependent launch of the brick sweeps: 0 off, 1 dependents released at entry, 2 at the end of each block.
 // Measured (profiles/r1g_README.md): sweeps of many waves gain 1-3 % from 1 and lose with 2.  Sweeps of about one wave lose with 1 (the
-// next sweep's blocks are placed while this one's still hold their SMs, unevenly); with 2 they gain 14 % when the kernels were compiled
-// by NVRTC 12.9 and lose 4 % with NVRTC 12.8 (the one a process that imported torch has loaded), so the automatic choice leaves them alone.
+// next sweep's blocks are placed while this one's still hold their SMs, unevenly); with 2 they gain 10-14 % when the kernels were
+// compiled by NVRTC 12.9 and lose 4 % with NVRTC 12.8, so the automatic choice depends on the compiler that was found.
+static bool nvrtc_at_least(int major, int minor);
 static int pdl_mode(const spin_system *s) {
     if (s->opt_pdl >= 0) return s->opt_pdl;
     dim3 grid, block;
     jit_brick_launch(s, grid, block);
     const long blocks = (long)grid.x * grid.y * s->n_img;
-    return blocks <= 6L * sm_count(s) ? 0 : 1;
+    if (blocks > 6L * sm_count(s)) return 1;
+    return nvrtc_at_least(12, 9) ? 2 : 0;
 }
 static void jit_brick_launch(const spin_system *s, dim3 &grid, dim3 &block) {
     int b[3];
@@ -389,31 +393,101 @@ std::mutex g_cache_mutex;
 std::map<std::string, std::string> g_cubin_cache;
 }
 
+// NVRTC is bound at run time, by PATH: a process that imported torch has torch's own libnvrtc.so.12 (12.8) loaded under the same
+// soname, and a link-time dependency would silently resolve to it.  The toolkit's 12.9 (the one nvcc built this library with) keeps the
+// corrector at 40 registers where 12.8 needs 48 (6 instead of 5 blocks per SM, 4 % of the cfg3 step).  Order: $SPINLLG_NVRTC, the
+// toolkit the library was built with (SPIN_NVRTC_PATH, set by build.py), then whatever the loader finds under the soname.
+namespace {
+struct Nvrtc {
+    decltype(&nvrtcCreateProgram) CreateProgram;
+    decltype(&nvrtcCompileProgram) CompileProgram;
+    decltype(&nvrtcGetProgramLogSize) GetProgramLogSize;
+    decltype(&nvrtcGetProgramLog) GetProgramLog;
+    decltype(&nvrtcGetCUBINSize) GetCUBINSize;
+    decltype(&nvrtcGetCUBIN) GetCUBIN;
+    decltype(&nvrtcDestroyProgram) DestroyProgram;
+    decltype(&nvrtcGetErrorString) GetErrorString;
+    decltype(&nvrtcVersion) Version;
+    std::string path;
+    bool ok;
+};
+const Nvrtc &nvrtc() {
+    static const Nvrtc api = [] {
+        Nvrtc a;
+        memset((void *)&a, 0, offsetof(Nvrtc, path));
+        a.ok = false;
+        std::vector<std::string> cands;
+        if (const char *e = getenv("SPINLLG_NVRTC")) cands.push_back(e);
+#ifdef SPIN_NVRTC_PATH
+        cands.push_back(SPIN_NVRTC_PATH);
+#endif
+        cands.push_back("libnvrtc.so.12");
+        cands.push_back("libnvrtc.so");
+        for (const std::string &c : cands) {
+            void *h = dlopen(c.c_str(), RTLD_NOW | RTLD_LOCAL);
+            if (!h) continue;
+#define SPIN_NVRTC_SYM(f) a.f = (decltype(a.f))dlsym(h, "nvrtc" #f)
+            SPIN_NVRTC_SYM(CreateProgram); SPIN_NVRTC_SYM(CompileProgram); SPIN_NVRTC_SYM(GetProgramLogSize); SPIN_NVRTC_SYM(GetProgramLog);
+            SPIN_NVRTC_SYM(GetCUBINSize); SPIN_NVRTC_SYM(GetCUBIN); SPIN_NVRTC_SYM(DestroyProgram); SPIN_NVRTC_SYM(GetErrorString);
+            SPIN_NVRTC_SYM(Version);
+#undef SPIN_NVRTC_SYM
+            if (a.CreateProgram && a.CompileProgram && a.GetProgramLogSize && a.GetProgramLog && a.GetCUBINSize && a.GetCUBIN &&
+                a.DestroyProgram && a.GetErrorString && a.Version) {
+                a.path = c;
+                a.ok = true;
+                break;
+            }
+            dlclose(h);
+        }
+        return a;
+    }();
+    return api;
+}
+}  // namespace
+
+static bool nvrtc_at_least(int major, int minor) {
+    const Nvrtc &rt = nvrtc();
+    int ma = 0, mi = 0;
+    if (!rt.ok || rt.Version(&ma, &mi) != NVRTC_SUCCESS) return false;
+    return ma > major || (ma == major && mi >= minor);
+}
+
+// "12.9 (/usr/local/cuda/lib64/libnvrtc.so.12)" or why there is none
+std::string spin::jit_compiler_info() {
+    const Nvrtc &rt = nvrtc();
+    if (!rt.ok) return "NVRTC not found";
+    int major = 0, minor = 0;
+    rt.Version(&major, &minor);
+    return std::to_string(major) + "." + std::to_string(minor) + " (" + rt.path + ")";
+}
+
 int spin::jit_compile(const std::string &source, std::string &cubin, std::string &log) {
+    const Nvrtc &rt = nvrtc();
+    if (!rt.ok) return spin::fail(SPIN_ERR_CUDA, "NVRTC (libnvrtc.so.12) could not be loaded");
     {
         std::lock_guard<std::mutex> lock(g_cache_mutex);
         auto it = g_cubin_cache.find(source);
         if (it != g_cubin_cache.end() && !getenv("SPINLLG_JIT_DUMP")) { cubin = it->second; log.clear(); return SPIN_OK; }
     }
     nvrtcProgram prog;
-    if (nvrtcCreateProgram(&prog, source.c_str(), "spin_jit_spec.cu", 0, nullptr, nullptr) != NVRTC_SUCCESS)
+    if (rt.CreateProgram(&prog, source.c_str(), "spin_jit_spec.cu", 0, nullptr, nullptr) != NVRTC_SUCCESS)
         return spin::fail(SPIN_ERR_CUDA, "nvrtcCreateProgram failed");
     const std::string inc = "-I" + csrc_dir();
     const char *opts[] = {"--gpu-architecture=sm_100a", "--std=c++17", "-lineinfo", "-default-device", inc.c_str()};
-    const nvrtcResult r = nvrtcCompileProgram(prog, 5, opts);
+    const nvrtcResult r = rt.CompileProgram(prog, 5, opts);
     size_t n = 0;
-    nvrtcGetProgramLogSize(prog, &n);
+    rt.GetProgramLogSize(prog, &n);
     log.assign(n, '\0');
-    if (n) nvrtcGetProgramLog(prog, &log[0]);
+    if (n) rt.GetProgramLog(prog, &log[0]);
     if (r != NVRTC_SUCCESS) {
-        nvrtcDestroyProgram(&prog);
-        return spin::fail(SPIN_ERR_CUDA, "NVRTC compilation failed: %s | %.300s", nvrtcGetErrorString(r), log.c_str());
+        rt.DestroyProgram(&prog);
+        return spin::fail(SPIN_ERR_CUDA, "NVRTC compilation failed: %s | %.300s", rt.GetErrorString(r), log.c_str());
     }
     size_t nc = 0;
-    nvrtcGetCUBINSize(prog, &nc);
+    rt.GetCUBINSize(prog, &nc);
     cubin.assign(nc, '\0');
-    nvrtcGetCUBIN(prog, &cubin[0]);
-    nvrtcDestroyProgram(&prog);
+    rt.GetCUBIN(prog, &cubin[0]);
+    rt.DestroyProgram(&prog);
     {
         std::lock_guard<std::mutex> lock(g_cache_mutex);
         if (g_cubin_cache.size() >= 64) g_cubin_cache.clear();

@@ -174,6 +174,7 @@ void ddi_release(spin_system *s);
 // spin_jit.cu
 std::string jit_source(const spin_system *s);
 int jit_compile(const std::string &source, std::string &cubin, std::string &log);
+std::string jit_compiler_info();      // version and path of the NVRTC in use
 int jit_prepare(spin_system *s);
 void jit_release(spin_system *s);
 bool jit_ready(const spin_system *s);

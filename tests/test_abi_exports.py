@@ -122,3 +122,14 @@ int main(void) {{
     env = dict(os.environ, SPINLLG_PLANNER_ONLY="1")
     r = subprocess.run([str(exe)], env=env, capture_output=True, text=True)
     assert r.returncode == 0, (r.returncode, r.stdout, r.stderr)
+
+
+def test_jit_compiler_is_bound_by_path_even_with_torch_loaded():
+    # torch preloads its own libnvrtc.so.12 (another version, same soname); the library must still find the toolkit's by path
+    import torch  # noqa: F401
+    import paper_1901_11350_b200 as P
+    info = P.spin_jit_compiler_info()
+    assert info.split(".")[0].isdigit(), info
+    toolkit = "/usr/local/cuda/lib64/libnvrtc.so.12"
+    if os.path.exists(toolkit) and not os.environ.get("SPINLLG_NVRTC"):
+        assert toolkit in info, info
