@@ -62,15 +62,16 @@ class ClockSampler:
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
          "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
 
-    def __init__(self, index=0):
+    def __init__(self, index=0, period_ms=200):
         self.index = index
+        self.period_ms = int(period_ms)
         self.rows = []
         self.proc = None
 
     def start(self):
         try:
             self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
-                                          "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+                                          "-lms", str(self.period_ms)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.t = threading.Thread(target=self._read, daemon=True)
             self.t.start()
         except Exception:
@@ -149,6 +150,7 @@ def main():
     ap.add_argument("--inner", type=int, default=128, help="LLG iterations per bench step (a multiple of the 16-step CUDA graph)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--store-A", type=int, default=0)
+    ap.add_argument("--clock-period-ms", type=int, default=200, help="nvidia-smi sampling period during the timed region (the recipe's 200 ms)")
     ap.add_argument("--option", action="append", default=[], metavar="NAME=VALUE", help="spin_set_option pass-through (e.g. use_pdl=0) for A/B runs")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
@@ -193,7 +195,7 @@ def main():
         for _ in range(args.warmup):
             sys_.llg_iterate(inner)
     barrier()
-    sampler = ClockSampler(local)
+    sampler = ClockSampler(local, args.clock_period_ms)
     if rank == 0:
         sampler.start()
         time.sleep(0.3)
