@@ -11,6 +11,8 @@
 // One padded array per sublattice and one spectrum product per sublattice pair (:87).
 #include <math.h>
 #include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
 
 #include "spinllg_internal.h"
 
@@ -42,6 +44,7 @@ struct DdiState {
     double *s_in, *s_out;
     cufftDoubleComplex *s_a, *s_b, *s_d;
     double *d_Kre;             // [6][PZ][S2] real: the tensor spectrum is real for a single basis atom (the kernel is even)
+    bool mirror;               // K(kz) = +-K(PZ - kz) (c perpendicular to the film): the contraction reads PZ/2 + 1 of the PZ planes
 };
 
 namespace {
@@ -188,7 +191,7 @@ __constant__ double DDI_WR[16], DDI_WI[16];
 // registers and spills its accumulators; the kernel is bound by its 200 MB of traffic, not by the sums.)
 // M2 / H2: element (kb, slab = c NZ + z, ka) at (kb SL + slab) S1p + ka, S1p the row pitch (H2 may be M2: every thread reads its column, then writes it);
 // Kre: [6][PZ][S2] with q = kb S1 + ka.
-template <int NZ, int PZ>
+template <int NZ, int PZ, bool MIRROR>
 __global__ void __launch_bounds__(128) ddi_slab_contract_kernel(const double *__restrict__ Kre, const cufftDoubleComplex *__restrict__ M2,
                                                                  cufftDoubleComplex *H2, long long S2, int S1, int S1p) {
     const long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -203,8 +206,8 @@ __global__ void __launch_bounds__(128) ddi_slab_contract_kernel(const double *__
             const cufftDoubleComplex v = M2[col + (size_t)(c * NZ + z) * S1p];
             mr[c][z] = v.x; mi[c][z] = v.y; hr[c][z] = 0.0; hi[c][z] = 0.0;
         }
-#pragma unroll
-    for (int kz = 0; kz < PZ; ++kz) {
+    // one wave number along c: forward sum, contraction with the six tensor components, inverse sum into hr / hi
+    auto one_kz = [&](const int kz, const double kxx, const double kxy, const double kxz, const double kyy, const double kyz, const double kzz) {
         double Mr[3], Mi[3];
 #pragma unroll
         for (int c = 0; c < 3; ++c) {
@@ -217,8 +220,6 @@ __global__ void __launch_bounds__(128) ddi_slab_contract_kernel(const double *__
             }
             Mr[c] = ar; Mi[c] = ai;
         }
-        const size_t o = (size_t)kz * S2 + q, st = (size_t)PZ * S2;
-        const double kxx = Kre[o], kxy = Kre[st + o], kxz = Kre[2 * st + o], kyy = Kre[3 * st + o], kyz = Kre[4 * st + o], kzz = Kre[5 * st + o];
         const double Hr[3] = {kxx * Mr[0] + kxy * Mr[1] + kxz * Mr[2], kxy * Mr[0] + kyy * Mr[1] + kyz * Mr[2], kxz * Mr[0] + kyz * Mr[1] + kzz * Mr[2]};
         const double Hi[3] = {kxx * Mi[0] + kxy * Mi[1] + kxz * Mi[2], kxy * Mi[0] + kyy * Mi[1] + kyz * Mi[2], kxz * Mi[0] + kyz * Mi[1] + kzz * Mi[2]};
 #pragma unroll
@@ -229,11 +230,45 @@ __global__ void __launch_bounds__(128) ddi_slab_contract_kernel(const double *__
                 hr[c][z] = fma(Hr[c], wr, fma(-Hi[c], wi, hr[c][z]));
                 hi[c][z] = fma(Hr[c], wi, fma(Hi[c], wr, hi[c][z]));
             }
+    };
+    const size_t st = (size_t)PZ * S2;
+#pragma unroll
+    for (int kz = 0; kz < (MIRROR ? PZ / 2 + 1 : PZ); ++kz) {
+        const size_t o = (size_t)kz * S2 + q;
+        const double kxx = Kre[o], kxy = Kre[st + o], kxz = Kre[2 * st + o], kyy = Kre[3 * st + o], kyz = Kre[4 * st + o], kzz = Kre[5 * st + o];
+        one_kz(kz, kxx, kxy, kxz, kyy, kyz, kzz);
+        // mirrored tensor (ddi_mirror_check_kernel): the plane PZ - kz holds the same values, xz and yz with the opposite sign
+        if constexpr (MIRROR) { if (kz > 0 && 2 * kz < PZ) one_kz(PZ - kz, kxx, kxy, -kxz, kyy, -kyz, kzz); }
     }
 #pragma unroll
     for (int c = 0; c < 3; ++c)
 #pragma unroll
         for (int z = 0; z < NZ; ++z) H2[col + (size_t)(c * NZ + z) * S1p] = make_cuDoubleComplex(hr[c][z], hi[c][z]);
+}
+
+// Is the tensor spectrum mirror symmetric along c, K_ab(kz) = s_ab K_ab(PZ - kz) with s = -1 for xz, yz and +1 otherwise?  (True when c is
+// perpendicular to a and b.)  out[0] = max |K(kz) - s K(PZ - kz)|, out[1] = max |K| as the bit patterns of non-negative doubles,
+// which order like unsigned integers.
+__global__ void ddi_mirror_check_kernel(const double *__restrict__ Kre, int PZ, long long S2, unsigned long long *out) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    double dev = 0.0, mag = 0.0;
+    if (i < 6LL * PZ * S2) {
+        const int comp = (int)(i / ((long long)PZ * S2));
+        const long long r = i - (long long)comp * PZ * S2;
+        const int kz = (int)(r / S2);
+        const long long q = r - (long long)kz * S2;
+        const double sgn = (comp == 2 || comp == 4) ? -1.0 : 1.0;
+        const double a = Kre[i], b = Kre[((long long)comp * PZ + (PZ - kz) % PZ) * S2 + q];
+        dev = fabs(a - sgn * b); mag = fabs(a);
+    }
+    for (int o = 16; o > 0; o >>= 1) {
+        dev = fmax(dev, __shfl_xor_sync(0xffffffffu, dev, o));
+        mag = fmax(mag, __shfl_xor_sync(0xffffffffu, mag, o));
+    }
+    if ((threadIdx.x & 31) == 0) {
+        atomicMax(out, (unsigned long long)__double_as_longlong(dev));
+        atomicMax(out + 1, (unsigned long long)__double_as_longlong(mag));
+    }
 }
 
 #define SPIN_FFT(call)                                                                                         \
@@ -347,6 +382,19 @@ int spin::ddi_prepare(spin_system *s) {
         SPIN_CUDA(cudaMalloc(&d->d_Kre, (size_t)nk * sizeof(double)));
         real_part_kernel<<<(unsigned)((nk + 255) / 256), 256, 0, s->stream>>>(d->d_Khat, d->d_Kre, nk);
         s->n_launch++;
+        // mirror symmetry along c, checked on the numbers themselves (relative 1e-13; rounding of the transform leaves about 1e-16)
+        unsigned long long *d_chk = nullptr, h_chk[2] = {0ull, 0ull};
+        SPIN_CUDA(cudaMalloc(&d_chk, 2 * sizeof(unsigned long long)));
+        SPIN_CUDA(cudaMemsetAsync(d_chk, 0, 2 * sizeof(unsigned long long), s->stream));
+        ddi_mirror_check_kernel<<<(unsigned)((nk + 255) / 256), 256, 0, s->stream>>>(d->d_Kre, d->PZ, (long long)d->S2, d_chk);
+        s->n_launch++;
+        SPIN_CUDA(cudaMemcpyAsync(h_chk, d_chk, sizeof(h_chk), cudaMemcpyDeviceToHost, s->stream));
+        SPIN_CUDA(cudaStreamSynchronize(s->stream));
+        cudaFree(d_chk);
+        double dev, mag;
+        memcpy(&dev, &h_chk[0], 8); memcpy(&mag, &h_chk[1], 8);
+        const char *e = getenv("SPINLLG_DDI_MIRROR");
+        d->mirror = d->PZ > 2 && dev <= 1e-13 * mag && !(e && atoi(e) == 0);
     }
     SPIN_CUDA(cudaStreamSynchronize(s->stream));
     SPIN_CUDA(cudaGetLastError());
@@ -367,13 +415,15 @@ int spin::ddi_field(spin_system *s, const double *d_n, double *d_f) {
         SPIN_FFT(cufftExecD2Z(d->plan_a_fwd, d->s_in, d->s_a));                       // a-pass over the occupied rows only
         SPIN_FFT(cufftExecZ2Z(d->plan_b, d->s_a, d->s_b, CUFFT_FORWARD));            // b-pass
         const unsigned gq = (unsigned)((d->S2 + 127) / 128);
+#define SPIN_CONTRACT(NZ_, PZ_, MIR_) ddi_slab_contract_kernel<NZ_, PZ_, MIR_><<<gq, 128, 0, s->stream>>>(d->d_Kre, d->s_b, d->s_b, (long long)d->S2, d->S1, d->S1p)
         switch (d->PZ) {                                                              // c-pass + contraction + inverse c-pass, in place
-            case 1: ddi_slab_contract_kernel<1, 1><<<gq, 128, 0, s->stream>>>(d->d_Kre, d->s_b, d->s_b, (long long)d->S2, d->S1, d->S1p); break;
-            case 2: ddi_slab_contract_kernel<1, 2><<<gq, 128, 0, s->stream>>>(d->d_Kre, d->s_b, d->s_b, (long long)d->S2, d->S1, d->S1p); break;
-            case 4: ddi_slab_contract_kernel<2, 4><<<gq, 128, 0, s->stream>>>(d->d_Kre, d->s_b, d->s_b, (long long)d->S2, d->S1, d->S1p); break;
-            case 8: ddi_slab_contract_kernel<4, 8><<<gq, 128, 0, s->stream>>>(d->d_Kre, d->s_b, d->s_b, (long long)d->S2, d->S1, d->S1p); break;
-            default: ddi_slab_contract_kernel<8, 16><<<gq, 128, 0, s->stream>>>(d->d_Kre, d->s_b, d->s_b, (long long)d->S2, d->S1, d->S1p); break;
+            case 1: SPIN_CONTRACT(1, 1, false); break;
+            case 2: SPIN_CONTRACT(1, 2, false); break;
+            case 4: if (d->mirror) SPIN_CONTRACT(2, 4, true); else SPIN_CONTRACT(2, 4, false); break;
+            case 8: if (d->mirror) SPIN_CONTRACT(4, 8, true); else SPIN_CONTRACT(4, 8, false); break;
+            default: if (d->mirror) SPIN_CONTRACT(8, 16, true); else SPIN_CONTRACT(8, 16, false); break;
         }
+#undef SPIN_CONTRACT
         SPIN_FFT(cufftExecZ2Z(d->plan_b, d->s_b, d->s_d, CUFFT_INVERSE));            // inverse b-pass
         SPIN_FFT(cufftExecZ2D(d->plan_a_inv, d->s_d, d->s_out));                      // inverse a-pass, occupied rows only
         ddi_slab_gather_kernel<<<gcell, nt, 0, s->stream>>>(s->plan, d->s_out, d->P[0], d->SL, s->mu[0] * C_DD / (double)d->Ptot, d_f);

@@ -343,6 +343,29 @@ def test_ddi_slab_path_matches_oracle_and_3d_path(P, O, cells, per, img):
     assert np.abs(g.spins_get() - o.spins()).max() <= SPIN_ATOL
 
 
+# The slab contraction reads only PZ/2 + 1 of the PZ tensor planes when the spectrum is mirror symmetric along c (c perpendicular to the
+# film; checked numerically when the plan is built).  Tilted c: no symmetry, all planes are read; oblique a, b with c perpendicular: symmetric.
+@pytest.mark.parametrize("bravais", [[[1, 0, 0], [0, 1, 0], [0.3, 0.2, 1.0]], [[1, 0, 0], [0.5, 0.9, 0], [0, 0, 1.1]], [[1, 0, 0], [0, 1, 0], [0, 0, 1]]])
+@pytest.mark.parametrize("cells", [(14, 10, 4), (12, 10, 8), (10, 6, 2)])
+def test_ddi_slab_mirror_symmetry_of_the_tensor(P, O, bravais, cells, monkeypatch):
+    w = dataclasses.replace(W.config5().resized(cells, 10), bravais=np.array(bravais, float), periodic=(1, 1, 0), ddi_images=(2, 2, 0))
+    g, o = pair(P, O, w)
+    Bo = o.effective_field()
+    Bg = g.effective_field()
+    assert_fields_close(Bg, Bo)
+    w0 = dataclasses.replace(w, pair_J=w.pair_J * 0, pair_D=w.pair_D * 0, B=0.0, aniso=[])
+    g0, o0 = pair(P, O, w0)
+    Fd = o0.ddi_field(direct=True) / (w.mu_s[0] * O.MU_B)
+    assert np.abs(g0.effective_field() - Fd).max() <= 1e-11 * np.abs(Fd).max()
+    monkeypatch.setenv("SPINLLG_DDI_MIRROR", "0")      # all planes read, whatever the symmetry
+    h = P.SpinSystem.from_workload(w)
+    Bh = h.effective_field()
+    assert_fields_close(Bh, Bo)
+    assert np.abs(Bh - Bg).max() <= 1e-13 * np.abs(Bo).max()
+    g.llg_iterate(10); o.iterate(10)
+    assert np.abs(g.spins_get() - o.spins()).max() <= SPIN_ATOL
+
+
 # ---------------------------------------------------------------------------------------------------------------------
 # Column-marching sweeps (csrc/spin_jit_col.cuh), option use_col=1 (measured slower than the bricks): same arithmetic
 @pytest.mark.parametrize("cfg,cells,steps,geo", [(3, (35, 9, 7), 100, None), (3, (70, 37, 45), 20, "32,8,16"), (3, (33, 5, 40), 20, "64,2,7"),
