@@ -433,9 +433,20 @@ const Nvrtc &nvrtc() {
 #undef SPIN_NVRTC_SYM
             if (a.CreateProgram && a.CompileProgram && a.GetProgramLogSize && a.GetProgramLog && a.GetCUBINSize && a.GetCUBIN &&
                 a.DestroyProgram && a.GetErrorString && a.Version) {
-                a.path = c;
-                a.ok = true;
-                break;
+                // a trial compilation: an NVRTC that cannot find its builtins library loads fine and fails only here
+                nvrtcProgram prog;
+                bool works = false;
+                if (a.CreateProgram(&prog, "extern \"C\" __global__ void spin_probe(double *x) { x[0] = 1.0; }\n", "spin_probe.cu", 0, nullptr,
+                                    nullptr) == NVRTC_SUCCESS) {
+                    const char *opts[] = {"--gpu-architecture=sm_100a"};
+                    works = a.CompileProgram(prog, 1, opts) == NVRTC_SUCCESS;
+                    a.DestroyProgram(&prog);
+                }
+                if (works) {
+                    a.path = c;
+                    a.ok = true;
+                    break;
+                }
             }
             dlclose(h);
         }
