@@ -192,14 +192,16 @@ def main():
     inner = args.inner
 
     # ---------------- device-resident timing
-    with torch.cuda.stream(stream):
-        for _ in range(args.warmup):
-            sys_.llg_iterate(inner)
-    barrier()
+    # the clock sampler starts before the warm-up and the timed steps follow the warm-up without an idle gap: after idling the board
+    # runs the first 40 ms about 8 % faster than in its steady state, and a pause here would time mostly that
     sampler = ClockSampler(local, args.clock_period_ms)
     if rank == 0:
         sampler.start()
         time.sleep(0.3)
+    with torch.cuda.stream(stream):
+        for _ in range(args.warmup):
+            sys_.llg_iterate(inner)
+    barrier()
     l0, f0 = sys_.spin_launch_counts()
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
