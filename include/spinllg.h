@@ -211,6 +211,10 @@ int spin_set_option(spin_system *sys, const char *name, int value);
  * ddi_slab (default 1): thin films with one basis atom take the dipolar slab path (2-D cuFFT + fused transform along c).
  * spin_kernel_info writes "jit+fused", "jit+cluster", "jit+coop", "jit+pair", "jit+col", "jit+tma", "jit (brick sweeps)" or "generic: <why>" into buf: which sweep kernels are in use.  */
 int spin_kernel_info(spin_system *sys, char *buf, int len);
+/* Which dipolar path the plan chose: "off", "3d" (general zero-padded 3-D transform), "slab" (thin film of one basis atom: transforms in
+ * the a-b plane by cuFFT, hand-written transform along c fused with the contraction) or "slab+mirror" (the same, reading PZ/2 + 1 of the
+ * PZ tensor planes because the spectrum was found mirror symmetric along c).  */
+int spin_ddi_info(spin_system *sys, char *buf, int len);
 /* The run-time compiler of the specialised sweeps, e.g. "12.9 (/usr/local/cuda/lib64/libnvrtc.so.12)".  NVRTC is bound at run time by
  * path -- $SPINLLG_NVRTC, then the toolkit the library was built with, then the loader's libnvrtc.so.12 -- so that a different NVRTC
  * already loaded into the process (torch ships 12.8) does not change the generated kernels.  No device needed.  */

@@ -23,7 +23,7 @@ EXPORTS = [
     "llg_configure", "llg_set_solver", "llg_set_damping_only", "minimise_vp", "minimise_vp_reset", "llg_iterate", "llg_get_step", "llg_set_step", "spin_synchronize",
     "effective_field", "effective_field_device", "energy", "observables", "topological_charge",
     "spin_launch_counts", "spin_measure_fp64_tflops", "spin_profile_enable", "spin_profile_get", "spin_set_option",
-    "spin_kernel_info", "spin_jit_compiler_info", "spin_jit_source", "spin_last_error", "spin_version",
+    "spin_kernel_info", "spin_ddi_info", "spin_jit_compiler_info", "spin_jit_source", "spin_last_error", "spin_version",
 ]
 
 
@@ -88,6 +88,7 @@ def lib() -> C.CDLL:
         "spin_set_option": (C.c_int, [vp, C.c_char_p, C.c_int]),
         "spin_kernel_info": (C.c_int, [vp, C.c_char_p, C.c_int]),
         "spin_jit_compiler_info": (C.c_int, [C.c_char_p, C.c_int]),
+        "spin_ddi_info": (C.c_int, [vp, C.c_char_p, C.c_int]),
         "spin_jit_source": (C.c_int, [vp, C.c_char_p, C.c_int, C.c_int, i64p]),
         "spin_last_error": (C.c_char_p, []),
         "spin_version": (C.c_char_p, []),
@@ -341,6 +342,11 @@ class SpinSystem:
     def spin_kernel_info(self):
         buf = C.create_string_buffer(1024)
         _check(lib().spin_kernel_info(self._h, buf, 1024))
+        return buf.value.decode()
+
+    def spin_ddi_info(self):
+        buf = C.create_string_buffer(64)
+        _check(lib().spin_ddi_info(self._h, buf, 64))
         return buf.value.decode()
 
     def spin_jit_source(self, compile=False):

@@ -1207,6 +1207,12 @@ extern "C" int spin_kernel_info(spin_system *s, char *buf, int len) {
     else snprintf(buf, (size_t)len, "generic: %s", s->jit_note.c_str());
     return SPIN_OK;
 }
+extern "C" int spin_ddi_info(spin_system *s, char *buf, int len) {
+    REQUIRE(s && buf && len > 0, "bad argument");
+    if (s->has_device) { int rc = ensure_plan(s); if (rc) return rc; }
+    snprintf(buf, (size_t)len, "%s", ddi_path_name(s));
+    return SPIN_OK;
+}
 extern "C" int spin_jit_compiler_info(char *buf, int len) {
     REQUIRE(buf && len > 0, "bad argument");
     snprintf(buf, (size_t)len, "%s", jit_compiler_info().c_str());

@@ -280,6 +280,13 @@ __global__ void ddi_mirror_check_kernel(const double *__restrict__ Kre, int PZ, 
 
 }  // namespace
 
+const char *spin::ddi_path_name(const spin_system *s) {
+    const DdiState *d = s->ddi;
+    if (!s->ddi_on || !d) return "off";
+    if (!d->slab) return "3d";
+    return d->mirror ? "slab+mirror" : "slab";
+}
+
 void spin::ddi_release(spin_system *s) {
     DdiState *d = s->ddi;
     if (!d) return;

@@ -170,6 +170,7 @@ int fail(int code, const char *fmt, ...);
 int ddi_prepare(spin_system *s);                                   // (re)build tensor spectra and FFT plans
 int ddi_field(spin_system *s, const double *d_n, double *d_f);     // d_f (SoA, meV) = dipolar force of d_n
 void ddi_release(spin_system *s);
+const char *ddi_path_name(const spin_system *s);                      // "off", "3d", "slab", "slab+mirror"
 
 // spin_jit.cu
 std::string jit_source(const spin_system *s);

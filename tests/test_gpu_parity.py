@@ -353,6 +353,8 @@ def test_ddi_slab_mirror_symmetry_of_the_tensor(P, O, bravais, cells, monkeypatc
     Bo = o.effective_field()
     Bg = g.effective_field()
     assert_fields_close(Bg, Bo)
+    tilted = abs(bravais[2][0]) + abs(bravais[2][1]) > 0
+    assert g.spin_ddi_info() == ("slab" if tilted else "slab+mirror"), g.spin_ddi_info()
     w0 = dataclasses.replace(w, pair_J=w.pair_J * 0, pair_D=w.pair_D * 0, B=0.0, aniso=[])
     g0, o0 = pair(P, O, w0)
     Fd = o0.ddi_field(direct=True) / (w.mu_s[0] * O.MU_B)
@@ -360,6 +362,7 @@ def test_ddi_slab_mirror_symmetry_of_the_tensor(P, O, bravais, cells, monkeypatc
     monkeypatch.setenv("SPINLLG_DDI_MIRROR", "0")      # all planes read, whatever the symmetry
     h = P.SpinSystem.from_workload(w)
     Bh = h.effective_field()
+    assert h.spin_ddi_info() == "slab"
     assert_fields_close(Bh, Bo)
     assert np.abs(Bh - Bg).max() <= 1e-13 * np.abs(Bo).max()
     g.llg_iterate(10); o.iterate(10)
