@@ -260,7 +260,7 @@ def main():
             "config": {"workload": w.name, "spins": N, "llg_iterations_per_step": inner, "solver": "Depondt", "parallelism": f"replicas x{world}",
                        "l2": "state arrays n, n^p, n' = %.0f MB > 126 MB L2 (no flush needed)" % (3 * 24 * N / 1e6) if 72 * N > 126e6 else
                              "state %.1f MB is L2-resident; effective bandwidth reported" % (3 * 24 * N / 1e6),
-                       "store_A": args.store_A, "kernels": sys_.spin_kernel_info(), "nvrtc": P.spin_jit_compiler_info()},
+                       "store_A": args.store_A, "kernels": sys_.spin_kernel_info(), "ddi": sys_.spin_ddi_info(), "nvrtc": P.spin_jit_compiler_info()},
             "clocks": clocks,
             "e2e": {"value": e2e_value, "unit": "spin-updates/s", "h2d_bytes_per_step": int(host_in.numel() * 8), "d2h_bytes_per_step": int(host_out.numel() * 8),
                     "steps": e2e_steps},
