@@ -33,9 +33,12 @@
  * dynamics: tanh at fixed azimuth; velocity projection: (k + 1/2) dt^2 F / m and the FM ground state; pinned spins: Eq. 12 about the
  * pinned neighbour; vacancies: decoupled neighbours; several anisotropy axes: biaxial closed form; topological charge: octant area,
  * Girard's excess, Q = -1 / +1 / 0 / -2; GNEB: geodesic distance, force geometry, equidistant relaxation, barrier = K with a climbing
- * image; image noise streams: moments and cross-correlations; current-driven wall of Fig. 6: velocity (beta / alpha) u.
+ * image; image noise streams: moments and cross-correlations; current-driven wall of Fig. 6: velocity (beta / alpha) u;
+ * orc_effective_field: free spins feel the applied field in Tesla for mu_s = 2 and 5, ferromagnet B + (2K + zJ)/(mu_s mu_B), per-atom
+ * moments; orc_observables: M of a known configuration, max torque mu_s mu_B B sin(theta) of one tilted spin and |n x F| with a bond.
  * "parity unpinned" (convention only): DMI chirality sign of the helper conventions (R15), DDI image count (R16),
- * periodic self-wrap (R21), max-torque norm (R22), the optimiser of the GNEB chain (steepest descent, R31).
+ * periodic self-wrap (R21), the choice of the max norm over spins for "max torque" (R22; its value is pinned), the optimiser of the
+ * GNEB chain (steepest descent, R31).
  *
  * Build: gcc -O2 -ffp-contract=off -fopenmp -shared -fPIC (see oracle/build.py).
  */

@@ -821,3 +821,72 @@ def test_current_driven_domain_wall_moves_at_beta_over_alpha_u():
     v = np.polyfit(ts[120:], xs[120:], 1)[0]
     assert v == pytest.approx(beta / alpha * u, rel=0.04), v
     assert np.array_equal(s.spins()[0], n0[0]) and np.array_equal(s.spins()[-1], n0[-1])
+
+
+# ------------------------------------------------------------------ what the boundary returns: effective field in Tesla, observables
+@pytest.mark.parametrize("mu_s", [2.0, 5.0])
+def test_effective_field_of_free_spins_is_the_applied_field_in_tesla(mu_s):
+    """PAPER.md:155 "B_eff = -dH/dn_i", reading R2: the boundary returns F / (mu_s mu_B) in Tesla.  Free spins in a field B: the Zeeman
+    force is mu_s mu_B B (Eq. 1 :61), so the effective field is B itself whatever the moment -- a dropped or doubled mu_B, or a
+    field left in meV, fails this."""
+    s = OracleSystem(np.eye(3), [[0, 0, 0]], (4, 3, 2), (0, 0, 0))
+    s.set_mu_s([mu_s])
+    d = np.array([1.0, 2.0, -2.0]) / 3.0
+    s.set_field(1.7, d)
+    s.set_spins(rand_spins(s.N, 11))
+    B = s.effective_field()
+    assert np.allclose(B, 1.7 * d, rtol=0, atol=1e-15)
+    # the force itself (meV) does scale with the moment
+    F = s.gradient()
+    assert np.allclose(F, mu_s * O.MU_B * 1.7 * d, rtol=1e-15, atol=0)
+
+
+@pytest.mark.parametrize("cfg,cells,z", [(1, (8, 6, 1), 4), (3, (6, 5, 4), 6)])
+def test_effective_field_of_the_ferromagnet_in_tesla(cfg, cells, z):
+    """All n = z, periodic (O1): F_z = mu_s mu_B B + 2 K + z J (unique pairs, each bond felt from both ends), DMI cancels, so
+    B_eff,z = B + (2 K + z J) / (mu_s mu_B) in Tesla, to 1e-13 (readings R2-R4)."""
+    w = small(cfg, cells)
+    s = OracleSystem.from_workload(w)
+    s.set_spins(np.tile([0.0, 0.0, 1.0], (s.N, 1)))
+    K = w.aniso[0][1] if w.aniso else 0.0
+    mu = w.mu_s[0] * O.MU_B
+    B = s.effective_field()
+    expect = w.B + (2.0 * K + z * 1.0) / mu
+    assert np.allclose(B[:, 2], expect, rtol=1e-13, atol=0)
+    assert np.abs(B[:, :2]).max() < 1e-12 * expect
+
+
+def test_effective_field_uses_the_moment_of_each_basis_atom():
+    """Two sublattices with different moments in the same applied field: both see B Tesla, and the pair term J n_j enters as
+    J / (mu_b mu_B), with the moment of the atom the field acts ON."""
+    s = OracleSystem(np.eye(3), [[0, 0, 0], [0.5, 0.5, 0.5]], (3, 3, 3), (1, 1, 1))
+    s.set_mu_s([2.0, 5.0])
+    s.set_field(0.5, (0, 0, 1))
+    s.set_pairs([0], [1], [[0, 0, 0]], [1.5])
+    s.set_spins(np.tile([0.0, 0.0, 1.0], (s.N, 1)))
+    B = s.effective_field()
+    assert np.allclose(B[0::2, 2], 0.5 + 1.5 / (2.0 * O.MU_B), rtol=1e-14)
+    assert np.allclose(B[1::2, 2], 0.5 + 1.5 / (5.0 * O.MU_B), rtol=1e-14)
+
+
+def test_observables_magnetisation_and_max_torque_closed_forms():
+    """PAPER.md:131 m = (1/N) sum_i n_i; reading R22: max torque = max_i |F_i - (F_i . n_i) n_i| in meV.  One spin tilted by theta away
+    from the field among aligned free spins: M is known exactly and the largest torque is mu_s mu_B B sin(theta) (= |n x F|)."""
+    mu_s, Bf, theta = 3.0, 2.0, 0.4
+    s = OracleSystem(np.eye(3), [[0, 0, 0]], (5, 4, 1), (0, 0, 0))
+    s.set_mu_s([mu_s]); s.set_field(Bf, (0, 0, 1))
+    n = np.tile([0.0, 0.0, 1.0], (s.N, 1))
+    n[7] = [math.sin(theta), 0.0, math.cos(theta)]
+    n[3] = [0.0, 0.0, -1.0]                         # antiparallel: no torque, but it counts in M
+    s.set_spins(n)
+    M, tq = s.observables()
+    assert M[0] == pytest.approx(math.sin(theta) / s.N, rel=1e-14)
+    assert M[1] == 0.0
+    assert M[2] == pytest.approx((s.N - 2 + math.cos(theta) - 1.0) / s.N, rel=1e-14)
+    assert tq == pytest.approx(mu_s * O.MU_B * Bf * math.sin(theta), rel=1e-13)
+    # with an exchange bond the torque on the pair is |n x (F_Zeeman + J n_j)|
+    s.set_pairs([0], [0], [[1, 0, 0]], [0.8])
+    F = s.gradient()
+    expect = max(np.linalg.norm(np.cross(n[i], F[i])) for i in range(s.N))
+    M2, tq2 = s.observables()
+    assert tq2 == pytest.approx(expect, rel=1e-13) and np.array_equal(M, M2)
