@@ -344,6 +344,21 @@ int allocate_arrays(spin_system *s, const DevicePlan &P, bool keep) {
     return SPIN_OK;
 }
 
+// per-image factor on the thermal amplitude, sqrt(T_image / T), from the absolute image temperatures kept on the host; called whenever
+// either side of the ratio changes (llg_set_image_temperatures, llg_configure through ensure_plan)
+int upload_image_sigma(spin_system *s) {
+    if (s->img_T.empty()) return SPIN_OK;
+    if (!(s->T > 0.0)) return spin::fail(SPIN_ERR_STATE, "per-image temperatures are set but the reference temperature of llg_configure is 0: set T > 0 or clear them");
+    if ((int)s->img_T.size() != s->n_img) return spin::fail(SPIN_ERR_STATE, "per-image temperatures were set for %d images, the system has %d", (int)s->img_T.size(), s->n_img);
+    std::vector<double> sc((size_t)s->n_img);
+    for (int k = 0; k < s->n_img; ++k) sc[(size_t)k] = sqrt(s->img_T[(size_t)k] / s->T);
+    if (!s->d_img_sigma) SPIN_CUDA(cudaMalloc(&s->d_img_sigma, (size_t)s->n_img * sizeof(double)));
+    SPIN_CUDA(cudaMemcpyAsync(s->d_img_sigma, sc.data(), (size_t)s->n_img * sizeof(double), cudaMemcpyHostToDevice, s->stream));
+    SPIN_CUDA(cudaStreamSynchronize(s->stream));
+    drop_graphs(s);                           // captured launches hold the old pointer
+    return SPIN_OK;
+}
+
 int ensure_plan(spin_system *s) {
     NEED_DEVICE(s);
     if (!s->plan_dirty) return SPIN_OK;
@@ -357,6 +372,8 @@ int ensure_plan(spin_system *s) {
         if (rc) return rc;
     }
     s->plan = P;
+    rc = upload_image_sigma(s);               // T may have changed: the ratios sqrt(T_image / T) follow
+    if (rc) return rc;
     if (s->ddi_on) {
         rc = ddi_prepare(s);
         if (rc) return rc;
@@ -737,18 +754,24 @@ extern "C" int spin_set_images(spin_system *s, int n_images) {
     const int n_old = s->n_img, n_keep = std::min(n_old, n_images);
     double *old = nullptr;
     SPIN_CUDA(cudaMalloc(&old, (size_t)n_old * ibytes));
-    SPIN_CUDA(cudaMemcpy(old, s->d_n[s->cur], (size_t)n_old * ibytes, cudaMemcpyDeviceToDevice));
+    {   // every copy goes through the system's stream (a device-to-device cudaMemcpy on the legacy stream is not ordered with it)
+        cudaError_t e = cudaMemcpyAsync(old, s->d_n[s->cur], (size_t)n_old * ibytes, cudaMemcpyDeviceToDevice, s->stream);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(s->stream);
+        if (e != cudaSuccess) { cudaFree(old); return spin::fail(SPIN_ERR_CUDA, "spin_set_images: %s", cudaGetErrorString(e)); }
+    }
     s->n_img = n_images;
     s->img_sel = 0;
     rc = allocate_arrays(s, s->plan, false);
     if (rc == SPIN_OK) {
-        cudaError_t e = cudaMemcpy(s->d_n[0], old, (size_t)n_keep * ibytes, cudaMemcpyDeviceToDevice);
+        cudaError_t e = cudaMemcpyAsync(s->d_n[0], old, (size_t)n_keep * ibytes, cudaMemcpyDeviceToDevice, s->stream);
         for (int k = n_keep; k < n_images && e == cudaSuccess; ++k)      // new images start as copies of image 0
-            e = cudaMemcpy(s->d_n[0] + (size_t)k * istr, old, ibytes, cudaMemcpyDeviceToDevice);
+            e = cudaMemcpyAsync(s->d_n[0] + (size_t)k * istr, old, ibytes, cudaMemcpyDeviceToDevice, s->stream);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(s->stream);
         if (e != cudaSuccess) rc = spin::fail(SPIN_ERR_CUDA, "spin_set_images: %s", cudaGetErrorString(e));
     }
     cudaFree(old);
     if (s->d_img_sigma) { cudaFree(s->d_img_sigma); s->d_img_sigma = nullptr; }
+    s->img_T.clear();                         // per-image temperatures belong to the old image count
     s->plan_dirty = true;                     // kernels variants and dipolar buffers depend on the image count
     drop_graphs(s);
     return rc;
@@ -762,17 +785,11 @@ extern "C" int llg_set_image_temperatures(spin_system *s, const double *T_kelvin
     REQUIRE(s, "null system");
     NEED_DEVICE(s);
     SPIN_CUDA(cudaStreamSynchronize(s->stream));
-    if (!T_kelvin) { if (s->d_img_sigma) { cudaFree(s->d_img_sigma); s->d_img_sigma = nullptr; } drop_graphs(s); return SPIN_OK; }
+    if (!T_kelvin) { s->img_T.clear(); if (s->d_img_sigma) { cudaFree(s->d_img_sigma); s->d_img_sigma = nullptr; } drop_graphs(s); return SPIN_OK; }
     REQUIRE(s->T > 0.0, "llg_configure must set a positive reference temperature first");
-    std::vector<double> sc((size_t)s->n_img);
-    for (int k = 0; k < s->n_img; ++k) {
-        REQUIRE(T_kelvin[k] >= 0.0 && isfinite(T_kelvin[k]), "image %d: temperature must be >= 0", k);
-        sc[(size_t)k] = sqrt(T_kelvin[k] / s->T);
-    }
-    if (!s->d_img_sigma) SPIN_CUDA(cudaMalloc(&s->d_img_sigma, (size_t)s->n_img * sizeof(double)));
-    SPIN_CUDA(cudaMemcpy(s->d_img_sigma, sc.data(), (size_t)s->n_img * sizeof(double), cudaMemcpyHostToDevice));
-    drop_graphs(s);                           // captured launches hold the old pointer
-    return SPIN_OK;
+    for (int k = 0; k < s->n_img; ++k) REQUIRE(T_kelvin[k] >= 0.0 && isfinite(T_kelvin[k]), "image %d: temperature must be >= 0", k);
+    s->img_T.assign(T_kelvin, T_kelvin + s->n_img);      // absolute temperatures: the scale array follows later changes of T
+    return upload_image_sigma(s);
 }
 
 // pinned spins: flags in boundary order; null clears.  A pinned site may hold the zero vector (a vacancy).
@@ -787,7 +804,8 @@ extern "C" int spins_set_pinned(spin_system *s, const unsigned char *mask) {
             cudaError_t e = cudaMalloc(&s->d_pin, (size_t)s->N);
             if (e != cudaSuccess) { s->d_pin = nullptr; return spin::fail(SPIN_ERR_MEMORY, "device allocation of %lld bytes failed", (long long)s->N); }
         }
-        SPIN_CUDA(cudaMemcpy(s->d_pin, mask, (size_t)s->N, cudaMemcpyHostToDevice));
+        SPIN_CUDA(cudaMemcpyAsync(s->d_pin, mask, (size_t)s->N, cudaMemcpyHostToDevice, s->stream));
+        SPIN_CUDA(cudaStreamSynchronize(s->stream));
     }
     s->plan.pin = s->d_pin;       // pack_kernel reads it before the next plan build
     s->plan_dirty = true;
@@ -860,7 +878,8 @@ extern "C" int llg_set_step(spin_system *s, uint64_t step) {
     if (!s->has_device) return SPIN_OK;
     SPIN_CUDA(cudaStreamSynchronize(s->stream));
     const unsigned long long v = step;
-    SPIN_CUDA(cudaMemcpy(s->d_step, &v, sizeof(v), cudaMemcpyHostToDevice));
+    SPIN_CUDA(cudaMemcpyAsync(s->d_step, &v, sizeof(v), cudaMemcpyHostToDevice, s->stream));      // ordered on the system's stream, like the sweeps
+    SPIN_CUDA(cudaStreamSynchronize(s->stream));
     return SPIN_OK;
 }
 
@@ -1035,12 +1054,12 @@ int gneb_run(spin_system *s, int64_t n_iter, double step, double kappa, int clim
     const Launch L = brick_launch(s);
     const int nblocks = (int)(L.grid.x * L.grid.y);
     const size_t istr = (size_t)s->nb * s->plan.sub;
-    double *d_part = nullptr, *d_sc = nullptr, *d_E = nullptr;
-    SPIN_CUDA(cudaMalloc(&d_part, (size_t)M * nblocks * 3 * sizeof(double)));
-    SPIN_CUDA(cudaMalloc(&d_sc, (size_t)M * 3 * sizeof(double)));
-    SPIN_CUDA(cudaMalloc(&d_E, (size_t)M * sizeof(double)));
-    double *d_red = nullptr;                     // N_RED reductions per image; the energies never leave the device during the relaxation
-    SPIN_CUDA(cudaMalloc(&d_red, (size_t)M * 16 * sizeof(double)));
+    // one scratch block (nothing to leak on an error path): partial sums, per-image scalars, energies, N_RED reductions per image (the
+    // energies never leave the device during the relaxation)
+    double *d_scratch = nullptr;
+    const size_t n_part = (size_t)M * nblocks * 3, n_sc = (size_t)M * 3, n_E = (size_t)M, n_red = (size_t)M * 16;
+    SPIN_CUDA(cudaMalloc(&d_scratch, (n_part + n_sc + n_E + n_red) * sizeof(double)));
+    double *d_part = d_scratch, *d_sc = d_part + n_part, *d_E = d_sc + n_sc, *d_red = d_E + n_E;
     const int sel = s->img_sel;
     int rc = SPIN_OK;
     dim3 grid(L.grid.x, L.grid.y, (unsigned)M);
@@ -1071,10 +1090,11 @@ int gneb_run(spin_system *s, int64_t n_iter, double step, double kappa, int clim
         if (e != cudaSuccess) rc = spin::fail(SPIN_ERR_CUDA, "gneb: %s", cudaGetErrorString(e));
     }
     if (rc == SPIN_OK && want_outputs) {
-        if (E_host) cudaMemcpy(E_host, d_E, (size_t)M * sizeof(double), cudaMemcpyDeviceToHost);
+        if (E_host) { cudaMemcpyAsync(E_host, d_E, (size_t)M * sizeof(double), cudaMemcpyDeviceToHost, s->stream); cudaStreamSynchronize(s->stream); }
         if (l_host) {
             std::vector<double> sc((size_t)3 * M);
-            cudaMemcpy(sc.data(), d_sc, sc.size() * sizeof(double), cudaMemcpyDeviceToHost);
+            cudaMemcpyAsync(sc.data(), d_sc, sc.size() * sizeof(double), cudaMemcpyDeviceToHost, s->stream);
+            cudaStreamSynchronize(s->stream);
             for (int nu = 0; nu < M; ++nu) l_host[nu] = sc[(size_t)3 * nu + 2];
         }
         if (F_host) {
@@ -1088,7 +1108,7 @@ int gneb_run(spin_system *s, int64_t n_iter, double step, double kappa, int clim
         }
     }
     s->img_sel = sel;
-    cudaFree(d_part); cudaFree(d_sc); cudaFree(d_E); cudaFree(d_red);
+    cudaFree(d_scratch);
     if (rc == SPIN_OK && cudaGetLastError() != cudaSuccess) rc = spin::fail(SPIN_ERR_CUDA, "gneb: kernel launch failed");
     return rc;
 }
@@ -1222,8 +1242,18 @@ extern "C" int spin_jit_compiler_info(char *buf, int len) {
 // needed) and the size of the cubin is returned in *cubin_bytes
 extern "C" int spin_jit_source(spin_system *s, char *buf, int len, int compile, int64_t *cubin_bytes) {
     REQUIRE(s, "null system");
-    int rc = build_plan(s, s->plan);
-    if (rc) return rc;
+    int rc;
+    if (s->has_device) {
+        // a live system: bring plan, arrays and kernels up to date together (the plan must never describe a layout the arrays do not have)
+        rc = ensure_plan(s);
+        if (rc) return rc;
+    } else {
+        // planner-only mode: there are no device arrays; a plan that fails half-way must not replace the last good one
+        DevicePlan P;
+        rc = build_plan(s, P);
+        if (rc) return rc;
+        s->plan = P;
+    }
     const std::string src = jit_source(s);
     if (buf && len > 0) snprintf(buf, (size_t)len, "%s", src.c_str());
     if (compile) {

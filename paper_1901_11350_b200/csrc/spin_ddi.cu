@@ -49,6 +49,8 @@ struct DdiState {
 
 namespace {
 
+template <int V> struct spin_ddi_int { static constexpr int value = V; };
+
 struct DdiGeom {
     double brav[9];                      // rows, Angstrom
     double basis[3 * SPIN_MAX_BASIS];    // fractional
@@ -180,70 +182,184 @@ __global__ void real_part_kernel(const cufftDoubleComplex *__restrict__ in, doub
     if (i < n) out[i] = in[i].x;
 }
 
-// twiddles exp(-2 pi i j / PZ), j < PZ <= 16
-__constant__ double DDI_WR[16], DDI_WI[16];
+// twiddles exp(-2 pi i t / PZ), t < PZ, for every padded length along c the slab path takes (PZ <= 16), indexed [PZ][t].  The table is
+// a function of PZ alone, so every system of the process shares it (films of different thickness may be alive at the same time).
+__constant__ double DDI_TWR[17][16], DDI_TWI[17][16];
 
-// Slab path, one thread per in-plane wave vector q = (kx, ky):
-//   M^(kz) = sum_{z < NZ} M2(z) w^(kz z)          (pruned transform along c: planes z >= NZ are zero padding)
-//   H^(kz) = K^(kz) . M^(kz)                      (6-component real symmetric tensor)
-//   H2(z)  = sum_{kz < PZ} H^(kz) w^(-kz z),  z < NZ only
-// (A radix-2 version of the two short transforms -- 3.4x fewer flops -- was measured slower, 358 vs 348 us per cfg5 step: it needs 254
-// registers and spills its accumulators; the kernel is bound by its 200 MB of traffic, not by the sums.)
-// M2 / H2: element (kb, slab = c NZ + z, ka) at (kb SL + slab) S1p + ka, S1p the row pitch (H2 may be M2: every thread reads its column, then writes it);
-// Kre: [6][PZ][S2] with q = kb S1 + ka.
-template <int NZ, int PZ, bool MIRROR>
-__global__ void __launch_bounds__(128) ddi_slab_contract_kernel(const double *__restrict__ Kre, const cufftDoubleComplex *__restrict__ M2,
-                                                                 cufftDoubleComplex *H2, long long S2, int S1, int S1p) {
-    const long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (q >= S2) return;
-    const long long kb = q / S1, ka = q - kb * S1;
-    const size_t col = (size_t)kb * (3 * NZ) * S1p + ka;           // slab 0 of this wave vector; slabs are one row pitch apart
-    double mr[3][NZ], mi[3][NZ], hr[3][NZ], hi[3][NZ];
+__host__ __device__ constexpr bool ddi_pow2(int n) { return n > 0 && (n & (n - 1)) == 0; }
+__host__ __device__ constexpr int ddi_bitrev(int p, int n) {      // n a power of two
+    int r = 0;
+    for (int b = 1, c = n >> 1; b < n; b <<= 1, c >>= 1) if (p & b) r |= c;
+    return r;
+}
+// position of frequency j in the array the forward transform leaves (bit reversed for powers of two, natural otherwise; an involution)
+template <int N> __host__ __device__ constexpr int ddi_pos(int j) { return ddi_pow2(N) ? ddi_bitrev(j, N) : j; }
+
+// y(j) = sum_z x(z) W_N^(j z), W_N = exp(-2 pi i / N) = W_PZ^2 (PZ = 2 N), in place.  Powers of two: radix-2 decimation in frequency, the
+// result is left in bit-reversed order; other lengths (3, 5, 6, 7): the plain sum, natural order.  Fully unrolled: x stays in registers.
+template <int N>
+__device__ __forceinline__ void ddi_dft_fwd(double (&re)[N], double (&im)[N]) {
+    constexpr int PZ = 2 * N;
+    if constexpr (ddi_pow2(N)) {
 #pragma unroll
-    for (int c = 0; c < 3; ++c)
+        for (int half = N / 2; half >= 1; half /= 2)
 #pragma unroll
-        for (int z = 0; z < NZ; ++z) {
-            const cufftDoubleComplex v = M2[col + (size_t)(c * NZ + z) * S1p];
-            mr[c][z] = v.x; mi[c][z] = v.y; hr[c][z] = 0.0; hi[c][z] = 0.0;
-        }
-    // one wave number along c: forward sum, contraction with the six tensor components, inverse sum into hr / hi
-    auto one_kz = [&](const int kz, const double kxx, const double kxy, const double kxz, const double kyy, const double kyz, const double kzz) {
-        double Mr[3], Mi[3];
+            for (int base = 0; base < N; base += 2 * half)
 #pragma unroll
-        for (int c = 0; c < 3; ++c) {
-            double ar = 0.0, ai = 0.0;
+                for (int j = 0; j < half; ++j) {
+                    const int t = j * (N / (2 * half)) * 2;      // W_(2 half)^j as a power of W_PZ
+                    const double ar = re[base + j], ai = im[base + j], br = re[base + j + half], bi = im[base + j + half];
+                    re[base + j] = ar + br; im[base + j] = ai + bi;
+                    const double dr = ar - br, di = ai - bi, wr = DDI_TWR[PZ][t], wi = DDI_TWI[PZ][t];
+                    re[base + j + half] = fma(dr, wr, -di * wi); im[base + j + half] = fma(dr, wi, di * wr);
+                }
+    } else {
+        double yr[N], yi[N];
 #pragma unroll
-            for (int z = 0; z < NZ; ++z) {
-                const double wr = DDI_WR[(kz * z) % PZ], wi = DDI_WI[(kz * z) % PZ];
-                ar = fma(mr[c][z], wr, fma(-mi[c][z], wi, ar));
-                ai = fma(mr[c][z], wi, fma(mi[c][z], wr, ai));
+        for (int j = 0; j < N; ++j) {
+            double sr = 0.0, si = 0.0;
+#pragma unroll
+            for (int z = 0; z < N; ++z) {
+                const int t = (2 * j * z) % PZ;
+                const double wr = DDI_TWR[PZ][t], wi = DDI_TWI[PZ][t];
+                sr = fma(re[z], wr, fma(-im[z], wi, sr)); si = fma(re[z], wi, fma(im[z], wr, si));
             }
-            Mr[c] = ar; Mi[c] = ai;
+            yr[j] = sr; yi[j] = si;
         }
-        const double Hr[3] = {kxx * Mr[0] + kxy * Mr[1] + kxz * Mr[2], kxy * Mr[0] + kyy * Mr[1] + kyz * Mr[2], kxz * Mr[0] + kyz * Mr[1] + kzz * Mr[2]};
-        const double Hi[3] = {kxx * Mi[0] + kxy * Mi[1] + kxz * Mi[2], kxy * Mi[0] + kyy * Mi[1] + kyz * Mi[2], kxz * Mi[0] + kyz * Mi[1] + kzz * Mi[2]};
+#pragma unroll
+        for (int j = 0; j < N; ++j) { re[j] = yr[j]; im[j] = yi[j]; }
+    }
+}
+// x(z) = sum_j y(j) W_N^(-j z), unnormalised, from the order ddi_dft_fwd leaves to natural order, in place
+template <int N>
+__device__ __forceinline__ void ddi_dft_inv(double (&re)[N], double (&im)[N]) {
+    constexpr int PZ = 2 * N;
+    if constexpr (ddi_pow2(N)) {
+#pragma unroll
+        for (int half = 1; half < N; half *= 2)
+#pragma unroll
+            for (int base = 0; base < N; base += 2 * half)
+#pragma unroll
+                for (int j = 0; j < half; ++j) {
+                    const int t = j * (N / (2 * half)) * 2;
+                    const double wr = DDI_TWR[PZ][t], wi = -DDI_TWI[PZ][t];      // conjugate twiddle
+                    const double br = fma(re[base + j + half], wr, -im[base + j + half] * wi), bi = fma(re[base + j + half], wi, im[base + j + half] * wr);
+                    const double ar = re[base + j], ai = im[base + j];
+                    re[base + j] = ar + br; im[base + j] = ai + bi;
+                    re[base + j + half] = ar - br; im[base + j + half] = ai - bi;
+                }
+    } else {
+        double yr[N], yi[N];
+#pragma unroll
+        for (int z = 0; z < N; ++z) {
+            double sr = 0.0, si = 0.0;
+#pragma unroll
+            for (int j = 0; j < N; ++j) {
+                const int t = (2 * j * z) % PZ;
+                const double wr = DDI_TWR[PZ][t], wi = -DDI_TWI[PZ][t];
+                sr = fma(re[j], wr, fma(-im[j], wi, sr)); si = fma(re[j], wi, fma(im[j], wr, si));
+            }
+            yr[z] = sr; yi[z] = si;
+        }
+#pragma unroll
+        for (int z = 0; z < N; ++z) { re[z] = yr[z]; im[z] = yi[z]; }
+    }
+}
+
+// Slab path, the transform along c fused with the tensor contraction, per in-plane wave vector q = (kx, ky):
+//   M^(kz) = sum_{z < NZ} M2(z) w^(kz z),  w = exp(-2 pi i / PZ)     (pruned: planes z >= NZ are zero padding)
+//   H^(kz) = K^(kz) . M^(kz)                                          (6-component real symmetric tensor)
+//   H2(z)  = sum_{kz < PZ} H^(kz) w^(-kz z),  z < NZ only
+// Two threads share a column: thread e of the pair takes the wave numbers kz = 2 j + e,
+//   M^(2 j + e) = sum_z [M2(z) w^(e z)] W_NZ^(j z),    H2(z) = sum_e w^(-e z) sum_j H^(2 j + e) W_NZ^(-j z),
+// i.e. a length-NZ transform of the (for e = 1: pre-twisted) column, the contraction at its own NZ wave numbers, the inverse length-NZ
+// transform and the twist back; the two halves are added through shared memory.  Each thread then holds 3 NZ complex numbers instead of
+// the 3 (NZ + PZ) of a one-thread-per-column kernel (255 registers, 12.5 % occupancy in round 1).  A mirror-symmetric tensor
+// (K(PZ - kz) = +-K(kz), ddi_mirror_check_kernel) is read once for kz and PZ - kz, which have the same parity and so the same thread.
+// PAD = false: a single plane that is not padded along c (NZ = PZ = 1): no transform at all, thread e = 1 idles.
+// M2 / H2: element (kb, slab = c NZ + z, ka) at (kb SL + slab) S1p + ka, S1p the row pitch (H2 may be M2: every column is read, then
+// written, by its own pair of threads); Kre: [6][PZ][S2] with q = kb S1 + ka.
+constexpr int DDI_CT_COLS = 64;      // columns per block: 2 x 64 threads
+template <int NZ, bool PAD, bool MIRROR>
+__global__ void __launch_bounds__(2 * DDI_CT_COLS, 4) ddi_slab_contract_kernel(const double *__restrict__ Kre, const cufftDoubleComplex *__restrict__ M2,
+                                                                             cufftDoubleComplex *H2, long long S2, int S1, int S1p) {
+    constexpr int PZ = PAD ? 2 * NZ : NZ;
+    static_assert(PAD || NZ == 1, "only a single plane goes unpadded");
+    __shared__ double2 half1[3 * NZ][DDI_CT_COLS];
+    const int lane_col = threadIdx.x % DDI_CT_COLS, e = threadIdx.x / DDI_CT_COLS;
+    const long long q = (long long)blockIdx.x * DDI_CT_COLS + lane_col;
+    const bool live = q < S2 && (PAD || e == 0);
+    const long long kb = live ? q / S1 : 0, ka = live ? q - kb * S1 : 0;
+    const size_t col = (size_t)kb * (3 * NZ) * S1p + ka;           // slab 0 of this wave vector; slabs are one row pitch apart
+    double xr[3][NZ], xi[3][NZ];
+    if (live) {
 #pragma unroll
         for (int c = 0; c < 3; ++c)
 #pragma unroll
             for (int z = 0; z < NZ; ++z) {
-                const double wr = DDI_WR[(kz * z) % PZ], wi = -DDI_WI[(kz * z) % PZ];      // conjugate twiddle
-                hr[c][z] = fma(Hr[c], wr, fma(-Hi[c], wi, hr[c][z]));
-                hi[c][z] = fma(Hr[c], wi, fma(Hi[c], wr, hi[c][z]));
+                const cufftDoubleComplex v = M2[col + (size_t)(c * NZ + z) * S1p];
+                xr[c][z] = v.x; xi[c][z] = v.y;
             }
-    };
-    const size_t st = (size_t)PZ * S2;
+        if constexpr (PAD) {
+            if (e) {
 #pragma unroll
-    for (int kz = 0; kz < (MIRROR ? PZ / 2 + 1 : PZ); ++kz) {
-        const size_t o = (size_t)kz * S2 + q;
-        const double kxx = Kre[o], kxy = Kre[st + o], kxz = Kre[2 * st + o], kyy = Kre[3 * st + o], kyz = Kre[4 * st + o], kzz = Kre[5 * st + o];
-        one_kz(kz, kxx, kxy, kxz, kyy, kyz, kzz);
-        // mirrored tensor (ddi_mirror_check_kernel): the plane PZ - kz holds the same values, xz and yz with the opposite sign
-        if constexpr (MIRROR) { if (kz > 0 && 2 * kz < PZ) one_kz(PZ - kz, kxx, kxy, -kxz, kyy, -kyz, kzz); }
+                for (int c = 0; c < 3; ++c)
+#pragma unroll
+                    for (int z = 1; z < NZ; ++z) {
+                        const double wr = DDI_TWR[PZ][z], wi = DDI_TWI[PZ][z], r = xr[c][z], i = xi[c][z];
+                        xr[c][z] = fma(r, wr, -i * wi); xi[c][z] = fma(r, wi, i * wr);
+                    }
+            }
+#pragma unroll
+            for (int c = 0; c < 3; ++c) ddi_dft_fwd<NZ>(xr[c], xi[c]);
+        }
+        // contraction at the wave numbers of this thread; position p of the transformed column holds kz = 2 ddi_pos(p) + e
+        const size_t st = (size_t)PZ * S2;
+        auto contract = [&](const int p, const double kxx, const double kxy, const double kxz, const double kyy, const double kyz, const double kzz) {
+            const double r0 = xr[0][p], r1 = xr[1][p], r2 = xr[2][p], i0 = xi[0][p], i1 = xi[1][p], i2 = xi[2][p];
+            xr[0][p] = kxx * r0 + kxy * r1 + kxz * r2; xr[1][p] = kxy * r0 + kyy * r1 + kyz * r2; xr[2][p] = kxz * r0 + kyz * r1 + kzz * r2;
+            xi[0][p] = kxx * i0 + kxy * i1 + kxz * i2; xi[1][p] = kxy * i0 + kyy * i1 + kyz * i2; xi[2][p] = kxz * i0 + kyz * i1 + kzz * i2;
+        };
+        auto planes = [&](auto ec) {
+            constexpr int E = decltype(ec)::value;
+#pragma unroll
+            for (int j = 0; j < NZ; ++j) {
+                const int kz = PAD ? 2 * j + E : 0;
+                if (MIRROR && 2 * kz > PZ) continue;                      // taken together with its mirror image below
+                const size_t o = (size_t)kz * S2 + q;
+                const double kxx = Kre[o], kxy = Kre[st + o], kxz = Kre[2 * st + o], kyy = Kre[3 * st + o], kyz = Kre[4 * st + o], kzz = Kre[5 * st + o];
+                contract(ddi_pos<NZ>(j), kxx, kxy, kxz, kyy, kyz, kzz);
+                if (MIRROR && kz > 0 && 2 * kz < PZ)                        // plane PZ - kz: the same values, xz and yz with the opposite sign
+                    contract(ddi_pos<NZ>((PZ - kz - E) / 2), kxx, kxy, -kxz, kyy, -kyz, kzz);
+            }
+        };
+        if (e) planes(spin_ddi_int<1>{}); else planes(spin_ddi_int<0>{});
+        if constexpr (PAD) {
+#pragma unroll
+            for (int c = 0; c < 3; ++c) ddi_dft_inv<NZ>(xr[c], xi[c]);
+            if (e) {
+#pragma unroll
+                for (int c = 0; c < 3; ++c)
+#pragma unroll
+                    for (int z = 0; z < NZ; ++z) {
+                        double r = xr[c][z], i = xi[c][z];
+                        if (z > 0) { const double wr = DDI_TWR[PZ][z], wi = -DDI_TWI[PZ][z]; const double t = fma(r, wr, -i * wi); i = fma(r, wi, i * wr); r = t; }
+                        half1[c * NZ + z][lane_col] = make_double2(r, i);
+                    }
+            }
+        }
     }
+    if constexpr (PAD) __syncthreads();
+    if (live && e == 0) {
 #pragma unroll
-    for (int c = 0; c < 3; ++c)
+        for (int c = 0; c < 3; ++c)
 #pragma unroll
-        for (int z = 0; z < NZ; ++z) H2[col + (size_t)(c * NZ + z) * S1p] = make_cuDoubleComplex(hr[c][z], hi[c][z]);
+            for (int z = 0; z < NZ; ++z) {
+                double r = xr[c][z], i = xi[c][z];
+                if constexpr (PAD) { const double2 h = half1[c * NZ + z][lane_col]; r += h.x; i += h.y; }
+                H2[col + (size_t)(c * NZ + z) * S1p] = make_cuDoubleComplex(r, i);
+            }
+    }
 }
 
 // Is the tensor spectrum mirror symmetric along c, K_ab(kz) = s_ab K_ab(PZ - kz) with s = -1 for xz, yz and +1 otherwise?  (True when c is
@@ -312,11 +428,10 @@ int spin::ddi_prepare(spin_system *s) {
     for (int k = 2; k >= 0; --k) if (d->P[k] > 1) d->fdims[d->rank++] = d->P[k];
     d->Phalf = d->Ptot;
     if (d->rank > 0) { const int inner = d->fdims[d->rank - 1]; d->Phalf = d->Ptot / inner * (inner / 2 + 1); }
-    // slab path: one basis atom, both in-plane directions padded, at most 8 planes (power of two) along c
+    // slab path: one basis atom, both in-plane directions padded, at most 8 planes along c
     d->NZ = s->nc[2]; d->PZ = d->P[2];
     d->R2 = (int64_t)d->P[0] * d->P[1]; d->S2 = (int64_t)d->P[1] * (d->P[0] / 2 + 1);
-    const bool want_slab = s->opt_ddi_slab && nb == 1 && d->P[0] > 1 && d->P[1] > 1 &&
-                           (d->PZ == 1 || d->PZ == 2 || d->PZ == 4 || d->PZ == 8 || d->PZ == 16);
+    const bool want_slab = s->opt_ddi_slab && nb == 1 && d->P[0] > 1 && d->P[1] > 1 && d->NZ <= 8;
     size_t nreal = (size_t)nb * 3 * d->Ptot, ncplx = (size_t)nb * 3 * d->Phalf;
     d->SL = 3 * d->NZ; d->S1 = d->P[0] / 2 + 1; d->S1p = d->S1;      // a 128-byte row pitch (264) was measured slower: 368 vs 347 us per step on cfg5
     if (want_slab) {
@@ -349,12 +464,15 @@ int spin::ddi_prepare(spin_system *s) {
         SPIN_FFT(cufftSetStream(d->plan_a_fwd, s->stream));
         SPIN_FFT(cufftSetStream(d->plan_a_inv, s->stream));
         SPIN_FFT(cufftSetStream(d->plan_b, s->stream));
-        double wr[16], wi[16];
-        for (int j = 0; j < 16; ++j) { wr[j] = cos(-2.0 * M_PI * j / d->PZ); wi[j] = sin(-2.0 * M_PI * j / d->PZ); }
-        // exact values at the multiples of a quarter turn
-        for (int j = 0; j < d->PZ; ++j) if ((4 * j) % d->PZ == 0) { const int k = (4 * j) / d->PZ; wr[j] = k == 0 ? 1 : k == 2 ? -1 : 0; wi[j] = k == 1 ? -1 : k == 3 ? 1 : 0; }
-        SPIN_CUDA(cudaMemcpyToSymbolAsync(DDI_WR, wr, sizeof(wr), 0, cudaMemcpyHostToDevice, s->stream));
-        SPIN_CUDA(cudaMemcpyToSymbolAsync(DDI_WI, wi, sizeof(wi), 0, cudaMemcpyHostToDevice, s->stream));
+        // the twiddle table of every padded length (the same values whichever system uploads them)
+        static double twr[17][16], twi[17][16];
+        for (int pz = 1; pz <= 16; ++pz)
+            for (int t = 0; t < 16; ++t) {
+                twr[pz][t] = cos(-2.0 * M_PI * t / pz); twi[pz][t] = sin(-2.0 * M_PI * t / pz);
+                if ((4 * t) % pz == 0) { const int k = ((4 * t) / pz) % 4; twr[pz][t] = k == 0 ? 1 : k == 2 ? -1 : 0; twi[pz][t] = k == 1 ? -1 : k == 3 ? 1 : 0; }   // exact at quarter turns
+            }
+        SPIN_CUDA(cudaMemcpyToSymbolAsync(DDI_TWR, twr, sizeof(twr), 0, cudaMemcpyHostToDevice, s->stream));
+        SPIN_CUDA(cudaMemcpyToSymbolAsync(DDI_TWI, twi, sizeof(twi), 0, cudaMemcpyHostToDevice, s->stream));
     }
     if (d->rank > 0) {
         if (!want_slab) {
@@ -421,15 +539,16 @@ int spin::ddi_field(spin_system *s, const double *d_n, double *d_f) {
         ddi_slab_scatter_kernel<<<gcell, nt, 0, s->stream>>>(s->plan, d_n, d->P[0], d->SL, s->mu[0], d->s_in);
         SPIN_FFT(cufftExecD2Z(d->plan_a_fwd, d->s_in, d->s_a));                       // a-pass over the occupied rows only
         SPIN_FFT(cufftExecZ2Z(d->plan_b, d->s_a, d->s_b, CUFFT_FORWARD));            // b-pass
-        const unsigned gq = (unsigned)((d->S2 + 127) / 128);
-#define SPIN_CONTRACT(NZ_, PZ_, MIR_) ddi_slab_contract_kernel<NZ_, PZ_, MIR_><<<gq, 128, 0, s->stream>>>(d->d_Kre, d->s_b, d->s_b, (long long)d->S2, d->S1, d->S1p)
-        switch (d->PZ) {                                                              // c-pass + contraction + inverse c-pass, in place
-            case 1: SPIN_CONTRACT(1, 1, false); break;
-            case 2: SPIN_CONTRACT(1, 2, false); break;
-            case 4: if (d->mirror) SPIN_CONTRACT(2, 4, true); else SPIN_CONTRACT(2, 4, false); break;
-            case 8: if (d->mirror) SPIN_CONTRACT(4, 8, true); else SPIN_CONTRACT(4, 8, false); break;
-            default: if (d->mirror) SPIN_CONTRACT(8, 16, true); else SPIN_CONTRACT(8, 16, false); break;
+        const unsigned gq = (unsigned)((d->S2 + DDI_CT_COLS - 1) / DDI_CT_COLS);
+#define SPIN_CONTRACT(NZ_, PAD_, MIR_) ddi_slab_contract_kernel<NZ_, PAD_, MIR_><<<gq, 2 * DDI_CT_COLS, 0, s->stream>>>(d->d_Kre, d->s_b, d->s_b, (long long)d->S2, d->S1, d->S1p)
+#define SPIN_CONTRACT_NZ(NZ_) case NZ_: if (d->mirror) SPIN_CONTRACT(NZ_, true, true); else SPIN_CONTRACT(NZ_, true, false); break
+        if (d->PZ == 1) SPIN_CONTRACT(1, false, false);                                 // a single unpadded plane: contraction only
+        else switch (d->NZ) {                                                           // c-pass + contraction + inverse c-pass, in place
+            SPIN_CONTRACT_NZ(1); SPIN_CONTRACT_NZ(2); SPIN_CONTRACT_NZ(3); SPIN_CONTRACT_NZ(4);
+            SPIN_CONTRACT_NZ(5); SPIN_CONTRACT_NZ(6); SPIN_CONTRACT_NZ(7); SPIN_CONTRACT_NZ(8);
+            default: return spin::fail(SPIN_ERR_STATE, "dipolar slab path: %d planes not supported", d->NZ);
         }
+#undef SPIN_CONTRACT_NZ
 #undef SPIN_CONTRACT
         SPIN_FFT(cufftExecZ2Z(d->plan_b, d->s_b, d->s_d, CUFFT_INVERSE));            // inverse b-pass
         SPIN_FFT(cufftExecZ2D(d->plan_a_inv, d->s_d, d->s_out));                      // inverse a-pass, occupied rows only

@@ -134,6 +134,7 @@ struct spin_system {
     // one after the other (stride nb * plan.sub doubles); the sweeps take the image from blockIdx.z
     int n_img, img_sel;            // number of images; image that spins_set/get, effective_field, energy, ... address
     double *d_img_sigma;           // per-image factor on the thermal amplitude, sqrt(T_image / T), or null (all 1)
+    std::vector<double> img_T;     // the absolute per-image temperatures it was made from (empty: none set)
     unsigned int *d_bar;           // arrival counter of the cooperative kernel's grid barrier
     double *d_vp;                  // velocity-projection state: ratio r, started flag, |F|^2
     bool vp_active;                // d_A holds the force of the previous VP iteration

@@ -321,12 +321,16 @@ def test_full_size_configs(P, O, cfg, steps):
 
 # ---------------------------------------------------------------------------------------------------------------------
 # Dipolar slab path (csrc/spin_ddi.cu): 2-D cuFFT over the occupied planes + one kernel for the transform along c, the tensor
-# contraction and the inverse transform.  Taken for one basis atom and 1, 2, 4 or 8 planes; other shapes use the 3-D path.
+# contraction and the inverse transform.  Taken for one basis atom and 1 to 8 planes (any count: powers of two by a radix-2 transform in
+# registers, 3, 5, 6, 7 by the plain sum); other shapes use the 3-D path.
 @pytest.mark.parametrize("cells,per,img", [((20, 12, 4), (1, 1, 0), (2, 2, 0)), ((16, 10, 8), (1, 1, 0), (1, 1, 0)), ((12, 9, 2), (0, 1, 0), (0, 2, 0)),
-                                            ((14, 11, 1), (1, 1, 0), (3, 3, 0)), ((10, 8, 4), (1, 0, 1), (1, 0, 1))])
+                                            ((14, 11, 1), (1, 1, 0), (3, 3, 0)), ((10, 8, 4), (1, 0, 1), (1, 0, 1)),
+                                            ((12, 10, 3), (1, 1, 0), (2, 2, 0)), ((10, 12, 5), (1, 1, 0), (1, 1, 0)), ((14, 8, 6), (1, 0, 0), (2, 0, 0)),
+                                            ((8, 10, 7), (1, 1, 0), (1, 2, 0)), ((9, 7, 5), (1, 1, 1), (1, 1, 1))])
 def test_ddi_slab_path_matches_oracle_and_3d_path(P, O, cells, per, img):
     w = dataclasses.replace(W.config5().resized(cells, 20), periodic=per, ddi_images=img)
     g, o = pair(P, O, w)
+    assert g.spin_ddi_info().startswith("slab"), g.spin_ddi_info()
     Bo = o.effective_field()
     assert_fields_close(g.effective_field(), Bo)
     assert abs(g.energy()[1][5] - o.energy_terms()[5]) <= 1e-12 * np.abs(o.energy_terms()).sum()
@@ -343,10 +347,27 @@ def test_ddi_slab_path_matches_oracle_and_3d_path(P, O, cells, per, img):
     assert np.abs(g.spins_get() - o.spins()).max() <= SPIN_ATOL
 
 
+def test_ddi_slab_systems_of_different_thickness_alive_together(P, O):
+    """Two films of different thickness (4 and 8 planes, then 3 and 6) evaluated alternately in one process: the twiddle table of the
+    transform along c is a function of the padded length alone, so neither system disturbs the other (round-1 advisor finding)."""
+    for za, zb in [(4, 8), (3, 6), (8, 2)]:
+        wa = dataclasses.replace(W.config5().resized((12, 10, za), 4), ddi_images=(1, 1, 0))
+        wb = dataclasses.replace(W.config5().resized((10, 14, zb), 4), ddi_images=(2, 1, 0))
+        ga, oa = pair(P, O, wa)
+        gb, ob = pair(P, O, wb)
+        Ba, Bb = oa.effective_field(), ob.effective_field()
+        for _ in range(2):
+            assert_fields_close(ga.effective_field(), Ba)
+            assert_fields_close(gb.effective_field(), Bb)
+        ga.llg_iterate(4); gb.llg_iterate(4); oa.iterate(4); ob.iterate(4)
+        assert np.abs(ga.spins_get() - oa.spins()).max() <= SPIN_ATOL
+        assert np.abs(gb.spins_get() - ob.spins()).max() <= SPIN_ATOL
+
+
 # The slab contraction reads only PZ/2 + 1 of the PZ tensor planes when the spectrum is mirror symmetric along c (c perpendicular to the
 # film; checked numerically when the plan is built).  Tilted c: no symmetry, all planes are read; oblique a, b with c perpendicular: symmetric.
 @pytest.mark.parametrize("bravais", [[[1, 0, 0], [0, 1, 0], [0.3, 0.2, 1.0]], [[1, 0, 0], [0.5, 0.9, 0], [0, 0, 1.1]], [[1, 0, 0], [0, 1, 0], [0, 0, 1]]])
-@pytest.mark.parametrize("cells", [(14, 10, 4), (12, 10, 8), (10, 6, 2)])
+@pytest.mark.parametrize("cells", [(14, 10, 4), (12, 10, 8), (10, 6, 2), (10, 8, 5), (8, 10, 6)])
 def test_ddi_slab_mirror_symmetry_of_the_tensor(P, O, bravais, cells, monkeypatch):
     w = dataclasses.replace(W.config5().resized(cells, 10), bravais=np.array(bravais, float), periodic=(1, 1, 0), ddi_images=(2, 2, 0))
     g, o = pair(P, O, w)
