@@ -1207,7 +1207,7 @@ extern "C" int spin_set_option(spin_system *s, const char *name, int value) {
     else if (!strcmp(name, "use_pdl")) { s->opt_pdl = value > 2 ? -1 : value < 0 ? -1 : value; s->plan_dirty = true; }
     else if (!strcmp(name, "use_pair")) { s->opt_pair = value ? 1 : 0; s->plan_dirty = true; }
     else if (!strcmp(name, "use_col")) { s->opt_col = value ? 1 : 0; s->plan_dirty = true; }
-    else if (!strcmp(name, "ddi_slab")) { s->opt_ddi_slab = value ? 1 : 0; s->plan_dirty = true; }
+    else if (!strcmp(name, "ddi_slab")) { s->opt_ddi_slab = value < 0 ? 0 : (value > 2 ? 2 : value); s->plan_dirty = true; }      // 0: 3-D path, 1: slab path, 2: slab path with cuFFT's a-pass
     else if (!strcmp(name, "use_tma")) { s->opt_tma = value < 0 ? 0 : (value > 2 ? 2 : value); s->plan_dirty = true; }
     else return spin::fail(SPIN_ERR_ARG, "unknown option '%s'", name);
     drop_graphs(s);

@@ -14,6 +14,8 @@
 #include <stdlib.h>
 #include <string.h>
 
+#include <vector>
+
 #include "spinllg_internal.h"
 
 using namespace spin;
@@ -44,6 +46,10 @@ struct DdiState {
     double *s_in, *s_out;
     cufftDoubleComplex *s_a, *s_b, *s_d;
     double *d_Kre;             // [6][PZ][S2] real: the tensor spectrum is real for a single basis atom (the kernel is even)
+    bool own_a;                // the a-pass is ddi_apass_fwd / ddi_apass_inv (rows of power-of-two length) instead of scatter + cuFFT + gather
+    int a_rows_per_block;      // rows (warps) per block of those kernels
+    size_t a_smem;
+    double2 *d_tw;             // exp(-2 pi i t / P0), t < P0
     bool mirror;               // K(kz) = +-K(PZ - kz) (c perpendicular to the film): the contraction reads PZ/2 + 1 of the PZ planes
 };
 
@@ -164,6 +170,139 @@ __global__ void ddi_slab_gather_kernel(const __grid_constant__ DevicePlan L, con
     const int j = ((ic + L.LC) * L.PB + (ib + L.LB)) * (3 * L.PA) + (ia + L.LA);
 #pragma unroll
     for (int k = 0; k < 3; ++k) f[j + k * L.PA] = scale * out[((size_t)ib * SL + (k * L.Nc + ic)) * P0 + ia];
+}
+
+
+// ---------------------------------------------------------------------------------------------------------------------------
+// The a-pass of the slab path, hand-written for power-of-two rows ("FFTs ... power of two"): the padding scatter and the
+// transform along a are one kernel, the inverse transform and the field gather another.  A row holds Na real values followed by Na zeros
+// (P0 = 2 Na); its transform is taken as ONE complex transform of length M = P0 / 2 = Na of z(j) = x(2j) + i x(2j+1) (only j < M / 2 is
+// non-zero) followed by the usual split  X(k) = E(k) + W^k O(k),  E = (Z(k) + Z*(M-k)) / 2,  O = (Z(k) - Z*(M-k)) / (2i),  W = exp(-2 pi i / P0).
+// One warp per row; the complex transform is a Stockham autosort (radix 8, closed by one pass of radix 4 or 2) ping-ponging between two
+// padded shared-memory rows, the first twiddle of a butterfly from a table of exp(-2 pi i t / P0) in global memory.  Compared with scatter + cuFFT D2Z this reads the
+// spins once where they live (no padded real copy: 12.6 instead of 12.6 + 12.6 + 25.2 MB on cfg5) and launches one kernel instead of two.
+__device__ __forceinline__ double2 ddi_cadd(const double2 a, const double2 b) { return make_double2(a.x + b.x, a.y + b.y); }
+__device__ __forceinline__ double2 ddi_csub(const double2 a, const double2 b) { return make_double2(a.x - b.x, a.y - b.y); }
+__device__ __forceinline__ double2 ddi_cmul(const double2 a, const double2 b) { return make_double2(fma(a.x, b.x, -a.y * b.y), fma(a.x, b.y, a.y * b.x)); }
+// times -i (forward, SIGN < 0) or +i (inverse)
+template <int SIGN> __device__ __forceinline__ double2 ddi_rot90(const double2 a) { return SIGN < 0 ? make_double2(a.y, -a.x) : make_double2(-a.y, a.x); }
+// times exp(SIGN i pi / 4)
+template <int SIGN> __device__ __forceinline__ double2 ddi_rot45(const double2 a) {
+    const double h = 0.70710678118654752440;
+    return SIGN < 0 ? make_double2(h * (a.x + a.y), h * (a.y - a.x)) : make_double2(h * (a.x - a.y), h * (a.y + a.x));
+}
+// shared-memory rows are padded by one element in eight: the stores of the first passes (stride R elements between lanes) and the loads
+// (consecutive elements) are then both free of bank conflicts for 16-byte elements
+__device__ __forceinline__ int ddi_pad(const int i) { return i + (i >> 3); }
+
+// One warp, complex transform of length M (a power of two >= 8) as a Stockham autosort: passes of radix 8 (then one of radix 4 or 2),
+// ping-ponging between the padded rows a and b; returns the row that holds the result (natural order).  Twiddles exp(SIGN 2 pi i k r /
+// (Ns R)): the first power from the table tw[t] = exp(-2 pi i t / (2 M)), the others by multiplication (depth 3).
+template <int SIGN>      // -1 forward, +1 inverse (unnormalised)
+__device__ __forceinline__ double2 *ddi_warp_fft(double2 *a, double2 *b, const int M, const double2 *__restrict__ tw, const int lane) {
+    for (int Ns = 1; Ns < M;) {
+        const int rem = M / Ns;
+        const int R = (rem % 8 == 0) ? 8 : ((rem % 4 == 0) ? 4 : 2);
+        const int span = M / R, tstep = 2 * (M / (Ns * R));
+        for (int j = lane; j < span; j += 32) {
+            const int k = j & (Ns - 1), j0 = (j - k) * R + k;
+            double2 w1 = make_double2(1.0, 0.0);
+            if (k) { w1 = __ldg(tw + k * tstep); if (SIGN > 0) w1.y = -w1.y; }
+            if (R == 8) {
+                double2 v[8];
+#pragma unroll
+                for (int r = 0; r < 8; ++r) v[r] = a[ddi_pad(j + r * span)];
+                if (k) {
+                    const double2 w2 = ddi_cmul(w1, w1), w3 = ddi_cmul(w2, w1), w4 = ddi_cmul(w2, w2);
+                    v[1] = ddi_cmul(v[1], w1); v[2] = ddi_cmul(v[2], w2); v[3] = ddi_cmul(v[3], w3); v[4] = ddi_cmul(v[4], w4);
+                    v[5] = ddi_cmul(v[5], ddi_cmul(w4, w1)); v[6] = ddi_cmul(v[6], ddi_cmul(w3, w3)); v[7] = ddi_cmul(v[7], ddi_cmul(w4, w3));
+                }
+                // 8-point transform: three radix-2 stages, result in bit-reversed order
+                double2 t;
+                t = ddi_csub(v[0], v[4]); v[0] = ddi_cadd(v[0], v[4]); v[4] = t;
+                t = ddi_csub(v[1], v[5]); v[1] = ddi_cadd(v[1], v[5]); v[5] = ddi_rot45<SIGN>(t);
+                t = ddi_csub(v[2], v[6]); v[2] = ddi_cadd(v[2], v[6]); v[6] = ddi_rot90<SIGN>(t);
+                t = ddi_csub(v[3], v[7]); v[3] = ddi_cadd(v[3], v[7]); v[7] = ddi_rot90<SIGN>(ddi_rot45<SIGN>(t));
+#pragma unroll
+                for (int h = 0; h < 8; h += 4) {
+                    t = ddi_csub(v[h], v[h + 2]); v[h] = ddi_cadd(v[h], v[h + 2]); v[h + 2] = t;
+                    t = ddi_csub(v[h + 1], v[h + 3]); v[h + 1] = ddi_cadd(v[h + 1], v[h + 3]); v[h + 3] = ddi_rot90<SIGN>(t);
+                }
+#pragma unroll
+                for (int h = 0; h < 8; h += 2) { t = ddi_csub(v[h], v[h + 1]); v[h] = ddi_cadd(v[h], v[h + 1]); v[h + 1] = t; }
+                b[ddi_pad(j0)] = v[0]; b[ddi_pad(j0 + 4 * Ns)] = v[1]; b[ddi_pad(j0 + 2 * Ns)] = v[2]; b[ddi_pad(j0 + 6 * Ns)] = v[3];
+                b[ddi_pad(j0 + Ns)] = v[4]; b[ddi_pad(j0 + 5 * Ns)] = v[5]; b[ddi_pad(j0 + 3 * Ns)] = v[6]; b[ddi_pad(j0 + 7 * Ns)] = v[7];
+            } else if (R == 4) {
+                double2 v0 = a[ddi_pad(j)], v1 = a[ddi_pad(j + span)], v2 = a[ddi_pad(j + 2 * span)], v3 = a[ddi_pad(j + 3 * span)];
+                if (k) { const double2 w2 = ddi_cmul(w1, w1); v1 = ddi_cmul(v1, w1); v2 = ddi_cmul(v2, w2); v3 = ddi_cmul(v3, ddi_cmul(w2, w1)); }
+                const double2 t0 = ddi_cadd(v0, v2), t1 = ddi_csub(v0, v2), t2 = ddi_cadd(v1, v3), t3 = ddi_rot90<SIGN>(ddi_csub(v1, v3));
+                b[ddi_pad(j0)] = ddi_cadd(t0, t2); b[ddi_pad(j0 + Ns)] = ddi_cadd(t1, t3);
+                b[ddi_pad(j0 + 2 * Ns)] = ddi_csub(t0, t2); b[ddi_pad(j0 + 3 * Ns)] = ddi_csub(t1, t3);
+            } else {
+                const double2 v0 = a[ddi_pad(j)];
+                double2 v1 = a[ddi_pad(j + span)];
+                if (k) v1 = ddi_cmul(v1, w1);
+                b[ddi_pad(j0)] = ddi_cadd(v0, v1); b[ddi_pad(j0 + Ns)] = ddi_csub(v0, v1);
+            }
+        }
+        __syncwarp();
+        double2 *t = a; a = b; b = t;
+        Ns *= R;
+    }
+    return a;
+}
+
+// rows = Nb * SL occupied rows, row = ib SL + slab, slab = comp Nc + ic; out: element k of the row at row * S1p + k, k = 0 .. M
+__global__ void __launch_bounds__(256) ddi_apass_fwd_kernel(const __grid_constant__ DevicePlan L, const double *__restrict__ n, int M, int SL, int S1p, int rows,
+                                                            int rows_per_block, double mu, const double2 *__restrict__ tw, cufftDoubleComplex *__restrict__ out) {
+    extern __shared__ double2 ddi_sm[];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int row = blockIdx.x * rows_per_block + warp;
+    if (warp >= rows_per_block || row >= rows) return;
+    const int ib = row / SL, slab = row - ib * SL, comp = slab / L.Nc, ic = slab - comp * L.Nc;
+    const double2 *src = (const double2 *)(n + ((size_t)(ic + L.LC) * L.PB + (ib + L.LB)) * (3 * L.PA) + comp * L.PA + L.LA);
+    const int MP = M + (M >> 3);                        // padded row
+    double2 *a = ddi_sm + (size_t)warp * 2 * MP, *b = a + MP;
+    for (int j = lane; j < M; j += 32) {
+        double2 v = make_double2(0.0, 0.0);
+        if (j < M / 2) { v = __ldg(src + j); v.x *= mu; v.y *= mu; }
+        a[ddi_pad(j)] = v;
+    }
+    __syncwarp();
+    const double2 *Z = ddi_warp_fft<-1>(a, b, M, tw, lane);
+    cufftDoubleComplex *dst = out + (size_t)row * S1p;
+    for (int k = lane; k <= M; k += 32) {
+        const double2 zk = Z[ddi_pad(k & (M - 1))], zm = Z[ddi_pad((M - k) & (M - 1))];
+        const double er = 0.5 * (zk.x + zm.x), ei = 0.5 * (zk.y - zm.y);            // E = (Z(k) + conj Z(M-k)) / 2
+        const double orr = 0.5 * (zk.y + zm.y), oi = -0.5 * (zk.x - zm.x);          // O = (Z(k) - conj Z(M-k)) / (2i)
+        const double2 w = __ldg(tw + k);                                            // exp(-2 pi i k / P0)
+        dst[k] = make_cuDoubleComplex(er + fma(orr, w.x, -oi * w.y), ei + fma(orr, w.y, oi * w.x));
+    }
+}
+
+// inverse: from the half spectrum X(k), k = 0 .. M, of every occupied row to P0 x(ia), ia < Na, scaled and written as the dipolar force
+__global__ void __launch_bounds__(256) ddi_apass_inv_kernel(const __grid_constant__ DevicePlan L, const cufftDoubleComplex *__restrict__ in, int M, int SL, int S1p,
+                                                            int rows, int rows_per_block, double scale, const double2 *__restrict__ tw, double *__restrict__ f) {
+    extern __shared__ double2 ddi_sm[];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int row = blockIdx.x * rows_per_block + warp;
+    if (warp >= rows_per_block || row >= rows) return;
+    const int ib = row / SL, slab = row - ib * SL, comp = slab / L.Nc, ic = slab - comp * L.Nc;
+    const cufftDoubleComplex *src = in + (size_t)row * S1p;
+    const int MP = M + (M >> 3);
+    double2 *a = ddi_sm + (size_t)warp * 2 * MP, *b = a + MP;
+    for (int k = lane; k < M; k += 32) {
+        const cufftDoubleComplex xk = src[k], xm = src[M - k];
+        const double er = xk.x + xm.x, ei = xk.y - xm.y;                            // E = X(k) + conj X(M-k)
+        const double dr = xk.x - xm.x, di = xk.y + xm.y;                            // X(k) - conj X(M-k)
+        const double2 w = __ldg(tw + k);                                            // times exp(+2 pi i k / P0)
+        const double orr = fma(dr, w.x, di * w.y), oi = fma(di, w.x, -dr * w.y);
+        a[ddi_pad(k)] = make_double2(er - oi, ei + orr);                            // Z = E + i O
+    }
+    __syncwarp();
+    const double2 *z = ddi_warp_fft<+1>(a, b, M, tw, lane);
+    double2 *dst = (double2 *)(f + ((size_t)(ic + L.LC) * L.PB + (ib + L.LB)) * (3 * L.PA) + comp * L.PA + L.LA);
+    for (int j = lane; j < M / 2; j += 32) { const double2 v = z[ddi_pad(j)]; dst[j] = make_double2(scale * v.x, scale * v.y); }
 }
 
 // rank-0 case (a single cell): the "transform" of one point is the point itself
@@ -293,6 +432,17 @@ __global__ void __launch_bounds__(2 * DDI_CT_COLS, 4) ddi_slab_contract_kernel(c
     const size_t col = (size_t)kb * (3 * NZ) * S1p + ka;           // slab 0 of this wave vector; slabs are one row pitch apart
     double xr[3][NZ], xi[3][NZ];
     if (live) {
+        // the tensor planes of this thread are needed only after the forward transform, when no registers are left to hold them: ask L2
+        // for their lines now (one line per 16 threads), so that the loads below the transform find them there
+        if ((lane_col & 15) == 0) {
+#pragma unroll
+            for (int j = 0; j < NZ; ++j) {
+                const int kz = PAD ? 2 * j + e : 0;
+                if (MIRROR && 2 * kz > PZ) continue;
+#pragma unroll
+                for (int m = 0; m < 6; ++m) asm volatile("prefetch.global.L2 [%0];" ::"l"(Kre + ((size_t)m * PZ + kz) * S2 + q));
+            }
+        }
 #pragma unroll
         for (int c = 0; c < 3; ++c)
 #pragma unroll
@@ -400,6 +550,7 @@ const char *spin::ddi_path_name(const spin_system *s) {
     const DdiState *d = s->ddi;
     if (!s->ddi_on || !d) return "off";
     if (!d->slab) return "3d";
+    if (d->own_a) return d->mirror ? "slab+mirror+own-a" : "slab+own-a";
     return d->mirror ? "slab+mirror" : "slab";
 }
 
@@ -409,7 +560,7 @@ void spin::ddi_release(spin_system *s) {
     if (d->have_plans) { cufftDestroy(d->plan_r2c); cufftDestroy(d->plan_c2r); }
     if (d->slab) { cufftDestroy(d->plan_a_fwd); cufftDestroy(d->plan_a_inv); cufftDestroy(d->plan_b); }
     cudaFree(d->s_in); cudaFree(d->s_out); cudaFree(d->s_a); cudaFree(d->s_b); cudaFree(d->s_d);
-    cudaFree(d->d_Kre);
+    cudaFree(d->d_Kre); cudaFree(d->d_tw);
     cudaFree(d->d_Mpad); cudaFree(d->d_Hpad); cudaFree(d->d_Mhat); cudaFree(d->d_Hhat); cudaFree(d->d_Khat); cudaFree(d->d_geom);
     delete d;
     s->ddi = nullptr;
@@ -434,6 +585,9 @@ int spin::ddi_prepare(spin_system *s) {
     const bool want_slab = s->opt_ddi_slab && nb == 1 && d->P[0] > 1 && d->P[1] > 1 && d->NZ <= 8;
     size_t nreal = (size_t)nb * 3 * d->Ptot, ncplx = (size_t)nb * 3 * d->Phalf;
     d->SL = 3 * d->NZ; d->S1 = d->P[0] / 2 + 1; d->S1p = d->S1;      // a 128-byte row pitch (264) was measured slower: 368 vs 347 us per step on cfg5
+    // own a-pass: rows of power-of-two length, 8 <= Na <= 2048 (option ddi_slab = 2 keeps cuFFT's, for comparison)
+    const int Na = s->nc[0];
+    d->own_a = want_slab && s->opt_ddi_slab == 1 && Na >= 8 && Na <= 2048 && (Na & (Na - 1)) == 0;
     if (want_slab) {
         const size_t nr = (size_t)s->nc[1] * d->SL * d->P[0], nc_ = (size_t)d->P[1] * d->SL * d->S1p;
         SPIN_CUDA(cudaMalloc(&d->s_in, nr * sizeof(double)));
@@ -473,6 +627,27 @@ int spin::ddi_prepare(spin_system *s) {
             }
         SPIN_CUDA(cudaMemcpyToSymbolAsync(DDI_TWR, twr, sizeof(twr), 0, cudaMemcpyHostToDevice, s->stream));
         SPIN_CUDA(cudaMemcpyToSymbolAsync(DDI_TWI, twi, sizeof(twi), 0, cudaMemcpyHostToDevice, s->stream));
+        if (d->own_a) {
+            const int P0 = d->P[0];
+            std::vector<double2> tw((size_t)P0);
+            for (int t = 0; t < P0; ++t) {
+                tw[(size_t)t] = make_double2(cos(-2.0 * M_PI * t / P0), sin(-2.0 * M_PI * t / P0));
+                if ((8 * t) % P0 == 0) {      // exact at the multiples of an eighth of a turn
+                    const int k = (8 * t) / P0;
+                    const double h = 0.70710678118654752440;
+                    const double cr[8] = {1, h, 0, -h, -1, -h, 0, h}, ci[8] = {0, -h, -1, -h, 0, h, 1, h};
+                    tw[(size_t)t] = make_double2(cr[k], ci[k]);
+                }
+            }
+            SPIN_CUDA(cudaMalloc(&d->d_tw, (size_t)P0 * sizeof(double2)));
+            SPIN_CUDA(cudaMemcpyAsync(d->d_tw, tw.data(), (size_t)P0 * sizeof(double2), cudaMemcpyHostToDevice, s->stream));
+            SPIN_CUDA(cudaStreamSynchronize(s->stream));      // tw is a local
+            const int M = P0 / 2;
+            d->a_rows_per_block = M <= 256 ? 8 : (M <= 512 ? 4 : (M <= 1024 ? 2 : 1));
+            d->a_smem = (size_t)d->a_rows_per_block * 2 * (M + M / 8) * sizeof(double2);
+            SPIN_CUDA(cudaFuncSetAttribute(ddi_apass_fwd_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)d->a_smem));
+            SPIN_CUDA(cudaFuncSetAttribute(ddi_apass_inv_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)d->a_smem));
+        }
     }
     if (d->rank > 0) {
         if (!want_slab) {
@@ -536,8 +711,15 @@ int spin::ddi_field(spin_system *s, const double *d_n, double *d_f) {
     const unsigned gs = (unsigned)((nspin + nt - 1) / nt);
     if (d->slab) {
         const unsigned gcell = (unsigned)((Ncell + nt - 1) / nt);
-        ddi_slab_scatter_kernel<<<gcell, nt, 0, s->stream>>>(s->plan, d_n, d->P[0], d->SL, s->mu[0], d->s_in);
-        SPIN_FFT(cufftExecD2Z(d->plan_a_fwd, d->s_in, d->s_a));                       // a-pass over the occupied rows only
+        const int a_rows = s->nc[1] * d->SL;
+        const unsigned ga = d->own_a ? (unsigned)((a_rows + d->a_rows_per_block - 1) / d->a_rows_per_block) : 0u;
+        if (d->own_a) {                                                               // scatter + a-pass over the occupied rows, one kernel
+            ddi_apass_fwd_kernel<<<ga, 32 * d->a_rows_per_block, d->a_smem, s->stream>>>(s->plan, d_n, d->P[0] / 2, d->SL, d->S1p, a_rows, d->a_rows_per_block,
+                                                                                        s->mu[0], d->d_tw, d->s_a);
+        } else {
+            ddi_slab_scatter_kernel<<<gcell, nt, 0, s->stream>>>(s->plan, d_n, d->P[0], d->SL, s->mu[0], d->s_in);
+            SPIN_FFT(cufftExecD2Z(d->plan_a_fwd, d->s_in, d->s_a));                   // a-pass over the occupied rows only
+        }
         SPIN_FFT(cufftExecZ2Z(d->plan_b, d->s_a, d->s_b, CUFFT_FORWARD));            // b-pass
         const unsigned gq = (unsigned)((d->S2 + DDI_CT_COLS - 1) / DDI_CT_COLS);
 #define SPIN_CONTRACT(NZ_, PAD_, MIR_) ddi_slab_contract_kernel<NZ_, PAD_, MIR_><<<gq, 2 * DDI_CT_COLS, 0, s->stream>>>(d->d_Kre, d->s_b, d->s_b, (long long)d->S2, d->S1, d->S1p)
@@ -551,9 +733,15 @@ int spin::ddi_field(spin_system *s, const double *d_n, double *d_f) {
 #undef SPIN_CONTRACT_NZ
 #undef SPIN_CONTRACT
         SPIN_FFT(cufftExecZ2Z(d->plan_b, d->s_b, d->s_d, CUFFT_INVERSE));            // inverse b-pass
-        SPIN_FFT(cufftExecZ2D(d->plan_a_inv, d->s_d, d->s_out));                      // inverse a-pass, occupied rows only
-        ddi_slab_gather_kernel<<<gcell, nt, 0, s->stream>>>(s->plan, d->s_out, d->P[0], d->SL, s->mu[0] * C_DD / (double)d->Ptot, d_f);
-        s->n_launch += 3; s->n_fft += 4;
+        if (d->own_a) {                                                               // inverse a-pass + gather, one kernel
+            ddi_apass_inv_kernel<<<ga, 32 * d->a_rows_per_block, d->a_smem, s->stream>>>(s->plan, d->s_d, d->P[0] / 2, d->SL, d->S1p, a_rows, d->a_rows_per_block,
+                                                                                        s->mu[0] * C_DD / (double)d->Ptot, d->d_tw, d_f);
+            s->n_launch += 3; s->n_fft += 2;
+        } else {
+            SPIN_FFT(cufftExecZ2D(d->plan_a_inv, d->s_d, d->s_out));                  // inverse a-pass, occupied rows only
+            ddi_slab_gather_kernel<<<gcell, nt, 0, s->stream>>>(s->plan, d->s_out, d->P[0], d->SL, s->mu[0] * C_DD / (double)d->Ptot, d_f);
+            s->n_launch += 3; s->n_fft += 4;
+        }
         return SPIN_OK;
     }
     ddi_scatter_kernel<<<gs, nt, 0, s->stream>>>(s->plan, d_n, d->P[0], d->P[1], (long long)d->Ptot, d->d_geom, d->d_Mpad);
