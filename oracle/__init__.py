@@ -39,6 +39,7 @@ def lib():
         L.orc_threads.argtypes = [vp]
         L.orc_set_threads.argtypes = [vp, C.c_int]
         L.orc_set_mu_s.argtypes = [vp, dp]
+        L.orc_set_site_mu_s.argtypes = [vp, dp]
         L.orc_set_field.argtypes = [vp, C.c_double, dp]
         L.orc_set_anisotropy.argtypes = [vp, C.c_int, ip, dp, dp]
         L.orc_set_pairs.argtypes = [vp, C.c_int, ip, ip, ip, dp, dp]
@@ -147,6 +148,14 @@ class OracleSystem:
     def set_mu_s(self, mu):
         a, p = _d(np.broadcast_to(np.asarray(mu, float), (self.n_basis,)))
         lib().orc_set_mu_s(self._h, p)
+
+    def set_site_mu_s(self, mu_site):
+        """Per-site moments (PAPER.md:79 'atoms of different types'), N values in boundary order; None clears."""
+        if mu_site is None:
+            lib().orc_set_site_mu_s(self._h, None)
+            return
+        a, p = _d(np.asarray(mu_site, float).reshape(self.N))
+        lib().orc_set_site_mu_s(self._h, p)
 
     def set_field(self, B, direction):
         a, p = _d(direction)

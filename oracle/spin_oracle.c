@@ -68,6 +68,9 @@ typedef struct orc_system {
     double alat;             /* lattice constant, Angstrom                         */
     long ncell, N;
     double *mu;              /* nb, mu_B                                           */
+    double *mu_site;         /* N moments in boundary order or NULL: ":79 atoms of different types" -- a per-site moment that
+                                replaces the basis atom's wherever mu_i enters (Zeeman term and dipolar sum of Eq. 1, the 1/mu_i of
+                                Eq. 10, the thermal amplitude of Eq. 11, the conversion of the boundary to Tesla); reading R32  */
     double Bext[3];          /* Tesla                                              */
     double *K, *Kax;         /* legacy single-axis view (first entry per atom); the sums run over the entry list below */
     int nani; int *ab; double *aK, *aax;   /* anisotropy entries: basis atom, K, unit axis -- "sum_i sum_j K_j (K^_j . n_i)^2" (Eq. 1 :61)
@@ -90,6 +93,10 @@ typedef struct orc_system {
     int damping_only;        /* 1: the precession term of Eq. 10 is dropped (:168), the solvers become minimisers                */
     int solver;              /* 0 Depondt (App. B B5-B7), 1 Heun (B3-B4), 2 SIB semi-implicit midpoint (App. C), 3 RK4 (:168) */
 } orc_system;
+
+/* moment of spin i (mu_B): its own if per-site moments are set, else its basis atom's (i = b + nb * cell) */
+static inline double mu_at(const orc_system *s, long i) { return s->mu_site ? s->mu_site[i] : s->mu[i % s->nb]; }
+
 
 /* ------------------------------------------------------------------ helpers */
 static inline long cell_index(const orc_system *s, const int c[3]) {
@@ -159,7 +166,7 @@ void orc_destroy(orc_system *s) {
     if (!s) return;
     free(s->basis); free(s->mu); free(s->K); free(s->Kax); free(s->ab); free(s->aK); free(s->aax);
     free(s->pi); free(s->pj); free(s->pt); free(s->pJ); free(s->pD);
-    free(s->qb); free(s->qt); free(s->qK); free(s->Khat); free(s->n); free(s->pinned); free(s->vp_v); free(s->vp_F);
+    free(s->qb); free(s->qt); free(s->qK); free(s->Khat); free(s->n); free(s->pinned); free(s->mu_site); free(s->vp_v); free(s->vp_F);
     free(s);
 }
 long orc_nspins(const orc_system *s) { return s->N; }
@@ -173,6 +180,11 @@ void orc_set_threads(orc_system *s, int n) {
 #endif
 }
 void orc_set_mu_s(orc_system *s, const double *mu) { memcpy(s->mu, mu, s->nb * sizeof(double)); free(s->Khat); s->Khat = NULL; }
+/* per-site moments (":79 atoms of different types"), N values in boundary order; NULL goes back to the basis atoms' moments */
+void orc_set_site_mu_s(orc_system *s, const double *mu_site) {
+    free(s->mu_site); s->mu_site = NULL;
+    if (mu_site) { s->mu_site = (double *)malloc(s->N * sizeof(double)); memcpy(s->mu_site, mu_site, s->N * sizeof(double)); }
+}
 void orc_set_field(orc_system *s, double B, const double dir[3]) {
     double nrm = sqrt(dot3(dir, dir));
     for (int k = 0; k < 3; ++k) s->Bext[k] = (nrm > 0) ? B * dir[k] / nrm : 0.0;
@@ -246,7 +258,7 @@ void orc_energy(orc_system *s, const double *n, double E[6]) {
         cell_coords(s, cell, c);
         for (int b = 0; b < s->nb; ++b) {
             const double *ni = n + 3 * spin_index(s, c, b);
-            ez -= (long double)(s->mu[b] * ORC_MU_B * dot3(s->Bext, ni));
+            ez -= (long double)(mu_at(s, spin_index(s, c, b)) * ORC_MU_B * dot3(s->Bext, ni));
             for (int e = 0; e < s->nani; ++e) if (s->ab[e] == b) {
                 double p = dot3(s->aax + 3*e, ni);
                 ea -= (long double)(s->aK[e] * p * p);
@@ -301,7 +313,7 @@ double orc_energy_ddi_pairsum(const orc_system *s, const double *n) {
                 double r[3]; frac_to_cart(s, f, r);
                 double r2 = dot3(r, r), rn = sqrt(r2);
                 double rh[3] = { r[0]/rn, r[1]/rn, r[2]/rn };
-                e -= 0.5L * (long double)(ORC_C_DD * s->mu[a] * s->mu[b] *
+                e -= 0.5L * (long double)(ORC_C_DD * mu_at(s, spin_index(s, ci, a)) * mu_at(s, spin_index(s, cj, b)) *
                         (3.0 * dot3(ni, rh) * dot3(nj, rh) - dot3(ni, nj)) / (r2 * rn));
             }
         }
@@ -323,7 +335,7 @@ void orc_gradient_scatter(orc_system *s, const double *n, double *F, int mask) {
         cell_coords(s, cell, c);
         for (int b = 0; b < s->nb; ++b) {
             long i = spin_index(s, c, b);
-            if (mask & T_ZEE) for (int k = 0; k < 3; ++k) F[3*i+k] += s->mu[b] * ORC_MU_B * s->Bext[k];
+            if (mask & T_ZEE) for (int k = 0; k < 3; ++k) F[3*i+k] += mu_at(s, i) * ORC_MU_B * s->Bext[k];
             if (mask & T_ANI) for (int e = 0; e < s->nani; ++e) if (s->ab[e] == b) {
                 double p = dot3(s->aax + 3*e, n + 3*i);
                 for (int k = 0; k < 3; ++k) F[3*i+k] += 2.0 * s->aK[e] * p * s->aax[3*e+k];
@@ -378,7 +390,7 @@ static void gather_one(const orc_system *s, const double *n, long cell, int b, i
     cell_coords(s, cell, c);
     const double *ni = n + 3 * spin_index(s, c, b);
     F[0] = F[1] = F[2] = 0.0;
-    if (mask & T_ZEE) for (int k = 0; k < 3; ++k) F[k] += s->mu[b] * ORC_MU_B * s->Bext[k];
+    if (mask & T_ZEE) for (int k = 0; k < 3; ++k) F[k] += mu_at(s, spin_index(s, c, b)) * ORC_MU_B * s->Bext[k];
     if (mask & T_ANI) for (int e = 0; e < s->nani; ++e) if (s->ab[e] == b) {
         double p = dot3(s->aax + 3*e, ni);
         for (int k = 0; k < 3; ++k) F[k] += 2.0 * s->aK[e] * p * s->aax[3*e+k];
@@ -425,7 +437,7 @@ static void gather_one(const orc_system *s, const double *n, long cell, int b, i
 }
 
 void orc_gradient(orc_system *s, const double *n, double *F, int mask) {
-    long N = s->N; int nb = s->nb;
+    long N = s->N; int nb = s->nb; (void)nb;
 #pragma omp parallel for schedule(static) num_threads(s->nthreads)
     for (long i = 0; i < N; ++i) gather_one(s, n, i / nb, (int)(i % nb), mask, F + 3*i);
     if ((mask & T_DDI) && s->ddi) {
@@ -441,7 +453,7 @@ void orc_gradient(orc_system *s, const double *n, double *F, int mask) {
  * Images: t_d in [-nimg_d, nimg_d] in periodic directions, 0 in open ones (reading R16);
  * self images (i == j, t != 0) are included.                                              */
 void orc_ddi_direct(const orc_system *s, const double *n, double *F) {
-    long N = s->N; int nb = s->nb;
+    long N = s->N; int nb = s->nb; (void)nb;
     int lim[3]; for (int d = 0; d < 3; ++d) lim[d] = s->per[d] ? s->nimg[d] : 0;
 #pragma omp parallel for schedule(static) num_threads(s->nthreads)
     for (long i = 0; i < N; ++i) {
@@ -460,11 +472,11 @@ void orc_ddi_direct(const orc_system *s, const double *n, double *F) {
                 double r[3]; frac_to_cart(s, f, r);
                 double r2 = dot3(r, r), rn = sqrt(r2);
                 double rh[3] = { r[0]/rn, r[1]/rn, r[2]/rn };
-                double p = dot3(nj, rh), w = s->mu[b] / (r2 * rn);
+                double p = dot3(nj, rh), w = mu_at(s, j) / (r2 * rn);
                 for (int k = 0; k < 3; ++k) acc[k] += w * (3.0 * rh[k] * p - nj[k]);
             }
         }
-        for (int k = 0; k < 3; ++k) F[3*i+k] = s->mu[a] * ORC_C_DD * acc[k];
+        for (int k = 0; k < 3; ++k) F[3*i+k] = mu_at(s, i) * ORC_C_DD * acc[k];
     }
 }
 
@@ -599,7 +611,7 @@ void orc_ddi_fft(orc_system *s, const double *n, double *F) {
         cell_coords(s, cell, c);
         long pidx = c[0] + (long)s->P[0] * (c[1] + (long)s->P[1] * c[2]);
         for (int b = 0; b < nb; ++b) for (int k = 0; k < 3; ++k)
-            M[2 * ((size_t)(b * 3 + k) * Pt + pidx)] = s->mu[b] * n[3 * spin_index(s, c, b) + k];
+            M[2 * ((size_t)(b * 3 + k) * Pt + pidx)] = mu_at(s, spin_index(s, c, b)) * n[3 * spin_index(s, c, b) + k];
     }
     for (int b = 0; b < nb; ++b) for (int k = 0; k < 3; ++k) fft3d(M + 2 * (size_t)(b * 3 + k) * Pt, s->P, -1, s->nthreads);
     for (int a = 0; a < nb; ++a) {
@@ -627,7 +639,7 @@ void orc_ddi_fft(orc_system *s, const double *n, double *F) {
             cell_coords(s, cell, c);
             long pidx = c[0] + (long)s->P[0] * (c[1] + (long)s->P[1] * c[2]);
             for (int k = 0; k < 3; ++k)
-                F[3 * spin_index(s, c, a) + k] = s->mu[a] * ORC_C_DD * H[2 * ((size_t)k * Pt + pidx)] / (double)Pt;
+                F[3 * spin_index(s, c, a) + k] = mu_at(s, spin_index(s, c, a)) * ORC_C_DD * H[2 * ((size_t)k * Pt + pidx)] / (double)Pt;
         }
     }
     free(M); free(H);
@@ -675,6 +687,10 @@ void orc_thermal_xi(uint64_t seed, uint64_t step, uint32_t spin, double xi[3]) {
 double orc_thermal_sigma(const orc_system *s, int b) {
     return sqrt(2.0 * s->alpha * ORC_K_B * s->T * s->mu[b] * ORC_MU_B / (ORC_GAMMA * s->dt));
 }
+/* the same for spin i, with its own moment when per-site moments are set */
+static double thermal_sigma_site(const orc_system *s, long i) {
+    return sqrt(2.0 * s->alpha * ORC_K_B * s->T * mu_at(s, i) * ORC_MU_B / (ORC_GAMMA * s->dt));
+}
 
 /* ------------------------------------------------------------------ (j_e . grad) n on the lattice (reading R14)
  * j^ is expanded in the Bravais vectors of the directions with more than one cell
@@ -715,7 +731,7 @@ static void stt_coeffs(const orc_system *s, double cd[3]) {
 }
 void orc_stt_gradient(orc_system *s, const double *n, double *sg) {
     double cd[3]; stt_coeffs(s, cd);
-    long N = s->N; int nb = s->nb;
+    long N = s->N; int nb = s->nb; (void)nb;
 #pragma omp parallel for schedule(static) num_threads(s->nthreads)
     for (long i = 0; i < N; ++i) {
         int c[3], cp[3], cm[3]; cell_coords(s, i / nb, c); int b = (int)(i % nb);
@@ -737,10 +753,10 @@ void orc_stt_gradient(orc_system *s, const double *n, double *sg) {
 /* ------------------------------------------------------------------ Eq. 10 as dn/dt = n x A (B1)
  * A = -gamma/((1+alpha^2) mu) [F + alpha n x F] + u/(1+alpha^2) [-(alpha-beta) s + (1+alpha beta) n x s]
  * with F in meV (incl. thermal), mu = mu_s mu_B in meV/T, s = (j^.grad) n in 1/Angstrom, u in A/ps. */
-static inline void rot_field(const orc_system *s, int b, const double *n, const double *F, const double *sg, double *A) {
+static inline void rot_field(const orc_system *s, long i, const double *n, const double *F, const double *sg, double *A) {
     double nxF[3], nxs[3] = {0, 0, 0};
     cross3(n, F, nxF);
-    double pre = -ORC_GAMMA / ((1.0 + s->alpha * s->alpha) * s->mu[b] * ORC_MU_B);
+    double pre = -ORC_GAMMA / ((1.0 + s->alpha * s->alpha) * mu_at(s, i) * ORC_MU_B);
     double us = s->u / (1.0 + s->alpha * s->alpha);
     if (s->u != 0.0) cross3(n, sg, nxs);
     for (int k = 0; k < 3; ++k) {
@@ -796,7 +812,7 @@ static inline void imp_update(const double *A, double dt, const double *n, doubl
 static void orc_rk4_step(orc_system *s);
 void orc_llg_step(orc_system *s) {
     if (s->solver == 3) { orc_rk4_step(s); return; }
-    long N = s->N; int nb = s->nb;
+    long N = s->N; int nb = s->nb; (void)nb;
     double *F = (double *)malloc(3 * N * sizeof(double)), *A = (double *)malloc(3 * N * sizeof(double));
     double *np_ = (double *)malloc(3 * N * sizeof(double)), *sg = (double *)calloc(3 * N, sizeof(double));
     double *Fth = NULL;
@@ -805,7 +821,7 @@ void orc_llg_step(orc_system *s) {
 #pragma omp parallel for schedule(static) num_threads(s->nthreads)
         for (long i = 0; i < N; ++i) {
             double xi[3]; orc_thermal_xi_image(s->seed, s->step, (uint32_t)i, s->image, xi);
-            double sig = orc_thermal_sigma(s, (int)(i % nb));
+            double sig = thermal_sigma_site(s, i);
             for (int k = 0; k < 3; ++k) Fth[3*i+k] = sig * xi[k];
         }
     }
@@ -813,7 +829,7 @@ void orc_llg_step(orc_system *s) {
     if (s->u != 0.0) orc_stt_gradient(s, s->n, sg);
 #pragma omp parallel for schedule(static) num_threads(s->nthreads)
     for (long i = 0; i < N; ++i) {
-        rot_field(s, (int)(i % nb), s->n + 3*i, F + 3*i, sg + 3*i, A + 3*i);
+        rot_field(s, i, s->n + 3*i, F + 3*i, sg + 3*i, A + 3*i);
         if (s->pinned && s->pinned[i]) { for (int k = 0; k < 3; ++k) np_[3*i+k] = s->n[3*i+k]; continue; }   /* pinned: n^p = n */
         if (s->solver == 0) rotate(A + 3*i, s->dt, s->n + 3*i, np_ + 3*i);                       /* B5 */
         else if (s->solver == 1) {                                                               /* B3 */
@@ -830,7 +846,7 @@ void orc_llg_step(orc_system *s) {
     for (long i = 0; i < N; ++i) {
         double Ap[3], Ac[3], out[3];
         if (s->pinned && s->pinned[i]) continue;                               /* pinned: n_i(t+dt) = n_i(t) */
-        rot_field(s, (int)(i % nb), second + 3*i, F + 3*i, sg + 3*i, Ap);
+        rot_field(s, i, second + 3*i, F + 3*i, sg + 3*i, Ap);
         if (s->solver == 0) {
             for (int k = 0; k < 3; ++k) Ac[k] = 0.5 * (A[3*i+k] + Ap[k]);     /* B6 */
             rotate(Ac, s->dt, s->n + 3*i, out);                               /* B7 */
@@ -852,14 +868,14 @@ void orc_llg_step(orc_system *s) {
  * n <- n + dt/6 (k1 + 2 k2 + 2 k3 + k4), renormalised every step ("all [Runge-Kutta methods] have this property", :367).
  * The stage configurations are not renormalised; the thermal field of the step is the same in all four stages (R11).    */
 static void orc_rk4_step(orc_system *s) {
-    long N = s->N; int nb = s->nb;
+    long N = s->N; int nb = s->nb; (void)nb;
     double *F = (double *)malloc(3 * N * sizeof(double)), *y = (double *)malloc(3 * N * sizeof(double));
     double *acc = (double *)calloc(3 * N, sizeof(double)), *sg = (double *)calloc(3 * N, sizeof(double)), *Fth = NULL;
     if (s->T > 0.0) {
         Fth = (double *)malloc(3 * N * sizeof(double));
         for (long i = 0; i < N; ++i) {
             double xi[3]; orc_thermal_xi_image(s->seed, s->step, (uint32_t)i, s->image, xi);
-            double sig = orc_thermal_sigma(s, (int)(i % nb));
+            double sig = thermal_sigma_site(s, i);
             for (int k = 0; k < 3; ++k) Fth[3*i+k] = sig * xi[k];
         }
     }
@@ -870,7 +886,7 @@ static void orc_rk4_step(orc_system *s) {
         if (s->u != 0.0) orc_stt_gradient(s, y, sg);
         for (long i = 0; i < N; ++i) {
             double A[3], k[3];
-            rot_field(s, (int)(i % nb), y + 3*i, F + 3*i, sg + 3*i, A);
+            rot_field(s, i, y + 3*i, F + 3*i, sg + 3*i, A);
             cross3(y + 3*i, A, k);
             for (int c = 0; c < 3; ++c) acc[3*i+c] += wacc[st] * k[c];
             if (s->pinned && s->pinned[i]) continue;
@@ -892,19 +908,19 @@ void orc_llg_iterate(orc_system *s, long nsteps) { for (long k = 0; k < nsteps; 
 /* Heun's method, B3-B4 with f = n x A, renormalised every step.  Only used to pin Fig. 5's
  * "Heun within 1e-6 / Depondt 3e-7" statement; no thermal field, no current.                */
 void orc_heun_step(orc_system *s) {
-    long N = s->N; int nb = s->nb;
+    long N = s->N; int nb = s->nb; (void)nb;
     double *F = (double *)malloc(3 * N * sizeof(double)), *f0 = (double *)malloc(3 * N * sizeof(double));
     double *np_ = (double *)malloc(3 * N * sizeof(double)), *sg = (double *)calloc(3 * N, sizeof(double));
     total_force(s, s->n, NULL, F);
     for (long i = 0; i < N; ++i) {
-        double A[3]; rot_field(s, (int)(i % nb), s->n + 3*i, F + 3*i, sg + 3*i, A);
+        double A[3]; rot_field(s, i, s->n + 3*i, F + 3*i, sg + 3*i, A);
         cross3(s->n + 3*i, A, f0 + 3*i);
         for (int k = 0; k < 3; ++k) np_[3*i+k] = s->n[3*i+k] + s->dt * f0[3*i+k];
     }
     total_force(s, np_, NULL, F);
     for (long i = 0; i < N; ++i) {
         double A[3], f1[3], out[3];
-        rot_field(s, (int)(i % nb), np_ + 3*i, F + 3*i, sg + 3*i, A);
+        rot_field(s, i, np_ + 3*i, F + 3*i, sg + 3*i, A);
         cross3(np_ + 3*i, A, f1);
         for (int k = 0; k < 3; ++k) out[k] = s->n[3*i+k] + 0.5 * s->dt * (f0[3*i+k] + f1[k]);
         double nrm = sqrt(dot3(out, out));
@@ -925,7 +941,7 @@ void orc_heun_step(orc_system *s) {
  * The first iteration starts from v = 0 and F(t) = F(t+dt).  Pinned spins do not move and carry no force.            */
 void orc_vp_reset(orc_system *s) { free(s->vp_v); free(s->vp_F); s->vp_v = NULL; s->vp_F = NULL; }
 void orc_vp_iterate(orc_system *s, long n_iter, double dt, double mass) {
-    long N = s->N;
+    long N = s->N; int nb = s->nb; (void)nb;
     double *F = (double *)malloc(3 * N * sizeof(double));
     for (long it = 0; it < n_iter; ++it) {
         orc_gradient(s, s->n, F, T_ALL);
@@ -981,7 +997,7 @@ static double geodesic_distance(long N, const double *a, const double *b) {
 }
 double orc_geodesic_distance(const orc_system *s, const double *a, const double *b) { return geodesic_distance(s->N, a, b); }
 void orc_gneb_forces(orc_system *s, int M, const double *chain, double kappa, int climbing, double *F_out, double *E_out, double *l_out) {
-    long N = s->N;
+    long N = s->N; int nb = s->nb; (void)nb;
     double *E = (double *)malloc(M * sizeof(double)), *l = (double *)calloc(M, sizeof(double));
     double *G = (double *)malloc(3 * N * sizeof(double)), *tau = (double *)malloc(3 * N * sizeof(double));
     for (int nu = 0; nu < M; ++nu) {
@@ -1030,7 +1046,7 @@ void orc_gneb_forces(orc_system *s, int M, const double *chain, double kappa, in
 }
 /* one relaxation step of the chain: x <- x + step F, renormalised (plain steepest descent; the paper does not fix the optimiser) */
 void orc_gneb_iterate(orc_system *s, int M, double *chain, long n_iter, double step, double kappa, int climbing) {
-    long N = s->N;
+    long N = s->N; int nb = s->nb; (void)nb;
     double *F = (double *)malloc((size_t)M * 3 * N * sizeof(double));
     for (long it = 0; it < n_iter; ++it) {
         orc_gneb_forces(s, M, chain, kappa, climbing, F, NULL, NULL);
@@ -1092,7 +1108,7 @@ double orc_topological_charge(const orc_system *s, const double *n) {
 void orc_effective_field(orc_system *s, double *B) {
     orc_gradient(s, s->n, B, T_ALL);
     for (long i = 0; i < s->N; ++i) {
-        double m = s->mu[i % s->nb] * ORC_MU_B;
+        double m = mu_at(s, i) * ORC_MU_B;
         for (int k = 0; k < 3; ++k) B[3*i+k] /= m;
     }
 }

@@ -544,7 +544,7 @@ extern "C" int spin_geometry_create(const double bravais[9], int n_basis, const 
     s->opt_graph = 1; s->opt_store_A = 0; s->graph_exec[0] = s->graph_exec[1] = nullptr; s->graph_steps = 0;
     s->n_launch = s->n_fft = 0; s->profile_on = 0;
     for (int k = 0; k < 3; ++k) { s->prof_ms[k] = 0; s->prof_n[k] = 0; }
-    s->ev0 = s->ev1 = nullptr;
+    s->ev0 = s->ev1 = s->ev2 = s->ev3 = nullptr;
     const Launch L = brick_launch(s);
     memset(&s->plan, 0, sizeof(s->plan));
     if (!has_device) { *out = s; return SPIN_OK; }
@@ -559,6 +559,8 @@ extern "C" int spin_geometry_create(const double bravais[9], int n_basis, const 
     if (e == cudaSuccess) e = cudaMemset(s->d_step, 0, sizeof(unsigned long long));
     if (e == cudaSuccess) e = cudaEventCreate(&s->ev0);
     if (e == cudaSuccess) e = cudaEventCreate(&s->ev1);
+    if (e == cudaSuccess) e = cudaEventCreate(&s->ev2);
+    if (e == cudaSuccess) e = cudaEventCreate(&s->ev3);
     if (e == cudaSuccess) e = cudaDeviceSynchronize();
     if (e != cudaSuccess) {
         const int code = (e == cudaErrorMemoryAllocation) ? SPIN_ERR_MEMORY : SPIN_ERR_CUDA;
@@ -589,6 +591,8 @@ extern "C" void spin_system_destroy(spin_system *s) {
     cudaFree(s->d_aos); cudaFree(s->d_partials); cudaFree(s->d_result); cudaFree(s->d_step);
     if (s->ev0) cudaEventDestroy(s->ev0);
     if (s->ev1) cudaEventDestroy(s->ev1);
+    if (s->ev2) cudaEventDestroy(s->ev2);
+    if (s->ev3) cudaEventDestroy(s->ev3);
     delete s;
 }
 

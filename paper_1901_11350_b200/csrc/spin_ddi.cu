@@ -724,6 +724,7 @@ int spin::ddi_field(spin_system *s, const double *d_n, double *d_f) {
         const unsigned gq = (unsigned)((d->S2 + DDI_CT_COLS - 1) / DDI_CT_COLS);
 #define SPIN_CONTRACT(NZ_, PAD_, MIR_) ddi_slab_contract_kernel<NZ_, PAD_, MIR_><<<gq, 2 * DDI_CT_COLS, 0, s->stream>>>(d->d_Kre, d->s_b, d->s_b, (long long)d->S2, d->S1, d->S1p)
 #define SPIN_CONTRACT_NZ(NZ_) case NZ_: if (d->mirror) SPIN_CONTRACT(NZ_, true, true); else SPIN_CONTRACT(NZ_, true, false); break
+        if (s->profile_on) cudaEventRecord(s->ev2, s->stream);
         if (d->PZ == 1) SPIN_CONTRACT(1, false, false);                                 // a single unpadded plane: contraction only
         else switch (d->NZ) {                                                           // c-pass + contraction + inverse c-pass, in place
             SPIN_CONTRACT_NZ(1); SPIN_CONTRACT_NZ(2); SPIN_CONTRACT_NZ(3); SPIN_CONTRACT_NZ(4);
@@ -732,6 +733,11 @@ int spin::ddi_field(spin_system *s, const double *d_n, double *d_f) {
         }
 #undef SPIN_CONTRACT_NZ
 #undef SPIN_CONTRACT
+        if (s->profile_on) {      // the contraction alone (bench.py's roofline kernel on dipolar workloads)
+            cudaEventRecord(s->ev3, s->stream); cudaEventSynchronize(s->ev3);
+            float ms = 0.f; cudaEventElapsedTime(&ms, s->ev2, s->ev3);
+            s->prof_ms[3] += ms; s->prof_n[3]++;
+        }
         SPIN_FFT(cufftExecZ2Z(d->plan_b, d->s_b, d->s_d, CUFFT_INVERSE));            // inverse b-pass
         if (d->own_a) {                                                               // inverse a-pass + gather, one kernel
             ddi_apass_inv_kernel<<<ga, 32 * d->a_rows_per_block, d->a_smem, s->stream>>>(s->plan, d->s_d, d->P[0] / 2, d->SL, d->S1p, a_rows, d->a_rows_per_block,

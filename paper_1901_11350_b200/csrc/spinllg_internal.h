@@ -151,8 +151,9 @@ struct spin_system {
     int graph_steps;
     int64_t n_launch, n_fft;
     int profile_on;
-    double prof_ms[3];
-    int64_t prof_n[3];
+    double prof_ms[4];             // predictor, corrector, dipolar evaluation (whole), dipolar contraction kernel alone
+    int64_t prof_n[4];
+    cudaEvent_t ev2, ev3;          // around the dipolar contraction kernel (inside the evaluation that ev0/ev1 bracket)
     cudaEvent_t ev0, ev1;
 };
 

@@ -890,3 +890,86 @@ def test_observables_magnetisation_and_max_torque_closed_forms():
     expect = max(np.linalg.norm(np.cross(n[i], F[i])) for i in range(s.N))
     M2, tq2 = s.observables()
     assert tq2 == pytest.approx(expect, rel=1e-13) and np.array_equal(M, M2)
+
+
+# ------------------------------------------------------------------ atoms of different types: per-site moments (reading R32)
+def test_site_moments_zeeman_energy_and_larmor_frequency():
+    """A chain of free spins of two species (mu = 1.5 and 4 mu_B, alternating along the chain although the basis has one atom) in a field:
+    E = -sum_i mu_i mu_B B . n_i (Eq. 1 :61) depends on the moments; the effective field in Tesla and the whole trajectory (Eq. 12: the
+    precession and damping rates are gamma' B and alpha gamma' B, the moment cancels between Eq. 1 and the 1/mu_i of Eq. 10) do not."""
+    N = 6
+    s = OracleSystem(np.eye(3), [[0, 0, 0]], (N, 1, 1), (0, 0, 0))
+    s.set_mu_s([2.0]); s.set_field(1.3, (0, 0, 1))
+    mu = np.array([1.5, 4.0] * 3)
+    s.set_site_mu_s(mu)
+    n0 = rand_spins(N, 4)
+    s.set_spins(n0)
+    assert s.energy_terms()[0] == pytest.approx(-(mu * O.MU_B * 1.3 * n0[:, 2]).sum(), rel=1e-14)
+    assert np.allclose(s.gradient(), (mu * O.MU_B * 1.3)[:, None] * [0, 0, 1], rtol=1e-15)
+    assert np.allclose(s.effective_field(), [0.0, 0.0, 1.3], rtol=0, atol=1e-15)
+    s.llg_configure(10.0, 0.1)
+    s.iterate(500)
+    alpha, t = 0.1, 5.0
+    gp = O.GAMMA / (1 + alpha * alpha)
+    nz = np.tanh(alpha * gp * 1.3 * t + np.arctanh(n0[:, 2]))
+    assert np.abs(s.spins()[:, 2] - nz).max() < 5e-7                      # both species follow Eq. 12
+    r = OracleSystem(np.eye(3), [[0, 0, 0]], (N, 1, 1), (0, 0, 0))       # the same chain with one species
+    r.set_mu_s([2.0]); r.set_field(1.3, (0, 0, 1)); r.llg_configure(10.0, 0.1); r.set_spins(n0); r.iterate(500)
+    assert np.abs(s.spins() - r.spins()).max() < 1e-12
+    s.set_site_mu_s(None)                                                 # cleared: the basis atom's moment again
+    s.set_spins(n0)
+    assert s.energy_terms()[0] == pytest.approx(-(2.0 * O.MU_B * 1.3 * n0[:, 2]).sum(), rel=1e-14)
+
+
+def test_site_moments_in_the_exchange_field_and_the_dipolar_sum():
+    """(i) A bond J between two sites of different moment: the field ON site i in Tesla is J n_j / (mu_i mu_B), so with a field the
+    precession rates of the two species differ.  (ii) Two dipoles mu_1 != mu_2 head to tail at distance r: E = -2 C_dd mu_1 mu_2 / r^3,
+    force on each C_dd mu_1 mu_2 2 / r^3 along the axis (the product of BOTH moments).  (iii) the padded-FFT path equals the direct sum
+    with per-site moments on a periodic lattice."""
+    s = OracleSystem(np.eye(3), [[0, 0, 0]], (2, 1, 1), (0, 0, 0))
+    s.set_mu_s([1.0]); s.set_site_mu_s([2.0, 5.0])
+    s.set_pairs([0], [0], [[1, 0, 0]], [0.7])
+    s.set_spins([[0, 0, 1.0], [1.0, 0, 0]])
+    B = s.effective_field()
+    assert np.allclose(B[0], np.array([0.7, 0, 0]) / (2.0 * O.MU_B), rtol=1e-15)
+    assert np.allclose(B[1], np.array([0, 0, 0.7]) / (5.0 * O.MU_B), rtol=1e-15)
+    d = OracleSystem(np.eye(3), [[0, 0, 0]], (2, 1, 1), (0, 0, 0), 2.0)
+    d.set_mu_s([1.0]); d.set_site_mu_s([2.0, 5.0]); d.set_ddi(True, (0, 0, 0), direct=True)
+    n = np.array([[1.0, 0, 0], [1.0, 0, 0]])
+    d.set_spins(n)
+    r3 = 8.0
+    assert d.energy_terms()[5] == pytest.approx(-2 * O.C_DD * 10.0 / r3, rel=1e-14)
+    assert d.energy_ddi_pairsum() == pytest.approx(-2 * O.C_DD * 10.0 / r3, rel=1e-14)
+    assert np.allclose(d.ddi_field(direct=True), [[2 * O.C_DD * 10.0 / r3, 0, 0]] * 2, rtol=1e-14)
+    assert np.allclose(d.ddi_field(direct=False), d.ddi_field(direct=True), rtol=1e-13)
+    p = OracleSystem([[1, 0, 0], [0.3, 0.9, 0], [0, 0.1, 1.2]], [[0, 0, 0], [0.4, 0.3, 0.2]], (4, 3, 2), (1, 1, 0), 1.1)
+    p.set_mu_s([1.0, 2.0]); p.set_ddi(True, (2, 1, 0))
+    mu = np.random.default_rng(5).uniform(0.5, 3.0, p.N)
+    p.set_site_mu_s(mu)
+    nn = rand_spins(p.N, 6)
+    Ff, Fd = p.ddi_field(nn, direct=False), p.ddi_field(nn, direct=True)
+    assert np.abs(Ff - Fd).max() <= 1e-13 * np.abs(Fd).max()
+    # Euler identity with per-site moments: E_ddi = -(1/2) sum n . F_ddi
+    p.set_spins(nn)
+    assert p.energy_terms()[5] == pytest.approx(-0.5 * (nn * Fd).sum(), rel=1e-12)
+
+
+def test_site_moments_set_the_thermal_amplitude():
+    """Eq. 11 (:157): sigma_i = sqrt(2 alpha k_B T mu_i mu_B / (gamma dt)).  Two decoupled species in the same field at the same temperature
+    equilibrate to their own Langevin magnetisation coth(x_i) - 1/x_i, x_i = mu_i mu_B B / (k_B T)."""
+    B, T, alpha = 30.0, 20.0, 0.5
+    s = OracleSystem(np.eye(3), [[0, 0, 0]], (48, 40, 1), (0, 0, 0))
+    s.set_mu_s([1.0]); s.set_field(B, (0, 0, 1)); s.llg_configure(5.0, alpha, T=T, seed=12)
+    mu = np.where(np.arange(s.N) % 2 == 0, 1.0, 3.0)
+    s.set_site_mu_s(mu)
+    s.set_spins(rand_spins(s.N, 2))
+    s.iterate(800)
+    acc = [[], []]
+    for _ in range(60):
+        s.iterate(40)
+        nz = s.spins()[:, 2]
+        acc[0].append(nz[0::2].mean()); acc[1].append(nz[1::2].mean())
+    for k, m in enumerate((1.0, 3.0)):
+        x = m * O.MU_B * B / (O.K_B * T)
+        L = 1 / math.tanh(x) - 1 / x
+        assert abs(float(np.mean(acc[k])) - L) < 0.012, (m, np.mean(acc[k]), L)
