@@ -176,44 +176,41 @@ int observables(spin_system *sys, double M[3], double *max_torque_meV);
  * One basis atom (SPIN_ERR_ARG otherwise).  Periodic directions wrap; triangles leaving an open edge are skipped (:343).  */
 int topological_charge(spin_system *sys, double *Q);
 
-/* ---- introspection (measurement support) -------------------------------------------------------------- */
+/* ---- execution options ------------------------------------------------------------------------------------------------
+ * spin_set_option(name, value) changes how the path is executed, never what it computes (every combination is bit-identical; tested).
+ * The defaults are the measured choices; the options exist for A/B measurements and for the tests.
+ *   use_jit     (1)  the sweeps are specialised per system at run time with NVRTC -- lattice extents, gather tables and prefactors become
+ *                    compile-time constants; 0: the table-driven kernels (also taken, with the reason kept, when NVRTC is unavailable)
+ *   use_graph   (1)  16 steps are captured once into a CUDA graph and replayed (no host work per step)
+ *   use_coop    (1)  lattices of up to 4096 spins without dipolar coupling run ALL steps of an llg_iterate call in one launch: as one
+ *                    thread-block cluster with its hardware barrier between the sweeps (up to 16 bricks), else as a cooperative launch
+ *                    with a grid barrier; 2 forces the path for any size, 3 forces the grid barrier, 0 switches it off
+ *   use_pdl     (-1) programmatic dependent launch of the brick sweeps (griddepcontrol.wait inside the kernel): -1 automatic, 0 off,
+ *                    1 dependents released at entry, 2 at the end of each block
+ *   store_A     (0)  1: the predictor stores the rotation field A(n) and the corrector reads it instead of recomputing it
+ *   cache_noise (1)  the predictor keeps the thermal field of the step (24 B/spin) for the corrector instead of generating it twice
+ *   ddi_slab    (1)  thin films with one basis atom take the dipolar slab path; 2: the same with cuFFT's transform along a instead of
+ *                    the hand-written one; 0: the general 3-D transform
+ *   ddi_mirror  (1)  the slab contraction reads PZ/2 + 1 tensor planes when the spectrum is mirror symmetric along c; 0: all PZ planes    */
+int spin_set_option(spin_system *sys, const char *name, int value);
+
+/* ==== MEASUREMENT SUPPORT ===========================================================================================
+ * Nothing below is needed to use the library.  bench.py and the tests read these to say which kernels ran, how often and how long.  */
 /* number of kernel launches (own kernels) and cuFFT executions issued by this system so far */
 int spin_launch_counts(const spin_system *sys, int64_t *own_kernels, int64_t *cufft_execs);
-/* per-kernel device timing: when enabled, CUDA events bracket every launch of the step kernels; get returns the
- * accumulated milliseconds and launch counts for kind = 0 predictor, 1 corrector, 2 ddi (all ddi stages).   */
+/* per-kernel device timing: when enabled, CUDA events bracket the launches of the step kernels (plain launches, no graph, no
+ * all-steps-in-one-launch path); get returns the accumulated milliseconds and launch counts for kind = 0 predictor, 1 corrector,
+ * 2 one dipolar evaluation (all its stages), 3 the dipolar contraction kernel alone (slab path).                                 */
 int spin_profile_enable(spin_system *sys, int enabled);
 int spin_profile_get(spin_system *sys, int kind, double *total_ms, int64_t *launches);
 /* measured fp64 FMA throughput of this device in TFLOP/s (register-only kernel, best of 5): the ALU ceiling next to the HBM one */
 int spin_measure_fp64_tflops(spin_system *sys, double *tflops);
-/* execution options: use_graph (capture steps into a CUDA graph; default 1), store_A (1: predictor stores the
- * rotation field A, 0: corrector recomputes it; default 0)                                                  */
-int spin_set_option(spin_system *sys, const char *name, int value);
-/* further option: use_jit (1: the two sweeps are specialised per system at run time with NVRTC -- lattice extents, gather
- * tables and prefactors become compile-time constants; 0: table-driven kernels; default 1).
- * use_tma (default 0): 1 runs the specialised sweeps as persistent kernels that stage lattice planes in shared memory with TMA
- * tensor copies (lattices of at least 16384 spins; 2 forces it for any size).  Measured slower than the brick kernels on
- * cfg3, hence off by default.
- * use_col (default 0): 1 runs them as column-marching kernels (one thread per lattice column, own spin at z-1, z, z+1 kept in
- * registers; 3-D lattices).  Also measured slower than the brick kernels.
- * use_pair (default 0): 1 runs them with two sites (ia, ia+1) per thread and 128-bit loads and stores (even Na; Depondt solver, no
- * pinned spins, one image); 26 % fewer instructions and fewer L1 wavefronts, measured equal (predictor) or slower (corrector).
- * use_fused (default 0): 1 runs the Depondt step in one pass (predictor for tile + rim into shared memory, corrector from it; 48 B
- * per spin-update of HBM traffic; lattices of at least 16384 spins, 2 forces it).  Measured slower than the brick kernels on cfg3.
- * use_coop (default 1): lattices of up to 4096 spins without dipolar coupling run ALL steps of an llg_iterate call in one launch
- * instead of two launches per step: as one thread-block cluster with its hardware barrier between the sweeps (up to 16 bricks), else
- * as a cooperative launch with a grid barrier; 2 forces the path for any size (slower beyond about 10^4 spins), 3 forces the grid
- * barrier, 0 switches it off.
- * use_pdl (default -1 = automatic): programmatic dependent launch of the two brick sweeps -- each sweep is launched with programmatic
- * stream serialisation and waits inside the kernel (griddepcontrol.wait) for the previous kernel, so its launch latency and block ramp
- * overlap the tail of the one before; 1 releases the dependents at entry (the automatic choice for lattices of many waves of blocks),
- * 2 at the end of each block, 0 switches it off (the automatic choice for lattices of about one wave).  The order of all memory accesses, and with it every result bit, is unchanged.
- * cache_noise (default 1): the predictor keeps the thermal field of the step (24 B/spin) for the corrector instead of generating it twice.
- * ddi_slab (default 1): thin films with one basis atom take the dipolar slab path (2-D cuFFT + fused transform along c).
- * spin_kernel_info writes "jit+fused", "jit+cluster", "jit+coop", "jit+pair", "jit+col", "jit+tma", "jit (brick sweeps)" or "generic: <why>" into buf: which sweep kernels are in use.  */
+/* which sweep kernels are in use: "jit+cluster", "jit+coop", "jit (brick sweeps)" or "generic: <why>"                              */
 int spin_kernel_info(spin_system *sys, char *buf, int len);
-/* Which dipolar path the plan chose: "off", "3d" (general zero-padded 3-D transform), "slab" (thin film of one basis atom: transforms in
- * the a-b plane by cuFFT, hand-written transform along c fused with the contraction) or "slab+mirror" (the same, reading PZ/2 + 1 of the
- * PZ tensor planes because the spectrum was found mirror symmetric along c).  */
+/* Which dipolar path the plan chose: "off", "3d" (general zero-padded 3-D transform) or "slab" (thin film of one basis atom, 1-8 planes:
+ * transforms in the a-b plane, hand-written transform along c fused with the tensor contraction), followed by "+mirror" when the
+ * contraction reads PZ/2 + 1 of the PZ tensor planes (spectrum found mirror symmetric along c) and by "+own-a" when the transform along a
+ * is the hand-written one (rows of power-of-two length) instead of cuFFT's.                                                        */
 int spin_ddi_info(spin_system *sys, char *buf, int len);
 /* The run-time compiler of the specialised sweeps, e.g. "12.9 (/usr/local/cuda/lib64/libnvrtc.so.12)".  NVRTC is bound at run time by
  * path -- $SPINLLG_NVRTC, then the toolkit the library was built with, then the loader's libnvrtc.so.12 -- so that a different NVRTC

@@ -412,15 +412,6 @@ int enqueue_step_t(spin_system *s, const Launch &L, unsigned step_add) {
         return SPIN_OK;
     }
     const bool prof = s->profile_on != 0;
-    if (jit_fused_ready(s)) {          // one pass: predictor into shared memory, corrector from it
-        if (prof) cudaEventRecord(s->ev0, s->stream);
-        int rc = jit_launch_fused(s, n, nout, step_add);
-        if (rc) return rc;
-        s->n_launch++;
-        if (prof) { cudaEventRecord(s->ev1, s->stream); cudaEventSynchronize(s->ev1); float ms; cudaEventElapsedTime(&ms, s->ev0, s->ev1); s->prof_ms[1] += ms; s->prof_n[1]++; }
-        s->cur ^= 1;
-        return SPIN_OK;
-    }
     const size_t istr = (size_t)s->nb * s->plan.sub;       // image stride
     if (s->ddi_on) {
         if (prof) cudaEventRecord(s->ev0, s->stream);
@@ -429,12 +420,9 @@ int enqueue_step_t(spin_system *s, const Launch &L, unsigned step_add) {
         if (rc) return rc;
         if (prof) { cudaEventRecord(s->ev1, s->stream); cudaEventSynchronize(s->ev1); float ms; cudaEventElapsedTime(&ms, s->ev0, s->ev1); s->prof_ms[2] += ms; s->prof_n[2]++; }
     }
-    const bool jit = jit_ready(s), pair = jit_pair_ready(s), col = !pair && jit_col_ready(s), tma = !pair && !col && jit_tma_ready(s);
+    const bool jit = jit_ready(s);
     if (prof) cudaEventRecord(s->ev0, s->stream);
-    if (pair) { int rc = jit_launch_predictor_pair(s, n, s->d_fddi[0], s->d_np, step_add); if (rc) return rc; }
-    else if (col) { int rc = jit_launch_predictor_col(s, n, s->d_fddi[0], s->d_np, step_add); if (rc) return rc; }
-    else if (tma) { int rc = jit_launch_predictor_tma(s, s->cur, s->d_fddi[0], s->d_np, step_add); if (rc) return rc; }
-    else if (jit) { int rc = jit_launch_predictor(s, L.grid, L.block, n, s->d_fddi[0], s->d_np, s->d_A, step_add); if (rc) return rc; }
+    if (jit) { int rc = jit_launch_predictor(s, L.grid, L.block, n, s->d_fddi[0], s->d_np, s->d_A, step_add); if (rc) return rc; }
     else if (s->opt_store_A)
         predictor_kernel<BX, BY, BZ, true><<<L.grid, L.block, 0, s->stream>>>(s->plan, n, s->d_fddi[0], s->d_np, s->d_A, s->d_step, step_add);
     else
@@ -449,10 +437,7 @@ int enqueue_step_t(spin_system *s, const Launch &L, unsigned step_add) {
         if (prof) { cudaEventRecord(s->ev1, s->stream); cudaEventSynchronize(s->ev1); float ms; cudaEventElapsedTime(&ms, s->ev0, s->ev1); s->prof_ms[2] += ms; s->prof_n[2]++; }
     }
     if (prof) cudaEventRecord(s->ev0, s->stream);
-    if (pair) { int rc = jit_launch_corrector_pair(s, n, s->d_np, s->d_fddi[0], s->d_fddi[1], nout, step_add); if (rc) return rc; }
-    else if (col) { int rc = jit_launch_corrector_col(s, n, s->d_np, s->d_fddi[0], s->d_fddi[1], nout, step_add); if (rc) return rc; }
-    else if (tma) { int rc = jit_launch_corrector_tma(s, s->cur, s->d_fddi[0], s->d_fddi[1], nout, step_add); if (rc) return rc; }
-    else if (jit) { int rc = jit_launch_corrector(s, L.grid, L.block, n, s->d_np, s->d_fddi[0], s->d_fddi[1], s->d_A, nout, step_add); if (rc) return rc; }
+    if (jit) { int rc = jit_launch_corrector(s, L.grid, L.block, n, s->d_np, s->d_fddi[0], s->d_fddi[1], s->d_A, nout, step_add); if (rc) return rc; }
     else if (s->opt_store_A)
         corrector_kernel<BX, BY, BZ, true><<<L.grid, L.block, 0, s->stream>>>(s->plan, n, s->d_np, s->d_fddi[0], s->d_fddi[1], s->d_A, nout, s->d_step, step_add);
     else
@@ -523,7 +508,7 @@ extern "C" int spin_geometry_create(const double bravais[9], int n_basis, const 
     if (!has_device) cudaGetLastError();
     spin_system *s = new spin_system();
     s->has_device = has_device;
-    s->jit = nullptr; s->opt_jit = 1; s->opt_tma = 0; s->opt_ddi_slab = 1; s->opt_col = 0; s->opt_pair = 0; s->opt_pdl = -1; s->opt_cache_noise = 1; s->opt_coop = 1; s->opt_fused = 0; s->d_bar = nullptr;
+    s->jit = nullptr; s->opt_jit = 1; s->opt_ddi_slab = 1; s->opt_ddi_mirror = 1; s->opt_pdl = -1; s->opt_cache_noise = 1; s->opt_coop = 1; s->d_bar = nullptr;
     s->n_img = 1; s->img_sel = 0; s->d_img_sigma = nullptr;
     memcpy(s->brav, bravais, sizeof(s->brav));
     s->nb = n_basis;
@@ -902,7 +887,7 @@ extern "C" int llg_iterate(spin_system *s, int64_t n_steps) {
     // (a grid barrier costs about as much as a launch inside a CUDA graph, and it empties L1), so the limit is low; option
     // use_coop = 2 forces it for any lattice without dipolar coupling.
     const int64_t COOP_CHUNK = 8192;
-    if (s->opt_coop && !s->profile_on && !s->ddi_on && (s->N <= SPIN_COOP_MAX_SPINS || s->opt_coop >= 2) && jit_coop_ready(s) && !jit_fused_ready(s) &&
+    if (s->opt_coop && !s->profile_on && !s->ddi_on && (s->N <= SPIN_COOP_MAX_SPINS || s->opt_coop >= 2) && jit_coop_ready(s) &&
         n_steps > 0) {
         while (done < n_steps) {
             const unsigned chunk = (unsigned)std::min<int64_t>(COOP_CHUNK, n_steps - done);
@@ -940,7 +925,7 @@ extern "C" int llg_iterate(spin_system *s, int64_t n_steps) {
         }
         while (n_steps - done >= G) {
             SPIN_CUDA(cudaGraphLaunch(gexec, s->stream));
-            s->n_launch += (s->solver == SPIN_SOLVER_RK4 ? 4 : (jit_fused_ready(s) ? 1 : 2)) * G + 1;
+            s->n_launch += (s->solver == SPIN_SOLVER_RK4 ? 4 : 2) * G + 1;
             done += G;
         }
     }
@@ -1205,14 +1190,11 @@ extern "C" int spin_set_option(spin_system *s, const char *name, int value) {
     if (!strcmp(name, "use_graph")) s->opt_graph = value ? 1 : 0;
     else if (!strcmp(name, "store_A")) { s->opt_store_A = value ? 1 : 0; s->plan_dirty = true; }
     else if (!strcmp(name, "use_jit")) { s->opt_jit = value ? 1 : 0; s->plan_dirty = true; }
-    else if (!strcmp(name, "use_fused")) { s->opt_fused = value < 0 ? 0 : (value > 2 ? 2 : value); s->plan_dirty = true; }
     else if (!strcmp(name, "use_coop")) { s->opt_coop = value < 0 ? 0 : (value > 3 ? 3 : value); s->plan_dirty = true; }
     else if (!strcmp(name, "cache_noise")) { s->opt_cache_noise = value ? 1 : 0; s->plan_dirty = true; }
     else if (!strcmp(name, "use_pdl")) { s->opt_pdl = value > 2 ? -1 : value < 0 ? -1 : value; s->plan_dirty = true; }
-    else if (!strcmp(name, "use_pair")) { s->opt_pair = value ? 1 : 0; s->plan_dirty = true; }
-    else if (!strcmp(name, "use_col")) { s->opt_col = value ? 1 : 0; s->plan_dirty = true; }
+    else if (!strcmp(name, "ddi_mirror")) { s->opt_ddi_mirror = value ? 1 : 0; s->plan_dirty = true; }
     else if (!strcmp(name, "ddi_slab")) { s->opt_ddi_slab = value < 0 ? 0 : (value > 2 ? 2 : value); s->plan_dirty = true; }      // 0: 3-D path, 1: slab path, 2: slab path with cuFFT's a-pass
-    else if (!strcmp(name, "use_tma")) { s->opt_tma = value < 0 ? 0 : (value > 2 ? 2 : value); s->plan_dirty = true; }
     else return spin::fail(SPIN_ERR_ARG, "unknown option '%s'", name);
     drop_graphs(s);
     return SPIN_OK;
@@ -1222,11 +1204,7 @@ extern "C" int spin_set_option(spin_system *s, const char *name, int value) {
 extern "C" int spin_kernel_info(spin_system *s, char *buf, int len) {
     REQUIRE(s && buf && len > 0, "bad argument");
     if (s->has_device) { int rc = ensure_plan(s); if (rc) return rc; }
-    if (jit_fused_ready(s)) snprintf(buf, (size_t)len, "jit+fused");
-    else if (jit_coop_ready(s) && s->opt_coop && !s->ddi_on && (s->N <= SPIN_COOP_MAX_SPINS || s->opt_coop >= 2)) snprintf(buf, (size_t)len, jit_cluster_ready(s) ? "jit+cluster" : "jit+coop");
-    else if (jit_pair_ready(s)) snprintf(buf, (size_t)len, "jit+pair");
-    else if (jit_col_ready(s)) snprintf(buf, (size_t)len, "jit+col");
-    else if (jit_tma_ready(s)) snprintf(buf, (size_t)len, "jit+tma");
+    if (jit_coop_ready(s) && s->opt_coop && !s->ddi_on && (s->N <= SPIN_COOP_MAX_SPINS || s->opt_coop >= 2)) snprintf(buf, (size_t)len, jit_cluster_ready(s) ? "jit+cluster" : "jit+coop");
     else if (jit_ready(s)) snprintf(buf, (size_t)len, "jit (brick sweeps)");
     else snprintf(buf, (size_t)len, "generic: %s", s->jit_note.c_str());
     return SPIN_OK;

@@ -693,8 +693,7 @@ int spin::ddi_prepare(spin_system *s) {
         cudaFree(d_chk);
         double dev, mag;
         memcpy(&dev, &h_chk[0], 8); memcpy(&mag, &h_chk[1], 8);
-        const char *e = getenv("SPINLLG_DDI_MIRROR");
-        d->mirror = d->PZ > 2 && dev <= 1e-13 * mag && !(e && atoi(e) == 0);
+        d->mirror = d->PZ > 2 && dev <= 1e-13 * mag && s->opt_ddi_mirror;
     }
     SPIN_CUDA(cudaStreamSynchronize(s->stream));
     SPIN_CUDA(cudaGetLastError());

@@ -90,8 +90,7 @@ __device__ __forceinline__ void store_spin(double *__restrict__ q, const Coord &
 }
 
 // Site accessors: where the partner (sublattice BJ at translation DA, DB, DC) of a site of sublattice B is read from.
-// GlobalAcc: the ghost-cell arrays in global memory (own address + immediate); RingAcc (spin_jit_tma.cuh): the ring of lattice
-// planes that TMA stages in shared memory.
+// GlobalAcc: the ghost-cell arrays in global memory (own address + immediate).
 template <int NCONF, bool CG = false>
 struct GlobalAcc {
     const double *cfg[NCONF];      // x component of the own site in configuration k
@@ -556,16 +555,3 @@ extern "C" __global__ void SPIN_BOUNDS(spec::BX *spec::BY *spec::BZ)
                       const unsigned char *__restrict__ pin) {
     spinjit::all_steps(n0, n1, np, aux, *d_step, nsteps, seed_lo, seed_hi, pin, []() { spinjit::cluster_barrier(); });
 }
-
-#ifdef SPIN_FUSED
-#include "spin_jit_fused.cuh"
-#endif
-#ifdef SPIN_COL
-#include "spin_jit_col.cuh"
-#endif
-#ifdef SPIN_PAIR
-#include "spin_jit_pair.cuh"
-#endif
-#ifdef SPIN_TMA
-#include "spin_jit_tma.cuh"
-#endif

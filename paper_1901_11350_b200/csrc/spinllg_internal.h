@@ -146,7 +146,7 @@ struct spin_system {
     bool has_device;               // false only in the planner-only mode used by the CPU tests
     std::string jit_note;          // why the specialised sweeps are not in use, if they are not
     // ---- execution options / bookkeeping
-    int opt_graph, opt_store_A, opt_jit, opt_tma, opt_ddi_slab, opt_col, opt_pair, opt_pdl, opt_cache_noise, opt_coop, opt_fused;
+    int opt_graph, opt_store_A, opt_jit, opt_ddi_slab, opt_ddi_mirror, opt_pdl, opt_cache_noise, opt_coop;
     cudaGraphExec_t graph_exec[2];   // one captured graph per ping-pong parity
     int graph_steps;
     int64_t n_launch, n_fft;
@@ -182,9 +182,6 @@ int jit_prepare(spin_system *s);
 void jit_release(spin_system *s);
 bool jit_ready(const spin_system *s);
 const char *jit_log(const spin_system *s);
-// one-pass Depondt step (jit_depondt_fused)
-bool jit_fused_ready(const spin_system *s);
-int jit_launch_fused(spin_system *s, const double *n, double *nout, unsigned step_add);
 // one stage of the RK4 solver (jit_rk4_stage)
 int jit_launch_rk4_stage(spin_system *s, const double *base, const double *y, double *ynext, double *acc, double *noise, const double *fddi,
                          int stage, unsigned step_add);
@@ -192,21 +189,6 @@ int jit_launch_rk4_stage(spin_system *s, const double *base, const double *y, do
 bool jit_coop_ready(const spin_system *s);
 bool jit_cluster_ready(const spin_system *s);
 int jit_launch_steps_coop(spin_system *s, unsigned nsteps);
-// two sites per thread with 128-bit accesses (spin_jit_pair.cuh)
-bool jit_pair_ready(const spin_system *s);
-int jit_launch_predictor_pair(spin_system *s, const double *n, const double *fddi, double *np, unsigned step_add);
-int jit_launch_corrector_pair(spin_system *s, const double *n, const double *np, const double *fddi_n, const double *fddi_np, double *nout,
-                              unsigned step_add);
-// column-marching versions of the two sweeps (spin_jit_col.cuh)
-bool jit_col_ready(const spin_system *s);
-int jit_launch_predictor_col(spin_system *s, const double *n, const double *fddi, double *np, unsigned step_add);
-int jit_launch_corrector_col(spin_system *s, const double *n, const double *np, const double *fddi_n, const double *fddi_np, double *nout,
-                             unsigned step_add);
-// TMA-fed plane-marching versions of the two sweeps (spin_jit_tma.cuh); cur = index of the current n buffer
-bool jit_tma_ready(const spin_system *s);
-const char *jit_tma_note(const spin_system *s);
-int jit_launch_predictor_tma(spin_system *s, int cur, const double *fddi, double *np, unsigned step_add);
-int jit_launch_corrector_tma(spin_system *s, int cur, const double *fddi_n, const double *fddi_np, double *nout, unsigned step_add);
 int jit_launch_predictor(spin_system *s, dim3 grid, dim3 block, const double *n, const double *fddi, double *np, double *Aout,
                          unsigned step_add);
 int jit_launch_corrector(spin_system *s, dim3 grid, dim3 block, const double *n, const double *np, const double *fddi_n,

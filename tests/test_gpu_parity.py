@@ -258,44 +258,6 @@ def test_specialised_and_table_driven_sweeps_agree(P, O, cfg):
 
 
 # ---------------------------------------------------------------------------------------------------------------------
-# TMA-fed plane-marching sweeps (csrc/spin_jit_tma.cuh): forced on for small replicas (use_tma=2), several items per CTA
-TMA_CASES = [
-    (1, (37, 19, 1), 200, None),
-    (2, (45, 33, 1), 200, None),
-    (3, (35, 9, 7), 200, None),
-    (3, (70, 37, 45), 20, "0,0,0,45"),       # 15 columns x 45 chunks = 675 items > resident CTAs: every CTA marches several items
-    (3, (70, 37, 45), 20, "0,16,2,3"),       # 32x16 tiles, look-ahead 2, 3 chunks of 15 planes
-    (4, (33, 17, 1), 200, None),
-    (5, (20, 12, 5), 30, None),
-]
-
-
-@pytest.mark.parametrize("cfg,cells,steps,geo", TMA_CASES)
-def test_tma_sweeps_match_oracle(P, O, cfg, cells, steps, geo, monkeypatch):
-    if geo:
-        monkeypatch.setenv("SPINLLG_TMA_P", geo)
-        monkeypatch.setenv("SPINLLG_TMA_C", geo)
-    w = W.CONFIGS[cfg]().resized(cells, steps)
-    g, o = pair(P, O, w)
-    g.spin_set_option("use_col", 0)
-    g.spin_set_option("use_coop", 0)
-    g.spin_set_option("use_tma", 2)
-    assert g.spin_kernel_info() == "jit+tma", g.spin_kernel_info()
-    g.llg_iterate(steps); o.iterate(steps)
-    d = np.abs(g.spins_get() - o.spins()).max()
-    print(f"tma cfg{cfg} {cells} steps={steps}: max|dn| = {d:.3e}")
-    assert d <= SPIN_ATOL
-    # bit-identical to the brick kernels: same arithmetic, only the staging differs
-    b = P.SpinSystem.from_workload(w)
-    b.spin_set_option("use_tma", 0)
-    b.spin_set_option("use_col", 0)
-    b.spin_set_option("use_coop", 0)
-    assert b.spin_kernel_info().startswith("jit (brick")
-    b.llg_iterate(steps)
-    assert np.array_equal(b.spins_get(), g.spins_get())
-
-
-# ---------------------------------------------------------------------------------------------------------------------
 # BASELINE.json's full sizes in the launch configuration bench.py times (specialised kernels, CUDA-graph replay of 16-step
 # batches).  The oracle computes the whole lattice for the field; trajectories run as many steps as it finishes in seconds.
 FULL_SIZE = [(2, 2000), (3, 48), (4, 200), (5, 4)]
@@ -393,49 +355,14 @@ def test_ddi_slab_mirror_symmetry_of_the_tensor(P, O, bravais, cells, monkeypatc
     g0, o0 = pair(P, O, w0)
     Fd = o0.ddi_field(direct=True) / (w.mu_s[0] * O.MU_B)
     assert np.abs(g0.effective_field() - Fd).max() <= 1e-11 * np.abs(Fd).max()
-    monkeypatch.setenv("SPINLLG_DDI_MIRROR", "0")      # all planes read, whatever the symmetry
     h = P.SpinSystem.from_workload(w)
+    h.spin_set_option("ddi_mirror", 0)                  # all planes read, whatever the symmetry
     Bh = h.effective_field()
     assert h.spin_ddi_info().replace("+own-a", "") == "slab"
     assert_fields_close(Bh, Bo)
     assert np.abs(Bh - Bg).max() <= 1e-13 * np.abs(Bo).max()
     g.llg_iterate(10); o.iterate(10)
     assert np.abs(g.spins_get() - o.spins()).max() <= SPIN_ATOL
-
-
-# ---------------------------------------------------------------------------------------------------------------------
-# Column-marching sweeps (csrc/spin_jit_col.cuh), option use_col=1 (measured slower than the bricks): same arithmetic
-@pytest.mark.parametrize("cfg,cells,steps,geo", [(3, (35, 9, 7), 100, None), (3, (70, 37, 45), 20, "32,8,16"), (3, (33, 5, 40), 20, "64,2,7"),
-                                                 (5, (20, 12, 5), 20, None), (5, (20, 12, 4), 20, "32,4,3"), (3, (6, 5, 2), 50, None)])
-def test_column_marching_sweeps(P, O, cfg, cells, steps, geo, monkeypatch):
-    if geo:
-        monkeypatch.setenv("SPINLLG_COL", geo)
-    w = W.CONFIGS[cfg]().resized(cells, steps)
-    g, o = pair(P, O, w)
-    g.spin_set_option("use_col", 1)
-    g.spin_set_option("use_coop", 0)
-    assert g.spin_kernel_info() == "jit+col", g.spin_kernel_info()
-    g.llg_iterate(steps); o.iterate(steps)
-    d = np.abs(g.spins_get() - o.spins()).max()
-    print(f"col cfg{cfg} {cells} steps={steps}: max|dn| = {d:.3e}")
-    assert d <= SPIN_ATOL
-    b = P.SpinSystem.from_workload(w)
-    b.spin_set_option("use_col", 0)
-    b.spin_set_option("use_coop", 0)
-    assert b.spin_kernel_info().startswith("jit (brick")
-    b.llg_iterate(steps)
-    assert np.array_equal(b.spins_get(), g.spins_get())
-
-
-def test_column_marching_with_open_and_mixed_boundaries(P, O):
-    for per in [(0, 0, 0), (1, 0, 1), (0, 1, 0)]:
-        w = dataclasses.replace(W.config3().resized((21, 10, 9), 30), periodic=per)
-        g, o = pair(P, O, w)
-        g.spin_set_option("use_col", 1)
-        g.spin_set_option("use_coop", 0)
-        assert g.spin_kernel_info() == "jit+col"
-        g.llg_iterate(30); o.iterate(30)
-        assert np.abs(g.spins_get() - o.spins()).max() <= SPIN_ATOL
 
 
 # ---------------------------------------------------------------------------------------------------------------------
@@ -458,49 +385,6 @@ def test_programmatic_dependent_launch_is_bit_identical(P, O, cfg, cells, steps)
     o = O.OracleSystem.from_workload(w)
     o.iterate(steps)
     assert np.abs(out[0] - o.spins()).max() <= SPIN_ATOL
-
-
-# ---------------------------------------------------------------------------------------------------------------------
-# Two sites per thread with 128-bit accesses (csrc/spin_jit_pair.cuh), option use_pair=1: same arithmetic, bit-identical
-@pytest.mark.parametrize("cfg,cells,steps,geo", [(1, (34, 9, 1), 100, None), (2, (70, 33, 1), 100, None), (3, (36, 9, 7), 60, None),
-                                                 (3, (70, 37, 11), 20, "64,2,2"), (3, (2, 5, 3), 50, None), (4, (34, 17, 1), 100, None),
-                                                 (5, (20, 12, 5), 20, None), (5, (20, 12, 4), 20, "16,4,4")])
-def test_pair_sweeps(P, O, cfg, cells, steps, geo, monkeypatch):
-    if geo:
-        monkeypatch.setenv("SPINLLG_PAIR", geo)
-    w = W.CONFIGS[cfg]().resized(cells, steps)
-    g, o = pair(P, O, w)
-    g.spin_set_option("use_pair", 1)
-    g.spin_set_option("use_coop", 0)
-    assert g.spin_kernel_info() == "jit+pair", g.spin_kernel_info()
-    g.llg_iterate(steps); o.iterate(steps)
-    d = np.abs(g.spins_get() - o.spins()).max()
-    print(f"pair cfg{cfg} {cells} steps={steps}: max|dn| = {d:.3e}")
-    assert d <= SPIN_ATOL
-    b = P.SpinSystem.from_workload(w)
-    b.spin_set_option("use_coop", 0)
-    assert b.spin_kernel_info().startswith("jit (brick")
-    b.llg_iterate(steps)
-    assert np.array_equal(b.spins_get(), g.spins_get())
-
-
-def test_pair_sweeps_boundaries_and_fallback(P, O):
-    for per in [(0, 0, 0), (1, 0, 1), (0, 1, 0)]:
-        w = dataclasses.replace(W.config3().resized((22, 10, 9), 30), periodic=per)
-        g, o = pair(P, O, w)
-        g.spin_set_option("use_pair", 1)
-        g.spin_set_option("use_coop", 0)
-        assert g.spin_kernel_info() == "jit+pair"
-        g.llg_iterate(30); o.iterate(30)
-        assert np.abs(g.spins_get() - o.spins()).max() <= SPIN_ATOL
-    # an odd row length cannot be paired: the option is ignored, the brick sweeps run
-    w = W.config3().resized((21, 10, 9), 10)
-    g, o = pair(P, O, w)
-    g.spin_set_option("use_pair", 1)
-    g.spin_set_option("use_coop", 0)
-    assert g.spin_kernel_info().startswith("jit (brick"), g.spin_kernel_info()
-    g.llg_iterate(10); o.iterate(10)
-    assert np.abs(g.spins_get() - o.spins()).max() <= SPIN_ATOL
 
 
 # ---------------------------------------------------------------------------------------------------------------------
@@ -693,42 +577,6 @@ def test_cooperative_kernel_matches_two_launch_path(P, O, cfg, cells, steps):
 
 
 # ---------------------------------------------------------------------------------------------------------------------
-# One-pass Depondt step (csrc/spin_jit_fused.cuh): predictor for tile + rim into shared memory, corrector from it
-FUSED_CASES = [
-    (1, (37, 19, 1), 100, None, (1, 1, 0)),
-    (2, (45, 33, 1), 100, None, (1, 1, 0)),          # reach 2, thermal field kept in shared memory
-    (3, (35, 9, 7), 100, None, (1, 1, 1)),
-    (3, (70, 37, 45), 20, "32,8,8,512", (1, 1, 1)),
-    (3, (70, 37, 45), 20, "16,4,4,256", (0, 1, 0)),  # small tiles, open and periodic edges mixed
-    (3, (33, 5, 40), 20, "32,4,16,1024", (1, 0, 1)),
-    (4, (33, 17, 1), 100, None, (1, 1, 0)),          # two sublattices, quadruplets, current
-    (4, (33, 17, 1), 50, "32,8,1,256", (0, 0, 0)),
-    (3, (2, 2, 2), 30, None, (1, 1, 1)),             # the rim wraps onto the tile itself
-]
-
-
-@pytest.mark.parametrize("cfg,cells,steps,geo,per", FUSED_CASES)
-def test_one_pass_step_matches_two_sweep_kernels(P, O, cfg, cells, steps, geo, per, monkeypatch):
-    if geo:
-        monkeypatch.setenv("SPINLLG_FUSED", geo)
-    w = dataclasses.replace(W.CONFIGS[cfg]().resized(cells, steps), periodic=per)
-    mask = (np.random.default_rng(7).random(w.n_spins) < 0.05).astype(np.uint8)
-    g, o = pair(P, O, w)
-    g.spin_set_option("use_fused", 2)
-    g.spins_set_pinned(mask); o.set_pinned(mask)
-    assert g.spin_kernel_info() == "jit+fused", g.spin_kernel_info()
-    g.llg_iterate(steps); o.iterate(steps)
-    d = np.abs(g.spins_get() - o.spins()).max()
-    print(f"fused cfg{cfg} {cells} steps={steps}: max|dn| = {d:.3e}")
-    assert d <= SPIN_ATOL
-    b = P.SpinSystem.from_workload(w)
-    b.spin_set_option("use_coop", 0)
-    b.spins_set_pinned(mask)
-    assert b.spin_kernel_info().startswith("jit (brick")
-    b.llg_iterate(steps)
-    assert np.array_equal(b.spins_get(), g.spins_get())          # same arithmetic, bit for bit
-
-
 def test_checkpoint_resume(P, O):
     """SURVEY section 5 "checkpoint / resume": spins_get + llg_get_step, then spins_set + llg_set_step on a fresh system, continues
     the same trajectory (the noise is keyed by the step counter).  spins_set renormalises, so agreement is to rounding, not bitwise."""
