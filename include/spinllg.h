@@ -65,6 +65,11 @@ int spin_set_stream(spin_system *sys, void *cuda_stream);
 /* ---- Hamiltonian, Eq. 1 (:61-67) and Eq. 2 (:75) ------------------------------------------------------- */
 /* magnetic moments mu_i per basis atom, in mu_B, > 0 (":59 m_i = mu_i n_i") */
 int hamiltonian_set_mu_s(spin_system *sys, const double *mu_s /*host, n_basis*/);
+/* ":79 defects, such as vacancies and atoms of different types": one moment per SITE (host, N values in mu_B in boundary order, > 0),
+ * replacing the basis atom's wherever mu_i enters -- the Zeeman term and the dipolar sum of Eq. 1, the 1/mu_i of Eq. 10, the thermal
+ * amplitude of Eq. 11 and the conversion of effective_field to Tesla.  NULL goes back to the basis atoms' moments.  The array is copied.
+ * Costs one extra 8-byte read per spin and sweep.                                                                                  */
+int hamiltonian_set_site_mu_s(spin_system *sys, const double *mu_site /*host, N, or NULL*/);
 /* Zeeman term -sum_i mu_i B.n_i: field magnitude in Tesla and direction (normalised internally) */
 int hamiltonian_set_field(spin_system *sys, double B_tesla, const double dir[3]);
 /* uniaxial anisotropy -sum_i sum_j K_j (K^_j.n_i)^2 (Eq. 1 :61, ":69 axes ... of the basis cell"): n entries (basis_idx, K_meV, axis);

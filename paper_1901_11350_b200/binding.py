@@ -17,7 +17,7 @@ _LIB = None
 
 EXPORTS = [
     "spin_geometry_create", "spin_system_destroy", "spin_system_nspins", "spin_set_stream",
-    "hamiltonian_set_mu_s", "hamiltonian_set_field", "hamiltonian_set_anisotropy", "hamiltonian_set_pairs",
+    "hamiltonian_set_mu_s", "hamiltonian_set_site_mu_s", "hamiltonian_set_field", "hamiltonian_set_anisotropy", "hamiltonian_set_pairs",
     "hamiltonian_set_exchange_shells", "hamiltonian_set_dmi_shells", "hamiltonian_set_quadruplets",
     "hamiltonian_set_ddi", "spin_set_images", "spin_select_image", "llg_set_image_temperatures", "gneb_forces", "gneb_iterate", "spins_set_pinned", "spins_set", "spins_get", "spins_set_device", "spins_get_device",
     "llg_configure", "llg_set_solver", "llg_set_damping_only", "minimise_vp", "minimise_vp_reset", "llg_iterate", "llg_get_step", "llg_set_step", "spin_synchronize",
@@ -50,6 +50,7 @@ def lib() -> C.CDLL:
         "spin_system_nspins": (C.c_int64, [vp]),
         "spin_set_stream": (C.c_int, [vp, vp]),
         "hamiltonian_set_mu_s": (C.c_int, [vp, dp]),
+        "hamiltonian_set_site_mu_s": (C.c_int, [vp, dp]),
         "hamiltonian_set_field": (C.c_int, [vp, C.c_double, dp]),
         "hamiltonian_set_anisotropy": (C.c_int, [vp, C.c_int, ip, dp, dp]),
         "hamiltonian_set_pairs": (C.c_int, [vp, C.c_int, ip, ip, ip, dp, dp]),
@@ -171,6 +172,13 @@ class SpinSystem:
     def hamiltonian_set_mu_s(self, mu):
         a, p = _d(np.broadcast_to(np.asarray(mu, float), (self.n_basis,)))
         _check(lib().hamiltonian_set_mu_s(self._h, p))
+
+    def hamiltonian_set_site_mu_s(self, mu_site):
+        if mu_site is None:
+            _check(lib().hamiltonian_set_site_mu_s(self._h, None))
+            return
+        a, p = _d(np.asarray(mu_site, float).reshape(self.N))
+        _check(lib().hamiltonian_set_site_mu_s(self._h, p))
 
     def hamiltonian_set_field(self, B, direction):
         a, p = _d(direction)

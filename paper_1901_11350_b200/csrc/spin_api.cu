@@ -192,6 +192,7 @@ int build_plan(const spin_system *s, DevicePlan &P) {
     P.has_ddi = s->ddi_on ? 1 : 0;
     P.damping_only = s->damping_only;
     P.pin = s->d_pin;
+    P.mu_ratio = s->d_mu_ratio;
     P.stt_on = (s->u != 0.0) ? 1 : 0;
     if (P.stt_on) {
         if (stt_coefficients(s, P.stt_c) != 0) return spin::fail(SPIN_ERR_ARG, "current direction: singular lattice metric");
@@ -359,12 +360,28 @@ int upload_image_sigma(spin_system *s) {
     return SPIN_OK;
 }
 
+// mu_i / mu_b(i) in boundary order from the per-site moments kept on the host
+int upload_mu_ratio(spin_system *s) {
+    if (s->mu_site.empty()) return SPIN_OK;
+    std::vector<double> r((size_t)s->N);
+    for (int64_t i = 0; i < s->N; ++i) r[(size_t)i] = s->mu_site[(size_t)i] / s->mu[(size_t)(i % s->nb)];
+    if (!s->d_mu_ratio) {
+        cudaError_t e = cudaMalloc(&s->d_mu_ratio, (size_t)s->N * sizeof(double));
+        if (e != cudaSuccess) { s->d_mu_ratio = nullptr; return spin::fail(SPIN_ERR_MEMORY, "device allocation of %lld bytes failed", (long long)(s->N * 8)); }
+    }
+    SPIN_CUDA(cudaMemcpyAsync(s->d_mu_ratio, r.data(), (size_t)s->N * sizeof(double), cudaMemcpyHostToDevice, s->stream));
+    SPIN_CUDA(cudaStreamSynchronize(s->stream));
+    return SPIN_OK;
+}
+
 int ensure_plan(spin_system *s) {
     NEED_DEVICE(s);
     if (!s->plan_dirty) return SPIN_OK;
     s->vp_active = false;
+    int rc = upload_mu_ratio(s);               // per-site moments relative to the (possibly changed) basis moments
+    if (rc) return rc;
     DevicePlan P;
-    int rc = build_plan(s, P);
+    rc = build_plan(s, P);
     if (rc) return rc;
     drop_graphs(s);
     if (!s->d_n[0] || !same_layout(P, s->plan)) {
@@ -525,7 +542,7 @@ extern "C" int spin_geometry_create(const double bravais[9], int n_basis, const 
     s->stream = nullptr; s->own_stream = nullptr; s->cur = 0;
     s->d_n[0] = s->d_n[1] = s->d_np = s->d_A = s->d_fddi[0] = s->d_fddi[1] = s->d_aos = s->d_partials = s->d_result = nullptr;
     s->d_vp = nullptr; s->vp_active = false; s->vp_cur = 0;
-    s->d_step = nullptr; s->d_pin = nullptr; s->ddi = nullptr; s->plan_dirty = true;
+    s->d_step = nullptr; s->d_pin = nullptr; s->d_mu_ratio = nullptr; s->ddi = nullptr; s->plan_dirty = true;
     s->opt_graph = 1; s->opt_store_A = 0; s->graph_exec[0] = s->graph_exec[1] = nullptr; s->graph_steps = 0;
     s->n_launch = s->n_fft = 0; s->profile_on = 0;
     for (int k = 0; k < 3; ++k) { s->prof_ms[k] = 0; s->prof_n[k] = 0; }
@@ -573,7 +590,7 @@ extern "C" void spin_system_destroy(spin_system *s) {
     jit_release(s);
     cudaFree(s->d_n[0]); cudaFree(s->d_n[1]); cudaFree(s->d_np); cudaFree(s->d_A); cudaFree(s->d_fddi[0]); cudaFree(s->d_fddi[1]);
     cudaFree(s->d_pin); cudaFree(s->d_vp); cudaFree(s->d_bar); cudaFree(s->d_img_sigma);
-    cudaFree(s->d_aos); cudaFree(s->d_partials); cudaFree(s->d_result); cudaFree(s->d_step);
+    cudaFree(s->d_aos); cudaFree(s->d_partials); cudaFree(s->d_result); cudaFree(s->d_step); cudaFree(s->d_mu_ratio);
     if (s->ev0) cudaEventDestroy(s->ev0);
     if (s->ev1) cudaEventDestroy(s->ev1);
     if (s->ev2) cudaEventDestroy(s->ev2);
@@ -599,6 +616,21 @@ extern "C" int hamiltonian_set_mu_s(spin_system *s, const double *mu) {
     for (int b = 0; b < s->nb; ++b) REQUIRE(mu[b] > 0.0 && isfinite(mu[b]), "mu_s must be positive");
     s->mu.assign(mu, mu + s->nb);
     s->plan_dirty = true;
+    return SPIN_OK;
+}
+// PAPER.md:79 "defects, such as vacancies and atoms of different types": a moment per site (mu_B, boundary order) that replaces the basis
+// atom's wherever mu_i enters: Zeeman force, dipolar sums, the 1/mu_i of Eq. 10, the thermal amplitude of Eq. 11, the conversion to Tesla
+extern "C" int hamiltonian_set_site_mu_s(spin_system *s, const double *mu_site) {
+    REQUIRE(s, "null system");
+    if (!mu_site) {
+        s->mu_site.clear();
+        if (s->d_mu_ratio) { if (s->has_device) cudaStreamSynchronize(s->stream); cudaFree(s->d_mu_ratio); s->d_mu_ratio = nullptr; }
+    } else {
+        for (int64_t i = 0; i < s->N; ++i) REQUIRE(mu_site[i] > 0.0 && isfinite(mu_site[i]), "site %lld: moment must be positive and finite", (long long)i);
+        s->mu_site.assign(mu_site, mu_site + s->N);
+    }
+    s->plan_dirty = true;
+    drop_graphs(s);
     return SPIN_OK;
 }
 extern "C" int hamiltonian_set_field(spin_system *s, double B, const double dir[3]) {

@@ -109,7 +109,7 @@ __global__ void ddi_scatter_kernel(const __grid_constant__ DevicePlan L, const d
     const int ia = cell % L.Na, ib = (cell / L.Na) % L.Nb, ic = cell / (L.Na * L.Nb);
     const long long p = ia + (long long)P0 * (ib + (long long)P1 * ic);
     const int j = b * L.sub + ((ic + L.LC) * L.PB + (ib + L.LB)) * (3 * L.PA) + (ia + L.LA);
-    const double m = mu[b];
+    const double m = mu[b] * (L.mu_ratio ? L.mu_ratio[b + L.nb * cell] : 1.0);      // per-site moments
 #pragma unroll
     for (int k = 0; k < 3; ++k) Mpad[(size_t)(b * 3 + k) * Ptot + p] = m * n[j + k * L.PA];
 }
@@ -147,7 +147,7 @@ __global__ void ddi_gather_kernel(const __grid_constant__ DevicePlan L, const do
     const int ia = cell % L.Na, ib = (cell / L.Na) % L.Nb, ic = cell / (L.Na * L.Nb);
     const long long p = ia + (long long)P0 * (ib + (long long)P1 * ic);
     const int j = b * L.sub + ((ic + L.LC) * L.PB + (ib + L.LB)) * (3 * L.PA) + (ia + L.LA);
-    const double m = mu[b] * scale;
+    const double m = mu[b] * scale * (L.mu_ratio ? L.mu_ratio[b + L.nb * cell] : 1.0);
 #pragma unroll
     for (int k = 0; k < 3; ++k) f[j + k * L.PA] = m * Hpad[(size_t)(b * 3 + k) * Ptot + p];
 }
@@ -160,7 +160,9 @@ __global__ void ddi_slab_scatter_kernel(const __grid_constant__ DevicePlan L, co
     const int ia = cell % L.Na, ib = (cell / L.Na) % L.Nb, ic = cell / (L.Na * L.Nb);
     const int j = ((ic + L.LC) * L.PB + (ib + L.LB)) * (3 * L.PA) + (ia + L.LA);
 #pragma unroll
-    for (int k = 0; k < 3; ++k) in[((size_t)ib * SL + (k * L.Nc + ic)) * P0 + ia] = mu * n[j + k * L.PA];
+    const double m = mu * (L.mu_ratio ? L.mu_ratio[cell] : 1.0);
+#pragma unroll
+    for (int k = 0; k < 3; ++k) in[((size_t)ib * SL + (k * L.Nc + ic)) * P0 + ia] = m * n[j + k * L.PA];
 }
 __global__ void ddi_slab_gather_kernel(const __grid_constant__ DevicePlan L, const double *__restrict__ out, int P0, int SL, double scale,
                                        double *__restrict__ f) {
@@ -169,7 +171,9 @@ __global__ void ddi_slab_gather_kernel(const __grid_constant__ DevicePlan L, con
     const int ia = cell % L.Na, ib = (cell / L.Na) % L.Nb, ic = cell / (L.Na * L.Nb);
     const int j = ((ic + L.LC) * L.PB + (ib + L.LB)) * (3 * L.PA) + (ia + L.LA);
 #pragma unroll
-    for (int k = 0; k < 3; ++k) f[j + k * L.PA] = scale * out[((size_t)ib * SL + (k * L.Nc + ic)) * P0 + ia];
+    const double m = scale * (L.mu_ratio ? L.mu_ratio[cell] : 1.0);
+#pragma unroll
+    for (int k = 0; k < 3; ++k) f[j + k * L.PA] = m * out[((size_t)ib * SL + (k * L.Nc + ic)) * P0 + ia];
 }
 
 
@@ -265,7 +269,12 @@ __global__ void __launch_bounds__(256) ddi_apass_fwd_kernel(const __grid_constan
     double2 *a = ddi_sm + (size_t)warp * 2 * MP, *b = a + MP;
     for (int j = lane; j < M; j += 32) {
         double2 v = make_double2(0.0, 0.0);
-        if (j < M / 2) { v = __ldg(src + j); v.x *= mu; v.y *= mu; }
+        if (j < M / 2) {
+            v = __ldg(src + j);
+            double m0 = mu, m1 = mu;
+            if (L.mu_ratio) { const double2 r = __ldg((const double2 *)(L.mu_ratio + (size_t)L.Na * (ib + (size_t)L.Nb * ic)) + j); m0 *= r.x; m1 *= r.y; }
+            v.x *= m0; v.y *= m1;
+        }
         a[ddi_pad(j)] = v;
     }
     __syncwarp();
@@ -302,7 +311,12 @@ __global__ void __launch_bounds__(256) ddi_apass_inv_kernel(const __grid_constan
     __syncwarp();
     const double2 *z = ddi_warp_fft<+1>(a, b, M, tw, lane);
     double2 *dst = (double2 *)(f + ((size_t)(ic + L.LC) * L.PB + (ib + L.LB)) * (3 * L.PA) + comp * L.PA + L.LA);
-    for (int j = lane; j < M / 2; j += 32) { const double2 v = z[ddi_pad(j)]; dst[j] = make_double2(scale * v.x, scale * v.y); }
+    for (int j = lane; j < M / 2; j += 32) {
+        const double2 v = z[ddi_pad(j)];
+        double m0 = scale, m1 = scale;
+        if (L.mu_ratio) { const double2 r = __ldg((const double2 *)(L.mu_ratio + (size_t)L.Na * (ib + (size_t)L.Nb * ic)) + j); m0 *= r.x; m1 *= r.y; }
+        dst[j] = make_double2(m0 * v.x, m1 * v.y);
+    }
 }
 
 // rank-0 case (a single cell): the "transform" of one point is the point itself

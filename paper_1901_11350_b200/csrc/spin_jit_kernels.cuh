@@ -12,7 +12,7 @@
 //
 // namespace spec must define (all constexpr):
 //   int NA, NB, NC, NBASIS, BX, BY, BZ;  int LA, LB, LC, PA, PB, PC, SUB, RA, RB, RC;  bool GA, GB, GC, PER_A, PER_B, PER_C;
-//   bool STORE_A, HAS_DDI, THERMAL_ON, STT_ON;
+//   bool STORE_A, HAS_DDI, THERMAL_ON, STT_ON, HAS_PIN, HAS_SITE_MU;
 //   int PAIR_BEGIN[NBASIS+1], P_DA[], P_DB[], P_DC[], P_BJ[];  double P_J[], P_DX[], P_DY[], P_DZ[];
 //   int QUAD_BEGIN[NBASIS+1], Q_D[][9], Q_B[][3];  double Q_K[];
 //   int ANI_BEGIN[NBASIS+1];  double ZEE[NBASIS][3], K2[n_ani], KAX[n_ani][3], PRE[NBASIS], SIGMA[NBASIS];
@@ -112,15 +112,22 @@ struct MidAcc {
 };
 
 // F += (Zeeman + anisotropy + pairs + quadruplets) of basis atom B for NCONF configurations sharing the lattice
+// zr: mu_i / mu_b of the site when per-site moments are set (spec::HAS_SITE_MU), the Zeeman force scales with it
 template <int B, int NCONF, class Acc>
-__device__ __forceinline__ void force(const Acc &cfg, const double (&own)[NCONF][3], double (&F)[NCONF][3]) {
+__device__ __forceinline__ void force(const Acc &cfg, const double (&own)[NCONF][3], double (&F)[NCONF][3], const double zr = 1.0) {
 #pragma unroll
     for (int k = 0; k < NCONF; ++k) {
         // spec:: holds the values as constexpr (zero terms vanish at compile time); specc:: holds the same values in constant
         // memory, from where an fp64 instruction reads them as an operand (a 64-bit immediate would cost two extra moves)
-        if constexpr (spec::ZEE[B][0] != 0.0) F[k][0] += specc::ZEE[B][0];
-        if constexpr (spec::ZEE[B][1] != 0.0) F[k][1] += specc::ZEE[B][1];
-        if constexpr (spec::ZEE[B][2] != 0.0) F[k][2] += specc::ZEE[B][2];
+        if constexpr (spec::HAS_SITE_MU) {
+            if constexpr (spec::ZEE[B][0] != 0.0) F[k][0] = fma(zr, specc::ZEE[B][0], F[k][0]);
+            if constexpr (spec::ZEE[B][1] != 0.0) F[k][1] = fma(zr, specc::ZEE[B][1], F[k][1]);
+            if constexpr (spec::ZEE[B][2] != 0.0) F[k][2] = fma(zr, specc::ZEE[B][2], F[k][2]);
+        } else {
+            if constexpr (spec::ZEE[B][0] != 0.0) F[k][0] += specc::ZEE[B][0];
+            if constexpr (spec::ZEE[B][1] != 0.0) F[k][1] += specc::ZEE[B][1];
+            if constexpr (spec::ZEE[B][2] != 0.0) F[k][2] += specc::ZEE[B][2];
+        }
         static_for<spec::ANI_BEGIN[B], spec::ANI_BEGIN[B + 1]>([&](auto ae) {      // every anisotropy axis of this atom (Eq. 1 sums over axes)
             constexpr int A = decltype(ae)::value;
             if constexpr (spec::K2[A] != 0.0) {
@@ -191,9 +198,10 @@ __device__ __forceinline__ void stt_gradient(const Acc &cfg, const Coord &c, con
 }
 
 // A = pre [F + alpha n x F] + stt_s s + stt_x n x s   (Eq. 10 as dn/dt = n x A)
+// ir: mu_b / mu_i of the site when per-site moments are set (the 1/mu_i of Eq. 10)
 template <int B>
-__device__ __forceinline__ void rotation_field(const double (&n)[3], const double (&F)[3], const double (&sg)[3], double (&A)[3]) {
-    const double pre = specc::PRE[B], pa = specc::PREA[B];
+__device__ __forceinline__ void rotation_field(const double (&n)[3], const double (&F)[3], const double (&sg)[3], double (&A)[3], const double ir = 1.0) {
+    const double pre = spec::HAS_SITE_MU ? specc::PRE[B] * ir : specc::PRE[B], pa = spec::HAS_SITE_MU ? specc::PREA[B] * ir : specc::PREA[B];
     const double cx = fma(n[1], F[2], -n[2] * F[1]), cy = fma(n[2], F[0], -n[0] * F[2]), cz = fma(n[0], F[1], -n[1] * F[0]);
     if constexpr (spec::DAMPING_ONLY) {      // :168 "only the damping part of the LLG equation": the solvers become minimisers
         A[0] = pa * cx; A[1] = pa * cy; A[2] = pa * cz;
@@ -247,6 +255,13 @@ __device__ __forceinline__ bool is_pinned(const unsigned char *__restrict__ pin,
     else return false;
 }
 
+// per-site moments ("atoms of different types"): mu_i / mu_b in boundary order, like the pinning flags
+template <int B>
+__device__ __forceinline__ double site_ratio(const double *__restrict__ mur, const Coord &c) {
+    if constexpr (spec::HAS_SITE_MU) return __ldg(mur + (B + spec::NBASIS * (c.ia + spec::NA * (c.ib + spec::NB * c.ic))));
+    else return 1.0;
+}
+
 // Programmatic dependent launch (spec::PDL; the host then launches the sweep with programmatic stream serialisation): let the next
 // kernel of the stream become resident as soon as every block of this one has started, and wait here -- before the first access to
 // anything another kernel writes -- until the previous kernel has completed and its stores are visible.  Semantics of the stream
@@ -261,8 +276,8 @@ __device__ __forceinline__ void pdl_exit() {
 
 template <int B, bool CG = false>
 __device__ __forceinline__ void predictor_body(const double *__restrict__ n, const double *__restrict__ fddi, double *__restrict__ np,
-                                               double *__restrict__ Aout, u64 step, u32 seed_lo, u32 seed_hi, const unsigned char *__restrict__ pin, int brick,
-                                               u32 image = 0u, double sigma_scale = 1.0) {
+                                               double *__restrict__ Aout, u64 step, u32 seed_lo, u32 seed_hi, const unsigned char *__restrict__ pin,
+                                               const double *__restrict__ mur, int brick, u32 image = 0u, double sigma_scale = 1.0) {
     Coord c;
     int idx;
     if (!locate<B>(c, idx, brick)) return;
@@ -271,15 +286,17 @@ __device__ __forceinline__ void predictor_body(const double *__restrict__ n, con
     double own[1][3], F[1][3], sg[1][3] = {{0.0, 0.0, 0.0}};
     load3<0, CG>(cfg.cfg[0], own[0]);
     if (is_pinned<B>(pin, c)) { store_spin(np + idx, c, own[0]); return; }
+    const double zr = site_ratio<B>(mur, c), ir = spec::HAS_SITE_MU ? 1.0 / zr : 1.0;
+    if constexpr (spec::HAS_SITE_MU && spec::THERMAL_ON) sigma_scale *= sqrt(zr);      // sigma_i ~ sqrt(mu_i) (Eq. 11)
     thermal_force<B>(c, step, seed_lo, seed_hi, F[0], image, sigma_scale);
     // the thermal field of the step is the same in both sweeps (R11): generating it costs two Philox blocks, two logarithms and three
     // trigonometric evaluations per spin, so the predictor keeps it for the corrector (24 B/spin written and read back)
     if constexpr (spec::CACHE_NOISE) store3(Aout + idx, F[0]);
-    force<B, 1>(cfg, own, F);
+    force<B, 1>(cfg, own, F, zr);
     if constexpr (spec::HAS_DDI) { double d[3]; load3<0, CG>(fddi + idx, d); F[0][0] += d[0]; F[0][1] += d[1]; F[0][2] += d[2]; }
     if constexpr (spec::STT_ON) stt_gradient<B, 1>(cfg, c, own, sg);
     double A[3], out[3];
-    rotation_field<B>(own[0], F[0], sg[0], A);
+    rotation_field<B>(own[0], F[0], sg[0], A, ir);
     if constexpr (spec::SOLVER == 0) spin::rodrigues(A, specc::DT, specc::DT2, own[0], out);                 // B5
     else if constexpr (spec::SOLVER == 1) { out[0] = own[0][0]; out[1] = own[0][1]; out[2] = own[0][2]; spin::heun_add(own[0], A, specc::DT, out); }   // B3
     else spin::imp_update(A, specc::HDT, own[0], out);                                                        // C5
@@ -290,14 +307,16 @@ __device__ __forceinline__ void predictor_body(const double *__restrict__ n, con
 template <int B, bool CG = false>
 __device__ __forceinline__ void corrector_body(const double *__restrict__ n, const double *__restrict__ np, const double *__restrict__ fddi_n,
                                                const double *__restrict__ fddi_np, const double *__restrict__ Ain, double *__restrict__ nout,
-                                               u64 step, u32 seed_lo, u32 seed_hi, const unsigned char *__restrict__ pin, int brick, u32 image = 0u,
-                                               double sigma_scale = 1.0) {
+                                               u64 step, u32 seed_lo, u32 seed_hi, const unsigned char *__restrict__ pin, const double *__restrict__ mur, int brick,
+                                               u32 image = 0u, double sigma_scale = 1.0) {
     Coord c;
     int idx;
     if (!locate<B>(c, idx, brick)) return;
     double th[3], A[3], Ap[3], n0[3];
     load3<0, CG>(n + idx, n0);
     if (is_pinned<B>(pin, c)) { store_spin(nout + idx, c, n0); return; }
+    const double zr = site_ratio<B>(mur, c), ir = spec::HAS_SITE_MU ? 1.0 / zr : 1.0;
+    if constexpr (spec::HAS_SITE_MU && spec::THERMAL_ON) sigma_scale *= sqrt(zr);
     if constexpr (spec::CACHE_NOISE) load3<0, CG>(Ain + idx, th);
     else thermal_force<B>(c, step, seed_lo, seed_hi, th, image, sigma_scale);
     if constexpr (spec::SOLVER == 2) {
@@ -305,14 +324,14 @@ __device__ __forceinline__ void corrector_body(const double *__restrict__ n, con
         const MidAcc<CG> cfg = {n + idx, np + idx};
         double own[1][3], F[1][3] = {{th[0], th[1], th[2]}}, sg[1][3] = {{0.0, 0.0, 0.0}};
         cfg.template load<B, B, 0, 0, 0>(0, own[0]);
-        force<B, 1>(cfg, own, F);
+        force<B, 1>(cfg, own, F, zr);
         if constexpr (spec::HAS_DDI) {      // the dipolar force is linear in the configuration: its value at the midpoint is the mean
             double d[3], e[3];
             load3<0, CG>(fddi_n + idx, d); load3<0, CG>(fddi_np + idx, e);
             F[0][0] += 0.5 * (d[0] + e[0]); F[0][1] += 0.5 * (d[1] + e[1]); F[0][2] += 0.5 * (d[2] + e[2]);
         }
         if constexpr (spec::STT_ON) stt_gradient<B, 1>(cfg, c, own, sg);
-        rotation_field<B>(own[0], F[0], sg[0], Ap);
+        rotation_field<B>(own[0], F[0], sg[0], Ap, ir);
         double out[3];
         spin::imp_update(Ap, specc::HDT, n0, out);
         store_spin(nout + idx, c, out);
@@ -324,10 +343,10 @@ __device__ __forceinline__ void corrector_body(const double *__restrict__ n, con
         cfg.cfg[0] = np + idx;
         double own[1][3], F[1][3] = {{th[0], th[1], th[2]}}, sg[1][3] = {{0.0, 0.0, 0.0}};
         load3<0, CG>(cfg.cfg[0], own[0]);
-        force<B, 1>(cfg, own, F);
+        force<B, 1>(cfg, own, F, zr);
         if constexpr (spec::HAS_DDI) { double d[3]; load3<0, CG>(fddi_np + idx, d); F[0][0] += d[0]; F[0][1] += d[1]; F[0][2] += d[2]; }
         if constexpr (spec::STT_ON) stt_gradient<B, 1>(cfg, c, own, sg);
-        rotation_field<B>(own[0], F[0], sg[0], Ap);
+        rotation_field<B>(own[0], F[0], sg[0], Ap, ir);
         load3<0, CG>(Ain + idx, A);
     } else if constexpr (spec::SPLIT_CORR) {
         // the two fields one after the other (fewer live registers, more resident warps) instead of interleaved
@@ -335,10 +354,10 @@ __device__ __forceinline__ void corrector_body(const double *__restrict__ n, con
             GlobalAcc<1, CG> cfg;
             cfg.cfg[0] = n + idx;
             double own[1][3] = {{n0[0], n0[1], n0[2]}}, F[1][3] = {{th[0], th[1], th[2]}}, sg[1][3] = {{0.0, 0.0, 0.0}};
-            force<B, 1>(cfg, own, F);
+            force<B, 1>(cfg, own, F, zr);
             if constexpr (spec::HAS_DDI) { double d[3]; load3<0, CG>(fddi_n + idx, d); F[0][0] += d[0]; F[0][1] += d[1]; F[0][2] += d[2]; }
             if constexpr (spec::STT_ON) stt_gradient<B, 1>(cfg, c, own, sg);
-            rotation_field<B>(own[0], F[0], sg[0], A);
+            rotation_field<B>(own[0], F[0], sg[0], A, ir);
         }
         {
             GlobalAcc<1, CG> cfg;
@@ -346,10 +365,10 @@ __device__ __forceinline__ void corrector_body(const double *__restrict__ n, con
             double own[1][3], F[1][3] = {{th[0], th[1], th[2]}}, sg[1][3] = {{0.0, 0.0, 0.0}};
             load3<0, CG>(cfg.cfg[0], own[0]);
             np0[0] = own[0][0]; np0[1] = own[0][1]; np0[2] = own[0][2];
-            force<B, 1>(cfg, own, F);
+            force<B, 1>(cfg, own, F, zr);
             if constexpr (spec::HAS_DDI) { double d[3]; load3<0, CG>(fddi_np + idx, d); F[0][0] += d[0]; F[0][1] += d[1]; F[0][2] += d[2]; }
             if constexpr (spec::STT_ON) stt_gradient<B, 1>(cfg, c, own, sg);
-            rotation_field<B>(own[0], F[0], sg[0], Ap);
+            rotation_field<B>(own[0], F[0], sg[0], Ap, ir);
         }
     } else {
         GlobalAcc<2, CG> cfg;
@@ -358,15 +377,15 @@ __device__ __forceinline__ void corrector_body(const double *__restrict__ n, con
         own[0][0] = n0[0]; own[0][1] = n0[1]; own[0][2] = n0[2];
         load3<0, CG>(cfg.cfg[1], own[1]);
         np0[0] = own[1][0]; np0[1] = own[1][1]; np0[2] = own[1][2];
-        force<B, 2>(cfg, own, F);
+        force<B, 2>(cfg, own, F, zr);
         if constexpr (spec::HAS_DDI) {
             double d[3];
             load3<0, CG>(fddi_n + idx, d); F[0][0] += d[0]; F[0][1] += d[1]; F[0][2] += d[2];
             load3<0, CG>(fddi_np + idx, d); F[1][0] += d[0]; F[1][1] += d[1]; F[1][2] += d[2];
         }
         if constexpr (spec::STT_ON) stt_gradient<B, 2>(cfg, c, own, sg);
-        rotation_field<B>(own[0], F[0], sg[0], A);
-        rotation_field<B>(own[1], F[1], sg[1], Ap);
+        rotation_field<B>(own[0], F[0], sg[0], A, ir);
+        rotation_field<B>(own[1], F[1], sg[1], Ap, ir);
     }
     double out[3];
     if constexpr (spec::SOLVER == 1) {
@@ -390,28 +409,31 @@ __device__ __forceinline__ void corrector_body(const double *__restrict__ n, con
 template <int B>
 __device__ __forceinline__ void rk4_stage_body(const double *__restrict__ base, const double *__restrict__ y, double *__restrict__ ynext,
                                                double *__restrict__ acc, double *__restrict__ noise, const double *__restrict__ fddi, int stage,
-                                               u64 step, u32 seed_lo, u32 seed_hi, const unsigned char *__restrict__ pin, int brick) {
+                                               u64 step, u32 seed_lo, u32 seed_hi, const unsigned char *__restrict__ pin, const double *__restrict__ mur,
+                                               int brick) {
     Coord c;
     int idx;
     if (!locate<B>(c, idx, brick)) return;
     double n0[3];
     load3<0>(base + idx, n0);
     if (is_pinned<B>(pin, c)) { store_spin(ynext + idx, c, n0); return; }
+    const double zr = site_ratio<B>(mur, c), ir = spec::HAS_SITE_MU ? 1.0 / zr : 1.0;
+    const double sscale = (spec::HAS_SITE_MU && spec::THERMAL_ON) ? sqrt(zr) : 1.0;
     GlobalAcc<1> cfg;
     cfg.cfg[0] = y + idx;
     double own[1][3], F[1][3], sg[1][3] = {{0.0, 0.0, 0.0}};
     load3<0>(cfg.cfg[0], own[0]);
     if constexpr (spec::THERMAL_ON && !spec::HAS_DDI) {      // generated once per step, kept for the other three stages
-        if (stage == 0) { thermal_force<B>(c, step, seed_lo, seed_hi, F[0]); store3(noise + idx, F[0]); }
+        if (stage == 0) { thermal_force<B>(c, step, seed_lo, seed_hi, F[0], 0u, sscale); store3(noise + idx, F[0]); }
         else load3<0>(noise + idx, F[0]);
     } else {
-        thermal_force<B>(c, step, seed_lo, seed_hi, F[0]);
+        thermal_force<B>(c, step, seed_lo, seed_hi, F[0], 0u, sscale);
     }
-    force<B, 1>(cfg, own, F);
+    force<B, 1>(cfg, own, F, zr);
     if constexpr (spec::HAS_DDI) { double d[3]; load3<0>(fddi + idx, d); F[0][0] += d[0]; F[0][1] += d[1]; F[0][2] += d[2]; }
     if constexpr (spec::STT_ON) stt_gradient<B, 1>(cfg, c, own, sg);
     double A[3], k[3] = {0.0, 0.0, 0.0};
-    rotation_field<B>(own[0], F[0], sg[0], A);
+    rotation_field<B>(own[0], F[0], sg[0], A, ir);
     spin::heun_add(own[0], A, 1.0, k);                      // k = y x A
     double a[3] = {0.0, 0.0, 0.0};
     if (stage > 0) load3<0>(acc + idx, a);
@@ -442,7 +464,7 @@ __device__ __forceinline__ void dispatch_basis(int b, Fn &&fn) {
 extern "C" __global__ void SPIN_BOUNDS(spec::BX *spec::BY *spec::BZ)
     jit_predictor(const double *__restrict__ n, const double *__restrict__ fddi, double *__restrict__ np, double *__restrict__ Aout,
                   const unsigned long long *__restrict__ d_step, unsigned int step_add, unsigned int seed_lo, unsigned int seed_hi,
-                  const unsigned char *__restrict__ pin, const double *__restrict__ img_sigma) {
+                  const unsigned char *__restrict__ pin, const double *__restrict__ img_sigma, const double *__restrict__ mu_ratio) {
     spinjit::pdl_entry();
     const unsigned long long step = *d_step + step_add;
     // batched images: blockIdx.z selects the image; every per-spin array holds the images one after the other
@@ -450,7 +472,7 @@ extern "C" __global__ void SPIN_BOUNDS(spec::BX *spec::BY *spec::BZ)
     const size_t off = spec::MULTI_IMAGE ? (size_t)image * ((size_t)spec::NBASIS * spec::SUB) : (size_t)0;
     const double scale = (spec::MULTI_IMAGE && img_sigma) ? img_sigma[image] : 1.0;
     spinjit::dispatch_basis<0>((int)blockIdx.y, [&](auto b) {
-        spinjit::predictor_body<decltype(b)::value>(n + off, fddi + off, np + off, Aout + off, step, seed_lo, seed_hi, pin, (int)blockIdx.x, image, scale);
+        spinjit::predictor_body<decltype(b)::value>(n + off, fddi + off, np + off, Aout + off, step, seed_lo, seed_hi, pin, mu_ratio, (int)blockIdx.x, image, scale);
     });
     spinjit::pdl_exit();
 }
@@ -459,7 +481,7 @@ extern "C" __global__ void SPIN_BOUNDS(spec::BX *spec::BY *spec::BZ)
     jit_corrector(const double *__restrict__ n, const double *__restrict__ np, const double *__restrict__ fddi_n,
                   const double *__restrict__ fddi_np, const double *__restrict__ Ain, double *__restrict__ nout,
                   const unsigned long long *__restrict__ d_step, unsigned int step_add, unsigned int seed_lo, unsigned int seed_hi,
-                  const unsigned char *__restrict__ pin, const double *__restrict__ img_sigma) {
+                  const unsigned char *__restrict__ pin, const double *__restrict__ img_sigma, const double *__restrict__ mu_ratio) {
     spinjit::pdl_entry();
     const unsigned long long step = *d_step + step_add;
     const unsigned int image = spec::MULTI_IMAGE ? blockIdx.z : 0u;
@@ -470,7 +492,7 @@ extern "C" __global__ void SPIN_BOUNDS(spec::BX *spec::BY *spec::BZ)
         // n^p) is still in the 126 MB L2 and is read first; it ends at brick 0, where the next predictor starts.
         const int brick = spec::REVERSE_CORR ? (int)(gridDim.x - 1u - blockIdx.x) : (int)blockIdx.x;
         spinjit::corrector_body<decltype(b)::value>(n + off, np + off, fddi_n + off, fddi_np + off, Ain + off, nout + off, step, seed_lo, seed_hi, pin,
-                                                    brick, image, scale);
+                                                    mu_ratio, brick, image, scale);
     });
     spinjit::pdl_exit();
 }
@@ -478,10 +500,11 @@ extern "C" __global__ void SPIN_BOUNDS(spec::BX *spec::BY *spec::BZ)
 extern "C" __global__ void SPIN_BOUNDS(spec::BX *spec::BY *spec::BZ)
     jit_rk4_stage(const double *__restrict__ base, const double *__restrict__ y, double *__restrict__ ynext, double *__restrict__ acc,
                   double *__restrict__ noise, const double *__restrict__ fddi, int stage, const unsigned long long *__restrict__ d_step,
-                  unsigned int step_add, unsigned int seed_lo, unsigned int seed_hi, const unsigned char *__restrict__ pin) {
+                  unsigned int step_add, unsigned int seed_lo, unsigned int seed_hi, const unsigned char *__restrict__ pin,
+                  const double *__restrict__ mu_ratio) {
     const unsigned long long step = *d_step + step_add;
     spinjit::dispatch_basis<0>((int)blockIdx.y, [&](auto b) {
-        spinjit::rk4_stage_body<decltype(b)::value>(base, y, ynext, acc, noise, fddi, stage, step, seed_lo, seed_hi, pin, (int)blockIdx.x);
+        spinjit::rk4_stage_body<decltype(b)::value>(base, y, ynext, acc, noise, fddi, stage, step, seed_lo, seed_hi, pin, mu_ratio, (int)blockIdx.x);
     });
 }
 
@@ -520,7 +543,7 @@ __device__ __forceinline__ void cluster_barrier() {
 template <class Barrier>
 __device__ __forceinline__ void all_steps(double *__restrict__ n0, double *__restrict__ n1, double *__restrict__ np, double *__restrict__ aux,
                                           u64 step0, unsigned int nsteps, u32 seed_lo, u32 seed_hi, const unsigned char *__restrict__ pin,
-                                          Barrier &&barrier) {
+                                          const double *__restrict__ mur, Barrier &&barrier) {
     constexpr int NBRICKS = ((spec::NA + spec::BX - 1) / spec::BX) * ((spec::NB + spec::BY - 1) / spec::BY) * ((spec::NC + spec::BZ - 1) / spec::BZ);
     for (unsigned int k = 0; k < nsteps; ++k) {
         const double *n = (k & 1u) ? n1 : n0;
@@ -528,12 +551,12 @@ __device__ __forceinline__ void all_steps(double *__restrict__ n0, double *__res
         const u64 step = step0 + k;
         for (int item = blockIdx.x; item < NBRICKS * spec::NBASIS; item += gridDim.x)
             dispatch_basis<0>(item / NBRICKS, [&](auto b) {
-                predictor_body<decltype(b)::value, true>(n, nullptr, np, aux, step, seed_lo, seed_hi, pin, item % NBRICKS);
+                predictor_body<decltype(b)::value, true>(n, nullptr, np, aux, step, seed_lo, seed_hi, pin, mur, item % NBRICKS);
             });
         barrier();
         for (int item = blockIdx.x; item < NBRICKS * spec::NBASIS; item += gridDim.x)
             dispatch_basis<0>(item / NBRICKS, [&](auto b) {
-                corrector_body<decltype(b)::value, true>(n, np, nullptr, nullptr, aux, nout, step, seed_lo, seed_hi, pin, item % NBRICKS);
+                corrector_body<decltype(b)::value, true>(n, np, nullptr, nullptr, aux, nout, step, seed_lo, seed_hi, pin, mur, item % NBRICKS);
             });
         barrier();
     }
@@ -543,15 +566,15 @@ __device__ __forceinline__ void all_steps(double *__restrict__ n0, double *__res
 extern "C" __global__ void SPIN_BOUNDS(spec::BX *spec::BY *spec::BZ)
     jit_steps_coop(double *__restrict__ n0, double *__restrict__ n1, double *__restrict__ np, double *__restrict__ aux,
                    const unsigned long long *__restrict__ d_step, unsigned int nsteps, unsigned int seed_lo, unsigned int seed_hi,
-                   const unsigned char *__restrict__ pin, unsigned int *bar) {
+                   const unsigned char *__restrict__ pin, unsigned int *bar, const double *__restrict__ mu_ratio) {
     unsigned int target = 0;
-    spinjit::all_steps(n0, n1, np, aux, *d_step, nsteps, seed_lo, seed_hi, pin, [&]() { spinjit::grid_barrier(bar, gridDim.x, target); });
+    spinjit::all_steps(n0, n1, np, aux, *d_step, nsteps, seed_lo, seed_hi, pin, mu_ratio, [&]() { spinjit::grid_barrier(bar, gridDim.x, target); });
 }
 
 // the same for lattices of at most 16 bricks: the whole grid is ONE thread-block cluster and the barrier is the cluster's hardware barrier
 extern "C" __global__ void SPIN_BOUNDS(spec::BX *spec::BY *spec::BZ)
     jit_steps_cluster(double *__restrict__ n0, double *__restrict__ n1, double *__restrict__ np, double *__restrict__ aux,
                       const unsigned long long *__restrict__ d_step, unsigned int nsteps, unsigned int seed_lo, unsigned int seed_hi,
-                      const unsigned char *__restrict__ pin) {
-    spinjit::all_steps(n0, n1, np, aux, *d_step, nsteps, seed_lo, seed_hi, pin, []() { spinjit::cluster_barrier(); });
+                      const unsigned char *__restrict__ pin, const double *__restrict__ mu_ratio) {
+    spinjit::all_steps(n0, n1, np, aux, *d_step, nsteps, seed_lo, seed_hi, pin, mu_ratio, []() { spinjit::cluster_barrier(); });
 }

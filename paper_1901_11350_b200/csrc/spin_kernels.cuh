@@ -70,6 +70,12 @@ __device__ __forceinline__ void store_spin(const DevicePlan &P, double *__restri
     }
 }
 
+// per-site moments: mu_i / mu_b of the site, 1 when none are set.  The moment enters the Zeeman force (x r), the prefactor
+// of Eq. 10 (/ r), the thermal amplitude (x sqrt r), the dipolar sums (x r on both sides) and the conversion to Tesla (/ r).
+__device__ __forceinline__ double mu_ratio(const DevicePlan &P, const Site &s) {
+    return P.mu_ratio != nullptr ? __ldg(P.mu_ratio + (s.b + P.nb * (s.ia + P.Na * (s.ib + P.Nb * s.ic)))) : 1.0;
+}
+
 // ---------------------------------------------------------------------------------------------------------
 // Short-range force of NCONF configurations that share the lattice (n and n^p in the corrector).
 template <int NCONF>
@@ -78,7 +84,9 @@ __device__ __forceinline__ void short_range_force(const DevicePlan &P, const dou
     const int b = s.b;
     if (mask & T_ZEE) {
 #pragma unroll
-        for (int c = 0; c < NCONF; ++c) { F[c][0] += P.zee[b][0]; F[c][1] += P.zee[b][1]; F[c][2] += P.zee[b][2]; }
+        const double r = mu_ratio(P, s);
+#pragma unroll
+        for (int c = 0; c < NCONF; ++c) { F[c][0] += r * P.zee[b][0]; F[c][1] += r * P.zee[b][1]; F[c][2] += r * P.zee[b][2]; }
     }
     if (mask & T_ANI) {
         for (int e = P.ani_begin[b]; e < P.ani_begin[b + 1]; ++e) {
@@ -146,8 +154,8 @@ __device__ __forceinline__ void stt_gradient(const DevicePlan &P, const double *
 // ---------------------------------------------------------------------------------------------------------
 // Eq. 10 as dn/dt = n x A:  A = pre [F + alpha n x F] + stt_s s + stt_x n x s
 __device__ __forceinline__ void rotation_field(const DevicePlan &P, int b, const double (&n)[3], const double (&F)[3],
-                                               const double (&sg)[3], double (&A)[3]) {
-    const double pre = P.pre[b], al = P.alpha;
+                                               const double (&sg)[3], double (&A)[3], double inv_ratio = 1.0) {
+    const double pre = P.pre[b] * inv_ratio, al = P.alpha;
     const double cx = n[1] * F[2] - n[2] * F[1], cy = n[2] * F[0] - n[0] * F[2], cz = n[0] * F[1] - n[1] * F[0];
     const double pr = P.damping_only ? 0.0 : 1.0;      // :168 "only the damping part of the LLG equation"
     A[0] = pre * (pr * F[0] + al * cx);
@@ -166,7 +174,8 @@ __device__ __forceinline__ void thermal_force(const DevicePlan &P, const Site &s
     if (P.thermal_on) {
         const unsigned int cell = (unsigned int)(s.ia + P.Na * (s.ib + P.Nb * s.ic));
         thermal_xi(P.seed_lo, P.seed_hi, step, (unsigned int)s.b + (unsigned int)P.nb * cell, f);
-        const double sg = P.sigma[s.b];
+        double sg = P.sigma[s.b];
+        if (P.mu_ratio != nullptr) sg *= sqrt(mu_ratio(P, s));
         f[0] *= sg; f[1] *= sg; f[2] *= sg;
     }
 }
@@ -194,7 +203,7 @@ __global__ void __launch_bounds__(BX *BY *BZ)
     if (P.has_ddi) { double d[3]; load3(P, fddi, s.idx, d); F[0][0] += d[0]; F[0][1] += d[1]; F[0][2] += d[2]; }
     if (P.stt_on) stt_gradient<1>(P, cfg, s, own, sg);
     double A[3], out[3];
-    rotation_field(P, s.b, own[0], F[0], sg[0], A);
+    rotation_field(P, s.b, own[0], F[0], sg[0], A, P.mu_ratio != nullptr ? 1.0 / mu_ratio(P, s) : 1.0);
     rodrigues(A, P.dt, P.dt2, own[0], out);
     store_spin(P, np, s.ia, s.ib, s.ic, s.idx, out);
     if (STORE_A) store3(P, Aout, s.idx, A);
@@ -220,7 +229,7 @@ __global__ void __launch_bounds__(BX *BY *BZ)
         short_range_force<1>(P, cfg, s, own, T_ALL, F);
         if (P.has_ddi) { double d[3]; load3(P, fddi_np, s.idx, d); F[0][0] += d[0]; F[0][1] += d[1]; F[0][2] += d[2]; }
         if (P.stt_on) stt_gradient<1>(P, cfg, s, own, sg);
-        rotation_field(P, s.b, own[0], F[0], sg[0], Ap);
+        rotation_field(P, s.b, own[0], F[0], sg[0], Ap, P.mu_ratio != nullptr ? 1.0 / mu_ratio(P, s) : 1.0);
         load3(P, Ain, s.idx, A);
     } else {
         const double *const cfg[2] = {n, np};
@@ -234,8 +243,8 @@ __global__ void __launch_bounds__(BX *BY *BZ)
             load3(P, fddi_np, s.idx, d); F[1][0] += d[0]; F[1][1] += d[1]; F[1][2] += d[2];
         }
         if (P.stt_on) stt_gradient<2>(P, cfg, s, own, sg);
-        rotation_field(P, s.b, own[0], F[0], sg[0], A);
-        rotation_field(P, s.b, own[1], F[1], sg[1], Ap);
+        rotation_field(P, s.b, own[0], F[0], sg[0], A, P.mu_ratio != nullptr ? 1.0 / mu_ratio(P, s) : 1.0);
+        rotation_field(P, s.b, own[1], F[1], sg[1], Ap, P.mu_ratio != nullptr ? 1.0 / mu_ratio(P, s) : 1.0);
     }
     const double Ac[3] = {0.5 * (A[0] + Ap[0]), 0.5 * (A[1] + Ap[1]), 0.5 * (A[2] + Ap[2])};
     double out[3];
@@ -275,7 +284,8 @@ __global__ void unpack_kernel(const __grid_constant__ DevicePlan P, const double
     boundary_to_site(P, i, b, ia, ib, ic, idx);
     double v[3];
     load3(P, src, idx, v);
-    const double sc = scale_by_inv_mu ? P.inv_mu[b] : 1.0;
+    double sc = scale_by_inv_mu ? P.inv_mu[b] : 1.0;
+    if (scale_by_inv_mu && P.mu_ratio != nullptr) sc /= P.mu_ratio[i];
     aos[3 * (size_t)i] = sc * v[0]; aos[3 * (size_t)i + 1] = sc * v[1]; aos[3 * (size_t)i + 2] = sc * v[2];
 }
 

@@ -85,6 +85,7 @@ struct DevicePlan {
     int thermal_on;
     int damping_only;                        // 1: the precession term of Eq. 10 is dropped (:168)
     const unsigned char *pin;                // N flags in boundary order (b + nb*cell) or null: pinned spins are never updated
+    const double *mu_ratio;                  // N ratios mu_i / mu_b(i) in boundary order or null: per-site moments ("atoms of different types")
     PairEntry pairs[SPIN_MAX_PAIR_ENTRIES];
     QuadEntry quads[SPIN_MAX_QUAD_ENTRIES];
 };
@@ -130,6 +131,8 @@ struct spin_system {
     double *d_result;              // reduction result (16 doubles)
     unsigned long long *d_step;    // device copy of the step counter (read by the kernels)
     unsigned char *d_pin;          // pinned-spin flags (boundary order), null if none
+    std::vector<double> mu_site;   // per-site moments in mu_B (boundary order), empty if none
+    double *d_mu_ratio;            // mu_i / mu_b(i) on the device (rebuilt with the plan: the basis moments may change), null if none
     // ---- batched images: n_img independent configurations of the same lattice and Hamiltonian; every per-spin array holds them
     // one after the other (stride nb * plan.sub doubles); the sweeps take the image from blockIdx.z
     int n_img, img_sel;            // number of images; image that spins_set/get, effective_field, energy, ... address

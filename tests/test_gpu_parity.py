@@ -818,9 +818,11 @@ def test_randomised_systems(P, O, seed):
     N = g.N
     n0 = rng.standard_normal((N, 3)); n0 /= np.linalg.norm(n0, axis=1, keepdims=True)
     mask = (rng.random(N) < 0.1).astype(np.uint8)
+    site_mu = rng.uniform(0.5, 3.0, N) if seed % 2 else None      # atoms of different types on every other system
     for s_ in (g, h):
         s_.spins_set_pinned(mask); s_.spins_set(n0)
-    o.set_pinned(mask); o.set_spins(n0)
+        s_.hamiltonian_set_site_mu_s(site_mu)
+    o.set_pinned(mask); o.set_spins(n0); o.set_site_mu_s(site_mu)
     Bo = o.effective_field()
     assert_fields_close(g.effective_field(), Bo)
     To = o.energy_terms()
@@ -833,6 +835,57 @@ def test_randomised_systems(P, O, seed):
     h.llg_iterate(25)                                    # table-driven Depondt
     if solver == 0:
         assert np.abs(h.spins_get() - o.spins()).max() <= SPIN_ATOL
+
+
+# Atoms of different types: one moment per site, on every config's replica (thermal field, two
+# sublattices + current, dipolar coupling on the 3-D, slab and hand-written-a-pass paths, all-steps-in-one-launch kernels) and every solver
+@pytest.mark.parametrize("cfg,cells,steps", [(1, (33, 17, 1), 100), (2, (45, 33, 1), 100), (3, (35, 9, 7), 60), (4, (33, 17, 1), 60), (5, (20, 12, 5), 10),
+                                             (5, (32, 12, 4), 10), (5, (9, 7, 5), 10), (3, (64, 32, 16), 32)])
+def test_site_moments_match_oracle(P, O, cfg, cells, steps):
+    w = W.CONFIGS[cfg]().resized(cells, steps)
+    if cfg == 5 and cells == (9, 7, 5):
+        w = dataclasses.replace(w, periodic=(1, 1, 1), ddi_images=(1, 1, 1))      # the general 3-D dipolar path
+    g, o = pair(P, O, w)
+    rng = np.random.default_rng(77 + cfg)
+    mu = rng.uniform(0.5, 4.0, g.N)
+    g.hamiltonian_set_site_mu_s(mu); o.set_site_mu_s(mu)
+    Bo = o.effective_field()
+    assert_fields_close(g.effective_field(), Bo)
+    To = o.energy_terms()
+    assert np.abs(g.energy()[1] - To).max() <= ENERGY_RTOL * np.abs(To).sum()
+    Mg, tg = g.observables(); Mo, to = o.observables()
+    assert np.abs(Mg - Mo).max() < 1e-13 and abs(tg - to) <= 1e-12 * to
+    g.llg_iterate(steps); o.iterate(steps)
+    assert np.abs(g.spins_get() - o.spins()).max() <= SPIN_ATOL
+    # the table-driven kernels, and every other solver on the specialised ones
+    h = P.SpinSystem.from_workload(w); h.spin_set_option("use_jit", 0); h.hamiltonian_set_site_mu_s(mu)
+    h.llg_iterate(steps)
+    assert np.abs(h.spins_get() - o.spins()).max() <= SPIN_ATOL
+    for solver in (1, 2, 3):
+        g2, o2 = pair(P, O, w)
+        g2.hamiltonian_set_site_mu_s(mu); o2.set_site_mu_s(mu)
+        g2.llg_set_solver(solver); o2.set_solver(solver)
+        k = min(steps, 20)
+        g2.llg_iterate(k); o2.iterate(k)
+        assert np.abs(g2.spins_get() - o2.spins()).max() <= SPIN_ATOL, solver
+    # cleared: the basis atoms' moments again, bit for bit what a system that never had per-site moments gives
+    g.hamiltonian_set_site_mu_s(None)
+    g.spins_set(w.initial_spins()); g.llg_set_step(0); g.llg_iterate(8)
+    r = P.SpinSystem.from_workload(w); r.llg_iterate(8)
+    assert np.array_equal(g.spins_get(), r.spins_get())
+    # changing the basis moment afterwards keeps the per-site moments absolute
+    g.hamiltonian_set_site_mu_s(mu); g.hamiltonian_set_mu_s(np.asarray(w.mu_s) * 1.7)
+    g.spins_set(w.initial_spins())
+    o3 = O.OracleSystem.from_workload(w); o3.set_site_mu_s(mu)
+    assert_fields_close(g.effective_field(), o3.effective_field())
+
+
+def test_site_moments_reject_bad_values(P):
+    s = P.SpinSystem(np.eye(3), [[0, 0, 0]], (4, 4, 1), (1, 1, 0))
+    with pytest.raises(P.SpinError):
+        s.hamiltonian_set_site_mu_s(np.r_[np.ones(15), 0.0])
+    with pytest.raises(P.SpinError):
+        s.hamiltonian_set_site_mu_s(np.r_[np.ones(15), np.nan])
 
 
 def test_biaxial_anisotropy_several_axes_per_atom(P, O):
