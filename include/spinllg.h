@@ -181,6 +181,29 @@ int observables(spin_system *sys, double M[3], double *max_torque_meV);
  * One basis atom (SPIN_ERR_ARG otherwise).  Periodic directions wrap; triangles leaving an open edge are skipped (:343).  */
 int topological_charge(spin_system *sys, double *Q);
 
+/* ---- slab decomposition along c over several GPUs (SURVEY 8(e); the paper has no counterpart: MPI only as a scripting remark, :143) ----
+ * One process per GPU holds `n_cells[2]` consecutive planes of a lattice of `global_cells_c` planes, starting at plane `c_offset`.  Its
+ * ghost layers along c (as wide as the Hamiltonian reaches along c) are then NOT its own periodic images but its neighbours' boundary
+ * planes, delivered by a halo exchange before every sweep (twice per step: n, then n^p); translations along c are folded with the global
+ * extent and boundary condition, and the thermal field is keyed by the GLOBAL spin index, so N slabs reproduce the single-GPU trajectory
+ * bit for bit.  The library provides the pieces below; paper_1901_11350_b200/slab.py orders them and owns the transport
+ * (torch.distributed / NCCL, or device copies between slabs of one process).  Not with the dipolar term (its transform needs all-to-all
+ * transposes), batched images, RK4, or a current with a component along c.                                                          */
+int spin_set_slab(spin_system *sys, int enabled, int c_offset, int global_cells_c, int global_periodic_c);
+/* doubles held by one side of the halo: reach along c x padded plane x sublattices (contiguous, sublattice-major); reach_c (may be
+ * NULL) receives the reach = number of planes per side                                                                              */
+int spin_halo_doubles(spin_system *sys, int64_t *doubles_per_side, int *reach_c);
+/* array: 0 the current configuration n, 1 the predictor n^p, 2 the next configuration (corrector output, before llg_slab_advance);
+ * side: 0 towards lower c, 1 towards higher c.  get copies the outermost OWN planes of that side to dst (DEVICE pointer); put copies src
+ * (DEVICE pointer) into the GHOST planes of that side.  Enqueued on cuda_stream (NULL: the system's stream), never synchronised.     */
+int spin_halo_get(spin_system *sys, int array, int side, double *dst_device, void *cuda_stream);
+int spin_halo_put(spin_system *sys, int array, int side, const double *src_device, void *cuda_stream);
+/* one sweep of the current step over part of the slab: stage 0 predictor, 1 corrector; part 0 all bricks, 1 the brick layers a neighbour
+ * needs (within reach of either face), 2 the layers in between (launched while the halos of part 1 travel)                          */
+int llg_slab_sweep(spin_system *sys, int stage, int part);
+/* after the corrector sweeps: the next configuration becomes current, the step counter (noise stream) advances by one             */
+int llg_slab_advance(spin_system *sys);
+
 /* ---- execution options ------------------------------------------------------------------------------------------------
  * spin_set_option(name, value) changes how the path is executed, never what it computes (every combination is bit-identical; tested).
  * The defaults are the measured choices; the options exist for A/B measurements and for the tests.

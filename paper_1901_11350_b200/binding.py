@@ -22,6 +22,7 @@ EXPORTS = [
     "hamiltonian_set_ddi", "spin_set_images", "spin_select_image", "llg_set_image_temperatures", "gneb_forces", "gneb_iterate", "spins_set_pinned", "spins_set", "spins_get", "spins_set_device", "spins_get_device",
     "llg_configure", "llg_set_solver", "llg_set_damping_only", "minimise_vp", "minimise_vp_reset", "llg_iterate", "llg_get_step", "llg_set_step", "spin_synchronize",
     "effective_field", "effective_field_device", "energy", "observables", "topological_charge",
+    "spin_set_slab", "spin_halo_doubles", "spin_halo_get", "spin_halo_put", "llg_slab_sweep", "llg_slab_advance",
     "spin_launch_counts", "spin_measure_fp64_tflops", "spin_profile_enable", "spin_profile_get", "spin_set_option",
     "spin_kernel_info", "spin_ddi_info", "spin_jit_compiler_info", "spin_jit_source", "spin_last_error", "spin_version",
 ]
@@ -84,6 +85,12 @@ def lib() -> C.CDLL:
         "observables": (C.c_int, [vp, dp, dp]),
         "topological_charge": (C.c_int, [vp, dp]),
         "spin_launch_counts": (C.c_int, [vp, i64p, i64p]),
+        "spin_set_slab": (C.c_int, [vp, C.c_int, C.c_int, C.c_int, C.c_int]),
+        "spin_halo_doubles": (C.c_int, [vp, i64p, ip]),
+        "spin_halo_get": (C.c_int, [vp, C.c_int, C.c_int, vp, vp]),
+        "spin_halo_put": (C.c_int, [vp, C.c_int, C.c_int, vp, vp]),
+        "llg_slab_sweep": (C.c_int, [vp, C.c_int, C.c_int]),
+        "llg_slab_advance": (C.c_int, [vp]),
         "spin_profile_enable": (C.c_int, [vp, C.c_int]),
         "spin_profile_get": (C.c_int, [vp, C.c_int, dp, i64p]),
         "spin_set_option": (C.c_int, [vp, C.c_char_p, C.c_int]),
@@ -330,6 +337,28 @@ class SpinSystem:
         mt = C.c_double(0.0)
         _check(lib().observables(self._h, M.ctypes.data_as(C.POINTER(C.c_double)), C.byref(mt)))
         return M, float(mt.value)
+
+    # ---- slab decomposition (device pointers and streams are plain integers here: torch's data_ptr() / cuda_stream)
+    def spin_set_slab(self, enabled, c_offset=0, global_cells_c=0, global_periodic_c=0):
+        _check(lib().spin_set_slab(self._h, int(bool(enabled)), int(c_offset), int(global_cells_c), int(bool(global_periodic_c))))
+
+    def spin_halo_doubles(self):
+        """(doubles per side of the halo, reach along c in planes)"""
+        n, r = C.c_int64(0), C.c_int(0)
+        _check(lib().spin_halo_doubles(self._h, C.byref(n), C.byref(r)))
+        return int(n.value), int(r.value)
+
+    def spin_halo_get(self, array, side, dst_device_ptr, stream=0):
+        _check(lib().spin_halo_get(self._h, int(array), int(side), C.c_void_p(int(dst_device_ptr)), C.c_void_p(int(stream) or None)))
+
+    def spin_halo_put(self, array, side, src_device_ptr, stream=0):
+        _check(lib().spin_halo_put(self._h, int(array), int(side), C.c_void_p(int(src_device_ptr)), C.c_void_p(int(stream) or None)))
+
+    def llg_slab_sweep(self, stage, part=0):
+        _check(lib().llg_slab_sweep(self._h, int(stage), int(part)))
+
+    def llg_slab_advance(self):
+        _check(lib().llg_slab_advance(self._h))
 
     def spin_launch_counts(self):
         a, b = C.c_int64(0), C.c_int64(0)

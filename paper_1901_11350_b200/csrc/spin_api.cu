@@ -206,7 +206,10 @@ int build_plan(const spin_system *s, DevicePlan &P) {
     all.insert(all.end(), s->pairs_explicit.begin(), s->pairs_explicit.end());
     all.insert(all.end(), s->pairs_exch_shells.begin(), s->pairs_exch_shells.end());
     all.insert(all.end(), s->pairs_dmi_shells.begin(), s->pairs_dmi_shells.end());
-    const int Nd[3] = {s->nc[0], s->nc[1], s->nc[2]};
+    // slab decomposition: translations along c are folded with the extent and boundary condition of the WHOLE lattice; the partner planes
+    // outside this slab are its ghost layers, filled by the halo exchange
+    const int Nd[3] = {s->nc[0], s->nc[1], s->slab_on ? s->slab_gnc : s->nc[2]};
+    const int perd[3] = {s->per[0], s->per[1], s->slab_on ? s->slab_gper : s->per[2]};
     int ne = 0;
     for (int b = 0; b < s->nb; ++b) {
         P.pair_begin[b] = ne;
@@ -219,8 +222,8 @@ int build_plan(const spin_system *s, DevicePlan &P) {
                 int t[3];
                 bool dead = false;
                 for (int d = 0; d < 3; ++d) {
-                    t[d] = reduce_translation((dir == 0 ? 1 : -1) * p.t[d], Nd[d], s->per[d]);
-                    if (!s->per[d] && abs(t[d]) >= Nd[d]) dead = true;      // never inside an open lattice
+                    t[d] = reduce_translation((dir == 0 ? 1 : -1) * p.t[d], Nd[d], perd[d]);
+                    if (!perd[d] && abs(t[d]) >= Nd[d]) dead = true;      // never inside an open lattice
                 }
                 if (dead) continue;
                 e.da = t[0]; e.db = t[1]; e.dc = t[2];
@@ -261,8 +264,8 @@ int build_plan(const spin_system *s, DevicePlan &P) {
                 bool dead = false;
                 for (int m = 0; m < 3; ++m) {
                     for (int d = 0; d < 3; ++d) {
-                        const int t = reduce_translation(tm[mem[m]][d] - tm[role][d], Nd[d], s->per[d]);
-                        if (!s->per[d] && abs(t) >= Nd[d]) dead = true;
+                        const int t = reduce_translation(tm[mem[m]][d] - tm[role][d], Nd[d], perd[d]);
+                        if (!perd[d] && abs(t) >= Nd[d]) dead = true;
                         e.d[m][d] = t;
                     }
                     e.b[m] = q.b[mem[m]];
@@ -279,7 +282,13 @@ int build_plan(const spin_system *s, DevicePlan &P) {
     P.quad_begin[s->nb] = nq;
     // ---- layout with ghost cells (spinllg_internal.h): ghost width = reach; rows start on 128-byte lines
     P.rA = reach[0]; P.rB = reach[1]; P.rC = reach[2];
-    P.gA = (P.perA && P.rA > 0) ? 1 : 0; P.gB = (P.perB && P.rB > 0) ? 1 : 0; P.gC = (P.perC && P.rC > 0) ? 1 : 0;
+    P.gA = (P.perA && P.rA > 0) ? 1 : 0; P.gB = (P.perB && P.rB > 0) ? 1 : 0; P.gC = (P.perC && P.rC > 0 && !s->slab_on) ? 1 : 0;
+    if (s->slab_on) {
+        if (P.rC > P.Nc) return spin::fail(SPIN_ERR_ARG, "slab of %d planes is thinner than the reach %d of the Hamiltonian along c", P.Nc, P.rC);
+        if (P.stt_on && P.stt_c[2] != 0.0) return spin::fail(SPIN_ERR_STATE, "slab decomposition needs an in-plane current (no component along c)");
+        if (s->ddi_on) return spin::fail(SPIN_ERR_STATE, "the dipolar transform does not decompose into slabs (DESIGN.md section 8)");
+        P.cell_off = s->slab_off * P.Na * P.Nb;
+    }
     P.LA = (P.rA + 15) / 16 * 16; P.LB = P.rB; P.LC = P.rC;
     P.PA = P.LA + (P.Na + P.rA + 15) / 16 * 16; P.PB = P.Nb + 2 * P.rB; P.PC = P.Nc + 2 * P.rC;
     const int64_t sub = (int64_t)3 * P.PA * P.PB * P.PC;
@@ -542,6 +551,7 @@ extern "C" int spin_geometry_create(const double bravais[9], int n_basis, const 
     s->stream = nullptr; s->own_stream = nullptr; s->cur = 0;
     s->d_n[0] = s->d_n[1] = s->d_np = s->d_A = s->d_fddi[0] = s->d_fddi[1] = s->d_aos = s->d_partials = s->d_result = nullptr;
     s->d_vp = nullptr; s->vp_active = false; s->vp_cur = 0;
+    s->slab_on = 0; s->slab_off = 0; s->slab_gnc = 0; s->slab_gper = 0;
     s->d_step = nullptr; s->d_pin = nullptr; s->d_mu_ratio = nullptr; s->ddi = nullptr; s->plan_dirty = true;
     s->opt_graph = 1; s->opt_store_A = 0; s->graph_exec[0] = s->graph_exec[1] = nullptr; s->graph_steps = 0;
     s->n_launch = s->n_fft = 0; s->profile_on = 0;
@@ -908,6 +918,7 @@ extern "C" int llg_iterate(spin_system *s, int64_t n_steps) {
     REQUIRE(s && n_steps >= 0, "bad argument");
     int rc = ensure_plan(s);
     if (rc) return rc;
+    if (s->slab_on) return spin::fail(SPIN_ERR_STATE, "a slab advances through llg_slab_sweep / spin_halo_* / llg_slab_advance (its ghost layers need the halo exchange)");
     s->vp_active = false;
     if (s->n_img > 1 && (!jit_ready(s) || s->solver == SPIN_SOLVER_RK4))
         return spin::fail(SPIN_ERR_STATE, "batched images need the run-time specialised kernels and a two-stage solver (%s)", s->jit_note.c_str());
@@ -971,6 +982,112 @@ extern "C" int llg_iterate(spin_system *s, int64_t n_steps) {
         s->n_launch++;
     }
     s->step += (uint64_t)n_steps;
+    SPIN_CUDA(cudaGetLastError());
+    return SPIN_OK;
+}
+
+// ---------------------------------------------------------------------------------------------- slab decomposition along c
+// Several GPUs share one lattice: each holds a slab of planes and the ghost layers along c are filled by a halo exchange before every
+// sweep.  The library provides the pieces -- the ghost-aware plan, sweeps over brick ranges, the halo
+// planes as contiguous device chunks; the driver (paper_1901_11350_b200/slab.py) orders them and owns the transport (NCCL / peer copies).
+extern "C" int spin_set_slab(spin_system *s, int enabled, int c_offset, int global_cells_c, int global_periodic_c) {
+    REQUIRE(s, "null system");
+    if (!enabled) { s->slab_on = 0; s->slab_off = 0; s->slab_gnc = 0; s->slab_gper = 0; s->plan_dirty = true; drop_graphs(s); return SPIN_OK; }
+    REQUIRE(global_cells_c >= s->nc[2] && c_offset >= 0 && c_offset + s->nc[2] <= global_cells_c, "slab [%d, %d) does not lie inside %d planes", c_offset,
+            c_offset + s->nc[2], global_cells_c);
+    REQUIRE(s->n_img == 1, "slab decomposition and batched images are separate axes of parallelism");
+    s->slab_on = 1; s->slab_off = c_offset; s->slab_gnc = global_cells_c; s->slab_gper = global_periodic_c ? 1 : 0;
+    s->plan_dirty = true;
+    drop_graphs(s);
+    return SPIN_OK;
+}
+namespace {
+// the per-spin array a halo call addresses: 0 the current configuration n, 1 the predictor n^p, 2 the next configuration (corrector output)
+double *slab_array(spin_system *s, int array) { return array == 0 ? s->d_n[s->cur] : (array == 1 ? s->d_np : s->d_n[s->cur ^ 1]); }
+int slab_ready(spin_system *s) {
+    int rc = ensure_plan(s);
+    if (rc) return rc;
+    if (!s->slab_on) return spin::fail(SPIN_ERR_STATE, "not a slab: call spin_set_slab first");
+    if (!jit_ready(s)) return spin::fail(SPIN_ERR_STATE, "slab sweeps need the run-time specialised kernels (%s)", s->jit_note.c_str());
+    if (s->solver == SPIN_SOLVER_RK4) return spin::fail(SPIN_ERR_STATE, "slab sweeps are the two-stage solvers (Depondt, Heun, SIB)");
+    return SPIN_OK;
+}
+}  // namespace
+// doubles one side of the halo holds: reach along c x padded plane (ghost rows and columns included: they carry the in-plane images) x sublattices
+extern "C" int spin_halo_doubles(spin_system *s, int64_t *doubles_per_side, int *reach_c) {
+    REQUIRE(s && doubles_per_side, "null argument");
+    int rc = slab_ready(s);
+    if (rc) return rc;
+    *doubles_per_side = (int64_t)s->nb * s->plan.rC * 3 * s->plan.PA * s->plan.PB;
+    if (reach_c) *reach_c = s->plan.rC;
+    return SPIN_OK;
+}
+// side 0 / 1 = towards lower / higher c.  get: the rC outermost OWN planes on that side -> dst (device, contiguous, sublattice-major);
+// put: src -> the rC GHOST planes on that side.  Copies are enqueued on `stream` (NULL: the system's stream); nothing is synchronised.
+extern "C" int spin_halo_get(spin_system *s, int array, int side, double *dst_device, void *stream) {
+    REQUIRE(s && dst_device && array >= 0 && array <= 2 && (side == 0 || side == 1), "bad argument");
+    int rc = slab_ready(s);
+    if (rc) return rc;
+    const DevicePlan &P = s->plan;
+    const size_t plane = (size_t)3 * P.PA * P.PB, chunk = plane * P.rC;
+    const size_t first = (size_t)(side == 0 ? P.LC : P.LC + P.Nc - P.rC) * plane;
+    cudaStream_t st = stream ? (cudaStream_t)stream : s->stream;
+    for (int b = 0; b < s->nb; ++b)
+        SPIN_CUDA(cudaMemcpyAsync(dst_device + (size_t)b * chunk, slab_array(s, array) + (size_t)b * P.sub + first, chunk * sizeof(double), cudaMemcpyDeviceToDevice, st));
+    return SPIN_OK;
+}
+extern "C" int spin_halo_put(spin_system *s, int array, int side, const double *src_device, void *stream) {
+    REQUIRE(s && src_device && array >= 0 && array <= 2 && (side == 0 || side == 1), "bad argument");
+    int rc = slab_ready(s);
+    if (rc) return rc;
+    const DevicePlan &P = s->plan;
+    const size_t plane = (size_t)3 * P.PA * P.PB, chunk = plane * P.rC;
+    const size_t first = (size_t)(side == 0 ? P.LC - P.rC : P.LC + P.Nc) * plane;
+    cudaStream_t st = stream ? (cudaStream_t)stream : s->stream;
+    for (int b = 0; b < s->nb; ++b)
+        SPIN_CUDA(cudaMemcpyAsync(slab_array(s, array) + (size_t)b * P.sub + first, src_device + (size_t)b * chunk, chunk * sizeof(double), cudaMemcpyDeviceToDevice, st));
+    return SPIN_OK;
+}
+// One sweep of the current step over part of the slab: stage 0 predictor (n -> n^p), 1 corrector (n, n^p -> next n);
+// part 0 every brick, 1 the brick layers that hold planes a neighbour needs (within the reach of either face), 2 the layers in between.
+// The driver launches part 1, starts the halo copies of its output, and launches part 2 while they travel.
+extern "C" int llg_slab_sweep(spin_system *s, int stage, int part) {
+    REQUIRE(s && (stage == 0 || stage == 1) && part >= 0 && part <= 2, "bad argument");
+    int rc = slab_ready(s);
+    if (rc) return rc;
+    s->vp_active = false;
+    const DevicePlan &P = s->plan;
+    int b[3];
+    jit_brick_shape(s, b);
+    const int per_layer = ((P.Na + b[0] - 1) / b[0]) * ((P.Nb + b[1] - 1) / b[1]), layers = (P.Nc + b[2] - 1) / b[2];
+    const int lo_end = std::min(layers, (P.rC + b[2] - 1) / b[2]), hi_begin = std::max(lo_end, (P.Nc - P.rC) / b[2]);      // boundary layers: [0, lo_end) and [hi_begin, layers)
+    int ranges[2][2] = {{0, 0}, {0, 0}};
+    if (part == 0) { ranges[0][0] = 0; ranges[0][1] = layers; }
+    else if (part == 1) { ranges[0][0] = 0; ranges[0][1] = lo_end; ranges[1][0] = hi_begin; ranges[1][1] = layers; }
+    else { ranges[0][0] = lo_end; ranges[0][1] = hi_begin; }
+    double *n = s->d_n[s->cur], *nout = s->d_n[s->cur ^ 1];
+    const Launch L = brick_launch(s);
+    for (int r = 0; r < 2; ++r) {
+        const int nl = ranges[r][1] - ranges[r][0];
+        if (nl <= 0) continue;
+        const unsigned brick0 = (unsigned)(ranges[r][0] * per_layer), count = (unsigned)(nl * per_layer);
+        rc = stage == 0 ? jit_launch_predictor(s, L.grid, L.block, n, s->d_fddi[0], s->d_np, s->d_A, 0u, brick0, count)
+                        : jit_launch_corrector(s, L.grid, L.block, n, s->d_np, s->d_fddi[0], s->d_fddi[1], s->d_A, nout, 0u, brick0, count);
+        if (rc) return rc;
+        s->n_launch++;
+    }
+    SPIN_CUDA(cudaGetLastError());
+    return SPIN_OK;
+}
+// after the corrector sweeps of a step: the next configuration becomes the current one and the step counter (the noise stream) advances
+extern "C" int llg_slab_advance(spin_system *s) {
+    REQUIRE(s, "null system");
+    int rc = slab_ready(s);
+    if (rc) return rc;
+    s->cur ^= 1;
+    advance_step_kernel<<<1, 1, 0, s->stream>>>(s->d_step, 1ull);
+    s->n_launch++;
+    s->step += 1;
     SPIN_CUDA(cudaGetLastError());
     return SPIN_OK;
 }
@@ -1212,7 +1329,7 @@ extern "C" int spin_profile_enable(spin_system *s, int on) {
     return SPIN_OK;
 }
 extern "C" int spin_profile_get(spin_system *s, int kind, double *ms, int64_t *n) {
-    REQUIRE(s && kind >= 0 && kind < 3, "bad argument");
+    REQUIRE(s && kind >= 0 && kind < 4, "bad argument");
     if (ms) *ms = s->prof_ms[kind];
     if (n) *n = s->prof_n[kind];
     return SPIN_OK;

@@ -237,7 +237,7 @@ template <int B>
 __device__ __forceinline__ void thermal_force(const Coord &c, u64 step, u32 seed_lo, u32 seed_hi, double (&f)[3], u32 image = 0u,
                                               double sigma_scale = 1.0) {
     if constexpr (spec::THERMAL_ON) {
-        const u32 cell = (u32)(c.ia + spec::NA * c.ib + (spec::NA * spec::NB) * c.ic);
+        const u32 cell = (u32)(c.ia + spec::NA * c.ib + (spec::NA * spec::NB) * c.ic) + (u32)spec::CELL_OFF;      // the GLOBAL cell (slab decomposition)
         double xi[3];
         spin::thermal_xi(seed_lo, seed_hi, step, (u32)B + (u32)spec::NBASIS * cell, xi, image);
         const double sg = __dmul_rn(specc::SIGMA[B], sigma_scale);
@@ -464,7 +464,8 @@ __device__ __forceinline__ void dispatch_basis(int b, Fn &&fn) {
 extern "C" __global__ void SPIN_BOUNDS(spec::BX *spec::BY *spec::BZ)
     jit_predictor(const double *__restrict__ n, const double *__restrict__ fddi, double *__restrict__ np, double *__restrict__ Aout,
                   const unsigned long long *__restrict__ d_step, unsigned int step_add, unsigned int seed_lo, unsigned int seed_hi,
-                  const unsigned char *__restrict__ pin, const double *__restrict__ img_sigma, const double *__restrict__ mu_ratio) {
+                  const unsigned char *__restrict__ pin, const double *__restrict__ img_sigma, const double *__restrict__ mu_ratio,
+                  unsigned int brick0) {
     spinjit::pdl_entry();
     const unsigned long long step = *d_step + step_add;
     // batched images: blockIdx.z selects the image; every per-spin array holds the images one after the other
@@ -472,7 +473,7 @@ extern "C" __global__ void SPIN_BOUNDS(spec::BX *spec::BY *spec::BZ)
     const size_t off = spec::MULTI_IMAGE ? (size_t)image * ((size_t)spec::NBASIS * spec::SUB) : (size_t)0;
     const double scale = (spec::MULTI_IMAGE && img_sigma) ? img_sigma[image] : 1.0;
     spinjit::dispatch_basis<0>((int)blockIdx.y, [&](auto b) {
-        spinjit::predictor_body<decltype(b)::value>(n + off, fddi + off, np + off, Aout + off, step, seed_lo, seed_hi, pin, mu_ratio, (int)blockIdx.x, image, scale);
+        spinjit::predictor_body<decltype(b)::value>(n + off, fddi + off, np + off, Aout + off, step, seed_lo, seed_hi, pin, mu_ratio, (int)(brick0 + blockIdx.x), image, scale);
     });
     spinjit::pdl_exit();
 }
@@ -481,7 +482,8 @@ extern "C" __global__ void SPIN_BOUNDS(spec::BX *spec::BY *spec::BZ)
     jit_corrector(const double *__restrict__ n, const double *__restrict__ np, const double *__restrict__ fddi_n,
                   const double *__restrict__ fddi_np, const double *__restrict__ Ain, double *__restrict__ nout,
                   const unsigned long long *__restrict__ d_step, unsigned int step_add, unsigned int seed_lo, unsigned int seed_hi,
-                  const unsigned char *__restrict__ pin, const double *__restrict__ img_sigma, const double *__restrict__ mu_ratio) {
+                  const unsigned char *__restrict__ pin, const double *__restrict__ img_sigma, const double *__restrict__ mu_ratio,
+                  unsigned int brick0) {
     spinjit::pdl_entry();
     const unsigned long long step = *d_step + step_add;
     const unsigned int image = spec::MULTI_IMAGE ? blockIdx.z : 0u;
@@ -490,7 +492,7 @@ extern "C" __global__ void SPIN_BOUNDS(spec::BX *spec::BY *spec::BZ)
     spinjit::dispatch_basis<0>((int)blockIdx.y, [&](auto b) {
         // The corrector walks the bricks in the opposite order to the predictor: what the predictor touched last (the tail of n and of
         // n^p) is still in the 126 MB L2 and is read first; it ends at brick 0, where the next predictor starts.
-        const int brick = spec::REVERSE_CORR ? (int)(gridDim.x - 1u - blockIdx.x) : (int)blockIdx.x;
+        const int brick = (int)brick0 + (spec::REVERSE_CORR ? (int)(gridDim.x - 1u - blockIdx.x) : (int)blockIdx.x);      // brick0: first brick of a range launch
         spinjit::corrector_body<decltype(b)::value>(n + off, np + off, fddi_n + off, fddi_np + off, Ain + off, nout + off, step, seed_lo, seed_hi, pin,
                                                     mu_ratio, brick, image, scale);
     });

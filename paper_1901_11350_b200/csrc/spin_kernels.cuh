@@ -172,7 +172,7 @@ __device__ __forceinline__ void rotation_field(const DevicePlan &P, int b, const
 __device__ __forceinline__ void thermal_force(const DevicePlan &P, const Site &s, unsigned long long step, double (&f)[3]) {
     f[0] = 0.0; f[1] = 0.0; f[2] = 0.0;
     if (P.thermal_on) {
-        const unsigned int cell = (unsigned int)(s.ia + P.Na * (s.ib + P.Nb * s.ic));
+        const unsigned int cell = (unsigned int)(s.ia + P.Na * (s.ib + P.Nb * s.ic)) + (unsigned int)P.cell_off;      // the GLOBAL cell (slab decomposition)
         thermal_xi(P.seed_lo, P.seed_hi, step, (unsigned int)s.b + (unsigned int)P.nb * cell, f);
         double sg = P.sigma[s.b];
         if (P.mu_ratio != nullptr) sg *= sqrt(mu_ratio(P, s));

@@ -79,6 +79,7 @@ struct DevicePlan {
     double alpha, dt, dt2;
     int stt_on;
     int has_ddi;
+    int cell_off;                            // slab decomposition: global cell index of local cell 0 (the thermal field is keyed by the GLOBAL spin)
     double stt_c[3];                         // j^ = sum_d stt_c[d] a_d   (1/Angstrom)
     double stt_s, stt_x;                     // -u (alpha-beta)/(1+alpha^2),  u (1+alpha beta)/(1+alpha^2)
     uint32_t seed_lo, seed_hi;
@@ -133,6 +134,9 @@ struct spin_system {
     unsigned char *d_pin;          // pinned-spin flags (boundary order), null if none
     std::vector<double> mu_site;   // per-site moments in mu_B (boundary order), empty if none
     double *d_mu_ratio;            // mu_i / mu_b(i) on the device (rebuilt with the plan: the basis moments may change), null if none
+    // ---- slab decomposition along c over several GPUs: this system holds planes [slab_off, slab_off + nc[2]) of a
+    // lattice of slab_gnc planes; its ghost layers along c are filled by the halo exchange, not by its own periodic images
+    int slab_on, slab_off, slab_gnc, slab_gper;
     // ---- batched images: n_img independent configurations of the same lattice and Hamiltonian; every per-spin array holds them
     // one after the other (stride nb * plan.sub doubles); the sweeps take the image from blockIdx.z
     int n_img, img_sel;            // number of images; image that spins_set/get, effective_field, energy, ... address
@@ -193,7 +197,8 @@ bool jit_coop_ready(const spin_system *s);
 bool jit_cluster_ready(const spin_system *s);
 int jit_launch_steps_coop(spin_system *s, unsigned nsteps);
 int jit_launch_predictor(spin_system *s, dim3 grid, dim3 block, const double *n, const double *fddi, double *np, double *Aout,
-                         unsigned step_add);
+                         unsigned step_add, unsigned brick0 = 0, unsigned nbricks = 0);
 int jit_launch_corrector(spin_system *s, dim3 grid, dim3 block, const double *n, const double *np, const double *fddi_n,
-                         const double *fddi_np, const double *Ain, double *nout, unsigned step_add);
+                         const double *fddi_np, const double *Ain, double *nout, unsigned step_add, unsigned brick0 = 0, unsigned nbricks = 0);
+void jit_brick_shape(const spin_system *s, int b[3]);
 }  // namespace spin

@@ -1,0 +1,251 @@
+"""Slab decomposition of one lattice along c over several GPUs.
+
+Each rank holds a slab of consecutive planes; before every sweep its ghost layers along c receive the neighbours' boundary planes
+(twice per Depondt step: n before the predictor, n^p before the corrector).  The kernels, the ghost-aware plan and the halo planes as
+contiguous device chunks are the C library's (include/spinllg.h "slab decomposition"); this module holds the HOST logic:
+
+  * `partition`        which planes a rank owns (balanced, contiguous);
+  * `HaloPlan`         who a rank's neighbours are (periodic ring or open chain) and which of its planes go where;
+  * `exchange`         one halo exchange of one array over a transport (`DistTransport`: torch.distributed point-to-point, NCCL between
+                       GPUs, gloo in the CPU tests);
+  * `SlabDriver`       one rank's step: boundary bricks first, their halos travel on a second stream while the interior bricks run;
+  * `LocalGroup`       all slabs in one process on one device (device copies as transport): the 1-GPU emulation of N ranks.
+
+Only argument marshalling and ordering happen here; every arithmetic step of the path runs in the library's kernels.  The paper has no
+counterpart (MPI appears only as a remark on scripting).
+"""
+from __future__ import annotations
+
+import dataclasses
+from typing import List, Optional, Sequence, Tuple
+
+
+def partition(n_planes: int, world: int) -> List[Tuple[int, int]]:
+    """[(first plane, plane count)] per rank: contiguous, sizes differ by at most one, larger slabs first."""
+    if world < 1 or n_planes < world:
+        raise ValueError(f"cannot cut {n_planes} planes into {world} slabs")
+    base, extra = divmod(n_planes, world)
+    out, first = [], 0
+    for r in range(world):
+        cnt = base + (1 if r < extra else 0)
+        out.append((first, cnt))
+        first += cnt
+    return out
+
+
+@dataclasses.dataclass(frozen=True)
+class HaloPlan:
+    """Neighbours and plane ranges of one rank.  `reach` = ghost width along c (the Hamiltonian's largest |translation| along c)."""
+    rank: int
+    world: int
+    first: int            # first global plane of the slab
+    count: int            # planes in the slab
+    n_planes: int         # planes of the whole lattice
+    periodic: bool
+    reach: int
+
+    @staticmethod
+    def make(rank: int, world: int, n_planes: int, periodic: bool, reach: int) -> "HaloPlan":
+        first, count = partition(n_planes, world)[rank]
+        if reach > count:
+            raise ValueError(f"rank {rank}: slab of {count} planes is thinner than the reach {reach}")
+        return HaloPlan(rank, world, first, count, n_planes, bool(periodic), int(reach))
+
+    # neighbour towards lower / higher c, or None at an open end
+    @property
+    def lower(self) -> Optional[int]:
+        if self.rank > 0:
+            return self.rank - 1
+        return self.world - 1 if self.periodic else None
+
+    @property
+    def upper(self) -> Optional[int]:
+        if self.rank < self.world - 1:
+            return self.rank + 1
+        return 0 if self.periodic else None
+
+    def neighbour(self, side: int) -> Optional[int]:
+        return self.lower if side == 0 else self.upper
+
+    def own_planes(self, side: int) -> range:
+        """global planes this rank SENDS towards `side` (its outermost `reach` planes on that side)"""
+        return range(self.first, self.first + self.reach) if side == 0 else range(self.first + self.count - self.reach, self.first + self.count)
+
+    def ghost_planes(self, side: int) -> range:
+        """global planes (modulo the lattice when periodic) this rank RECEIVES into its ghost layer on `side`"""
+        lo = self.first - self.reach if side == 0 else self.first + self.count
+        return range(lo, lo + self.reach)
+
+
+class DistTransport:
+    """Halo messages over torch.distributed point-to-point calls (NCCL between GPUs; gloo in the CPU tests)."""
+
+    def __init__(self, dist, group=None):
+        self.dist, self.group = dist, group
+
+    def sendrecv(self, plan: HaloPlan, send: Sequence, recv: Sequence):
+        """send[side] / recv[side]: tensors (or None where there is no neighbour).  The message towards `side` is what the neighbour on
+        that side puts into ITS opposite ghost layer.  All four operations are posted before any is waited for (no ordering deadlock);
+        tag = the side the message travels towards, so the two messages between a pair of ranks (world = 2, periodic) stay apart."""
+        ops = []
+        for side in (0, 1):                      # sends in the order low, high ...
+            peer = plan.neighbour(side)
+            if peer is not None and peer != plan.rank:
+                ops.append(self.dist.P2POp(self.dist.isend, send[side], peer, self.group, tag=side))
+        for side in (1, 0):                      # ... receives in the order high, low: with ONE peer on both sides (two ranks on a ring) the
+            peer = plan.neighbour(side)          # peer's first send (its low planes) is this rank's high ghost layer -- NCCL matches by order,
+            if peer is not None and peer != plan.rank:      # gloo by tag
+                ops.append(self.dist.P2POp(self.dist.irecv, recv[side], peer, self.group, tag=1 - side))
+        if plan.world == 1 and plan.periodic:        # a ring of one: the slab is its own neighbour
+            recv[0].copy_(send[1]); recv[1].copy_(send[0])
+        for w in (self.dist.batch_isend_irecv(ops) if ops else []):
+            w.wait()
+
+
+def exchange(plan: HaloPlan, get, put, send_buf, recv_buf, transport) -> None:
+    """One halo exchange of one array: get(side, buffer) fills buffer with the own boundary planes of `side`; the transport moves
+    send_buf[side] to the neighbour on that side, whose message arrives in recv_buf[side]; put(side, buffer) writes the ghost planes."""
+    for side in (0, 1):
+        if plan.neighbour(side) is not None:
+            get(side, send_buf[side])
+    transport.sendrecv(plan, send_buf, recv_buf)
+    for side in (0, 1):
+        if plan.neighbour(side) is not None:
+            put(side, recv_buf[side])
+
+
+class SlabDriver:
+    """One rank's slab of a workload and its time stepping.
+
+        drv = SlabDriver(P, torch, workload, rank, world, transport)      # builds the local system on the current device
+        drv.iterate(n)                                                      # n steps, halos exchanged twice per step
+        drv.spins()                                                         # this rank's spins (boundary order of the slab)
+
+    A stage (predictor or corrector) runs in three phases so that N slabs of one process can be driven in lockstep too:
+      begin_stage   sweep the brick layers the neighbours need, copy their planes into the send buffers on a second stream, launch the
+                    interior layers on the system's stream (they run while the halos travel)
+      transport     move send[side] to the neighbour on that side (DistTransport: inside iterate; LocalGroup: between the phases)
+      end_stage     write the received planes into the ghost layers; the system's stream waits for that before its next sweep
+    """
+
+    def __init__(self, P, torch, w, rank: int, world: int, transport=None, stream=None):
+        self.P, self.torch = P, torch
+        na, nb_, nc = (int(x) for x in w.n_cells)
+        first, count = partition(nc, world)[rank]
+        lw = dataclasses.replace(w, n_cells=(na, nb_, count))
+        self.stream = stream if stream is not None else torch.cuda.Stream()
+        self.copy_stream = torch.cuda.Stream()
+        self.sys = P.SpinSystem.from_workload(lw, stream=self.stream.cuda_stream)
+        self.sys.spin_set_slab(True, first, nc, int(w.periodic[2]))
+        per_plane = self.sys.N // count
+        self.sys.spins_set(w.initial_spins().reshape(nc, per_plane, 3)[first:first + count].reshape(-1, 3))      # boundary order: planes are contiguous
+        nd, reach = self.sys.spin_halo_doubles()
+        self.plan = HaloPlan.make(rank, world, nc, bool(w.periodic[2]), reach)
+        self.transport = transport
+        dev = torch.device("cuda", torch.cuda.current_device())
+        self.send = [torch.zeros(nd, dtype=torch.float64, device=dev) for _ in range(2)]
+        self.recv = [torch.zeros(nd, dtype=torch.float64, device=dev) for _ in range(2)]
+        self.sent = torch.cuda.Event()
+        self.halo_bytes_per_exchange = 8 * nd * sum(1 for side in (0, 1) if self.plan.neighbour(side) is not None)
+
+    # ---- the three phases of one halo exchange of `array` (0 n, 1 n^p, 2 next n)
+    def post(self, array: int) -> None:
+        """own boundary planes -> send buffers, on the copy stream, after everything enqueued so far on the system's stream"""
+        ev = self.torch.cuda.Event()
+        ev.record(self.stream)
+        self.copy_stream.wait_event(ev)
+        for side in (0, 1):
+            if self.plan.neighbour(side) is not None:
+                self.sys.spin_halo_get(array, side, self.send[side].data_ptr(), self.copy_stream.cuda_stream)
+        self.sent.record(self.copy_stream)
+
+    def deliver(self, array: int) -> None:
+        """received planes -> ghost layers; the system's stream waits for them"""
+        for side in (0, 1):
+            if self.plan.neighbour(side) is not None:
+                self.sys.spin_halo_put(array, side, self.recv[side].data_ptr(), self.copy_stream.cuda_stream)
+        done = self.torch.cuda.Event()
+        done.record(self.copy_stream)
+        self.stream.wait_event(done)
+
+    def begin_stage(self, stage: int, array: int) -> None:
+        self.sys.llg_slab_sweep(stage, 1)
+        self.post(array)
+        self.sys.llg_slab_sweep(stage, 2)
+
+    def _transport(self) -> None:
+        with self.torch.cuda.stream(self.copy_stream):
+            self.transport.sendrecv(self.plan, self.send, self.recv)
+
+    def exchange_initial(self) -> None:
+        self.post(0); self._transport(); self.deliver(0)
+
+    def iterate(self, n_steps: int) -> None:
+        """n steps of this rank (every rank calls it with the same n)"""
+        if not getattr(self, "_primed", False):              # ghosts of the configuration the run starts from
+            self.exchange_initial()
+            self._primed = True
+        for _ in range(int(n_steps)):
+            self.begin_stage(0, 1); self._transport(); self.deliver(1)      # predictor, halos of n^p
+            self.begin_stage(1, 2); self._transport(); self.deliver(2)      # corrector, halos of the next n
+            self.sys.llg_slab_advance()
+
+    def spins(self):
+        self.synchronize()
+        return self.sys.spins_get()
+
+    def synchronize(self):
+        self.copy_stream.synchronize()
+        self.sys.spin_synchronize()
+
+
+class LocalGroup:
+    """All slabs of a lattice in ONE process on one device: the emulation of N ranks on one GPU (never run ranks that wait on one another as
+    separate launches, B200_PROFILING.md).  The slabs advance in lockstep; a halo message is a device copy from the sender's send buffer
+    into the receiver's receive buffer, ordered by the sender's event."""
+
+    def __init__(self, P, torch, w, world: int):
+        self.torch = torch
+        self.drivers = [SlabDriver(P, torch, w, r, world) for r in range(world)]
+        self._exchange(0, post=True)
+
+    def _move(self) -> None:
+        for d in self.drivers:
+            for side in (0, 1):
+                peer = d.plan.neighbour(side)
+                if peer is None:
+                    continue
+                src = self.drivers[peer]
+                d.copy_stream.wait_event(src.sent)
+                with self.torch.cuda.stream(d.copy_stream):
+                    d.recv[side].copy_(src.send[1 - side], non_blocking=True)      # the peer's message towards the opposite side
+        # nobody refills a send buffer before every copy out of it has run
+        moved = []
+        for d in self.drivers:
+            ev = self.torch.cuda.Event()
+            ev.record(d.copy_stream)
+            moved.append(ev)
+        for d in self.drivers:
+            for ev in moved:
+                d.copy_stream.wait_event(ev)
+
+    def _exchange(self, array: int, post: bool) -> None:
+        if post:
+            for d in self.drivers:
+                d.post(array)
+        self._move()
+        for d in self.drivers:
+            d.deliver(array)
+
+    def iterate(self, n_steps: int) -> None:
+        for _ in range(int(n_steps)):
+            for stage, array in ((0, 1), (1, 2)):
+                for d in self.drivers:
+                    d.begin_stage(stage, array)
+                self._exchange(array, post=False)
+            for d in self.drivers:
+                d.sys.llg_slab_advance()
+
+    def spins(self):
+        import numpy as np
+        return np.concatenate([d.spins() for d in self.drivers], axis=0)

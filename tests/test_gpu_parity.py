@@ -939,3 +939,60 @@ def test_rodrigues_branches(P, O, B, branch):
         g.spin_set_option("use_jit", use_jit)
         g.llg_iterate(60); o.iterate(60)
         assert np.abs(g.spins_get() - o.spins()).max() < 1e-12, (branch, use_jit)
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# Slab decomposition along c (paper_1901_11350_b200/slab.py): N slabs of one lattice, each with its own system, ghost layers
+# along c filled by the halo exchange, boundary bricks first and the interior while the halos travel.  All slabs live in this process on
+# one GPU (device copies stand in for NCCL; ranks that wait on one another must not run as separate launches on one GPU).  The result
+# must be the single-lattice trajectory BIT FOR BIT: same arithmetic per site, global noise index, global folding of translations.
+@pytest.mark.parametrize("cfg,cells,per_c,world,steps,T", [
+    (3, (35, 9, 12), 1, 2, 40, 0.0),          # periodic ring of two: the same peer on both sides
+    (3, (35, 9, 13), 1, 3, 30, 15.0),         # uneven slabs (5, 4, 4), thermal field keyed by the global spin
+    (3, (33, 12, 10), 0, 2, 30, 0.0),         # open along c: the outer ghost layers stay zero
+    (3, (64, 16, 16), 1, 4, 20, 0.0),         # slabs of 4 planes: boundary layers only, no interior
+    (5, (20, 12, 9), 0, 3, 20, 5.0),          # film Hamiltonian (in-plane DMI), dipolar term off, open c
+])
+def test_slab_decomposition_is_bit_identical(P, O, cfg, cells, per_c, world, steps, T):
+    import torch
+    from paper_1901_11350_b200 import slab as S
+    w = W.CONFIGS[cfg]().resized(cells, steps)
+    w = dataclasses.replace(w, periodic=(w.periodic[0], w.periodic[1], per_c), T=T, ddi=False)
+    ref = P.SpinSystem.from_workload(w)
+    ref.spin_set_option("use_coop", 0)
+    ref.llg_iterate(steps)
+    grp = S.LocalGroup(P, torch, w, world)
+    assert [d.plan.count for d in grp.drivers] == [c for _, c in S.partition(cells[2], world)]
+    grp.iterate(steps)
+    got = grp.spins()
+    assert np.array_equal(got, ref.spins_get()), np.abs(got - ref.spins_get()).max()
+    # and the oracle on the whole lattice
+    o = O.OracleSystem.from_workload(w)
+    o.iterate(steps)
+    assert np.abs(got - o.spins()).max() <= SPIN_ATOL
+    # fields of a slab (ghosts current after the last exchange) = the rows of the whole lattice's field
+    B = ref.effective_field()
+    off = 0
+    for d in grp.drivers:
+        Bd = d.sys.effective_field()
+        assert np.array_equal(Bd, B[off:off + d.sys.N])
+        off += d.sys.N
+
+
+def test_slab_reach_two_and_other_solvers(P, O):
+    """Pairs reaching two planes along c (ghost width 2) and the Heun / SIB solvers on slabs; llg_iterate refuses a slab."""
+    import torch
+    from paper_1901_11350_b200 import slab as S
+    w = W.config3().resized((34, 10, 12), 20)
+    pt = np.vstack([w.pair_t, [[0, 0, 2], [1, 0, 2]]]); pi = np.r_[w.pair_i, 0, 0]; pj = np.r_[w.pair_j, 0, 0]
+    w = dataclasses.replace(w, pair_i=pi, pair_j=pj, pair_t=pt, pair_J=np.r_[w.pair_J, 0.3, -0.2], pair_D=np.vstack([w.pair_D, [[0.05, 0, 0.1], [0, 0.07, 0]]]))
+    for solver in (0, 1, 2):
+        ref = P.SpinSystem.from_workload(w); ref.llg_set_solver(solver); ref.spin_set_option("use_coop", 0); ref.llg_iterate(20)
+        grp = S.LocalGroup(P, torch, w, 3)
+        for d in grp.drivers:
+            d.sys.llg_set_solver(solver)
+        assert grp.drivers[0].plan.reach == 2
+        grp.iterate(20)
+        assert np.array_equal(grp.spins(), ref.spins_get()), solver
+    with pytest.raises(P.SpinError):
+        grp.drivers[0].sys.llg_iterate(1)
