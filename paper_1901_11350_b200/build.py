@@ -12,7 +12,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libspinllg.so")
 SOURCES = ["spin_api.cu", "spin_ddi.cu", "spin_jit.cu"]
-HEADERS = ["spinllg_internal.h", "spin_kernels.cuh", "spin_device_math.cuh", "spin_jit_kernels.cuh", os.path.join("..", "..", "include", "spinllg.h")]
+HEADERS = ["spinllg_internal.h", "spin_kernels.cuh", "spin_device_math.cuh", "spin_jit_kernels.cuh", "spin_jit_march.cuh", os.path.join("..", "..", "include", "spinllg.h")]
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
 
 

@@ -159,6 +159,14 @@ int stt_coefficients(const spin_system *s, double cd[3]) {
     return 0;
 }
 
+}  // namespace
+// The one-pass plane-marching Depondt kernel (spin_jit_march.cuh) applies to 3-D lattices of one basis atom advanced by the Depondt solver
+// without dipolar coupling, images or slab decomposition; lattices small enough for the all-steps-in-one-launch path keep that path.
+bool spin::march_eligible(const spin_system *s) {
+    return s->opt_march && s->opt_jit && s->nb == 1 && s->solver == SPIN_SOLVER_DEPONDT && !s->ddi_on && s->n_img == 1 && !s->slab_on && !s->opt_store_A &&
+           s->nc[0] >= 32 && s->nc[1] >= 8 && s->nc[2] >= 8 && (s->opt_march >= 2 || s->N >= 65536);
+}
+namespace {
 int build_plan(const spin_system *s, DevicePlan &P) {
     memset(&P, 0, sizeof(P));
     int reach[3] = {0, 0, 0};
@@ -281,7 +289,8 @@ int build_plan(const spin_system *s, DevicePlan &P) {
     }
     P.quad_begin[s->nb] = nq;
     // ---- layout with ghost cells (spinllg_internal.h): ghost width = reach; rows start on 128-byte lines
-    P.rA = reach[0]; P.rB = reach[1]; P.rC = reach[2];
+    P.ghost_mult = march_eligible(s) ? 2 : 1;
+    P.rA = P.ghost_mult * reach[0]; P.rB = P.ghost_mult * reach[1]; P.rC = P.ghost_mult * reach[2];
     P.gA = (P.perA && P.rA > 0) ? 1 : 0; P.gB = (P.perB && P.rB > 0) ? 1 : 0; P.gC = (P.perC && P.rC > 0 && !s->slab_on) ? 1 : 0;
     if (s->slab_on) {
         if (P.rC > P.Nc) return spin::fail(SPIN_ERR_ARG, "slab of %d planes is thinner than the reach %d of the Hamiltonian along c", P.Nc, P.rC);
@@ -438,6 +447,15 @@ int enqueue_step_t(spin_system *s, const Launch &L, unsigned step_add) {
         return SPIN_OK;
     }
     const bool prof = s->profile_on != 0;
+    if (jit_march_ready(s)) {          // the whole step in one pass (n^p stays in shared memory)
+        if (prof) cudaEventRecord(s->ev0, s->stream);
+        int rc = jit_launch_march(s, s->cur, nout, step_add);
+        if (rc) return rc;
+        s->n_launch++;
+        if (prof) { cudaEventRecord(s->ev1, s->stream); cudaEventSynchronize(s->ev1); float ms; cudaEventElapsedTime(&ms, s->ev0, s->ev1); s->prof_ms[1] += ms; s->prof_n[1]++; }
+        s->cur ^= 1;
+        return SPIN_OK;
+    }
     const size_t istr = (size_t)s->nb * s->plan.sub;       // image stride
     if (s->ddi_on) {
         if (prof) cudaEventRecord(s->ev0, s->stream);
@@ -534,7 +552,7 @@ extern "C" int spin_geometry_create(const double bravais[9], int n_basis, const 
     if (!has_device) cudaGetLastError();
     spin_system *s = new spin_system();
     s->has_device = has_device;
-    s->jit = nullptr; s->opt_jit = 1; s->opt_ddi_slab = 1; s->opt_ddi_mirror = 1; s->opt_pdl = -1; s->opt_cache_noise = 1; s->opt_coop = 1; s->d_bar = nullptr;
+    s->jit = nullptr; s->opt_jit = 1; s->opt_march = 1; s->opt_ddi_slab = 1; s->opt_ddi_mirror = 1; s->opt_pdl = -1; s->opt_cache_noise = 1; s->opt_coop = 1; s->d_bar = nullptr;
     s->n_img = 1; s->img_sel = 0; s->d_img_sigma = nullptr;
     memcpy(s->brav, bravais, sizeof(s->brav));
     s->nb = n_basis;
@@ -930,7 +948,7 @@ extern "C" int llg_iterate(spin_system *s, int64_t n_steps) {
     // (a grid barrier costs about as much as a launch inside a CUDA graph, and it empties L1), so the limit is low; option
     // use_coop = 2 forces it for any lattice without dipolar coupling.
     const int64_t COOP_CHUNK = 8192;
-    if (s->opt_coop && !s->profile_on && !s->ddi_on && (s->N <= SPIN_COOP_MAX_SPINS || s->opt_coop >= 2) && jit_coop_ready(s) &&
+    if (s->opt_coop && !s->profile_on && !s->ddi_on && (s->N <= SPIN_COOP_MAX_SPINS || s->opt_coop >= 2) && jit_coop_ready(s) && !jit_march_ready(s) &&
         n_steps > 0) {
         while (done < n_steps) {
             const unsigned chunk = (unsigned)std::min<int64_t>(COOP_CHUNK, n_steps - done);
@@ -968,7 +986,7 @@ extern "C" int llg_iterate(spin_system *s, int64_t n_steps) {
         }
         while (n_steps - done >= G) {
             SPIN_CUDA(cudaGraphLaunch(gexec, s->stream));
-            s->n_launch += (s->solver == SPIN_SOLVER_RK4 ? 4 : 2) * G + 1;
+            s->n_launch += (s->solver == SPIN_SOLVER_RK4 ? 4 : (jit_march_ready(s) ? 1 : 2)) * G + 1;
             done += G;
         }
     }
@@ -1342,6 +1360,7 @@ extern "C" int spin_set_option(spin_system *s, const char *name, int value) {
     else if (!strcmp(name, "use_coop")) { s->opt_coop = value < 0 ? 0 : (value > 3 ? 3 : value); s->plan_dirty = true; }
     else if (!strcmp(name, "cache_noise")) { s->opt_cache_noise = value ? 1 : 0; s->plan_dirty = true; }
     else if (!strcmp(name, "use_pdl")) { s->opt_pdl = value > 2 ? -1 : value < 0 ? -1 : value; s->plan_dirty = true; }
+    else if (!strcmp(name, "use_march")) { s->opt_march = value < 0 ? 0 : (value > 2 ? 2 : value); s->plan_dirty = true; }
     else if (!strcmp(name, "ddi_mirror")) { s->opt_ddi_mirror = value ? 1 : 0; s->plan_dirty = true; }
     else if (!strcmp(name, "ddi_slab")) { s->opt_ddi_slab = value < 0 ? 0 : (value > 2 ? 2 : value); s->plan_dirty = true; }      // 0: 3-D path, 1: slab path, 2: slab path with cuFFT's a-pass
     else return spin::fail(SPIN_ERR_ARG, "unknown option '%s'", name);
@@ -1353,7 +1372,8 @@ extern "C" int spin_set_option(spin_system *s, const char *name, int value) {
 extern "C" int spin_kernel_info(spin_system *s, char *buf, int len) {
     REQUIRE(s && buf && len > 0, "bad argument");
     if (s->has_device) { int rc = ensure_plan(s); if (rc) return rc; }
-    if (jit_coop_ready(s) && s->opt_coop && !s->ddi_on && (s->N <= SPIN_COOP_MAX_SPINS || s->opt_coop >= 2)) snprintf(buf, (size_t)len, jit_cluster_ready(s) ? "jit+cluster" : "jit+coop");
+    if (jit_march_ready(s)) snprintf(buf, (size_t)len, "jit+march");
+    else if (jit_coop_ready(s) && s->opt_coop && !s->ddi_on && (s->N <= SPIN_COOP_MAX_SPINS || s->opt_coop >= 2)) snprintf(buf, (size_t)len, jit_cluster_ready(s) ? "jit+cluster" : "jit+coop");
     else if (jit_ready(s)) snprintf(buf, (size_t)len, "jit (brick sweeps)");
     else snprintf(buf, (size_t)len, "generic: %s", s->jit_note.c_str());
     return SPIN_OK;

@@ -159,7 +159,6 @@ __global__ void ddi_slab_scatter_kernel(const __grid_constant__ DevicePlan L, co
     if (cell >= L.Ncell) return;
     const int ia = cell % L.Na, ib = (cell / L.Na) % L.Nb, ic = cell / (L.Na * L.Nb);
     const int j = ((ic + L.LC) * L.PB + (ib + L.LB)) * (3 * L.PA) + (ia + L.LA);
-#pragma unroll
     const double m = mu * (L.mu_ratio ? L.mu_ratio[cell] : 1.0);
 #pragma unroll
     for (int k = 0; k < 3; ++k) in[((size_t)ib * SL + (k * L.Nc + ic)) * P0 + ia] = m * n[j + k * L.PA];
@@ -170,7 +169,6 @@ __global__ void ddi_slab_gather_kernel(const __grid_constant__ DevicePlan L, con
     if (cell >= L.Ncell) return;
     const int ia = cell % L.Na, ib = (cell / L.Na) % L.Nb, ic = cell / (L.Na * L.Nb);
     const int j = ((ic + L.LC) * L.PB + (ib + L.LB)) * (3 * L.PA) + (ia + L.LA);
-#pragma unroll
     const double m = scale * (L.mu_ratio ? L.mu_ratio[cell] : 1.0);
 #pragma unroll
     for (int k = 0; k < 3; ++k) f[j + k * L.PA] = m * out[((size_t)ib * SL + (k * L.Nc + ic)) * P0 + ia];

@@ -5,6 +5,7 @@
 // cubin is loaded through the runtime's library API.  The result is cached per system and rebuilt when the plan changes.
 // If NVRTC is unavailable or compilation fails the system keeps using the table-driven kernels and records why
 // (spin_kernel_info reports which path is active; nothing is silently computed on the CPU either way).
+#include <cuda.h>
 #include <dlfcn.h>
 #include <nvrtc.h>
 #include <stdlib.h>
@@ -28,6 +29,12 @@ struct JitState {
     cudaKernel_t k_pred, k_corr, k_rk4;
     bool loaded;
     std::string source, log;
+    // the whole Depondt step in one pass (spin_jit_march.cuh)
+    bool march;
+    cudaKernel_t k_march;
+    int march_ty, march_nzc, march_threads, march_items;
+    size_t march_smem;
+    CUtensorMap tm_march[2];          // n[0], n[1] with the staged plane of the kernel as box
     // all steps in one cooperative launch (launch-bound lattices)
     bool coop;
     cudaKernel_t k_coop;
@@ -102,6 +109,46 @@ static void jit_brick_launch(const spin_system *s, dim3 &grid, dim3 &block) {
     grid = dim3((unsigned)(((s->nc[0] + b[0] - 1) / b[0]) * ((s->nc[1] + b[1] - 1) / b[1]) * ((s->nc[2] + b[2] - 1) / b[2])), (unsigned)s->nb, 1);
     block = dim3((unsigned)(b[0] * b[1] * b[2]), 1, 1);
 }
+
+// geometry of the one-pass plane-marching kernel: rows per tile, chunks along c, threads, shared memory; false if it does not apply
+namespace {
+struct MarchGeo { int ra, rb, rc, ty, nzc, threads, items; size_t smem; };
+bool plan_march(const spin_system *s, MarchGeo &g) {
+    const DevicePlan &P = s->plan;
+    if (!spin::march_eligible(s) || P.ghost_mult != 2) return false;
+    g.ra = P.rA / 2; g.rb = P.rB / 2; g.rc = P.rC / 2;
+    if (g.rc < 1 || g.ra > 4 || g.rb > 4 || g.rc > 2) return false;
+    const int hx = (2 * g.ra + 1) / 2 * 2;
+    if (P.LA < hx) return false;
+    const int sms = sm_count(s);
+    double best = -1.0;
+    bool found = false;
+    int force_ty = 0, force_nzc = 0;
+    if (const char *e = getenv("SPINLLG_MARCH_GEO")) sscanf(e, "%d,%d", &force_ty, &force_nzc);      // TEMPORARY tuning hook
+    for (int ty : {8, 12, 16, 6, 4}) {                       // tile rows; prefer tiles that divide the lattice
+        if (force_ty && ty != force_ty) continue;
+        const int py = ty + 2 * g.rb, rimw = (2 * g.ra * py + 31) / 32, threads = 32 * (py + rimw);
+        if (threads > 1024) continue;
+        const size_t nslot = ((size_t)3 * (32 + 2 * hx) * (ty + 4 * g.rb) + 15) / 16 * 16, ppl = (size_t)3 * (32 + 2 * g.ra) * py;
+        const size_t smem = ((size_t)(2 * g.rc + 3) * nslot + (size_t)(2 * g.rc + 2) * ppl) * 8 + (size_t)(2 * g.rc + 3) * 8;
+        if (smem > 200 * 1024) continue;
+        const int per_sm = (int)std::min<size_t>((size_t)(227 * 1024) / (smem + 1024), (size_t)std::min(2048 / threads, 65536 / (threads * 72)));
+        if (per_sm < 1) continue;
+        const int cols = ((P.Na + 31) / 32) * ((P.Nb + ty - 1) / ty), slots = sms * per_sm;
+        for (int nzc = 1; nzc <= P.Nc / 4; ++nzc) {
+            if (force_nzc && nzc != force_nzc) continue;
+            const long items = (long)cols * nzc;
+            const long waves = (items + slots - 1) / slots;
+            const double cz = (double)P.Nc / nzc;
+            // useful fraction: full waves x chunk overlap of the predictor x rim of the tile x rows that hang over the lattice
+            const double eff = (double)items / (double)(waves * slots) * cz / (cz + 2.0 * g.rc) * (32.0 * ty) / (double)((32 + 2 * g.ra) * py) *
+                               (double)P.Nb / (double)(((P.Nb + ty - 1) / ty) * ty);
+            if (eff > best + 1e-9) { best = eff; found = true; g.ty = ty; g.nzc = nzc; g.threads = threads; g.items = (int)items; g.smem = smem; }
+        }
+    }
+    return found;
+}
+}  // namespace
 
 std::string spin::jit_source(const spin_system *s) {
     const DevicePlan &P = s->plan;
@@ -209,6 +256,10 @@ std::string spin::jit_source(const spin_system *s) {
       << ", STT_S = " << hexd(P.stt_s) << ", STT_X = " << hexd(P.stt_x) << ";\n";
     o << "}  // namespace specc\nnamespace spec {\n";
     o << "}  // namespace spec\n";
+    MarchGeo mg;
+    if (plan_march(s, mg))
+        o << "namespace spec { constexpr int MRA = " << mg.ra << ", MRB = " << mg.rb << ", MRC = " << mg.rc << ", MTY = " << mg.ty << ", MNZC = " << mg.nzc
+          << "; }\n#define SPIN_MARCH 1\n";
     o << "#include \"spin_jit_kernels.cuh\"\n";
     return o.str();
 }
@@ -349,7 +400,46 @@ void spin::jit_release(spin_system *s) {
 }
 
 // which variants of the sweeps this system can use (depends on options, solver, pins, image count -- not only on the source)
+// tensor map of one spin array for the marching kernel: dims (x: PA, comp: 3, y: PB, z: PC), box = one staged plane (tile + rim)
+static int encode_march_map(const spin_system *s, const MarchGeo &g, const double *base, CUtensorMap *tm) {
+    typedef CUresult (*encode_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *, const cuuint32_t *,
+                                  const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    static encode_fn encode = nullptr;
+    if (!encode) {
+        void *fn = nullptr;
+        cudaDriverEntryPointQueryResult qr;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qr) != cudaSuccess || !fn || qr != cudaDriverEntryPointSuccess)
+            return spin::fail(SPIN_ERR_CUDA, "cuTensorMapEncodeTiled is not available from this driver");
+        encode = (encode_fn)fn;
+    }
+    const DevicePlan &P = s->plan;
+    const int hx = (2 * g.ra + 1) / 2 * 2;
+    const cuuint64_t dims[4] = {(cuuint64_t)P.PA, 3, (cuuint64_t)P.PB, (cuuint64_t)P.PC};
+    const cuuint64_t strides[3] = {(cuuint64_t)P.PA * 8, (cuuint64_t)3 * P.PA * 8, (cuuint64_t)3 * P.PA * P.PB * 8};
+    const cuuint32_t box[4] = {(cuuint32_t)(32 + 2 * hx), 3, (cuuint32_t)(g.ty + 4 * g.rb), 1};
+    const cuuint32_t estr[4] = {1, 1, 1, 1};
+    const CUresult r = encode(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, (void *)base, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                              CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return spin::fail(SPIN_ERR_CUDA, "cuTensorMapEncodeTiled failed with code %d", (int)r);
+    return SPIN_OK;
+}
+
 static void variants_prepare(spin_system *s, JitState *j) {
+    j->march = false;
+    MarchGeo mg;
+    if (plan_march(s, mg)) {
+        cudaError_t e = cudaLibraryGetKernel(&j->k_march, j->lib, "jit_depondt_march");
+        if (e == cudaSuccess) e = cudaFuncSetAttribute((const void *)j->k_march, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)mg.smem);
+        int occ = 0;
+        if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, (const void *)j->k_march, mg.threads, mg.smem);
+        if (e == cudaSuccess && occ >= 1 && encode_march_map(s, mg, s->d_n[0], &j->tm_march[0]) == SPIN_OK &&
+            encode_march_map(s, mg, s->d_n[1], &j->tm_march[1]) == SPIN_OK) {
+            j->march = true;
+            j->march_ty = mg.ty; j->march_nzc = mg.nzc; j->march_threads = mg.threads; j->march_items = mg.items; j->march_smem = mg.smem;
+        } else {
+            cudaGetLastError();
+        }
+    }
     j->coop = false;
     j->cluster = false;
     if (s->opt_coop && !s->ddi_on && s->solver != SPIN_SOLVER_RK4 && s->n_img == 1) {
@@ -399,6 +489,7 @@ int spin::jit_prepare(spin_system *s) {
     JitState *j = new JitState();
     j->loaded = false;
     j->coop = false;
+    j->march = false;
     j->source = src;
     s->jit = j;
     std::string cubin;
@@ -476,6 +567,20 @@ int spin::jit_launch_rk4_stage(spin_system *s, const double *base, const double 
     dim3 grid, block;
     jit_brick_launch(s, grid, block);
     SPIN_CUDA(cudaLaunchKernel((const void *)s->jit->k_rk4, grid, block, args, 0, s->stream));
+    return SPIN_OK;
+}
+
+bool spin::jit_march_ready(const spin_system *s) { return s->jit && s->jit->loaded && s->jit->march; }
+
+// one Depondt step in one pass: reads d_n[cur] through its tensor map, writes nout
+int spin::jit_launch_march(spin_system *s, int cur, double *nout, unsigned step_add) {
+    JitState *j = s->jit;
+    unsigned seed_lo = s->plan.seed_lo, seed_hi = s->plan.seed_hi;
+    const unsigned long long *d_step = s->d_step;
+    const unsigned char *pin = s->d_pin;
+    const double *mu_ratio = s->d_mu_ratio;
+    void *args[] = {(void *)&j->tm_march[cur], (void *)&nout, (void *)&d_step, (void *)&step_add, (void *)&seed_lo, (void *)&seed_hi, (void *)&pin, (void *)&mu_ratio};
+    SPIN_CUDA(cudaLaunchKernel((const void *)j->k_march, dim3((unsigned)j->march_items), dim3((unsigned)j->march_threads), args, j->march_smem, s->stream));
     return SPIN_OK;
 }
 

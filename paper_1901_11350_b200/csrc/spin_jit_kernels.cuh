@@ -580,3 +580,7 @@ extern "C" __global__ void SPIN_BOUNDS(spec::BX *spec::BY *spec::BZ)
                       const unsigned char *__restrict__ pin, const double *__restrict__ mu_ratio) {
     spinjit::all_steps(n0, n1, np, aux, *d_step, nsteps, seed_lo, seed_hi, pin, mu_ratio, []() { spinjit::cluster_barrier(); });
 }
+
+#ifdef SPIN_MARCH
+#include "spin_jit_march.cuh"
+#endif

@@ -1,0 +1,189 @@
+// spin_jit_march.cuh -- the whole Depondt step (B5-B7) of a 3-D lattice in ONE pass: a plane-marching kernel
+// (sm_100a; included by spin_jit_kernels.cuh when SPIN_MARCH is defined; one basis atom, Depondt solver, no dipolar term).
+//
+// Why.  The two brick sweeps move 120 B per spin-update through HBM (n^p written and read back, n read twice), fetch every line
+// 2.8 times from L2 (brick halos) and evaluate F(n) twice.  On B200 that is not bandwidth- but POWER-bound: a 2-s run of cfg3 sits at
+// the 1000 W cap and the SM clock falls from 1965 to about 1650 MHz (profiles/r2_README.md).  This kernel removes the n^p round trip,
+// the second evaluation of F(n) and most of the L2 re-fetches:
+//   * a block owns a column of 32 x TY sites and marches along c through a chunk of planes;
+//   * one elected thread streams the n planes (tile + a rim of twice the Hamiltonian's reach) into a shared-memory ring with one TMA
+//     tensor copy per plane (cp.async.bulk.tensor, completion on an mbarrier), two planes ahead of the compute;
+//   * per iteration every thread computes the PREDICTOR of one site of plane zP -- tile plus a rim of one reach: TY + 2 RB aligned rows of
+//     32 sites by as many warps, the 2 RA rim columns by extra warps -- and writes n^p into a second ring that never leaves the SM;
+//   * after one __syncthreads the tile's threads compute the CORRECTOR of plane zP - RC from that ring: A(n), n and the thermal field of
+//     their site are still in their registers, so F(n) is evaluated once per step, and write n(t + dt) (and its periodic images).
+// The arithmetic is the brick kernels' (force<>, rotation_field<>, rodrigues, same order): results are bit-identical (tested).
+// Ghost layers are twice the reach wide in this mode (the planner doubles them): the rim predictor needs n two reaches out.
+// HBM traffic: read n once (+ chunk overlap), write n once = 48-60 B per spin-update instead of 120.
+//
+// spec must also define: int MRA, MRB, MRC (reach of the Hamiltonian; ghost widths RA, RB, RC are twice that), MTY (rows per tile),
+// MNZC (chunks along c).
+#pragma once
+
+namespace spinmarch {
+using namespace spinjit;
+
+struct __align__(64) TensorMap { unsigned long long opaque[16]; };      // CUtensorMap, passed as a __grid_constant__ parameter
+
+constexpr int RA = spec::MRA, RB = spec::MRB, RC = spec::MRC, TY = spec::MTY, NZC = spec::MNZC;
+constexpr int HX = (2 * RA + 1) / 2 * 2;                         // rim of a staged n row, even: TMA box rows start 16-byte aligned
+constexpr int NX = 32 + 2 * HX, NY = TY + 4 * RB;                // staged n plane (rim of two reaches), sites
+constexpr int NROW = 3 * NX, NPL = NROW * NY, NSLOT = (NPL + 15) / 16 * 16;      // doubles; slots are 128-byte multiples
+constexpr int PX = 32 + 2 * RA, PY = TY + 2 * RB;                // n^p plane (rim of one reach)
+constexpr int PROW = 3 * PX, PPL = PROW * PY;
+constexpr int RN = 2 * RC + 3, RP = 2 * RC + 2;                  // ring depths: n planes (two of look-ahead), n^p planes
+constexpr int RIM = 2 * RA * PY, RIMW = (RIM + 31) / 32;         // sites of the rim columns, warps that take them
+constexpr int NWARP = PY + RIMW, NTHREADS = 32 * NWARP;
+constexpr int NTX = (spec::NA + 31) / 32, NTY = (spec::NB + TY - 1) / TY;
+static_assert(spec::NBASIS == 1 && spec::SOLVER == 0 && !spec::HAS_DDI && !spec::MULTI_IMAGE, "one-pass kernel: one basis atom, Depondt, no dipolar term");
+static_assert(spec::RA == 2 * RA && spec::RB == 2 * RB && spec::RC == 2 * RC, "ghost layers must be twice the reach");
+
+extern __shared__ __align__(128) double smem[];
+
+__device__ __forceinline__ u32 smem_u32(const void *p) { return (u32)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(u32 bar, u32 count) { asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count)); }
+__device__ __forceinline__ void mbar_expect_tx(u32 bar, u32 bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(u32 bar, u32 parity) {
+    u32 done = 0;
+    for (int spin = 0; !done; ++spin) {
+        asm volatile("{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}"
+                     : "=r"(done) : "r"(bar), "r"(parity) : "memory");
+        if (spin > (1 << 24)) __trap();      // a lost copy must end the launch with an error, never hang the device
+    }
+}
+__device__ __forceinline__ void tma_load_4d(u32 dst, const TensorMap *tm, int c0, int c1, int c2, int c3, u32 bar) {
+    asm volatile("cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];"
+                 ::"r"(dst), "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(bar) : "memory");
+}
+
+// partner of a site in a ring of staged planes: pl[dz + RC] points at the x component of the own site in the plane z + dz
+template <int XS, int ROWS>      // doubles between the components of a row (= sites per row), between rows
+struct RingAcc {
+    const double *pl[2 * RC + 1];
+    template <int B, int BJ, int DA, int DB, int DC>
+    __device__ __forceinline__ void load(int, double (&v)[3]) const {
+        const double *q = pl[DC + RC] + (DB * ROWS + DA);
+        v[0] = q[0]; v[1] = q[XS]; v[2] = q[2 * XS];
+    }
+};
+}  // namespace spinmarch
+
+extern "C" __global__ void SPIN_BOUNDS(spinmarch::NTHREADS)
+    jit_depondt_march(const __grid_constant__ spinmarch::TensorMap tm_n, double *__restrict__ nout, const unsigned long long *__restrict__ d_step,
+                      unsigned int step_add, unsigned int seed_lo, unsigned int seed_hi, const unsigned char *__restrict__ pin,
+                      const double *__restrict__ mu_ratio) {
+    using namespace spinmarch;
+    const unsigned long long step = *d_step + step_add;
+    const int item = blockIdx.x, col = item % (NTX * NTY), chunk = item / (NTX * NTY);
+    const int x0 = (col % NTX) * 32, y0 = (col / NTX) * TY;
+    const int za = (int)((long long)chunk * spec::NC / NZC), zb = (int)((long long)(chunk + 1) * spec::NC / NZC);
+    const int NP = zb - za + 4 * RC;                              // n planes za - 2 RC .. zb - 1 + 2 RC
+    double *nring = smem, *pring = smem + RN * NSLOT;
+    const u32 bars = smem_u32(pring + RP * PPL);
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    auto issue = [&](int p) {
+        const u32 bar = bars + 8u * (p % RN);
+        mbar_expect_tx(bar, (u32)(NPL * 8));
+        tma_load_4d(smem_u32(nring + (p % RN) * NSLOT), &tm_n, spec::LA + x0 - HX, 0, spec::LB + y0 - 2 * RB, spec::LC + za - 2 * RC + p, bar);
+    };
+    if (tid == 0) {
+        for (int s = 0; s < RN; ++s) mbar_init(bars + 8u * s, 1u);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    if (tid == 0) for (int p = 0; p < RN - 1 && p < NP; ++p) issue(p);
+    // the site of this thread relative to the tile: the first PY warps hold the aligned rows, the others the rim columns
+    int sx, sy;
+    bool mine = true;
+    if (warp < PY) { sx = lane; sy = warp - RB; }
+    else {
+        const int r = (warp - PY) * 32 + lane;                    // rim site: row r / (2 RA), column r % (2 RA)
+        mine = r < RIM;
+        const int cr = mine ? r % (2 * RA) : 0;
+        sy = (mine ? r / (2 * RA) : 0) - RB;
+        sx = cr < RA ? cr - RA : 32 + (cr - RA);
+    }
+    const int gx = x0 + sx, gy = y0 + sy;                          // lattice coordinates, possibly in the ghost region
+    // a predictor site is live if it is a lattice site or the periodic image of one; elsewhere (open edges, tiles hanging over the
+    // lattice) n^p is the zero vector, exactly what the ghost cells of the brick kernels hold there
+    const bool live_xy = mine && (spec::PER_A ? (gx >= -RA && gx < spec::NA + RA) : (gx >= 0 && gx < spec::NA)) &&
+                         (spec::PER_B ? (gy >= -RB && gy < spec::NB + RB) : (gy >= 0 && gy < spec::NB));
+    const bool tile_site = warp < PY && sy >= 0 && sy < TY && gx < spec::NA && gy < spec::NB;      // corrector sites
+    Coord c;                                                       // the lattice site this one is (an image of)
+    c.ia = gx < 0 ? gx + spec::NA : (gx >= spec::NA ? gx - spec::NA : gx);
+    c.ib = gy < 0 ? gy + spec::NB : (gy >= spec::NB ? gy - spec::NB : gy);
+    const int ncell = ((sy + 2 * RB) * 3) * NX + (sx + HX);       // x component of the own site in a staged n plane
+    const int pcell = ((sy + RB) * 3) * PX + (sx + RA);           // the same in an n^p plane
+    // what the corrector of plane zC needs from the predictor of the same site, RC iterations earlier
+    double n_q[RC][3], A_q[RC][3], th_q[RC][3];
+#pragma unroll
+    for (int r = 0; r < RC; ++r)
+#pragma unroll
+        for (int k = 0; k < 3; ++k) { n_q[r][k] = 0.0; A_q[r][k] = 0.0; th_q[r][k] = 0.0; }
+#pragma unroll
+    for (int p = 0; p < 2 * RC; ++p) mbar_wait(bars + 8u * p, 0u);
+    const int NIT = zb - za + 2 * RC;
+    for (int k = 0; k < NIT; ++k) {                                // predictor plane zP = za - RC + k from n planes k .. k + 2 RC
+        mbar_wait(bars + 8u * ((k + 2 * RC) % RN), (u32)(((k + 2 * RC) / RN) & 1));
+        const int zP = za - RC + k;
+        double n_cur[3] = {0.0, 0.0, 0.0}, A_cur[3] = {0.0, 0.0, 0.0}, th_cur[3] = {0.0, 0.0, 0.0};
+        double *pslot = pring + (k % RP) * PPL;
+        if (mine) {
+            double out[3] = {0.0, 0.0, 0.0};
+            const bool live = live_xy && (spec::PER_C || (zP >= 0 && zP < spec::NC));
+            if (live) {
+                c.ic = zP < 0 ? zP + spec::NC : (zP >= spec::NC ? zP - spec::NC : zP);
+                RingAcc<NX, NROW> acc;
+#pragma unroll
+                for (int dz = -RC; dz <= RC; ++dz) acc.pl[dz + RC] = nring + ((k + RC + dz) % RN) * NSLOT + ncell;
+                double own[1][3], F[1][3], sg[1][3] = {{0.0, 0.0, 0.0}};
+                acc.template load<0, 0, 0, 0, 0>(0, own[0]);
+                n_cur[0] = own[0][0]; n_cur[1] = own[0][1]; n_cur[2] = own[0][2];
+                if (is_pinned<0>(pin, c)) { out[0] = n_cur[0]; out[1] = n_cur[1]; out[2] = n_cur[2]; }
+                else {
+                    const double zr = site_ratio<0>(mu_ratio, c), ir = spec::HAS_SITE_MU ? 1.0 / zr : 1.0;      // per-site moment
+                    const double sscale = (spec::HAS_SITE_MU && spec::THERMAL_ON) ? sqrt(zr) : 1.0;
+                    thermal_force<0>(c, step, seed_lo, seed_hi, F[0], 0u, sscale);
+                    th_cur[0] = F[0][0]; th_cur[1] = F[0][1]; th_cur[2] = F[0][2];
+                    force<0, 1>(acc, own, F, zr);
+                    if constexpr (spec::STT_ON) stt_gradient<0, 1>(acc, c, own, sg);
+                    rotation_field<0>(own[0], F[0], sg[0], A_cur, ir);
+                    spin::rodrigues(A_cur, specc::DT, specc::DT2, own[0], out);                 // B5
+                }
+            }
+            pslot[pcell] = out[0]; pslot[pcell + PX] = out[1]; pslot[pcell + 2 * PX] = out[2];
+        }
+        __syncthreads();                                           // n^p(zP) is complete; nobody reads n plane k any more
+        if (tid == 0 && k + RN - 1 < NP) issue(k + RN - 1);        // refill a free slot, two planes ahead of the next predictor
+        const int zC = zP - RC;
+        if (k >= 2 * RC && tile_site) {                            // corrector of plane zC from n^p planes zC - RC .. zC + RC = zP
+            c.ic = zC;
+            double o[3];
+            if (is_pinned<0>(pin, c)) { o[0] = n_q[0][0]; o[1] = n_q[0][1]; o[2] = n_q[0][2]; }
+            else {
+                const double zr = site_ratio<0>(mu_ratio, c), ir = spec::HAS_SITE_MU ? 1.0 / zr : 1.0;
+                RingAcc<PX, PROW> acc;
+#pragma unroll
+                for (int dz = -RC; dz <= RC; ++dz) acc.pl[dz + RC] = pring + ((k - RC + dz) % RP) * PPL + pcell;
+                double own[1][3], F[1][3] = {{th_q[0][0], th_q[0][1], th_q[0][2]}}, sg[1][3] = {{0.0, 0.0, 0.0}}, Ap[3];
+                acc.template load<0, 0, 0, 0, 0>(0, own[0]);
+                force<0, 1>(acc, own, F, zr);
+                if constexpr (spec::STT_ON) stt_gradient<0, 1>(acc, c, own, sg);
+                rotation_field<0>(own[0], F[0], sg[0], Ap, ir);
+                const double Ac[3] = {A_q[0][0] + Ap[0], A_q[0][1] + Ap[1], A_q[0][2] + Ap[2]};
+                spin::rodrigues(Ac, specc::HDT, specc::QDT2, n_q[0], o);                          // B6-B7: R((A + A^p) / 2) n(t)
+                spin::renormalise(o);
+            }
+            store_spin(nout + ((size_t)(zC + spec::LC) * PLANE + (size_t)(c.ib + spec::LB) * ROW + (c.ia + spec::LA)), c, o);
+        }
+        // the queue moves on: slot 0 is the oldest (the plane the next corrector takes)
+#pragma unroll
+        for (int r = 0; r + 1 < RC; ++r)
+#pragma unroll
+            for (int q = 0; q < 3; ++q) { n_q[r][q] = n_q[r + 1][q]; A_q[r][q] = A_q[r + 1][q]; th_q[r][q] = th_q[r + 1][q]; }
+#pragma unroll
+        for (int q = 0; q < 3; ++q) { n_q[RC - 1][q] = n_cur[q]; A_q[RC - 1][q] = A_cur[q]; th_q[RC - 1][q] = th_cur[q]; }
+    }
+}

@@ -83,7 +83,6 @@ __device__ __forceinline__ void short_range_force(const DevicePlan &P, const dou
                                                   const double (&own)[NCONF][3], int mask, double (&F)[NCONF][3]) {
     const int b = s.b;
     if (mask & T_ZEE) {
-#pragma unroll
         const double r = mu_ratio(P, s);
 #pragma unroll
         for (int c = 0; c < NCONF; ++c) { F[c][0] += r * P.zee[b][0]; F[c][1] += r * P.zee[b][1]; F[c][2] += r * P.zee[b][2]; }

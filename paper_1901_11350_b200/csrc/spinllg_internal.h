@@ -65,7 +65,8 @@ struct DevicePlan {
     int LA, LB, LC;
     int PA, PB, PC;
     int sub;                                 // 3*PA*PB*PC
-    int rA, rB, rC;                          // ghost width = max |translation| per direction over all table entries
+    int rA, rB, rC;                          // ghost width: the reach (max |translation| per direction over all table entries) times ghost_mult
+    int ghost_mult;                          // 1, or 2 when the one-pass plane-marching kernel is in use (its rim predictor reads n two reaches out)
     int gA, gB, gC;                          // periodic images to maintain in that direction
     int pair_begin[SPIN_MAX_BASIS + 1];
     int quad_begin[SPIN_MAX_BASIS + 1];
@@ -153,7 +154,7 @@ struct spin_system {
     bool has_device;               // false only in the planner-only mode used by the CPU tests
     std::string jit_note;          // why the specialised sweeps are not in use, if they are not
     // ---- execution options / bookkeeping
-    int opt_graph, opt_store_A, opt_jit, opt_ddi_slab, opt_ddi_mirror, opt_pdl, opt_cache_noise, opt_coop;
+    int opt_graph, opt_store_A, opt_jit, opt_ddi_slab, opt_ddi_mirror, opt_pdl, opt_cache_noise, opt_coop, opt_march;
     cudaGraphExec_t graph_exec[2];   // one captured graph per ping-pong parity
     int graph_steps;
     int64_t n_launch, n_fft;
@@ -192,6 +193,10 @@ const char *jit_log(const spin_system *s);
 // one stage of the RK4 solver (jit_rk4_stage)
 int jit_launch_rk4_stage(spin_system *s, const double *base, const double *y, double *ynext, double *acc, double *noise, const double *fddi,
                          int stage, unsigned step_add);
+// the whole Depondt step in one pass (jit_depondt_march, spin_jit_march.cuh): 3-D lattices of one basis atom without dipolar coupling
+bool march_eligible(const spin_system *s);      // spin_api.cu: decided from the system alone (the planner doubles the ghost layers for it)
+bool jit_march_ready(const spin_system *s);
+int jit_launch_march(spin_system *s, int cur, double *nout, unsigned step_add);
 // all steps of an llg_iterate call in one cooperative launch (jit_steps_coop)
 bool jit_coop_ready(const spin_system *s);
 bool jit_cluster_ready(const spin_system *s);

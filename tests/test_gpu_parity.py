@@ -996,3 +996,67 @@ def test_slab_reach_two_and_other_solvers(P, O):
         assert np.array_equal(grp.spins(), ref.spins_get()), solver
     with pytest.raises(P.SpinError):
         grp.drivers[0].sys.llg_iterate(1)
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# One-pass plane-marching Depondt step (csrc/spin_jit_march.cuh; option use_march, default for 3-D lattices of one basis atom from 65536
+# spins on, 2 forces it): n planes staged by TMA, predictor for tile + rim into a shared-memory ring, corrector from the ring.  Same
+# arithmetic as the brick sweeps: bit-identical results, whatever the tile, chunking, boundary conditions, noise, pins or moments.
+MARCH_CASES = [
+    (3, (64, 32, 16), (1, 1, 1), 0.0, 30),
+    (3, (70, 37, 45), (1, 1, 1), 0.0, 20),        # ragged in a and b: tiles hang over the lattice
+    (3, (33, 9, 8), (1, 0, 1), 20.0, 30),         # open along b, thermal field
+    (3, (40, 24, 12), (0, 0, 0), 0.0, 30),        # open everywhere
+    (3, (96, 16, 24), (1, 1, 0), 10.0, 20),       # open along c (the marching direction)
+    (5, (64, 24, 10), (1, 1, 0), 0.0, 20),        # film Hamiltonian without the dipolar term
+]
+
+
+@pytest.mark.parametrize("cfg,cells,per,T,steps", MARCH_CASES)
+def test_one_pass_marching_step_is_bit_identical(P, O, cfg, cells, per, T, steps):
+    w = dataclasses.replace(W.CONFIGS[cfg]().resized(cells, steps), periodic=per, T=T, ddi=False)
+    g, o = pair(P, O, w)
+    g.spin_set_option("use_march", 2)
+    assert g.spin_kernel_info() == "jit+march", g.spin_kernel_info()
+    assert_fields_close(g.effective_field(), o.effective_field())          # the wider ghost layers change nothing the other kernels see
+    g.llg_iterate(steps); o.iterate(steps)
+    d = np.abs(g.spins_get() - o.spins()).max()
+    assert d <= SPIN_ATOL, d
+    b = P.SpinSystem.from_workload(w)
+    b.spin_set_option("use_march", 0); b.spin_set_option("use_coop", 0)
+    assert b.spin_kernel_info() == "jit (brick sweeps)"
+    b.llg_iterate(steps)
+    assert np.array_equal(b.spins_get(), g.spins_get())
+    # split calls, graph replay (16-step graphs) and single steps give the same trajectory
+    h = P.SpinSystem.from_workload(w); h.spin_set_option("use_march", 2)
+    h.llg_iterate(steps - 3); h.llg_iterate(3)
+    assert np.array_equal(h.spins_get(), g.spins_get())
+
+
+def test_one_pass_marching_step_with_pins_moments_current_and_long_reach(P, O):
+    """Pinned spins and vacancies, per-site moments, a current with all three components, pairs reaching two sites along every direction."""
+    w = W.config3().resized((48, 20, 16), 20)
+    pt = np.vstack([w.pair_t, [[0, 0, 2], [2, 0, 0], [0, 2, 1], [1, -2, 0]]]); z4 = np.zeros(4, int)
+    w = dataclasses.replace(w, pair_i=np.r_[w.pair_i, z4], pair_j=np.r_[w.pair_j, z4], pair_t=pt, pair_J=np.r_[w.pair_J, 0.3, -0.2, 0.15, 0.1],
+                            pair_D=np.vstack([w.pair_D, [[0.05, 0, 0.1], [0, 0.07, 0], [0.02, 0.01, 0], [0, 0, 0.03]]]), T=8.0, u=0.3, j_dir=(0.5, 0.3, 0.8), beta=0.07)
+    rng = np.random.default_rng(5)
+    g, o = pair(P, O, w)
+    N = g.N
+    mask = (rng.random(N) < 0.08).astype(np.uint8)
+    n0 = w.initial_spins(); n0[(rng.random(N) < 0.03) & (mask == 1)] = 0.0          # some pinned sites are vacancies
+    mu = rng.uniform(0.8, 3.0, N)
+    for s_ in (g,):
+        s_.spin_set_option("use_march", 2); s_.spins_set_pinned(mask); s_.spins_set(n0); s_.hamiltonian_set_site_mu_s(mu)
+    o.set_pinned(mask); o.set_spins(n0); o.set_site_mu_s(mu)
+    assert g.spin_kernel_info() == "jit+march"
+    g.llg_iterate(20); o.iterate(20)
+    assert np.abs(g.spins_get() - o.spins()).max() <= SPIN_ATOL
+    b = P.SpinSystem.from_workload(w); b.spin_set_option("use_march", 0); b.spin_set_option("use_coop", 0)
+    b.spins_set_pinned(mask); b.spins_set(n0); b.hamiltonian_set_site_mu_s(mu)
+    b.llg_iterate(20)
+    assert np.array_equal(b.spins_get(), g.spins_get())
+
+
+def test_full_size_cfg3_takes_the_one_pass_kernel(P):
+    g = P.SpinSystem.from_workload(W.config3(), set_spins=False)
+    assert g.spin_kernel_info() == "jit+march"
