@@ -112,7 +112,7 @@ static void jit_brick_launch(const spin_system *s, dim3 &grid, dim3 &block) {
 
 // geometry of the one-pass plane-marching kernel: rows per tile, chunks along c, threads, shared memory; false if it does not apply
 namespace {
-struct MarchGeo { int ra, rb, rc, ty, nzc, threads, items; size_t smem; };
+struct MarchGeo { int ra, rb, rc, ty, nzc, look, blocks, threads, items; size_t smem; };
 bool plan_march(const spin_system *s, MarchGeo &g) {
     const DevicePlan &P = s->plan;
     if (!spin::march_eligible(s) || P.ghost_mult != 2) return false;
@@ -123,16 +123,18 @@ bool plan_march(const spin_system *s, MarchGeo &g) {
     const int sms = sm_count(s);
     double best = -1.0;
     bool found = false;
-    int force_ty = 0, force_nzc = 0;
-    if (const char *e = getenv("SPINLLG_MARCH_GEO")) sscanf(e, "%d,%d", &force_ty, &force_nzc);      // TEMPORARY tuning hook
+    int force_ty = 0, force_nzc = 0, force_look = 0;
+    if (const char *e = getenv("SPINLLG_MARCH_GEO")) sscanf(e, "%d,%d,%d", &force_ty, &force_nzc, &force_look);      // TEMPORARY tuning hook
+    for (int look : {2, 3, 1})
     for (int ty : {8, 12, 16, 6, 4}) {                       // tile rows; prefer tiles that divide the lattice
         if (force_ty && ty != force_ty) continue;
+        if (force_look && look != force_look) continue;
         const int py = ty + 2 * g.rb, rimw = (2 * g.ra * py + 31) / 32, threads = 32 * (py + rimw);
         if (threads > 1024) continue;
         const size_t nslot = ((size_t)3 * (32 + 2 * hx) * (ty + 4 * g.rb) + 15) / 16 * 16, ppl = (size_t)3 * (32 + 2 * g.ra) * py;
-        const size_t smem = ((size_t)(2 * g.rc + 3) * nslot + (size_t)(2 * g.rc + 2) * ppl) * 8 + (size_t)(2 * g.rc + 3) * 8;
+        const size_t smem = ((size_t)(2 * g.rc + 1 + look) * nslot + (size_t)(2 * g.rc + 2) * ppl) * 8 + (size_t)(2 * g.rc + 1 + look) * 8;
         if (smem > 200 * 1024) continue;
-        const int per_sm = (int)std::min<size_t>((size_t)(227 * 1024) / (smem + 1024), (size_t)std::min(2048 / threads, 65536 / (threads * 72)));
+        const int per_sm = (int)std::min<size_t>((size_t)(227 * 1024) / (smem + 1024), (size_t)std::min(2048 / threads, 65536 / (threads * 56)));
         if (per_sm < 1) continue;
         const int cols = ((P.Na + 31) / 32) * ((P.Nb + ty - 1) / ty), slots = sms * per_sm;
         for (int nzc = 1; nzc <= P.Nc / 4; ++nzc) {
@@ -141,9 +143,11 @@ bool plan_march(const spin_system *s, MarchGeo &g) {
             const long waves = (items + slots - 1) / slots;
             const double cz = (double)P.Nc / nzc;
             // useful fraction: full waves x chunk overlap of the predictor x rim of the tile x rows that hang over the lattice
+            // (one block per SM stalls the whole SM at its barrier, and one plane of look-ahead does not cover the HBM latency: measured 7 % and
+            // 12-20 % slower on cfg3, profiles/r2_README.md)
             const double eff = (double)items / (double)(waves * slots) * cz / (cz + 2.0 * g.rc) * (32.0 * ty) / (double)((32 + 2 * g.ra) * py) *
-                               (double)P.Nb / (double)(((P.Nb + ty - 1) / ty) * ty);
-            if (eff > best + 1e-9) { best = eff; found = true; g.ty = ty; g.nzc = nzc; g.threads = threads; g.items = (int)items; g.smem = smem; }
+                               (double)P.Nb / (double)(((P.Nb + ty - 1) / ty) * ty) * (per_sm == 1 ? 0.85 : 1.0) * (look == 1 ? 0.8 : (look == 3 ? 0.99 : 1.0));
+            if (eff > best + 1e-9) { best = eff; found = true; g.ty = ty; g.nzc = nzc; g.look = look; g.blocks = per_sm; g.threads = threads; g.items = (int)items; g.smem = smem; }
         }
     }
     return found;
@@ -259,7 +263,7 @@ std::string spin::jit_source(const spin_system *s) {
     MarchGeo mg;
     if (plan_march(s, mg))
         o << "namespace spec { constexpr int MRA = " << mg.ra << ", MRB = " << mg.rb << ", MRC = " << mg.rc << ", MTY = " << mg.ty << ", MNZC = " << mg.nzc
-          << "; }\n#define SPIN_MARCH 1\n";
+          << ", MLOOK = " << mg.look << ", MBLOCKS = " << mg.blocks << "; }\n#define SPIN_MARCH 1\n";
     o << "#include \"spin_jit_kernels.cuh\"\n";
     return o.str();
 }

@@ -17,7 +17,7 @@
 // HBM traffic: read n once (+ chunk overlap), write n once = 48-60 B per spin-update instead of 120.
 //
 // spec must also define: int MRA, MRB, MRC (reach of the Hamiltonian; ghost widths RA, RB, RC are twice that), MTY (rows per tile),
-// MNZC (chunks along c).
+// MNZC (chunks along c), MLOOK (planes of look-ahead), MBLOCKS (blocks per SM the geometry was planned for).
 #pragma once
 
 namespace spinmarch {
@@ -31,7 +31,8 @@ constexpr int NX = 32 + 2 * HX, NY = TY + 4 * RB;                // staged n pla
 constexpr int NROW = 3 * NX, NPL = NROW * NY, NSLOT = (NPL + 15) / 16 * 16;      // doubles; slots are 128-byte multiples
 constexpr int PX = 32 + 2 * RA, PY = TY + 2 * RB;                // n^p plane (rim of one reach)
 constexpr int PROW = 3 * PX, PPL = PROW * PY;
-constexpr int RN = 2 * RC + 3, RP = 2 * RC + 2;                  // ring depths: n planes (two of look-ahead), n^p planes
+constexpr int LOOK = spec::MLOOK;                                // n planes in flight beyond the ones the current predictor reads
+constexpr int RN = 2 * RC + 1 + LOOK, RP = 2 * RC + 2;           // ring depths: n planes, n^p planes
 constexpr int RIM = 2 * RA * PY, RIMW = (RIM + 31) / 32;         // sites of the rim columns, warps that take them
 constexpr int NWARP = PY + RIMW, NTHREADS = 32 * NWARP;
 constexpr int NTX = (spec::NA + 31) / 32, NTY = (spec::NB + TY - 1) / TY;
@@ -70,7 +71,7 @@ struct RingAcc {
 };
 }  // namespace spinmarch
 
-extern "C" __global__ void SPIN_BOUNDS(spinmarch::NTHREADS)
+extern "C" __global__ void __launch_bounds__(spinmarch::NTHREADS, spec::MBLOCKS)
     jit_depondt_march(const __grid_constant__ spinmarch::TensorMap tm_n, double *__restrict__ nout, const unsigned long long *__restrict__ d_step,
                       unsigned int step_add, unsigned int seed_lo, unsigned int seed_hi, const unsigned char *__restrict__ pin,
                       const double *__restrict__ mu_ratio) {
@@ -125,11 +126,15 @@ extern "C" __global__ void SPIN_BOUNDS(spinmarch::NTHREADS)
 #pragma unroll
     for (int p = 0; p < 2 * RC; ++p) mbar_wait(bars + 8u * p, 0u);
     const int NIT = zb - za + 2 * RC;
+    // ring positions kept incrementally (no division in the loop): ns = k mod RN, ps = k mod RP, (wslot, wpar) = slot and parity of plane k + 2 RC
+    int ns = 0, ps = 0, wslot = (2 * RC) % RN, wpar = ((2 * RC) / RN) & 1;
+    auto nslot_of = [&](int d) { int t = ns + d; return t >= RN ? t - RN : t; };                 // slot of n plane k + d, 0 <= d <= 2 RC
+    auto pslot_of = [&](int d) { int t = ps + d; return t < 0 ? t + RP : t; };                   // slot of n^p plane k + d, -2 RC <= d <= 0
     for (int k = 0; k < NIT; ++k) {                                // predictor plane zP = za - RC + k from n planes k .. k + 2 RC
-        mbar_wait(bars + 8u * ((k + 2 * RC) % RN), (u32)(((k + 2 * RC) / RN) & 1));
+        mbar_wait(bars + 8u * wslot, (u32)wpar);
         const int zP = za - RC + k;
         double n_cur[3] = {0.0, 0.0, 0.0}, A_cur[3] = {0.0, 0.0, 0.0}, th_cur[3] = {0.0, 0.0, 0.0};
-        double *pslot = pring + (k % RP) * PPL;
+        double *pslot = pring + ps * PPL;
         if (mine) {
             double out[3] = {0.0, 0.0, 0.0};
             const bool live = live_xy && (spec::PER_C || (zP >= 0 && zP < spec::NC));
@@ -137,7 +142,7 @@ extern "C" __global__ void SPIN_BOUNDS(spinmarch::NTHREADS)
                 c.ic = zP < 0 ? zP + spec::NC : (zP >= spec::NC ? zP - spec::NC : zP);
                 RingAcc<NX, NROW> acc;
 #pragma unroll
-                for (int dz = -RC; dz <= RC; ++dz) acc.pl[dz + RC] = nring + ((k + RC + dz) % RN) * NSLOT + ncell;
+                for (int dz = -RC; dz <= RC; ++dz) acc.pl[dz + RC] = nring + nslot_of(RC + dz) * NSLOT + ncell;
                 double own[1][3], F[1][3], sg[1][3] = {{0.0, 0.0, 0.0}};
                 acc.template load<0, 0, 0, 0, 0>(0, own[0]);
                 n_cur[0] = own[0][0]; n_cur[1] = own[0][1]; n_cur[2] = own[0][2];
@@ -156,7 +161,7 @@ extern "C" __global__ void SPIN_BOUNDS(spinmarch::NTHREADS)
             pslot[pcell] = out[0]; pslot[pcell + PX] = out[1]; pslot[pcell + 2 * PX] = out[2];
         }
         __syncthreads();                                           // n^p(zP) is complete; nobody reads n plane k any more
-        if (tid == 0 && k + RN - 1 < NP) issue(k + RN - 1);        // refill a free slot, two planes ahead of the next predictor
+        if (tid == 0 && k + RN - 1 < NP) issue(k + RN - 1);        // refill a free slot, LOOK planes ahead of the next predictor
         const int zC = zP - RC;
         if (k >= 2 * RC && tile_site) {                            // corrector of plane zC from n^p planes zC - RC .. zC + RC = zP
             c.ic = zC;
@@ -166,7 +171,7 @@ extern "C" __global__ void SPIN_BOUNDS(spinmarch::NTHREADS)
                 const double zr = site_ratio<0>(mu_ratio, c), ir = spec::HAS_SITE_MU ? 1.0 / zr : 1.0;
                 RingAcc<PX, PROW> acc;
 #pragma unroll
-                for (int dz = -RC; dz <= RC; ++dz) acc.pl[dz + RC] = pring + ((k - RC + dz) % RP) * PPL + pcell;
+                for (int dz = -RC; dz <= RC; ++dz) acc.pl[dz + RC] = pring + pslot_of(dz - RC) * PPL + pcell;
                 double own[1][3], F[1][3] = {{th_q[0][0], th_q[0][1], th_q[0][2]}}, sg[1][3] = {{0.0, 0.0, 0.0}}, Ap[3];
                 acc.template load<0, 0, 0, 0, 0>(0, own[0]);
                 force<0, 1>(acc, own, F, zr);
@@ -185,5 +190,8 @@ extern "C" __global__ void SPIN_BOUNDS(spinmarch::NTHREADS)
             for (int q = 0; q < 3; ++q) { n_q[r][q] = n_q[r + 1][q]; A_q[r][q] = A_q[r + 1][q]; th_q[r][q] = th_q[r + 1][q]; }
 #pragma unroll
         for (int q = 0; q < 3; ++q) { n_q[RC - 1][q] = n_cur[q]; A_q[RC - 1][q] = A_cur[q]; th_q[RC - 1][q] = th_cur[q]; }
+        if (++ns == RN) ns = 0;
+        if (++ps == RP) ps = 0;
+        if (++wslot == RN) { wslot = 0; wpar ^= 1; }
     }
 }
