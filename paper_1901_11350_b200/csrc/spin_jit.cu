@@ -123,12 +123,8 @@ bool plan_march(const spin_system *s, MarchGeo &g) {
     const int sms = sm_count(s);
     double best = -1.0;
     bool found = false;
-    int force_ty = 0, force_nzc = 0, force_look = 0;
-    if (const char *e = getenv("SPINLLG_MARCH_GEO")) sscanf(e, "%d,%d,%d", &force_ty, &force_nzc, &force_look);      // TEMPORARY tuning hook
     for (int look : {2, 3, 1})
     for (int ty : {8, 12, 16, 6, 4}) {                       // tile rows; prefer tiles that divide the lattice
-        if (force_ty && ty != force_ty) continue;
-        if (force_look && look != force_look) continue;
         const int py = ty + 2 * g.rb, rimw = (2 * g.ra * py + 31) / 32, threads = 32 * (py + rimw);
         if (threads > 1024) continue;
         const size_t nslot = ((size_t)3 * (32 + 2 * hx) * (ty + 4 * g.rb) + 15) / 16 * 16, ppl = (size_t)3 * (32 + 2 * g.ra) * py;
@@ -138,7 +134,6 @@ bool plan_march(const spin_system *s, MarchGeo &g) {
         if (per_sm < 1) continue;
         const int cols = ((P.Na + 31) / 32) * ((P.Nb + ty - 1) / ty), slots = sms * per_sm;
         for (int nzc = 1; nzc <= P.Nc / 4; ++nzc) {
-            if (force_nzc && nzc != force_nzc) continue;
             const long items = (long)cols * nzc;
             const long waves = (items + slots - 1) / slots;
             const double cz = (double)P.Nc / nzc;
