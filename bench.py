@@ -219,6 +219,13 @@ def measure_workload(P, torch, w, stream, steps, warmup, min_seconds, barrier=No
         share = per_iter["ddi_contract"] / tot
         launch_ms = ms_iter * share / 2
         roof["note"] = "dominant kernel of the dipolar evaluation (cuFFT's b-passes are library kernels); two launches per Depondt iteration"
+    elif "march" in kinfo:
+        # the whole Depondt step is ONE kernel (n^p never leaves the SM): one launch = one iteration.  The roofline figure stays the method's
+        # 120 B per spin-update (read n, write n^p; read n^p, read n, write n); the kernel's own DRAM traffic (`traffic`, about
+        # 43 B per spin-update) is lower because it skips the n^p round trip and the second read of n.
+        kernel, nbytes = "jit_depondt_march", step_bytes
+        share, launch_ms = 1.0, ms_iter
+        roof["note"] = "one-pass plane-marching kernel: one launch per Depondt iteration; algorithmic bytes of the two-sweep method (120 B per spin-update)"
     elif "cluster" in kinfo or "coop" in kinfo:
         # launch-bound lattices: all steps in one launch, the state (24 KB-100 KB) never leaves L2; the figure is the effective bandwidth of
         # a step and says how far from HBM-bound the workload is, not how good the kernel is (its bound is the barrier latency)
