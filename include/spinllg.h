@@ -217,7 +217,7 @@ int llg_slab_advance(spin_system *sys);
  *                    1 dependents released at entry, 2 at the end of each block
  *   store_A     (0)  1: the predictor stores the rotation field A(n) and the corrector reads it instead of recomputing it
  *   cache_noise (1)  the predictor keeps the thermal field of the step (24 B/spin) for the corrector instead of generating it twice
- *   ddi_slab    (1)  thin films with one basis atom take the dipolar slab path; 2: the same with cuFFT's transform along a instead of
+ *   ddi_slab    (1)  thin films (up to 8 planes; 4 with several basis atoms) take the dipolar slab path; 2: the same with cuFFT's transform along a instead of
  *                    the hand-written one; 0: the general 3-D transform
  *   ddi_mirror  (1)  the slab contraction reads PZ/2 + 1 tensor planes when the spectrum is mirror symmetric along c; 0: all PZ planes    */
 int spin_set_option(spin_system *sys, const char *name, int value);
@@ -235,7 +235,7 @@ int spin_profile_get(spin_system *sys, int kind, double *total_ms, int64_t *laun
 int spin_measure_fp64_tflops(spin_system *sys, double *tflops);
 /* which sweep kernels are in use: "jit+cluster", "jit+coop", "jit (brick sweeps)" or "generic: <why>"                              */
 int spin_kernel_info(spin_system *sys, char *buf, int len);
-/* Which dipolar path the plan chose: "off", "3d" (general zero-padded 3-D transform) or "slab" (thin film of one basis atom, 1-8 planes:
+/* Which dipolar path the plan chose: "off", "3d" (general zero-padded 3-D transform) or "slab" (thin film of 1-8 planes, or 1-4 planes with several basis atoms:
  * transforms in the a-b plane, hand-written transform along c fused with the tensor contraction), followed by "+mirror" when the
  * contraction reads PZ/2 + 1 of the PZ tensor planes (spectrum found mirror symmetric along c) and by "+own-a" when the transform along a
  * is the hand-written one (rows of power-of-two length) instead of cuFFT's.                                                        */

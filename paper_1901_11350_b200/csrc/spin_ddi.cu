@@ -44,7 +44,7 @@ struct DdiState {
     // s_b complex (b-pass output, contracted in place), s_d complex (inverse b-pass), s_out real [Nb][SL][P0].
     cufftHandle plan_a_fwd, plan_a_inv, plan_b;
     double *s_in, *s_out;
-    cufftDoubleComplex *s_a, *s_b, *s_d;
+    cufftDoubleComplex *s_a, *s_b, *s_c, *s_d;
     double *d_Kre;             // [6][PZ][S2] real: the tensor spectrum is real for a single basis atom (the kernel is even)
     bool own_a;                // the a-pass is ddi_apass_fwd / ddi_apass_inv (rows of power-of-two length) instead of scatter + cuFFT + gather
     int a_rows_per_block;      // rows (warps) per block of those kernels
@@ -152,26 +152,28 @@ __global__ void ddi_gather_kernel(const __grid_constant__ DevicePlan L, const do
     for (int k = 0; k < 3; ++k) f[j + k * L.PA] = m * Hpad[(size_t)(b * 3 + k) * Ptot + p];
 }
 
-// slab path: the same two copies in the row-interleaved layout [ib][slab = comp NZ + ic][ia] (one basis atom)
-__global__ void ddi_slab_scatter_kernel(const __grid_constant__ DevicePlan L, const double *__restrict__ n, int P0, int SL, double mu,
+// slab path: the same two copies in the row-interleaved layout [ib][slab = (b 3 + comp) NZ + ic][ia]
+__global__ void ddi_slab_scatter_kernel(const __grid_constant__ DevicePlan L, const double *__restrict__ n, int P0, int SL, const double *__restrict__ mu,
                                         double *__restrict__ in) {
-    const int cell = blockIdx.x * blockDim.x + threadIdx.x;
-    if (cell >= L.Ncell) return;
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;      // b * Ncell + cell
+    if (i >= L.nb * L.Ncell) return;
+    const int b = i / L.Ncell, cell = i - b * L.Ncell;
     const int ia = cell % L.Na, ib = (cell / L.Na) % L.Nb, ic = cell / (L.Na * L.Nb);
-    const int j = ((ic + L.LC) * L.PB + (ib + L.LB)) * (3 * L.PA) + (ia + L.LA);
-    const double m = mu * (L.mu_ratio ? L.mu_ratio[cell] : 1.0);
+    const int j = b * L.sub + ((ic + L.LC) * L.PB + (ib + L.LB)) * (3 * L.PA) + (ia + L.LA);
+    const double m = mu[b] * (L.mu_ratio ? L.mu_ratio[b + L.nb * cell] : 1.0);
 #pragma unroll
-    for (int k = 0; k < 3; ++k) in[((size_t)ib * SL + (k * L.Nc + ic)) * P0 + ia] = m * n[j + k * L.PA];
+    for (int k = 0; k < 3; ++k) in[((size_t)ib * SL + ((b * 3 + k) * L.Nc + ic)) * P0 + ia] = m * n[j + k * L.PA];
 }
-__global__ void ddi_slab_gather_kernel(const __grid_constant__ DevicePlan L, const double *__restrict__ out, int P0, int SL, double scale,
-                                       double *__restrict__ f) {
-    const int cell = blockIdx.x * blockDim.x + threadIdx.x;
-    if (cell >= L.Ncell) return;
+__global__ void ddi_slab_gather_kernel(const __grid_constant__ DevicePlan L, const double *__restrict__ out, int P0, int SL, const double *__restrict__ mu,
+                                       double scale, double *__restrict__ f) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= L.nb * L.Ncell) return;
+    const int b = i / L.Ncell, cell = i - b * L.Ncell;
     const int ia = cell % L.Na, ib = (cell / L.Na) % L.Nb, ic = cell / (L.Na * L.Nb);
-    const int j = ((ic + L.LC) * L.PB + (ib + L.LB)) * (3 * L.PA) + (ia + L.LA);
-    const double m = scale * (L.mu_ratio ? L.mu_ratio[cell] : 1.0);
+    const int j = b * L.sub + ((ic + L.LC) * L.PB + (ib + L.LB)) * (3 * L.PA) + (ia + L.LA);
+    const double m = mu[b] * scale * (L.mu_ratio ? L.mu_ratio[b + L.nb * cell] : 1.0);
 #pragma unroll
-    for (int k = 0; k < 3; ++k) f[j + k * L.PA] = m * out[((size_t)ib * SL + (k * L.Nc + ic)) * P0 + ia];
+    for (int k = 0; k < 3; ++k) f[j + k * L.PA] = m * out[((size_t)ib * SL + ((b * 3 + k) * L.Nc + ic)) * P0 + ia];
 }
 
 
@@ -254,15 +256,24 @@ __device__ __forceinline__ double2 *ddi_warp_fft(double2 *a, double2 *b, const i
     return a;
 }
 
-// rows = Nb * SL occupied rows, row = ib SL + slab, slab = comp Nc + ic; out: element k of the row at row * S1p + k, k = 0 .. M
+// per-site moment ratios of the sites 2j, 2j+1 of row (b, ib, ic) in boundary order b + nb * cell (one vector load for one sublattice)
+__device__ __forceinline__ double2 ddi_row_ratio(const DevicePlan &L, int b, int ib, int ic, int j) {
+    const size_t cell0 = (size_t)L.Na * (ib + (size_t)L.Nb * ic) + 2 * (size_t)j;
+    if (L.nb == 1) return __ldg((const double2 *)(L.mu_ratio + cell0));
+    return make_double2(__ldg(L.mu_ratio + b + (size_t)L.nb * cell0), __ldg(L.mu_ratio + b + (size_t)L.nb * (cell0 + 1)));
+}
+
+// rows = Nb * SL occupied rows, row = ib SL + slab, slab = (b 3 + comp) Nc + ic; out: element k of the row at row * S1p + k, k = 0 .. M
 __global__ void __launch_bounds__(256) ddi_apass_fwd_kernel(const __grid_constant__ DevicePlan L, const double *__restrict__ n, int M, int SL, int S1p, int rows,
-                                                            int rows_per_block, double mu, const double2 *__restrict__ tw, cufftDoubleComplex *__restrict__ out) {
+                                                            int rows_per_block, const double *__restrict__ mu_b, const double2 *__restrict__ tw,
+                                                            cufftDoubleComplex *__restrict__ out) {
     extern __shared__ double2 ddi_sm[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int row = blockIdx.x * rows_per_block + warp;
     if (warp >= rows_per_block || row >= rows) return;
-    const int ib = row / SL, slab = row - ib * SL, comp = slab / L.Nc, ic = slab - comp * L.Nc;
-    const double2 *src = (const double2 *)(n + ((size_t)(ic + L.LC) * L.PB + (ib + L.LB)) * (3 * L.PA) + comp * L.PA + L.LA);
+    const int ib = row / SL, slab = row - ib * SL, bc = slab / L.Nc, ic = slab - bc * L.Nc, sb = bc / 3, comp = bc - 3 * sb;
+    const double mu = mu_b[sb];
+    const double2 *src = (const double2 *)(n + (size_t)sb * L.sub + ((size_t)(ic + L.LC) * L.PB + (ib + L.LB)) * (3 * L.PA) + comp * L.PA + L.LA);
     const int MP = M + (M >> 3);                        // padded row
     double2 *a = ddi_sm + (size_t)warp * 2 * MP, *b = a + MP;
     for (int j = lane; j < M; j += 32) {
@@ -270,7 +281,7 @@ __global__ void __launch_bounds__(256) ddi_apass_fwd_kernel(const __grid_constan
         if (j < M / 2) {
             v = __ldg(src + j);
             double m0 = mu, m1 = mu;
-            if (L.mu_ratio) { const double2 r = __ldg((const double2 *)(L.mu_ratio + (size_t)L.Na * (ib + (size_t)L.Nb * ic)) + j); m0 *= r.x; m1 *= r.y; }
+            if (L.mu_ratio) { const double2 r = ddi_row_ratio(L, sb, ib, ic, j); m0 *= r.x; m1 *= r.y; }
             v.x *= m0; v.y *= m1;
         }
         a[ddi_pad(j)] = v;
@@ -289,12 +300,14 @@ __global__ void __launch_bounds__(256) ddi_apass_fwd_kernel(const __grid_constan
 
 // inverse: from the half spectrum X(k), k = 0 .. M, of every occupied row to P0 x(ia), ia < Na, scaled and written as the dipolar force
 __global__ void __launch_bounds__(256) ddi_apass_inv_kernel(const __grid_constant__ DevicePlan L, const cufftDoubleComplex *__restrict__ in, int M, int SL, int S1p,
-                                                            int rows, int rows_per_block, double scale, const double2 *__restrict__ tw, double *__restrict__ f) {
+                                                            int rows, int rows_per_block, const double *__restrict__ mu_b, double scale0, const double2 *__restrict__ tw,
+                                                            double *__restrict__ f) {
     extern __shared__ double2 ddi_sm[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int row = blockIdx.x * rows_per_block + warp;
     if (warp >= rows_per_block || row >= rows) return;
-    const int ib = row / SL, slab = row - ib * SL, comp = slab / L.Nc, ic = slab - comp * L.Nc;
+    const int ib = row / SL, slab = row - ib * SL, bc = slab / L.Nc, ic = slab - bc * L.Nc, sb = bc / 3, comp = bc - 3 * sb;
+    const double scale = mu_b[sb] * scale0;
     const cufftDoubleComplex *src = in + (size_t)row * S1p;
     const int MP = M + (M >> 3);
     double2 *a = ddi_sm + (size_t)warp * 2 * MP, *b = a + MP;
@@ -308,11 +321,11 @@ __global__ void __launch_bounds__(256) ddi_apass_inv_kernel(const __grid_constan
     }
     __syncwarp();
     const double2 *z = ddi_warp_fft<+1>(a, b, M, tw, lane);
-    double2 *dst = (double2 *)(f + ((size_t)(ic + L.LC) * L.PB + (ib + L.LB)) * (3 * L.PA) + comp * L.PA + L.LA);
+    double2 *dst = (double2 *)(f + (size_t)sb * L.sub + ((size_t)(ic + L.LC) * L.PB + (ib + L.LB)) * (3 * L.PA) + comp * L.PA + L.LA);
     for (int j = lane; j < M / 2; j += 32) {
         const double2 v = z[ddi_pad(j)];
         double m0 = scale, m1 = scale;
-        if (L.mu_ratio) { const double2 r = __ldg((const double2 *)(L.mu_ratio + (size_t)L.Na * (ib + (size_t)L.Nb * ic)) + j); m0 *= r.x; m1 *= r.y; }
+        if (L.mu_ratio) { const double2 r = ddi_row_ratio(L, sb, ib, ic, j); m0 *= r.x; m1 *= r.y; }
         dst[j] = make_double2(m0 * v.x, m1 * v.y);
     }
 }
@@ -524,6 +537,99 @@ __global__ void __launch_bounds__(2 * DDI_CT_COLS, 4) ddi_slab_contract_kernel(c
     }
 }
 
+// The same for several basis atoms ("one FFT per sublattice + inter-sublattice convolutions"): H_a^(kz) = sum_b K_ab^(kz) . M_b^(kz)
+// with COMPLEX tensor spectra (K_ab(-Delta) = K_ba(Delta): only the diagonal blocks are even), read from the 3-D half spectrum
+// Khat[a][b][6][PZ][S2].  blockIdx.y = target sublattice a; the thread transforms the column of every source sublattice b in turn and
+// accumulates the contracted spectrum, then transforms back.  Out of place (M2 is read by every a): slabs are (b 3 + c) NZ + z.
+template <int NZ, bool PAD>
+__global__ void __launch_bounds__(2 * DDI_CT_COLS) ddi_slab_contract_mb_kernel(const cufftDoubleComplex *__restrict__ Khat, const cufftDoubleComplex *__restrict__ M2,
+                                                                                cufftDoubleComplex *__restrict__ H2, int nb, long long S2, int S1, int S1p) {
+    constexpr int PZ = PAD ? 2 * NZ : NZ;
+    static_assert(PAD || NZ == 1, "only a single plane goes unpadded");
+    __shared__ double2 half1[3 * NZ][DDI_CT_COLS];
+    const int lane_col = threadIdx.x % DDI_CT_COLS, e = threadIdx.x / DDI_CT_COLS, a = blockIdx.y;
+    const long long q = (long long)blockIdx.x * DDI_CT_COLS + lane_col;
+    const bool live = q < S2 && (PAD || e == 0);
+    const long long kb = live ? q / S1 : 0, ka = live ? q - kb * S1 : 0;
+    const size_t SLr = (size_t)nb * 3 * NZ;
+    const size_t col = (size_t)kb * SLr * S1p + ka;                // slab 0 of this wave vector
+    const size_t Ph = (size_t)PZ * S2;                             // points of one tensor component
+    double hr[3][NZ], hi[3][NZ];
+#pragma unroll
+    for (int c = 0; c < 3; ++c)
+#pragma unroll
+        for (int z = 0; z < NZ; ++z) { hr[c][z] = 0.0; hi[c][z] = 0.0; }
+    if (live) {
+        for (int b = 0; b < nb; ++b) {
+            double xr[3][NZ], xi[3][NZ];
+#pragma unroll
+            for (int c = 0; c < 3; ++c)
+#pragma unroll
+                for (int z = 0; z < NZ; ++z) {
+                    const cufftDoubleComplex v = M2[col + (size_t)((b * 3 + c) * NZ + z) * S1p];
+                    xr[c][z] = v.x; xi[c][z] = v.y;
+                }
+            if constexpr (PAD) {
+                if (e) {
+#pragma unroll
+                    for (int c = 0; c < 3; ++c)
+#pragma unroll
+                        for (int z = 1; z < NZ; ++z) {
+                            const double wr = DDI_TWR[PZ][z], wi = DDI_TWI[PZ][z], r = xr[c][z], i = xi[c][z];
+                            xr[c][z] = fma(r, wr, -i * wi); xi[c][z] = fma(r, wi, i * wr);
+                        }
+                }
+#pragma unroll
+                for (int c = 0; c < 3; ++c) ddi_dft_fwd<NZ>(xr[c], xi[c]);
+            }
+            const cufftDoubleComplex *K = Khat + (size_t)(a * nb + b) * 6 * Ph + q;
+            auto planes = [&](auto ec) {
+                constexpr int E = decltype(ec)::value;
+#pragma unroll
+                for (int j = 0; j < NZ; ++j) {
+                    const int kz = PAD ? 2 * j + E : 0, p = ddi_pos<NZ>(j);
+                    const size_t o = (size_t)kz * S2;
+                    const cufftDoubleComplex kxx = K[o], kxy = K[Ph + o], kxz = K[2 * Ph + o], kyy = K[3 * Ph + o], kyz = K[4 * Ph + o], kzz = K[5 * Ph + o];
+                    const double r0 = xr[0][p], r1 = xr[1][p], r2 = xr[2][p], i0 = xi[0][p], i1 = xi[1][p], i2 = xi[2][p];
+                    // complex (k . m): re = k.x m.x - k.y m.y, im = k.x m.y + k.y m.x
+                    hr[0][p] += kxx.x * r0 - kxx.y * i0 + kxy.x * r1 - kxy.y * i1 + kxz.x * r2 - kxz.y * i2;
+                    hi[0][p] += kxx.x * i0 + kxx.y * r0 + kxy.x * i1 + kxy.y * r1 + kxz.x * i2 + kxz.y * r2;
+                    hr[1][p] += kxy.x * r0 - kxy.y * i0 + kyy.x * r1 - kyy.y * i1 + kyz.x * r2 - kyz.y * i2;
+                    hi[1][p] += kxy.x * i0 + kxy.y * r0 + kyy.x * i1 + kyy.y * r1 + kyz.x * i2 + kyz.y * r2;
+                    hr[2][p] += kxz.x * r0 - kxz.y * i0 + kyz.x * r1 - kyz.y * i1 + kzz.x * r2 - kzz.y * i2;
+                    hi[2][p] += kxz.x * i0 + kxz.y * r0 + kyz.x * i1 + kyz.y * r1 + kzz.x * i2 + kzz.y * r2;
+                }
+            };
+            if (e) planes(spin_ddi_int<1>{}); else planes(spin_ddi_int<0>{});
+        }
+        if constexpr (PAD) {
+#pragma unroll
+            for (int c = 0; c < 3; ++c) ddi_dft_inv<NZ>(hr[c], hi[c]);
+            if (e) {
+#pragma unroll
+                for (int c = 0; c < 3; ++c)
+#pragma unroll
+                    for (int z = 0; z < NZ; ++z) {
+                        double r = hr[c][z], i = hi[c][z];
+                        if (z > 0) { const double wr = DDI_TWR[PZ][z], wi = -DDI_TWI[PZ][z]; const double t = fma(r, wr, -i * wi); i = fma(r, wi, i * wr); r = t; }
+                        half1[c * NZ + z][lane_col] = make_double2(r, i);
+                    }
+            }
+        }
+    }
+    if constexpr (PAD) __syncthreads();
+    if (live && e == 0) {
+#pragma unroll
+        for (int c = 0; c < 3; ++c)
+#pragma unroll
+            for (int z = 0; z < NZ; ++z) {
+                double r = hr[c][z], i = hi[c][z];
+                if constexpr (PAD) { const double2 h = half1[c * NZ + z][lane_col]; r += h.x; i += h.y; }
+                H2[col + (size_t)((a * 3 + c) * NZ + z) * S1p] = make_cuDoubleComplex(r, i);
+            }
+    }
+}
+
 // Is the tensor spectrum mirror symmetric along c, K_ab(kz) = s_ab K_ab(PZ - kz) with s = -1 for xz, yz and +1 otherwise?  (True when c is
 // perpendicular to a and b.)  out[0] = max |K(kz) - s K(PZ - kz)|, out[1] = max |K| as the bit patterns of non-negative doubles,
 // which order like unsigned integers.
@@ -571,7 +677,7 @@ void spin::ddi_release(spin_system *s) {
     if (!d) return;
     if (d->have_plans) { cufftDestroy(d->plan_r2c); cufftDestroy(d->plan_c2r); }
     if (d->slab) { cufftDestroy(d->plan_a_fwd); cufftDestroy(d->plan_a_inv); cufftDestroy(d->plan_b); }
-    cudaFree(d->s_in); cudaFree(d->s_out); cudaFree(d->s_a); cudaFree(d->s_b); cudaFree(d->s_d);
+    cudaFree(d->s_in); cudaFree(d->s_out); cudaFree(d->s_a); cudaFree(d->s_b); cudaFree(d->s_c); cudaFree(d->s_d);
     cudaFree(d->d_Kre); cudaFree(d->d_tw);
     cudaFree(d->d_Mpad); cudaFree(d->d_Hpad); cudaFree(d->d_Mhat); cudaFree(d->d_Hhat); cudaFree(d->d_Khat); cudaFree(d->d_geom);
     delete d;
@@ -591,12 +697,13 @@ int spin::ddi_prepare(spin_system *s) {
     for (int k = 2; k >= 0; --k) if (d->P[k] > 1) d->fdims[d->rank++] = d->P[k];
     d->Phalf = d->Ptot;
     if (d->rank > 0) { const int inner = d->fdims[d->rank - 1]; d->Phalf = d->Ptot / inner * (inner / 2 + 1); }
-    // slab path: one basis atom, both in-plane directions padded, at most 8 planes along c
+    // slab path: both in-plane directions padded, at most 8 planes along c
     d->NZ = s->nc[2]; d->PZ = d->P[2];
     d->R2 = (int64_t)d->P[0] * d->P[1]; d->S2 = (int64_t)d->P[1] * (d->P[0] / 2 + 1);
-    const bool want_slab = s->opt_ddi_slab && nb == 1 && d->P[0] > 1 && d->P[1] > 1 && d->NZ <= 8;
+    // several basis atoms: complex tensor spectra per sublattice pair, up to 4 planes (the contraction holds two columns in registers)
+    const bool want_slab = s->opt_ddi_slab && d->P[0] > 1 && d->P[1] > 1 && d->NZ <= (nb == 1 ? 8 : 4);
     size_t nreal = (size_t)nb * 3 * d->Ptot, ncplx = (size_t)nb * 3 * d->Phalf;
-    d->SL = 3 * d->NZ; d->S1 = d->P[0] / 2 + 1; d->S1p = d->S1;      // a 128-byte row pitch (264) was measured slower: 368 vs 347 us per step on cfg5
+    d->SL = 3 * d->NZ * nb; d->S1 = d->P[0] / 2 + 1; d->S1p = d->S1;      // a 128-byte row pitch (264) was measured slower: 368 vs 347 us per step on cfg5
     // own a-pass: rows of power-of-two length, 8 <= Na <= 2048 (option ddi_slab = 2 keeps cuFFT's, for comparison)
     const int Na = s->nc[0];
     d->own_a = want_slab && s->opt_ddi_slab == 1 && Na >= 8 && Na <= 2048 && (Na & (Na - 1)) == 0;
@@ -607,6 +714,7 @@ int spin::ddi_prepare(spin_system *s) {
         SPIN_CUDA(cudaMalloc(&d->s_a, nc_ * sizeof(cufftDoubleComplex)));
         SPIN_CUDA(cudaMalloc(&d->s_b, nc_ * sizeof(cufftDoubleComplex)));
         SPIN_CUDA(cudaMalloc(&d->s_d, nc_ * sizeof(cufftDoubleComplex)));
+        if (nb > 1) SPIN_CUDA(cudaMalloc(&d->s_c, nc_ * sizeof(cufftDoubleComplex)));      // the contraction of several sublattices is out of place
         SPIN_CUDA(cudaMemsetAsync(d->s_in, 0, nr * sizeof(double), s->stream));                    // ia >= Na: zero padding, never written
         SPIN_CUDA(cudaMemsetAsync(d->s_a, 0, nc_ * sizeof(cufftDoubleComplex), s->stream));        // rows >= Nb: zero padding, never written
         nreal = 1; ncplx = 1;      // the buffers of the general path are not needed
@@ -689,7 +797,7 @@ int spin::ddi_prepare(spin_system *s) {
             if (d->rank > 0) { SPIN_FFT(cufftExecD2Z(plan6, d_K6, dst)); s->n_fft++; }
             else { real_to_complex_kernel<<<1, 32, 0, s->stream>>>(d_K6, dst, 6); s->n_launch++; }
         }
-    if (want_slab) {       // keep the real part only (exactly real for one basis atom: K(-Delta) = K(Delta))
+    if (want_slab && nb == 1) {       // keep the real part only (exactly real for one basis atom: K(-Delta) = K(Delta))
         const long long nk = (long long)6 * d->Phalf;
         SPIN_CUDA(cudaMalloc(&d->d_Kre, (size_t)nk * sizeof(double)));
         real_part_kernel<<<(unsigned)((nk + 255) / 256), 256, 0, s->stream>>>(d->d_Khat, d->d_Kre, nk);
@@ -711,7 +819,7 @@ int spin::ddi_prepare(spin_system *s) {
     SPIN_CUDA(cudaGetLastError());
     cudaFree(d_K6);
     if (plan6) cufftDestroy(plan6);
-    if (want_slab) { cudaFree(d->d_Khat); d->d_Khat = nullptr; }
+    if (want_slab && nb == 1) { cudaFree(d->d_Khat); d->d_Khat = nullptr; }
     return SPIN_OK;
 }
 
@@ -721,14 +829,13 @@ int spin::ddi_field(spin_system *s, const double *d_n, double *d_f) {
     const int nb = s->nb, Ncell = (int)s->ncell, nspin = nb * Ncell, nt = 256;
     const unsigned gs = (unsigned)((nspin + nt - 1) / nt);
     if (d->slab) {
-        const unsigned gcell = (unsigned)((Ncell + nt - 1) / nt);
         const int a_rows = s->nc[1] * d->SL;
         const unsigned ga = d->own_a ? (unsigned)((a_rows + d->a_rows_per_block - 1) / d->a_rows_per_block) : 0u;
         if (d->own_a) {                                                               // scatter + a-pass over the occupied rows, one kernel
             ddi_apass_fwd_kernel<<<ga, 32 * d->a_rows_per_block, d->a_smem, s->stream>>>(s->plan, d_n, d->P[0] / 2, d->SL, d->S1p, a_rows, d->a_rows_per_block,
-                                                                                        s->mu[0], d->d_tw, d->s_a);
+                                                                                        d->d_geom, d->d_tw, d->s_a);
         } else {
-            ddi_slab_scatter_kernel<<<gcell, nt, 0, s->stream>>>(s->plan, d_n, d->P[0], d->SL, s->mu[0], d->s_in);
+            ddi_slab_scatter_kernel<<<gs, nt, 0, s->stream>>>(s->plan, d_n, d->P[0], d->SL, d->d_geom, d->s_in);
             SPIN_FFT(cufftExecD2Z(d->plan_a_fwd, d->s_in, d->s_a));                   // a-pass over the occupied rows only
         }
         SPIN_FFT(cufftExecZ2Z(d->plan_b, d->s_a, d->s_b, CUFFT_FORWARD));            // b-pass
@@ -736,7 +843,21 @@ int spin::ddi_field(spin_system *s, const double *d_n, double *d_f) {
 #define SPIN_CONTRACT(NZ_, PAD_, MIR_) ddi_slab_contract_kernel<NZ_, PAD_, MIR_><<<gq, 2 * DDI_CT_COLS, 0, s->stream>>>(d->d_Kre, d->s_b, d->s_b, (long long)d->S2, d->S1, d->S1p)
 #define SPIN_CONTRACT_NZ(NZ_) case NZ_: if (d->mirror) SPIN_CONTRACT(NZ_, true, true); else SPIN_CONTRACT(NZ_, true, false); break
         if (s->profile_on) cudaEventRecord(s->ev2, s->stream);
-        if (d->PZ == 1) SPIN_CONTRACT(1, false, false);                                 // a single unpadded plane: contraction only
+        cufftDoubleComplex *spec_out = d->s_b;                                          // what the inverse b-pass reads
+        if (nb > 1) {                                                                   // several sublattices: complex tensors, out of place
+            const dim3 gm(gq, (unsigned)nb);
+#define SPIN_CONTRACT_MB(NZ_, PAD_) ddi_slab_contract_mb_kernel<NZ_, PAD_><<<gm, 2 * DDI_CT_COLS, 0, s->stream>>>(d->d_Khat, d->s_b, d->s_c, nb, (long long)d->S2, d->S1, d->S1p)
+            if (d->PZ == 1) SPIN_CONTRACT_MB(1, false);
+            else switch (d->NZ) {
+                case 1: SPIN_CONTRACT_MB(1, true); break;
+                case 2: SPIN_CONTRACT_MB(2, true); break;
+                case 3: SPIN_CONTRACT_MB(3, true); break;
+                case 4: SPIN_CONTRACT_MB(4, true); break;
+                default: return spin::fail(SPIN_ERR_STATE, "dipolar slab path: %d planes with %d sublattices not supported", d->NZ, nb);
+            }
+#undef SPIN_CONTRACT_MB
+            spec_out = d->s_c;
+        } else if (d->PZ == 1) SPIN_CONTRACT(1, false, false);                          // a single unpadded plane: contraction only
         else switch (d->NZ) {                                                           // c-pass + contraction + inverse c-pass, in place
             SPIN_CONTRACT_NZ(1); SPIN_CONTRACT_NZ(2); SPIN_CONTRACT_NZ(3); SPIN_CONTRACT_NZ(4);
             SPIN_CONTRACT_NZ(5); SPIN_CONTRACT_NZ(6); SPIN_CONTRACT_NZ(7); SPIN_CONTRACT_NZ(8);
@@ -749,14 +870,14 @@ int spin::ddi_field(spin_system *s, const double *d_n, double *d_f) {
             float ms = 0.f; cudaEventElapsedTime(&ms, s->ev2, s->ev3);
             s->prof_ms[3] += ms; s->prof_n[3]++;
         }
-        SPIN_FFT(cufftExecZ2Z(d->plan_b, d->s_b, d->s_d, CUFFT_INVERSE));            // inverse b-pass
+        SPIN_FFT(cufftExecZ2Z(d->plan_b, spec_out, d->s_d, CUFFT_INVERSE));          // inverse b-pass
         if (d->own_a) {                                                               // inverse a-pass + gather, one kernel
             ddi_apass_inv_kernel<<<ga, 32 * d->a_rows_per_block, d->a_smem, s->stream>>>(s->plan, d->s_d, d->P[0] / 2, d->SL, d->S1p, a_rows, d->a_rows_per_block,
-                                                                                        s->mu[0] * C_DD / (double)d->Ptot, d->d_tw, d_f);
+                                                                                        d->d_geom, C_DD / (double)d->Ptot, d->d_tw, d_f);
             s->n_launch += 3; s->n_fft += 2;
         } else {
             SPIN_FFT(cufftExecZ2D(d->plan_a_inv, d->s_d, d->s_out));                  // inverse a-pass, occupied rows only
-            ddi_slab_gather_kernel<<<gcell, nt, 0, s->stream>>>(s->plan, d->s_out, d->P[0], d->SL, s->mu[0] * C_DD / (double)d->Ptot, d_f);
+            ddi_slab_gather_kernel<<<gs, nt, 0, s->stream>>>(s->plan, d->s_out, d->P[0], d->SL, d->d_geom, C_DD / (double)d->Ptot, d_f);
             s->n_launch += 3; s->n_fft += 4;
         }
         return SPIN_OK;

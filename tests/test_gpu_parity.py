@@ -322,6 +322,40 @@ def test_ddi_slab_path_matches_oracle_and_3d_path(P, O, cells, per, img):
     assert np.abs(g.spins_get() - o.spins()).max() <= SPIN_ATOL
 
 
+@pytest.mark.parametrize("cells,per,img,nbasis", [((12, 10, 1), (1, 1, 0), (2, 2, 0), 2), ((16, 6, 2), (1, 0, 0), (1, 0, 0), 2), ((8, 9, 4), (1, 1, 0), (1, 1, 0), 3),
+                                                   ((32, 8, 3), (0, 0, 0), (0, 0, 0), 2), ((10, 7, 4), (1, 1, 1), (1, 1, 1), 2)])
+def test_ddi_slab_path_with_several_basis_atoms(P, O, cells, per, img, nbasis):
+    """PAPER.md:87 "one FFT per sublattice + inter-sublattice convolutions", :89 "basis cells without inversion symmetry": films of 2 and 3
+    atoms per cell on the slab path (complex tensor spectra per sublattice pair), against the oracle's FFT path and its O(N^2) direct sum,
+    with per-site moments, and for a few steps of the trajectory."""
+    brav = np.array([[1, 0, 0], [0.45, 0.85, 0], [0.1, 0.15, 1.05]])
+    basis = [[0, 0, 0], [0.31, 0.17, 0.23], [0.62, 0.55, 0.4]][:nbasis]
+    g = P.SpinSystem(brav, basis, cells, per, 1.2)
+    o = O.OracleSystem(brav, basis, cells, per, 1.2)
+    mu = np.linspace(1.0, 2.5, nbasis)
+    g.hamiltonian_set_mu_s(mu); o.set_mu_s(mu)
+    g.hamiltonian_set_ddi(True, img); o.set_ddi(True, img)
+    g.hamiltonian_set_pairs([0], [1], [[0, 0, 0]], [0.8]); o.set_pairs([0], [1], [[0, 0, 0]], [0.8])
+    g.llg_configure(1.0, 0.3); o.llg_configure(1.0, 0.3)
+    rng = np.random.default_rng(9)
+    n = rng.standard_normal((g.N, 3)); n /= np.linalg.norm(n, axis=1, keepdims=True)
+    g.spins_set(n); o.set_spins(n)
+    assert g.spin_ddi_info().startswith("slab"), g.spin_ddi_info()
+    assert ("own-a" in g.spin_ddi_info()) == (cells[0] in (8, 16, 32))
+    assert_fields_close(g.effective_field(), o.effective_field())
+    assert abs(g.energy()[1][5] - o.energy_terms()[5]) <= 1e-12 * np.abs(o.energy_terms()).sum()
+    h = P.SpinSystem(brav, basis, cells, per, 1.2)
+    h.hamiltonian_set_mu_s(mu); h.hamiltonian_set_ddi(True, img); h.spin_set_option("ddi_slab", 0); h.spins_set(n)
+    assert h.spin_ddi_info() == "3d"
+    Fd = o.ddi_field(n, direct=True) / (mu[np.arange(g.N) % nbasis] * O.MU_B)[:, None]
+    assert np.abs(h.effective_field() - Fd).max() <= 1e-11 * np.abs(Fd).max()
+    site_mu = rng.uniform(0.5, 3.0, g.N)
+    g.hamiltonian_set_site_mu_s(site_mu); o.set_site_mu_s(site_mu)
+    assert_fields_close(g.effective_field(), o.effective_field())
+    g.llg_iterate(8); o.iterate(8)
+    assert np.abs(g.spins_get() - o.spins()).max() <= SPIN_ATOL
+
+
 def test_ddi_slab_systems_of_different_thickness_alive_together(P, O):
     """Two films of different thickness (4 and 8 planes, then 3 and 6) evaluated alternately in one process: the twiddle table of the
     transform along c is a function of the padded length alone, so neither system disturbs the other (round-1 advisor finding)."""
