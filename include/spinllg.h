@@ -217,8 +217,10 @@ int llg_slab_advance(spin_system *sys);
  *                    1 dependents released at entry, 2 at the end of each block
  *   store_A     (0)  1: the predictor stores the rotation field A(n) and the corrector reads it instead of recomputing it
  *   cache_noise (1)  the predictor keeps the thermal field of the step (24 B/spin) for the corrector instead of generating it twice
- *   ddi_slab    (1)  thin films (up to 8 planes; 4 with several basis atoms) take the dipolar slab path; 2: the same with cuFFT's transform along a instead of
- *                    the hand-written one; 0: the general 3-D transform
+ *   ddi_slab    (1)  thin films (up to 8 planes; 4 with several basis atoms) take the dipolar slab path: hand-written transforms along a and, for one
+ *                    basis atom and power-of-two columns, one fused kernel for the transforms along b and c and the contraction;
+ *                    3: cuFFT's transform along b and a separate contraction kernel; 2: cuFFT's transforms along a and b; 0: the general
+ *                    3-D transform
  *   ddi_mirror  (1)  the slab contraction reads PZ/2 + 1 tensor planes when the spectrum is mirror symmetric along c; 0: all PZ planes    */
 int spin_set_option(spin_system *sys, const char *name, int value);
 

@@ -1362,7 +1362,7 @@ extern "C" int spin_set_option(spin_system *s, const char *name, int value) {
     else if (!strcmp(name, "use_pdl")) { s->opt_pdl = value > 2 ? -1 : value < 0 ? -1 : value; s->plan_dirty = true; }
     else if (!strcmp(name, "use_march")) { s->opt_march = value < 0 ? 0 : (value > 2 ? 2 : value); s->plan_dirty = true; }
     else if (!strcmp(name, "ddi_mirror")) { s->opt_ddi_mirror = value ? 1 : 0; s->plan_dirty = true; }
-    else if (!strcmp(name, "ddi_slab")) { s->opt_ddi_slab = value < 0 ? 0 : (value > 2 ? 2 : value); s->plan_dirty = true; }      // 0: 3-D path, 1: slab path, 2: slab path with cuFFT's a-pass
+    else if (!strcmp(name, "ddi_slab")) { s->opt_ddi_slab = value < 0 ? 0 : (value > 3 ? 3 : value); s->plan_dirty = true; }      // 0: 3-D path, 1: slab path, 2: slab path with cuFFT's a-pass, 3: own a-pass, cuFFT b-pass + separate contraction
     else return spin::fail(SPIN_ERR_ARG, "unknown option '%s'", name);
     drop_graphs(s);
     return SPIN_OK;

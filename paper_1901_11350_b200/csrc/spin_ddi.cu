@@ -50,6 +50,12 @@ struct DdiState {
     int a_rows_per_block;      // rows (warps) per block of those kernels
     size_t a_smem;
     double2 *d_tw;             // exp(-2 pi i t / P0), t < P0
+    // fused b-pass (ddi_bfused_kernel): the a-pass kernels work in the transposed layout, s_a = [ka][slab][ib], s_d = the two partial
+    // results [r][ka][slab][ib]; the full spectra and cuFFT's b-pass are not used
+    bool fused_b;
+    double2 *d_tw_b;           // exp(-2 pi i t / P1), t < P1
+    double *d_Kb;              // [ka][r][6][planes][k'], ddi_bfused_tensor_kernel
+    size_t bf_smem;
     bool mirror;               // K(kz) = +-K(PZ - kz) (c perpendicular to the film): the contraction reads PZ/2 + 1 of the PZ planes
 };
 
@@ -199,59 +205,104 @@ template <int SIGN> __device__ __forceinline__ double2 ddi_rot45(const double2 a
 // (consecutive elements) are then both free of bank conflicts for 16-byte elements
 __device__ __forceinline__ int ddi_pad(const int i) { return i + (i >> 3); }
 
-// One warp, complex transform of length M (a power of two >= 8) as a Stockham autosort: passes of radix 8 (then one of radix 4 or 2),
-// ping-ponging between the padded rows a and b; returns the row that holds the result (natural order).  Twiddles exp(SIGN 2 pi i k r /
-// (Ns R)): the first power from the table tw[t] = exp(-2 pi i t / (2 M)), the others by multiplication (depth 3).
-template <int SIGN>      // -1 forward, +1 inverse (unnormalised)
-__device__ __forceinline__ double2 *ddi_warp_fft(double2 *a, double2 *b, const int M, const double2 *__restrict__ tw, const int lane) {
-    for (int Ns = 1; Ns < M;) {
-        const int rem = M / Ns;
-        const int R = (rem % 8 == 0) ? 8 : ((rem % 4 == 0) ? 4 : 2);
-        const int span = M / R, tstep = 2 * (M / (Ns * R));
-        for (int j = lane; j < span; j += 32) {
-            const int k = j & (Ns - 1), j0 = (j - k) * R + k;
-            double2 w1 = make_double2(1.0, 0.0);
-            if (k) { w1 = __ldg(tw + k * tstep); if (SIGN > 0) w1.y = -w1.y; }
-            if (R == 8) {
-                double2 v[8];
+// One butterfly of radix R (8, 4 or 2): v[r] times w1^r (twiddle = false: w1 = 1), then the R-point transform.  Result r of the transform
+// is left in v[ddi_perm<R>(r)]... read it through ddi_out<R>(r): the position in v that holds output r.
+template <int R> __host__ __device__ constexpr int ddi_out(int r) { return R == 8 ? ((r & 1) << 2 | (r & 2) | (r & 4) >> 2) : (R == 4 ? ((r & 1) << 1 | (r & 2) >> 1) : r); }
+template <int SIGN, int R>      // SIGN -1 forward, +1 inverse (unnormalised)
+__device__ __forceinline__ void ddi_butterfly(double2 (&v)[R], const bool twiddle, const double2 w1) {
+    if constexpr (R == 8) {
+        if (twiddle) {
+            const double2 w2 = ddi_cmul(w1, w1), w3 = ddi_cmul(w2, w1), w4 = ddi_cmul(w2, w2);
+            v[1] = ddi_cmul(v[1], w1); v[2] = ddi_cmul(v[2], w2); v[3] = ddi_cmul(v[3], w3); v[4] = ddi_cmul(v[4], w4);
+            v[5] = ddi_cmul(v[5], ddi_cmul(w4, w1)); v[6] = ddi_cmul(v[6], ddi_cmul(w3, w3)); v[7] = ddi_cmul(v[7], ddi_cmul(w4, w3));
+        }
+        // three radix-2 stages, result in bit-reversed order
+        double2 t;
+        t = ddi_csub(v[0], v[4]); v[0] = ddi_cadd(v[0], v[4]); v[4] = t;
+        t = ddi_csub(v[1], v[5]); v[1] = ddi_cadd(v[1], v[5]); v[5] = ddi_rot45<SIGN>(t);
+        t = ddi_csub(v[2], v[6]); v[2] = ddi_cadd(v[2], v[6]); v[6] = ddi_rot90<SIGN>(t);
+        t = ddi_csub(v[3], v[7]); v[3] = ddi_cadd(v[3], v[7]); v[7] = ddi_rot90<SIGN>(ddi_rot45<SIGN>(t));
 #pragma unroll
-                for (int r = 0; r < 8; ++r) v[r] = a[ddi_pad(j + r * span)];
-                if (k) {
-                    const double2 w2 = ddi_cmul(w1, w1), w3 = ddi_cmul(w2, w1), w4 = ddi_cmul(w2, w2);
-                    v[1] = ddi_cmul(v[1], w1); v[2] = ddi_cmul(v[2], w2); v[3] = ddi_cmul(v[3], w3); v[4] = ddi_cmul(v[4], w4);
-                    v[5] = ddi_cmul(v[5], ddi_cmul(w4, w1)); v[6] = ddi_cmul(v[6], ddi_cmul(w3, w3)); v[7] = ddi_cmul(v[7], ddi_cmul(w4, w3));
-                }
-                // 8-point transform: three radix-2 stages, result in bit-reversed order
-                double2 t;
-                t = ddi_csub(v[0], v[4]); v[0] = ddi_cadd(v[0], v[4]); v[4] = t;
-                t = ddi_csub(v[1], v[5]); v[1] = ddi_cadd(v[1], v[5]); v[5] = ddi_rot45<SIGN>(t);
-                t = ddi_csub(v[2], v[6]); v[2] = ddi_cadd(v[2], v[6]); v[6] = ddi_rot90<SIGN>(t);
-                t = ddi_csub(v[3], v[7]); v[3] = ddi_cadd(v[3], v[7]); v[7] = ddi_rot90<SIGN>(ddi_rot45<SIGN>(t));
+        for (int h = 0; h < 8; h += 4) {
+            t = ddi_csub(v[h], v[h + 2]); v[h] = ddi_cadd(v[h], v[h + 2]); v[h + 2] = t;
+            t = ddi_csub(v[h + 1], v[h + 3]); v[h + 1] = ddi_cadd(v[h + 1], v[h + 3]); v[h + 3] = ddi_rot90<SIGN>(t);
+        }
 #pragma unroll
-                for (int h = 0; h < 8; h += 4) {
-                    t = ddi_csub(v[h], v[h + 2]); v[h] = ddi_cadd(v[h], v[h + 2]); v[h + 2] = t;
-                    t = ddi_csub(v[h + 1], v[h + 3]); v[h + 1] = ddi_cadd(v[h + 1], v[h + 3]); v[h + 3] = ddi_rot90<SIGN>(t);
-                }
+        for (int h = 0; h < 8; h += 2) { t = ddi_csub(v[h], v[h + 1]); v[h] = ddi_cadd(v[h], v[h + 1]); v[h + 1] = t; }
+    } else if constexpr (R == 4) {
+        if (twiddle) { const double2 w2 = ddi_cmul(w1, w1); v[1] = ddi_cmul(v[1], w1); v[2] = ddi_cmul(v[2], w2); v[3] = ddi_cmul(v[3], ddi_cmul(w2, w1)); }
+        const double2 t0 = ddi_cadd(v[0], v[2]), t1 = ddi_csub(v[0], v[2]), t2 = ddi_cadd(v[1], v[3]), t3 = ddi_rot90<SIGN>(ddi_csub(v[1], v[3]));
+        v[0] = ddi_cadd(t0, t2); v[2] = ddi_cadd(t1, t3); v[1] = ddi_csub(t0, t2); v[3] = ddi_csub(t1, t3);      // bit-reversed: v[2] holds output 1
+    } else {
+        if (twiddle) v[1] = ddi_cmul(v[1], w1);
+        const double2 t = ddi_csub(v[0], v[1]);
+        v[0] = ddi_cadd(v[0], v[1]); v[1] = t;
+    }
+}
+
+// One Stockham pass of radix R of a transform of length M = 2^lgM by one warp: element i of the source is ld(i), element i of the
+// destination goes to st(i, v) (natural index; shared-memory rows, or global memory for the first / last pass of a fused kernel).
+// Ns = 2^lgNs = product of the radices of the passes before this one.  Twiddles exp(SIGN 2 pi i k r / (Ns R)): the first power from the
+// table tw[t] = exp(-2 pi i t / (2 M)), the others by multiplication (depth 3).  Index arithmetic is shifts and masks only.
+// INPLACE: source and destination are the same row -- every lane loads all its butterflies (at most NB, i.e. M <= 32 NB R; the fused kernel: M <= 256), the warp
+// synchronises, then the lanes store; otherwise butterfly by butterfly (NB is ignored).
+template <int SIGN, int R, class Store>
+__device__ __forceinline__ void ddi_fft_finish(double2 (&v)[R], const int j, const int lgNs, const int tshift, const double2 *__restrict__ tw, Store &&st) {
+    constexpr int lgR = R == 8 ? 3 : (R == 4 ? 2 : 1);
+    const int k = j & ((1 << lgNs) - 1), j0 = ((j - k) << lgR) + k;
+    double2 w1 = make_double2(1.0, 0.0);
+    if (k) { w1 = tw[k << tshift]; if (SIGN > 0) w1.y = -w1.y; }
+    ddi_butterfly<SIGN, R>(v, k != 0, w1);
 #pragma unroll
-                for (int h = 0; h < 8; h += 2) { t = ddi_csub(v[h], v[h + 1]); v[h] = ddi_cadd(v[h], v[h + 1]); v[h + 1] = t; }
-                b[ddi_pad(j0)] = v[0]; b[ddi_pad(j0 + 4 * Ns)] = v[1]; b[ddi_pad(j0 + 2 * Ns)] = v[2]; b[ddi_pad(j0 + 6 * Ns)] = v[3];
-                b[ddi_pad(j0 + Ns)] = v[4]; b[ddi_pad(j0 + 5 * Ns)] = v[5]; b[ddi_pad(j0 + 3 * Ns)] = v[6]; b[ddi_pad(j0 + 7 * Ns)] = v[7];
-            } else if (R == 4) {
-                double2 v0 = a[ddi_pad(j)], v1 = a[ddi_pad(j + span)], v2 = a[ddi_pad(j + 2 * span)], v3 = a[ddi_pad(j + 3 * span)];
-                if (k) { const double2 w2 = ddi_cmul(w1, w1); v1 = ddi_cmul(v1, w1); v2 = ddi_cmul(v2, w2); v3 = ddi_cmul(v3, ddi_cmul(w2, w1)); }
-                const double2 t0 = ddi_cadd(v0, v2), t1 = ddi_csub(v0, v2), t2 = ddi_cadd(v1, v3), t3 = ddi_rot90<SIGN>(ddi_csub(v1, v3));
-                b[ddi_pad(j0)] = ddi_cadd(t0, t2); b[ddi_pad(j0 + Ns)] = ddi_cadd(t1, t3);
-                b[ddi_pad(j0 + 2 * Ns)] = ddi_csub(t0, t2); b[ddi_pad(j0 + 3 * Ns)] = ddi_csub(t1, t3);
-            } else {
-                const double2 v0 = a[ddi_pad(j)];
-                double2 v1 = a[ddi_pad(j + span)];
-                if (k) v1 = ddi_cmul(v1, w1);
-                b[ddi_pad(j0)] = ddi_cadd(v0, v1); b[ddi_pad(j0 + Ns)] = ddi_csub(v0, v1);
-            }
+    for (int r = 0; r < R; ++r) st(j0 + (r << lgNs), v[ddi_out<R>(r)]);
+}
+template <int SIGN, int R, bool INPLACE, int NB, class Load, class Store>
+__device__ __forceinline__ void ddi_fft_pass(const int lgM, const int lgNs, const double2 *__restrict__ tw, const int lane, Load &&ld, Store &&st) {
+    constexpr int lgR = R == 8 ? 3 : (R == 4 ? 2 : 1);
+    const int span = 1 << (lgM - lgR), tshift = lgM - lgNs - lgR + 1;
+    if constexpr (INPLACE) {
+        double2 v[NB][R];
+#pragma unroll
+        for (int b = 0; b < NB; ++b) {
+            const int j = min(lane + 32 * b, span - 1);      // idle lanes load a valid element too (a guarded load costs ptxas 1.5 KB of spills)
+#pragma unroll
+            for (int r = 0; r < R; ++r) v[b][r] = ld(j + (r << (lgM - lgR)));
         }
         __syncwarp();
+#pragma unroll
+        for (int b = 0; b < NB; ++b) {
+            const int j = lane + 32 * b;
+            if (j < span) ddi_fft_finish<SIGN, R>(v[b], j, lgNs, tshift, tw, st);
+        }
+    } else {
+        for (int j = lane; j < span; j += 32) {
+            double2 v[R];
+#pragma unroll
+            for (int r = 0; r < R; ++r) v[r] = ld(j + (r << (lgM - lgR)));
+            ddi_fft_finish<SIGN, R>(v, j, lgNs, tshift, tw, st);
+        }
+    }
+}
+// radix of the pass that follows passes of product 2^lgNs: 8 while it divides what is left, then 4 or 2
+__host__ __device__ __forceinline__ int ddi_radix(const int lgM, const int lgNs) { const int rem = lgM - lgNs; return rem >= 3 ? 8 : (rem == 2 ? 4 : 2); }
+// the pass after passes of product 2^lgNs, whatever its radix; returns log2 of that radix
+template <int SIGN, bool INPLACE, class Load, class Store>
+__device__ __forceinline__ int ddi_fft_next_pass(const int lgM, const int lgNs, const double2 *__restrict__ tw, const int lane, Load &&ld, Store &&st) {
+    const int R = ddi_radix(lgM, lgNs);
+    if (R == 8) { ddi_fft_pass<SIGN, 8, INPLACE, 1>(lgM, lgNs, tw, lane, ld, st); return 3; }      // in place: M <= 256 = 32 lanes x 8 elements
+    if (R == 4) { ddi_fft_pass<SIGN, 4, INPLACE, 2>(lgM, lgNs, tw, lane, ld, st); return 2; }
+    ddi_fft_pass<SIGN, 2, INPLACE, 4>(lgM, lgNs, tw, lane, ld, st);
+    return 1;
+}
+
+// One warp, complex transform of length M = 2^lgM >= 8 as a Stockham autosort, ping-ponging between the padded shared-memory rows
+// a and b; returns the row that holds the result (natural order).
+template <int SIGN>
+__device__ __forceinline__ double2 *ddi_warp_fft(double2 *a, double2 *b, const int lgM, const double2 *__restrict__ tw, const int lane) {
+    for (int lgNs = 0; lgNs < lgM;) {
+        lgNs += ddi_fft_next_pass<SIGN, false>(lgM, lgNs, tw, lane, [&](int i) { return a[ddi_pad(i)]; }, [&](int i, const double2 v) { b[ddi_pad(i)] = v; });
+        __syncwarp();
         double2 *t = a; a = b; b = t;
-        Ns *= R;
     }
     return a;
 }
@@ -263,54 +314,95 @@ __device__ __forceinline__ double2 ddi_row_ratio(const DevicePlan &L, int b, int
     return make_double2(__ldg(L.mu_ratio + b + (size_t)L.nb * cell0), __ldg(L.mu_ratio + b + (size_t)L.nb * (cell0 + 1)));
 }
 
-// rows = Nb * SL occupied rows, row = ib SL + slab, slab = (b 3 + comp) Nc + ic; out: element k of the row at row * S1p + k, k = 0 .. M
+// rows = Nb * SL occupied rows, slab = (b 3 + comp) Nc + ic.
+// TR = false: row = ib SL + slab, element k of the row at row * S1p + k, k = 0 .. M (the layout cuFFT's b-pass works on).
+// TR = true (fused b-pass): a block takes rows_per_block consecutive ib of ONE slab and writes [ka][slab][ib] -- its warps' results go
+// through shared memory so that consecutive lanes write consecutive ib (whole 32-byte sectors and more).  `nbr` = Nb.
+template <bool TR>
 __global__ void __launch_bounds__(256) ddi_apass_fwd_kernel(const __grid_constant__ DevicePlan L, const double *__restrict__ n, int M, int SL, int S1p, int rows,
                                                             int rows_per_block, const double *__restrict__ mu_b, const double2 *__restrict__ tw,
                                                             cufftDoubleComplex *__restrict__ out) {
     extern __shared__ double2 ddi_sm[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int row = blockIdx.x * rows_per_block + warp;
-    if (warp >= rows_per_block || row >= rows) return;
-    const int ib = row / SL, slab = row - ib * SL, bc = slab / L.Nc, ic = slab - bc * L.Nc, sb = bc / 3, comp = bc - 3 * sb;
+    if (!TR && (warp >= rows_per_block || row >= rows)) return;      // (TR: rows is a multiple of rows_per_block, every warp has a row)
+    const int ib = TR ? row % L.Nb : row / SL, slab = TR ? row / L.Nb : row - ib * SL;
+    const int bc = slab / L.Nc, ic = slab - bc * L.Nc, sb = bc / 3, comp = bc - 3 * sb;
     const double mu = mu_b[sb];
     const double2 *src = (const double2 *)(n + (size_t)sb * L.sub + ((size_t)(ic + L.LC) * L.PB + (ib + L.LB)) * (3 * L.PA) + comp * L.PA + L.LA);
-    const int MP = M + (M >> 3);                        // padded row
-    double2 *a = ddi_sm + (size_t)warp * 2 * MP, *b = a + MP;
-    for (int j = lane; j < M; j += 32) {
-        double2 v = make_double2(0.0, 0.0);
-        if (j < M / 2) {
-            v = __ldg(src + j);
-            double m0 = mu, m1 = mu;
-            if (L.mu_ratio) { const double2 r = ddi_row_ratio(L, sb, ib, ic, j); m0 *= r.x; m1 *= r.y; }
-            v.x *= m0; v.y *= m1;
-        }
+    const int MP = M + (M >> 3), WS = 2 * MP + 1;       // padded row; buffers of a warp (the odd stride keeps the transposed reads conflict-free)
+    double2 *a = ddi_sm + (size_t)warp * WS, *b = a + MP;
+    for (int j = M / 2 + lane; j < M; j += 32) a[ddi_pad(j)] = make_double2(0.0, 0.0);      // the zero padding of the row
+#pragma unroll 4
+    for (int j = lane; j < M / 2; j += 32) {                                                  // (unrolled: the loads of a lane are in flight together)
+        double2 v = __ldg(src + j);
+        double m0 = mu, m1 = mu;
+        if (L.mu_ratio) { const double2 r = ddi_row_ratio(L, sb, ib, ic, j); m0 *= r.x; m1 *= r.y; }
+        v.x *= m0; v.y *= m1;
         a[ddi_pad(j)] = v;
     }
     __syncwarp();
-    const double2 *Z = ddi_warp_fft<-1>(a, b, M, tw, lane);
+    const double2 *Z = ddi_warp_fft<-1>(a, b, 31 - __clz(M), tw, lane);
+    double2 *X = (Z == a) ? b : a;                       // TR: the half spectrum of the row, unpadded, in the warp's other buffer
     cufftDoubleComplex *dst = out + (size_t)row * S1p;
     for (int k = lane; k <= M; k += 32) {
         const double2 zk = Z[ddi_pad(k & (M - 1))], zm = Z[ddi_pad((M - k) & (M - 1))];
         const double er = 0.5 * (zk.x + zm.x), ei = 0.5 * (zk.y - zm.y);            // E = (Z(k) + conj Z(M-k)) / 2
         const double orr = 0.5 * (zk.y + zm.y), oi = -0.5 * (zk.x - zm.x);          // O = (Z(k) - conj Z(M-k)) / (2i)
         const double2 w = __ldg(tw + k);                                            // exp(-2 pi i k / P0)
-        dst[k] = make_cuDoubleComplex(er + fma(orr, w.x, -oi * w.y), ei + fma(orr, w.y, oi * w.x));
+        const double2 x = make_double2(er + fma(orr, w.x, -oi * w.y), ei + fma(orr, w.y, oi * w.x));
+        if (TR) X[k] = x; else dst[k] = x;
+    }
+    if (TR) {
+        __syncthreads();
+        const int xoff = (int)(X - a);                   // the same for every warp (same number of passes)
+        const int ib0 = (blockIdx.x * rows_per_block) % L.Nb;
+        const int lgr = __ffs(rows_per_block) - 1;       // (a power of two)
+        cufftDoubleComplex *o = out + (size_t)slab * L.Nb + ib0;
+        for (int idx = threadIdx.x; idx < (M + 1) << lgr; idx += blockDim.x) {
+            const int k = idx >> lgr, w = idx & (rows_per_block - 1);
+            o[(size_t)k * SL * L.Nb + w] = ddi_sm[w * WS + xoff + k];
+        }
     }
 }
 
-// inverse: from the half spectrum X(k), k = 0 .. M, of every occupied row to P0 x(ia), ia < Na, scaled and written as the dipolar force
+// inverse: from the half spectrum X(k), k = 0 .. M, of every occupied row to P0 x(ia), ia < Na, scaled and written as the dipolar force.
+// TR = true: the input is the two partial results of ddi_bfused_kernel, [r][ka][slab][ib] (in + part1 apart), added while loading.
+template <bool TR>
 __global__ void __launch_bounds__(256) ddi_apass_inv_kernel(const __grid_constant__ DevicePlan L, const cufftDoubleComplex *__restrict__ in, int M, int SL, int S1p,
                                                             int rows, int rows_per_block, const double *__restrict__ mu_b, double scale0, const double2 *__restrict__ tw,
-                                                            double *__restrict__ f) {
+                                                            double *__restrict__ f, size_t part1) {
     extern __shared__ double2 ddi_sm[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int row = blockIdx.x * rows_per_block + warp;
-    if (warp >= rows_per_block || row >= rows) return;
-    const int ib = row / SL, slab = row - ib * SL, bc = slab / L.Nc, ic = slab - bc * L.Nc, sb = bc / 3, comp = bc - 3 * sb;
+    if (!TR && (warp >= rows_per_block || row >= rows)) return;
+    const int ib = TR ? row % L.Nb : row / SL, slab = TR ? row / L.Nb : row - ib * SL;
+    const int bc = slab / L.Nc, ic = slab - bc * L.Nc, sb = bc / 3, comp = bc - 3 * sb;
     const double scale = mu_b[sb] * scale0;
-    const cufftDoubleComplex *src = in + (size_t)row * S1p;
-    const int MP = M + (M >> 3);
-    double2 *a = ddi_sm + (size_t)warp * 2 * MP, *b = a + MP;
+    const int MP = M + (M >> 3), WS = 2 * MP + 1;
+    double2 *a = ddi_sm + (size_t)warp * WS, *b = a + MP;
+    const cufftDoubleComplex *src = TR ? b : in + (size_t)row * S1p;                // TR: the row's half spectrum, gathered into b first
+    if (TR) {
+        const int ib0 = (blockIdx.x * rows_per_block) % L.Nb;
+        const int lgr = __ffs(rows_per_block) - 1, total = (M + 1) << lgr;      // (a power of two)
+        const cufftDoubleComplex *g0 = in + (size_t)slab * L.Nb + ib0, *g1 = g0 + part1;
+        constexpr int U = 4;                                 // loads of U elements in flight per thread
+        for (int base = threadIdx.x; base < total; base += U * blockDim.x) {
+            double2 p0[U], p1[U];
+#pragma unroll
+            for (int u = 0; u < U; ++u) {
+                const int idx = min(base + u * (int)blockDim.x, total - 1);
+                const size_t o = (size_t)(idx >> lgr) * SL * L.Nb + (idx & (rows_per_block - 1));
+                p0[u] = __ldg(g0 + o); p1[u] = __ldg(g1 + o);
+            }
+#pragma unroll
+            for (int u = 0; u < U; ++u) {
+                const int idx = base + u * (int)blockDim.x;
+                if (idx < total) ddi_sm[(idx & (rows_per_block - 1)) * WS + MP + (idx >> lgr)] = make_double2(p0[u].x + p1[u].x, p0[u].y + p1[u].y);
+            }
+        }
+        __syncthreads();
+    }
     for (int k = lane; k < M; k += 32) {
         const cufftDoubleComplex xk = src[k], xm = src[M - k];
         const double er = xk.x + xm.x, ei = xk.y - xm.y;                            // E = X(k) + conj X(M-k)
@@ -320,7 +412,7 @@ __global__ void __launch_bounds__(256) ddi_apass_inv_kernel(const __grid_constan
         a[ddi_pad(k)] = make_double2(er - oi, ei + orr);                            // Z = E + i O
     }
     __syncwarp();
-    const double2 *z = ddi_warp_fft<+1>(a, b, M, tw, lane);
+    const double2 *z = ddi_warp_fft<+1>(a, b, 31 - __clz(M), tw, lane);
     double2 *dst = (double2 *)(f + (size_t)sb * L.sub + ((size_t)(ic + L.LC) * L.PB + (ib + L.LB)) * (3 * L.PA) + comp * L.PA + L.LA);
     for (int j = lane; j < M / 2; j += 32) {
         const double2 v = z[ddi_pad(j)];
@@ -351,6 +443,33 @@ __global__ void real_part_kernel(const cufftDoubleComplex *__restrict__ in, doub
 __constant__ double DDI_TWR[17][16], DDI_TWI[17][16];
 
 __host__ __device__ constexpr bool ddi_pow2(int n) { return n > 0 && (n & (n - 1)) == 0; }
+// (re + i im) times exp(-2 pi i a / 16).  Called with `a` known after unrolling, so the switch folds away: quarter turns cost nothing,
+// eighth turns two additions and two products, the others a full complex product with literal constants.  The power-of-two lengths along c
+// (PZ = 2, 4, 8, 16) take their twiddles from here instead of the table: of the 12 butterflies of a length-8 transform only 2 multiply.
+__device__ __forceinline__ void ddi_rot16(const int a, double &re, double &im) {
+    const double h = 0.70710678118654752440, c = 0.92387953251128675613, s = 0.38268343236508977173;      // cos pi/4, cos pi/8, sin pi/8
+    const double r = re, i = im;
+    double cw = 0.0, sw = 0.0;
+    switch (a & 15) {
+        case 0: return;
+        case 4: re = i; im = -r; return;
+        case 8: re = -r; im = -i; return;
+        case 12: re = -i; im = r; return;
+        case 2: re = h * (r + i); im = h * (i - r); return;
+        case 6: re = h * (i - r); im = -h * (r + i); return;
+        case 10: re = -h * (r + i); im = h * (r - i); return;
+        case 14: re = h * (r - i); im = h * (r + i); return;
+        case 1: cw = c; sw = s; break;
+        case 3: cw = s; sw = c; break;
+        case 5: cw = -s; sw = c; break;
+        case 7: cw = -c; sw = s; break;
+        case 9: cw = -c; sw = -s; break;
+        case 11: cw = -s; sw = -c; break;
+        case 13: cw = s; sw = -c; break;
+        default: cw = c; sw = -s; break;
+    }
+    re = fma(r, cw, i * sw); im = fma(i, cw, -r * sw);
+}
 __host__ __device__ constexpr int ddi_bitrev(int p, int n) {      // n a power of two
     int r = 0;
     for (int b = 1, c = n >> 1; b < n; b <<= 1, c >>= 1) if (p & b) r |= c;
@@ -374,8 +493,8 @@ __device__ __forceinline__ void ddi_dft_fwd(double (&re)[N], double (&im)[N]) {
                     const int t = j * (N / (2 * half)) * 2;      // W_(2 half)^j as a power of W_PZ
                     const double ar = re[base + j], ai = im[base + j], br = re[base + j + half], bi = im[base + j + half];
                     re[base + j] = ar + br; im[base + j] = ai + bi;
-                    const double dr = ar - br, di = ai - bi, wr = DDI_TWR[PZ][t], wi = DDI_TWI[PZ][t];
-                    re[base + j + half] = fma(dr, wr, -di * wi); im[base + j + half] = fma(dr, wi, di * wr);
+                    re[base + j + half] = ar - br; im[base + j + half] = ai - bi;
+                    ddi_rot16(t * (16 / PZ), re[base + j + half], im[base + j + half]);
                 }
     } else {
         double yr[N], yi[N];
@@ -406,8 +525,8 @@ __device__ __forceinline__ void ddi_dft_inv(double (&re)[N], double (&im)[N]) {
 #pragma unroll
                 for (int j = 0; j < half; ++j) {
                     const int t = j * (N / (2 * half)) * 2;
-                    const double wr = DDI_TWR[PZ][t], wi = -DDI_TWI[PZ][t];      // conjugate twiddle
-                    const double br = fma(re[base + j + half], wr, -im[base + j + half] * wi), bi = fma(re[base + j + half], wi, im[base + j + half] * wr);
+                    double br = re[base + j + half], bi = im[base + j + half];
+                    ddi_rot16(16 - t * (16 / PZ), br, bi);                         // conjugate twiddle
                     const double ar = re[base + j], ai = im[base + j];
                     re[base + j] = ar + br; im[base + j] = ai + bi;
                     re[base + j + half] = ar - br; im[base + j + half] = ai - bi;
@@ -443,6 +562,69 @@ __device__ __forceinline__ void ddi_dft_inv(double (&re)[N], double (&im)[N]) {
 // PAD = false: a single plane that is not padded along c (NZ = PZ = 1): no transform at all, thread e = 1 idles.
 // M2 / H2: element (kb, slab = c NZ + z, ka) at (kb SL + slab) S1p + ka, S1p the row pitch (H2 may be M2: every column is read, then
 // written, by its own pair of threads); Kre: [6][PZ][S2] with q = kb S1 + ka.
+// The work of thread e on its column x (3 components x NZ planes, complex): twist, forward transform, contraction at its NZ wave numbers
+// with the tensor planes that kload(plane, k[6]) delivers (xx, xy, xz, yy, yz, zz), inverse transform, twist back.  In place.
+template <int NZ, bool PAD, bool MIRROR, class KLoad>
+__device__ __forceinline__ void ddi_column_half(double (&xr)[3][NZ], double (&xi)[3][NZ], const int e, KLoad &&kload) {
+    constexpr int PZ = PAD ? 2 * NZ : NZ;
+    if constexpr (PAD) {
+        if (e) {
+#pragma unroll
+            for (int c = 0; c < 3; ++c)
+#pragma unroll
+                for (int z = 1; z < NZ; ++z) {
+                    if constexpr (ddi_pow2(NZ)) ddi_rot16(z * (16 / PZ), xr[c][z], xi[c][z]);
+                    else {
+                        const double wr = DDI_TWR[PZ][z], wi = DDI_TWI[PZ][z], r = xr[c][z], i = xi[c][z];
+                        xr[c][z] = fma(r, wr, -i * wi); xi[c][z] = fma(r, wi, i * wr);
+                    }
+                }
+        }
+#pragma unroll
+        for (int c = 0; c < 3; ++c) ddi_dft_fwd<NZ>(xr[c], xi[c]);
+    }
+    // contraction at the wave numbers of this thread; position p of the transformed column holds kz = 2 ddi_pos(p) + e
+    auto contract = [&](const int p, const double kxx, const double kxy, const double kxz, const double kyy, const double kyz, const double kzz) {
+        const double r0 = xr[0][p], r1 = xr[1][p], r2 = xr[2][p], i0 = xi[0][p], i1 = xi[1][p], i2 = xi[2][p];
+        xr[0][p] = kxx * r0 + kxy * r1 + kxz * r2; xr[1][p] = kxy * r0 + kyy * r1 + kyz * r2; xr[2][p] = kxz * r0 + kyz * r1 + kzz * r2;
+        xi[0][p] = kxx * i0 + kxy * i1 + kxz * i2; xi[1][p] = kxy * i0 + kyy * i1 + kyz * i2; xi[2][p] = kxz * i0 + kyz * i1 + kzz * i2;
+    };
+    auto planes = [&](auto ec) {
+        constexpr int E = decltype(ec)::value;
+        // planes this thread reads: kz = 2 j + E, j < NJ (MIRROR: up to PZ / 2 only, the rest are mirror images); the tensor of plane
+        // j + 1 is loaded before plane j is contracted
+        constexpr int NJ = !PAD ? 1 : (MIRROR ? (PZ / 2 - E) / 2 + 1 : NZ);
+        double k[2][6];
+        kload(PAD ? E : 0, k[0]);
+#pragma unroll
+        for (int j = 0; j < NJ; ++j) {
+            const int kz = PAD ? 2 * j + E : 0;
+            if (j + 1 < NJ) kload(kz + 2, k[(j + 1) & 1]);
+            const double(&kk)[6] = k[j & 1];
+            contract(ddi_pos<NZ>(j), kk[0], kk[1], kk[2], kk[3], kk[4], kk[5]);
+            if (MIRROR && kz > 0 && 2 * kz < PZ)                        // plane PZ - kz: the same values, xz and yz with the opposite sign
+                contract(ddi_pos<NZ>((PZ - kz - E) / 2), kk[0], kk[1], -kk[2], kk[3], -kk[4], kk[5]);
+        }
+    };
+    if (e) planes(spin_ddi_int<1>{}); else planes(spin_ddi_int<0>{});
+    if constexpr (PAD) {
+#pragma unroll
+        for (int c = 0; c < 3; ++c) ddi_dft_inv<NZ>(xr[c], xi[c]);
+        if (e) {
+#pragma unroll
+            for (int c = 0; c < 3; ++c)
+#pragma unroll
+                for (int z = 1; z < NZ; ++z) {
+                    if constexpr (ddi_pow2(NZ)) ddi_rot16(16 - z * (16 / PZ), xr[c][z], xi[c][z]);
+                    else {
+                        const double wr = DDI_TWR[PZ][z], wi = -DDI_TWI[PZ][z], r = xr[c][z], i = xi[c][z];
+                        xr[c][z] = fma(r, wr, -i * wi); xi[c][z] = fma(r, wi, i * wr);
+                    }
+                }
+        }
+    }
+}
+
 constexpr int DDI_CT_COLS = 64;      // columns per block: 2 x 64 threads
 template <int NZ, bool PAD, bool MIRROR>
 __global__ void __launch_bounds__(2 * DDI_CT_COLS, 4) ddi_slab_contract_kernel(const double *__restrict__ Kre, const cufftDoubleComplex *__restrict__ M2,
@@ -475,52 +657,18 @@ __global__ void __launch_bounds__(2 * DDI_CT_COLS, 4) ddi_slab_contract_kernel(c
                 const cufftDoubleComplex v = M2[col + (size_t)(c * NZ + z) * S1p];
                 xr[c][z] = v.x; xi[c][z] = v.y;
             }
-        if constexpr (PAD) {
-            if (e) {
-#pragma unroll
-                for (int c = 0; c < 3; ++c)
-#pragma unroll
-                    for (int z = 1; z < NZ; ++z) {
-                        const double wr = DDI_TWR[PZ][z], wi = DDI_TWI[PZ][z], r = xr[c][z], i = xi[c][z];
-                        xr[c][z] = fma(r, wr, -i * wi); xi[c][z] = fma(r, wi, i * wr);
-                    }
-            }
-#pragma unroll
-            for (int c = 0; c < 3; ++c) ddi_dft_fwd<NZ>(xr[c], xi[c]);
-        }
-        // contraction at the wave numbers of this thread; position p of the transformed column holds kz = 2 ddi_pos(p) + e
         const size_t st = (size_t)PZ * S2;
-        auto contract = [&](const int p, const double kxx, const double kxy, const double kxz, const double kyy, const double kyz, const double kzz) {
-            const double r0 = xr[0][p], r1 = xr[1][p], r2 = xr[2][p], i0 = xi[0][p], i1 = xi[1][p], i2 = xi[2][p];
-            xr[0][p] = kxx * r0 + kxy * r1 + kxz * r2; xr[1][p] = kxy * r0 + kyy * r1 + kyz * r2; xr[2][p] = kxz * r0 + kyz * r1 + kzz * r2;
-            xi[0][p] = kxx * i0 + kxy * i1 + kxz * i2; xi[1][p] = kxy * i0 + kyy * i1 + kyz * i2; xi[2][p] = kxz * i0 + kyz * i1 + kzz * i2;
-        };
-        auto planes = [&](auto ec) {
-            constexpr int E = decltype(ec)::value;
+        ddi_column_half<NZ, PAD, MIRROR>(xr, xi, e, [&](const int kz, double (&k)[6]) {
+            const size_t o = (size_t)kz * S2 + q;
 #pragma unroll
-            for (int j = 0; j < NZ; ++j) {
-                const int kz = PAD ? 2 * j + E : 0;
-                if (MIRROR && 2 * kz > PZ) continue;                      // taken together with its mirror image below
-                const size_t o = (size_t)kz * S2 + q;
-                const double kxx = Kre[o], kxy = Kre[st + o], kxz = Kre[2 * st + o], kyy = Kre[3 * st + o], kyz = Kre[4 * st + o], kzz = Kre[5 * st + o];
-                contract(ddi_pos<NZ>(j), kxx, kxy, kxz, kyy, kyz, kzz);
-                if (MIRROR && kz > 0 && 2 * kz < PZ)                        // plane PZ - kz: the same values, xz and yz with the opposite sign
-                    contract(ddi_pos<NZ>((PZ - kz - E) / 2), kxx, kxy, -kxz, kyy, -kyz, kzz);
-            }
-        };
-        if (e) planes(spin_ddi_int<1>{}); else planes(spin_ddi_int<0>{});
+            for (int m = 0; m < 6; ++m) k[m] = Kre[m * st + o];
+        });
         if constexpr (PAD) {
-#pragma unroll
-            for (int c = 0; c < 3; ++c) ddi_dft_inv<NZ>(xr[c], xi[c]);
             if (e) {
 #pragma unroll
                 for (int c = 0; c < 3; ++c)
 #pragma unroll
-                    for (int z = 0; z < NZ; ++z) {
-                        double r = xr[c][z], i = xi[c][z];
-                        if (z > 0) { const double wr = DDI_TWR[PZ][z], wi = -DDI_TWI[PZ][z]; const double t = fma(r, wr, -i * wi); i = fma(r, wi, i * wr); r = t; }
-                        half1[c * NZ + z][lane_col] = make_double2(r, i);
-                    }
+                    for (int z = 0; z < NZ; ++z) half1[c * NZ + z][lane_col] = make_double2(xr[c][z], xi[c][z]);
             }
         }
     }
@@ -535,6 +683,139 @@ __global__ void __launch_bounds__(2 * DDI_CT_COLS, 4) ddi_slab_contract_kernel(c
                 H2[col + (size_t)(c * NZ + z) * S1p] = make_cuDoubleComplex(r, i);
             }
     }
+}
+
+// ---------------------------------------------------------------------------------------------------------------------------
+// Fused b-pass (round 2; one basis atom, rows and columns of power-of-two length): forward transform along b, transform along c,
+// tensor contraction, inverse transform along c and inverse transform along b in ONE kernel, so that the full spectra (2 x 50 MB per
+// pass on cfg5) never exist in HBM.  The column of length P1 = 2 Nb has Nb occupied rows followed by Nb zeros, and only Nb rows of the
+// result are needed, so the wave numbers kb split by parity r:
+//     X(2 k' + r) = sum_{ib < Nb} [x(ib) W^(r ib)] W_Nb^(k' ib),        y(ib) = sum_r W^(-r ib) sum_k' Y(2 k' + r) W_Nb^(-k' ib),   W = exp(-2 pi i / P1):
+// two independent transforms of length Nb.  A block takes one ka and one parity r: it reads its 3 NZ columns of Nb rows (contiguous in the
+// [ka][slab][ib] layout the a-pass kernels write in this mode), transforms them (one warp per column, Stockham passes in place; the first pass
+// reads global memory and applies the twist), contracts every wave
+// vector (ka, kb = 2 k' + r) along c exactly like ddi_slab_contract_kernel (two threads per column, tensor from a copy laid out
+// [ka][r][component][plane][k'] when the plan is built), transforms back and writes its partial result; the inverse a-pass adds the two
+// parities.  (One block per ka taking the two parities in turn and adding them itself was measured slower: 76 instead of 66 us.)  Shared memory: 3 NZ padded columns of Nb complex numbers (cfg5: 24 columns x 4.6 KB = 110.6 KB, two blocks of 256 threads per SM,
+// so that one block's loads overlap the other's arithmetic).
+constexpr int DDI_BF_THREADS = 256, DDI_BF_WARPS = DDI_BF_THREADS / 32;
+template <int NZ, bool MIRROR>
+__global__ void __launch_bounds__(DDI_BF_THREADS, 2) ddi_bfused_kernel(const double *__restrict__ Kb, const double2 *__restrict__ Tin, double2 *__restrict__ Tout,
+                                                                        const int lgM, const int S1, const double2 *__restrict__ tw) {
+    constexpr int SL = 3 * NZ, NPL = MIRROR ? NZ + 1 : 2 * NZ;
+    extern __shared__ double2 ddi_sm[];
+    const int M = 1 << lgM, LP = M + (M >> 3);
+    const int ka = blockIdx.x >> 1, r = blockIdx.x & 1;
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const double *Kme = Kb + (((size_t)ka * 2 + r) * 6 * NPL << lgM);
+    // ask L2 for this block's tensor planes while the columns are transformed
+    for (size_t i = (size_t)tid * 16; i < ((size_t)6 * NPL << lgM); i += (size_t)DDI_BF_THREADS * 16) asm volatile("prefetch.global.L2 [%0];" ::"l"(Kme + i));
+    // the first M entries of the twiddle table, in shared memory behind the columns (all a pass or the twist ever reads)
+    double2 *tws = ddi_sm + (size_t)SL * LP;
+    for (int i = tid; i < M; i += DDI_BF_THREADS) tws[i] = __ldg(tw + i);
+    // ---- forward: one warp per column, in place in the column's shared-memory row (every lane holds its M / 32 elements between the
+    // loads and the stores of a pass).  The first pass (always radix 8) reads global memory and applies the twist of the odd wave
+    // numbers; the loads of the warp's next column are in flight while it transforms the current one.
+    {
+        constexpr int NIT = (SL + DDI_BF_WARPS - 1) / DDI_BF_WARPS;
+        const int span = M >> 3, j = min(lane, span - 1);
+        double2 buf[2][8];
+        auto fetch = [&](const int slab, double2 (&v)[8]) {
+            const double2 *src = Tin + (((size_t)ka * SL + slab) << lgM) + j;
+#pragma unroll
+            for (int q = 0; q < 8; ++q) v[q] = __ldg(src + q * span);
+        };
+        if (warp < SL) fetch(warp, buf[0]);
+        __syncthreads();                                                       // tws is complete
+#pragma unroll
+        for (int it = 0; it < NIT; ++it) {
+            const int slab = warp + it * DDI_BF_WARPS;
+            if (it + 1 < NIT && slab + DDI_BF_WARPS < SL) fetch(slab + DDI_BF_WARPS, buf[(it + 1) & 1]);
+            if (slab < SL) {
+                double2(&v)[8] = buf[it & 1];
+                double2 *row = ddi_sm + (size_t)slab * LP;
+                auto st = [&](int i, const double2 x) { row[ddi_pad(i)] = x; };
+                if (r) {
+#pragma unroll
+                    for (int q = 0; q < 8; ++q) v[q] = ddi_cmul(v[q], tws[j + q * span]);
+                }
+                if (lane < span) ddi_fft_finish<-1, 8>(v, lane, 0, lgM - 2, tws, st);
+                for (int lgNs = 3; lgNs < lgM;) {
+                    __syncwarp();
+                    lgNs += ddi_fft_next_pass<-1, true>(lgM, lgNs, tws, lane, [&](int i) { return row[ddi_pad(i)]; }, st);
+                }
+            }
+        }
+    }
+    __syncthreads();
+    // ---- contraction along c: thread (k', e) of a round takes the wave numbers kz = 2 j + e of the wave vector (ka, kb = 2 k' + r)
+    constexpr int half = DDI_BF_THREADS / 2;
+    const int e = tid / half;
+    for (int k0 = 0; k0 < M; k0 += half) {
+        const int kp = k0 + (tid - e * half);
+        const bool live = kp < M;
+        double2 *col = ddi_sm + ddi_pad(kp);
+        double xr[3][NZ], xi[3][NZ];
+        if (live) {
+#pragma unroll
+            for (int c = 0; c < 3; ++c)
+#pragma unroll
+                for (int z = 0; z < NZ; ++z) { const double2 v = col[(size_t)(c * NZ + z) * LP]; xr[c][z] = v.x; xi[c][z] = v.y; }
+            ddi_column_half<NZ, true, MIRROR>(xr, xi, e, [&](const int kz, double (&k)[6]) {
+#pragma unroll
+                for (int m = 0; m < 6; ++m) k[m] = __ldg(Kme + ((size_t)(m * NPL + kz) << lgM) + kp);
+            });
+        }
+        __syncthreads();                                                      // both halves have read the column
+        if (live && e) {
+#pragma unroll
+            for (int c = 0; c < 3; ++c)
+#pragma unroll
+                for (int z = 0; z < NZ; ++z) col[(size_t)(c * NZ + z) * LP] = make_double2(xr[c][z], xi[c][z]);
+        }
+        __syncthreads();
+        if (live && !e) {
+#pragma unroll
+            for (int c = 0; c < 3; ++c)
+#pragma unroll
+                for (int z = 0; z < NZ; ++z) {
+                    double2 *q = col + (size_t)(c * NZ + z) * LP;
+                    const double2 h = *q;
+                    *q = make_double2(xr[c][z] + h.x, xi[c][z] + h.y);
+                }
+        }
+    }
+    __syncthreads();
+    // ---- inverse: one warp per column, the last pass writes the partial result of this parity (twisted back) to global memory
+    for (int slab = warp; slab < SL; slab += DDI_BF_WARPS) {
+        double2 *dstg = Tout + ((((size_t)r * S1 + ka) * SL + slab) << lgM);
+        double2 *row = ddi_sm + (size_t)slab * LP;
+        auto ld = [&](int i) { return row[ddi_pad(i)]; };
+        int lgNs = 0;
+        while (lgM - lgNs > 3) {
+            lgNs += ddi_fft_next_pass<+1, true>(lgM, lgNs, tws, lane, ld, [&](int i, const double2 v) { row[ddi_pad(i)] = v; });
+            __syncwarp();
+        }
+        ddi_fft_next_pass<+1, false>(lgM, lgNs, tws, lane, ld, [&](int i, double2 v) {
+            if (r) { double2 w = tws[i]; w.y = -w.y; v = ddi_cmul(v, w); }
+            dstg[i] = v;
+        });
+    }
+}
+
+// the tensor in the order ddi_bfused_kernel reads it: Kb[ka][r][component][plane][k'] = Kre[component][plane][kb = 2 k' + r][ka]
+__global__ void ddi_bfused_tensor_kernel(const double *__restrict__ Kre, double *__restrict__ Kb, int PZ, int NPL, int M, int S1) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long long total = (long long)S1 * 2 * 6 * NPL * M;
+    if (i >= total) return;
+    const int kp = (int)(i % M);
+    long long t = i / M;
+    const int m = (int)(t % NPL); t /= NPL;
+    const int comp = (int)(t % 6); t /= 6;
+    const int r = (int)(t % 2);
+    const int ka = (int)(t / 2);
+    const long long S2 = (long long)(2 * M) * S1;
+    Kb[i] = Kre[((long long)comp * PZ + m) * S2 + (long long)(2 * kp + r) * S1 + ka];
 }
 
 // The same for several basis atoms ("one FFT per sublattice + inter-sublattice convolutions"): H_a^(kz) = sum_b K_ab^(kz) . M_b^(kz)
@@ -668,6 +949,7 @@ const char *spin::ddi_path_name(const spin_system *s) {
     const DdiState *d = s->ddi;
     if (!s->ddi_on || !d) return "off";
     if (!d->slab) return "3d";
+    if (d->fused_b) return d->mirror ? "slab+mirror+own-a+fused-b" : "slab+own-a+fused-b";
     if (d->own_a) return d->mirror ? "slab+mirror+own-a" : "slab+own-a";
     return d->mirror ? "slab+mirror" : "slab";
 }
@@ -676,9 +958,13 @@ void spin::ddi_release(spin_system *s) {
     DdiState *d = s->ddi;
     if (!d) return;
     if (d->have_plans) { cufftDestroy(d->plan_r2c); cufftDestroy(d->plan_c2r); }
-    if (d->slab) { cufftDestroy(d->plan_a_fwd); cufftDestroy(d->plan_a_inv); cufftDestroy(d->plan_b); }
+    if (d->slab) {
+        if (d->plan_a_fwd) cufftDestroy(d->plan_a_fwd);
+        if (d->plan_a_inv) cufftDestroy(d->plan_a_inv);
+        if (d->plan_b) cufftDestroy(d->plan_b);
+    }
     cudaFree(d->s_in); cudaFree(d->s_out); cudaFree(d->s_a); cudaFree(d->s_b); cudaFree(d->s_c); cudaFree(d->s_d);
-    cudaFree(d->d_Kre); cudaFree(d->d_tw);
+    cudaFree(d->d_Kre); cudaFree(d->d_tw); cudaFree(d->d_tw_b); cudaFree(d->d_Kb);
     cudaFree(d->d_Mpad); cudaFree(d->d_Hpad); cudaFree(d->d_Mhat); cudaFree(d->d_Hhat); cudaFree(d->d_Khat); cudaFree(d->d_geom);
     delete d;
     s->ddi = nullptr;
@@ -706,16 +992,23 @@ int spin::ddi_prepare(spin_system *s) {
     d->SL = 3 * d->NZ * nb; d->S1 = d->P[0] / 2 + 1; d->S1p = d->S1;      // a 128-byte row pitch (264) was measured slower: 368 vs 347 us per step on cfg5
     // own a-pass: rows of power-of-two length, 8 <= Na <= 2048 (option ddi_slab = 2 keeps cuFFT's, for comparison)
     const int Na = s->nc[0];
-    d->own_a = want_slab && s->opt_ddi_slab == 1 && Na >= 8 && Na <= 2048 && (Na & (Na - 1)) == 0;
+    d->own_a = want_slab && s->opt_ddi_slab != 2 && Na >= 8 && Na <= 2048 && (Na & (Na - 1)) == 0;
+    // fused b-pass: one basis atom, power-of-two columns too, padded along c, and the block's columns fit into shared memory
+    // (option ddi_slab = 3 keeps cuFFT's b-pass and the separate contraction, for comparison)
+    const int Nb_ = s->nc[1];
+    d->bf_smem = ((size_t)(3 * d->NZ) * (size_t)(Nb_ + Nb_ / 8) + (size_t)Nb_) * sizeof(double2);      // columns + twiddles
+    d->fused_b = d->own_a && s->opt_ddi_slab == 1 && nb == 1 && Nb_ >= 8 && Nb_ <= 256 && (Nb_ & (Nb_ - 1)) == 0 && d->PZ == 2 * d->NZ && d->bf_smem <= 220 * 1024;
     if (want_slab) {
         const size_t nr = (size_t)s->nc[1] * d->SL * d->P[0], nc_ = (size_t)d->P[1] * d->SL * d->S1p;
-        SPIN_CUDA(cudaMalloc(&d->s_in, nr * sizeof(double)));
-        SPIN_CUDA(cudaMalloc(&d->s_out, nr * sizeof(double)));
-        SPIN_CUDA(cudaMalloc(&d->s_a, nc_ * sizeof(cufftDoubleComplex)));
-        SPIN_CUDA(cudaMalloc(&d->s_b, nc_ * sizeof(cufftDoubleComplex)));
+        if (!d->own_a) {
+            SPIN_CUDA(cudaMalloc(&d->s_in, nr * sizeof(double)));
+            SPIN_CUDA(cudaMalloc(&d->s_out, nr * sizeof(double)));
+            SPIN_CUDA(cudaMemsetAsync(d->s_in, 0, nr * sizeof(double), s->stream));                // ia >= Na: zero padding, never written
+        }
+        SPIN_CUDA(cudaMalloc(&d->s_a, nc_ * sizeof(cufftDoubleComplex)));                          // (fused b-pass: half of it is used)
         SPIN_CUDA(cudaMalloc(&d->s_d, nc_ * sizeof(cufftDoubleComplex)));
+        if (!d->fused_b) SPIN_CUDA(cudaMalloc(&d->s_b, nc_ * sizeof(cufftDoubleComplex)));
         if (nb > 1) SPIN_CUDA(cudaMalloc(&d->s_c, nc_ * sizeof(cufftDoubleComplex)));      // the contraction of several sublattices is out of place
-        SPIN_CUDA(cudaMemsetAsync(d->s_in, 0, nr * sizeof(double), s->stream));                    // ia >= Na: zero padding, never written
         SPIN_CUDA(cudaMemsetAsync(d->s_a, 0, nc_ * sizeof(cufftDoubleComplex), s->stream));        // rows >= Nb: zero padding, never written
         nreal = 1; ncplx = 1;      // the buffers of the general path are not needed
     }
@@ -731,13 +1024,17 @@ int spin::ddi_prepare(spin_system *s) {
     if (want_slab) {
         int na[1] = {d->P[0]}, nb1[1] = {d->P[1]};
         const int rows = s->nc[1] * d->SL, cols = d->SL * d->S1p;      // the pad columns of a row hold zeros and stay zero
-        SPIN_FFT(cufftPlanMany(&d->plan_a_fwd, 1, na, na, 1, d->P[0], na, 1, d->S1p, CUFFT_D2Z, rows));
-        SPIN_FFT(cufftPlanMany(&d->plan_a_inv, 1, na, na, 1, d->S1p, na, 1, d->P[0], CUFFT_Z2D, rows));
-        SPIN_FFT(cufftPlanMany(&d->plan_b, 1, nb1, nb1, cols, 1, nb1, cols, 1, CUFFT_Z2Z, cols));
+        if (!d->own_a) {
+            SPIN_FFT(cufftPlanMany(&d->plan_a_fwd, 1, na, na, 1, d->P[0], na, 1, d->S1p, CUFFT_D2Z, rows));
+            SPIN_FFT(cufftPlanMany(&d->plan_a_inv, 1, na, na, 1, d->S1p, na, 1, d->P[0], CUFFT_Z2D, rows));
+            SPIN_FFT(cufftSetStream(d->plan_a_fwd, s->stream));
+            SPIN_FFT(cufftSetStream(d->plan_a_inv, s->stream));
+        }
+        if (!d->fused_b) {
+            SPIN_FFT(cufftPlanMany(&d->plan_b, 1, nb1, nb1, cols, 1, nb1, cols, 1, CUFFT_Z2Z, cols));
+            SPIN_FFT(cufftSetStream(d->plan_b, s->stream));
+        }
         d->slab = true;      // from here on ddi_release destroys these plans
-        SPIN_FFT(cufftSetStream(d->plan_a_fwd, s->stream));
-        SPIN_FFT(cufftSetStream(d->plan_a_inv, s->stream));
-        SPIN_FFT(cufftSetStream(d->plan_b, s->stream));
         // the twiddle table of every padded length (the same values whichever system uploads them)
         static double twr[17][16], twi[17][16];
         for (int pz = 1; pz <= 16; ++pz)
@@ -748,25 +1045,32 @@ int spin::ddi_prepare(spin_system *s) {
         SPIN_CUDA(cudaMemcpyToSymbolAsync(DDI_TWR, twr, sizeof(twr), 0, cudaMemcpyHostToDevice, s->stream));
         SPIN_CUDA(cudaMemcpyToSymbolAsync(DDI_TWI, twi, sizeof(twi), 0, cudaMemcpyHostToDevice, s->stream));
         if (d->own_a) {
-            const int P0 = d->P[0];
-            std::vector<double2> tw((size_t)P0);
-            for (int t = 0; t < P0; ++t) {
-                tw[(size_t)t] = make_double2(cos(-2.0 * M_PI * t / P0), sin(-2.0 * M_PI * t / P0));
-                if ((8 * t) % P0 == 0) {      // exact at the multiples of an eighth of a turn
-                    const int k = (8 * t) / P0;
-                    const double h = 0.70710678118654752440;
-                    const double cr[8] = {1, h, 0, -h, -1, -h, 0, h}, ci[8] = {0, -h, -1, -h, 0, h, 1, h};
-                    tw[(size_t)t] = make_double2(cr[k], ci[k]);
+            // exp(-2 pi i t / P), t < P, exact at the multiples of an eighth of a turn
+            auto upload_table = [&](const int P, double2 **dst) -> int {
+                std::vector<double2> tw((size_t)P);
+                for (int t = 0; t < P; ++t) {
+                    tw[(size_t)t] = make_double2(cos(-2.0 * M_PI * t / P), sin(-2.0 * M_PI * t / P));
+                    if ((8 * t) % P == 0) {
+                        const int k = (8 * t) / P;
+                        const double h = 0.70710678118654752440;
+                        const double cr[8] = {1, h, 0, -h, -1, -h, 0, h}, ci[8] = {0, -h, -1, -h, 0, h, 1, h};
+                        tw[(size_t)t] = make_double2(cr[k], ci[k]);
+                    }
                 }
-            }
-            SPIN_CUDA(cudaMalloc(&d->d_tw, (size_t)P0 * sizeof(double2)));
-            SPIN_CUDA(cudaMemcpyAsync(d->d_tw, tw.data(), (size_t)P0 * sizeof(double2), cudaMemcpyHostToDevice, s->stream));
-            SPIN_CUDA(cudaStreamSynchronize(s->stream));      // tw is a local
-            const int M = P0 / 2;
+                SPIN_CUDA(cudaMalloc(dst, (size_t)P * sizeof(double2)));
+                SPIN_CUDA(cudaMemcpyAsync(*dst, tw.data(), (size_t)P * sizeof(double2), cudaMemcpyHostToDevice, s->stream));
+                SPIN_CUDA(cudaStreamSynchronize(s->stream));      // tw is a local
+                return SPIN_OK;
+            };
+            if (int rc = upload_table(d->P[0], &d->d_tw)) return rc;
+            const int M = d->P[0] / 2;
             d->a_rows_per_block = M <= 256 ? 8 : (M <= 512 ? 4 : (M <= 1024 ? 2 : 1));
-            d->a_smem = (size_t)d->a_rows_per_block * 2 * (M + M / 8) * sizeof(double2);
-            SPIN_CUDA(cudaFuncSetAttribute(ddi_apass_fwd_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)d->a_smem));
-            SPIN_CUDA(cudaFuncSetAttribute(ddi_apass_inv_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)d->a_smem));
+            d->a_smem = (size_t)d->a_rows_per_block * (2 * (M + M / 8) + 1) * sizeof(double2);
+            SPIN_CUDA(cudaFuncSetAttribute(ddi_apass_fwd_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)d->a_smem));
+            SPIN_CUDA(cudaFuncSetAttribute(ddi_apass_inv_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)d->a_smem));
+            SPIN_CUDA(cudaFuncSetAttribute(ddi_apass_fwd_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)d->a_smem));
+            SPIN_CUDA(cudaFuncSetAttribute(ddi_apass_inv_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)d->a_smem));
+            if (d->fused_b) if (int rc = upload_table(d->P[1], &d->d_tw_b)) return rc;
         }
     }
     if (d->rank > 0) {
@@ -814,6 +1118,23 @@ int spin::ddi_prepare(spin_system *s) {
         double dev, mag;
         memcpy(&dev, &h_chk[0], 8); memcpy(&mag, &h_chk[1], 8);
         d->mirror = d->PZ > 2 && dev <= 1e-13 * mag && s->opt_ddi_mirror;
+        if (d->fused_b) {      // the tensor in the fused kernel's order; the [6][PZ][S2] copy is not needed any more
+            const int Mb = s->nc[1], NPL = d->mirror ? d->PZ / 2 + 1 : d->PZ;
+            const long long nkb = (long long)d->S1 * 2 * 6 * NPL * Mb;
+            SPIN_CUDA(cudaMalloc(&d->d_Kb, (size_t)nkb * sizeof(double)));
+            ddi_bfused_tensor_kernel<<<(unsigned)((nkb + 255) / 256), 256, 0, s->stream>>>(d->d_Kre, d->d_Kb, d->PZ, NPL, Mb, d->S1);
+            s->n_launch++;
+            SPIN_CUDA(cudaStreamSynchronize(s->stream));
+            cudaFree(d->d_Kre); d->d_Kre = nullptr;
+#define SPIN_BF_ATTR(NZ_) case NZ_: \
+            SPIN_CUDA(cudaFuncSetAttribute(ddi_bfused_kernel<NZ_, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)d->bf_smem)); \
+            SPIN_CUDA(cudaFuncSetAttribute(ddi_bfused_kernel<NZ_, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)d->bf_smem)); break
+            switch (d->NZ) {
+                SPIN_BF_ATTR(1); SPIN_BF_ATTR(2); SPIN_BF_ATTR(3); SPIN_BF_ATTR(4); SPIN_BF_ATTR(5); SPIN_BF_ATTR(6); SPIN_BF_ATTR(7); SPIN_BF_ATTR(8);
+                default: return spin::fail(SPIN_ERR_STATE, "dipolar slab path: %d planes not supported", d->NZ);
+            }
+#undef SPIN_BF_ATTR
+        }
     }
     SPIN_CUDA(cudaStreamSynchronize(s->stream));
     SPIN_CUDA(cudaGetLastError());
@@ -831,8 +1152,34 @@ int spin::ddi_field(spin_system *s, const double *d_n, double *d_f) {
     if (d->slab) {
         const int a_rows = s->nc[1] * d->SL;
         const unsigned ga = d->own_a ? (unsigned)((a_rows + d->a_rows_per_block - 1) / d->a_rows_per_block) : 0u;
+        if (d->fused_b) {      // a-pass into [ka][slab][ib]; b-pass, c-pass, contraction and their inverses in one kernel; inverse a-pass
+            const int Ma = d->P[0] / 2, Mb = s->nc[1];
+            const size_t part1 = (size_t)d->S1 * d->SL * Mb;
+            int lgMb = 0;
+            while ((1 << lgMb) < Mb) ++lgMb;
+            ddi_apass_fwd_kernel<true><<<ga, 32 * d->a_rows_per_block, d->a_smem, s->stream>>>(s->plan, d_n, Ma, d->SL, d->S1p, a_rows, d->a_rows_per_block,
+                                                                                              d->d_geom, d->d_tw, d->s_a);
+            if (s->profile_on) cudaEventRecord(s->ev2, s->stream);
+#define SPIN_BF(NZ_) case NZ_: \
+            if (d->mirror) ddi_bfused_kernel<NZ_, true><<<2 * d->S1, DDI_BF_THREADS, d->bf_smem, s->stream>>>(d->d_Kb, (const double2 *)d->s_a, (double2 *)d->s_d, lgMb, d->S1, d->d_tw_b); \
+            else ddi_bfused_kernel<NZ_, false><<<2 * d->S1, DDI_BF_THREADS, d->bf_smem, s->stream>>>(d->d_Kb, (const double2 *)d->s_a, (double2 *)d->s_d, lgMb, d->S1, d->d_tw_b); break
+            switch (d->NZ) {
+                SPIN_BF(1); SPIN_BF(2); SPIN_BF(3); SPIN_BF(4); SPIN_BF(5); SPIN_BF(6); SPIN_BF(7); SPIN_BF(8);
+                default: return spin::fail(SPIN_ERR_STATE, "dipolar slab path: %d planes not supported", d->NZ);
+            }
+#undef SPIN_BF
+            if (s->profile_on) {      // the fused kernel alone (bench.py's roofline kernel on dipolar workloads)
+                cudaEventRecord(s->ev3, s->stream); cudaEventSynchronize(s->ev3);
+                float ms = 0.f; cudaEventElapsedTime(&ms, s->ev2, s->ev3);
+                s->prof_ms[3] += ms; s->prof_n[3]++;
+            }
+            ddi_apass_inv_kernel<true><<<ga, 32 * d->a_rows_per_block, d->a_smem, s->stream>>>(s->plan, d->s_d, Ma, d->SL, d->S1p, a_rows, d->a_rows_per_block,
+                                                                                              d->d_geom, C_DD / (double)d->Ptot, d->d_tw, d_f, part1);
+            s->n_launch += 3;
+            return SPIN_OK;
+        }
         if (d->own_a) {                                                               // scatter + a-pass over the occupied rows, one kernel
-            ddi_apass_fwd_kernel<<<ga, 32 * d->a_rows_per_block, d->a_smem, s->stream>>>(s->plan, d_n, d->P[0] / 2, d->SL, d->S1p, a_rows, d->a_rows_per_block,
+            ddi_apass_fwd_kernel<false><<<ga, 32 * d->a_rows_per_block, d->a_smem, s->stream>>>(s->plan, d_n, d->P[0] / 2, d->SL, d->S1p, a_rows, d->a_rows_per_block,
                                                                                         d->d_geom, d->d_tw, d->s_a);
         } else {
             ddi_slab_scatter_kernel<<<gs, nt, 0, s->stream>>>(s->plan, d_n, d->P[0], d->SL, d->d_geom, d->s_in);
@@ -872,8 +1219,8 @@ int spin::ddi_field(spin_system *s, const double *d_n, double *d_f) {
         }
         SPIN_FFT(cufftExecZ2Z(d->plan_b, spec_out, d->s_d, CUFFT_INVERSE));          // inverse b-pass
         if (d->own_a) {                                                               // inverse a-pass + gather, one kernel
-            ddi_apass_inv_kernel<<<ga, 32 * d->a_rows_per_block, d->a_smem, s->stream>>>(s->plan, d->s_d, d->P[0] / 2, d->SL, d->S1p, a_rows, d->a_rows_per_block,
-                                                                                        d->d_geom, C_DD / (double)d->Ptot, d->d_tw, d_f);
+            ddi_apass_inv_kernel<false><<<ga, 32 * d->a_rows_per_block, d->a_smem, s->stream>>>(s->plan, d->s_d, d->P[0] / 2, d->SL, d->S1p, a_rows, d->a_rows_per_block,
+                                                                                        d->d_geom, C_DD / (double)d->Ptot, d->d_tw, d_f, 0);
             s->n_launch += 3; s->n_fft += 2;
         } else {
             SPIN_FFT(cufftExecZ2D(d->plan_a_inv, d->s_d, d->s_out));                  // inverse a-pass, occupied rows only

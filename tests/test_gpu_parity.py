@@ -373,6 +373,41 @@ def test_ddi_slab_systems_of_different_thickness_alive_together(P, O):
         assert np.abs(gb.spins_get() - ob.spins()).max() <= SPIN_ATOL
 
 
+# Fused b-pass (ddi_bfused_kernel): columns of power-of-two length too -> the transforms along b and c, the contraction and their inverses
+# are one kernel between the two a-pass kernels (transposed layout); option ddi_slab = 3 keeps cuFFT's b-pass + the separate contraction.
+@pytest.mark.parametrize("cells,per,img,tilt", [((16, 16, 8), (1, 1, 0), (2, 2, 0), 0), ((32, 8, 3), (1, 1, 0), (1, 1, 0), 0), ((8, 16, 5), (0, 1, 0), (0, 2, 0), 1),
+                                                 ((64, 32, 2), (1, 1, 0), (1, 1, 0), 0), ((16, 64, 4), (0, 0, 0), (0, 0, 0), 1), ((8, 8, 7), (1, 0, 0), (2, 0, 0), 0),
+                                                 ((128, 16, 6), (1, 1, 0), (1, 1, 0), 1), ((16, 128, 2), (1, 1, 0), (1, 1, 0), 0), ((8, 256, 3), (0, 0, 0), (0, 0, 0), 0)])
+def test_ddi_fused_b_pass(P, O, cells, per, img, tilt):
+    brav = np.array([[1, 0, 0], [0.2 * tilt, 1, 0], [0.3 * tilt, 0.2 * tilt, 1.0]], float)
+    w = dataclasses.replace(W.config5().resized(cells, 10), bravais=brav, periodic=per, ddi_images=img)
+    g, o = pair(P, O, w)
+    info = g.spin_ddi_info()
+    assert info.endswith("+own-a+fused-b") and ("mirror" in info) == (not tilt), info
+    Bo, Bg = o.effective_field(), g.effective_field()
+    assert_fields_close(Bg, Bo)
+    assert abs(g.energy()[1][5] - o.energy_terms()[5]) <= 1e-12 * np.abs(o.energy_terms()).sum()
+    h = P.SpinSystem.from_workload(w)
+    h.spin_set_option("ddi_slab", 3)
+    Bh = h.effective_field()
+    assert h.spin_ddi_info().endswith("+own-a"), h.spin_ddi_info()
+    assert_fields_close(Bh, Bo)
+    assert np.abs(Bh - Bg).max() <= 1e-13 * np.abs(Bo).max()
+    # the dipolar part alone against the O(N^2) direct sum
+    if w.n_spins <= 8192:
+        w0 = dataclasses.replace(w, pair_J=w.pair_J * 0, pair_D=w.pair_D * 0, B=0.0, aniso=[])
+        g0, o0 = pair(P, O, w0)
+        Fd = o0.ddi_field(direct=True) / (w.mu_s[0] * O.MU_B)
+        assert np.abs(g0.effective_field() - Fd).max() <= 1e-11 * np.abs(Fd).max()
+    # per-site moments go through the a-pass kernels of this layout too
+    rng = np.random.default_rng(4)
+    site_mu = rng.uniform(0.5, 3.0, g.N)
+    g.hamiltonian_set_site_mu_s(site_mu); o.set_site_mu_s(site_mu)
+    assert_fields_close(g.effective_field(), o.effective_field())
+    g.llg_iterate(10); o.iterate(10)
+    assert np.abs(g.spins_get() - o.spins()).max() <= SPIN_ATOL
+
+
 # The slab contraction reads only PZ/2 + 1 of the PZ tensor planes when the spectrum is mirror symmetric along c (c perpendicular to the
 # film; checked numerically when the plan is built).  Tilted c: no symmetry, all planes are read; oblique a, b with c perpendicular: symmetric.
 @pytest.mark.parametrize("bravais", [[[1, 0, 0], [0, 1, 0], [0.3, 0.2, 1.0]], [[1, 0, 0], [0.5, 0.9, 0], [0, 0, 1.1]], [[1, 0, 0], [0, 1, 0], [0, 0, 1]]])
@@ -384,7 +419,7 @@ def test_ddi_slab_mirror_symmetry_of_the_tensor(P, O, bravais, cells, monkeypatc
     Bg = g.effective_field()
     assert_fields_close(Bg, Bo)
     tilted = abs(bravais[2][0]) + abs(bravais[2][1]) > 0
-    assert g.spin_ddi_info().replace("+own-a", "") == ("slab" if tilted else "slab+mirror"), g.spin_ddi_info()
+    assert g.spin_ddi_info().replace("+own-a", "").replace("+fused-b", "") == ("slab" if tilted else "slab+mirror"), g.spin_ddi_info()
     w0 = dataclasses.replace(w, pair_J=w.pair_J * 0, pair_D=w.pair_D * 0, B=0.0, aniso=[])
     g0, o0 = pair(P, O, w0)
     Fd = o0.ddi_field(direct=True) / (w.mu_s[0] * O.MU_B)
@@ -392,7 +427,7 @@ def test_ddi_slab_mirror_symmetry_of_the_tensor(P, O, bravais, cells, monkeypatc
     h = P.SpinSystem.from_workload(w)
     h.spin_set_option("ddi_mirror", 0)                  # all planes read, whatever the symmetry
     Bh = h.effective_field()
-    assert h.spin_ddi_info().replace("+own-a", "") == "slab"
+    assert h.spin_ddi_info().replace("+own-a", "").replace("+fused-b", "") == "slab"
     assert_fields_close(Bh, Bo)
     assert np.abs(Bh - Bg).max() <= 1e-13 * np.abs(Bo).max()
     g.llg_iterate(10); o.iterate(10)
