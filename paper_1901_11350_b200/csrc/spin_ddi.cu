@@ -56,6 +56,7 @@ struct DdiState {
     double2 *d_tw_b;           // exp(-2 pi i t / P1), t < P1
     double *d_Kb;              // [ka][r][6][planes][k'], ddi_bfused_tensor_kernel
     size_t bf_smem;
+    bool a256, b256;           // rows / columns of length 256: the radix-16 kernels (ddi_apass256_*, ddi_bfused_kernel<.., true>)
     bool mirror;               // K(kz) = +-K(PZ - kz) (c perpendicular to the film): the contraction reads PZ/2 + 1 of the PZ planes
 };
 
@@ -549,6 +550,196 @@ __device__ __forceinline__ void ddi_dft_inv(double (&re)[N], double (&im)[N]) {
     }
 }
 
+// ---------------------------------------------------------------------------------------------------------------------------
+// Transforms of length 256 (the a- and b-direction of a 256 x 256 film): two passes of radix 16 by HALF a warp, one butterfly of 16
+// points per lane and pass, the row in place in shared memory.  x(n), n = l + 16 q;  X(p + 16 u) = sum_l [W^(l p) A(l, p)] W_16^(l u),
+// A(l, p) = sum_q x(l + 16 q) W_16^(q p),  W = exp(-+ 2 pi i / 256).  Pass 1: lane l transforms its 16 inputs over q, multiplies by
+// W^(l p) (table T[p - 1][l] in shared memory, conflict-free) and stores A(l, p) at l 16 + p; pass 2: lane p reads A(l, p) over l,
+// transforms, and holds X(p + 16 u).  Rows are padded by one element in 16 (position i + (i >> 4)): every access of the 16 lanes is then
+// either to consecutive elements or at a stride of 17 elements, both free of bank conflicts.  Against three passes of radix 8 / 8 / 4 by
+// a whole warp this is two instead of three round trips through shared memory, one instead of two twiddle stages, and no index
+// arithmetic beyond constant offsets.
+__device__ __forceinline__ int ddi_pad16(const int i) { return i + (i >> 4); }
+constexpr int DDI_LP256 = 272;             // 256 + 256 / 16
+// in-place 4-point transform, natural order
+template <int SIGN> __device__ __forceinline__ void ddi_dft4(double2 &a, double2 &b, double2 &c, double2 &d) {
+    const double2 t0 = ddi_cadd(a, c), t1 = ddi_csub(a, c), t2 = ddi_cadd(b, d), t3 = ddi_rot90<SIGN>(ddi_csub(b, d));
+    a = ddi_cadd(t0, t2); b = ddi_cadd(t1, t3); c = ddi_csub(t0, t2); d = ddi_csub(t1, t3);
+}
+// 16-point transform in registers: input v[n] in natural order, output k left in v[ddi_out16(k)].  HALF: v[8..15] are zero (not read).
+__host__ __device__ constexpr int ddi_out16(int k) { return ((k & 3) << 2) | (k >> 2); }
+template <int SIGN, bool HALF>
+__device__ __forceinline__ void ddi_fft16(double2 (&v)[16]) {
+    // over m for every s: (v[s], v[s+4], v[s+8], v[s+12]) -> A(s, t) in v[s + 4 t]
+#pragma unroll
+    for (int s = 0; s < 4; ++s) {
+        if constexpr (HALF) {
+            const double2 a = v[s], b = v[s + 4], rb = ddi_rot90<SIGN>(b);
+            v[s] = ddi_cadd(a, b); v[s + 4] = ddi_cadd(a, rb); v[s + 8] = ddi_csub(a, b); v[s + 12] = ddi_csub(a, rb);
+        } else ddi_dft4<SIGN>(v[s], v[s + 4], v[s + 8], v[s + 12]);
+    }
+    // times W_16^(s t), then over s for every t: X(t + 4 u) in v[4 t + u]
+#pragma unroll
+    for (int t = 1; t < 4; ++t)
+#pragma unroll
+        for (int s = 1; s < 4; ++s) ddi_rot16(SIGN < 0 ? s * t : 16 - s * t, v[s + 4 * t].x, v[s + 4 * t].y);
+    // the four values of one t sit at v[4 t' ...]: gather them as (v[0 + 4t], v[1 + 4t], v[2 + 4t], v[3 + 4t])
+#pragma unroll
+    for (int t = 0; t < 4; ++t) ddi_dft4<SIGN>(v[4 * t], v[4 * t + 1], v[4 * t + 2], v[4 * t + 3]);
+}
+// the table of pass 1: T[(p - 1) 16 + l] = exp(-2 pi i l p / 256) = tw[2 l p] of the table exp(-2 pi i t / 512); `nthreads` threads fill it
+__device__ __forceinline__ void ddi_fill_t256(double2 *T, const double2 *__restrict__ tw, const int tid, const int nthreads) {
+    for (int i = tid; i < 240; i += nthreads) T[i] = __ldg(tw + 2 * (i & 15) * ((i >> 4) + 1));
+}
+// pass 1 on the inputs v[q] = x(l + 16 q) of lane l: transform, twiddle, store A(l, p) into the row.  The caller has loaded v.
+template <int SIGN, bool HALF>
+__device__ __forceinline__ void ddi_fft256_pass1(double2 (&v)[16], double2 *row, const double2 *T, const int l) {
+    ddi_fft16<SIGN, HALF>(v);
+    double2 *dst = row + 17 * l;                  // ddi_pad16(16 l + p) = 17 l + p
+    dst[0] = v[ddi_out16(0)];
+#pragma unroll
+    for (int p = 1; p < 16; ++p) {
+        double2 w = T[(p - 1) * 16 + l];
+        if (SIGN > 0) w.y = -w.y;
+        dst[p] = ddi_cmul(v[ddi_out16(p)], w);
+    }
+}
+// pass 2 of lane p: reads A(l, p) over l, transforms; output X(p + 16 u) is left in v[ddi_out16(u)]
+template <int SIGN>
+__device__ __forceinline__ void ddi_fft256_pass2(double2 (&v)[16], const double2 *row, const int p) {
+#pragma unroll
+    for (int l = 0; l < 16; ++l) v[l] = row[17 * l + p];
+    ddi_fft16<SIGN, false>(v);
+}
+
+// The a-pass kernels for rows of 512 real values (M = 256) in the transposed layout of the fused b-pass: a block of 256 threads takes 16
+// consecutive ib of one slab, half a warp per row.  Forward: the 128 non-zero complex inputs z(j) = x(2j) + i x(2j+1) come straight from
+// the spin array (pass 1 with half its inputs zero), the split X(k) = E(k) + W^k O(k) is done in place for the pair (k, 256 - k), and the
+// rows leave through a transposed copy (16 consecutive ib = 256 contiguous bytes per wave number).
+constexpr int DDI_A256_ROWS = 16, DDI_A256_WS = DDI_LP256 + 1;      // rows per block; row stride (X(256) has a slot of its own)
+constexpr size_t DDI_A256_SMEM = ((size_t)DDI_A256_ROWS * DDI_A256_WS + 240) * sizeof(double2);
+__global__ void __launch_bounds__(256) ddi_apass256_fwd_kernel(const __grid_constant__ DevicePlan L, const double *__restrict__ n, int SL,
+                                                               const double *__restrict__ mu_b, const double2 *__restrict__ tw,
+                                                               cufftDoubleComplex *__restrict__ out) {
+    extern __shared__ double2 ddi_sm[];
+    constexpr int M = 256;
+    double2 *T = ddi_sm + DDI_A256_ROWS * DDI_A256_WS;
+    ddi_fill_t256(T, tw, threadIdx.x, blockDim.x);
+    const int hw = threadIdx.x >> 4, l = threadIdx.x & 15;                 // row of the block, lane of the half warp
+    const unsigned hmask = 0xffffu << (threadIdx.x & 16);      // the lanes of this half warp
+    const int rowid = blockIdx.x * DDI_A256_ROWS + hw;
+    const int ib = rowid % L.Nb, slab = rowid / L.Nb;
+    const int bc = slab / L.Nc, ic = slab - bc * L.Nc, sb = bc / 3, comp = bc - 3 * sb;
+    const double mu = mu_b[sb];
+    const double2 *src = (const double2 *)(n + (size_t)sb * L.sub + ((size_t)(ic + L.LC) * L.PB + (ib + L.LB)) * (3 * L.PA) + comp * L.PA + L.LA);
+    double2 *row = ddi_sm + hw * DDI_A256_WS;
+    double2 v[16];
+#pragma unroll
+    for (int q = 0; q < 8; ++q) v[q] = __ldg(src + l + 16 * q);
+#pragma unroll
+    for (int q = 0; q < 8; ++q) {
+        double m0 = mu, m1 = mu;
+        if (L.mu_ratio) { const double2 r = ddi_row_ratio(L, sb, ib, ic, l + 16 * q); m0 *= r.x; m1 *= r.y; }
+        v[q].x *= m0; v[q].y *= m1;
+    }
+    __syncthreads();                                                       // T is complete
+    ddi_fft256_pass1<-1, true>(v, row, T, l);
+    __syncwarp(hmask);
+    ddi_fft256_pass2<-1>(v, row, l);
+    __syncwarp(hmask);                                                          // every lane has read the row
+#pragma unroll
+    for (int u = 0; u < 16; ++u) row[l + 17 * u] = v[ddi_out16(u)];        // Z(l + 16 u), natural order
+    __syncwarp(hmask);
+    // split in place: lane l takes k = l + 16 i, i < 8 (and lane 0 also k = 128), together with 256 - k
+#pragma unroll
+    for (int i = 0; i <= 8; ++i) {
+        const int k = l + 16 * i;
+        if (i == 8 && l != 0) break;
+        const int km = (M - k) & (M - 1);
+        const double2 zk = row[ddi_pad16(k)], zm = row[ddi_pad16(km)];
+        const double er = 0.5 * (zk.x + zm.x), ei = 0.5 * (zk.y - zm.y);            // E = (Z(k) + conj Z(M-k)) / 2
+        const double orr = 0.5 * (zk.y + zm.y), oi = -0.5 * (zk.x - zm.x);          // O = (Z(k) - conj Z(M-k)) / (2i)
+        const double2 w = __ldg(tw + k);                                            // exp(-2 pi i k / 512)
+        const double pr = fma(orr, w.x, -oi * w.y), pi = fma(orr, w.y, oi * w.x);   // W^k O
+        row[ddi_pad16(k)] = make_double2(er + pr, ei + pi);                         // X(k) = E + W^k O
+        row[ddi_pad16(M - k)] = make_double2(er - pr, -(ei - pi));                  // X(M - k) = conj(E - W^k O)
+    }
+    __syncthreads();
+    const int ib0 = (blockIdx.x * DDI_A256_ROWS) % L.Nb;
+    cufftDoubleComplex *o = out + (size_t)slab * L.Nb + ib0;
+    for (int idx = threadIdx.x; idx < (M + 1) * DDI_A256_ROWS; idx += 256) {
+        const int k = idx >> 4, w = idx & 15;
+        o[(size_t)k * SL * L.Nb + w] = ddi_sm[w * DDI_A256_WS + ddi_pad16(k)];
+    }
+}
+
+// inverse: the two partial results [r][ka][slab][ib] are added while they are gathered into the rows; Z(k) = E + i O is rebuilt in place
+// for the pair (k, 256 - k); of the transform only the 128 outputs that are spins are stored (the rest is the zero padding's image).
+__global__ void __launch_bounds__(256) ddi_apass256_inv_kernel(const __grid_constant__ DevicePlan L, const cufftDoubleComplex *__restrict__ in, int SL,
+                                                               const double *__restrict__ mu_b, double scale0, const double2 *__restrict__ tw,
+                                                               double *__restrict__ f, size_t part1) {
+    extern __shared__ double2 ddi_sm[];
+    constexpr int M = 256;
+    double2 *T = ddi_sm + DDI_A256_ROWS * DDI_A256_WS;
+    ddi_fill_t256(T, tw, threadIdx.x, blockDim.x);
+    const int hw = threadIdx.x >> 4, l = threadIdx.x & 15;
+    const unsigned hmask = 0xffffu << (threadIdx.x & 16);      // the lanes of this half warp
+    const int rowid = blockIdx.x * DDI_A256_ROWS + hw;
+    const int ib = rowid % L.Nb, slab = rowid / L.Nb;
+    const int bc = slab / L.Nc, ic = slab - bc * L.Nc, sb = bc / 3, comp = bc - 3 * sb;
+    const double scale = mu_b[sb] * scale0;
+    double2 *row = ddi_sm + hw * DDI_A256_WS;
+    {
+        const int ib0 = (blockIdx.x * DDI_A256_ROWS) % L.Nb;
+        const cufftDoubleComplex *g0 = in + (size_t)slab * L.Nb + ib0, *g1 = g0 + part1;
+        constexpr int total = (M + 1) * DDI_A256_ROWS, U = 8;             // 4112 elements: 2 x 8 per thread and a tail of 16
+        for (int base = threadIdx.x; base < total; base += U * 256) {
+            double2 p0[U], p1[U];
+#pragma unroll
+            for (int u = 0; u < U; ++u) {
+                const int idx = min(base + u * 256, total - 1);
+                const size_t o = (size_t)(idx >> 4) * SL * L.Nb + (idx & 15);
+                p0[u] = __ldg(g0 + o); p1[u] = __ldg(g1 + o);
+            }
+#pragma unroll
+            for (int u = 0; u < U; ++u) {
+                const int idx = base + u * 256;
+                if (idx < total) ddi_sm[(idx & 15) * DDI_A256_WS + ddi_pad16(idx >> 4)] = make_double2(p0[u].x + p1[u].x, p0[u].y + p1[u].y);
+            }
+        }
+    }
+    __syncthreads();
+#pragma unroll
+    for (int i = 0; i <= 8; ++i) {
+        const int k = l + 16 * i;
+        if (i == 8 && l != 0) break;
+        const double2 xk = row[ddi_pad16(k)], xm = row[ddi_pad16(M - k)];
+        const double er = xk.x + xm.x, ei = xk.y - xm.y;                            // E = X(k) + conj X(M-k)
+        const double dr = xk.x - xm.x, di = xk.y + xm.y;                            // X(k) - conj X(M-k)
+        const double2 w = __ldg(tw + k);                                            // times exp(+2 pi i k / 512)
+        const double orr = fma(dr, w.x, di * w.y), oi = fma(di, w.x, -dr * w.y);
+        row[ddi_pad16(k)] = make_double2(er - oi, ei + orr);                        // Z(k) = E + i O
+        if (k) row[ddi_pad16(M - k)] = make_double2(er + oi, -(ei - orr));          // Z(M - k) = conj(E - i O)
+    }
+    __syncwarp(hmask);
+    double2 v[16];
+#pragma unroll
+    for (int q = 0; q < 16; ++q) v[q] = row[l + 17 * q];
+    __syncwarp(hmask);
+    ddi_fft256_pass1<+1, false>(v, row, T, l);
+    __syncwarp(hmask);
+    ddi_fft256_pass2<+1>(v, row, l);
+    double2 *dst = (double2 *)(f + (size_t)sb * L.sub + ((size_t)(ic + L.LC) * L.PB + (ib + L.LB)) * (3 * L.PA) + comp * L.PA + L.LA);
+#pragma unroll
+    for (int u = 0; u < 8; ++u) {                                                   // z(j), j = l + 16 u < 128
+        const int j = l + 16 * u;
+        const double2 z = v[ddi_out16(u)];
+        double m0 = scale, m1 = scale;
+        if (L.mu_ratio) { const double2 r = ddi_row_ratio(L, sb, ib, ic, j); m0 *= r.x; m1 *= r.y; }
+        dst[j] = make_double2(m0 * z.x, m1 * z.y);
+    }
+}
+
 // Slab path, the transform along c fused with the tensor contraction, per in-plane wave vector q = (kx, ky):
 //   M^(kz) = sum_{z < NZ} M2(z) w^(kz z),  w = exp(-2 pi i / PZ)     (pruned: planes z >= NZ are zero padding)
 //   H^(kz) = K^(kz) . M^(kz)                                          (6-component real symmetric tensor)
@@ -699,12 +890,15 @@ __global__ void __launch_bounds__(2 * DDI_CT_COLS, 4) ddi_slab_contract_kernel(c
 // parities.  (One block per ka taking the two parities in turn and adding them itself was measured slower: 76 instead of 66 us.)  Shared memory: 3 NZ padded columns of Nb complex numbers (cfg5: 24 columns x 4.6 KB = 110.6 KB, two blocks of 256 threads per SM,
 // so that one block's loads overlap the other's arithmetic).
 constexpr int DDI_BF_THREADS = 256, DDI_BF_WARPS = DDI_BF_THREADS / 32;
-template <int NZ, bool MIRROR>
+// F256: columns of length 256 -- half a warp per column, two passes of radix 16 (ddi_fft256_pass1 / 2), rows padded by one in 16.
+template <int NZ, bool MIRROR, bool F256>
 __global__ void __launch_bounds__(DDI_BF_THREADS, 2) ddi_bfused_kernel(const double *__restrict__ Kb, const double2 *__restrict__ Tin, double2 *__restrict__ Tout,
-                                                                        const int lgM, const int S1, const double2 *__restrict__ tw) {
-    constexpr int SL = 3 * NZ, NPL = MIRROR ? NZ + 1 : 2 * NZ;
+                                                                        const int lgM_, const int S1, const double2 *__restrict__ tw) {
+    constexpr int SL = 3 * NZ, NPL = MIRROR ? NZ + 1 : 2 * NZ, PADSH = F256 ? 4 : 3;
     extern __shared__ double2 ddi_sm[];
-    const int M = 1 << lgM, LP = M + (M >> 3);
+    const int lgM = F256 ? 8 : lgM_;
+    const int M = 1 << lgM, LP = M + (M >> PADSH);
+    auto pad = [](const int i) { return i + (i >> PADSH); };
     const int ka = blockIdx.x >> 1, r = blockIdx.x & 1;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const double *Kme = Kb + (((size_t)ka * 2 + r) * 6 * NPL << lgM);
@@ -713,10 +907,34 @@ __global__ void __launch_bounds__(DDI_BF_THREADS, 2) ddi_bfused_kernel(const dou
     // the first M entries of the twiddle table, in shared memory behind the columns (all a pass or the twist ever reads)
     double2 *tws = ddi_sm + (size_t)SL * LP;
     for (int i = tid; i < M; i += DDI_BF_THREADS) tws[i] = __ldg(tw + i);
+    if constexpr (F256) {
+        // ---- forward, length 256: half a warp per column; pass 1 reads global memory (16 loads per lane in flight) and applies the twist
+        double2 *T = tws + M;
+        ddi_fill_t256(T, tw, tid, DDI_BF_THREADS);
+        __syncthreads();                                                       // tws and T are complete
+        const int l = tid & 15;
+        const unsigned hmask = 0xffffu << (tid & 16);      // the lanes of this half warp (the other half may have no column)
+        for (int slab = tid >> 4; slab < SL; slab += DDI_BF_THREADS / 16) {
+            const double2 *src = Tin + (((size_t)ka * SL + slab) << 8) + l;
+            double2 *row = ddi_sm + slab * LP;
+            double2 v[16];
+#pragma unroll
+            for (int q = 0; q < 16; ++q) v[q] = __ldg(src + 16 * q);
+            if (r) {
+#pragma unroll
+                for (int q = 0; q < 16; ++q) v[q] = ddi_cmul(v[q], tws[l + 16 * q]);
+            }
+            ddi_fft256_pass1<-1, false>(v, row, T, l);
+            __syncwarp(hmask);
+            ddi_fft256_pass2<-1>(v, row, l);
+            __syncwarp(hmask);
+#pragma unroll
+            for (int u = 0; u < 16; ++u) row[l + 17 * u] = v[ddi_out16(u)];
+        }
+    } else {
     // ---- forward: one warp per column, in place in the column's shared-memory row (every lane holds its M / 32 elements between the
     // loads and the stores of a pass).  The first pass (always radix 8) reads global memory and applies the twist of the odd wave
     // numbers; the loads of the warp's next column are in flight while it transforms the current one.
-    {
         constexpr int NIT = (SL + DDI_BF_WARPS - 1) / DDI_BF_WARPS;
         const int span = M >> 3, j = min(lane, span - 1);
         double2 buf[2][8];
@@ -754,7 +972,7 @@ __global__ void __launch_bounds__(DDI_BF_THREADS, 2) ddi_bfused_kernel(const dou
     for (int k0 = 0; k0 < M; k0 += half) {
         const int kp = k0 + (tid - e * half);
         const bool live = kp < M;
-        double2 *col = ddi_sm + ddi_pad(kp);
+        double2 *col = ddi_sm + pad(kp);
         double xr[3][NZ], xi[3][NZ];
         if (live) {
 #pragma unroll
@@ -786,6 +1004,29 @@ __global__ void __launch_bounds__(DDI_BF_THREADS, 2) ddi_bfused_kernel(const dou
         }
     }
     __syncthreads();
+    if constexpr (F256) {
+        // ---- inverse, length 256: the outputs of pass 2 go straight to global memory (twisted back), 256 contiguous bytes per half warp
+        const double2 *T = tws + M;
+        const int l = tid & 15;
+        const unsigned hmask = 0xffffu << (tid & 16);
+        for (int slab = tid >> 4; slab < SL; slab += DDI_BF_THREADS / 16) {
+            double2 *dstg = Tout + ((((size_t)r * S1 + ka) * SL + slab) << 8) + l;
+            double2 *row = ddi_sm + slab * LP;
+            double2 v[16];
+#pragma unroll
+            for (int q = 0; q < 16; ++q) v[q] = row[l + 17 * q];
+            __syncwarp(hmask);
+            ddi_fft256_pass1<+1, false>(v, row, T, l);
+            __syncwarp(hmask);
+            ddi_fft256_pass2<+1>(v, row, l);
+#pragma unroll
+            for (int u = 0; u < 16; ++u) {
+                double2 x = v[ddi_out16(u)];
+                if (r) { double2 w = tws[l + 16 * u]; w.y = -w.y; x = ddi_cmul(x, w); }
+                dstg[16 * u] = x;
+            }
+        }
+    } else {
     // ---- inverse: one warp per column, the last pass writes the partial result of this parity (twisted back) to global memory
     for (int slab = warp; slab < SL; slab += DDI_BF_WARPS) {
         double2 *dstg = Tout + ((((size_t)r * S1 + ka) * SL + slab) << lgM);
@@ -800,6 +1041,7 @@ __global__ void __launch_bounds__(DDI_BF_THREADS, 2) ddi_bfused_kernel(const dou
             if (r) { double2 w = tws[i]; w.y = -w.y; v = ddi_cmul(v, w); }
             dstg[i] = v;
         });
+    }
     }
 }
 
@@ -997,6 +1239,7 @@ int spin::ddi_prepare(spin_system *s) {
     // (option ddi_slab = 3 keeps cuFFT's b-pass and the separate contraction, for comparison)
     const int Nb_ = s->nc[1];
     d->bf_smem = ((size_t)(3 * d->NZ) * (size_t)(Nb_ + Nb_ / 8) + (size_t)Nb_) * sizeof(double2);      // columns + twiddles
+    if (Nb_ == 256) d->bf_smem = ((size_t)(3 * d->NZ) * DDI_LP256 + 256 + 240) * sizeof(double2);         // columns (padded by 1 in 16) + twiddles + pass-1 table
     d->fused_b = d->own_a && s->opt_ddi_slab == 1 && nb == 1 && Nb_ >= 8 && Nb_ <= 256 && (Nb_ & (Nb_ - 1)) == 0 && d->PZ == 2 * d->NZ && d->bf_smem <= 220 * 1024;
     if (want_slab) {
         const size_t nr = (size_t)s->nc[1] * d->SL * d->P[0], nc_ = (size_t)d->P[1] * d->SL * d->S1p;
@@ -1071,6 +1314,12 @@ int spin::ddi_prepare(spin_system *s) {
             SPIN_CUDA(cudaFuncSetAttribute(ddi_apass_fwd_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)d->a_smem));
             SPIN_CUDA(cudaFuncSetAttribute(ddi_apass_inv_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)d->a_smem));
             if (d->fused_b) if (int rc = upload_table(d->P[1], &d->d_tw_b)) return rc;
+            d->a256 = d->fused_b && M == 256 && Nb_ % DDI_A256_ROWS == 0;
+            d->b256 = d->fused_b && Nb_ == 256;
+            if (d->a256) {
+                SPIN_CUDA(cudaFuncSetAttribute(ddi_apass256_fwd_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)DDI_A256_SMEM));
+                SPIN_CUDA(cudaFuncSetAttribute(ddi_apass256_inv_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)DDI_A256_SMEM));
+            }
         }
     }
     if (d->rank > 0) {
@@ -1127,8 +1376,10 @@ int spin::ddi_prepare(spin_system *s) {
             SPIN_CUDA(cudaStreamSynchronize(s->stream));
             cudaFree(d->d_Kre); d->d_Kre = nullptr;
 #define SPIN_BF_ATTR(NZ_) case NZ_: \
-            SPIN_CUDA(cudaFuncSetAttribute(ddi_bfused_kernel<NZ_, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)d->bf_smem)); \
-            SPIN_CUDA(cudaFuncSetAttribute(ddi_bfused_kernel<NZ_, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)d->bf_smem)); break
+            SPIN_CUDA(cudaFuncSetAttribute(ddi_bfused_kernel<NZ_, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)d->bf_smem)); \
+            SPIN_CUDA(cudaFuncSetAttribute(ddi_bfused_kernel<NZ_, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)d->bf_smem)); \
+            SPIN_CUDA(cudaFuncSetAttribute(ddi_bfused_kernel<NZ_, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)d->bf_smem)); \
+            SPIN_CUDA(cudaFuncSetAttribute(ddi_bfused_kernel<NZ_, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)d->bf_smem)); break
             switch (d->NZ) {
                 SPIN_BF_ATTR(1); SPIN_BF_ATTR(2); SPIN_BF_ATTR(3); SPIN_BF_ATTR(4); SPIN_BF_ATTR(5); SPIN_BF_ATTR(6); SPIN_BF_ATTR(7); SPIN_BF_ATTR(8);
                 default: return spin::fail(SPIN_ERR_STATE, "dipolar slab path: %d planes not supported", d->NZ);
@@ -1157,24 +1408,32 @@ int spin::ddi_field(spin_system *s, const double *d_n, double *d_f) {
             const size_t part1 = (size_t)d->S1 * d->SL * Mb;
             int lgMb = 0;
             while ((1 << lgMb) < Mb) ++lgMb;
-            ddi_apass_fwd_kernel<true><<<ga, 32 * d->a_rows_per_block, d->a_smem, s->stream>>>(s->plan, d_n, Ma, d->SL, d->S1p, a_rows, d->a_rows_per_block,
-                                                                                              d->d_geom, d->d_tw, d->s_a);
+            if (d->a256)
+                ddi_apass256_fwd_kernel<<<a_rows / DDI_A256_ROWS, 256, DDI_A256_SMEM, s->stream>>>(s->plan, d_n, d->SL, d->d_geom, d->d_tw, d->s_a);
+            else
+                ddi_apass_fwd_kernel<true><<<ga, 32 * d->a_rows_per_block, d->a_smem, s->stream>>>(s->plan, d_n, Ma, d->SL, d->S1p, a_rows, d->a_rows_per_block,
+                                                                                                  d->d_geom, d->d_tw, d->s_a);
             if (s->profile_on) cudaEventRecord(s->ev2, s->stream);
+#define SPIN_BF1(NZ_, MIR_, F_) ddi_bfused_kernel<NZ_, MIR_, F_><<<2 * d->S1, DDI_BF_THREADS, d->bf_smem, s->stream>>>(d->d_Kb, (const double2 *)d->s_a, (double2 *)d->s_d, lgMb, d->S1, d->d_tw_b)
 #define SPIN_BF(NZ_) case NZ_: \
-            if (d->mirror) ddi_bfused_kernel<NZ_, true><<<2 * d->S1, DDI_BF_THREADS, d->bf_smem, s->stream>>>(d->d_Kb, (const double2 *)d->s_a, (double2 *)d->s_d, lgMb, d->S1, d->d_tw_b); \
-            else ddi_bfused_kernel<NZ_, false><<<2 * d->S1, DDI_BF_THREADS, d->bf_smem, s->stream>>>(d->d_Kb, (const double2 *)d->s_a, (double2 *)d->s_d, lgMb, d->S1, d->d_tw_b); break
+            if (d->b256) { if (d->mirror) SPIN_BF1(NZ_, true, true); else SPIN_BF1(NZ_, false, true); } \
+            else { if (d->mirror) SPIN_BF1(NZ_, true, false); else SPIN_BF1(NZ_, false, false); } break
             switch (d->NZ) {
                 SPIN_BF(1); SPIN_BF(2); SPIN_BF(3); SPIN_BF(4); SPIN_BF(5); SPIN_BF(6); SPIN_BF(7); SPIN_BF(8);
                 default: return spin::fail(SPIN_ERR_STATE, "dipolar slab path: %d planes not supported", d->NZ);
             }
 #undef SPIN_BF
+#undef SPIN_BF1
             if (s->profile_on) {      // the fused kernel alone (bench.py's roofline kernel on dipolar workloads)
                 cudaEventRecord(s->ev3, s->stream); cudaEventSynchronize(s->ev3);
                 float ms = 0.f; cudaEventElapsedTime(&ms, s->ev2, s->ev3);
                 s->prof_ms[3] += ms; s->prof_n[3]++;
             }
-            ddi_apass_inv_kernel<true><<<ga, 32 * d->a_rows_per_block, d->a_smem, s->stream>>>(s->plan, d->s_d, Ma, d->SL, d->S1p, a_rows, d->a_rows_per_block,
-                                                                                              d->d_geom, C_DD / (double)d->Ptot, d->d_tw, d_f, part1);
+            if (d->a256)
+                ddi_apass256_inv_kernel<<<a_rows / DDI_A256_ROWS, 256, DDI_A256_SMEM, s->stream>>>(s->plan, d->s_d, d->SL, d->d_geom, C_DD / (double)d->Ptot, d->d_tw, d_f, part1);
+            else
+                ddi_apass_inv_kernel<true><<<ga, 32 * d->a_rows_per_block, d->a_smem, s->stream>>>(s->plan, d->s_d, Ma, d->SL, d->S1p, a_rows, d->a_rows_per_block,
+                                                                                                  d->d_geom, C_DD / (double)d->Ptot, d->d_tw, d_f, part1);
             s->n_launch += 3;
             return SPIN_OK;
         }

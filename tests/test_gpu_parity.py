@@ -377,7 +377,10 @@ def test_ddi_slab_systems_of_different_thickness_alive_together(P, O):
 # are one kernel between the two a-pass kernels (transposed layout); option ddi_slab = 3 keeps cuFFT's b-pass + the separate contraction.
 @pytest.mark.parametrize("cells,per,img,tilt", [((16, 16, 8), (1, 1, 0), (2, 2, 0), 0), ((32, 8, 3), (1, 1, 0), (1, 1, 0), 0), ((8, 16, 5), (0, 1, 0), (0, 2, 0), 1),
                                                  ((64, 32, 2), (1, 1, 0), (1, 1, 0), 0), ((16, 64, 4), (0, 0, 0), (0, 0, 0), 1), ((8, 8, 7), (1, 0, 0), (2, 0, 0), 0),
-                                                 ((128, 16, 6), (1, 1, 0), (1, 1, 0), 1), ((16, 128, 2), (1, 1, 0), (1, 1, 0), 0), ((8, 256, 3), (0, 0, 0), (0, 0, 0), 0)])
+                                                 ((128, 16, 6), (1, 1, 0), (1, 1, 0), 1), ((16, 128, 2), (1, 1, 0), (1, 1, 0), 0), ((8, 256, 3), (0, 0, 0), (0, 0, 0), 0),
+                                                 # rows / columns of length 256: the radix-16 kernels
+                                                 ((256, 16, 2), (1, 1, 0), (1, 1, 0), 0), ((256, 32, 3), (0, 1, 0), (0, 1, 0), 1), ((16, 256, 4), (1, 1, 0), (1, 1, 0), 1),
+                                                 ((256, 256, 2), (1, 1, 0), (1, 1, 0), 0), ((256, 256, 5), (0, 0, 0), (0, 0, 0), 1)])
 def test_ddi_fused_b_pass(P, O, cells, per, img, tilt):
     brav = np.array([[1, 0, 0], [0.2 * tilt, 1, 0], [0.3 * tilt, 0.2 * tilt, 1.0]], float)
     w = dataclasses.replace(W.config5().resized(cells, 10), bravais=brav, periodic=per, ddi_images=img)
