@@ -618,7 +618,7 @@ __device__ __forceinline__ void ddi_fft256_pass2(double2 (&v)[16], const double2
 // rows leave through a transposed copy (16 consecutive ib = 256 contiguous bytes per wave number).
 constexpr int DDI_A256_ROWS = 16, DDI_A256_WS = DDI_LP256 + 1;      // rows per block; row stride (X(256) has a slot of its own)
 constexpr size_t DDI_A256_SMEM = ((size_t)DDI_A256_ROWS * DDI_A256_WS + 240) * sizeof(double2);
-__global__ void __launch_bounds__(256) ddi_apass256_fwd_kernel(const __grid_constant__ DevicePlan L, const double *__restrict__ n, int SL,
+__global__ void __launch_bounds__(256, 3) ddi_apass256_fwd_kernel(const __grid_constant__ DevicePlan L, const double *__restrict__ n, int SL,
                                                                const double *__restrict__ mu_b, const double2 *__restrict__ tw,
                                                                cufftDoubleComplex *__restrict__ out) {
     extern __shared__ double2 ddi_sm[];
@@ -783,15 +783,17 @@ __device__ __forceinline__ void ddi_column_half(double (&xr)[3][NZ], double (&xi
     auto planes = [&](auto ec) {
         constexpr int E = decltype(ec)::value;
         // planes this thread reads: kz = 2 j + E, j < NJ (MIRROR: up to PZ / 2 only, the rest are mirror images); the tensor of plane
-        // j + 1 is loaded before plane j is contracted
+        // j + AHEAD is loaded before plane j is contracted
         constexpr int NJ = !PAD ? 1 : (MIRROR ? (PZ / 2 - E) / 2 + 1 : NZ);
-        double k[2][6];
-        kload(PAD ? E : 0, k[0]);
+        constexpr int AHEAD = 2;
+        double k[AHEAD + 1][6];
+#pragma unroll
+        for (int j = 0; j < AHEAD && j < NJ; ++j) kload(PAD ? 2 * j + E : 0, k[j]);
 #pragma unroll
         for (int j = 0; j < NJ; ++j) {
             const int kz = PAD ? 2 * j + E : 0;
-            if (j + 1 < NJ) kload(kz + 2, k[(j + 1) & 1]);
-            const double(&kk)[6] = k[j & 1];
+            if (j + AHEAD < NJ) kload(kz + 2 * AHEAD, k[(j + AHEAD) % (AHEAD + 1)]);
+            const double(&kk)[6] = k[j % (AHEAD + 1)];
             contract(ddi_pos<NZ>(j), kk[0], kk[1], kk[2], kk[3], kk[4], kk[5]);
             if (MIRROR && kz > 0 && 2 * kz < PZ)                        // plane PZ - kz: the same values, xz and yz with the opposite sign
                 contract(ddi_pos<NZ>((PZ - kz - E) / 2), kk[0], kk[1], -kk[2], kk[3], -kk[4], kk[5]);
