@@ -965,7 +965,8 @@ extern "C" int llg_iterate(spin_system *s, int64_t n_steps) {
     }
     // Larger lattices: replay a captured graph of G steps (an even number, so the ping-pong buffers return to the
     // same roles); the kernels read the step counter from device memory, the graph's last node advances it by G.
-    const bool graph_ok = s->opt_graph && !s->profile_on && !s->ddi_on;
+    // (dipolar coupling: only the path that is kernels throughout -- cuFFT's transforms stay outside a capture)
+    const bool graph_ok = s->opt_graph && !s->profile_on && (!s->ddi_on || ddi_graph_ok(s));
     const int G = 16;
     if (graph_ok && n_steps >= G) {
         cudaGraphExec_t &gexec = s->graph_exec[s->cur];
@@ -975,6 +976,7 @@ extern "C" int llg_iterate(spin_system *s, int64_t n_steps) {
             const int64_t launches_before = s->n_launch;
             for (int k = 0; k < G && rc == SPIN_OK; ++k) rc = enqueue_step(s, (unsigned)k);
             advance_step_kernel<<<1, 1, 0, s->stream>>>(s->d_step, (unsigned long long)G);
+            s->graph_launches = s->n_launch - launches_before + 1;      // what one replay launches
             s->n_launch = launches_before;
             cudaError_t e = cudaStreamEndCapture(s->stream, &graph);
             if (rc) { if (graph) cudaGraphDestroy(graph); return rc; }
@@ -986,7 +988,7 @@ extern "C" int llg_iterate(spin_system *s, int64_t n_steps) {
         }
         while (n_steps - done >= G) {
             SPIN_CUDA(cudaGraphLaunch(gexec, s->stream));
-            s->n_launch += (s->solver == SPIN_SOLVER_RK4 ? 4 : (jit_march_ready(s) ? 1 : 2)) * G + 1;
+            s->n_launch += s->graph_launches;
             done += G;
         }
     }

@@ -692,21 +692,27 @@ __global__ void __launch_bounds__(256) ddi_apass256_inv_kernel(const __grid_cons
     {
         const int ib0 = (blockIdx.x * DDI_A256_ROWS) % L.Nb;
         const cufftDoubleComplex *g0 = in + (size_t)slab * L.Nb + ib0, *g1 = g0 + part1;
-        constexpr int total = (M + 1) * DDI_A256_ROWS, U = 8;             // 4112 elements: 2 x 8 per thread and a tail of 16
+        constexpr int total = M * DDI_A256_ROWS, U = 8;                   // wave numbers k < 256: 2 x 8 elements per thread ...
+        double2 q0 = make_double2(0.0, 0.0), q1 = q0;                      // ... and k = 256: one element for the first 16 threads
+        if (threadIdx.x < DDI_A256_ROWS) {
+            const size_t o = (size_t)M * SL * L.Nb + threadIdx.x;
+            q0 = __ldg(g0 + o); q1 = __ldg(g1 + o);
+        }
         for (int base = threadIdx.x; base < total; base += U * 256) {
             double2 p0[U], p1[U];
 #pragma unroll
             for (int u = 0; u < U; ++u) {
-                const int idx = min(base + u * 256, total - 1);
+                const int idx = base + u * 256;
                 const size_t o = (size_t)(idx >> 4) * SL * L.Nb + (idx & 15);
                 p0[u] = __ldg(g0 + o); p1[u] = __ldg(g1 + o);
             }
 #pragma unroll
             for (int u = 0; u < U; ++u) {
                 const int idx = base + u * 256;
-                if (idx < total) ddi_sm[(idx & 15) * DDI_A256_WS + ddi_pad16(idx >> 4)] = make_double2(p0[u].x + p1[u].x, p0[u].y + p1[u].y);
+                ddi_sm[(idx & 15) * DDI_A256_WS + ddi_pad16(idx >> 4)] = make_double2(p0[u].x + p1[u].x, p0[u].y + p1[u].y);
             }
         }
+        if (threadIdx.x < DDI_A256_ROWS) ddi_sm[threadIdx.x * DDI_A256_WS + ddi_pad16(M)] = make_double2(q0.x + q1.x, q0.y + q1.y);
     }
     __syncthreads();
 #pragma unroll
@@ -1188,6 +1194,8 @@ __global__ void ddi_mirror_check_kernel(const double *__restrict__ Kre, int PZ, 
     } while (0)
 
 }  // namespace
+
+bool spin::ddi_graph_ok(const spin_system *s) { return s->ddi && s->ddi->fused_b; }
 
 const char *spin::ddi_path_name(const spin_system *s) {
     const DdiState *d = s->ddi;

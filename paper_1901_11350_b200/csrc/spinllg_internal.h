@@ -157,6 +157,7 @@ struct spin_system {
     int opt_graph, opt_store_A, opt_jit, opt_ddi_slab, opt_ddi_mirror, opt_pdl, opt_cache_noise, opt_coop, opt_march;
     cudaGraphExec_t graph_exec[2];   // one captured graph per ping-pong parity
     int graph_steps;
+    int64_t graph_launches;    // kernel launches of one replay of the captured graph (counted while capturing)
     int64_t n_launch, n_fft;
     int profile_on;
     double prof_ms[4];             // predictor, corrector, dipolar evaluation (whole), dipolar contraction kernel alone
@@ -180,6 +181,7 @@ int fail(int code, const char *fmt, ...);
 int ddi_prepare(spin_system *s);                                   // (re)build tensor spectra and FFT plans
 int ddi_field(spin_system *s, const double *d_n, double *d_f);     // d_f (SoA, meV) = dipolar force of d_n
 void ddi_release(spin_system *s);
+bool ddi_graph_ok(const spin_system *s);                              // the evaluation is kernels of this library only (no cuFFT call)
 const char *ddi_path_name(const spin_system *s);                      // "off", "3d", "slab", "slab+mirror"
 
 // spin_jit.cu
