@@ -52,6 +52,16 @@ def ddi_contract_bytes(w):
     return s2 * (2 * 16 * 3 * nz + 6 * 8 * (pz // 2 + 1))
 
 
+def ddi_fused_bytes(w, mirror=True):
+    """Algorithmic bytes of one launch of the fused b-pass kernel: the a-pass spectra [ka][slab][ib] are read once
+    (16 B per element), the real 6-component tensor is read at NZ + 1 (mirror symmetric) or 2 NZ planes for every in-plane wave vector,
+    and the two partial results (one per parity of kb) are written."""
+    na, nb, nz = w.n_cells
+    s1 = na + 1                                   # wave numbers along a of the half spectrum: P0 / 2 + 1
+    planes = nz + 1 if mirror else 2 * nz
+    return s1 * nb * (16 * 3 * nz + 2 * 16 * 3 * nz) + s1 * 2 * nb * 6 * 8 * planes
+
+
 def measured_peaks():
     path = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(path):
@@ -214,11 +224,19 @@ def measure_workload(P, torch, w, stream, steps, warmup, min_seconds, barrier=No
     roof = {"bound": "hbm", "peak": peak, "unit": "GB/s", "peak_source": peak_src, "profiled_ms": per_iter,
             "step_algorithmic_bytes": step_bytes, "step_effective_gbs": step_bytes / (ms_iter * 1e-3) / 1e9}
     if dinfo.startswith("slab") and per_iter["ddi_contract"] > 0:
-        # dipolar workloads: the evaluations are most of the step and the contraction is their longest kernel (two launches per iteration)
-        kernel, nbytes = "ddi_slab_contract_kernel", ddi_contract_bytes(w)
-        share = per_iter["ddi_contract"] / tot
-        launch_ms = ms_iter * share / 2
-        roof["note"] = "dominant kernel of the dipolar evaluation (cuFFT's b-passes are library kernels); two launches per Depondt iteration"
+        # dipolar workloads: the evaluations are most of the step; their longest kernel is the fused b-pass (transforms along b and c, the
+        # contraction and their inverses) or, without it, the contraction kernel; two launches per Depondt iteration
+        if "fused-b" in dinfo:
+            kernel, nbytes = "ddi_bfused_kernel", ddi_fused_bytes(w, "mirror" in dinfo)
+            roof["note"] = ("dominant kernel of the dipolar evaluation (fused b-pass + c-pass + contraction); two launches per Depondt "
+                            "iteration; fp64 issue and load latency co-limit it (profiles/r2_README.md)")
+        else:
+            kernel, nbytes = "ddi_slab_contract_kernel", ddi_contract_bytes(w)
+            roof["note"] = "dominant kernel of the dipolar evaluation (cuFFT's b-passes are library kernels); two launches per Depondt iteration"
+        # the kernel's own duration: CUDA events around it alone on the library's stream (profile mode; it runs between two host
+        # synchronisations there, so nothing overlaps it); its share of the timed step follows from that
+        launch_ms = per_iter["ddi_contract"] / 2
+        share = min(1.0, 2 * launch_ms / ms_iter)
     elif "march" in kinfo:
         # the whole Depondt step is ONE kernel (n^p never leaves the SM): one launch = one iteration.  The roofline figure stays the method's
         # 120 B per spin-update (read n, write n^p; read n^p, read n, write n); the kernel's own DRAM traffic (`traffic`, about
