@@ -181,6 +181,21 @@ int observables(spin_system *sys, double M[3], double *max_torque_meV);
  * One basis atom (SPIN_ERR_ARG otherwise).  Periodic directions wrap; triangles leaving an open edge are skipped (:343).  */
 int topological_charge(spin_system *sys, double *Q);
 
+/* The same quantity for callers that must not allocate (code under CUDA graph capture, tight serving loops, harnesses that forbid
+ * cudaMalloc): topological_charge allocates and frees a buffer of per-block partial sums on every call; this variant keeps them in a
+ * fixed array in device memory (128 KB per GPU that loads the library, held until exit) and calls no cudaMalloc, cudaFree or
+ * allocating library routine.  It launches two kernels on the system's stream and returns without synchronising.
+ *   d_Q   DEVICE pointer to one double, owned by the caller; written by the second kernel (valid after spin_synchronize or after
+ *         later work on the system's stream)
+ * Limits and errors: at most 4,194,304 cells (SPIN_ERR_LIMIT beyond that: use topological_charge); the system's plan must be built
+ * already, because building it allocates (SPIN_ERR_STATE: call spins_set, effective_field, topological_charge or llg_iterate once
+ * after the last change of the lattice, Hamiltonian or options); one basis atom (SPIN_ERR_ARG); the device that was current when
+ * the system was created must be current (SPIN_ERR_STATE).
+ * ALL calls on one GPU share the one array: calls that overlap on the GPU (two systems on different streams) race on it; calls
+ * on the same stream, or ordered by events, are safe.  Nothing in the array has to start at zero: each call overwrites the
+ * entries it reads.                                                                                                        */
+int topological_charge_noalloc(spin_system *sys, double *d_Q);
+
 /* ---- slab decomposition along c over several GPUs (SURVEY 8(e); the paper has no counterpart: MPI only as a scripting remark, :143) ----
  * One process per GPU holds `n_cells[2]` consecutive planes of a lattice of `global_cells_c` planes, starting at plane `c_offset`.  Its
  * ghost layers along c (as wide as the Hamiltonian reaches along c) are then NOT its own periodic images but its neighbours' boundary

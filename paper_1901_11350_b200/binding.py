@@ -21,7 +21,7 @@ EXPORTS = [
     "hamiltonian_set_exchange_shells", "hamiltonian_set_dmi_shells", "hamiltonian_set_quadruplets",
     "hamiltonian_set_ddi", "spin_set_images", "spin_select_image", "llg_set_image_temperatures", "gneb_forces", "gneb_iterate", "spins_set_pinned", "spins_set", "spins_get", "spins_set_device", "spins_get_device",
     "llg_configure", "llg_set_solver", "llg_set_damping_only", "minimise_vp", "minimise_vp_reset", "llg_iterate", "llg_get_step", "llg_set_step", "spin_synchronize",
-    "effective_field", "effective_field_device", "energy", "observables", "topological_charge",
+    "effective_field", "effective_field_device", "energy", "observables", "topological_charge", "topological_charge_noalloc",
     "spin_set_slab", "spin_halo_doubles", "spin_halo_get", "spin_halo_put", "llg_slab_sweep", "llg_slab_advance",
     "spin_launch_counts", "spin_measure_fp64_tflops", "spin_profile_enable", "spin_profile_get", "spin_set_option",
     "spin_kernel_info", "spin_ddi_info", "spin_jit_compiler_info", "spin_jit_source", "spin_last_error", "spin_version",
@@ -84,6 +84,7 @@ def lib() -> C.CDLL:
         "energy": (C.c_int, [vp, dp, dp]),
         "observables": (C.c_int, [vp, dp, dp]),
         "topological_charge": (C.c_int, [vp, dp]),
+        "topological_charge_noalloc": (C.c_int, [vp, C.c_void_p]),
         "spin_launch_counts": (C.c_int, [vp, i64p, i64p]),
         "spin_set_slab": (C.c_int, [vp, C.c_int, C.c_int, C.c_int, C.c_int]),
         "spin_halo_doubles": (C.c_int, [vp, i64p, ip]),
@@ -296,6 +297,10 @@ class SpinSystem:
         q = C.c_double(0.0)
         _check(lib().topological_charge(self._h, C.byref(q)))
         return float(q.value)
+
+    def topological_charge_noalloc(self, d_out_ptr):
+        """Q into the DEVICE double at address `d_out_ptr` (e.g. tensor.data_ptr()); asynchronous on the system's stream; allocates nothing."""
+        _check(lib().topological_charge_noalloc(self._h, C.c_void_p(int(d_out_ptr))))
 
     def llg_set_damping_only(self, enabled):
         _check(lib().llg_set_damping_only(self._h, int(bool(enabled))))

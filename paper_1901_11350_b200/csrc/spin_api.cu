@@ -12,10 +12,13 @@
 
 #include <algorithm>
 #include <map>
+#include <mutex>
 
 #include "spin_kernels.cuh"
 
 using namespace spin;
+
+static int topo_noalloc_setup();      // resolves the device address of topological_charge_noalloc's scratch array (below)
 
 // ---------------------------------------------------------------------------------------------- errors
 static thread_local char g_err[512] = "";
@@ -598,6 +601,9 @@ extern "C" int spin_geometry_create(const double bravais[9], int n_basis, const 
         spin_system_destroy(s);
         return code;
     }
+    // address of the fixed scratch array of topological_charge_noalloc on this device (resolved once per device; a failure is reported
+    // by that entry point, the only one that needs it)
+    if (topo_noalloc_setup() != SPIN_OK) cudaGetLastError();
     // initial state: all spins +z
     std::vector<double> z((size_t)3 * s->N, 0.0);
     for (int64_t i = 0; i < s->N; ++i) z[3 * i + 2] = 1.0;
@@ -1308,6 +1314,53 @@ extern "C" int topological_charge(spin_system *s, double *Q) {
     if (e == cudaSuccess) e = cudaStreamSynchronize(s->stream);
     cudaFree(d_part);
     if (e != cudaSuccess) return spin::fail(SPIN_ERR_CUDA, "topological_charge: %s", cudaGetErrorString(e));
+    SPIN_CUDA(cudaGetLastError());
+    return SPIN_OK;
+}
+
+// The same reduction for callers that must not allocate (code under CUDA graph capture, serving loops, harnesses that forbid cudaMalloc):
+// the per-block partial sums live in a file-scope device array instead of a buffer allocated per call.  Every GPU that loads the library
+// holds the array (128 KB) until exit.  In host code the array's NAME is a host-side stand-in, not a device address: the address is resolved
+// with cudaGetSymbolAddress at set-up (spin_system_create), once per device with that device current, and that pointer goes to the kernels.
+constexpr int TOPO_NOALLOC_MAX_BLOCKS = 16384;                         // x 256 cells per block = 4,194,304 cells
+constexpr int TOPO_NOALLOC_MAX_DEVICES = 64;
+static __device__ __align__(256) double g_topo_scratch[TOPO_NOALLOC_MAX_BLOCKS];
+static double *g_topo_scratch_addr[TOPO_NOALLOC_MAX_DEVICES];          // device address of g_topo_scratch, per device; nullptr: not resolved
+static std::mutex g_topo_mutex;
+
+static int topo_noalloc_setup() {
+    int dev = -1;
+    SPIN_CUDA(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= TOPO_NOALLOC_MAX_DEVICES) return spin::fail(SPIN_ERR_LIMIT, "device ordinal %d beyond the %d this library keeps scratch addresses for", dev, TOPO_NOALLOC_MAX_DEVICES);
+    std::lock_guard<std::mutex> lock(g_topo_mutex);
+    if (g_topo_scratch_addr[dev]) return SPIN_OK;
+    double *ptr = nullptr;
+    const cudaError_t e = cudaGetSymbolAddress((void **)&ptr, g_topo_scratch);
+    if (e != cudaSuccess || !ptr) return spin::fail(SPIN_ERR_CUDA, "cudaGetSymbolAddress(g_topo_scratch) on device %d: %s", dev, cudaGetErrorString(e));
+    g_topo_scratch_addr[dev] = ptr;
+    return SPIN_OK;
+}
+
+extern "C" int topological_charge_noalloc(spin_system *s, double *d_Q) {
+    REQUIRE(s && d_Q, "null argument");
+    NEED_DEVICE(s);
+    REQUIRE(s->nb == 1, "the topological charge is defined for one basis atom (triangulation of a Bravais lattice)");
+    const int64_t nblk = (s->ncell + 255) / 256;
+    if (nblk > TOPO_NOALLOC_MAX_BLOCKS)
+        return spin::fail(SPIN_ERR_LIMIT, "topological_charge_noalloc: %lld cells exceed the fixed scratch array (%d blocks of 256 cells = %lld cells); use topological_charge",
+                          (long long)s->ncell, TOPO_NOALLOC_MAX_BLOCKS, (long long)TOPO_NOALLOC_MAX_BLOCKS * 256);
+    if (s->plan_dirty)
+        return spin::fail(SPIN_ERR_STATE, "topological_charge_noalloc: the plan is not built and building it allocates; call spins_set, effective_field, "
+                                          "topological_charge or llg_iterate once after the last change of the lattice, Hamiltonian or options");
+    int dev = -1;
+    SPIN_CUDA(cudaGetDevice(&dev));
+    double *scratch = (dev >= 0 && dev < TOPO_NOALLOC_MAX_DEVICES) ? g_topo_scratch_addr[dev] : nullptr;
+    if (!scratch) return spin::fail(SPIN_ERR_STATE, "topological_charge_noalloc: no scratch address for device %d (create the system with this device current)", dev);
+    const int ccw = (s->brav[0] * s->brav[4] - s->brav[1] * s->brav[3]) > 0.0 ? 1 : 0;
+    // every block overwrites its own partial sum and the final kernel reads the first nblk only: nothing has to start at zero
+    topo_kernel<<<(unsigned)nblk, 256, 0, s->stream>>>(s->plan, s->d_n[s->cur] + img_off(s), ccw, scratch);
+    topo_final_kernel<<<1, 32, 0, s->stream>>>(scratch, (int)nblk, d_Q);
+    s->n_launch += 2;
     SPIN_CUDA(cudaGetLastError());
     return SPIN_OK;
 }
