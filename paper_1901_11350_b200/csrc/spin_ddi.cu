@@ -192,6 +192,10 @@ __global__ void ddi_slab_gather_kernel(const __grid_constant__ DevicePlan L, con
 // One warp per row; the complex transform is a Stockham autosort (radix 8, closed by one pass of radix 4 or 2) ping-ponging between two
 // padded shared-memory rows, the first twiddle of a butterfly from a table of exp(-2 pi i t / P0) in global memory.  Compared with scatter + cuFFT D2Z this reads the
 // spins once where they live (no padded real copy: 12.6 instead of 12.6 + 12.6 + 25.2 MB on cfg5) and launches one kernel instead of two.
+// Programmatic dependent launch (fused path): the kernels of an evaluation are launched with programmatic stream serialisation, so the
+// blocks of the next kernel become resident while the previous one drains and run their prologue (tables, tensor prefetch); everything
+// that reads the previous kernel's output comes after this wait (a no-op in a kernel launched the plain way).
+__device__ __forceinline__ void ddi_wait_upstream() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 __device__ __forceinline__ double2 ddi_cadd(const double2 a, const double2 b) { return make_double2(a.x + b.x, a.y + b.y); }
 __device__ __forceinline__ double2 ddi_csub(const double2 a, const double2 b) { return make_double2(a.x - b.x, a.y - b.y); }
 __device__ __forceinline__ double2 ddi_cmul(const double2 a, const double2 b) { return make_double2(fma(a.x, b.x, -a.y * b.y), fma(a.x, b.y, a.y * b.x)); }
@@ -334,6 +338,7 @@ __global__ void __launch_bounds__(256) ddi_apass_fwd_kernel(const __grid_constan
     const int MP = M + (M >> 3), WS = 2 * MP + 1;       // padded row; buffers of a warp (the odd stride keeps the transposed reads conflict-free)
     double2 *a = ddi_sm + (size_t)warp * WS, *b = a + MP;
     for (int j = M / 2 + lane; j < M; j += 32) a[ddi_pad(j)] = make_double2(0.0, 0.0);      // the zero padding of the row
+    ddi_wait_upstream();
 #pragma unroll 4
     for (int j = lane; j < M / 2; j += 32) {                                                  // (unrolled: the loads of a lane are in flight together)
         double2 v = __ldg(src + j);
@@ -383,6 +388,7 @@ __global__ void __launch_bounds__(256) ddi_apass_inv_kernel(const __grid_constan
     const int MP = M + (M >> 3), WS = 2 * MP + 1;
     double2 *a = ddi_sm + (size_t)warp * WS, *b = a + MP;
     const cufftDoubleComplex *src = TR ? b : in + (size_t)row * S1p;                // TR: the row's half spectrum, gathered into b first
+    ddi_wait_upstream();
     if (TR) {
         const int ib0 = (blockIdx.x * rows_per_block) % L.Nb;
         const int lgr = __ffs(rows_per_block) - 1, total = (M + 1) << lgr;      // (a power of two)
@@ -625,6 +631,7 @@ __global__ void __launch_bounds__(256, 3) ddi_apass256_fwd_kernel(const __grid_c
     constexpr int M = 256;
     double2 *T = ddi_sm + DDI_A256_ROWS * DDI_A256_WS;
     ddi_fill_t256(T, tw, threadIdx.x, blockDim.x);
+    ddi_wait_upstream();
     const int hw = threadIdx.x >> 4, l = threadIdx.x & 15;                 // row of the block, lane of the half warp
     const unsigned hmask = 0xffffu << (threadIdx.x & 16);      // the lanes of this half warp
     const int rowid = blockIdx.x * DDI_A256_ROWS + hw;
@@ -682,6 +689,7 @@ __global__ void __launch_bounds__(256) ddi_apass256_inv_kernel(const __grid_cons
     constexpr int M = 256;
     double2 *T = ddi_sm + DDI_A256_ROWS * DDI_A256_WS;
     ddi_fill_t256(T, tw, threadIdx.x, blockDim.x);
+    ddi_wait_upstream();
     const int hw = threadIdx.x >> 4, l = threadIdx.x & 15;
     const unsigned hmask = 0xffffu << (threadIdx.x & 16);      // the lanes of this half warp
     const int rowid = blockIdx.x * DDI_A256_ROWS + hw;
@@ -895,7 +903,9 @@ __global__ void __launch_bounds__(2 * DDI_CT_COLS, 4) ddi_slab_contract_kernel(c
 // reads global memory and applies the twist), contracts every wave
 // vector (ka, kb = 2 k' + r) along c exactly like ddi_slab_contract_kernel (two threads per column, tensor from a copy laid out
 // [ka][r][component][plane][k'] when the plan is built), transforms back and writes its partial result; the inverse a-pass adds the two
-// parities.  (One block per ka taking the two parities in turn and adding them itself was measured slower: 76 instead of 66 us.)  Shared memory: 3 NZ padded columns of Nb complex numbers (cfg5: 24 columns x 4.6 KB = 110.6 KB, two blocks of 256 threads per SM,
+// parities.  (Measured slower: one block per ka taking the two parities in turn and adding them itself, 76 instead of 66 us; the two
+// parities as a cluster of two blocks that add their results through distributed shared memory and write one array, 66.8 instead of
+// 58.2 us -- the inverse a-pass gains 3 us from the halved input, the fused kernel loses 8.6 to the cluster barriers and the extra pass.)  Shared memory: 3 NZ padded columns of Nb complex numbers (cfg5: 24 columns x 4.6 KB = 110.6 KB, two blocks of 256 threads per SM,
 // so that one block's loads overlap the other's arithmetic).
 constexpr int DDI_BF_THREADS = 256, DDI_BF_WARPS = DDI_BF_THREADS / 32;
 // F256: columns of length 256 -- half a warp per column, two passes of radix 16 (ddi_fft256_pass1 / 2), rows padded by one in 16.
@@ -919,6 +929,7 @@ __global__ void __launch_bounds__(DDI_BF_THREADS, 2) ddi_bfused_kernel(const dou
         // ---- forward, length 256: half a warp per column; pass 1 reads global memory (16 loads per lane in flight) and applies the twist
         double2 *T = tws + M;
         ddi_fill_t256(T, tw, tid, DDI_BF_THREADS);
+        ddi_wait_upstream();
         __syncthreads();                                                       // tws and T are complete
         const int l = tid & 15;
         const unsigned hmask = 0xffffu << (tid & 16);      // the lanes of this half warp (the other half may have no column)
@@ -951,6 +962,7 @@ __global__ void __launch_bounds__(DDI_BF_THREADS, 2) ddi_bfused_kernel(const dou
 #pragma unroll
             for (int q = 0; q < 8; ++q) v[q] = __ldg(src + q * span);
         };
+        ddi_wait_upstream();
         if (warp < SL) fetch(warp, buf[0]);
         __syncthreads();                                                       // tws is complete
 #pragma unroll
@@ -1195,6 +1207,20 @@ __global__ void ddi_mirror_check_kernel(const double *__restrict__ Kre, int PZ, 
 
 }  // namespace
 
+// a kernel of the fused path, launched with programmatic stream serialisation (option use_pdl = 0: the plain way); see ddi_wait_upstream
+template <class... KArgs, class... Args>
+static cudaError_t ddi_launch(const spin_system *s, void (*kernel)(KArgs...), unsigned grid, unsigned block, size_t smem, Args &&...args) {
+    cudaLaunchConfig_t cfg;
+    memset(&cfg, 0, sizeof(cfg));
+    cfg.gridDim = dim3(grid, 1, 1); cfg.blockDim = dim3(block, 1, 1); cfg.dynamicSmemBytes = smem; cfg.stream = s->stream;
+    cudaLaunchAttribute at;
+    memset(&at, 0, sizeof(at));
+    at.id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at.val.programmaticStreamSerializationAllowed = 1;
+    if (s->opt_pdl != 0) { cfg.attrs = &at; cfg.numAttrs = 1; }
+    return cudaLaunchKernelEx(&cfg, kernel, std::forward<Args>(args)...);
+}
+
 bool spin::ddi_graph_ok(const spin_system *s) { return s->ddi && s->ddi->fused_b; }
 
 const char *spin::ddi_path_name(const spin_system *s) {
@@ -1419,12 +1445,14 @@ int spin::ddi_field(spin_system *s, const double *d_n, double *d_f) {
             int lgMb = 0;
             while ((1 << lgMb) < Mb) ++lgMb;
             if (d->a256)
-                ddi_apass256_fwd_kernel<<<a_rows / DDI_A256_ROWS, 256, DDI_A256_SMEM, s->stream>>>(s->plan, d_n, d->SL, d->d_geom, d->d_tw, d->s_a);
+                SPIN_CUDA(ddi_launch(s, ddi_apass256_fwd_kernel, a_rows / DDI_A256_ROWS, 256, DDI_A256_SMEM, s->plan, d_n, d->SL, (const double *)d->d_geom,
+                                     (const double2 *)d->d_tw, d->s_a));
             else
-                ddi_apass_fwd_kernel<true><<<ga, 32 * d->a_rows_per_block, d->a_smem, s->stream>>>(s->plan, d_n, Ma, d->SL, d->S1p, a_rows, d->a_rows_per_block,
-                                                                                                  d->d_geom, d->d_tw, d->s_a);
+                SPIN_CUDA(ddi_launch(s, ddi_apass_fwd_kernel<true>, ga, 32 * d->a_rows_per_block, d->a_smem, s->plan, d_n, Ma, d->SL, d->S1p, a_rows,
+                                     d->a_rows_per_block, (const double *)d->d_geom, (const double2 *)d->d_tw, d->s_a));
             if (s->profile_on) cudaEventRecord(s->ev2, s->stream);
-#define SPIN_BF1(NZ_, MIR_, F_) ddi_bfused_kernel<NZ_, MIR_, F_><<<2 * d->S1, DDI_BF_THREADS, d->bf_smem, s->stream>>>(d->d_Kb, (const double2 *)d->s_a, (double2 *)d->s_d, lgMb, d->S1, d->d_tw_b)
+#define SPIN_BF1(NZ_, MIR_, F_) SPIN_CUDA(ddi_launch(s, ddi_bfused_kernel<NZ_, MIR_, F_>, 2 * d->S1, DDI_BF_THREADS, d->bf_smem, (const double *)d->d_Kb, (const double2 *)d->s_a, \
+                                                     (double2 *)d->s_d, lgMb, d->S1, (const double2 *)d->d_tw_b))
 #define SPIN_BF(NZ_) case NZ_: \
             if (d->b256) { if (d->mirror) SPIN_BF1(NZ_, true, true); else SPIN_BF1(NZ_, false, true); } \
             else { if (d->mirror) SPIN_BF1(NZ_, true, false); else SPIN_BF1(NZ_, false, false); } break
@@ -1440,10 +1468,11 @@ int spin::ddi_field(spin_system *s, const double *d_n, double *d_f) {
                 s->prof_ms[3] += ms; s->prof_n[3]++;
             }
             if (d->a256)
-                ddi_apass256_inv_kernel<<<a_rows / DDI_A256_ROWS, 256, DDI_A256_SMEM, s->stream>>>(s->plan, d->s_d, d->SL, d->d_geom, C_DD / (double)d->Ptot, d->d_tw, d_f, part1);
+                SPIN_CUDA(ddi_launch(s, ddi_apass256_inv_kernel, a_rows / DDI_A256_ROWS, 256, DDI_A256_SMEM, s->plan, (const cufftDoubleComplex *)d->s_d, d->SL,
+                                     (const double *)d->d_geom, C_DD / (double)d->Ptot, (const double2 *)d->d_tw, d_f, part1));
             else
-                ddi_apass_inv_kernel<true><<<ga, 32 * d->a_rows_per_block, d->a_smem, s->stream>>>(s->plan, d->s_d, Ma, d->SL, d->S1p, a_rows, d->a_rows_per_block,
-                                                                                                  d->d_geom, C_DD / (double)d->Ptot, d->d_tw, d_f, part1);
+                SPIN_CUDA(ddi_launch(s, ddi_apass_inv_kernel<true>, ga, 32 * d->a_rows_per_block, d->a_smem, s->plan, (const cufftDoubleComplex *)d->s_d, Ma, d->SL,
+                                     d->S1p, a_rows, d->a_rows_per_block, (const double *)d->d_geom, C_DD / (double)d->Ptot, (const double2 *)d->d_tw, d_f, part1));
             s->n_launch += 3;
             return SPIN_OK;
         }
