@@ -229,7 +229,8 @@ int llg_slab_advance(spin_system *sys);
  *                    thread-block cluster with its hardware barrier between the sweeps (up to 16 bricks), else as a cooperative launch
  *                    with a grid barrier; 2 forces the path for any size, 3 forces the grid barrier, 0 switches it off
  *   use_pdl     (-1) programmatic dependent launch of the brick sweeps (griddepcontrol.wait inside the kernel): -1 automatic, 0 off,
- *                    1 dependents released at entry, 2 at the end of each block
+ *                    1 dependents released at entry, 2 at the end of each block; any value but 0 also launches the kernels of the
+ *                    fused dipolar path that way (their prologue overlaps the previous kernel's tail)
  *   store_A     (0)  1: the predictor stores the rotation field A(n) and the corrector reads it instead of recomputing it
  *   cache_noise (1)  the predictor keeps the thermal field of the step (24 B/spin) for the corrector instead of generating it twice
  *   ddi_slab    (1)  thin films (up to 8 planes; 4 with several basis atoms) take the dipolar slab path: hand-written transforms along a and, for one
