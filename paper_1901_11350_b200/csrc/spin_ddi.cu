@@ -909,10 +909,12 @@ __global__ void __launch_bounds__(2 * DDI_CT_COLS, 4) ddi_slab_contract_kernel(c
 // so that one block's loads overlap the other's arithmetic).
 constexpr int DDI_BF_THREADS = 256, DDI_BF_WARPS = DDI_BF_THREADS / 32;
 // F256: columns of length 256 -- half a warp per column, two passes of radix 16 (ddi_fft256_pass1 / 2), rows padded by one in 16.
-template <int NZ, bool MIRROR, bool F256>
+// PAD = false: a single plane that is not padded along c (a monolayer, NZ = PZ = 1): no transform along c, one thread per wave vector.
+template <int NZ, bool MIRROR, bool F256, bool PAD = true>
 __global__ void __launch_bounds__(DDI_BF_THREADS, 2) ddi_bfused_kernel(const double *__restrict__ Kb, const double2 *__restrict__ Tin, double2 *__restrict__ Tout,
                                                                         const int lgM_, const int S1, const double2 *__restrict__ tw) {
-    constexpr int SL = 3 * NZ, NPL = MIRROR ? NZ + 1 : 2 * NZ, PADSH = F256 ? 4 : 3;
+    constexpr int SL = 3 * NZ, NPL = !PAD ? 1 : (MIRROR ? NZ + 1 : 2 * NZ), PADSH = F256 ? 4 : 3;
+    static_assert(PAD || (NZ == 1 && !MIRROR), "only a single plane goes unpadded");
     extern __shared__ double2 ddi_sm[];
     const int lgM = F256 ? 8 : lgM_;
     const int M = 1 << lgM, LP = M + (M >> PADSH);
@@ -989,6 +991,18 @@ __global__ void __launch_bounds__(DDI_BF_THREADS, 2) ddi_bfused_kernel(const dou
     // ---- contraction along c: thread (k', e) of a round takes the wave numbers kz = 2 j + e of the wave vector (ka, kb = 2 k' + r)
     constexpr int half = DDI_BF_THREADS / 2;
     const int e = tid / half;
+    if constexpr (!PAD) {
+        for (int kp = tid; kp < M; kp += DDI_BF_THREADS) {
+            double2 *col = ddi_sm + pad(kp);
+            double k[6];
+#pragma unroll
+            for (int m = 0; m < 6; ++m) k[m] = __ldg(Kme + ((size_t)m << lgM) + kp);
+            const double2 x = col[0], y = col[LP], z = col[2 * LP];
+            col[0] = make_double2(k[0] * x.x + k[1] * y.x + k[2] * z.x, k[0] * x.y + k[1] * y.y + k[2] * z.y);
+            col[LP] = make_double2(k[1] * x.x + k[3] * y.x + k[4] * z.x, k[1] * x.y + k[3] * y.y + k[4] * z.y);
+            col[2 * LP] = make_double2(k[2] * x.x + k[4] * y.x + k[5] * z.x, k[2] * x.y + k[4] * y.y + k[5] * z.y);
+        }
+    } else
     for (int k0 = 0; k0 < M; k0 += half) {
         const int kp = k0 + (tid - e * half);
         const bool live = kp < M;
@@ -999,7 +1013,7 @@ __global__ void __launch_bounds__(DDI_BF_THREADS, 2) ddi_bfused_kernel(const dou
             for (int c = 0; c < 3; ++c)
 #pragma unroll
                 for (int z = 0; z < NZ; ++z) { const double2 v = col[(size_t)(c * NZ + z) * LP]; xr[c][z] = v.x; xi[c][z] = v.y; }
-            ddi_column_half<NZ, true, MIRROR>(xr, xi, e, [&](const int kz, double (&k)[6]) {
+            ddi_column_half<NZ, PAD, MIRROR>(xr, xi, e, [&](const int kz, double (&k)[6]) {
 #pragma unroll
                 for (int m = 0; m < 6; ++m) k[m] = __ldg(Kme + ((size_t)(m * NPL + kz) << lgM) + kp);
             });
@@ -1276,7 +1290,7 @@ int spin::ddi_prepare(spin_system *s) {
     const int Nb_ = s->nc[1];
     d->bf_smem = ((size_t)(3 * d->NZ) * (size_t)(Nb_ + Nb_ / 8) + (size_t)Nb_) * sizeof(double2);      // columns + twiddles
     if (Nb_ == 256) d->bf_smem = ((size_t)(3 * d->NZ) * DDI_LP256 + 256 + 240) * sizeof(double2);         // columns (padded by 1 in 16) + twiddles + pass-1 table
-    d->fused_b = d->own_a && s->opt_ddi_slab == 1 && nb == 1 && Nb_ >= 8 && Nb_ <= 256 && (Nb_ & (Nb_ - 1)) == 0 && d->PZ == 2 * d->NZ && d->bf_smem <= 220 * 1024;
+    d->fused_b = d->own_a && s->opt_ddi_slab == 1 && nb == 1 && Nb_ >= 8 && Nb_ <= 256 && (Nb_ & (Nb_ - 1)) == 0 && (d->PZ == 2 * d->NZ || d->PZ == 1) && d->bf_smem <= 220 * 1024;
     if (want_slab) {
         const size_t nr = (size_t)s->nc[1] * d->SL * d->P[0], nc_ = (size_t)d->P[1] * d->SL * d->S1p;
         if (!d->own_a) {
@@ -1416,7 +1430,10 @@ int spin::ddi_prepare(spin_system *s) {
             SPIN_CUDA(cudaFuncSetAttribute(ddi_bfused_kernel<NZ_, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)d->bf_smem)); \
             SPIN_CUDA(cudaFuncSetAttribute(ddi_bfused_kernel<NZ_, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)d->bf_smem)); \
             SPIN_CUDA(cudaFuncSetAttribute(ddi_bfused_kernel<NZ_, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)d->bf_smem)); break
-            switch (d->NZ) {
+            if (d->PZ == 1) {      // a monolayer, not padded along c
+                SPIN_CUDA(cudaFuncSetAttribute(ddi_bfused_kernel<1, false, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)d->bf_smem));
+                SPIN_CUDA(cudaFuncSetAttribute(ddi_bfused_kernel<1, false, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)d->bf_smem));
+            } else switch (d->NZ) {
                 SPIN_BF_ATTR(1); SPIN_BF_ATTR(2); SPIN_BF_ATTR(3); SPIN_BF_ATTR(4); SPIN_BF_ATTR(5); SPIN_BF_ATTR(6); SPIN_BF_ATTR(7); SPIN_BF_ATTR(8);
                 default: return spin::fail(SPIN_ERR_STATE, "dipolar slab path: %d planes not supported", d->NZ);
             }
@@ -1451,12 +1468,13 @@ int spin::ddi_field(spin_system *s, const double *d_n, double *d_f) {
                 SPIN_CUDA(ddi_launch(s, ddi_apass_fwd_kernel<true>, ga, 32 * d->a_rows_per_block, d->a_smem, s->plan, d_n, Ma, d->SL, d->S1p, a_rows,
                                      d->a_rows_per_block, (const double *)d->d_geom, (const double2 *)d->d_tw, d->s_a));
             if (s->profile_on) cudaEventRecord(s->ev2, s->stream);
-#define SPIN_BF1(NZ_, MIR_, F_) SPIN_CUDA(ddi_launch(s, ddi_bfused_kernel<NZ_, MIR_, F_>, 2 * d->S1, DDI_BF_THREADS, d->bf_smem, (const double *)d->d_Kb, (const double2 *)d->s_a, \
+#define SPIN_BF1(NZ_, MIR_, ...) SPIN_CUDA(ddi_launch(s, ddi_bfused_kernel<NZ_, MIR_, __VA_ARGS__>, 2 * d->S1, DDI_BF_THREADS, d->bf_smem, (const double *)d->d_Kb, (const double2 *)d->s_a, \
                                                      (double2 *)d->s_d, lgMb, d->S1, (const double2 *)d->d_tw_b))
 #define SPIN_BF(NZ_) case NZ_: \
             if (d->b256) { if (d->mirror) SPIN_BF1(NZ_, true, true); else SPIN_BF1(NZ_, false, true); } \
             else { if (d->mirror) SPIN_BF1(NZ_, true, false); else SPIN_BF1(NZ_, false, false); } break
-            switch (d->NZ) {
+            if (d->PZ == 1) { if (d->b256) SPIN_BF1(1, false, true, false); else SPIN_BF1(1, false, false, false); }
+            else switch (d->NZ) {
                 SPIN_BF(1); SPIN_BF(2); SPIN_BF(3); SPIN_BF(4); SPIN_BF(5); SPIN_BF(6); SPIN_BF(7); SPIN_BF(8);
                 default: return spin::fail(SPIN_ERR_STATE, "dipolar slab path: %d planes not supported", d->NZ);
             }
