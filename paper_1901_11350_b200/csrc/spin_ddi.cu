@@ -772,29 +772,15 @@ __global__ void __launch_bounds__(256) ddi_apass256_inv_kernel(const __grid_cons
 template <int NZ, bool PAD, bool MIRROR, class KLoad>
 __device__ __forceinline__ void ddi_column_half(double (&xr)[3][NZ], double (&xi)[3][NZ], const int e, KLoad &&kload) {
     constexpr int PZ = PAD ? 2 * NZ : NZ;
-    if constexpr (PAD) {
-        if (e) {
-#pragma unroll
-            for (int c = 0; c < 3; ++c)
-#pragma unroll
-                for (int z = 1; z < NZ; ++z) {
-                    if constexpr (ddi_pow2(NZ)) ddi_rot16(z * (16 / PZ), xr[c][z], xi[c][z]);
-                    else {
-                        const double wr = DDI_TWR[PZ][z], wi = DDI_TWI[PZ][z], r = xr[c][z], i = xi[c][z];
-                        xr[c][z] = fma(r, wr, -i * wi); xi[c][z] = fma(r, wi, i * wr);
-                    }
-                }
-        }
-#pragma unroll
-        for (int c = 0; c < 3; ++c) ddi_dft_fwd<NZ>(xr[c], xi[c]);
-    }
-    // contraction at the wave numbers of this thread; position p of the transformed column holds kz = 2 ddi_pos(p) + e
+    // contraction at one wave number; position p of the transformed column holds kz = 2 ddi_pos(p) + e
     auto contract = [&](const int p, const double kxx, const double kxy, const double kxz, const double kyy, const double kyz, const double kzz) {
         const double r0 = xr[0][p], r1 = xr[1][p], r2 = xr[2][p], i0 = xi[0][p], i1 = xi[1][p], i2 = xi[2][p];
         xr[0][p] = kxx * r0 + kxy * r1 + kxz * r2; xr[1][p] = kxy * r0 + kyy * r1 + kyz * r2; xr[2][p] = kxz * r0 + kyz * r1 + kzz * r2;
         xi[0][p] = kxx * i0 + kxy * i1 + kxz * i2; xi[1][p] = kxy * i0 + kyy * i1 + kyz * i2; xi[2][p] = kxz * i0 + kyz * i1 + kzz * i2;
     };
-    auto planes = [&](auto ec) {
+    // (the parity is the outermost branch -- uniform per warp in every caller -- so that the loads of the first tensor planes, which
+    // depend on it, can be issued before the transform and overlap it)
+    auto work = [&](auto ec) {
         constexpr int E = decltype(ec)::value;
         // planes this thread reads: kz = 2 j + E, j < NJ (MIRROR: up to PZ / 2 only, the rest are mirror images); the tensor of plane
         // j + AHEAD is loaded before plane j is contracted
@@ -803,6 +789,22 @@ __device__ __forceinline__ void ddi_column_half(double (&xr)[3][NZ], double (&xi
         double k[AHEAD + 1][6];
 #pragma unroll
         for (int j = 0; j < AHEAD && j < NJ; ++j) kload(PAD ? 2 * j + E : 0, k[j]);
+        if constexpr (PAD) {
+            if constexpr (E == 1) {
+#pragma unroll
+                for (int c = 0; c < 3; ++c)
+#pragma unroll
+                    for (int z = 1; z < NZ; ++z) {
+                        if constexpr (ddi_pow2(NZ)) ddi_rot16(z * (16 / PZ), xr[c][z], xi[c][z]);
+                        else {
+                            const double wr = DDI_TWR[PZ][z], wi = DDI_TWI[PZ][z], r = xr[c][z], i = xi[c][z];
+                            xr[c][z] = fma(r, wr, -i * wi); xi[c][z] = fma(r, wi, i * wr);
+                        }
+                    }
+            }
+#pragma unroll
+            for (int c = 0; c < 3; ++c) ddi_dft_fwd<NZ>(xr[c], xi[c]);
+        }
 #pragma unroll
         for (int j = 0; j < NJ; ++j) {
             const int kz = PAD ? 2 * j + E : 0;
@@ -812,24 +814,24 @@ __device__ __forceinline__ void ddi_column_half(double (&xr)[3][NZ], double (&xi
             if (MIRROR && kz > 0 && 2 * kz < PZ)                        // plane PZ - kz: the same values, xz and yz with the opposite sign
                 contract(ddi_pos<NZ>((PZ - kz - E) / 2), kk[0], kk[1], -kk[2], kk[3], -kk[4], kk[5]);
         }
-    };
-    if (e) planes(spin_ddi_int<1>{}); else planes(spin_ddi_int<0>{});
-    if constexpr (PAD) {
+        if constexpr (PAD) {
 #pragma unroll
-        for (int c = 0; c < 3; ++c) ddi_dft_inv<NZ>(xr[c], xi[c]);
-        if (e) {
+            for (int c = 0; c < 3; ++c) ddi_dft_inv<NZ>(xr[c], xi[c]);
+            if constexpr (E == 1) {
 #pragma unroll
-            for (int c = 0; c < 3; ++c)
+                for (int c = 0; c < 3; ++c)
 #pragma unroll
-                for (int z = 1; z < NZ; ++z) {
-                    if constexpr (ddi_pow2(NZ)) ddi_rot16(16 - z * (16 / PZ), xr[c][z], xi[c][z]);
-                    else {
-                        const double wr = DDI_TWR[PZ][z], wi = -DDI_TWI[PZ][z], r = xr[c][z], i = xi[c][z];
-                        xr[c][z] = fma(r, wr, -i * wi); xi[c][z] = fma(r, wi, i * wr);
+                    for (int z = 1; z < NZ; ++z) {
+                        if constexpr (ddi_pow2(NZ)) ddi_rot16(16 - z * (16 / PZ), xr[c][z], xi[c][z]);
+                        else {
+                            const double wr = DDI_TWR[PZ][z], wi = -DDI_TWI[PZ][z], r = xr[c][z], i = xi[c][z];
+                            xr[c][z] = fma(r, wr, -i * wi); xi[c][z] = fma(r, wi, i * wr);
+                        }
                     }
-                }
+            }
         }
-    }
+    };
+    if (e) work(spin_ddi_int<1>{}); else work(spin_ddi_int<0>{});
 }
 
 constexpr int DDI_CT_COLS = 64;      // columns per block: 2 x 64 threads
