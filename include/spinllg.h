@@ -218,6 +218,13 @@ int spin_halo_put(spin_system *sys, int array, int side, const double *src_devic
 int llg_slab_sweep(spin_system *sys, int stage, int part);
 /* after the corrector sweeps: the next configuration becomes current, the step counter (noise stream) advances by one             */
 int llg_slab_advance(spin_system *sys);
+/* The whole Depondt step of a slab in ONE pass (the plane-marching kernel; available when spin_kernel_info reports "jit+march": one basis
+ * atom, Depondt, no pinned spins or per-site moments, slab of at least 32 x 8 x 8 cells): the kernel recomputes the predictor of the
+ * neighbours' boundary planes itself, so a step needs ONE halo exchange of depth 2 x reach (of the new configuration, array 2, before
+ * llg_slab_advance) instead of two of depth reach.  spin_halo_doubles reports the depth in use.  part 0: the whole slab; 1: the first and
+ * last chunk of planes, which hold everything the neighbours need; 2: the chunks in between (launched after the halo copies of part 1
+ * have been started, they run while the halos travel).  SPIN_ERR_STATE if the kernel does not apply to this system (use llg_slab_sweep). */
+int llg_slab_step(spin_system *sys, int part);
 
 /* ---- execution options ------------------------------------------------------------------------------------------------
  * spin_set_option(name, value) changes how the path is executed, never what it computes (every combination is bit-identical; tested).

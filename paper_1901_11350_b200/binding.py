@@ -22,7 +22,7 @@ EXPORTS = [
     "hamiltonian_set_ddi", "spin_set_images", "spin_select_image", "llg_set_image_temperatures", "gneb_forces", "gneb_iterate", "spins_set_pinned", "spins_set", "spins_get", "spins_set_device", "spins_get_device",
     "llg_configure", "llg_set_solver", "llg_set_damping_only", "minimise_vp", "minimise_vp_reset", "llg_iterate", "llg_get_step", "llg_set_step", "spin_synchronize",
     "effective_field", "effective_field_device", "energy", "observables", "topological_charge", "topological_charge_noalloc",
-    "spin_set_slab", "spin_halo_doubles", "spin_halo_get", "spin_halo_put", "llg_slab_sweep", "llg_slab_advance",
+    "spin_set_slab", "spin_halo_doubles", "spin_halo_get", "spin_halo_put", "llg_slab_sweep", "llg_slab_step", "llg_slab_advance",
     "spin_launch_counts", "spin_measure_fp64_tflops", "spin_profile_enable", "spin_profile_get", "spin_set_option",
     "spin_kernel_info", "spin_ddi_info", "spin_jit_compiler_info", "spin_jit_source", "spin_last_error", "spin_version",
 ]
@@ -91,6 +91,7 @@ def lib() -> C.CDLL:
         "spin_halo_get": (C.c_int, [vp, C.c_int, C.c_int, vp, vp]),
         "spin_halo_put": (C.c_int, [vp, C.c_int, C.c_int, vp, vp]),
         "llg_slab_sweep": (C.c_int, [vp, C.c_int, C.c_int]),
+        "llg_slab_step": (C.c_int, [vp, C.c_int]),
         "llg_slab_advance": (C.c_int, [vp]),
         "spin_profile_enable": (C.c_int, [vp, C.c_int]),
         "spin_profile_get": (C.c_int, [vp, C.c_int, dp, i64p]),
@@ -361,6 +362,9 @@ class SpinSystem:
 
     def llg_slab_sweep(self, stage, part=0):
         _check(lib().llg_slab_sweep(self._h, int(stage), int(part)))
+
+    def llg_slab_step(self, part=0):
+        _check(lib().llg_slab_step(self._h, int(part)))
 
     def llg_slab_advance(self):
         _check(lib().llg_slab_advance(self._h))

@@ -164,9 +164,12 @@ int stt_coefficients(const spin_system *s, double cd[3]) {
 
 }  // namespace
 // The one-pass plane-marching Depondt kernel (spin_jit_march.cuh) applies to 3-D lattices of one basis atom advanced by the Depondt solver
-// without dipolar coupling, images or slab decomposition; lattices small enough for the all-steps-in-one-launch path keep that path.
+// without dipolar coupling or images; lattices small enough for the all-steps-in-one-launch path keep that path.  A slab of a decomposed
+// lattice takes it too (llg_slab_step: ONE halo exchange of depth 2 x reach per step instead of two of depth reach) unless it has pinned
+// spins or per-site moments: the kernel recomputes the predictor of the neighbours' boundary planes and would need their flags.
 bool spin::march_eligible(const spin_system *s) {
-    return s->opt_march && s->opt_jit && s->nb == 1 && s->solver == SPIN_SOLVER_DEPONDT && !s->ddi_on && s->n_img == 1 && !s->slab_on && !s->opt_store_A &&
+    if (s->slab_on && (s->d_pin || !s->mu_site.empty())) return false;
+    return s->opt_march && s->opt_jit && s->nb == 1 && s->solver == SPIN_SOLVER_DEPONDT && !s->ddi_on && s->n_img == 1 && !s->opt_store_A &&
            s->nc[0] >= 32 && s->nc[1] >= 8 && s->nc[2] >= 8 && (s->opt_march >= 2 || s->N >= 65536);
 }
 namespace {
@@ -1102,6 +1105,22 @@ extern "C" int llg_slab_sweep(spin_system *s, int stage, int part) {
         if (rc) return rc;
         s->n_launch++;
     }
+    SPIN_CUDA(cudaGetLastError());
+    return SPIN_OK;
+}
+// The whole Depondt step of a slab in one pass (the plane-marching kernel; spin_kernel_info says "jit+march"): reads the current
+// configuration with ghost layers of depth 2 x reach along c (spin_halo_doubles reports that depth), writes the next configuration's own
+// planes.  The driver then exchanges the halos of the next configuration (array 2) ONCE and calls llg_slab_advance.  part 0: the whole
+// slab; 1: the first and the last chunk of planes (they hold what the neighbours need); 2: the chunks in between, which run while the halos travel.
+extern "C" int llg_slab_step(spin_system *s, int part) {
+    REQUIRE(s && part >= 0 && part <= 2, "bad argument");
+    int rc = slab_ready(s);
+    if (rc) return rc;
+    if (!jit_march_ready(s)) return spin::fail(SPIN_ERR_STATE, "llg_slab_step needs the one-pass marching kernel (spin_kernel_info: %s); use llg_slab_sweep", "not jit+march");
+    s->vp_active = false;
+    rc = jit_launch_march(s, s->cur, s->d_n[s->cur ^ 1], 0u, part);
+    if (rc) return rc;
+    if (part == 0) s->n_launch++;
     SPIN_CUDA(cudaGetLastError());
     return SPIN_OK;
 }

@@ -176,6 +176,8 @@ std::string spin::jit_source(const spin_system *s) {
     o << "constexpr bool DAMPING_ONLY = " << (s->damping_only ? "true" : "false") << ";\n";
     o << "constexpr bool HAS_PIN = " << (s->d_pin ? "true" : "false") << ";\n";
     o << "constexpr int CELL_OFF = " << P.cell_off << ";      // global index of local cell 0 (slab decomposition)\n";
+    // slab decomposition: first plane of this slab in the whole lattice and the planes of the whole lattice (else 0 and NC)
+    o << "constexpr int C_OFF = " << (s->slab_on ? s->slab_off : 0) << ", GNC = " << (s->slab_on ? s->slab_gnc : P.Nc) << ";\n";
     o << "constexpr bool HAS_SITE_MU = " << (s->d_mu_ratio ? "true" : "false") << ";      // per-site moments (PAPER.md:79)\n";
     o << "constexpr int SOLVER = " << s->solver << ";      // 0 Depondt, 1 Heun, 2 SIB, 3 RK4 (own stage kernel)\n";
     o << "constexpr bool STORE_A = " << ((s->opt_store_A && s->solver == 0) ? "true" : "false") << ", HAS_DDI = " << (P.has_ddi ? "true" : "false")
@@ -572,14 +574,26 @@ int spin::jit_launch_rk4_stage(spin_system *s, const double *base, const double 
 bool spin::jit_march_ready(const spin_system *s) { return s->jit && s->jit->loaded && s->jit->march; }
 
 // one Depondt step in one pass: reads d_n[cur] through its tensor map, writes nout
-int spin::jit_launch_march(spin_system *s, int cur, double *nout, unsigned step_add) {
+// part 0: every item; 1: the first and the last chunk along c (the planes a neighbouring slab needs), two launches; 2: the chunks in between
+int spin::jit_launch_march(spin_system *s, int cur, double *nout, unsigned step_add, int part) {
     JitState *j = s->jit;
     unsigned seed_lo = s->plan.seed_lo, seed_hi = s->plan.seed_hi;
     const unsigned long long *d_step = s->d_step;
     const unsigned char *pin = s->d_pin;
     const double *mu_ratio = s->d_mu_ratio;
-    void *args[] = {(void *)&j->tm_march[cur], (void *)&nout, (void *)&d_step, (void *)&step_add, (void *)&seed_lo, (void *)&seed_hi, (void *)&pin, (void *)&mu_ratio};
-    SPIN_CUDA(cudaLaunchKernel((const void *)j->k_march, dim3((unsigned)j->march_items), dim3((unsigned)j->march_threads), args, j->march_smem, s->stream));
+    unsigned item0 = 0;
+    void *args[] = {(void *)&j->tm_march[cur], (void *)&nout, (void *)&d_step, (void *)&step_add, (void *)&seed_lo, (void *)&seed_hi, (void *)&pin, (void *)&mu_ratio,
+                    (void *)&item0};
+    const unsigned items = (unsigned)j->march_items, cols = items / (unsigned)j->march_nzc;      // items = chunk x column tile, chunk-major
+    unsigned ranges[2][2] = {{0u, items}, {0u, 0u}};
+    if (part == 1) { ranges[0][1] = cols; if (j->march_nzc > 1) { ranges[1][0] = items - cols; ranges[1][1] = items; } }
+    else if (part == 2) { ranges[0][0] = cols; ranges[0][1] = j->march_nzc > 1 ? items - cols : cols; }
+    for (int r = 0; r < 2; ++r) {
+        if (ranges[r][1] <= ranges[r][0]) continue;
+        item0 = ranges[r][0];
+        SPIN_CUDA(cudaLaunchKernel((const void *)j->k_march, dim3(ranges[r][1] - ranges[r][0]), dim3((unsigned)j->march_threads), args, j->march_smem, s->stream));
+        if (part) s->n_launch++;      // (part 0: counted by the caller)
+    }
     return SPIN_OK;
 }
 

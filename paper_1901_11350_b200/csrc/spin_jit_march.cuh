@@ -74,10 +74,10 @@ struct RingAcc {
 extern "C" __global__ void __launch_bounds__(spinmarch::NTHREADS, spec::MBLOCKS)
     jit_depondt_march(const __grid_constant__ spinmarch::TensorMap tm_n, double *__restrict__ nout, const unsigned long long *__restrict__ d_step,
                       unsigned int step_add, unsigned int seed_lo, unsigned int seed_hi, const unsigned char *__restrict__ pin,
-                      const double *__restrict__ mu_ratio) {
+                      const double *__restrict__ mu_ratio, unsigned int item0) {
     using namespace spinmarch;
     const unsigned long long step = *d_step + step_add;
-    const int item = blockIdx.x, col = item % (NTX * NTY), chunk = item / (NTX * NTY);
+    const int item = (int)(blockIdx.x + item0), col = item % (NTX * NTY), chunk = item / (NTX * NTY);      // (item0: a launch over a range of chunks)
     const int x0 = (col % NTX) * 32, y0 = (col / NTX) * TY;
     const int za = (int)((long long)chunk * spec::NC / NZC), zb = (int)((long long)(chunk + 1) * spec::NC / NZC);
     const int NP = zb - za + 4 * RC;                              // n planes za - 2 RC .. zb - 1 + 2 RC
@@ -137,9 +137,12 @@ extern "C" __global__ void __launch_bounds__(spinmarch::NTHREADS, spec::MBLOCKS)
         double *pslot = pring + ps * PPL;
         if (mine) {
             double out[3] = {0.0, 0.0, 0.0};
-            const bool live = live_xy && (spec::PER_C || (zP >= 0 && zP < spec::NC));
+            // plane of the WHOLE lattice (slab decomposition: planes beyond the slab are the neighbours', staged from the ghost layers the
+            // halo exchange fills; their predictor is recomputed here like the rim of a tile)
+            const int gz = spec::C_OFF + zP;
+            const bool live = live_xy && (spec::PER_C || (gz >= 0 && gz < spec::GNC));
             if (live) {
-                c.ic = zP < 0 ? zP + spec::NC : (zP >= spec::NC ? zP - spec::NC : zP);
+                c.ic = (gz < 0 ? gz + spec::GNC : (gz >= spec::GNC ? gz - spec::GNC : gz)) - spec::C_OFF;      // (outside [0, NC) only in a slab: noise index)
                 RingAcc<NX, NROW> acc;
 #pragma unroll
                 for (int dz = -RC; dz <= RC; ++dz) acc.pl[dz + RC] = nring + nslot_of(RC + dz) * NSLOT + ncell;

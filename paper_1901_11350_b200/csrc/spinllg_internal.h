@@ -198,7 +198,7 @@ int jit_launch_rk4_stage(spin_system *s, const double *base, const double *y, do
 // the whole Depondt step in one pass (jit_depondt_march, spin_jit_march.cuh): 3-D lattices of one basis atom without dipolar coupling
 bool march_eligible(const spin_system *s);      // spin_api.cu: decided from the system alone (the planner doubles the ghost layers for it)
 bool jit_march_ready(const spin_system *s);
-int jit_launch_march(spin_system *s, int cur, double *nout, unsigned step_add);
+int jit_launch_march(spin_system *s, int cur, double *nout, unsigned step_add, int part = 0);
 // all steps of an llg_iterate call in one cooperative launch (jit_steps_coop)
 bool jit_coop_ready(const spin_system *s);
 bool jit_cluster_ready(const spin_system *s);

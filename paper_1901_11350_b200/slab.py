@@ -128,7 +128,7 @@ class SlabDriver:
       end_stage     write the received planes into the ghost layers; the system's stream waits for that before its next sweep
     """
 
-    def __init__(self, P, torch, w, rank: int, world: int, transport=None, stream=None):
+    def __init__(self, P, torch, w, rank: int, world: int, transport=None, stream=None, options=()):
         self.P, self.torch = P, torch
         na, nb_, nc = (int(x) for x in w.n_cells)
         first, count = partition(nc, world)[rank]
@@ -136,10 +136,15 @@ class SlabDriver:
         self.stream = stream if stream is not None else torch.cuda.Stream()
         self.copy_stream = torch.cuda.Stream()
         self.sys = P.SpinSystem.from_workload(lw, stream=self.stream.cuda_stream)
+        for name, value in dict(options).items():             # execution options (spin_set_option), the same on every rank
+            self.sys.spin_set_option(name, int(value))
         self.sys.spin_set_slab(True, first, nc, int(w.periodic[2]))
         per_plane = self.sys.N // count
         self.sys.spins_set(w.initial_spins().reshape(nc, per_plane, 3)[first:first + count].reshape(-1, 3))      # boundary order: planes are contiguous
         nd, reach = self.sys.spin_halo_doubles()
+        # one-pass marching kernel (3-D lattices of one basis atom, Depondt): the slab recomputes the predictor of its neighbours' boundary
+        # planes, so a step needs ONE exchange (of the new configuration, ghost depth 2 x reach) instead of two
+        self.one_pass = "march" in self.sys.spin_kernel_info()
         self.plan = HaloPlan.make(rank, world, nc, bool(w.periodic[2]), reach)
         self.transport = transport
         dev = torch.device("cuda", torch.cuda.current_device())
@@ -173,6 +178,18 @@ class SlabDriver:
         self.post(array)
         self.sys.llg_slab_sweep(stage, 2)
 
+    def begin_step(self) -> None:
+        """one-pass mode: the chunks of planes the neighbours need, their halo copies on the second stream, the chunks in between"""
+        self.sys.llg_slab_step(1)
+        self.post(2)
+        self.sys.llg_slab_step(2)
+
+    def stages(self):
+        """(begin, array) of every exchange of one step"""
+        if self.one_pass:
+            return [(self.begin_step, 2)]
+        return [(lambda: self.begin_stage(0, 1), 1), (lambda: self.begin_stage(1, 2), 2)]
+
     def _transport(self) -> None:
         with self.torch.cuda.stream(self.copy_stream):
             self.transport.sendrecv(self.plan, self.send, self.recv)
@@ -186,8 +203,8 @@ class SlabDriver:
             self.exchange_initial()
             self._primed = True
         for _ in range(int(n_steps)):
-            self.begin_stage(0, 1); self._transport(); self.deliver(1)      # predictor, halos of n^p
-            self.begin_stage(1, 2); self._transport(); self.deliver(2)      # corrector, halos of the next n
+            for begin, array in self.stages():          # two-sweep mode: predictor + halos of n^p, corrector + halos of the next n
+                begin(); self._transport(); self.deliver(array)
             self.sys.llg_slab_advance()
 
     def spins(self):
@@ -204,9 +221,9 @@ class LocalGroup:
     separate launches, B200_PROFILING.md).  The slabs advance in lockstep; a halo message is a device copy from the sender's send buffer
     into the receiver's receive buffer, ordered by the sender's event."""
 
-    def __init__(self, P, torch, w, world: int):
+    def __init__(self, P, torch, w, world: int, options=()):
         self.torch = torch
-        self.drivers = [SlabDriver(P, torch, w, r, world) for r in range(world)]
+        self.drivers = [SlabDriver(P, torch, w, r, world, options=options) for r in range(world)]
         self._exchange(0, post=True)
 
     def _move(self) -> None:
@@ -239,10 +256,11 @@ class LocalGroup:
 
     def iterate(self, n_steps: int) -> None:
         for _ in range(int(n_steps)):
-            for stage, array in ((0, 1), (1, 2)):
-                for d in self.drivers:
-                    d.begin_stage(stage, array)
-                self._exchange(array, post=False)
+            plans = [d.stages() for d in self.drivers]      # (every slab is in the same mode: the same Hamiltonian and options)
+            for k in range(len(plans[0])):
+                for p in plans:
+                    p[k][0]()
+                self._exchange(plans[0][k][1], post=False)
             for d in self.drivers:
                 d.sys.llg_slab_advance()
 

@@ -1053,6 +1053,45 @@ def test_slab_decomposition_is_bit_identical(P, O, cfg, cells, per_c, world, ste
         off += d.sys.N
 
 
+@pytest.mark.parametrize("cfg,cells,per_c,world,steps,T,reach2", [
+    (3, (64, 32, 24), 1, 2, 20, 0.0, False),       # periodic ring of two slabs of 12 planes
+    (3, (70, 17, 27), 1, 3, 16, 15.0, False),      # ragged tiles, three slabs of 9 planes, thermal field keyed by the global spin
+    (3, (40, 24, 20), 0, 2, 20, 0.0, False),       # open along c: the outer ghost layers stay zero, the outer rim planes are dead
+    (5, (64, 24, 17), 0, 2, 16, 5.0, False),       # film Hamiltonian (in-plane DMI), dipolar term off, uneven slabs (9, 8)
+    (3, (64, 16, 24), 1, 2, 12, 0.0, True),        # pairs reaching two planes along c: ghost layers of four planes
+])
+def test_slab_decomposition_with_the_one_pass_kernel(P, O, cfg, cells, per_c, world, steps, T, reach2):
+    """Slabs advanced by the plane-marching kernel (llg_slab_step): ONE halo exchange per step (the new configuration, ghost depth
+    2 x reach) instead of two; the slab recomputes the predictor of its neighbours' boundary planes.  Bit-identical to the single lattice."""
+    import torch
+    from paper_1901_11350_b200 import slab as S
+    w = W.CONFIGS[cfg]().resized(cells, steps)
+    w = dataclasses.replace(w, periodic=(w.periodic[0], w.periodic[1], per_c), T=T, ddi=False)
+    if reach2:
+        pt = np.vstack([w.pair_t, [[0, 0, 2], [1, 0, 2]]]); pi = np.r_[w.pair_i, 0, 0]; pj = np.r_[w.pair_j, 0, 0]
+        w = dataclasses.replace(w, pair_i=pi, pair_j=pj, pair_t=pt, pair_J=np.r_[w.pair_J, 0.3, -0.2], pair_D=np.vstack([w.pair_D, [[0.05, 0, 0.1], [0, 0.07, 0]]]))
+    ref = P.SpinSystem.from_workload(w)
+    ref.spin_set_option("use_coop", 0); ref.spin_set_option("use_march", 2)
+    assert ref.spin_kernel_info() == "jit+march"
+    ref.llg_iterate(steps)
+    grp = S.LocalGroup(P, torch, w, world, options={"use_march": 2})
+    assert all(d.one_pass and d.plan.reach == (4 if reach2 else 2) for d in grp.drivers), [d.sys.spin_kernel_info() for d in grp.drivers]
+    assert len(grp.drivers[0].stages()) == 1
+    grp.iterate(steps)
+    got = grp.spins()
+    assert np.array_equal(got, ref.spins_get()), np.abs(got - ref.spins_get()).max()
+    o = O.OracleSystem.from_workload(w)
+    o.iterate(steps)
+    assert np.abs(got - o.spins()).max() <= SPIN_ATOL
+    # pinned spins or per-site moments: the slab falls back to the two-sweep kernels (it would need its neighbours' flags)
+    grp2 = S.LocalGroup(P, torch, w, world, options={"use_march": 2})
+    for d in grp2.drivers:
+        d.sys.hamiltonian_set_site_mu_s(np.full(d.sys.N, w.mu_s[0]))
+    assert not any("march" in d.sys.spin_kernel_info() for d in grp2.drivers)
+    with pytest.raises(P.SpinError):
+        grp2.drivers[0].sys.llg_slab_step(0)
+
+
 def test_slab_reach_two_and_other_solvers(P, O):
     """Pairs reaching two planes along c (ghost width 2) and the Heun / SIB solvers on slabs; llg_iterate refuses a slab."""
     import torch
