@@ -225,6 +225,33 @@ int llg_slab_advance(spin_system *sys);
  * last chunk of planes, which hold everything the neighbours need; 2: the chunks in between (launched after the halo copies of part 1
  * have been started, they run while the halos travel).  SPIN_ERR_STATE if the kernel does not apply to this system (use llg_slab_sweep). */
 int llg_slab_step(spin_system *sys, int part);
+/* The one-pass step with the halo exchange FUSED into the kernel: it writes the boundary planes of the next configuration straight into
+ * the neighbours' ghost layers, so no halo copy and no message follow a step.
+ *   peer_lo_next / peer_hi_next   DEVICE pointers to the NEXT-configuration arrays of the lower / upper neighbour (from its
+ *                                 spin_slab_arrays), writable from this GPU: peer access over NVLink, an opened CUDA IPC handle, or
+ *                                 another system on this device; NULL where there is no neighbour (open end).  Not owned.
+ *   peer_lo_cells_c               planes of the lower neighbour's slab (slabs may differ by one plane)
+ * The driver keeps ORDER only: the call must be enqueued after both neighbours' previous step has completed (they wrote this slab's ghost
+ * layers, and they read the arrays this step writes into).  Same conditions and errors as llg_slab_step.                    */
+int llg_slab_step_fused(spin_system *sys, double *peer_lo_next, int peer_lo_cells_c, double *peer_hi_next);
+/* device pointers of the current and the next configuration array of a slab (they swap at every llg_slab_advance); valid until the
+ * plan is rebuilt.  Owned by the system.                                                                                   */
+int spin_slab_arrays(spin_system *sys, double **current, double **next);
+/* The fused exchange between PROCESSES (one per GPU).  Memory: spin_ipc_export gives the 64-byte CUDA IPC handle of the allocation that
+ * holds a device pointer (a slab's arrays, its flags) and the pointer's offset in it; the neighbour's process maps it with spin_ipc_open
+ * (peer access is enabled on the way) and unmaps it with spin_ipc_close.  Order: events of another process cannot carry a step number, so
+ * each slab owns two flags in device memory (spin_slab_flags: [0] written by its lower, [1] by its upper neighbour, zero at first);
+ * spin_flag_signal enqueues, on the system's stream, a store of `value` into a flag (release, system scope: after everything enqueued
+ * before it), spin_flag_wait enqueues a wait until a flag holds at least `value` (a one-thread kernel that polls; after 30 s it traps
+ * instead of hanging; every kernel that is to run while a wait polls must have run once before -- its first launch may load code,
+ * which waits for the device).  A step k + 1 follows wait(own flags >= k) and is followed by signal(neighbours' flags = k + 1).  The waits depend
+ * on another GPU's progress: ranks that use them must not share a GPU.                                                      */
+int spin_ipc_export(const void *device_ptr, unsigned char handle[64], int64_t *offset);
+int spin_ipc_open(const unsigned char handle[64], int64_t offset, void **device_ptr);
+int spin_ipc_close(void *device_ptr, int64_t offset);
+int spin_slab_flags(spin_system *sys, unsigned long long **flags);
+int spin_flag_signal(spin_system *sys, unsigned long long *flag, unsigned long long value);
+int spin_flag_wait(spin_system *sys, const unsigned long long *flag, unsigned long long value);
 
 /* ---- execution options ------------------------------------------------------------------------------------------------
  * spin_set_option(name, value) changes how the path is executed, never what it computes (every combination is bit-identical; tested).

@@ -5,6 +5,6 @@
 
 The package never imports `oracle` (the CPU checker) and has no CPU fallback.
 """
-from .binding import EXPORTS, SpinError, SpinSystem, lib, spin_jit_compiler_info, version
+from .binding import EXPORTS, SpinError, SpinSystem, lib, spin_ipc_close, spin_ipc_export, spin_ipc_open, spin_jit_compiler_info, version
 
-__all__ = ["SpinSystem", "SpinError", "lib", "version", "spin_jit_compiler_info", "EXPORTS"]
+__all__ = ["SpinSystem", "SpinError", "lib", "version", "spin_jit_compiler_info", "EXPORTS", "spin_ipc_export", "spin_ipc_open", "spin_ipc_close"]

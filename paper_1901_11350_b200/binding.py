@@ -22,7 +22,8 @@ EXPORTS = [
     "hamiltonian_set_ddi", "spin_set_images", "spin_select_image", "llg_set_image_temperatures", "gneb_forces", "gneb_iterate", "spins_set_pinned", "spins_set", "spins_get", "spins_set_device", "spins_get_device",
     "llg_configure", "llg_set_solver", "llg_set_damping_only", "minimise_vp", "minimise_vp_reset", "llg_iterate", "llg_get_step", "llg_set_step", "spin_synchronize",
     "effective_field", "effective_field_device", "energy", "observables", "topological_charge", "topological_charge_noalloc",
-    "spin_set_slab", "spin_halo_doubles", "spin_halo_get", "spin_halo_put", "llg_slab_sweep", "llg_slab_step", "llg_slab_advance",
+    "spin_set_slab", "spin_halo_doubles", "spin_halo_get", "spin_halo_put", "llg_slab_sweep", "llg_slab_step", "llg_slab_step_fused", "spin_slab_arrays", "llg_slab_advance",
+    "spin_ipc_export", "spin_ipc_open", "spin_ipc_close", "spin_slab_flags", "spin_flag_signal", "spin_flag_wait",
     "spin_launch_counts", "spin_measure_fp64_tflops", "spin_profile_enable", "spin_profile_get", "spin_set_option",
     "spin_kernel_info", "spin_ddi_info", "spin_jit_compiler_info", "spin_jit_source", "spin_last_error", "spin_version",
 ]
@@ -92,6 +93,14 @@ def lib() -> C.CDLL:
         "spin_halo_put": (C.c_int, [vp, C.c_int, C.c_int, vp, vp]),
         "llg_slab_sweep": (C.c_int, [vp, C.c_int, C.c_int]),
         "llg_slab_step": (C.c_int, [vp, C.c_int]),
+        "llg_slab_step_fused": (C.c_int, [vp, C.c_void_p, C.c_int, C.c_void_p]),
+        "spin_slab_arrays": (C.c_int, [vp, C.POINTER(C.c_void_p), C.POINTER(C.c_void_p)]),
+        "spin_ipc_export": (C.c_int, [C.c_void_p, C.c_char_p, C.POINTER(C.c_int64)]),
+        "spin_ipc_open": (C.c_int, [C.c_char_p, C.c_int64, C.POINTER(C.c_void_p)]),
+        "spin_ipc_close": (C.c_int, [C.c_void_p, C.c_int64]),
+        "spin_slab_flags": (C.c_int, [vp, C.POINTER(C.c_void_p)]),
+        "spin_flag_signal": (C.c_int, [vp, C.c_void_p, C.c_uint64]),
+        "spin_flag_wait": (C.c_int, [vp, C.c_void_p, C.c_uint64]),
         "llg_slab_advance": (C.c_int, [vp]),
         "spin_profile_enable": (C.c_int, [vp, C.c_int]),
         "spin_profile_get": (C.c_int, [vp, C.c_int, dp, i64p]),
@@ -366,6 +375,28 @@ class SpinSystem:
     def llg_slab_step(self, part=0):
         _check(lib().llg_slab_step(self._h, int(part)))
 
+    def llg_slab_step_fused(self, peer_lo_next, peer_lo_cells_c, peer_hi_next):
+        """peer_*_next: device addresses (int) of the neighbours' next-configuration arrays, or None at an open end"""
+        _check(lib().llg_slab_step_fused(self._h, C.c_void_p(peer_lo_next or None), int(peer_lo_cells_c), C.c_void_p(peer_hi_next or None)))
+
+    def spin_slab_arrays(self):
+        """(current, next): device addresses of the configuration arrays (they swap at every llg_slab_advance)"""
+        a, b = C.c_void_p(0), C.c_void_p(0)
+        _check(lib().spin_slab_arrays(self._h, C.byref(a), C.byref(b)))
+        return int(a.value), int(b.value)
+
+    def spin_slab_flags(self):
+        """device address of the slab's two step flags ([0] written by the lower, [1] by the upper neighbour)"""
+        p = C.c_void_p(0)
+        _check(lib().spin_slab_flags(self._h, C.byref(p)))
+        return int(p.value)
+
+    def spin_flag_signal(self, flag_addr, value):
+        _check(lib().spin_flag_signal(self._h, C.c_void_p(int(flag_addr)), int(value)))
+
+    def spin_flag_wait(self, flag_addr, value):
+        _check(lib().spin_flag_wait(self._h, C.c_void_p(int(flag_addr)), int(value)))
+
     def llg_slab_advance(self):
         _check(lib().llg_slab_advance(self._h))
 
@@ -410,3 +441,23 @@ def spin_jit_compiler_info() -> str:
     buf = C.create_string_buffer(1024)
     _check(lib().spin_jit_compiler_info(buf, 1024))
     return buf.value.decode()
+
+
+def spin_ipc_export(device_addr):
+    """(64-byte CUDA IPC handle, offset) of the allocation that holds the device address: picklable, for the neighbour's process"""
+    h = C.create_string_buffer(64)
+    off = C.c_int64(0)
+    _check(lib().spin_ipc_export(C.c_void_p(int(device_addr)), h, C.byref(off)))
+    return bytes(h.raw), int(off.value)
+
+
+def spin_ipc_open(handle, offset):
+    """device address in THIS process of what another process exported"""
+    p = C.c_void_p(0)
+    _check(lib().spin_ipc_open(C.c_char_p(bytes(handle)), int(offset), C.byref(p)))
+    return int(p.value)
+
+
+def spin_ipc_close(device_addr, offset):
+    _check(lib().spin_ipc_close(C.c_void_p(int(device_addr)), int(offset)))
+

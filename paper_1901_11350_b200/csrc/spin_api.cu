@@ -558,7 +558,7 @@ extern "C" int spin_geometry_create(const double bravais[9], int n_basis, const 
     if (!has_device) cudaGetLastError();
     spin_system *s = new spin_system();
     s->has_device = has_device;
-    s->jit = nullptr; s->opt_jit = 1; s->opt_march = 1; s->opt_ddi_slab = 1; s->opt_ddi_mirror = 1; s->opt_pdl = -1; s->opt_cache_noise = 1; s->opt_coop = 1; s->d_bar = nullptr;
+    s->jit = nullptr; s->opt_jit = 1; s->opt_march = 1; s->opt_ddi_slab = 1; s->opt_ddi_mirror = 1; s->opt_pdl = -1; s->opt_cache_noise = 1; s->opt_coop = 1; s->d_bar = nullptr; s->d_flags = nullptr;
     s->n_img = 1; s->img_sel = 0; s->d_img_sigma = nullptr;
     memcpy(s->brav, bravais, sizeof(s->brav));
     s->nb = n_basis;
@@ -626,7 +626,7 @@ extern "C" void spin_system_destroy(spin_system *s) {
     ddi_release(s);
     jit_release(s);
     cudaFree(s->d_n[0]); cudaFree(s->d_n[1]); cudaFree(s->d_np); cudaFree(s->d_A); cudaFree(s->d_fddi[0]); cudaFree(s->d_fddi[1]);
-    cudaFree(s->d_pin); cudaFree(s->d_vp); cudaFree(s->d_bar); cudaFree(s->d_img_sigma);
+    cudaFree(s->d_pin); cudaFree(s->d_vp); cudaFree(s->d_bar); cudaFree(s->d_img_sigma); cudaFree(s->d_flags);
     cudaFree(s->d_aos); cudaFree(s->d_partials); cudaFree(s->d_result); cudaFree(s->d_step); cudaFree(s->d_mu_ratio);
     if (s->ev0) cudaEventDestroy(s->ev0);
     if (s->ev1) cudaEventDestroy(s->ev1);
@@ -1122,6 +1122,117 @@ extern "C" int llg_slab_step(spin_system *s, int part) {
     if (rc) return rc;
     if (part == 0) s->n_launch++;
     SPIN_CUDA(cudaGetLastError());
+    return SPIN_OK;
+}
+// The same step with the halo exchange FUSED into the kernel: the boundary planes of the next configuration are written by the kernel
+// itself into the neighbours' ghost layers (peer_lo_next / peer_hi_next: the neighbours' next-configuration arrays from spin_slab_arrays,
+// device pointers this GPU can write -- peer access over NVLink, an opened IPC handle, or another system of this device; NULL at an open
+// end).  No halo copy and no message follow; what remains for the driver is ORDER: this call must come after both neighbours' previous
+// step has completed (they wrote this slab's ghost layers and read the arrays this step overwrites), e.g. by stream waits on their events.
+extern "C" int llg_slab_step_fused(spin_system *s, double *peer_lo_next, int peer_lo_cells_c, double *peer_hi_next) {
+    REQUIRE(s, "null system");
+    int rc = slab_ready(s);
+    if (rc) return rc;
+    if (!jit_march_ready(s)) return spin::fail(SPIN_ERR_STATE, "llg_slab_step_fused needs the one-pass marching kernel (spin_kernel_info: %s); use llg_slab_sweep", "not jit+march");
+    REQUIRE(!peer_lo_next || peer_lo_cells_c >= s->plan.rC, "lower neighbour thinner than the ghost depth");
+    s->vp_active = false;
+    rc = jit_launch_march(s, s->cur, s->d_n[s->cur ^ 1], 0u, 0, peer_lo_next, peer_hi_next, peer_lo_cells_c);
+    if (rc) return rc;
+    s->n_launch++;
+    SPIN_CUDA(cudaGetLastError());
+    return SPIN_OK;
+}
+// device pointers of the current and the next configuration array (padded layout of DESIGN.md section 2, ghost layers included): what a
+// neighbouring slab writes into (llg_slab_step_fused).  They swap roles at every llg_slab_advance.
+extern "C" int spin_slab_arrays(spin_system *s, double **current, double **next) {
+    REQUIRE(s && current && next, "null argument");
+    int rc = slab_ready(s);
+    if (rc) return rc;
+    *current = s->d_n[s->cur]; *next = s->d_n[s->cur ^ 1];
+    return SPIN_OK;
+}
+// ---- between PROCESSES (one per GPU): the neighbours' arrays are mapped through CUDA IPC and the order of the steps is kept by flags in
+// device memory instead of events (an event of another process cannot say WHICH record a wait refers to): after its step k a slab writes
+// k into a flag of each neighbour (release, system scope, stream-ordered after the step's kernel); before its step k + 1 it waits until
+// both its flags hold k.  The wait is a one-thread kernel that polls with a bound and traps when the bound is hit (a lost neighbour ends
+// the launch with an error, never hangs the device).  Each kernel waits on ANOTHER GPU's progress: never run two such ranks on one GPU.
+namespace {
+__global__ void flag_signal_kernel(unsigned long long *flag, unsigned long long value) {
+    asm volatile("st.release.sys.global.u64 [%0], %1;" ::"l"(flag), "l"(value) : "memory");
+}
+__global__ void flag_wait_kernel(const unsigned long long *flag, unsigned long long value) {
+    unsigned long long v = 0, t0 = 0, t = 0;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t0));
+    for (;;) {
+        asm volatile("ld.acquire.sys.global.u64 %0, [%1];" : "=l"(v) : "l"(flag) : "memory");
+        if (v >= value) return;
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+        if (t - t0 > 30000000000ull) __trap();      // 30 s without the neighbour: an error, not a hang
+    }
+}
+}  // namespace
+extern "C" int spin_slab_flags(spin_system *s, unsigned long long **flags) {
+    REQUIRE(s && flags, "null argument");
+    NEED_DEVICE(s);
+    if (!s->d_flags) {
+        SPIN_CUDA(cudaMalloc(&s->d_flags, 2 * sizeof(unsigned long long)));
+        SPIN_CUDA(cudaMemsetAsync(s->d_flags, 0, 2 * sizeof(unsigned long long), s->stream));
+        // both kernels run once now: the first launch of a kernel may load its module, which cannot happen while a wait is polling
+        flag_signal_kernel<<<1, 1, 0, s->stream>>>(s->d_flags, 0ull);
+        flag_wait_kernel<<<1, 1, 0, s->stream>>>(s->d_flags, 0ull);
+        SPIN_CUDA(cudaStreamSynchronize(s->stream));
+    }
+    *flags = s->d_flags;
+    return SPIN_OK;
+}
+extern "C" int spin_flag_signal(spin_system *s, unsigned long long *flag, unsigned long long value) {
+    REQUIRE(s && flag, "null argument");
+    NEED_DEVICE(s);
+    flag_signal_kernel<<<1, 1, 0, s->stream>>>(flag, value);
+    s->n_launch++;
+    SPIN_CUDA(cudaGetLastError());
+    return SPIN_OK;
+}
+extern "C" int spin_flag_wait(spin_system *s, const unsigned long long *flag, unsigned long long value) {
+    REQUIRE(s && flag, "null argument");
+    NEED_DEVICE(s);
+    flag_wait_kernel<<<1, 1, 0, s->stream>>>(flag, value);
+    s->n_launch++;
+    SPIN_CUDA(cudaGetLastError());
+    return SPIN_OK;
+}
+// CUDA IPC: the handle of the ALLOCATION that holds `device_ptr` and the pointer's offset inside it (small allocations share one), to be
+// sent to the neighbour's process by any means; spin_ipc_open maps it there and returns the same address plus offset
+extern "C" int spin_ipc_export(const void *device_ptr, unsigned char handle[64], int64_t *offset) {
+    REQUIRE(device_ptr && handle && offset, "null argument");
+    static_assert(sizeof(cudaIpcMemHandle_t) == 64, "CUDA IPC handles are 64 bytes");
+    typedef int (*range_fn)(unsigned long long *, size_t *, unsigned long long);
+    void *fn = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    SPIN_CUDA(cudaGetDriverEntryPoint("cuMemGetAddressRange", &fn, cudaEnableDefault, &qres));
+    if (!fn || qres != cudaDriverEntryPointSuccess) return spin::fail(SPIN_ERR_CUDA, "cuMemGetAddressRange is not available from this driver");
+    unsigned long long base = 0;
+    size_t size = 0;
+    const int r = ((range_fn)fn)(&base, &size, (unsigned long long)(uintptr_t)device_ptr);
+    if (r != 0) return spin::fail(SPIN_ERR_CUDA, "cuMemGetAddressRange failed: driver error %d", r);
+    cudaIpcMemHandle_t h;
+    SPIN_CUDA(cudaIpcGetMemHandle(&h, (void *)(uintptr_t)base));
+    memcpy(handle, &h, 64);
+    *offset = (int64_t)((unsigned long long)(uintptr_t)device_ptr - base);
+    return SPIN_OK;
+}
+extern "C" int spin_ipc_open(const unsigned char handle[64], int64_t offset, void **device_ptr) {
+    REQUIRE(handle && device_ptr && offset >= 0, "bad argument");
+    cudaIpcMemHandle_t h;
+    memcpy(&h, handle, 64);
+    void *base = nullptr;
+    SPIN_CUDA(cudaIpcOpenMemHandle(&base, h, cudaIpcMemLazyEnablePeerAccess));
+    *device_ptr = (char *)base + offset;
+    return SPIN_OK;
+}
+extern "C" int spin_ipc_close(void *device_ptr, int64_t offset) {
+    REQUIRE(device_ptr && offset >= 0, "bad argument");
+    SPIN_CUDA(cudaIpcCloseMemHandle((char *)device_ptr - offset));
     return SPIN_OK;
 }
 // after the corrector sweeps of a step: the next configuration becomes the current one and the step counter (the noise stream) advances

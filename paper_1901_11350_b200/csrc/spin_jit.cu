@@ -178,6 +178,7 @@ std::string spin::jit_source(const spin_system *s) {
     o << "constexpr int CELL_OFF = " << P.cell_off << ";      // global index of local cell 0 (slab decomposition)\n";
     // slab decomposition: first plane of this slab in the whole lattice and the planes of the whole lattice (else 0 and NC)
     o << "constexpr int C_OFF = " << (s->slab_on ? s->slab_off : 0) << ", GNC = " << (s->slab_on ? s->slab_gnc : P.Nc) << ";\n";
+    o << "constexpr bool SLAB = " << (s->slab_on ? "true" : "false") << ";\n";
     o << "constexpr bool HAS_SITE_MU = " << (s->d_mu_ratio ? "true" : "false") << ";      // per-site moments (PAPER.md:79)\n";
     o << "constexpr int SOLVER = " << s->solver << ";      // 0 Depondt, 1 Heun, 2 SIB, 3 RK4 (own stage kernel)\n";
     o << "constexpr bool STORE_A = " << ((s->opt_store_A && s->solver == 0) ? "true" : "false") << ", HAS_DDI = " << (P.has_ddi ? "true" : "false")
@@ -575,7 +576,8 @@ bool spin::jit_march_ready(const spin_system *s) { return s->jit && s->jit->load
 
 // one Depondt step in one pass: reads d_n[cur] through its tensor map, writes nout
 // part 0: every item; 1: the first and the last chunk along c (the planes a neighbouring slab needs), two launches; 2: the chunks in between
-int spin::jit_launch_march(spin_system *s, int cur, double *nout, unsigned step_add, int part) {
+// peer_lo / peer_hi (slabs only, may be null): the neighbours' next configurations, into whose ghost layers the kernel writes its boundary planes
+int spin::jit_launch_march(spin_system *s, int cur, double *nout, unsigned step_add, int part, double *peer_lo, double *peer_hi, int peer_lo_nc) {
     JitState *j = s->jit;
     unsigned seed_lo = s->plan.seed_lo, seed_hi = s->plan.seed_hi;
     const unsigned long long *d_step = s->d_step;
@@ -583,7 +585,7 @@ int spin::jit_launch_march(spin_system *s, int cur, double *nout, unsigned step_
     const double *mu_ratio = s->d_mu_ratio;
     unsigned item0 = 0;
     void *args[] = {(void *)&j->tm_march[cur], (void *)&nout, (void *)&d_step, (void *)&step_add, (void *)&seed_lo, (void *)&seed_hi, (void *)&pin, (void *)&mu_ratio,
-                    (void *)&item0};
+                    (void *)&item0, (void *)&peer_lo, (void *)&peer_hi, (void *)&peer_lo_nc};
     const unsigned items = (unsigned)j->march_items, cols = items / (unsigned)j->march_nzc;      // items = chunk x column tile, chunk-major
     unsigned ranges[2][2] = {{0u, items}, {0u, 0u}};
     if (part == 1) { ranges[0][1] = cols; if (j->march_nzc > 1) { ranges[1][0] = items - cols; ranges[1][1] = items; } }

@@ -74,7 +74,8 @@ struct RingAcc {
 extern "C" __global__ void __launch_bounds__(spinmarch::NTHREADS, spec::MBLOCKS)
     jit_depondt_march(const __grid_constant__ spinmarch::TensorMap tm_n, double *__restrict__ nout, const unsigned long long *__restrict__ d_step,
                       unsigned int step_add, unsigned int seed_lo, unsigned int seed_hi, const unsigned char *__restrict__ pin,
-                      const double *__restrict__ mu_ratio, unsigned int item0) {
+                      const double *__restrict__ mu_ratio, unsigned int item0, double *__restrict__ peer_lo, double *__restrict__ peer_hi,
+                      int peer_lo_nc) {
     using namespace spinmarch;
     const unsigned long long step = *d_step + step_add;
     const int item = (int)(blockIdx.x + item0), col = item % (NTX * NTY), chunk = item / (NTX * NTY);      // (item0: a launch over a range of chunks)
@@ -184,7 +185,16 @@ extern "C" __global__ void __launch_bounds__(spinmarch::NTHREADS, spec::MBLOCKS)
                 spin::rodrigues(Ac, specc::HDT, specc::QDT2, n_q[0], o);                          // B6-B7: R((A + A^p) / 2) n(t)
                 spin::renormalise(o);
             }
-            store_spin(nout + ((size_t)(zC + spec::LC) * PLANE + (size_t)(c.ib + spec::LB) * ROW + (c.ia + spec::LA)), c, o);
+            const size_t in_plane = (size_t)(c.ib + spec::LB) * ROW + (c.ia + spec::LA);
+            store_spin(nout + ((size_t)(zC + spec::LC) * PLANE + in_plane), c, o);
+            // Slab decomposition, fused exchange (llg_slab_step_fused): the planes a neighbouring slab holds as ghost layers are written
+            // straight into ITS next configuration -- peer memory on another GPU (NVLink), or another array of this GPU -- with their
+            // in-plane images; no halo copy follows.  peer_lo: the lower neighbour (its ghost layer above its peer_lo_nc planes),
+            // peer_hi: the upper neighbour (its ghost layer below plane 0).  Same layout on every slab but for the number of planes.
+            if constexpr (spec::SLAB) {
+                if (peer_lo && zC < spec::LC) store_spin(peer_lo + ((size_t)(spec::LC + peer_lo_nc + zC) * PLANE + in_plane), c, o);
+                if (peer_hi && zC >= spec::NC - spec::LC) store_spin(peer_hi + ((size_t)(zC - (spec::NC - spec::LC)) * PLANE + in_plane), c, o);
+            }
         }
         // the queue moves on: slot 0 is the oldest (the plane the next corrector takes)
 #pragma unroll

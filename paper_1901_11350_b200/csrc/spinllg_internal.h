@@ -144,6 +144,7 @@ struct spin_system {
     double *d_img_sigma;           // per-image factor on the thermal amplitude, sqrt(T_image / T), or null (all 1)
     std::vector<double> img_T;     // the absolute per-image temperatures it was made from (empty: none set)
     unsigned int *d_bar;           // arrival counter of the cooperative kernel's grid barrier
+    unsigned long long *d_flags;   // step flags of a slab (spin_slab_flags): [0] written by the lower, [1] by the upper neighbour
     double *d_vp;                  // velocity-projection state: ratio r, started flag, |F|^2
     bool vp_active;                // d_A holds the force of the previous VP iteration
     int vp_cur;                    // which of {d_A, d_fddi[1]} holds it
@@ -198,7 +199,8 @@ int jit_launch_rk4_stage(spin_system *s, const double *base, const double *y, do
 // the whole Depondt step in one pass (jit_depondt_march, spin_jit_march.cuh): 3-D lattices of one basis atom without dipolar coupling
 bool march_eligible(const spin_system *s);      // spin_api.cu: decided from the system alone (the planner doubles the ghost layers for it)
 bool jit_march_ready(const spin_system *s);
-int jit_launch_march(spin_system *s, int cur, double *nout, unsigned step_add, int part = 0);
+int jit_launch_march(spin_system *s, int cur, double *nout, unsigned step_add, int part = 0, double *peer_lo = nullptr, double *peer_hi = nullptr,
+                     int peer_lo_nc = 0);
 // all steps of an llg_iterate call in one cooperative launch (jit_steps_coop)
 bool jit_coop_ready(const spin_system *s);
 bool jit_cluster_ready(const spin_system *s);

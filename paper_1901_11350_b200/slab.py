@@ -9,7 +9,12 @@ contiguous device chunks are the C library's (include/spinllg.h "slab decomposit
   * `exchange`         one halo exchange of one array over a transport (`DistTransport`: torch.distributed point-to-point, NCCL between
                        GPUs, gloo in the CPU tests);
   * `SlabDriver`       one rank's step: boundary bricks first, their halos travel on a second stream while the interior bricks run;
-  * `LocalGroup`       all slabs in one process on one device (device copies as transport): the 1-GPU emulation of N ranks.
+  * `LocalGroup`       all slabs in one process on one device (device copies as transport): the 1-GPU emulation of N ranks;
+  * one-pass mode      (3-D lattices of one basis atom, Depondt): the plane-marching kernel steps a slab in one pass, ONE exchange of
+                       depth 2 x reach per step (`llg_slab_step`);
+  * fused exchange     that kernel writes its boundary planes straight into the neighbours' ghost layers (`llg_slab_step_fused`):
+                       `LocalGroup(fused=True)` in one process, `SlabDriver.setup_fused` / `iterate_fused` between processes (CUDA IPC
+                       mappings, order kept by flags in device memory: `fused_links`, `fused_step_ops`).
 
 Only argument marshalling and ordering happen here; every arithmetic step of the path runs in the library's kernels.  The paper has no
 counterpart (MPI appears only as a remark on scripting).
@@ -114,6 +119,38 @@ def exchange(plan: HaloPlan, get, put, send_buf, recv_buf, transport) -> None:
             put(side, recv_buf[side])
 
 
+@dataclasses.dataclass(frozen=True)
+class FusedLink:
+    """What one rank needs to know about the neighbour on one side for the fused exchange between processes (llg_slab_step_fused)."""
+    rank: int                 # the neighbour
+    count: int                # planes of its slab
+    arrays: tuple             # exports (handle, offset) of its (current, next) configuration arrays AT SET-UP; they swap every step
+    flags: tuple              # export of its two step flags
+    signal_index: int         # which of ITS flags this rank writes: 1 if this rank is its upper neighbour, 0 if its lower
+
+
+def fused_links(plan: HaloPlan, infos: Sequence[dict]) -> List[Optional[FusedLink]]:
+    """links[side] from the gathered per-rank records {rank, count, arrays, flags}.  The lower neighbour (side 0) sees this rank as ITS
+    upper neighbour and keeps that neighbour's progress in its flag [1]; the upper neighbour (side 1) in its flag [0].  On a ring of two
+    both sides are the same peer: this rank writes both of its flags and waits on both of its own."""
+    by_rank = {int(r["rank"]): r for r in infos}
+    links: List[Optional[FusedLink]] = []
+    for side in (0, 1):
+        peer = plan.neighbour(side)
+        if peer is None or peer == plan.rank:
+            links.append(None)
+            continue
+        r = by_rank[peer]
+        links.append(FusedLink(peer, int(r["count"]), tuple(r["arrays"]), tuple(r["flags"]), 1 - side))
+    return links
+
+
+def fused_step_ops(step: int, sides: Sequence[int]) -> List[tuple]:
+    """The stream-ordered operations of fused step number `step` (1, 2, ...) of one rank with neighbours on `sides`: wait until every
+    neighbour has finished step - 1 (it wrote this rank's ghost layers and read the arrays this step writes into), step, tell them."""
+    return [("wait", side, step - 1) for side in sides] + [("step", step)] + [("signal", side, step) for side in sides]
+
+
 class SlabDriver:
     """One rank's slab of a workload and its time stepping.
 
@@ -207,6 +244,59 @@ class SlabDriver:
                 begin(); self._transport(); self.deliver(array)
             self.sys.llg_slab_advance()
 
+    # ---- fused exchange between processes: neighbours' arrays mapped through CUDA IPC, order kept by flags in device memory
+    def setup_fused(self, dist, group=None) -> None:
+        """Collective over the group, once: exchange the IPC exports and map the neighbours' arrays and flags.  Needs the one-pass kernel on
+        every rank, one rank per GPU with peer access between neighbours, and ghost layers that are current (iterate primes them).
+        Every kernel that runs while a wait polls has run before: the flag kernels in spin_slab_flags, the step's kernels in the first
+        step, whose waits (for step 0) pass at once -- a kernel's first launch may load code, which waits for the device."""
+        if not self.one_pass:
+            raise ValueError("the fused exchange needs the one-pass kernel (spin_kernel_info: %s)" % self.sys.spin_kernel_info())
+        if not getattr(self, "_primed", False):
+            self.exchange_initial()
+            self._primed = True
+        self.synchronize()
+        cur, nxt = self.sys.spin_slab_arrays()
+        self._flags = self.sys.spin_slab_flags()
+        mine = {"rank": self.plan.rank, "count": self.plan.count, "arrays": (self.P.spin_ipc_export(cur), self.P.spin_ipc_export(nxt)),
+                "flags": self.P.spin_ipc_export(self._flags)}
+        infos = [None] * self.plan.world
+        dist.all_gather_object(infos, mine, group=group)
+        self._links = fused_links(self.plan, infos)
+        self._peer = []                       # per side: [address of its current array, of its next array, of the flag this rank writes]
+        opened = {}                           # (a ring of two: one peer on both sides, each export mapped once)
+        for link in self._links:
+            if link is None:
+                self._peer.append(None)
+                continue
+            addr = []
+            for handle, off in (link.arrays[0], link.arrays[1], link.flags):
+                key = (link.rank, handle)
+                if key not in opened:
+                    opened[key] = self.P.spin_ipc_open(handle, 0)
+                addr.append(opened[key] + off)
+            self._peer.append([addr[0], addr[1], addr[2] + 8 * link.signal_index])
+        self._fused_step = 0
+        dist.barrier(group=group)             # nobody steps before every mapping exists
+
+    def iterate_fused(self, n_steps: int) -> None:
+        """n fused steps of this rank (every rank calls it with the same n): no halo copy, no message, no host synchronisation"""
+        sides = [side for side in (0, 1) if self._peer[side] is not None]
+        for _ in range(int(n_steps)):
+            for op in fused_step_ops(self._fused_step + 1, sides):
+                if op[0] == "wait":
+                    self.sys.spin_flag_wait(self._flags + 8 * op[1], op[2])
+                elif op[0] == "signal":
+                    self.sys.spin_flag_signal(self._peer[op[1]][2], op[2])
+                else:
+                    lo, hi = self._peer
+                    self.sys.llg_slab_step_fused(lo[1] if lo else None, self._links[0].count if lo else 0, hi[1] if hi else None)
+                    self.sys.llg_slab_advance()
+                    for p in self._peer:      # the neighbours advanced too: their arrays swapped roles
+                        if p is not None:
+                            p[0], p[1] = p[1], p[0]
+            self._fused_step += 1
+
     def spins(self):
         self.synchronize()
         return self.sys.spins_get()
@@ -221,10 +311,15 @@ class LocalGroup:
     separate launches, B200_PROFILING.md).  The slabs advance in lockstep; a halo message is a device copy from the sender's send buffer
     into the receiver's receive buffer, ordered by the sender's event."""
 
-    def __init__(self, P, torch, w, world: int, options=()):
+    def __init__(self, P, torch, w, world: int, options=(), fused: bool = False):
+        """fused: steps by llg_slab_step_fused -- every slab's kernel writes its boundary planes straight into its neighbours' ghost layers
+        (here: other arrays of the same device; across GPUs: peer memory), no halo copies; needs the one-pass kernel and two slabs or more."""
         self.torch = torch
         self.drivers = [SlabDriver(P, torch, w, r, world, options=options) for r in range(world)]
         self._exchange(0, post=True)
+        self.fused = bool(fused) and world >= 2 and all(d.one_pass for d in self.drivers)
+        if fused and not self.fused:
+            raise ValueError("fused halo exchange needs the one-pass kernel on every slab and at least two slabs")
 
     def _move(self) -> None:
         for d in self.drivers:
@@ -254,7 +349,31 @@ class LocalGroup:
         for d in self.drivers:
             d.deliver(array)
 
+    def _iterate_fused(self, n_steps: int) -> None:
+        ds, Event = self.drivers, self.torch.cuda.Event
+        nxt = [d.sys.spin_slab_arrays() for d in ds]          # (current, next) device addresses; they swap at every advance
+        done = []
+        for d in ds:                                           # everything enqueued so far (priming copies, earlier steps) is a dependency
+            ev = Event(); ev.record(d.stream); done.append(ev)
+        for _ in range(int(n_steps)):
+            # a slab's step k + 1 needs its neighbours' step k: they wrote its ghost layers, and they read the arrays it now writes into
+            for i, d in enumerate(ds):
+                for side in (0, 1):
+                    p = d.plan.neighbour(side)
+                    if p is not None and p != i:
+                        d.stream.wait_event(done[p])
+            for i, d in enumerate(ds):
+                lo, hi = d.plan.neighbour(0), d.plan.neighbour(1)
+                d.sys.llg_slab_step_fused(nxt[lo][1] if lo is not None else None, ds[lo].plan.count if lo is not None else 0,
+                                          nxt[hi][1] if hi is not None else None)
+            for i, d in enumerate(ds):
+                d.sys.llg_slab_advance()
+                ev = Event(); ev.record(d.stream); done[i] = ev
+                nxt[i] = (nxt[i][1], nxt[i][0])
+
     def iterate(self, n_steps: int) -> None:
+        if self.fused:
+            return self._iterate_fused(n_steps)
         for _ in range(int(n_steps)):
             plans = [d.stages() for d in self.drivers]      # (every slab is in the same mode: the same Hamiltonian and options)
             for k in range(len(plans[0])):

@@ -1083,6 +1083,15 @@ def test_slab_decomposition_with_the_one_pass_kernel(P, O, cfg, cells, per_c, wo
     o = O.OracleSystem.from_workload(w)
     o.iterate(steps)
     assert np.abs(got - o.spins()).max() <= SPIN_ATOL
+    # the exchange fused into the kernel: boundary planes written straight into the neighbours' ghost layers, no halo copies at all;
+    # then a few copy-based steps on the same group (the ghost layers are current after either kind of step) and back
+    fus = S.LocalGroup(P, torch, w, world, options={"use_march": 2}, fused=True)
+    l0 = [d.sys.spin_launch_counts()[0] for d in fus.drivers]
+    fus.iterate(steps // 2)
+    assert [d.sys.spin_launch_counts()[0] - a for d, a in zip(fus.drivers, l0)] == [2 * (steps // 2)] * world      # one kernel + the step counter per step
+    fus.fused = False; fus.iterate(2); fus.fused = True
+    fus.iterate(steps - steps // 2 - 2)
+    assert np.array_equal(fus.spins(), ref.spins_get()), np.abs(fus.spins() - ref.spins_get()).max()
     # pinned spins or per-site moments: the slab falls back to the two-sweep kernels (it would need its neighbours' flags)
     grp2 = S.LocalGroup(P, torch, w, world, options={"use_march": 2})
     for d in grp2.drivers:
@@ -1090,6 +1099,36 @@ def test_slab_decomposition_with_the_one_pass_kernel(P, O, cfg, cells, per_c, wo
     assert not any("march" in d.sys.spin_kernel_info() for d in grp2.drivers)
     with pytest.raises(P.SpinError):
         grp2.drivers[0].sys.llg_slab_step(0)
+
+
+def test_slab_step_flags_and_ipc_export(P):
+    """The pieces of the fused exchange BETWEEN processes that one process can exercise: a flag wait enqueued before the signal that
+    releases it (two streams of one GPU; across GPUs the same kernels order the steps of neighbouring slabs), and the IPC export of a
+    slab's arrays (handle of the allocation + offset).  Mapping the export needs a second process and is not run on one GPU."""
+    w = W.config3().resized((64, 16, 16), 4)
+    a, b = P.SpinSystem.from_workload(w), P.SpinSystem.from_workload(w)
+    for s_ in (a, b):
+        s_.spin_set_slab(True, 0, 32, 1)
+        s_.spin_halo_doubles()                # builds the plan (a rebuild synchronises the stream: not with a wait pending on it)
+        s_.llg_slab_sweep(0, 0)               # every kernel used below has run once (a first launch may load code, which waits for the device)
+        s_.spin_slab_flags()
+        s_.spin_synchronize()
+    flags = a.spin_slab_flags()
+    assert flags == a.spin_slab_flags() and flags != b.spin_slab_flags()
+    a.spin_flag_wait(flags, 0)                # already true
+    a.spin_flag_wait(flags + 8, 3)            # a's stream now waits for its upper neighbour ...
+    a.llg_slab_sweep(0, 0)                    # (a sweep queued behind the wait)
+    b.spin_flag_signal(flags + 8, 3)          # ... which reports step 3 from another stream
+    b.spin_synchronize(); a.spin_synchronize()
+    a.spin_flag_wait(flags + 8, 2)            # flags only grow: an older step is still satisfied
+    a.spin_synchronize()
+    cur, nxt = a.spin_slab_arrays()
+    h, off = P.spin_ipc_export(cur)
+    h2, off2 = P.spin_ipc_export(cur + 4096)
+    assert len(h) == 64 and off >= 0 and h2 == h and off2 == off + 4096
+    assert P.spin_ipc_export(nxt) != (h, off)
+    hf, offf = P.spin_ipc_export(flags + 8)
+    assert len(hf) == 64 and offf >= 8
 
 
 def test_slab_reach_two_and_other_solvers(P, O):
