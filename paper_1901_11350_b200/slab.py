@@ -107,6 +107,18 @@ class DistTransport:
             w.wait()
 
 
+class StagedTransport(DistTransport):
+    """The same messages staged through host memory: for backends that move host tensors only (gloo) -- tests, or a node without NCCL."""
+
+    def sendrecv(self, plan: HaloPlan, send: Sequence, recv: Sequence):
+        hs = [None if t is None else t.cpu() for t in send]
+        hr = [None if t is None else t.cpu() for t in recv]
+        super().sendrecv(plan, hs, hr)
+        for d, h in zip(recv, hr):
+            if d is not None:
+                d.copy_(h)
+
+
 def exchange(plan: HaloPlan, get, put, send_buf, recv_buf, transport) -> None:
     """One halo exchange of one array: get(side, buffer) fills buffer with the own boundary planes of `side`; the transport moves
     send_buf[side] to the neighbour on that side, whose message arrives in recv_buf[side]; put(side, buffer) writes the ghost planes."""
@@ -245,7 +257,7 @@ class SlabDriver:
             self.sys.llg_slab_advance()
 
     # ---- fused exchange between processes: neighbours' arrays mapped through CUDA IPC, order kept by flags in device memory
-    def setup_fused(self, dist, group=None) -> None:
+    def setup_fused(self, dist, group=None, order: str = "flags") -> None:
         """Collective over the group, once: exchange the IPC exports and map the neighbours' arrays and flags.  Needs the one-pass kernel on
         every rank, one rank per GPU with peer access between neighbours, and ghost layers that are current (iterate primes them).
         Every kernel that runs while a wait polls has run before: the flag kernels in spin_slab_flags, the step's kernels in the first
@@ -277,17 +289,23 @@ class SlabDriver:
                 addr.append(opened[key] + off)
             self._peer.append([addr[0], addr[1], addr[2] + 8 * link.signal_index])
         self._fused_step = 0
+        # order = "host": a host barrier after every step instead of the flags (slow; for ranks that share a GPU, where a polling kernel
+        # of one rank would keep the other rank's kernels from running)
+        self._order, self._dist, self._group = order, dist, group
         dist.barrier(group=group)             # nobody steps before every mapping exists
 
     def iterate_fused(self, n_steps: int) -> None:
         """n fused steps of this rank (every rank calls it with the same n): no halo copy, no message, no host synchronisation"""
         sides = [side for side in (0, 1) if self._peer[side] is not None]
+        flags = self._order == "flags"
         for _ in range(int(n_steps)):
             for op in fused_step_ops(self._fused_step + 1, sides):
                 if op[0] == "wait":
-                    self.sys.spin_flag_wait(self._flags + 8 * op[1], op[2])
+                    if flags:
+                        self.sys.spin_flag_wait(self._flags + 8 * op[1], op[2])
                 elif op[0] == "signal":
-                    self.sys.spin_flag_signal(self._peer[op[1]][2], op[2])
+                    if flags:
+                        self.sys.spin_flag_signal(self._peer[op[1]][2], op[2])
                 else:
                     lo, hi = self._peer
                     self.sys.llg_slab_step_fused(lo[1] if lo else None, self._links[0].count if lo else 0, hi[1] if hi else None)
@@ -296,6 +314,9 @@ class SlabDriver:
                         if p is not None:
                             p[0], p[1] = p[1], p[0]
             self._fused_step += 1
+            if not flags:
+                self.synchronize()
+                self._dist.barrier(group=self._group)
 
     def spins(self):
         self.synchronize()

@@ -1131,6 +1131,60 @@ def test_slab_step_flags_and_ipc_export(P):
     assert len(hf) == 64 and offf >= 8
 
 
+def _fused_ipc_worker(rank, world, port, out, cells, per_c, steps, T):
+    import os
+    import torch
+    import torch.distributed as dist
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        import paper_1901_11350_b200 as P
+        from paper_1901_11350_b200 import slab as S
+        torch.cuda.set_device(0)
+        w = W.config3().resized(cells, steps)
+        w = dataclasses.replace(w, periodic=(w.periodic[0], w.periodic[1], per_c), T=T)
+        drv = S.SlabDriver(P, torch, w, rank, world, transport=S.StagedTransport(dist), options={"use_march": 2})
+        drv.setup_fused(dist, order="host")          # the ranks share one GPU here: host barriers, no polling kernels
+        drv.iterate_fused(steps)
+        parts = [None] * world
+        dist.all_gather_object(parts, drv.spins())
+        if rank == 0:
+            ref = P.SpinSystem.from_workload(w)
+            ref.spin_set_option("use_coop", 0); ref.spin_set_option("use_march", 2)
+            ref.llg_iterate(steps)
+            out.put(bool(np.array_equal(np.concatenate(parts, axis=0), ref.spins_get())))
+        dist.barrier()
+    finally:
+        dist.destroy_process_group()
+
+
+@pytest.mark.timeout(300)
+@pytest.mark.parametrize("cells,per_c,world,steps,T", [((64, 16, 24), 1, 2, 6, 10.0), ((64, 16, 27), 0, 3, 5, 0.0)])
+def test_fused_exchange_between_processes_through_cuda_ipc(cells, per_c, world, steps, T):
+    """One process per slab, all on this GPU: the neighbours' arrays are mapped through CUDA IPC (spin_ipc_export / spin_ipc_open) and each
+    process's kernel writes its boundary planes into them (llg_slab_step_fused).  The steps are ordered by host barriers here, not by the
+    flag kernels: processes that share a GPU must not run kernels that wait on one another.  Bit-identical to the single lattice."""
+    import torch.multiprocessing as mp
+    import socket
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    ctx = mp.get_context("spawn")
+    out = ctx.Queue()
+    procs = [ctx.Process(target=_fused_ipc_worker, args=(r, world, port, out, cells, per_c, steps, T)) for r in range(world)]
+    for p in procs:
+        p.start()
+    try:
+        assert out.get(timeout=240) is True
+    finally:
+        for p in procs:
+            p.join(30)
+            if p.is_alive():
+                p.kill()
+    assert all(p.exitcode == 0 for p in procs), [p.exitcode for p in procs]
+
+
 def test_slab_reach_two_and_other_solvers(P, O):
     """Pairs reaching two planes along c (ghost width 2) and the Heun / SIB solvers on slabs; llg_iterate refuses a slab."""
     import torch
