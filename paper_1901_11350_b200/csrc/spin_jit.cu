@@ -86,7 +86,14 @@ int sm_count(const spin_system *s) {
 // shapes measured on B200 (profiles/r1c_README.md, profiles/r2_README.md: 32x2x2, 32x4x1, 64x2x1, 32x2x4, 32x8x2, ... are 0.5-18 % slower)
 static void jit_brick(const spin_system *s, int b[3]) {
     const bool flat = s->nc[2] < 2;
-    b[0] = 32; b[1] = flat ? 8 : 4; b[2] = flat ? 1 : 2;
+    b[0] = 32; b[1] = 4; b[2] = flat ? 1 : 2;
+    // flat lattices: bricks of 32 x 4 (128 threads) spread a sweep over more SMs than 32 x 8 did (cfg4 35.8 -> 33.6, cfg1 3.39 -> 3.13 us
+    // per step, cfg2 unchanged; 32 x 2: 33.8 / 3.25 / 15.1); 32 x 8 is kept where only that fits the one-cluster kernel (16 blocks)
+    if (flat) {
+        const int nbx = (s->nc[0] + 31) / 32;
+        const long items4 = (long)nbx * ((s->nc[1] + 3) / 4) * s->nb, items8 = (long)nbx * ((s->nc[1] + 7) / 8) * s->nb;
+        if (items4 > 16 && items8 <= 16) b[1] = 8;
+    }
 }
 static void jit_brick_launch(const spin_system *s, dim3 &grid, dim3 &block);
 // programmatic dependent launch of the brick sweeps: 0 off, 1 dependents released at entry, 2 at the end of each block.
