@@ -264,18 +264,21 @@ class SlabDriver:
         step, whose waits (for step 0) pass at once -- a kernel's first launch may load code, which waits for the device."""
         if not self.one_pass:
             raise ValueError("the fused exchange needs the one-pass kernel (spin_kernel_info: %s)" % self.sys.spin_kernel_info())
+        if getattr(self, "_links", None) is not None:
+            return                            # set up already: the mappings and the step count of the flags stay
         if not getattr(self, "_primed", False):
             self.exchange_initial()
             self._primed = True
         self.synchronize()
         cur, nxt = self.sys.spin_slab_arrays()
+        self._cur0 = cur                      # which of the two arrays was the current one at set-up: the same on every rank (lockstep)
         self._flags = self.sys.spin_slab_flags()
         mine = {"rank": self.plan.rank, "count": self.plan.count, "arrays": (self.P.spin_ipc_export(cur), self.P.spin_ipc_export(nxt)),
                 "flags": self.P.spin_ipc_export(self._flags)}
         infos = [None] * self.plan.world
         dist.all_gather_object(infos, mine, group=group)
         self._links = fused_links(self.plan, infos)
-        self._peer = []                       # per side: [address of its current array, of its next array, of the flag this rank writes]
+        self._peer = []                       # per side: [address of its current-at-set-up array, of its other array, of the flag this rank writes]
         opened = {}                           # (a ring of two: one peer on both sides, each export mapped once)
         for link in self._links:
             if link is None:
@@ -298,6 +301,8 @@ class SlabDriver:
         """n fused steps of this rank (every rank calls it with the same n): no halo copy, no message, no host synchronisation"""
         sides = [side for side in (0, 1) if self._peer[side] is not None]
         flags = self._order == "flags"
+        # every rank advances in lockstep (copy-based steps in between included), so the neighbours' arrays have the roles this rank's have
+        swapped = self.sys.spin_slab_arrays()[0] != self._cur0
         for _ in range(int(n_steps)):
             for op in fused_step_ops(self._fused_step + 1, sides):
                 if op[0] == "wait":
@@ -308,11 +313,10 @@ class SlabDriver:
                         self.sys.spin_flag_signal(self._peer[op[1]][2], op[2])
                 else:
                     lo, hi = self._peer
-                    self.sys.llg_slab_step_fused(lo[1] if lo else None, self._links[0].count if lo else 0, hi[1] if hi else None)
+                    nxt = 0 if swapped else 1             # the neighbours' NEXT array
+                    self.sys.llg_slab_step_fused(lo[nxt] if lo else None, self._links[0].count if lo else 0, hi[nxt] if hi else None)
                     self.sys.llg_slab_advance()
-                    for p in self._peer:      # the neighbours advanced too: their arrays swapped roles
-                        if p is not None:
-                            p[0], p[1] = p[1], p[0]
+                    swapped = not swapped
             self._fused_step += 1
             if not flags:
                 self.synchronize()

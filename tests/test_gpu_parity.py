@@ -1146,7 +1146,10 @@ def _fused_ipc_worker(rank, world, port, out, cells, per_c, steps, T):
         w = dataclasses.replace(w, periodic=(w.periodic[0], w.periodic[1], per_c), T=T)
         drv = S.SlabDriver(P, torch, w, rank, world, transport=S.StagedTransport(dist), options={"use_march": 2})
         drv.setup_fused(dist, order="host")          # the ranks share one GPU here: host barriers, no polling kernels
-        drv.iterate_fused(steps)
+        drv.iterate_fused(2)
+        drv.iterate(1)                               # a copy-based step in between (messages staged through the host): the arrays swap roles
+        drv.setup_fused(dist, order="host")          # (idempotent)
+        drv.iterate_fused(steps - 3)
         parts = [None] * world
         dist.all_gather_object(parts, drv.spins())
         if rank == 0:
