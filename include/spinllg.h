@@ -218,8 +218,8 @@ int spin_halo_put(spin_system *sys, int array, int side, const double *src_devic
 int llg_slab_sweep(spin_system *sys, int stage, int part);
 /* after the corrector sweeps: the next configuration becomes current, the step counter (noise stream) advances by one             */
 int llg_slab_advance(spin_system *sys);
-/* The whole Depondt step of a slab in ONE pass (the plane-marching kernel; available when spin_kernel_info reports "jit+march": one basis
- * atom, Depondt, no pinned spins or per-site moments, slab of at least 32 x 8 x 8 cells): the kernel recomputes the predictor of the
+/* The whole step of a slab in ONE pass (the plane-marching kernel; available when spin_kernel_info reports "jit+march": one basis
+ * atom, Depondt or Heun, no pinned spins or per-site moments, slab of at least 32 x 8 x 8 cells): the kernel recomputes the predictor of the
  * neighbours' boundary planes itself, so a step needs ONE halo exchange of depth 2 x reach (of the new configuration, array 2, before
  * llg_slab_advance) instead of two of depth reach.  spin_halo_doubles reports the depth in use.  part 0: the whole slab; 1: the first and
  * last chunk of planes, which hold everything the neighbours need; 2: the chunks in between (launched after the halo copies of part 1
@@ -267,6 +267,9 @@ int spin_flag_wait(spin_system *sys, const unsigned long long *flag, unsigned lo
  *                    fused dipolar path that way (their prologue overlaps the previous kernel's tail)
  *   store_A     (0)  1: the predictor stores the rotation field A(n) and the corrector reads it instead of recomputing it
  *   cache_noise (1)  the predictor keeps the thermal field of the step (24 B/spin) for the corrector instead of generating it twice
+ *   use_march   (1)  3-D lattices of one basis atom (>= 32 x 8 x 8 cells, >= 65536 spins) advanced by Depondt or Heun without dipolar coupling
+ *                    take the one-pass plane-marching kernel: the whole step in one launch, n^p never written to memory; 0: brick sweeps;
+ *                    2: also for smaller lattices (tests)
  *   ddi_slab    (1)  thin films (up to 8 planes; 4 with several basis atoms) take the dipolar slab path: hand-written transforms along a and, for one
  *                    basis atom and power-of-two columns, one fused kernel for the transforms along b and c and the contraction;
  *                    3: cuFFT's transform along b and a separate contraction kernel; 2: cuFFT's transforms along a and b; 0: the general

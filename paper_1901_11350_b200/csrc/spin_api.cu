@@ -163,13 +163,14 @@ int stt_coefficients(const spin_system *s, double cd[3]) {
 }
 
 }  // namespace
-// The one-pass plane-marching Depondt kernel (spin_jit_march.cuh) applies to 3-D lattices of one basis atom advanced by the Depondt solver
-// without dipolar coupling or images; lattices small enough for the all-steps-in-one-launch path keep that path.  A slab of a decomposed
+// The one-pass plane-marching kernel (spin_jit_march.cuh) applies to 3-D lattices of one basis atom advanced by the Depondt or the Heun
+// solver (the two-stage explicit schemes: predictor from n, corrector from n and n^p) without dipolar coupling or images; lattices small enough for the all-steps-in-one-launch path keep that path.  A slab of a decomposed
 // lattice takes it too (llg_slab_step: ONE halo exchange of depth 2 x reach per step instead of two of depth reach) unless it has pinned
 // spins or per-site moments: the kernel recomputes the predictor of the neighbours' boundary planes and would need their flags.
 bool spin::march_eligible(const spin_system *s) {
     if (s->slab_on && (s->d_pin || !s->mu_site.empty())) return false;
-    return s->opt_march && s->opt_jit && s->nb == 1 && s->solver == SPIN_SOLVER_DEPONDT && !s->ddi_on && s->n_img == 1 && !s->opt_store_A &&
+    return s->opt_march && s->opt_jit && s->nb == 1 && (s->solver == SPIN_SOLVER_DEPONDT || s->solver == SPIN_SOLVER_HEUN) && !s->ddi_on && s->n_img == 1 &&
+           !s->opt_store_A &&
            s->nc[0] >= 32 && s->nc[1] >= 8 && s->nc[2] >= 8 && (s->opt_march >= 2 || s->N >= 65536);
 }
 namespace {

@@ -36,7 +36,7 @@ constexpr int RN = 2 * RC + 1 + LOOK, RP = 2 * RC + 2;           // ring depths:
 constexpr int RIM = 2 * RA * PY, RIMW = (RIM + 31) / 32;         // sites of the rim columns, warps that take them
 constexpr int NWARP = PY + RIMW, NTHREADS = 32 * NWARP;
 constexpr int NTX = (spec::NA + 31) / 32, NTY = (spec::NB + TY - 1) / TY;
-static_assert(spec::NBASIS == 1 && spec::SOLVER == 0 && !spec::HAS_DDI && !spec::MULTI_IMAGE, "one-pass kernel: one basis atom, Depondt, no dipolar term");
+static_assert(spec::NBASIS == 1 && (spec::SOLVER == 0 || spec::SOLVER == 1) && !spec::HAS_DDI && !spec::MULTI_IMAGE, "one-pass kernel: one basis atom, Depondt or Heun, no dipolar term");
 static_assert(spec::RA == 2 * RA && spec::RB == 2 * RB && spec::RC == 2 * RC, "ghost layers must be twice the reach");
 
 extern __shared__ __align__(128) double smem[];
@@ -159,7 +159,8 @@ extern "C" __global__ void __launch_bounds__(spinmarch::NTHREADS, spec::MBLOCKS)
                     force<0, 1>(acc, own, F, zr);
                     if constexpr (spec::STT_ON) stt_gradient<0, 1>(acc, c, own, sg);
                     rotation_field<0>(own[0], F[0], sg[0], A_cur, ir);
-                    spin::rodrigues(A_cur, specc::DT, specc::DT2, own[0], out);                 // B5
+                    if constexpr (spec::SOLVER == 1) { out[0] = own[0][0]; out[1] = own[0][1]; out[2] = own[0][2]; spin::heun_add(own[0], A_cur, specc::DT, out); }   // Heun, B3
+                    else spin::rodrigues(A_cur, specc::DT, specc::DT2, own[0], out);             // Depondt, B5
                 }
             }
             pslot[pcell] = out[0]; pslot[pcell + PX] = out[1]; pslot[pcell + 2 * PX] = out[2];
@@ -181,9 +182,16 @@ extern "C" __global__ void __launch_bounds__(spinmarch::NTHREADS, spec::MBLOCKS)
                 force<0, 1>(acc, own, F, zr);
                 if constexpr (spec::STT_ON) stt_gradient<0, 1>(acc, c, own, sg);
                 rotation_field<0>(own[0], F[0], sg[0], Ap, ir);
-                const double Ac[3] = {A_q[0][0] + Ap[0], A_q[0][1] + Ap[1], A_q[0][2] + Ap[2]};
-                spin::rodrigues(Ac, specc::HDT, specc::QDT2, n_q[0], o);                          // B6-B7: R((A + A^p) / 2) n(t)
-                spin::renormalise(o);
+                if constexpr (spec::SOLVER == 1) {                                                // Heun, B4: n + dt/2 (n x A + n^p x A^p), renormalised
+                    o[0] = n_q[0][0]; o[1] = n_q[0][1]; o[2] = n_q[0][2];
+                    spin::heun_add(n_q[0], A_q[0], specc::HDT, o);
+                    spin::heun_add(own[0], Ap, specc::HDT, o);
+                    spin::renormalise_general(o);
+                } else {
+                    const double Ac[3] = {A_q[0][0] + Ap[0], A_q[0][1] + Ap[1], A_q[0][2] + Ap[2]};
+                    spin::rodrigues(Ac, specc::HDT, specc::QDT2, n_q[0], o);                      // Depondt, B6-B7: R((A + A^p) / 2) n(t)
+                    spin::renormalise(o);
+                }
             }
             const size_t in_plane = (size_t)(c.ib + spec::LB) * ROW + (c.ia + spec::LA);
             store_spin(nout + ((size_t)(zC + spec::LC) * PLANE + in_plane), c, o);

@@ -1242,6 +1242,36 @@ def test_one_pass_marching_step_is_bit_identical(P, O, cfg, cells, per, T, steps
     assert np.array_equal(h.spins_get(), g.spins_get())
 
 
+@pytest.mark.parametrize("cells,per,T,steps", [((64, 32, 16), (1, 1, 1), 0.0, 30), ((70, 19, 21), (1, 0, 0), 12.0, 20)])
+def test_one_pass_marching_step_heun(P, O, cells, per, T, steps):
+    """The Heun solver (App. B) has the same two-stage structure and takes the one-pass kernel too: bit-identical to its brick sweeps, on
+    one lattice and on slabs with the exchange fused into the kernel."""
+    import torch
+    from paper_1901_11350_b200 import slab as S
+    w = dataclasses.replace(W.config3().resized(cells, steps), periodic=per, T=T)
+    g, o = pair(P, O, w)
+    g.llg_set_solver(1); o.set_solver(1)
+    g.spin_set_option("use_march", 2)
+    assert g.spin_kernel_info() == "jit+march", g.spin_kernel_info()
+    g.llg_iterate(steps); o.iterate(steps)
+    assert np.abs(g.spins_get() - o.spins()).max() <= SPIN_ATOL
+    b = P.SpinSystem.from_workload(w)
+    b.llg_set_solver(1); b.spin_set_option("use_march", 0); b.spin_set_option("use_coop", 0)
+    assert b.spin_kernel_info() == "jit (brick sweeps)"
+    b.llg_iterate(steps)
+    assert np.array_equal(b.spins_get(), g.spins_get())
+    if cells[2] >= 16:
+        grp = S.LocalGroup(P, torch, w, 2, options={"use_march": 2}, fused=True)
+        for d in grp.drivers:
+            d.sys.llg_set_solver(1)               # (same layout: the arrays and their ghost layers stay)
+        assert all("march" in d.sys.spin_kernel_info() for d in grp.drivers)
+        grp.iterate(steps)
+        assert np.array_equal(grp.spins(), g.spins_get())
+    for solver in (2, 3):                      # SIB and RK4 keep their own kernels
+        h = P.SpinSystem.from_workload(w); h.llg_set_solver(solver); h.spin_set_option("use_march", 2)
+        assert "march" not in h.spin_kernel_info()
+
+
 def test_one_pass_marching_step_with_pins_moments_current_and_long_reach(P, O):
     """Pinned spins and vacancies, per-site moments, a current with all three components, pairs reaching two sites along every direction."""
     w = W.config3().resized((48, 20, 16), 20)
