@@ -1296,6 +1296,33 @@ def test_one_pass_marching_step_with_pins_moments_current_and_long_reach(P, O):
     assert np.array_equal(b.spins_get(), g.spins_get())
 
 
+def test_largest_lattice_by_translation_invariance(P):
+    """Maximum size: 512^3 = 134,217,728 spins (3.2 GB per array; the padded arrays stay below the 2^31 doubles of the 32-bit site index).
+    The oracle cannot step that in seconds, but a property can: a periodic lattice at T = 0 that starts as 16 x 16 x 16 copies of a 32^3
+    configuration is, site by site, the same problem as the periodic 32^3 lattice, so after any number of steps every copy must equal
+    the small lattice's result BIT FOR BIT (the small lattice is compared with the oracle elsewhere).  One size further is refused."""
+    small = dataclasses.replace(W.config3().resized((32, 32, 32), 3), periodic=(1, 1, 1), T=0.0)
+    gs = P.SpinSystem.from_workload(small)
+    n0 = small.initial_spins()
+    gs.llg_iterate(3)
+    ref = gs.spins_get().reshape(32, 32, 32, 3)
+    big = dataclasses.replace(small, n_cells=(512, 512, 512))
+    g = P.SpinSystem.from_workload(big, set_spins=False)
+    assert g.spin_kernel_info() == "jit+march" and g.N == 512 ** 3
+    g.spins_set(np.tile(n0.reshape(32, 32, 32, 3), (16, 16, 16, 1)).reshape(-1, 3))
+    g.llg_iterate(3)
+    out = g.spins_get().reshape(512, 512, 512, 3)
+    g.close()
+    rng = np.random.default_rng(3)
+    blocks = [(0, 0, 0), (15, 15, 15), (0, 15, 7)] + [tuple(int(x) for x in rng.integers(0, 16, 3)) for _ in range(9)]
+    for kc, kb, ka in blocks:
+        assert np.array_equal(out[32 * kc:32 * kc + 32, 32 * kb:32 * kb + 32, 32 * ka:32 * ka + 32], ref), (kc, kb, ka)
+    assert np.array_equal(out[::32, ::32, ::32], np.broadcast_to(ref[0, 0, 0], (16, 16, 16, 3)))          # one site of every copy
+    assert np.abs(np.linalg.norm(out[:, :, 100], axis=-1) - 1).max() < 4e-16
+    with pytest.raises(P.SpinError, match="too large"):
+        P.SpinSystem(np.eye(3), [[0, 0, 0]], (1024, 1024, 1024), (1, 1, 1), 1.0)
+
+
 def test_full_size_cfg3_takes_the_one_pass_kernel(P):
     g = P.SpinSystem.from_workload(W.config3(), set_spins=False)
     assert g.spin_kernel_info() == "jit+march"
