@@ -241,6 +241,8 @@ def measure_workload(P, torch, w, stream, steps, warmup, min_seconds, barrier=No
         # the whole Depondt step is ONE kernel (n^p never leaves the SM): one launch = one iteration.  The roofline figure stays the method's
         # 120 B per spin-update (read n, write n^p; read n^p, read n, write n); the kernel's own DRAM traffic (`traffic`, about
         # 43 B per spin-update) is lower because it skips the n^p round trip and the second read of n.
+        step_bytes = 120 * N                 # (the thermal field costs the method no traffic: regenerated from counters)
+        roof["step_algorithmic_bytes"], roof["step_effective_gbs"] = step_bytes, step_bytes / (ms_iter * 1e-3) / 1e9
         kernel, nbytes = "jit_depondt_march", step_bytes
         share, launch_ms = 1.0, ms_iter
         roof["note"] = "one-pass plane-marching kernel: one launch per Depondt iteration; algorithmic bytes of the two-sweep method (120 B per spin-update)"

@@ -267,8 +267,8 @@ int spin_flag_wait(spin_system *sys, const unsigned long long *flag, unsigned lo
  *                    fused dipolar path that way (their prologue overlaps the previous kernel's tail)
  *   store_A     (0)  1: the predictor stores the rotation field A(n) and the corrector reads it instead of recomputing it
  *   cache_noise (1)  the predictor keeps the thermal field of the step (24 B/spin) for the corrector instead of generating it twice
- *   use_march   (1)  3-D lattices of one basis atom (>= 32 x 8 x 8 cells, >= 65536 spins) advanced by Depondt or Heun without dipolar coupling
- *                    take the one-pass plane-marching kernel: the whole step in one launch, n^p never written to memory; 0: brick sweeps;
+ *   use_march   (1)  lattices of one basis atom, 3-D (>= 32 x 8 x 8 cells) or flat (one plane), from 65536 spins on, advanced by Depondt or Heun
+ *                    without dipolar coupling take the one-pass kernel: the whole step in one launch, n^p never written to memory; 0: brick sweeps;
  *                    2: also for smaller lattices (tests)
  *   ddi_slab    (1)  thin films (up to 8 planes; 4 with several basis atoms) take the dipolar slab path: hand-written transforms along a and, for one
  *                    basis atom and power-of-two columns, one fused kernel for the transforms along b and c and the contraction;

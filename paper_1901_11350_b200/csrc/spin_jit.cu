@@ -124,7 +124,8 @@ bool plan_march(const spin_system *s, MarchGeo &g) {
     const DevicePlan &P = s->plan;
     if (!spin::march_eligible(s) || P.ghost_mult != 2) return false;
     g.ra = P.rA / 2; g.rb = P.rB / 2; g.rc = P.rC / 2;
-    if (g.rc < 1 || g.ra > 4 || g.rb > 4 || g.rc > 2) return false;
+    const bool flat = P.Nc == 1;      // one plane: nothing to march along, the kernel is "predictor of tile + rim, corrector of the tile"
+    if ((g.rc < 1 && !flat) || g.ra > 4 || g.rb > 4 || g.rc > 2) return false;
     const int hx = (2 * g.ra + 1) / 2 * 2;
     if (P.LA < hx) return false;
     const int sms = sm_count(s);
@@ -140,7 +141,7 @@ bool plan_march(const spin_system *s, MarchGeo &g) {
         const int per_sm = (int)std::min<size_t>((size_t)(227 * 1024) / (smem + 1024), (size_t)std::min(2048 / threads, 65536 / (threads * 56)));
         if (per_sm < 1) continue;
         const int cols = ((P.Na + 31) / 32) * ((P.Nb + ty - 1) / ty), slots = sms * per_sm;
-        for (int nzc = 1; nzc <= P.Nc / 4; ++nzc) {
+        for (int nzc = 1; nzc <= (flat ? 1 : P.Nc / 4); ++nzc) {
             const long items = (long)cols * nzc;
             const long waves = (items + slots - 1) / slots;
             const double cz = (double)P.Nc / nzc;

@@ -118,10 +118,12 @@ extern "C" __global__ void __launch_bounds__(spinmarch::NTHREADS, spec::MBLOCKS)
     c.ib = gy < 0 ? gy + spec::NB : (gy >= spec::NB ? gy - spec::NB : gy);
     const int ncell = ((sy + 2 * RB) * 3) * NX + (sx + HX);       // x component of the own site in a staged n plane
     const int pcell = ((sy + RB) * 3) * PX + (sx + RA);           // the same in an n^p plane
-    // what the corrector of plane zC needs from the predictor of the same site, RC iterations earlier
-    double n_q[RC][3], A_q[RC][3], th_q[RC][3];
+    // what the corrector of plane zC needs from the predictor of the same site, RC iterations earlier (flat lattices, RC = 0: the one
+    // plane there is -- the predictor's values of this very iteration, and the queue is not used)
+    constexpr int QD = RC > 0 ? RC : 1;
+    double n_q[QD][3], A_q[QD][3], th_q[QD][3];
 #pragma unroll
-    for (int r = 0; r < RC; ++r)
+    for (int r = 0; r < QD; ++r)
 #pragma unroll
         for (int k = 0; k < 3; ++k) { n_q[r][k] = 0.0; A_q[r][k] = 0.0; th_q[r][k] = 0.0; }
 #pragma unroll
@@ -165,6 +167,10 @@ extern "C" __global__ void __launch_bounds__(spinmarch::NTHREADS, spec::MBLOCKS)
             }
             pslot[pcell] = out[0]; pslot[pcell + PX] = out[1]; pslot[pcell + 2 * PX] = out[2];
         }
+        if constexpr (RC == 0) {
+#pragma unroll
+            for (int q = 0; q < 3; ++q) { n_q[0][q] = n_cur[q]; A_q[0][q] = A_cur[q]; th_q[0][q] = th_cur[q]; }
+        }
         __syncthreads();                                           // n^p(zP) is complete; nobody reads n plane k any more
         if (tid == 0 && k + RN - 1 < NP) issue(k + RN - 1);        // refill a free slot, LOOK planes ahead of the next predictor
         const int zC = zP - RC;
@@ -205,12 +211,14 @@ extern "C" __global__ void __launch_bounds__(spinmarch::NTHREADS, spec::MBLOCKS)
             }
         }
         // the queue moves on: slot 0 is the oldest (the plane the next corrector takes)
+        if constexpr (RC > 0) {
 #pragma unroll
-        for (int r = 0; r + 1 < RC; ++r)
+            for (int r = 0; r + 1 < RC; ++r)
 #pragma unroll
-            for (int q = 0; q < 3; ++q) { n_q[r][q] = n_q[r + 1][q]; A_q[r][q] = A_q[r + 1][q]; th_q[r][q] = th_q[r + 1][q]; }
+                for (int q = 0; q < 3; ++q) { n_q[r][q] = n_q[r + 1][q]; A_q[r][q] = A_q[r + 1][q]; th_q[r][q] = th_q[r + 1][q]; }
 #pragma unroll
-        for (int q = 0; q < 3; ++q) { n_q[RC - 1][q] = n_cur[q]; A_q[RC - 1][q] = A_cur[q]; th_q[RC - 1][q] = th_cur[q]; }
+            for (int q = 0; q < 3; ++q) { n_q[QD - 1][q] = n_cur[q]; A_q[QD - 1][q] = A_cur[q]; th_q[QD - 1][q] = th_cur[q]; }
+        }
         if (++ns == RN) ns = 0;
         if (++ps == RP) ps = 0;
         if (++wslot == RN) { wslot = 0; wpar ^= 1; }

@@ -1218,6 +1218,10 @@ MARCH_CASES = [
     (3, (40, 24, 12), (0, 0, 0), 0.0, 30),        # open everywhere
     (3, (96, 16, 24), (1, 1, 0), 10.0, 20),       # open along c (the marching direction)
     (5, (64, 24, 10), (1, 1, 0), 0.0, 20),        # film Hamiltonian without the dipolar term
+    # flat lattices (one plane): nothing to march along -- predictor of tile + rim into shared memory, corrector of the tile, one launch
+    (2, (70, 37, 1), (1, 1, 0), 10.0, 30),        # triangular, three shells (reach 2), thermal field, ragged tiles
+    (1, (64, 40, 1), (1, 1, 0), 0.0, 40),         # square lattice with DMI and anisotropy
+    (2, (96, 33, 1), (0, 1, 0), 0.0, 30),         # open along a
 ]
 
 
@@ -1326,3 +1330,6 @@ def test_largest_lattice_by_translation_invariance(P):
 def test_full_size_cfg3_takes_the_one_pass_kernel(P):
     g = P.SpinSystem.from_workload(W.config3(), set_spins=False)
     assert g.spin_kernel_info() == "jit+march"
+    assert P.SpinSystem.from_workload(W.config2(), set_spins=False).spin_kernel_info() == "jit+march"          # flat, one basis atom, 65536 spins
+    assert P.SpinSystem.from_workload(W.config1(), set_spins=False).spin_kernel_info() == "jit+cluster"        # small: all steps in one launch
+    assert P.SpinSystem.from_workload(W.config4(), set_spins=False).spin_kernel_info() == "jit (brick sweeps)"  # two basis atoms
