@@ -637,6 +637,7 @@ def test_cooperative_kernel_matches_two_launch_path(P, O, cfg, cells, steps):
         a = P.SpinSystem.from_workload(w); b = P.SpinSystem.from_workload(w)
         for s_ in (a, b):
             s_.llg_set_solver(solver); s_.spins_set_pinned(mask if solver == 1 else None)
+            s_.spin_set_option("use_march", 0)          # (the full-size cfg2 lattice would take the one-pass kernel otherwise)
         a.spin_set_option("use_coop", 2)
         b.spin_set_option("use_coop", 0)
         assert a.spin_kernel_info() in ("jit+coop", "jit+cluster") and b.spin_kernel_info().startswith("jit (brick"), (a.spin_kernel_info(), b.spin_kernel_info())
@@ -644,7 +645,7 @@ def test_cooperative_kernel_matches_two_launch_path(P, O, cfg, cells, steps):
         assert np.array_equal(a.spins_get(), b.spins_get()), solver
     o = O.OracleSystem.from_workload(w)
     g = P.SpinSystem.from_workload(w)
-    g.spin_set_option("use_coop", 2)
+    g.spin_set_option("use_coop", 2); g.spin_set_option("use_march", 0)
     n_o = min(steps, 200)
     g.llg_iterate(n_o); o.iterate(n_o)
     assert np.abs(g.spins_get() - o.spins()).max() <= SPIN_ATOL
