@@ -171,7 +171,7 @@ bool spin::march_eligible(const spin_system *s) {
     if (s->slab_on && (s->d_pin || !s->mu_site.empty())) return false;
     return s->opt_march && s->opt_jit && s->nb == 1 && (s->solver == SPIN_SOLVER_DEPONDT || s->solver == SPIN_SOLVER_HEUN) && !s->ddi_on && s->n_img == 1 &&
            !s->opt_store_A &&
-           s->nc[0] >= 32 && s->nc[1] >= 8 && (s->nc[2] >= 8 || s->nc[2] == 1) && (s->opt_march >= 2 || s->N >= 65536);
+           s->nc[0] >= 32 && s->nc[1] >= 8 && (s->nc[2] >= 8 || s->nc[2] == 1) && (s->opt_march >= 2 || s->N >= (s->nc[2] == 1 ? 8192 : 65536));
 }
 namespace {
 int build_plan(const spin_system *s, DevicePlan &P) {

@@ -126,6 +126,10 @@ bool plan_march(const spin_system *s, MarchGeo &g) {
     g.ra = P.rA / 2; g.rb = P.rB / 2; g.rc = P.rC / 2;
     const bool flat = P.Nc == 1;      // one plane: nothing to march along, the kernel is "predictor of tile + rim, corrector of the tile"
     if ((g.rc < 1 && !flat) || g.ra > 4 || g.rb > 4 || g.rc > 2) return false;
+    // flat lattices: one launch instead of two always pays while the step is latency-bound (cfg2 Hamiltonian, reach 2, thermal field:
+    // 96^2 .. 256^2 sites 7.3-7.4 us against 8.2-9.3); at 512^2 the rim of two reaches (1.41 x the predictor work) loses to the brick
+    // sweeps (25.4 against 21.6 us), with a reach of one it does not (cfg1 Hamiltonian: 7.9 against 8.6; 1024^2: 23.3 / 23.5)
+    if (flat && s->opt_march < 2 && s->N > 131072 && std::max(g.ra, g.rb) > 1) return false;
     const int hx = (2 * g.ra + 1) / 2 * 2;
     if (P.LA < hx) return false;
     const int sms = sm_count(s);
