@@ -291,11 +291,21 @@ class SlabDriver:
                     opened[key] = self.P.spin_ipc_open(handle, 0)
                 addr.append(opened[key] + off)
             self._peer.append([addr[0], addr[1], addr[2] + 8 * link.signal_index])
+        self._opened = list(opened.values())
         self._fused_step = 0
         # order = "host": a host barrier after every step instead of the flags (slow; for ranks that share a GPU, where a polling kernel
         # of one rank would keep the other rank's kernels from running)
         self._order, self._dist, self._group = order, dist, group
         dist.barrier(group=group)             # nobody steps before every mapping exists
+
+    def close_fused(self) -> None:
+        """unmap the neighbours' arrays (after the last fused step of every rank; the systems themselves stay usable)"""
+        if getattr(self, "_links", None) is None:
+            return
+        self.synchronize()
+        for base in getattr(self, "_opened", []):
+            self.P.spin_ipc_close(base, 0)
+        self._opened, self._links, self._peer = [], None, None
 
     def iterate_fused(self, n_steps: int) -> None:
         """n fused steps of this rank (every rank calls it with the same n): no halo copy, no message, no host synchronisation"""

@@ -1153,6 +1153,8 @@ def _fused_ipc_worker(rank, world, port, out, cells, per_c, steps, T):
         drv.iterate_fused(steps - 3)
         parts = [None] * world
         dist.all_gather_object(parts, drv.spins())
+        dist.barrier()
+        drv.close_fused()                            # every rank is through: unmap the neighbours' arrays
         if rank == 0:
             ref = P.SpinSystem.from_workload(w)
             ref.spin_set_option("use_coop", 0); ref.spin_set_option("use_march", 2)
