@@ -169,7 +169,9 @@ int stt_coefficients(const spin_system *s, double cd[3]) {
 // spins or per-site moments: the kernel recomputes the predictor of the neighbours' boundary planes and would need their flags.
 bool spin::march_eligible(const spin_system *s) {
     if (s->slab_on && (s->d_pin || !s->mu_site.empty())) return false;
-    return s->opt_march && s->opt_jit && s->nb == 1 && (s->solver == SPIN_SOLVER_DEPONDT || s->solver == SPIN_SOLVER_HEUN) && !s->ddi_on && s->n_img == 1 &&
+    // (several basis atoms, up to four: only on request, use_march = 2 -- measured on cfg4)
+    const bool basis_ok = s->nb == 1 || (s->nb <= 4 && s->opt_march >= 2 && !s->slab_on);
+    return s->opt_march && s->opt_jit && basis_ok && (s->solver == SPIN_SOLVER_DEPONDT || s->solver == SPIN_SOLVER_HEUN) && !s->ddi_on && s->n_img == 1 &&
            !s->opt_store_A &&
            s->nc[0] >= 32 && s->nc[1] >= 8 && (s->nc[2] >= 8 || s->nc[2] == 1) && (s->opt_march >= 2 || s->N >= (s->nc[2] == 1 ? 8192 : 65536));
 }

@@ -34,7 +34,7 @@ struct JitState {
     cudaKernel_t k_march;
     int march_ty, march_nzc, march_threads, march_items;
     size_t march_smem;
-    CUtensorMap tm_march[2];          // n[0], n[1] with the staged plane of the kernel as box
+    CUtensorMap tm_march[2][SPIN_MAX_BASIS];      // n[0], n[1], per sublattice, with the staged plane of the kernel as box (the kernel takes nb of them)
     // all steps in one cooperative launch (launch-bound lattices)
     bool coop;
     cudaKernel_t k_coop;
@@ -140,7 +140,7 @@ bool plan_march(const spin_system *s, MarchGeo &g) {
         const int py = ty + 2 * g.rb, rimw = (2 * g.ra * py + 31) / 32, threads = 32 * (py + rimw);
         if (threads > 1024) continue;
         const size_t nslot = ((size_t)3 * (32 + 2 * hx) * (ty + 4 * g.rb) + 15) / 16 * 16, ppl = (size_t)3 * (32 + 2 * g.ra) * py;
-        const size_t smem = ((size_t)(2 * g.rc + 1 + look) * nslot + (size_t)(2 * g.rc + 2) * ppl) * 8 + (size_t)(2 * g.rc + 1 + look) * 8;
+        const size_t smem = ((size_t)(2 * g.rc + 1 + look) * nslot + (size_t)(2 * g.rc + 2) * ppl) * 8 * (size_t)s->nb + (size_t)(2 * g.rc + 1 + look) * 8;
         if (smem > 200 * 1024) continue;
         const int per_sm = (int)std::min<size_t>((size_t)(227 * 1024) / (smem + 1024), (size_t)std::min(2048 / threads, 65536 / (threads * 56)));
         if (per_sm < 1) continue;
@@ -446,8 +446,10 @@ static void variants_prepare(spin_system *s, JitState *j) {
         if (e == cudaSuccess) e = cudaFuncSetAttribute((const void *)j->k_march, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)mg.smem);
         int occ = 0;
         if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, (const void *)j->k_march, mg.threads, mg.smem);
-        if (e == cudaSuccess && occ >= 1 && encode_march_map(s, mg, s->d_n[0], &j->tm_march[0]) == SPIN_OK &&
-            encode_march_map(s, mg, s->d_n[1], &j->tm_march[1]) == SPIN_OK) {
+        bool maps = e == cudaSuccess && occ >= 1;
+        for (int a = 0; a < 2 && maps; ++a)
+            for (int b = 0; b < s->nb && maps; ++b) maps = encode_march_map(s, mg, s->d_n[a] + (size_t)b * s->plan.sub, &j->tm_march[a][b]) == SPIN_OK;
+        if (maps) {
             j->march = true;
             j->march_ty = mg.ty; j->march_nzc = mg.nzc; j->march_threads = mg.threads; j->march_items = mg.items; j->march_smem = mg.smem;
         } else {
@@ -596,7 +598,7 @@ int spin::jit_launch_march(spin_system *s, int cur, double *nout, unsigned step_
     const unsigned char *pin = s->d_pin;
     const double *mu_ratio = s->d_mu_ratio;
     unsigned item0 = 0;
-    void *args[] = {(void *)&j->tm_march[cur], (void *)&nout, (void *)&d_step, (void *)&step_add, (void *)&seed_lo, (void *)&seed_hi, (void *)&pin, (void *)&mu_ratio,
+    void *args[] = {(void *)&j->tm_march[cur][0], (void *)&nout, (void *)&d_step, (void *)&step_add, (void *)&seed_lo, (void *)&seed_hi, (void *)&pin, (void *)&mu_ratio,
                     (void *)&item0, (void *)&peer_lo, (void *)&peer_hi, (void *)&peer_lo_nc};
     const unsigned items = (unsigned)j->march_items, cols = items / (unsigned)j->march_nzc;      // items = chunk x column tile, chunk-major
     unsigned ranges[2][2] = {{0u, items}, {0u, 0u}};

@@ -1,5 +1,6 @@
 // spin_jit_march.cuh -- the whole Depondt step (B5-B7) of a 3-D lattice in ONE pass: a plane-marching kernel
-// (sm_100a; included by spin_jit_kernels.cuh when SPIN_MARCH is defined; one basis atom, Depondt solver, no dipolar term).
+// (sm_100a; included by spin_jit_kernels.cuh when SPIN_MARCH is defined; Depondt or Heun solver, no dipolar term; one basis atom by
+// default, up to four on request; flat lattices are the special case of one plane).
 //
 // Why.  The two brick sweeps move 120 B per spin-update through HBM (n^p written and read back, n read twice), fetch every line
 // 2.8 times from L2 (brick halos) and evaluate F(n) twice.  On B200 that is not bandwidth- but POWER-bound: a 2-s run of cfg3 sits at
@@ -24,19 +25,26 @@ namespace spinmarch {
 using namespace spinjit;
 
 struct __align__(64) TensorMap { unsigned long long opaque[16]; };      // CUtensorMap, passed as a __grid_constant__ parameter
+template <int V> struct spin_ddi_like_int { static constexpr int value = V; };
 
 constexpr int RA = spec::MRA, RB = spec::MRB, RC = spec::MRC, TY = spec::MTY, NZC = spec::MNZC;
 constexpr int HX = (2 * RA + 1) / 2 * 2;                         // rim of a staged n row, even: TMA box rows start 16-byte aligned
 constexpr int NX = 32 + 2 * HX, NY = TY + 4 * RB;                // staged n plane (rim of two reaches), sites
-constexpr int NROW = 3 * NX, NPL = NROW * NY, NSLOT = (NPL + 15) / 16 * 16;      // doubles; slots are 128-byte multiples
+constexpr int NBS = spec::NBASIS;                                // sublattices: each has its own sub-slot in a staged plane
+constexpr int NROW = 3 * NX, NPL = NROW * NY, NSLOTB = (NPL + 15) / 16 * 16, NSLOT = NBS * NSLOTB;      // doubles; (sub-)slots are 128-byte multiples
 constexpr int PX = 32 + 2 * RA, PY = TY + 2 * RB;                // n^p plane (rim of one reach)
-constexpr int PROW = 3 * PX, PPL = PROW * PY;
+constexpr int PROW = 3 * PX, PPLB = PROW * PY, PPL = NBS * PPLB;
 constexpr int LOOK = spec::MLOOK;                                // n planes in flight beyond the ones the current predictor reads
 constexpr int RN = 2 * RC + 1 + LOOK, RP = 2 * RC + 2;           // ring depths: n planes, n^p planes
 constexpr int RIM = 2 * RA * PY, RIMW = (RIM + 31) / 32;         // sites of the rim columns, warps that take them
 constexpr int NWARP = PY + RIMW, NTHREADS = 32 * NWARP;
 constexpr int NTX = (spec::NA + 31) / 32, NTY = (spec::NB + TY - 1) / TY;
-static_assert(spec::NBASIS == 1 && (spec::SOLVER == 0 || spec::SOLVER == 1) && !spec::HAS_DDI && !spec::MULTI_IMAGE, "one-pass kernel: one basis atom, Depondt or Heun, no dipolar term");
+static_assert(spec::NBASIS <= 4 && (spec::SOLVER == 0 || spec::SOLVER == 1) && !spec::HAS_DDI && !spec::MULTI_IMAGE, "one-pass kernel: up to four basis atoms, Depondt or Heun, no dipolar term");
+// the TMA descriptors of the sublattices' arrays (same shape, different base)
+struct __align__(64) TensorMaps { TensorMap m[NBS]; };
+template <int B = 0, class F> __device__ __forceinline__ void for_each_basis(F &&f) {
+    if constexpr (B < NBS) { f(spin_ddi_like_int<B>{}); for_each_basis<B + 1>(f); }
+}
 static_assert(spec::RA == 2 * RA && spec::RB == 2 * RB && spec::RC == 2 * RC, "ghost layers must be twice the reach");
 
 extern __shared__ __align__(128) double smem[];
@@ -60,19 +68,19 @@ __device__ __forceinline__ void tma_load_4d(u32 dst, const TensorMap *tm, int c0
 }
 
 // partner of a site in a ring of staged planes: pl[dz + RC] points at the x component of the own site in the plane z + dz
-template <int XS, int ROWS>      // doubles between the components of a row (= sites per row), between rows
+template <int XS, int ROWS, int SUBS>      // doubles between the components of a row (= sites per row), between rows, between sublattices
 struct RingAcc {
-    const double *pl[2 * RC + 1];
+    const double *pl[2 * RC + 1];            // (of the sublattice B the accessor was set up for)
     template <int B, int BJ, int DA, int DB, int DC>
     __device__ __forceinline__ void load(int, double (&v)[3]) const {
-        const double *q = pl[DC + RC] + (DB * ROWS + DA);
+        const double *q = pl[DC + RC] + ((BJ - B) * SUBS + DB * ROWS + DA);
         v[0] = q[0]; v[1] = q[XS]; v[2] = q[2 * XS];
     }
 };
 }  // namespace spinmarch
 
 extern "C" __global__ void __launch_bounds__(spinmarch::NTHREADS, spec::MBLOCKS)
-    jit_depondt_march(const __grid_constant__ spinmarch::TensorMap tm_n, double *__restrict__ nout, const unsigned long long *__restrict__ d_step,
+    jit_depondt_march(const __grid_constant__ spinmarch::TensorMaps tm_n, double *__restrict__ nout, const unsigned long long *__restrict__ d_step,
                       unsigned int step_add, unsigned int seed_lo, unsigned int seed_hi, const unsigned char *__restrict__ pin,
                       const double *__restrict__ mu_ratio, unsigned int item0, double *__restrict__ peer_lo, double *__restrict__ peer_hi,
                       int peer_lo_nc) {
@@ -87,8 +95,10 @@ extern "C" __global__ void __launch_bounds__(spinmarch::NTHREADS, spec::MBLOCKS)
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     auto issue = [&](int p) {
         const u32 bar = bars + 8u * (p % RN);
-        mbar_expect_tx(bar, (u32)(NPL * 8));
-        tma_load_4d(smem_u32(nring + (p % RN) * NSLOT), &tm_n, spec::LA + x0 - HX, 0, spec::LB + y0 - 2 * RB, spec::LC + za - 2 * RC + p, bar);
+        mbar_expect_tx(bar, (u32)(NBS * NPL * 8));
+#pragma unroll
+        for (int b = 0; b < NBS; ++b)
+            tma_load_4d(smem_u32(nring + (p % RN) * NSLOT + b * NSLOTB), &tm_n.m[b], spec::LA + x0 - HX, 0, spec::LB + y0 - 2 * RB, spec::LC + za - 2 * RC + p, bar);
     };
     if (tid == 0) {
         for (int s = 0; s < RN; ++s) mbar_init(bars + 8u * s, 1u);
@@ -119,13 +129,15 @@ extern "C" __global__ void __launch_bounds__(spinmarch::NTHREADS, spec::MBLOCKS)
     const int ncell = ((sy + 2 * RB) * 3) * NX + (sx + HX);       // x component of the own site in a staged n plane
     const int pcell = ((sy + RB) * 3) * PX + (sx + RA);           // the same in an n^p plane
     // what the corrector of plane zC needs from the predictor of the same site, RC iterations earlier (flat lattices, RC = 0: the one
-    // plane there is -- the predictor's values of this very iteration, and the queue is not used)
+    // plane there is -- the predictor's values of this very iteration, and the queue is not used); one set per sublattice
     constexpr int QD = RC > 0 ? RC : 1;
-    double n_q[QD][3], A_q[QD][3], th_q[QD][3];
+    double n_q[QD][NBS][3], A_q[QD][NBS][3], th_q[QD][NBS][3];
 #pragma unroll
     for (int r = 0; r < QD; ++r)
 #pragma unroll
-        for (int k = 0; k < 3; ++k) { n_q[r][k] = 0.0; A_q[r][k] = 0.0; th_q[r][k] = 0.0; }
+        for (int b = 0; b < NBS; ++b)
+#pragma unroll
+            for (int k = 0; k < 3; ++k) { n_q[r][b][k] = 0.0; A_q[r][b][k] = 0.0; th_q[r][b][k] = 0.0; }
 #pragma unroll
     for (int p = 0; p < 2 * RC; ++p) mbar_wait(bars + 8u * p, 0u);
     const int NIT = zb - za + 2 * RC;
@@ -136,88 +148,105 @@ extern "C" __global__ void __launch_bounds__(spinmarch::NTHREADS, spec::MBLOCKS)
     for (int k = 0; k < NIT; ++k) {                                // predictor plane zP = za - RC + k from n planes k .. k + 2 RC
         mbar_wait(bars + 8u * wslot, (u32)wpar);
         const int zP = za - RC + k;
-        double n_cur[3] = {0.0, 0.0, 0.0}, A_cur[3] = {0.0, 0.0, 0.0}, th_cur[3] = {0.0, 0.0, 0.0};
+        double n_cur[NBS][3], A_cur[NBS][3], th_cur[NBS][3];
+#pragma unroll
+        for (int b = 0; b < NBS; ++b)
+#pragma unroll
+            for (int q = 0; q < 3; ++q) { n_cur[b][q] = 0.0; A_cur[b][q] = 0.0; th_cur[b][q] = 0.0; }
         double *pslot = pring + ps * PPL;
         if (mine) {
-            double out[3] = {0.0, 0.0, 0.0};
             // plane of the WHOLE lattice (slab decomposition: planes beyond the slab are the neighbours', staged from the ghost layers the
             // halo exchange fills; their predictor is recomputed here like the rim of a tile)
             const int gz = spec::C_OFF + zP;
             const bool live = live_xy && (spec::PER_C || (gz >= 0 && gz < spec::GNC));
-            if (live) {
-                c.ic = (gz < 0 ? gz + spec::GNC : (gz >= spec::GNC ? gz - spec::GNC : gz)) - spec::C_OFF;      // (outside [0, NC) only in a slab: noise index)
-                RingAcc<NX, NROW> acc;
+            if (live) c.ic = (gz < 0 ? gz + spec::GNC : (gz >= spec::GNC ? gz - spec::GNC : gz)) - spec::C_OFF;      // (outside [0, NC) only in a slab: noise index)
+            for_each_basis([&](auto bc) {
+                constexpr int B = decltype(bc)::value;
+                double out[3] = {0.0, 0.0, 0.0};
+                if (live) {
+                    RingAcc<NX, NROW, NSLOTB> acc;
 #pragma unroll
-                for (int dz = -RC; dz <= RC; ++dz) acc.pl[dz + RC] = nring + nslot_of(RC + dz) * NSLOT + ncell;
-                double own[1][3], F[1][3], sg[1][3] = {{0.0, 0.0, 0.0}};
-                acc.template load<0, 0, 0, 0, 0>(0, own[0]);
-                n_cur[0] = own[0][0]; n_cur[1] = own[0][1]; n_cur[2] = own[0][2];
-                if (is_pinned<0>(pin, c)) { out[0] = n_cur[0]; out[1] = n_cur[1]; out[2] = n_cur[2]; }
-                else {
-                    const double zr = site_ratio<0>(mu_ratio, c), ir = spec::HAS_SITE_MU ? 1.0 / zr : 1.0;      // per-site moment
-                    const double sscale = (spec::HAS_SITE_MU && spec::THERMAL_ON) ? sqrt(zr) : 1.0;
-                    thermal_force<0>(c, step, seed_lo, seed_hi, F[0], 0u, sscale);
-                    th_cur[0] = F[0][0]; th_cur[1] = F[0][1]; th_cur[2] = F[0][2];
-                    force<0, 1>(acc, own, F, zr);
-                    if constexpr (spec::STT_ON) stt_gradient<0, 1>(acc, c, own, sg);
-                    rotation_field<0>(own[0], F[0], sg[0], A_cur, ir);
-                    if constexpr (spec::SOLVER == 1) { out[0] = own[0][0]; out[1] = own[0][1]; out[2] = own[0][2]; spin::heun_add(own[0], A_cur, specc::DT, out); }   // Heun, B3
-                    else spin::rodrigues(A_cur, specc::DT, specc::DT2, own[0], out);             // Depondt, B5
+                    for (int dz = -RC; dz <= RC; ++dz) acc.pl[dz + RC] = nring + nslot_of(RC + dz) * NSLOT + B * NSLOTB + ncell;
+                    double own[1][3], F[1][3], sg[1][3] = {{0.0, 0.0, 0.0}};
+                    acc.template load<B, B, 0, 0, 0>(0, own[0]);
+                    n_cur[B][0] = own[0][0]; n_cur[B][1] = own[0][1]; n_cur[B][2] = own[0][2];
+                    if (is_pinned<B>(pin, c)) { out[0] = own[0][0]; out[1] = own[0][1]; out[2] = own[0][2]; }
+                    else {
+                        const double zr = site_ratio<B>(mu_ratio, c), ir = spec::HAS_SITE_MU ? 1.0 / zr : 1.0;      // per-site moment
+                        const double sscale = (spec::HAS_SITE_MU && spec::THERMAL_ON) ? sqrt(zr) : 1.0;
+                        thermal_force<B>(c, step, seed_lo, seed_hi, F[0], 0u, sscale);
+                        th_cur[B][0] = F[0][0]; th_cur[B][1] = F[0][1]; th_cur[B][2] = F[0][2];
+                        force<B, 1>(acc, own, F, zr);
+                        if constexpr (spec::STT_ON) stt_gradient<B, 1>(acc, c, own, sg);
+                        rotation_field<B>(own[0], F[0], sg[0], A_cur[B], ir);
+                        if constexpr (spec::SOLVER == 1) { out[0] = own[0][0]; out[1] = own[0][1]; out[2] = own[0][2]; spin::heun_add(own[0], A_cur[B], specc::DT, out); }   // Heun, B3
+                        else spin::rodrigues(A_cur[B], specc::DT, specc::DT2, own[0], out);          // Depondt, B5
+                    }
                 }
-            }
-            pslot[pcell] = out[0]; pslot[pcell + PX] = out[1]; pslot[pcell + 2 * PX] = out[2];
+                double *pq = pslot + B * PPLB + pcell;
+                pq[0] = out[0]; pq[PX] = out[1]; pq[2 * PX] = out[2];
+            });
         }
         if constexpr (RC == 0) {
 #pragma unroll
-            for (int q = 0; q < 3; ++q) { n_q[0][q] = n_cur[q]; A_q[0][q] = A_cur[q]; th_q[0][q] = th_cur[q]; }
+            for (int b = 0; b < NBS; ++b)
+#pragma unroll
+                for (int q = 0; q < 3; ++q) { n_q[0][b][q] = n_cur[b][q]; A_q[0][b][q] = A_cur[b][q]; th_q[0][b][q] = th_cur[b][q]; }
         }
         __syncthreads();                                           // n^p(zP) is complete; nobody reads n plane k any more
         if (tid == 0 && k + RN - 1 < NP) issue(k + RN - 1);        // refill a free slot, LOOK planes ahead of the next predictor
         const int zC = zP - RC;
         if (k >= 2 * RC && tile_site) {                            // corrector of plane zC from n^p planes zC - RC .. zC + RC = zP
             c.ic = zC;
-            double o[3];
-            if (is_pinned<0>(pin, c)) { o[0] = n_q[0][0]; o[1] = n_q[0][1]; o[2] = n_q[0][2]; }
-            else {
-                const double zr = site_ratio<0>(mu_ratio, c), ir = spec::HAS_SITE_MU ? 1.0 / zr : 1.0;
-                RingAcc<PX, PROW> acc;
-#pragma unroll
-                for (int dz = -RC; dz <= RC; ++dz) acc.pl[dz + RC] = pring + pslot_of(dz - RC) * PPL + pcell;
-                double own[1][3], F[1][3] = {{th_q[0][0], th_q[0][1], th_q[0][2]}}, sg[1][3] = {{0.0, 0.0, 0.0}}, Ap[3];
-                acc.template load<0, 0, 0, 0, 0>(0, own[0]);
-                force<0, 1>(acc, own, F, zr);
-                if constexpr (spec::STT_ON) stt_gradient<0, 1>(acc, c, own, sg);
-                rotation_field<0>(own[0], F[0], sg[0], Ap, ir);
-                if constexpr (spec::SOLVER == 1) {                                                // Heun, B4: n + dt/2 (n x A + n^p x A^p), renormalised
-                    o[0] = n_q[0][0]; o[1] = n_q[0][1]; o[2] = n_q[0][2];
-                    spin::heun_add(n_q[0], A_q[0], specc::HDT, o);
-                    spin::heun_add(own[0], Ap, specc::HDT, o);
-                    spin::renormalise_general(o);
-                } else {
-                    const double Ac[3] = {A_q[0][0] + Ap[0], A_q[0][1] + Ap[1], A_q[0][2] + Ap[2]};
-                    spin::rodrigues(Ac, specc::HDT, specc::QDT2, n_q[0], o);                      // Depondt, B6-B7: R((A + A^p) / 2) n(t)
-                    spin::renormalise(o);
-                }
-            }
             const size_t in_plane = (size_t)(c.ib + spec::LB) * ROW + (c.ia + spec::LA);
-            store_spin(nout + ((size_t)(zC + spec::LC) * PLANE + in_plane), c, o);
-            // Slab decomposition, fused exchange (llg_slab_step_fused): the planes a neighbouring slab holds as ghost layers are written
-            // straight into ITS next configuration -- peer memory on another GPU (NVLink), or another array of this GPU -- with their
-            // in-plane images; no halo copy follows.  peer_lo: the lower neighbour (its ghost layer above its peer_lo_nc planes),
-            // peer_hi: the upper neighbour (its ghost layer below plane 0).  Same layout on every slab but for the number of planes.
-            if constexpr (spec::SLAB) {
-                if (peer_lo && zC < spec::LC) store_spin(peer_lo + ((size_t)(spec::LC + peer_lo_nc + zC) * PLANE + in_plane), c, o);
-                if (peer_hi && zC >= spec::NC - spec::LC) store_spin(peer_hi + ((size_t)(zC - (spec::NC - spec::LC)) * PLANE + in_plane), c, o);
-            }
+            for_each_basis([&](auto bc) {
+                constexpr int B = decltype(bc)::value;
+                double o[3];
+                if (is_pinned<B>(pin, c)) { o[0] = n_q[0][B][0]; o[1] = n_q[0][B][1]; o[2] = n_q[0][B][2]; }
+                else {
+                    const double zr = site_ratio<B>(mu_ratio, c), ir = spec::HAS_SITE_MU ? 1.0 / zr : 1.0;
+                    RingAcc<PX, PROW, PPLB> acc;
+#pragma unroll
+                    for (int dz = -RC; dz <= RC; ++dz) acc.pl[dz + RC] = pring + pslot_of(dz - RC) * PPL + B * PPLB + pcell;
+                    double own[1][3], F[1][3] = {{th_q[0][B][0], th_q[0][B][1], th_q[0][B][2]}}, sg[1][3] = {{0.0, 0.0, 0.0}}, Ap[3];
+                    acc.template load<B, B, 0, 0, 0>(0, own[0]);
+                    force<B, 1>(acc, own, F, zr);
+                    if constexpr (spec::STT_ON) stt_gradient<B, 1>(acc, c, own, sg);
+                    rotation_field<B>(own[0], F[0], sg[0], Ap, ir);
+                    if constexpr (spec::SOLVER == 1) {                                            // Heun, B4: n + dt/2 (n x A + n^p x A^p), renormalised
+                        o[0] = n_q[0][B][0]; o[1] = n_q[0][B][1]; o[2] = n_q[0][B][2];
+                        spin::heun_add(n_q[0][B], A_q[0][B], specc::HDT, o);
+                        spin::heun_add(own[0], Ap, specc::HDT, o);
+                        spin::renormalise_general(o);
+                    } else {
+                        const double Ac[3] = {A_q[0][B][0] + Ap[0], A_q[0][B][1] + Ap[1], A_q[0][B][2] + Ap[2]};
+                        spin::rodrigues(Ac, specc::HDT, specc::QDT2, n_q[0][B], o);                // Depondt, B6-B7: R((A + A^p) / 2) n(t)
+                        spin::renormalise(o);
+                    }
+                }
+                const size_t site = (size_t)B * spec::SUB + in_plane;
+                store_spin(nout + ((size_t)(zC + spec::LC) * PLANE + site), c, o);
+                // Slab decomposition, fused exchange (llg_slab_step_fused): the planes a neighbouring slab holds as ghost layers are written
+                // straight into ITS next configuration -- peer memory on another GPU (NVLink), or another array of this GPU -- with their
+                // in-plane images; no halo copy follows.  peer_lo: the lower neighbour (its ghost layer above its peer_lo_nc planes),
+                // peer_hi: the upper neighbour (its ghost layer below plane 0).  Same layout on every slab but for the number of planes.
+                if constexpr (spec::SLAB && NBS == 1) {
+                    if (peer_lo && zC < spec::LC) store_spin(peer_lo + ((size_t)(spec::LC + peer_lo_nc + zC) * PLANE + site), c, o);
+                    if (peer_hi && zC >= spec::NC - spec::LC) store_spin(peer_hi + ((size_t)(zC - (spec::NC - spec::LC)) * PLANE + site), c, o);
+                }
+            });
         }
         // the queue moves on: slot 0 is the oldest (the plane the next corrector takes)
         if constexpr (RC > 0) {
 #pragma unroll
-            for (int r = 0; r + 1 < RC; ++r)
+            for (int b = 0; b < NBS; ++b) {
 #pragma unroll
-                for (int q = 0; q < 3; ++q) { n_q[r][q] = n_q[r + 1][q]; A_q[r][q] = A_q[r + 1][q]; th_q[r][q] = th_q[r + 1][q]; }
+                for (int r = 0; r + 1 < RC; ++r)
 #pragma unroll
-            for (int q = 0; q < 3; ++q) { n_q[QD - 1][q] = n_cur[q]; A_q[QD - 1][q] = A_cur[q]; th_q[QD - 1][q] = th_cur[q]; }
+                    for (int q = 0; q < 3; ++q) { n_q[r][b][q] = n_q[r + 1][b][q]; A_q[r][b][q] = A_q[r + 1][b][q]; th_q[r][b][q] = th_q[r + 1][b][q]; }
+#pragma unroll
+                for (int q = 0; q < 3; ++q) { n_q[QD - 1][b][q] = n_cur[b][q]; A_q[QD - 1][b][q] = A_cur[b][q]; th_q[QD - 1][b][q] = th_cur[b][q]; }
+            }
         }
         if (++ns == RN) ns = 0;
         if (++ps == RP) ps = 0;

@@ -1225,6 +1225,9 @@ MARCH_CASES = [
     (2, (70, 37, 1), (1, 1, 0), 10.0, 30),        # triangular, three shells (reach 2), thermal field, ragged tiles
     (1, (64, 40, 1), (1, 1, 0), 0.0, 40),         # square lattice with DMI and anisotropy
     (2, (96, 33, 1), (0, 1, 0), 0.0, 30),         # open along a
+    # several basis atoms (on request only, use_march = 2: measured slower than the brick sweeps but on small flat lattices)
+    (4, (70, 37, 1), (1, 1, 0), 30.0, 30),        # honeycomb: two sublattices, quadruplets, current, thermal field
+    (4, (64, 16, 1), (0, 0, 0), 0.0, 30),         # open edges
 ]
 
 
